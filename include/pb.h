@@ -1,0 +1,133 @@
+/*
+ * pb.h -- C ABI of the B200-native Jacobi-PCG solver for the linear finite-difference
+ * Poisson-Boltzmann equation (arxiv 1704.02745; citations are /root/reference/PAPER.md lines).
+ *
+ * What the library solves (Eq. 3; Eq. 4):
+ *
+ *      sum over the six faces f of node c of  h^-2 eps_f [phi(c) - phi(nbr_f)]  +  kbar2(c) phi(c)  =  rhs(c)
+ *
+ * on an nx*ny*nz grid of unknowns (x fastest: idx = (k*ny + j)*nx + i), with Dirichlet
+ * values on a ghost layer one node outside the grid (the paper's free-space boundary
+ * condition).  The solver is the preconditioned conjugate-gradient iteration
+ * of PAPER.md:104-126 (steps 1-8) with the Jacobi preconditioner M = diag(A) of
+ * PAPER.md:138-140 and phi_0 = 0.  The library is unit-agnostic: the
+ * paper's right-hand side h^-3 q(i,j,k) is whatever the caller passes as `rhs`.
+ *
+ * All entry points are extern "C", take plain pointers and sizes, never throw or abort,
+ * and return a pb_status.  There is no global state.  One handle = one operator on one
+ * device and one CUDA stream.  A handle is not thread-safe; distinct handles are independent.
+ * There is NO CPU fallback: without a CUDA device every compute call returns PB_ERR_CUDA.
+ *
+ * Array layouts (all caller arrays are dense C arrays of fp64 unless stated otherwise):
+ *   eps_x [nz][ny][nx+1]  face f lies between node i=f-1 and node i=f; the paper's
+ *                         eps_i(i,j,k) (between (i,j,k) and (i+1,j,k)) is eps_x[k][j][i+1];
+ *                         f=0 and f=nx touch the ghost layer.
+ *   eps_y [nz][ny+1][nx]  likewise along y;   eps_z [nz+1][ny][nx]  likewise along z.
+ *   kbar2 [nz][ny][nx]    nodal Boltzmann coefficient ("all the related coefficients ...
+ *                         absorbed into kappa^2"), 1/length^2.  NULL = 0.
+ *   rhs   [nz][ny][nx]    right-hand side of Eq. 3.  NULL = 0.
+ *   bc    ghost Dirichlet values packed x-, x+ ([nz][ny] each), y-, y+ ([nz][nx] each),
+ *         z-, z+ ([ny][nx] each): 2*(nz*ny + nz*nx + ny*nx) values.  NULL = 0.
+ * `where` says whether the data pointers of THAT call are host (PB_HOST) or device
+ * (PB_DEVICE, on the handle's device) pointers.  Scalars out (iters_out, relres_out) are
+ * always host pointers.
+ */
+#ifndef PB_H_
+#define PB_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pb_handle pb_handle;
+
+typedef enum {
+    PB_OK = 0,
+    PB_ERR_INVALID_ARG = 1,
+    PB_ERR_ALLOC = 2,
+    PB_ERR_CUDA = 3,
+    PB_ERR_NOT_SPD = 4,     /* a diagonal entry <= 0 or a non-finite coefficient found at create      */
+    PB_ERR_BREAKDOWN = 5,   /* p.Ap <= 0 or NaN/Inf met during the solve; phi = last good iterate     */
+    PB_ERR_MAXITER = 6      /* not converged in maxiter; phi, iters and relres are still returned     */
+} pb_status;
+
+typedef enum { PB_F32 = 0, PB_F64 = 1 } pb_precision;
+typedef enum { PB_HOST = 0, PB_DEVICE = 1 } pb_memspace;
+
+/*
+ * pb_create -- build the operator of Eq. 3 and, if rhs or bc is given,
+ * the right-hand side b of Eq. 4 with the ghost Dirichlet terms eps_f*g/h^2 folded in.
+ * Inputs are COPIED (the caller may free them on return).  The handle owns all device
+ * memory it allocates.  cuda_stream is a cudaStream_t (NULL = the default stream) on
+ * which every later call of this handle enqueues its work.
+ * Errors: nx,ny,nz < 1, h <= 0 or non-finite, NULL eps/out pointers -> PB_ERR_INVALID_ARG;
+ * a node whose diagonal sum(eps_f)/h^2 + kbar2 is <= 0 or non-finite -> PB_ERR_NOT_SPD;
+ * allocation / CUDA failures -> PB_ERR_ALLOC / PB_ERR_CUDA.  On error *out = NULL.
+ */
+pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double h,
+                    const double *eps_x, const double *eps_y, const double *eps_z,
+                    const double *kbar2, const double *rhs, const double *bc,
+                    pb_memspace where, void *cuda_stream);
+
+/*
+ * pb_set_rhs -- same operator, new right-hand side (Eq. 4: b = rhs + ghost fold-in).
+ * Used for the many-snapshot workload the paper motivates.  Copies its inputs.
+ */
+pb_status pb_set_rhs(pb_handle *h, const double *rhs, const double *bc, pb_memspace where);
+
+/*
+ * pb_apply -- y = A x, the left-hand side of Eq. 3 with x = 0 on the ghost layer, 1/h^2
+ * included.  x and y are [nz][ny][nx] arrays of the requested precision (float for
+ * PB_F32, double for PB_F64); they must not alias.  Runs the same matrix-free stencil
+ * kernel the solver uses.
+ */
+pb_status pb_apply(pb_handle *h, pb_precision prec, const void *x, void *y, pb_memspace where);
+
+/*
+ * pb_solve -- Jacobi-PCG, PAPER.md:104-126 with M = diag(A), phi_0 = 0.
+ *   tol         delta of step 3: stop at the first l with ||r_l||_2 / ||b||_2 < tol, r_l the
+ *               recurrence residual, b the folded right-hand side of Eq. 4.
+ *   maxiter     largest l allowed (>= 0).
+ *   prec        storage/arithmetic type of the vectors; every dot product accumulates in fp64.
+ *   check_every the host reads the 8-byte on-device {done, iters} latch once per this many
+ *               iterations (>= 1); there is no other host<->device traffic during the solve.
+ *               The returned iterate is exactly the one at which the test first passed,
+ *               whatever check_every is.
+ *   phi_out     [nz][ny][nx] in `prec`, caller-allocated, host or device per `where`.
+ *   iters_out   l at exit = number of A*p products (may be NULL).
+ *   relres_out  ||r_l||/||b|| at exit (may be NULL).
+ * Returns PB_OK, PB_ERR_MAXITER or PB_ERR_BREAKDOWN (phi_out/iters/relres valid in all
+ * three), or an argument/CUDA error.  b = 0 gives phi = 0, iters = 0, relres = 0.
+ * Blocks until phi_out holds the result.
+ */
+pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
+                   void *phi_out, pb_memspace where, int *iters_out, double *relres_out);
+
+/*
+ * pb_iterate -- benchmarking/profiling entry: enqueue exactly `n_iter` PCG iterations
+ * (K_spmv + K_vec pairs, PAPER.md:115-126 steps 4-8) with the convergence latch disabled,
+ * continuing from the state left by pb_solve_begin.  Does not synchronise.  Used by
+ * bench.py to time the steady-state iteration with CUDA events.
+ */
+pb_status pb_solve_begin(pb_handle *h, pb_precision prec);              /* steps 1-2: x=0, r=b, z=r/D */
+pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter);
+
+/* pb_destroy(NULL) is a no-op.  Frees every device allocation of the handle. */
+pb_status pb_destroy(pb_handle *h);
+
+/* Static, never-NULL description of a status code. */
+const char *pb_strerror(pb_status s);
+
+/*
+ * pb_query -- read back derived quantities for tests (device -> host copies, fp64):
+ *   what = 0: diag(A) [nz][ny][nx] (1/h^2 included);  what = 1: folded b of Eq. 4 [nz][ny][nx].
+ */
+pb_status pb_query(pb_handle *h, int what, double *out_host);
+
+/* Compile-time facts about the built library (for the bench report). */
+int pb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PB_H_ */

@@ -1,0 +1,232 @@
+"""ctypes binding of include/pb.h -- same names, argument marshalling only.
+
+Arrays may be numpy arrays / CPU torch tensors (passed as PB_HOST pointers) or CUDA torch
+tensors (passed as PB_DEVICE pointers).  PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+PB_F32, PB_F64 = 0, 1
+PB_HOST, PB_DEVICE = 0, 1
+PB_OK, PB_ERR_INVALID_ARG, PB_ERR_ALLOC, PB_ERR_CUDA, PB_ERR_NOT_SPD, PB_ERR_BREAKDOWN, PB_ERR_MAXITER = range(7)
+STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_ERR_CUDA",
+                4: "PB_ERR_NOT_SPD", 5: "PB_ERR_BREAKDOWN", 6: "PB_ERR_MAXITER"}
+
+# every symbol include/pb.h declares
+EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
+           "pb_destroy", "pb_strerror", "pb_query", "pb_version")
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+
+class PBError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = int(status)
+        super().__init__(f"{where}: {STATUS_NAMES.get(status, status)} ({pb_strerror(status)})")
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libpb.so")
+
+
+def load_library():
+    """Load libpb.so (built in-tree by paper_1704_02745_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            f"{path} not found: build it with `python -m paper_1704_02745_b200.build` "
+            "(there is no CPU fallback)")
+    lib = ctypes.CDLL(path)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    lib.pb_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, vp, vp, vp, vp, vp, vp, ci, vp]
+    lib.pb_set_rhs.argtypes = [vp, vp, vp, ci]
+    lib.pb_apply.argtypes = [vp, ci, vp, vp, ci]
+    lib.pb_solve.argtypes = [vp, cd, ci, ci, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd)]
+    lib.pb_solve_begin.argtypes = [vp, ci]
+    lib.pb_iterate.argtypes = [vp, ci, ci]
+    lib.pb_destroy.argtypes = [vp]
+    lib.pb_query.argtypes = [vp, ci, vp]
+    lib.pb_strerror.argtypes = [ci]
+    lib.pb_strerror.restype = ctypes.c_char_p
+    lib.pb_version.restype = ci
+    for name in EXPORTS:
+        getattr(lib, name)
+    _lib = lib
+    return lib
+
+
+def pb_strerror(status: int) -> str:
+    try:
+        return load_library().pb_strerror(int(status)).decode()
+    except Exception:
+        return "?"
+
+
+def _is_torch(a) -> bool:
+    return type(a).__module__.startswith("torch")
+
+
+def _marshal(a, dtype, count=None, name="array"):
+    """-> (pointer, memspace, keepalive).  None -> (NULL, None, None)."""
+    if a is None:
+        return None, None, None
+    if _is_torch(a):
+        import torch
+
+        want = {np.float64: torch.float64, np.float32: torch.float32}[dtype]
+        if a.dtype != want:
+            raise TypeError(f"{name}: expected {want}, got {a.dtype}")
+        a = a.contiguous()
+        if count is not None and a.numel() != count:
+            raise ValueError(f"{name}: expected {count} elements, got {a.numel()}")
+        return ctypes.c_void_p(a.data_ptr()), (PB_DEVICE if a.is_cuda else PB_HOST), a
+    arr = np.ascontiguousarray(a, dtype=dtype)
+    if count is not None and arr.size != count:
+        raise ValueError(f"{name}: expected {count} elements, got {arr.size}")
+    return ctypes.c_void_p(arr.ctypes.data), PB_HOST, arr
+
+
+def _one_space(spaces, default=PB_HOST):
+    s = {x for x in spaces if x is not None}
+    if len(s) > 1:
+        raise ValueError("all arrays of one call must live in the same memory space (host or device)")
+    return s.pop() if s else default
+
+
+def _prec(precision):
+    if precision in (PB_F32, "f32", "fp32", "float32", np.float32):
+        return PB_F32, np.float32
+    if precision in (PB_F64, "f64", "fp64", "float64", np.float64):
+        return PB_F64, np.float64
+    raise ValueError(f"unknown precision {precision!r}")
+
+
+class PBSolver:
+    """One operator (Eq. 3) on one device/stream: pb_create ... pb_destroy."""
+
+    def __init__(self, nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2=None, rhs=None, bc=None, stream=None):
+        lib = load_library()
+        self.nx, self.ny, self.nz, self.h = int(nx), int(ny), int(nz), float(h)
+        n = self.nx * self.ny * self.nz
+        nbc = 2 * (self.nz * self.ny + self.nz * self.nx + self.ny * self.nx)
+        f8 = np.float64
+        ex, s1, k1 = _marshal(eps_x, f8, self.nz * self.ny * (self.nx + 1), "eps_x")
+        ey, s2, k2 = _marshal(eps_y, f8, self.nz * (self.ny + 1) * self.nx, "eps_y")
+        ez, s3, k3 = _marshal(eps_z, f8, (self.nz + 1) * self.ny * self.nx, "eps_z")
+        kb, s4, k4 = _marshal(kbar2, f8, n, "kbar2")
+        rh, s5, k5 = _marshal(rhs, f8, n, "rhs")
+        bv, s6, k6 = _marshal(bc, f8, nbc, "bc")
+        where = _one_space([s1, s2, s3, s4, s5, s6])
+        self._h = ctypes.c_void_p()
+        st = lib.pb_create(ctypes.byref(self._h), self.nx, self.ny, self.nz, self.h, ex, ey, ez, kb, rh, bv,
+                           where, ctypes.c_void_p(int(stream) if stream else None))
+        del k1, k2, k3, k4, k5, k6
+        if st != PB_OK:
+            self._h = None
+            raise PBError(st, "pb_create")
+
+    @property
+    def shape(self):
+        return (self.nz, self.ny, self.nx)
+
+    def set_rhs(self, rhs, bc):
+        n = self.nx * self.ny * self.nz
+        nbc = 2 * (self.nz * self.ny + self.nz * self.nx + self.ny * self.nx)
+        rh, s1, k1 = _marshal(rhs, np.float64, n, "rhs")
+        bv, s2, k2 = _marshal(bc, np.float64, nbc, "bc")
+        st = load_library().pb_set_rhs(self._h, rh, bv, _one_space([s1, s2]))
+        del k1, k2
+        if st != PB_OK:
+            raise PBError(st, "pb_set_rhs")
+
+    def apply(self, x, precision=None):
+        """y = A x (Eq. 3 left-hand side, ghost x = 0).  numpy in -> numpy out; CUDA tensor in -> CUDA tensor out."""
+        if precision is None:
+            is32 = (str(x.dtype).endswith("float32"))
+            precision = PB_F32 if is32 else PB_F64
+        pc, dt = _prec(precision)
+        n = self.nx * self.ny * self.nz
+        xp, sx, keep = _marshal(x, dt, n, "x")
+        if _is_torch(x):
+            import torch
+
+            y = torch.empty(self.shape, dtype=keep.dtype, device=keep.device)
+            yp = ctypes.c_void_p(y.data_ptr())
+        else:
+            y = np.empty(self.shape, dtype=dt)
+            yp = ctypes.c_void_p(y.ctypes.data)
+        st = load_library().pb_apply(self._h, pc, xp, yp, sx)
+        if st != PB_OK:
+            raise PBError(st, "pb_apply")
+        return y
+
+    def solve(self, tol, maxiter, precision="f64", check_every=32, out=None):
+        """Jacobi-PCG.  Returns dict(phi, iters, relres, status).
+
+        `out`: optional numpy array / torch tensor (host or CUDA) receiving phi; default a new numpy array.
+        PB_ERR_MAXITER and PB_ERR_BREAKDOWN are reported in `status`, other errors raise.
+        """
+        pc, dt = _prec(precision)
+        n = self.nx * self.ny * self.nz
+        if out is None:
+            out = np.empty(self.shape, dtype=dt)
+        if not _is_torch(out) and (out.dtype != dt or not out.flags.c_contiguous):
+            raise TypeError("out must be a C-contiguous array of the requested precision")
+        op, so, keep = _marshal(out, dt, n, "out")
+        if _is_torch(out) and keep.data_ptr() != out.data_ptr():
+            raise TypeError("out must be contiguous")
+        it = ctypes.c_int(0)
+        rel = ctypes.c_double(0.0)
+        st = load_library().pb_solve(self._h, float(tol), int(maxiter), pc, int(check_every), op, so,
+                                     ctypes.byref(it), ctypes.byref(rel))
+        if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
+            raise PBError(st, "pb_solve")
+        return dict(phi=out, iters=it.value, relres=rel.value, status=st)
+
+    def solve_begin(self, precision):
+        st = load_library().pb_solve_begin(self._h, _prec(precision)[0])
+        if st != PB_OK:
+            raise PBError(st, "pb_solve_begin")
+
+    def iterate(self, precision, n_iter):
+        st = load_library().pb_iterate(self._h, _prec(precision)[0], int(n_iter))
+        if st != PB_OK:
+            raise PBError(st, "pb_iterate")
+
+    def _query(self, what):
+        out = np.empty(self.shape, dtype=np.float64)
+        st = load_library().pb_query(self._h, what, ctypes.c_void_p(out.ctypes.data))
+        if st != PB_OK:
+            raise PBError(st, "pb_query")
+        return out
+
+    def diag(self):
+        return self._query(0)
+
+    def b(self):
+        return self._query(1)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().pb_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,511 @@
+// pb_api.cu -- the C ABI of include/pb.h on top of the sm_100a kernels.
+// Host logic only: argument checks, device memory, tile selection, the launch sequence of
+// the PCG loop with its poll-every-k convergence latch, CUDA graphs.
+// No step of the method runs on the host.  Product code: shares nothing with oracle/.
+#include "../../include/pb.h"
+#include "pb_kernels.cuh"
+#include "pb_setup.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+using namespace pb;
+
+namespace {
+
+template <typename T>
+struct Work {
+    T *exm = nullptr, *eym = nullptr, *ezm = nullptr, *D = nullptr, *Dinv = nullptr, *b = nullptr;
+    T *x = nullptr, *r = nullptr, *z = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr;
+    int P = 0;
+    size_t npad = 0;                 // nz*ny*P
+    bool ready = false, b_ready = false;
+    int TXV = 0, TY = 0, TZ = 0, ntx = 0, nty = 0, ntz = 0, vec_grid = 0;
+    size_t smem = 0;
+    cudaGraphExec_t graph = nullptr;
+    int graph_iters = 0;
+};
+
+}  // namespace
+
+struct pb_handle {
+    int nx, ny, nz;
+    double h;
+    int device;
+    cudaStream_t stream;
+    bool own_stream;
+    double *eps_x, *eps_y, *eps_z, *kbar2, *rhs, *bc;   // dense fp64 device copies of the inputs
+    State *st;
+    double *partials;
+    size_t partials_cap;
+    int *bad;
+    int *pinned;                 // 2 x 4 ints, page-locked
+    State *pinned_state;
+    cudaEvent_t ev[2];
+    void *stage;                 // dense staging buffer for host <-> device vectors
+    size_t stage_bytes;
+    Work<float> wf;
+    Work<double> wd;
+    int use_graph;
+};
+
+namespace {
+
+#define PB_CUDA(call)                                                          \
+    do {                                                                       \
+        cudaError_t e__ = (call);                                              \
+        if (e__ != cudaSuccess) {                                              \
+            if (getenv("PB_VERBOSE"))                                          \
+                fprintf(stderr, "pb: %s failed: %s (%s:%d)\n", #call,          \
+                        cudaGetErrorString(e__), __FILE__, __LINE__);          \
+            cudaGetLastError();                                                \
+            return (e__ == cudaErrorMemoryAllocation) ? PB_ERR_ALLOC : PB_ERR_CUDA; \
+        }                                                                      \
+    } while (0)
+
+#define PB_TRY(expr)                       \
+    do {                                   \
+        pb_status s__ = (expr);            \
+        if (s__ != PB_OK) return s__;      \
+    } while (0)
+
+template <typename T> Work<T> &work(pb_handle *h);
+template <> Work<float> &work<float>(pb_handle *h) { return h->wf; }
+template <> Work<double> &work<double>(pb_handle *h) { return h->wd; }
+
+int env_int(const char *name, int dflt)
+{
+    const char *s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+inline int grid_for(size_t n, int block, int cap)
+{
+    size_t g = (n + block - 1) / block;
+    if (g > (size_t)cap) g = cap;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+constexpr int kNumSM = 148;   // B200
+
+template <typename T>
+void choose_tiles(pb_handle *h, Work<T> &w)
+{
+    constexpr int VEC = VecN<T>::value;
+    const int rowvecs = w.P / VEC;
+    int ntx = (rowvecs + 127) / 128;
+    int TXV = (rowvecs + ntx - 1) / ntx;
+    int TY = 512 / TXV;
+    if (TY > 16) TY = 16;
+    if (TY > h->ny) TY = h->ny;
+    if (TY < 1) TY = 1;
+    int TZ = 16;
+    TXV = env_int("PB_TXV", TXV);
+    if (TXV < 1) TXV = 1;
+    if (TXV > 512) TXV = 512;
+    if (TXV > rowvecs) TXV = rowvecs;
+    TY = env_int("PB_TY", TY);
+    if (TY < 1) TY = 1;
+    if (TXV * TY > 512) TY = 512 / TXV;
+    TZ = env_int("PB_TZ", TZ);
+    if (TZ < 1) TZ = 1;
+    if (TZ > h->nz) TZ = h->nz;
+    w.TXV = TXV; w.TY = TY; w.TZ = TZ;
+    w.ntx = (rowvecs + TXV - 1) / TXV;
+    w.nty = (h->ny + TY - 1) / TY;
+    w.ntz = (h->nz + TZ - 1) / TZ;
+    w.smem = (size_t)3 * (TY + 2) * (TXV * VEC + 2 * VEC) * sizeof(T);
+    w.vec_grid = grid_for(w.npad / VEC, 256, kNumSM * env_int("PB_VEC_BPS", 8));
+}
+
+template <typename T>
+pb_status alloc_arr(T **p, size_t n)
+{
+    PB_CUDA(cudaMalloc((void **)p, (n + 64) * sizeof(T)));   // slack: vector tails never fault
+    return PB_OK;
+}
+
+template <typename T>
+void free_work(Work<T> &w)
+{
+    T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.z, &w.p0, &w.p1, &w.Ap};
+    for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
+    if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
+    w.ready = w.b_ready = false;
+}
+
+template <typename T>
+pb_status build_b(pb_handle *h, Work<T> &w)
+{
+    const double h2 = h->h * h->h;
+    k_setup_b<T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
+        h->eps_x, h->eps_y, h->eps_z, h->rhs, h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b);
+    PB_CUDA(cudaGetLastError());
+    w.b_ready = true;
+    return PB_OK;
+}
+
+// Lazily build the arrays of precision T (setup row a0).
+template <typename T>
+pb_status ensure(pb_handle *h)
+{
+    Work<T> &w = work<T>(h);
+    if (w.ready) {
+        if (!w.b_ready) PB_TRY(build_b<T>(h, w));
+        return PB_OK;
+    }
+    const int align = 32 / (int)sizeof(T);
+    w.P = ((h->nx + 1 + align - 1) / align) * align;
+    w.npad = (size_t)h->nz * h->ny * w.P;
+    const size_t n_ey = (size_t)h->nz * (h->ny + 1) * w.P, n_ez = (size_t)(h->nz + 1) * h->ny * w.P;
+    pb_status s = PB_OK;
+    if ((s = alloc_arr(&w.exm, w.npad)) || (s = alloc_arr(&w.eym, n_ey)) || (s = alloc_arr(&w.ezm, n_ez)) ||
+        (s = alloc_arr(&w.D, w.npad)) || (s = alloc_arr(&w.Dinv, w.npad)) || (s = alloc_arr(&w.b, w.npad)) ||
+        (s = alloc_arr(&w.x, w.npad)) || (s = alloc_arr(&w.r, w.npad)) || (s = alloc_arr(&w.z, w.npad)) ||
+        (s = alloc_arr(&w.p0, w.npad)) || (s = alloc_arr(&w.p1, w.npad)) || (s = alloc_arr(&w.Ap, w.npad))) {
+        free_work(w);
+        return s;
+    }
+    choose_tiles<T>(h, w);
+    const size_t need = (size_t)w.ntx * w.nty * w.ntz > (size_t)2 * w.vec_grid
+                            ? (size_t)w.ntx * w.nty * w.ntz : (size_t)2 * w.vec_grid;
+    if (need > h->partials_cap) {
+        if (h->partials) cudaFree(h->partials);
+        h->partials = nullptr;
+        h->partials_cap = 0;
+        PB_CUDA(cudaMalloc((void **)&h->partials, need * sizeof(double)));
+        h->partials_cap = need;
+    }
+    PB_CUDA(cudaFuncSetAttribute(k_spmv<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
+    PB_CUDA(cudaFuncSetAttribute(k_spmv<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
+    PB_CUDA(cudaMemsetAsync(h->bad, 0, sizeof(int), h->stream));
+    const size_t total = (size_t)(h->nz + 1) * (h->ny + 1) * w.P;
+    k_setup_coeff<T><<<grid_for(total, 256, kNumSM * 16), 256, 0, h->stream>>>(
+        h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
+        w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
+    PB_CUDA(cudaGetLastError());
+    PB_TRY(build_b<T>(h, w));
+    w.ready = true;
+    return PB_OK;
+}
+
+template <typename T>
+SpmvArgs<T> spmv_args(pb_handle *h, Work<T> &w)
+{
+    SpmvArgs<T> a;
+    a.z = w.z; a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap;
+    a.exm = w.exm; a.eym = w.eym; a.ezm = w.ezm; a.D = w.D;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
+    a.TXV = w.TXV; a.TY = w.TY; a.TZ = w.TZ; a.ntx = w.ntx; a.nty = w.nty; a.ntz = w.ntz;
+    a.st = h->st; a.partials = h->partials; a.out_scale = 1.0;
+    return a;
+}
+
+template <typename T>
+VecArgs<T> vec_args(pb_handle *h, Work<T> &w)
+{
+    VecArgs<T> a;
+    a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.x = w.x; a.r = w.r; a.z = w.z; a.Ap = w.Ap; a.Dinv = w.Dinv;
+    a.b = w.b; a.pzero = w.p0; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
+    return a;
+}
+
+// enqueue n PCG iterations: (k_spmv, k_vec) pairs, nothing else
+template <typename T>
+pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
+{
+    const SpmvArgs<T> sa = spmv_args<T>(h, w);
+    const VecArgs<T> va = vec_args<T>(h, w);
+    const int sgrid = w.ntx * w.nty * w.ntz, sblock = w.TXV * w.TY;
+    for (int it = 0; it < n; it++) {
+        k_spmv<T, 0><<<sgrid, sblock, w.smem, h->stream>>>(sa);
+        k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
+    }
+    PB_CUDA(cudaGetLastError());
+    return PB_OK;
+}
+
+template <typename T>
+pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch)
+{
+    PB_TRY(ensure<T>(h));
+    Work<T> &w = work<T>(h);
+    k_set_state<<<1, 1, 0, h->stream>>>(h->st, tol * tol, maxiter, latch);
+    k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w));
+    PB_CUDA(cudaGetLastError());
+    return PB_OK;
+}
+
+template <typename T>
+pb_status get_graph(pb_handle *h, Work<T> &w, int m)
+{
+    if (w.graph && w.graph_iters == m) return PB_OK;
+    if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
+    cudaGraph_t g = nullptr;
+    PB_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    pb_status s = enqueue_iterations<T>(h, w, m);
+    cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+    if (s != PB_OK || e != cudaSuccess || !g) { cudaGetLastError(); return PB_ERR_CUDA; }
+    e = cudaGraphInstantiate(&w.graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { w.graph = nullptr; cudaGetLastError(); return PB_ERR_CUDA; }
+    w.graph_iters = m;
+    return PB_OK;
+}
+
+pb_status ensure_stage(pb_handle *h, size_t bytes)
+{
+    if (bytes <= h->stage_bytes) return PB_OK;
+    if (h->stage) cudaFree(h->stage);
+    h->stage = nullptr;
+    h->stage_bytes = 0;
+    PB_CUDA(cudaMalloc(&h->stage, bytes));
+    h->stage_bytes = bytes;
+    return PB_OK;
+}
+
+template <typename T>
+pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, void *phi_out,
+                     pb_memspace where, int *iters_out, double *relres_out)
+{
+    PB_TRY(begin_solve<T>(h, tol, maxiter, 1));
+    Work<T> &w = work<T>(h);
+    const int m = check_every;
+    bool graph_ok = h->use_graph && get_graph<T>(h, w, m) == PB_OK;
+    // chunk c is enqueued before the latch of chunk c-1 is waited for, so the device never idles
+    const long max_chunks = (long)maxiter / m + 2;
+    int seen_done = 0;
+    for (long c = 0; c < max_chunks + 1 && !seen_done; c++) {
+        if (graph_ok) PB_CUDA(cudaGraphLaunch(w.graph, h->stream));
+        else PB_TRY(enqueue_iterations<T>(h, w, m));
+        int *slot = h->pinned + 4 * (c & 1);
+        PB_CUDA(cudaMemcpyAsync(slot, &h->st->done, 4 * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaEventRecord(h->ev[c & 1], h->stream));
+        if (c >= 1) {
+            PB_CUDA(cudaEventSynchronize(h->ev[(c - 1) & 1]));
+            seen_done = h->pinned[4 * ((c - 1) & 1)];
+        }
+    }
+    // a6: un-pad x -> phi_out, read the final scalars
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    T *dst = (T *)phi_out;
+    if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(T))); dst = (T *)h->stage; }
+    k_unpad<T, T><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(w.x, dst, h->nx, w.P, rows, 1.0);
+    PB_CUDA(cudaGetLastError());
+    if (where == PB_HOST)
+        PB_CUDA(cudaMemcpyAsync(phi_out, dst, n * sizeof(T), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    const State &st = *h->pinned_state;
+    if (!st.done) return PB_ERR_CUDA;   // cannot happen: maxiter latches
+    if (iters_out) *iters_out = st.iters;
+    if (relres_out) *relres_out = (st.bb > 0.0) ? sqrt(st.rr / st.bb) : 0.0;
+    return (pb_status)st.status;
+}
+
+template <typename T>
+pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
+{
+    PB_TRY(ensure<T>(h));
+    Work<T> &w = work<T>(h);
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    const T *src = (const T *)x;
+    T *dst = (T *)y;
+    if (where == PB_HOST) {
+        PB_TRY(ensure_stage(h, n * sizeof(T)));
+        PB_CUDA(cudaMemcpyAsync(h->stage, x, n * sizeof(T), cudaMemcpyHostToDevice, h->stream));
+        src = (const T *)h->stage;
+        dst = (T *)h->stage;
+    }
+    const int g = grid_for(w.npad, 256, kNumSM * 16);
+    k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.z, h->nx, w.P, rows);
+    SpmvArgs<T> sa = spmv_args<T>(h, w);
+    sa.out_scale = 1.0 / (h->h * h->h);
+    k_spmv<T, 1><<<w.ntx * w.nty * w.ntz, w.TXV * w.TY, w.smem, h->stream>>>(sa);
+    k_unpad<T, T><<<g, 256, 0, h->stream>>>(w.Ap, dst, h->nx, w.P, rows, 1.0);
+    PB_CUDA(cudaGetLastError());
+    if (where == PB_HOST)
+        PB_CUDA(cudaMemcpyAsync(y, dst, n * sizeof(T), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}
+
+// copy a caller array (host or device) into a fresh/existing device array of n doubles
+pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_memspace where)
+{
+    if (!src) {
+        if (*dst) cudaFree(*dst);
+        *dst = nullptr;
+        return PB_OK;
+    }
+    if (!*dst) PB_CUDA(cudaMalloc((void **)dst, (n + 8) * sizeof(double)));
+    PB_CUDA(cudaMemcpyAsync(*dst, src, n * sizeof(double),
+                            where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
+    return PB_OK;
+}
+
+bool valid_space(pb_memspace w) { return w == PB_HOST || w == PB_DEVICE; }
+bool valid_prec(pb_precision p) { return p == PB_F32 || p == PB_F64; }
+
+}  // namespace
+
+extern "C" {
+
+pb_status pb_destroy(pb_handle *h)
+{
+    if (!h) return PB_OK;
+    cudaSetDevice(h->device);
+    if (h->stream) cudaStreamSynchronize(h->stream);
+    free_work(h->wf);
+    free_work(h->wd);
+    double **ins[] = {&h->eps_x, &h->eps_y, &h->eps_z, &h->kbar2, &h->rhs, &h->bc};
+    for (double **a : ins) if (*a) cudaFree(*a);
+    if (h->st) cudaFree(h->st);
+    if (h->partials) cudaFree(h->partials);
+    if (h->bad) cudaFree(h->bad);
+    if (h->stage) cudaFree(h->stage);
+    if (h->pinned) cudaFreeHost(h->pinned);
+    if (h->pinned_state) cudaFreeHost(h->pinned_state);
+    for (int i = 0; i < 2; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+    cudaGetLastError();
+    delete h;
+    return PB_OK;
+}
+
+pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
+                    const double *eps_x, const double *eps_y, const double *eps_z,
+                    const double *kbar2, const double *rhs, const double *bc,
+                    pb_memspace where, void *cuda_stream)
+{
+    if (!out) return PB_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1 || !(hh > 0.0) || !std::isfinite(hh) || !eps_x || !eps_y || !eps_z ||
+        !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    if ((double)nx * ny * nz > 2.0e9) return PB_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return PB_ERR_CUDA; }
+    pb_handle *h = new (std::nothrow) pb_handle();
+    if (!h) return PB_ERR_ALLOC;
+    h->nx = nx; h->ny = ny; h->nz = nz; h->h = hh;
+    h->use_graph = env_int("PB_NO_GRAPH", 0) ? 0 : 1;
+    pb_status s = PB_OK;
+    auto body = [&]() -> pb_status {
+        PB_CUDA(cudaGetDevice(&h->device));
+        if (cuda_stream) { h->stream = (cudaStream_t)cuda_stream; h->own_stream = false; }
+        else { PB_CUDA(cudaStreamCreate(&h->stream)); h->own_stream = true; }   // blocking: orders with stream 0
+        PB_CUDA(cudaMalloc((void **)&h->st, sizeof(State)));
+        PB_CUDA(cudaMemsetAsync(h->st, 0, sizeof(State), h->stream));
+        PB_CUDA(cudaMalloc((void **)&h->bad, sizeof(int)));
+        PB_CUDA(cudaHostAlloc((void **)&h->pinned, 8 * sizeof(int), cudaHostAllocDefault));
+        PB_CUDA(cudaHostAlloc((void **)&h->pinned_state, sizeof(State), cudaHostAllocDefault));
+        PB_CUDA(cudaEventCreateWithFlags(&h->ev[0], cudaEventDisableTiming));
+        PB_CUDA(cudaEventCreateWithFlags(&h->ev[1], cudaEventDisableTiming));
+        const size_t n = (size_t)nx * ny * nz;
+        PB_TRY(take_copy(h, &h->eps_x, eps_x, (size_t)nz * ny * (nx + 1), where));
+        PB_TRY(take_copy(h, &h->eps_y, eps_y, (size_t)nz * (ny + 1) * nx, where));
+        PB_TRY(take_copy(h, &h->eps_z, eps_z, (size_t)(nz + 1) * ny * nx, where));
+        PB_TRY(take_copy(h, &h->kbar2, kbar2, n, where));
+        PB_TRY(take_copy(h, &h->rhs, rhs, n, where));
+        PB_TRY(take_copy(h, &h->bc, bc, 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx), where));
+        // the fp64 operator is always built: it carries the SPD check of the diagonal
+        PB_TRY(ensure<double>(h));
+        int bad = 0;
+        PB_CUDA(cudaMemcpyAsync(&bad, h->bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        if (bad) return PB_ERR_NOT_SPD;
+        return PB_OK;
+    };
+    s = body();
+    if (s != PB_OK) { pb_destroy(h); return s; }
+    *out = h;
+    return PB_OK;
+}
+
+pb_status pb_set_rhs(pb_handle *h, const double *rhs, const double *bc, pb_memspace where)
+{
+    if (!h || !valid_space(where)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    const size_t n = (size_t)h->nx * h->ny * h->nz;
+    PB_TRY(take_copy(h, &h->rhs, rhs, n, where));
+    PB_TRY(take_copy(h, &h->bc, bc, 2 * ((size_t)h->nz * h->ny + (size_t)h->nz * h->nx + (size_t)h->ny * h->nx), where));
+    h->wf.b_ready = false;
+    h->wd.b_ready = false;
+    if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));
+    if (h->wd.ready) PB_TRY(build_b<double>(h, h->wd));
+    if (where == PB_HOST) PB_CUDA(cudaStreamSynchronize(h->stream));   // caller may free on return
+    return PB_OK;
+}
+
+pb_status pb_apply(pb_handle *h, pb_precision prec, const void *x, void *y, pb_memspace where)
+{
+    if (!h || !x || !y || x == y || !valid_prec(prec) || !valid_space(where)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? apply_impl<float>(h, x, y, where) : apply_impl<double>(h, x, y, where);
+}
+
+pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
+                   void *phi_out, pb_memspace where, int *iters_out, double *relres_out)
+{
+    if (!h || !phi_out || !(tol > 0.0) || !std::isfinite(tol) || maxiter < 0 || check_every < 1 ||
+        !valid_prec(prec) || !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out)
+                          : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out);
+}
+
+pb_status pb_solve_begin(pb_handle *h, pb_precision prec)
+{
+    if (!h || !valid_prec(prec)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? begin_solve<float>(h, 1.0, 0, 0) : begin_solve<double>(h, 1.0, 0, 0);
+}
+
+pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
+{
+    if (!h || !valid_prec(prec) || n_iter < 0) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    if (prec == PB_F32) { if (!h->wf.ready) return PB_ERR_INVALID_ARG; return enqueue_iterations<float>(h, h->wf, n_iter); }
+    if (!h->wd.ready) return PB_ERR_INVALID_ARG;
+    return enqueue_iterations<double>(h, h->wd, n_iter);
+}
+
+pb_status pb_query(pb_handle *h, int what, double *out_host)
+{
+    if (!h || !out_host || (what != 0 && what != 1)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    PB_TRY(ensure<double>(h));
+    Work<double> &w = h->wd;
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    PB_TRY(ensure_stage(h, n * sizeof(double)));
+    k_unpad<double, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(
+        what == 0 ? w.D : w.b, (double *)h->stage, h->nx, w.P, rows, 1.0 / (h->h * h->h));
+    PB_CUDA(cudaGetLastError());
+    PB_CUDA(cudaMemcpyAsync(out_host, h->stage, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}
+
+const char *pb_strerror(pb_status s)
+{
+    switch (s) {
+    case PB_OK: return "ok";
+    case PB_ERR_INVALID_ARG: return "invalid argument";
+    case PB_ERR_ALLOC: return "out of memory";
+    case PB_ERR_CUDA: return "CUDA error or no CUDA device (this library has no CPU fallback)";
+    case PB_ERR_NOT_SPD: return "operator not symmetric positive definite (non-positive or non-finite diagonal)";
+    case PB_ERR_BREAKDOWN: return "PCG breakdown (p.Ap <= 0 or non-finite value)";
+    case PB_ERR_MAXITER: return "maximum number of iterations reached before convergence";
+    }
+    return "unknown status";
+}
+
+int pb_version(void) { return 100; }
+
+}  // extern "C"
