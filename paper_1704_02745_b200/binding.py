@@ -208,6 +208,19 @@ class PBSolver:
             raise PBError(st, "pb_query")
         return out
 
+    def state(self):
+        """Device-resident PCG scalars (pb_query what=2) as a dict; diagnostics only."""
+        out = np.zeros(10)
+        st = load_library().pb_query(self._h, 2, ctypes.c_void_p(out.ctypes.data))
+        if st != PB_OK:
+            raise PBError(st, "pb_query")
+        keys = ("rz", "pAp", "rr", "bb", "alpha", "beta", "l", "done", "status", "iters")
+        return dict(zip(keys, out.tolist()))
+
+    def vector(self, name):
+        """Work vector 'r','z','p','Ap' or 'x' of the last solve (h^2-scaled system), as fp64 numpy."""
+        return self._query({"r": 3, "z": 4, "p": 5, "Ap": 6, "x": 7}[name])
+
     def diag(self):
         return self._query(0)
 

@@ -50,6 +50,7 @@ struct pb_handle {
     Work<float> wf;
     Work<double> wd;
     int use_graph;
+    int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
 };
 
 namespace {
@@ -220,7 +221,7 @@ pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
 {
     const SpmvArgs<T> sa = spmv_args<T>(h, w);
     const VecArgs<T> va = vec_args<T>(h, w);
-    const int sgrid = w.ntx * w.nty * w.ntz, sblock = w.TXV * w.TY;
+    const int sgrid = w.ntx * w.nty * w.ntz, sblock = (w.TXV * w.TY + 31) / 32 * 32;
     for (int it = 0; it < n; it++) {
         k_spmv<T, 0><<<sgrid, sblock, w.smem, h->stream>>>(sa);
         k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
@@ -234,6 +235,7 @@ pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch)
 {
     PB_TRY(ensure<T>(h));
     Work<T> &w = work<T>(h);
+    h->last_prec = sizeof(T) == 4 ? PB_F32 : PB_F64;
     k_set_state<<<1, 1, 0, h->stream>>>(h->st, tol * tol, maxiter, latch);
     k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w));
     PB_CUDA(cudaGetLastError());
@@ -325,7 +327,7 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
     k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.z, h->nx, w.P, rows);
     SpmvArgs<T> sa = spmv_args<T>(h, w);
     sa.out_scale = 1.0 / (h->h * h->h);
-    k_spmv<T, 1><<<w.ntx * w.nty * w.ntz, w.TXV * w.TY, w.smem, h->stream>>>(sa);
+    k_spmv<T, 1><<<w.ntx * w.nty * w.ntz, (w.TXV * w.TY + 31) / 32 * 32, w.smem, h->stream>>>(sa);
     k_unpad<T, T><<<g, 256, 0, h->stream>>>(w.Ap, dst, h->nx, w.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
     if (where == PB_HOST)
@@ -478,12 +480,45 @@ pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
 
 pb_status pb_query(pb_handle *h, int what, double *out_host)
 {
-    if (!h || !out_host || (what != 0 && what != 1)) return PB_ERR_INVALID_ARG;
+    if (!h || !out_host || what < 0 || what > 7) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
-    PB_TRY(ensure<double>(h));
-    Work<double> &w = h->wd;
+    if (what == 2) {
+        PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        const State &st = *h->pinned_state;
+        const double v[10] = {st.rz, st.pAp, st.rr, st.bb, st.alpha, st.beta, (double)st.iter_cur,
+                              (double)st.done, (double)st.status, (double)st.iters};
+        memcpy(out_host, v, sizeof(v));
+        return PB_OK;
+    }
     const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
     PB_TRY(ensure_stage(h, n * sizeof(double)));
+    if (what >= 3) {   // work vectors of the last solve, h^2-scaled system, converted to fp64
+        const int g = grid_for(n, 256, kNumSM * 16);
+        if (h->last_prec == PB_F32) {
+            Work<float> &w = h->wf;
+            if (!w.ready) return PB_ERR_INVALID_ARG;
+            const float *src[] = {w.r, w.z, nullptr, w.Ap, w.x};
+            const float *sp = src[what - 3];
+            if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+                       PB_CUDA(cudaStreamSynchronize(h->stream)); sp = (h->pinned_state->iter_cur & 1) ? w.p1 : w.p0; }
+            k_unpad<float, double><<<g, 256, 0, h->stream>>>(sp, (double *)h->stage, h->nx, w.P, rows, 1.0);
+        } else {
+            Work<double> &w = h->wd;
+            if (!w.ready) return PB_ERR_INVALID_ARG;
+            const double *src[] = {w.r, w.z, nullptr, w.Ap, w.x};
+            const double *sp = src[what - 3];
+            if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+                       PB_CUDA(cudaStreamSynchronize(h->stream)); sp = (h->pinned_state->iter_cur & 1) ? w.p1 : w.p0; }
+            k_unpad<double, double><<<g, 256, 0, h->stream>>>(sp, (double *)h->stage, h->nx, w.P, rows, 1.0);
+        }
+        PB_CUDA(cudaGetLastError());
+        PB_CUDA(cudaMemcpyAsync(out_host, h->stage, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        return PB_OK;
+    }
+    PB_TRY(ensure<double>(h));
+    Work<double> &w = h->wd;
     k_unpad<double, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(
         what == 0 ? w.D : w.b, (double *)h->stage, h->nx, w.P, rows, 1.0 / (h->h * h->h));
     PB_CUDA(cudaGetLastError());

@@ -16,8 +16,9 @@
 //   exm          [nz][ny][P]      exm[k][j][i]  = eps_x face between i-1 and i (i = 0..nx), else 0
 //   eym          [nz][ny+1][P]    eym[k][f][i]  = eps_y face between j=f-1 and j=f
 //   ezm          [nz+1][ny][P]    ezm[f][j][i]  = eps_z face between k=f-1 and k=f
-// Pad columns (i >= nx) hold 0 in every vector and coefficient except D = Dinv = 1, so
-// they stay exactly 0 through the iteration and never contribute to a dot product.
+// Pad columns (i >= nx) hold 0 in every vector and coefficient except D = Dinv = 1 and
+// exm[nx] (the right-hand face of node nx-1); k_spmv writes A'p = 0 there explicitly, so the
+// pads stay exactly 0 through the iteration and never contribute to a dot product.
 #pragma once
 #include "pb_internal.cuh"
 
@@ -67,11 +68,12 @@ __global__ void __launch_bounds__(512) k_spmv(const SpmvArgs<T> a)
     const int tx = tid % TXV, ty = tid / TXV;
     const int x0 = bx * TXV * VEC, j0 = by * TY;
     const int i0 = x0 + tx * VEC, j = j0 + ty;
-    const bool active = (i0 < P) && (j < ny);
+    const bool intile = ty < TY;                 // blockDim is rounded up to whole warps
+    const bool active = intile && (i0 < P) && (j < ny);
     const int k0 = bz * a.TZ, k1 = min(k0 + a.TZ, nz);
     const int SW = TXV * VEC + 2 * VEC;          // smem row: VEC pad | TXV*VEC data | VEC pad
     const int planeSz = (TY + 2) * SW;
-    (void)nx;
+    const int nvalid = nx - i0;                  // elements e < nvalid of this thread's vector are grid nodes
 
     // p_new = z + beta*p_old at an arbitrary position (0 outside the grid: ghost p = 0)
     auto pnew_vec = [&](int k, int jj, int ii) -> Vec<T> {
@@ -95,7 +97,7 @@ __global__ void __launch_bounds__(512) k_spmv(const SpmvArgs<T> a)
     // stage plane k of p_new into shared buffer s: own vector + the tile's halo rows/columns
     auto stage = [&](int s, int k, const Vec<T> &own) {
         T *pl = sm + s * planeSz;
-        stv(pl + (ty + 1) * SW + VEC + tx * VEC, own);
+        if (intile) stv(pl + (ty + 1) * SW + VEC + tx * VEC, own);
         for (int h = tid; h < 2 * TXV; h += nthr) {           // halo rows j0-1 and j0+TY
             const int side = h / TXV, hx = h - side * TXV;
             const int jj = side ? j0 + TY : j0 - 1;
@@ -146,6 +148,7 @@ __global__ void __launch_bounds__(512) k_spmv(const SpmvArgs<T> a)
                 v = fma(-eyh.a[e], dn.a[e], v);
                 v = fma(-ezc.a[e], pm.a[e], v);
                 v = fma(-ezn.a[e], pn.a[e], v);
+                if (e >= nvalid) v = T(0);     // pad column: exm[nx] is node nx-1's face, not a row of A
                 if (MODE == 0) acc = fma((double)pc.a[e], (double)v, acc);
                 ap.a[e] = (MODE == 1) ? (T)((double)v * a.out_scale) : v;
             }
