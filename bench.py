@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- Jacobi-PCG on synthetic Poisson-Boltzmann grids: iterations/s, time-to-solution, roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--precision f32]
+
+A "step" is one complete pb_solve (rows a1-a6 of SURVEY.md section 8(a): init, K_spmv/K_vec iterations with
+the on-device convergence latch, un-pad) on one right-hand side.  At N=1 the workload is BASELINE.json
+configs[4] (385^3, 60 000 atoms, fp32 to relative residual 1e-5), the configuration the north-star metric is
+quoted on.  For N>1 every rank solves its own member of config 5's perturbed-charge batch on its own copy of
+the operator (replicas, no data-path collective): weak scaling.  One JSON line is printed by rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "pcg_iterations_per_s"
+UNIT = "iterations/s"
+WORDS_SPMV = 8      # z, p, eps_x, eps_y, eps_z, D read; p, Ap written
+WORDS_VEC = 8       # x, p, r, Ap, Dinv read; x, r, z written
+TOL = {"f32": 1e-5, "f64": 1e-10}
+GRID = {1: 33, 2: 65, 3: 129, 4: 257, 5: 385}
+
+
+def parse_args(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config (1-based); 5 = headline")
+    ap.add_argument("--precision", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--tol", type=float, default=None)
+    ap.add_argument("--check-every", type=int, default=32)
+    ap.add_argument("--maxiter", type=int, default=20000)
+    ap.add_argument("--profile-iters", type=int, default=40)
+    ap.add_argument("--cpu-sample-iters", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args(argv)
+
+
+def measured_peak():
+    """HBM GB/s denominator: MEASURED_PEAKS.json (driver-written) else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload_key):
+    """dram bytes per K_spmv launch from the committed ncu --set full summary, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(workload_key)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (pynvml, 100 ms period)."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+
+    def __init__(self, index):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+
+    def _run(self):
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+            while not self._stop.is_set():
+                self.samples.append(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                try:
+                    r = pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    r = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self._stop.wait(0.1)
+        except Exception as e:  # no NVML: report that instead of clocks
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        self._t.join(timeout=2)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def aggregate(local_units, local_ms, world, device=None):
+    """Whole-job numbers: sum of the units all ranks processed, max over ranks of the device time."""
+    if world == 1:
+        return float(local_units), float(local_ms)
+    import torch
+    import torch.distributed as dist
+
+    dev = device if device is not None else "cpu"
+    u = torch.tensor([float(local_units)], dtype=torch.float64, device=dev)
+    t = torch.tensor([float(local_ms)], dtype=torch.float64, device=dev)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(u.item()), float(t.item())
+
+
+def workload_name(cfg, prec, tol):
+    n = GRID[cfg]
+    return f"config{cfg}_{n}^3_{prec}_tol{tol:g}"
+
+
+def build_inputs(cfg, rank, world, device):
+    """Seeded synthetic inputs (workloads/): the operator of config `cfg`; rank r > 0 (or any rank of a
+    multi-GPU run) takes member r of the perturbed-charge batch as its right-hand side."""
+    from workloads import make_config, perturbed_charges
+
+    inp = make_config(cfg, device=device)
+    rhs, bc = inp.rhs, inp.bc
+    if world > 1 and "charges" in inp.meta:
+        rhs, bc = perturbed_charges(inp, rank, device=device)
+    return inp, np.ascontiguousarray(rhs), np.ascontiguousarray(bc)
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return None
+    from oracle import pbref
+
+    prec = args.precision
+    tol = args.tol or TOL[prec]
+    try:
+        import torch
+
+        dev = "cuda" if torch.cuda.is_available() else "cpu"
+    except Exception:
+        dev = "cpu"
+    inp, rhs, bc = build_inputs(args.config, 0, 1, dev)
+    n_node = inp.n
+    sample = args.cpu_sample_iters or max(2, min(200, int(3.0e8 / n_node)))
+    ref = pbref.from_inputs(inp)
+    for _ in range(args.warmup):
+        ref.solve(tol, min(sample, 2))
+    t0 = time.perf_counter()
+    iters = 0
+    for _ in range(args.steps):
+        iters += ref.solve(tol, sample)["iters"]
+    dt = time.perf_counter() - t0
+    ref.close()
+    val = iters / dt
+    desc = f"first {sample} PCG iterations of {workload_name(args.config, prec, tol)} per step (fp64 oracle)"
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": workload_name(args.config, prec, tol), "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": pbref.num_threads(), "kind": "oracle",
+                             "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1704_02745_b200 import build as pb_build
+
+    if rank == 0:
+        pb_build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_1704_02745_b200 as pkg
+
+    pkg.load_library()
+    prec = args.precision
+    tol = args.tol or TOL[prec]
+    tdt = torch.float32 if prec == "f32" else torch.float64
+    t_gen = time.perf_counter()
+    inp, rhs, bc = build_inputs(args.config, rank, world, f"cuda:{local_rank}")
+    t_gen = time.perf_counter() - t_gen
+    n_node, elt = inp.n, (4 if prec == "f32" else 8)
+
+    stream = torch.cuda.Stream(device=dev)
+    t_create = time.perf_counter()
+    solver = pkg.PBSolver(inp.nx, inp.ny, inp.nz, inp.h, inp.eps_x, inp.eps_y, inp.eps_z, inp.kbar2, rhs, bc,
+                          stream=stream.cuda_stream)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t_create
+    out_d = torch.empty(solver.shape, dtype=tdt, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident leg: `value` -------------------------------------------------------------
+    for _ in range(args.warmup):
+        res = solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)
+    barrier()
+    l0 = solver.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    iters = 0
+    with ClockSampler(physical_gpu_index(local_rank)) as clocks:
+        e0.record(stream)
+        for _ in range(args.steps):
+            res = solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)
+            iters += res["iters"]
+        e1.record(stream)
+        barrier()
+    ms_local = e0.elapsed_time(e1)
+    launches = solver.launch_count() - l0
+    tot_iters, ms = aggregate(iters, ms_local, world, dev)
+    value = tot_iters / (ms * 1e-3)
+
+    # ---- end-to-end leg: host buffers, H2D of rhs/bc and D2H of phi inside the timed region -------
+    e2e = None
+    if not args.no_e2e:
+        rhs_h = torch.from_numpy(rhs).pin_memory()
+        bc_h = torch.from_numpy(bc).pin_memory()
+        out_h = torch.empty(solver.shape, dtype=tdt).pin_memory()
+        for _ in range(min(args.warmup, 2)):
+            solver.set_rhs(rhs_h, bc_h)
+            solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_h)
+        barrier()
+        it2 = 0
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            solver.set_rhs(rhs_h, bc_h)
+            it2 += solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_h)["iters"]
+        torch.cuda.synchronize()
+        ms2_local = 1e3 * (time.perf_counter() - t0)
+        barrier()
+        tot2, ms2 = aggregate(it2, ms2_local, world, dev)
+        e2e = {"value": tot2 / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2 / args.steps,
+               "h2d_bytes_per_step": int(rhs.nbytes + bc.nbytes), "d2h_bytes_per_step": int(n_node * elt + 96)}
+        del rhs_h, bc_h, out_h
+
+    # ---- roofline of the dominant kernel (K_spmv), CUDA events around every launch ----------------
+    solver.solve_begin(prec)
+    solver.iterate(prec, 5)
+    ms_spmv, ms_vec = solver.profile(prec, args.profile_iters)
+    peak, peak_src = measured_peak()
+    wl = workload_name(args.config, prec, tol)
+    spmv_bytes = WORDS_SPMV * elt * n_node
+    ach = spmv_bytes / (ms_spmv * 1e-3) / 1e9
+    iter_bytes = (WORDS_SPMV + WORDS_VEC) * elt * n_node
+    roofline = {"bound": "hbm", "kernel": "k_spmv", "achieved": ach, "peak": peak, "unit": "GB/s",
+                "frac": ach / peak, "traffic": ncu_traffic(f"k_spmv:{wl}"), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": spmv_bytes, "ms_per_launch": ms_spmv,
+                "k_vec": {"achieved": WORDS_VEC * elt * n_node / (ms_vec * 1e-3) / 1e9, "ms_per_launch": ms_vec},
+                "iteration": {"achieved": iter_bytes * iters / (ms_local * 1e-3) / 1e9,
+                              "frac": iter_bytes * iters / (ms_local * 1e-3) / 1e9 / peak,
+                              "frac_of_8TBs": iter_bytes * iters / (ms_local * 1e-3) / 8e12,
+                              "note": "16 words/node/iteration over the whole timed solves (init, polls, un-pad included)"}}
+
+    line = None
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            from oracle import pbref
+
+            sample = args.cpu_sample_iters or max(2, min(400, int(1.2e10 / n_node)))
+            ref = pbref.from_inputs(inp)
+            t0 = time.perf_counter()
+            o = ref.solve(tol, sample)
+            dt = time.perf_counter() - t0
+            ref.close()
+            cpu = {"value": o["iters"] / dt, "unit": UNIT, "cores": pbref.num_threads(), "kind": "oracle",
+                   "sample": f"first {o['iters']} PCG iterations of {wl} (fp64 C/OpenMP oracle, {dt:.1f} s)"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
+                "config": {"workload": wl, "grid": [inp.nx, inp.ny, inp.nz], "unknowns_per_gpu": n_node,
+                           "tol": tol, "check_every": args.check_every, "iterations_per_solve": res["iters"],
+                           "final_relres": res["relres"], "time_to_solution_ms": ms / args.steps,
+                           "parallelism": f"replicas x{world} (one right-hand side per GPU)",
+                           "l2": "working set 11 arrays x %.0f MB >> 126 MB L2 (inputs larger than L2)"
+                                 % (n_node * elt / 1e6) if n_node * elt * 11 > 4e8 else "working set fits L2",
+                           "create_ms": 1e3 * t_create, "input_generation_s": t_gen},
+                "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu}
+    solver.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return line
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        line = run_reference(args, rank, world)
+    else:
+        line = run_ours(args, rank, local_rank, world)
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

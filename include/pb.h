@@ -112,6 +112,16 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
 pb_status pb_solve_begin(pb_handle *h, pb_precision prec);              /* steps 1-2: x=0, r=b, z=r/D */
 pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter);
 
+/*
+ * pb_profile -- like pb_iterate, but brackets every kernel with a CUDA event on the handle's
+ * stream and returns the mean device time (milliseconds) of K_spmv and of K_vec over the
+ * n_iter iterations.  Synchronises.  This is the roofline measurement of bench.py.
+ */
+pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spmv, double *ms_vec);
+
+/* Number of CUDA kernels this handle has enqueued so far (those inside launched graphs included). */
+long long pb_launch_count(pb_handle *h);
+
 /* pb_destroy(NULL) is a no-op.  Frees every device allocation of the handle. */
 pb_status pb_destroy(pb_handle *h);
 

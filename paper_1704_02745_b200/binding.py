@@ -18,7 +18,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
-           "pb_destroy", "pb_strerror", "pb_query", "pb_version")
+           "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -57,6 +57,9 @@ def load_library():
     lib.pb_strerror.argtypes = [ci]
     lib.pb_strerror.restype = ctypes.c_char_p
     lib.pb_version.restype = ci
+    lib.pb_profile.argtypes = [vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(cd)]
+    lib.pb_launch_count.argtypes = [vp]
+    lib.pb_launch_count.restype = ctypes.c_longlong
     for name in EXPORTS:
         getattr(lib, name)
     _lib = lib
@@ -200,6 +203,17 @@ class PBSolver:
         st = load_library().pb_iterate(self._h, _prec(precision)[0], int(n_iter))
         if st != PB_OK:
             raise PBError(st, "pb_iterate")
+
+    def profile(self, precision, n_iter):
+        """Mean device ms of (K_spmv, K_vec) over n_iter iterations continuing the current state."""
+        a, b = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        st = load_library().pb_profile(self._h, _prec(precision)[0], int(n_iter), ctypes.byref(a), ctypes.byref(b))
+        if st != PB_OK:
+            raise PBError(st, "pb_profile")
+        return a.value, b.value
+
+    def launch_count(self) -> int:
+        return int(load_library().pb_launch_count(self._h))
 
     def _query(self, what):
         out = np.empty(self.shape, dtype=np.float64)

@@ -50,6 +50,7 @@ struct pb_handle {
     Work<float> wf;
     Work<double> wd;
     int use_graph;
+    long long launches;          // kernels enqueued so far (graph-contained ones included)
     int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
 };
 
@@ -146,6 +147,7 @@ pb_status build_b(pb_handle *h, Work<T> &w)
     k_setup_b<T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
         h->eps_x, h->eps_y, h->eps_z, h->rhs, h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b);
     PB_CUDA(cudaGetLastError());
+    h->launches += 1;
     w.b_ready = true;
     return PB_OK;
 }
@@ -189,6 +191,7 @@ pb_status ensure(pb_handle *h)
         h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
         w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
     PB_CUDA(cudaGetLastError());
+    h->launches += 1;
     PB_TRY(build_b<T>(h, w));
     w.ready = true;
     return PB_OK;
@@ -227,6 +230,7 @@ pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
         k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
     }
     PB_CUDA(cudaGetLastError());
+    h->launches += 2LL * n;
     return PB_OK;
 }
 
@@ -239,6 +243,7 @@ pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch)
     k_set_state<<<1, 1, 0, h->stream>>>(h->st, tol * tol, maxiter, latch);
     k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w));
     PB_CUDA(cudaGetLastError());
+    h->launches += 2;
     return PB_OK;
 }
 
@@ -250,6 +255,7 @@ pb_status get_graph(pb_handle *h, Work<T> &w, int m)
     cudaGraph_t g = nullptr;
     PB_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
     pb_status s = enqueue_iterations<T>(h, w, m);
+    h->launches -= 2LL * m;          // captured, not executed
     cudaError_t e = cudaStreamEndCapture(h->stream, &g);
     if (s != PB_OK || e != cudaSuccess || !g) { cudaGetLastError(); return PB_ERR_CUDA; }
     e = cudaGraphInstantiate(&w.graph, g, 0);
@@ -282,7 +288,7 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     const long max_chunks = (long)maxiter / m + 2;
     int seen_done = 0;
     for (long c = 0; c < max_chunks + 1 && !seen_done; c++) {
-        if (graph_ok) PB_CUDA(cudaGraphLaunch(w.graph, h->stream));
+        if (graph_ok) { PB_CUDA(cudaGraphLaunch(w.graph, h->stream)); h->launches += 2LL * m; }
         else PB_TRY(enqueue_iterations<T>(h, w, m));
         int *slot = h->pinned + 4 * (c & 1);
         PB_CUDA(cudaMemcpyAsync(slot, &h->st->done, 4 * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
@@ -298,6 +304,7 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(T))); dst = (T *)h->stage; }
     k_unpad<T, T><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(w.x, dst, h->nx, w.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
+    h->launches += 1;
     if (where == PB_HOST)
         PB_CUDA(cudaMemcpyAsync(phi_out, dst, n * sizeof(T), cudaMemcpyDeviceToHost, h->stream));
     PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
@@ -330,6 +337,7 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
     k_spmv<T, 1><<<w.ntx * w.nty * w.ntz, (w.TXV * w.TY + 31) / 32 * 32, w.smem, h->stream>>>(sa);
     k_unpad<T, T><<<g, 256, 0, h->stream>>>(w.Ap, dst, h->nx, w.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
+    h->launches += 3;
     if (where == PB_HOST)
         PB_CUDA(cudaMemcpyAsync(y, dst, n * sizeof(T), cudaMemcpyDeviceToHost, h->stream));
     PB_CUDA(cudaStreamSynchronize(h->stream));
@@ -353,6 +361,49 @@ pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_
 bool valid_space(pb_memspace w) { return w == PB_HOST || w == PB_DEVICE; }
 bool valid_prec(pb_precision p) { return p == PB_F32 || p == PB_F64; }
 
+}  // namespace
+
+namespace {
+template <typename T>
+pb_status profile_impl(pb_handle *h, int n_iter, double *ms_spmv, double *ms_vec)
+{
+    Work<T> &w = work<T>(h);
+    if (!w.ready) return PB_ERR_INVALID_ARG;
+    const int ne = 2 * n_iter + 1;
+    cudaEvent_t *ev = (cudaEvent_t *)calloc(ne, sizeof(cudaEvent_t));
+    if (!ev) return PB_ERR_ALLOC;
+    pb_status s = PB_OK;
+    auto body = [&]() -> pb_status {
+        for (int i = 0; i < ne; i++) PB_CUDA(cudaEventCreate(&ev[i]));
+        const SpmvArgs<T> sa = spmv_args<T>(h, w);
+        const VecArgs<T> va = vec_args<T>(h, w);
+        const int sgrid = w.ntx * w.nty * w.ntz, sblock = (w.TXV * w.TY + 31) / 32 * 32;
+        PB_CUDA(cudaEventRecord(ev[0], h->stream));
+        for (int it = 0; it < n_iter; it++) {
+            k_spmv<T, 0><<<sgrid, sblock, w.smem, h->stream>>>(sa);
+            PB_CUDA(cudaEventRecord(ev[2 * it + 1], h->stream));
+            k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
+            PB_CUDA(cudaEventRecord(ev[2 * it + 2], h->stream));
+        }
+        PB_CUDA(cudaGetLastError());
+        h->launches += 2LL * n_iter;
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        double a = 0.0, b = 0.0;
+        for (int it = 0; it < n_iter; it++) {
+            float t1 = 0.f, t2 = 0.f;
+            PB_CUDA(cudaEventElapsedTime(&t1, ev[2 * it], ev[2 * it + 1]));
+            PB_CUDA(cudaEventElapsedTime(&t2, ev[2 * it + 1], ev[2 * it + 2]));
+            a += t1; b += t2;
+        }
+        if (ms_spmv) *ms_spmv = a / n_iter;
+        if (ms_vec) *ms_vec = b / n_iter;
+        return PB_OK;
+    };
+    s = body();
+    for (int i = 0; i < ne; i++) if (ev[i]) cudaEventDestroy(ev[i]);
+    free(ev);
+    return s;
+}
 }  // namespace
 
 extern "C" {
@@ -477,6 +528,16 @@ pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
     if (!h->wd.ready) return PB_ERR_INVALID_ARG;
     return enqueue_iterations<double>(h, h->wd, n_iter);
 }
+
+pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spmv, double *ms_vec)
+{
+    if (!h || !valid_prec(prec) || n_iter < 1) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? profile_impl<float>(h, n_iter, ms_spmv, ms_vec)
+                          : profile_impl<double>(h, n_iter, ms_spmv, ms_vec);
+}
+
+long long pb_launch_count(pb_handle *h) { return h ? h->launches : 0; }
 
 pb_status pb_query(pb_handle *h, int what, double *out_host)
 {
