@@ -4,6 +4,7 @@
 // No step of the method runs on the host.  Product code: shares nothing with oracle/.
 #include "../../include/pb.h"
 #include "pb_kernels.cuh"
+#include "pb_spmv_tma.cuh"
 #include "pb_setup.cuh"
 
 #include <cmath>
@@ -27,6 +28,11 @@ struct Work {
     size_t smem = 0;
     cudaGraphExec_t graph = nullptr;
     int graph_iters = 0;
+    // TMA pipeline configuration of k_spmv_tma (tile, ring depth, persistent grid, tensor maps)
+    bool use_tma = true;
+    int qTXV = 0, qTY = 0, qTZ = 0, qntx = 0, qnty = 0, qntz = 0, qns = 0, qgrid = 0, qthreads = 0;
+    size_t qsmem = 0;
+    CUtensorMap tm_z, tm_p0, tm_p1, tm_D, tm_ex, tm_ey, tm_ez;
 };
 
 }  // namespace
@@ -152,6 +158,8 @@ pb_status build_b(pb_handle *h, Work<T> &w)
     return PB_OK;
 }
 
+template <typename T> pb_status setup_tma(pb_handle *h, Work<T> &w);
+
 // Lazily build the arrays of precision T (setup row a0).
 template <typename T>
 pb_status ensure(pb_handle *h)
@@ -174,8 +182,11 @@ pb_status ensure(pb_handle *h)
         return s;
     }
     choose_tiles<T>(h, w);
-    const size_t need = (size_t)w.ntx * w.nty * w.ntz > (size_t)2 * w.vec_grid
-                            ? (size_t)w.ntx * w.nty * w.ntz : (size_t)2 * w.vec_grid;
+    w.use_tma = env_int("PB_LEGACY_SPMV", 0) == 0;
+    if (w.use_tma) PB_TRY(setup_tma<T>(h, w));
+    size_t need = (size_t)w.ntx * w.nty * w.ntz > (size_t)2 * w.vec_grid
+                      ? (size_t)w.ntx * w.nty * w.ntz : (size_t)2 * w.vec_grid;
+    if ((size_t)w.qgrid > need) need = (size_t)w.qgrid;
     if (need > h->partials_cap) {
         if (h->partials) cudaFree(h->partials);
         h->partials = nullptr;
@@ -218,15 +229,134 @@ VecArgs<T> vec_args(pb_handle *h, Work<T> &w)
     return a;
 }
 
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// 3-D tensor [planes][rows][P] of T, box = bx elements x by rows x 1 plane, zero fill outside
+template <typename T>
+pb_status make_map(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, int bx, int by)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return PB_ERR_CUDA;
+    const cuuint64_t dims[3] = {(cuuint64_t)P, (cuuint64_t)rows, (cuuint64_t)planes};
+    const cuuint64_t strides[2] = {(cuuint64_t)P * sizeof(T), (cuuint64_t)P * rows * sizeof(T)};
+    const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = fn(tm, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3,
+                          (void *)ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        if (getenv("PB_VERBOSE")) fprintf(stderr, "pb: cuTensorMapEncodeTiled failed (%d)\n", (int)r);
+        return PB_ERR_CUDA;
+    }
+    return PB_OK;
+}
+
+// tile / ring / grid selection and tensor maps for k_spmv_tma
+template <typename T>
+pb_status setup_tma(pb_handle *h, Work<T> &w)
+{
+    constexpr int VEC = VecN<T>::value;
+    const int rowvecs = w.P / VEC;
+    const int maxv = 256 / VEC - 2 < 62 ? 256 / VEC - 2 : 62;       // box inner dimension <= 256 elements
+    int ntx = (rowvecs + maxv - 1) / maxv;
+    int TXV = (rowvecs + ntx - 1) / ntx;
+    TXV = env_int("PB_TXV", TXV);
+    if (TXV < 1) TXV = 1;
+    if (TXV > maxv) TXV = maxv;
+    if (TXV > rowvecs) TXV = rowvecs;
+    int TY = env_int("PB_TY", 4);
+    if (TY < 1) TY = 1;
+    if (TY > h->ny) TY = h->ny;
+    while (TXV * TY > 448 && TY > 1) TY--;
+    int NS = env_int("PB_NS", 4);
+    if (NS < 3) NS = 3;
+    if (NS > kMaxStages) NS = kMaxStages;
+    w.qTXV = TXV; w.qTY = TY; w.qns = NS;
+    w.qntx = (rowvecs + TXV - 1) / TXV;
+    w.qnty = (h->ny + TY - 1) / TY;
+    w.qthreads = (TXV * TY + 31) / 32 * 32 + 32;
+    const SlotLayout L = slot_layout(TXV, TY);
+    w.qsmem = (size_t)NS * L.slot + 128;
+    if (w.qsmem > 227 * 1024) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.qsmem));
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.qsmem));
+    int bps = 1;
+    PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_spmv_tma<T, 0>, w.qthreads, w.qsmem));
+    if (bps < 1) bps = 1;
+    bps = env_int("PB_BPS", bps);
+    const int slots = kNumSM * bps;
+    // z-chunks: enough tiles for ~2 per resident block, chunks of at least 8 planes
+    const int xy = w.qntx * w.qnty;
+    int ntz = (2 * slots + xy - 1) / xy;
+    if (ntz < 1) ntz = 1;
+    int TZ = (h->nz + ntz - 1) / ntz;
+    if (TZ < 8) TZ = 8;
+    TZ = env_int("PB_TZ", TZ);
+    if (TZ < 1) TZ = 1;
+    if (TZ > h->nz) TZ = h->nz;
+    w.qTZ = TZ;
+    w.qntz = (h->nz + TZ - 1) / TZ;
+    const long ntiles = (long)xy * w.qntz;
+    w.qgrid = (int)(ntiles < slots ? ntiles : slots);
+    PB_TRY(make_map<T>(&w.tm_z, w.z, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_D, w.D, w.P, h->ny, h->nz, TXV * VEC, TY));
+    PB_TRY(make_map<T>(&w.tm_ex, w.exm, w.P, h->ny, h->nz, (TXV + 1) * VEC, TY));
+    PB_TRY(make_map<T>(&w.tm_ey, w.eym, w.P, h->ny + 1, h->nz, TXV * VEC, TY + 1));
+    PB_TRY(make_map<T>(&w.tm_ez, w.ezm, w.P, h->ny, h->nz + 1, TXV * VEC, TY));
+    if (getenv("PB_VERBOSE"))
+        fprintf(stderr, "pb: k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d tiles=%ldx grid=%d threads=%d smem=%zu bps=%d\n",
+                sizeof(T) == 4 ? "f32" : "f64", TXV, TY, TZ, NS, ntiles, w.qgrid, w.qthreads, w.qsmem, bps);
+    return PB_OK;
+}
+
+// one launch of the SpMV kernel (MODE 0: PCG step, MODE 1: y = scale*A'x)
+template <typename T, int MODE>
+void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
+{
+    if (w.use_tma) {
+        TmaArgs<T> a;
+        a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap;
+        a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
+        a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
+        a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns;
+        a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
+        k_spmv_tma<T, MODE><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+            w.tm_z, w.tm_p0, w.tm_p1, w.tm_D, w.tm_ex, w.tm_ey, w.tm_ez, a);
+    } else {
+        SpmvArgs<T> sa = spmv_args<T>(h, w);
+        sa.out_scale = out_scale;
+        k_spmv<T, MODE><<<w.ntx * w.nty * w.ntz, (w.TXV * w.TY + 31) / 32 * 32, w.smem, h->stream>>>(sa);
+    }
+}
+
 // enqueue n PCG iterations: (k_spmv, k_vec) pairs, nothing else
 template <typename T>
 pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
 {
-    const SpmvArgs<T> sa = spmv_args<T>(h, w);
     const VecArgs<T> va = vec_args<T>(h, w);
-    const int sgrid = w.ntx * w.nty * w.ntz, sblock = (w.TXV * w.TY + 31) / 32 * 32;
     for (int it = 0; it < n; it++) {
-        k_spmv<T, 0><<<sgrid, sblock, w.smem, h->stream>>>(sa);
+        launch_spmv<T, 0>(h, w, 1.0);
         k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
     }
     PB_CUDA(cudaGetLastError());
@@ -332,9 +462,7 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
     }
     const int g = grid_for(w.npad, 256, kNumSM * 16);
     k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.z, h->nx, w.P, rows);
-    SpmvArgs<T> sa = spmv_args<T>(h, w);
-    sa.out_scale = 1.0 / (h->h * h->h);
-    k_spmv<T, 1><<<w.ntx * w.nty * w.ntz, (w.TXV * w.TY + 31) / 32 * 32, w.smem, h->stream>>>(sa);
+    launch_spmv<T, 1>(h, w, 1.0 / (h->h * h->h));
     k_unpad<T, T><<<g, 256, 0, h->stream>>>(w.Ap, dst, h->nx, w.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
     h->launches += 3;
@@ -375,12 +503,10 @@ pb_status profile_impl(pb_handle *h, int n_iter, double *ms_spmv, double *ms_vec
     pb_status s = PB_OK;
     auto body = [&]() -> pb_status {
         for (int i = 0; i < ne; i++) PB_CUDA(cudaEventCreate(&ev[i]));
-        const SpmvArgs<T> sa = spmv_args<T>(h, w);
         const VecArgs<T> va = vec_args<T>(h, w);
-        const int sgrid = w.ntx * w.nty * w.ntz, sblock = (w.TXV * w.TY + 31) / 32 * 32;
         PB_CUDA(cudaEventRecord(ev[0], h->stream));
         for (int it = 0; it < n_iter; it++) {
-            k_spmv<T, 0><<<sgrid, sblock, w.smem, h->stream>>>(sa);
+            launch_spmv<T, 0>(h, w, 1.0);
             PB_CUDA(cudaEventRecord(ev[2 * it + 1], h->stream));
             k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
             PB_CUDA(cudaEventRecord(ev[2 * it + 2], h->stream));

@@ -1,0 +1,279 @@
+// pb_spmv_tma.cuh -- K_spmv, the dominant kernel of the PCG iteration, as a persistent,
+// warp-specialised TMA pipeline for sm_100a.
+//
+// Computes (steps 7b + 5a):  p <- z + beta*p ;  Ap = A'p ;  partial p.Ap
+// with A' rebuilt on the fly from the face dielectrics of Eq. 3.
+//
+// Structure.  A tile is TXV 16-byte vectors x TY rows x TZ planes.  Blocks are persistent and
+// stride over the tile list.  One producer lane streams "items" (one z-plane of the tile each)
+// through an NS-deep shared-memory ring with cp.async.bulk.tensor (TMA) and mbarriers:
+//     item q = { z(q), p_old(q) boxes with a 1-row / 1-vector halo,  ezm(q),  D(q), exm(q), eym(q) }
+// Out-of-range box elements are zero-filled by the TMA unit: that is the ghost layer p = 0.
+// The consumer warps turn the z/p_old boxes into p_new = z + beta*p_old in place (halo included:
+// the neighbours' p_new is recomputed, never re-read), keep the k-1/k/k+1 values of their own
+// column in registers, take the in-plane neighbours from the ring, and write Ap and p_new with
+// 128-bit stores.  One named barrier per plane among the consumers; no __syncthreads in the loop.
+#pragma once
+#include "pb_internal.cuh"
+#include "pb_tma.cuh"
+
+namespace pb {
+
+constexpr int kMaxStages = 8;
+
+template <typename T>
+struct TmaArgs {
+    T *pbuf0, *pbuf1;        // iteration l reads buf[l&1] (through its tensor map), writes buf[(l+1)&1]
+    T *Ap;
+    int nx, ny, nz, P;
+    int TXV, TY, TZ;
+    int ntx, nty, ntz, ntiles;
+    int nstage;
+    State *st;
+    double *partials;        // one per block
+    double out_scale;        // MODE 1 only
+};
+
+__host__ __device__ inline size_t align128(size_t v) { return (v + 127) & ~(size_t)127; }
+
+// byte sizes of the boxes of one item (also the smem carve-up of a ring slot)
+struct SlotLayout {
+    size_t szZ, szD, szEX, szEY, szEZ, slot;
+    uint32_t bZ, bD, bEX, bEY, bEZ;   // exact box bytes (what the TMA delivers)
+};
+__host__ __device__ inline SlotLayout slot_layout(int TXV, int TY) {
+    SlotLayout L;
+    L.bZ = (uint32_t)(TY + 2) * (TXV + 2) * 16;
+    L.bD = (uint32_t)TY * TXV * 16;
+    L.bEX = (uint32_t)TY * (TXV + 1) * 16;
+    L.bEY = (uint32_t)(TY + 1) * TXV * 16;
+    L.bEZ = L.bD;
+    L.szZ = align128(L.bZ); L.szD = align128(L.bD); L.szEX = align128(L.bEX);
+    L.szEY = align128(L.bEY); L.szEZ = align128(L.bEZ);
+    L.slot = 2 * L.szZ + L.szD + L.szEX + L.szEY + L.szEZ;
+    return L;
+}
+
+// MODE 0: PCG step;  MODE 1: y = out_scale * A' x (x behind tm_z, no p_old, no dot)
+template <typename T, int MODE>
+__global__ void __launch_bounds__(512)
+k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p0,
+           const __grid_constant__ CUtensorMap tm_p1, const __grid_constant__ CUtensorMap tm_D,
+           const __grid_constant__ CUtensorMap tm_ex, const __grid_constant__ CUtensorMap tm_ey,
+           const __grid_constant__ CUtensorMap tm_ez, const TmaArgs<T> a)
+{
+    constexpr int VEC = VecN<T>::value;
+    extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[kMaxStages];
+    __shared__ __align__(8) uint64_t empty_bar[kMaxStages];
+    __shared__ double red[32];
+    __shared__ int s_last;
+
+    const int tid = threadIdx.x;
+    const int nthr = blockDim.x;
+    const int NCT = nthr - 32;                 // consumer threads (whole warps); the last warp produces
+    const int NCW = NCT >> 5;
+    const int warp = tid >> 5, lane = tid & 31;
+    const bool is_producer = (warp == NCW);
+
+    T beta = T(0);
+    const CUtensorMap *tm_pin = &tm_p0;
+    T *pout = nullptr;
+    if (MODE == 0) {
+        if (a.st->done) return;
+        const int it = a.st->iter_cur;
+        beta = (T)a.st->beta;
+        tm_pin = (it & 1) ? &tm_p1 : &tm_p0;
+        pout = (it & 1) ? a.pbuf0 : a.pbuf1;
+    }
+    const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
+    const int TXV = a.TXV, TY = a.TY, TZ = a.TZ, NS = a.nstage;
+    const SlotLayout L = slot_layout(TXV, TY);
+    unsigned char *base = (unsigned char *)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; s++) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], NCW); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    double acc = 0.0;
+    if (is_producer) {
+        if (lane == 0) {
+            uint32_t cnt = 0;
+            for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+                int b = tile;
+                const int bx = b % a.ntx; b /= a.ntx;
+                const int by = b % a.nty;
+                const int bz = b / a.nty;
+                const int x0 = bx * TXV * VEC, j0 = by * TY;
+                const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
+                for (int q = k0 - 1; q <= k1; q++, cnt++) {
+                    const int s = cnt % NS;
+                    const uint32_t ph = (cnt / NS) & 1;
+                    mbar_wait(&empty_bar[s], ph ^ 1);
+                    unsigned char *slot = base + (size_t)s * L.slot;
+                    const bool coef = (q >= k0) && (q < k1);
+                    const bool ez = (q >= k0);
+                    uint32_t bytes = L.bZ * (MODE == 0 ? 2 : 1);
+                    if (ez) bytes += L.bEZ;
+                    if (coef) bytes += L.bD + L.bEX + L.bEY;
+                    mbar_expect_tx(&full_bar[s], bytes);
+                    tma_load_3d(slot, &tm_z, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                    if (MODE == 0) tma_load_3d(slot + L.szZ, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                    if (ez) tma_load_3d(slot + 2 * L.szZ + L.szD + L.szEX + L.szEY, &tm_ez, x0, j0, q, &full_bar[s]);
+                    if (coef) {
+                        tma_load_3d(slot + 2 * L.szZ, &tm_D, x0, j0, q, &full_bar[s]);
+                        tma_load_3d(slot + 2 * L.szZ + L.szD, &tm_ex, x0, j0, q, &full_bar[s]);
+                        tma_load_3d(slot + 2 * L.szZ + L.szD + L.szEX, &tm_ey, x0, j0, q, &full_bar[s]);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    } else {
+        const int BWc = TXV + 2;                       // vectors per row of the z/p boxes
+        const int tx = tid % TXV, ty = tid / TXV;
+        const bool intile = ty < TY;
+        const int own = (ty + 1) * BWc + tx + 1;       // own cell in the z/p boxes
+        const int cown = ty * TXV + tx;                // own cell in D / ezm boxes
+        const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
+
+        // p_new = z + beta*p_old in place over the halo cells of slot s; returns the own cell's p_new
+        auto update = [&](unsigned char *slot, bool with_halo) -> Vec<T> {
+            Vec<T> *Z = reinterpret_cast<Vec<T> *>(slot);
+            const Vec<T> *Pp = reinterpret_cast<const Vec<T> *>(slot + L.szZ);
+            Vec<T> v = zerov<T>();
+            if (intile) {
+                v = Z[own];
+                if (MODE == 0) {
+                    const Vec<T> pv = Pp[own];
+#pragma unroll
+                    for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], v.a[e]);
+                    if (with_halo) Z[own] = v;
+                }
+            }
+            if (MODE == 0 && with_halo) {
+                for (int h = NCT - 1 - tid; h < nextra; h += NCT) {
+                    int c;
+                    if (h < TXV) c = h + 1;
+                    else if (h < 2 * TXV) c = (TY + 1) * BWc + (h - TXV) + 1;
+                    else { const int cc = h - 2 * TXV, side = cc / TY, r = cc - side * TY; c = (r + 1) * BWc + (side ? TXV + 1 : 0); }
+                    Vec<T> w = Z[c];
+                    const Vec<T> pv = Pp[c];
+#pragma unroll
+                    for (int e = 0; e < VEC; e++) w.a[e] = fma(beta, pv.a[e], w.a[e]);
+                    Z[c] = w;
+                }
+            }
+            return v;
+        };
+        auto release = [&](int s) {                    // this warp is done with ring slot s
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[s]);
+        };
+
+        uint32_t cnt = 0;
+        for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+            int b = tile;
+            const int bx = b % a.ntx; b /= a.ntx;
+            const int by = b % a.nty;
+            const int bz = b / a.nty;
+            const int x0 = bx * TXV * VEC, j0 = by * TY;
+            const int i0 = x0 + tx * VEC, j = j0 + ty;
+            const bool active = intile && (i0 < P) && (j < ny);
+            const int nvalid = nx - i0;
+            const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
+
+            // item k0-1: only the own column's value is needed
+            int s = cnt % NS;
+            mbar_wait(&full_bar[s], (cnt / NS) & 1);
+            Vec<T> pm = update(base + (size_t)s * L.slot, false);
+            release(s);
+            cnt++;
+            // item k0
+            int sk = cnt % NS;
+            mbar_wait(&full_bar[sk], (cnt / NS) & 1);
+            unsigned char *slotk = base + (size_t)sk * L.slot;
+            Vec<T> pc = update(slotk, true);
+            Vec<T> ezc = intile ? reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ + L.szD + L.szEX + L.szEY)[cown] : zerov<T>();
+            cnt++;
+            named_bar_sync(1, NCT);
+
+            for (int k = k0; k < k1; k++) {
+                const int s1 = cnt % NS;
+                mbar_wait(&full_bar[s1], (cnt / NS) & 1);
+                unsigned char *slot1 = base + (size_t)s1 * L.slot;
+                const Vec<T> pn = update(slot1, k + 1 < k1);
+                const Vec<T> ezn = intile ? reinterpret_cast<const Vec<T> *>(slot1 + 2 * L.szZ + L.szD + L.szEX + L.szEY)[cown] : zerov<T>();
+                if (active) {
+                    const Vec<T> *Zk = reinterpret_cast<const Vec<T> *>(slotk);
+                    const Vec<T> *Dk = reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ);
+                    const Vec<T> *EXk = reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ + L.szD);
+                    const Vec<T> *EYk = reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ + L.szD + L.szEX);
+                    const Vec<T> up = Zk[own - BWc], dn = Zk[own + BWc];
+                    const T left = Zk[own - 1].a[VEC - 1], right = Zk[own + 1].a[0];
+                    const Vec<T> d = Dk[cown];
+                    const Vec<T> ex = EXk[ty * (TXV + 1) + tx];
+                    const T exr = EXk[ty * (TXV + 1) + tx + 1].a[0];
+                    const Vec<T> eyl = EYk[cown], eyh = EYk[cown + TXV];
+                    Vec<T> ap;
+#pragma unroll
+                    for (int e = 0; e < VEC; e++) {
+                        const T pl = (e == 0) ? left : pc.a[e == 0 ? 0 : e - 1];
+                        const T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
+                        const T exh = (e == VEC - 1) ? exr : ex.a[e == VEC - 1 ? e : e + 1];
+                        T v = d.a[e] * pc.a[e];
+                        v = fma(-ex.a[e], pl, v);
+                        v = fma(-exh, pr, v);
+                        v = fma(-eyl.a[e], up.a[e], v);
+                        v = fma(-eyh.a[e], dn.a[e], v);
+                        v = fma(-ezc.a[e], pm.a[e], v);
+                        v = fma(-ezn.a[e], pn.a[e], v);
+                        if (e >= nvalid) v = T(0);     // pad column: exm[nx] is node nx-1's face, not a row of A
+                        if (MODE == 0) acc = fma((double)pc.a[e], (double)v, acc);
+                        ap.a[e] = (MODE == 1) ? (T)((double)v * a.out_scale) : v;
+                    }
+                    const size_t idx = ((size_t)k * ny + j) * P + i0;
+                    stv(a.Ap + idx, ap);
+                    if (MODE == 0) stv(pout + idx, pc);
+                }
+                named_bar_sync(1, NCT);   // p_new(k+1) box complete; everyone is done with slot sk
+                release(sk);
+                pm = pc; pc = pn; ezc = ezn; sk = s1; slotk = slot1;
+                cnt++;
+            }
+            release(sk);                  // item k1 (only its own-column values were used)
+        }
+    }
+
+    if (MODE == 0) {
+        const double tot = block_sum(acc, red);
+        const int nblk = gridDim.x;
+        if (tid == 0) {
+            a.partials[blockIdx.x] = tot;
+            __threadfence();
+            const unsigned int t = atomicAdd(&a.st->ticket_spmv, 1u);
+            s_last = (t == (unsigned int)(nblk - 1));
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const double pAp = final_sum(a.partials, nblk, red);
+            if (tid == 0) {
+                State *st = a.st;
+                st->ticket_spmv = 0u;
+                st->pAp = pAp;
+                if (!(pAp > 0.0) || !isfinite(pAp)) {          // breakdown: not SPD / NaN
+                    if (st->latch) { st->done = 1; st->iters = st->iter_cur; st->status = 5; }
+                    st->alpha = 0.0;
+                } else {
+                    st->alpha = st->rz / pAp;                   // step 5
+                }
+            }
+        }
+    }
+}
+
+}  // namespace pb
