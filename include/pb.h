@@ -133,8 +133,9 @@ const char *pb_strerror(pb_status s);
  *   what = 0: diag(A) [nz][ny][nx] (1/h^2 included);  what = 1: folded b of Eq. 4 [nz][ny][nx];
  *   what = 2: the 10 device-resident scalars {r.z, p.Ap, r.r, b.b, alpha, beta, l, done, status, iters}
  *             of the h^2-scaled system as they stand on the stream (diagnostics, out_host[10]);
- *   what = 3..7: the work vectors r, z, p, A'p, x [nz][ny][nx] of the last pb_solve/pb_solve_begin
- *             precision, converted to fp64, in the h^2-scaled system A' = h^2 A (per-kernel parity tests).
+ *   what = 3..7: the work vectors r, Dinv, p, A'p, x [nz][ny][nx] of the last pb_solve/pb_solve_begin
+ *             precision, converted to fp64, in the h^2-scaled system A' = h^2 A (per-kernel parity tests);
+ *             x is the stored phi, i.e. without the still-pending alpha*p of the latest iteration.
  */
 pb_status pb_query(pb_handle *h, int what, double *out_host);
 

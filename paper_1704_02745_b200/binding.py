@@ -232,8 +232,9 @@ class PBSolver:
         return dict(zip(keys, out.tolist()))
 
     def vector(self, name):
-        """Work vector 'r','z','p','Ap' or 'x' of the last solve (h^2-scaled system), as fp64 numpy."""
-        return self._query({"r": 3, "z": 4, "p": 5, "Ap": 6, "x": 7}[name])
+        """Work vector 'r', 'Dinv', 'p', 'Ap' or 'x' of the last solve (h^2-scaled system), as fp64 numpy.
+        'x' is the stored phi: the update alpha*p of the latest iteration is still pending (see k_finish)."""
+        return self._query({"r": 3, "Dinv": 4, "p": 5, "Ap": 6, "x": 7}[name])
 
     def diag(self):
         return self._query(0)

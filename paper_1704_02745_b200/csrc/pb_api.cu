@@ -20,19 +20,17 @@ namespace {
 template <typename T>
 struct Work {
     T *exm = nullptr, *eym = nullptr, *ezm = nullptr, *D = nullptr, *Dinv = nullptr, *b = nullptr;
-    T *x = nullptr, *r = nullptr, *z = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr;
+    T *x = nullptr, *r = nullptr, *tmp = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr;   // tmp: pb_apply input
     int P = 0;
     size_t npad = 0;                 // nz*ny*P
     bool ready = false, b_ready = false;
-    int TXV = 0, TY = 0, TZ = 0, ntx = 0, nty = 0, ntz = 0, vec_grid = 0;
-    size_t smem = 0;
+    int vec_grid = 0;
     cudaGraphExec_t graph = nullptr;
     int graph_iters = 0;
     // TMA pipeline configuration of k_spmv_tma (tile, ring depth, persistent grid, tensor maps)
-    bool use_tma = true;
     int qTXV = 0, qTY = 0, qTZ = 0, qntx = 0, qnty = 0, qntz = 0, qns = 0, qgrid = 0, qthreads = 0;
     size_t qsmem = 0;
-    CUtensorMap tm_z, tm_p0, tm_p1, tm_D, tm_ex, tm_ey, tm_ez;
+    CUtensorMap tm_r, tm_tmp, tm_dinv, tm_p0, tm_p1, tm_x, tm_ex, tm_ey, tm_ez;
 };
 
 }  // namespace
@@ -101,36 +99,6 @@ inline int grid_for(size_t n, int block, int cap)
 constexpr int kNumSM = 148;   // B200
 
 template <typename T>
-void choose_tiles(pb_handle *h, Work<T> &w)
-{
-    constexpr int VEC = VecN<T>::value;
-    const int rowvecs = w.P / VEC;
-    int ntx = (rowvecs + 127) / 128;
-    int TXV = (rowvecs + ntx - 1) / ntx;
-    int TY = 512 / TXV;
-    if (TY > 16) TY = 16;
-    if (TY > h->ny) TY = h->ny;
-    if (TY < 1) TY = 1;
-    int TZ = 16;
-    TXV = env_int("PB_TXV", TXV);
-    if (TXV < 1) TXV = 1;
-    if (TXV > 512) TXV = 512;
-    if (TXV > rowvecs) TXV = rowvecs;
-    TY = env_int("PB_TY", TY);
-    if (TY < 1) TY = 1;
-    if (TXV * TY > 512) TY = 512 / TXV;
-    TZ = env_int("PB_TZ", TZ);
-    if (TZ < 1) TZ = 1;
-    if (TZ > h->nz) TZ = h->nz;
-    w.TXV = TXV; w.TY = TY; w.TZ = TZ;
-    w.ntx = (rowvecs + TXV - 1) / TXV;
-    w.nty = (h->ny + TY - 1) / TY;
-    w.ntz = (h->nz + TZ - 1) / TZ;
-    w.smem = (size_t)3 * (TY + 2) * (TXV * VEC + 2 * VEC) * sizeof(T);
-    w.vec_grid = grid_for(w.npad / VEC, 256, kNumSM * env_int("PB_VEC_BPS", 8));
-}
-
-template <typename T>
 pb_status alloc_arr(T **p, size_t n)
 {
     PB_CUDA(cudaMalloc((void **)p, (n + 64) * sizeof(T)));   // slack: vector tails never fault
@@ -140,7 +108,7 @@ pb_status alloc_arr(T **p, size_t n)
 template <typename T>
 void free_work(Work<T> &w)
 {
-    T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.z, &w.p0, &w.p1, &w.Ap};
+    T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.tmp, &w.p0, &w.p1, &w.Ap};
     for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
     w.ready = w.b_ready = false;
@@ -176,17 +144,14 @@ pb_status ensure(pb_handle *h)
     pb_status s = PB_OK;
     if ((s = alloc_arr(&w.exm, w.npad)) || (s = alloc_arr(&w.eym, n_ey)) || (s = alloc_arr(&w.ezm, n_ez)) ||
         (s = alloc_arr(&w.D, w.npad)) || (s = alloc_arr(&w.Dinv, w.npad)) || (s = alloc_arr(&w.b, w.npad)) ||
-        (s = alloc_arr(&w.x, w.npad)) || (s = alloc_arr(&w.r, w.npad)) || (s = alloc_arr(&w.z, w.npad)) ||
+        (s = alloc_arr(&w.x, w.npad)) || (s = alloc_arr(&w.r, w.npad)) || (s = alloc_arr(&w.tmp, w.npad)) ||
         (s = alloc_arr(&w.p0, w.npad)) || (s = alloc_arr(&w.p1, w.npad)) || (s = alloc_arr(&w.Ap, w.npad))) {
         free_work(w);
         return s;
     }
-    choose_tiles<T>(h, w);
-    w.use_tma = env_int("PB_LEGACY_SPMV", 0) == 0;
-    if (w.use_tma) PB_TRY(setup_tma<T>(h, w));
-    size_t need = (size_t)w.ntx * w.nty * w.ntz > (size_t)2 * w.vec_grid
-                      ? (size_t)w.ntx * w.nty * w.ntz : (size_t)2 * w.vec_grid;
-    if ((size_t)w.qgrid > need) need = (size_t)w.qgrid;
+    w.vec_grid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * env_int("PB_VEC_BPS", 8));
+    PB_TRY(setup_tma<T>(h, w));
+    const size_t need = (size_t)w.qgrid > (size_t)2 * w.vec_grid ? (size_t)w.qgrid : (size_t)2 * w.vec_grid;
     if (need > h->partials_cap) {
         if (h->partials) cudaFree(h->partials);
         h->partials = nullptr;
@@ -194,8 +159,6 @@ pb_status ensure(pb_handle *h)
         PB_CUDA(cudaMalloc((void **)&h->partials, need * sizeof(double)));
         h->partials_cap = need;
     }
-    PB_CUDA(cudaFuncSetAttribute(k_spmv<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
-    PB_CUDA(cudaFuncSetAttribute(k_spmv<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
     PB_CUDA(cudaMemsetAsync(h->bad, 0, sizeof(int), h->stream));
     const size_t total = (size_t)(h->nz + 1) * (h->ny + 1) * w.P;
     k_setup_coeff<T><<<grid_for(total, 256, kNumSM * 16), 256, 0, h->stream>>>(
@@ -209,23 +172,10 @@ pb_status ensure(pb_handle *h)
 }
 
 template <typename T>
-SpmvArgs<T> spmv_args(pb_handle *h, Work<T> &w)
-{
-    SpmvArgs<T> a;
-    a.z = w.z; a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap;
-    a.exm = w.exm; a.eym = w.eym; a.ezm = w.ezm; a.D = w.D;
-    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
-    a.TXV = w.TXV; a.TY = w.TY; a.TZ = w.TZ; a.ntx = w.ntx; a.nty = w.nty; a.ntz = w.ntz;
-    a.st = h->st; a.partials = h->partials; a.out_scale = 1.0;
-    return a;
-}
-
-template <typename T>
 VecArgs<T> vec_args(pb_handle *h, Work<T> &w)
 {
     VecArgs<T> a;
-    a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.x = w.x; a.r = w.r; a.z = w.z; a.Ap = w.Ap; a.Dinv = w.Dinv;
-    a.b = w.b; a.pzero = w.p0; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
+    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
     return a;
 }
 
@@ -287,7 +237,12 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     if (TY < 1) TY = 1;
     if (TY > h->ny) TY = h->ny;
     while (TXV * TY > 448 && TY > 1) TY--;
-    int NS = env_int("PB_NS", 4);
+    // ring depth: up to 4 slots with two blocks per SM if that leaves >= 3, else one block with a deep ring
+    const size_t slot_bytes = slot_layout(TXV, TY).slot;
+    int NS = (int)((116000 - 256) / slot_bytes);
+    if (NS > 4) NS = 4;
+    if (NS < 3) NS = (int)((232000 - 1280) / slot_bytes);
+    NS = env_int("PB_NS", NS);
     if (NS < 3) NS = 3;
     if (NS > kMaxStages) NS = kMaxStages;
     w.qTXV = TXV; w.qTY = TY; w.qns = NS;
@@ -317,10 +272,12 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     w.qntz = (h->nz + TZ - 1) / TZ;
     const long ntiles = (long)xy * w.qntz;
     w.qgrid = (int)(ntiles < slots ? ntiles : slots);
-    PB_TRY(make_map<T>(&w.tm_z, w.z, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_r, w.r, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_tmp, w.tmp, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
-    PB_TRY(make_map<T>(&w.tm_D, w.D, w.P, h->ny, h->nz, TXV * VEC, TY));
+    PB_TRY(make_map<T>(&w.tm_x, w.x, w.P, h->ny, h->nz, TXV * VEC, TY));
     PB_TRY(make_map<T>(&w.tm_ex, w.exm, w.P, h->ny, h->nz, (TXV + 1) * VEC, TY));
     PB_TRY(make_map<T>(&w.tm_ey, w.eym, w.P, h->ny + 1, h->nz, TXV * VEC, TY + 1));
     PB_TRY(make_map<T>(&w.tm_ez, w.ezm, w.P, h->ny, h->nz + 1, TXV * VEC, TY));
@@ -334,20 +291,14 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
 template <typename T, int MODE>
 void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
 {
-    if (w.use_tma) {
-        TmaArgs<T> a;
-        a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap;
-        a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
-        a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
-        a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns;
-        a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
-        k_spmv_tma<T, MODE><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
-            w.tm_z, w.tm_p0, w.tm_p1, w.tm_D, w.tm_ex, w.tm_ey, w.tm_ez, a);
-    } else {
-        SpmvArgs<T> sa = spmv_args<T>(h, w);
-        sa.out_scale = out_scale;
-        k_spmv<T, MODE><<<w.ntx * w.nty * w.ntz, (w.TXV * w.TY + 31) / 32 * 32, w.smem, h->stream>>>(sa);
-    }
+    TmaArgs<T> a;
+    a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap; a.x = w.x;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
+    a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
+    a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns;
+    a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
+    k_spmv_tma<T, MODE><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+        MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
 }
 
 // enqueue n PCG iterations: (k_spmv, k_vec) pairs, nothing else
@@ -432,7 +383,7 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
     T *dst = (T *)phi_out;
     if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(T))); dst = (T *)h->stage; }
-    k_unpad<T, T><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(w.x, dst, h->nx, w.P, rows, 1.0);
+    k_finish<T, T><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(w.x, w.p0, w.p1, h->st, dst, h->nx, w.P, rows);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     if (where == PB_HOST)
@@ -461,7 +412,7 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
         dst = (T *)h->stage;
     }
     const int g = grid_for(w.npad, 256, kNumSM * 16);
-    k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.z, h->nx, w.P, rows);
+    k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
     launch_spmv<T, 1>(h, w, 1.0 / (h->h * h->h));
     k_unpad<T, T><<<g, 256, 0, h->stream>>>(w.Ap, dst, h->nx, w.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
@@ -685,7 +636,7 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
         if (h->last_prec == PB_F32) {
             Work<float> &w = h->wf;
             if (!w.ready) return PB_ERR_INVALID_ARG;
-            const float *src[] = {w.r, w.z, nullptr, w.Ap, w.x};
+            const float *src[] = {w.r, w.Dinv, nullptr, w.Ap, w.x};
             const float *sp = src[what - 3];
             if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
                        PB_CUDA(cudaStreamSynchronize(h->stream)); sp = (h->pinned_state->iter_cur & 1) ? w.p1 : w.p0; }
@@ -693,7 +644,7 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
         } else {
             Work<double> &w = h->wd;
             if (!w.ready) return PB_ERR_INVALID_ARG;
-            const double *src[] = {w.r, w.z, nullptr, w.Ap, w.x};
+            const double *src[] = {w.r, w.Dinv, nullptr, w.Ap, w.x};
             const double *sp = src[what - 3];
             if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
                        PB_CUDA(cudaStreamSynchronize(h->stream)); sp = (h->pinned_state->iter_cur & 1) ? w.p1 : w.p0; }

@@ -1,15 +1,18 @@
 // pb_spmv_tma.cuh -- K_spmv, the dominant kernel of the PCG iteration, as a persistent,
 // warp-specialised TMA pipeline for sm_100a.
 //
-// Computes (steps 7b + 5a):  p <- z + beta*p ;  Ap = A'p ;  partial p.Ap
-// with A' rebuilt on the fly from the face dielectrics of Eq. 3.
+// Computes:  z = Dinv*r (step 6, Jacobi) ; p <- z + beta*p (step 7) ;
+// x += alpha_prev * p_old (the phi update of step 5, deferred by one kernel) ; Ap = A'p ; partial p.Ap
+// (step 5), with A' rebuilt on the fly from the face dielectrics of Eq. 3 and
+// D = 1/Dinv.  z is never stored: 10 words per node (reads r, Dinv, p, x, eps_x, eps_y, eps_z;
+// writes p, x, Ap) against k_vec's 4 -- the 14-word split of SURVEY.md section 8(d).
 //
 // Structure.  A tile is TXV 16-byte vectors x TY rows x TZ planes.  Blocks are persistent and
 // stride over the tile list.  One producer lane streams "items" (one z-plane of the tile each)
 // through an NS-deep shared-memory ring with cp.async.bulk.tensor (TMA) and mbarriers:
-//     item q = { z(q), p_old(q) boxes with a 1-row / 1-vector halo,  ezm(q),  D(q), exm(q), eym(q) }
+//     item q = { r(q), Dinv(q), p_old(q) boxes with a 1-row / 1-vector halo,  ezm(q),  x(q), exm(q), eym(q) }
 // Out-of-range box elements are zero-filled by the TMA unit: that is the ghost layer p = 0.
-// The consumer warps turn the z/p_old boxes into p_new = z + beta*p_old in place (halo included:
+// The consumer warps turn the r box into p_new = Dinv*r + beta*p_old in place (halo included:
 // the neighbours' p_new is recomputed, never re-read), keep the k-1/k/k+1 values of their own
 // column in registers, take the in-plane neighbours from the ring, and write Ap and p_new with
 // 128-bit stores.  One named barrier per plane among the consumers; no __syncthreads in the loop.
@@ -25,6 +28,7 @@ template <typename T>
 struct TmaArgs {
     T *pbuf0, *pbuf1;        // iteration l reads buf[l&1] (through its tensor map), writes buf[(l+1)&1]
     T *Ap;
+    T *x;                    // phi, updated with the previous iteration's alpha (MODE 0)
     int nx, ny, nz, P;
     int TXV, TY, TZ;
     int ntx, nty, ntz, ntiles;
@@ -39,7 +43,8 @@ __host__ __device__ inline size_t align128(size_t v) { return (v + 127) & ~(size
 // byte sizes of the boxes of one item (also the smem carve-up of a ring slot)
 struct SlotLayout {
     size_t szZ, szD, szEX, szEY, szEZ, slot;
-    uint32_t bZ, bD, bEX, bEY, bEZ;   // exact box bytes (what the TMA delivers)
+    size_t oR, oDv, oPp, oEZ, oX, oEX, oEY;   // offsets of the boxes inside a slot
+    uint32_t bZ, bD, bEX, bEY, bEZ;           // exact box bytes (what the TMA delivers)
 };
 __host__ __device__ inline SlotLayout slot_layout(int TXV, int TY) {
     SlotLayout L;
@@ -50,17 +55,20 @@ __host__ __device__ inline SlotLayout slot_layout(int TXV, int TY) {
     L.bEZ = L.bD;
     L.szZ = align128(L.bZ); L.szD = align128(L.bD); L.szEX = align128(L.bEX);
     L.szEY = align128(L.bEY); L.szEZ = align128(L.bEZ);
-    L.slot = 2 * L.szZ + L.szD + L.szEX + L.szEY + L.szEZ;
+    L.oR = 0; L.oDv = L.szZ; L.oPp = 2 * L.szZ;
+    L.oEZ = 3 * L.szZ; L.oX = L.oEZ + L.szEZ; L.oEX = L.oX + L.szD; L.oEY = L.oEX + L.szEX;
+    L.slot = L.oEY + L.szEY;
     return L;
 }
 
-// MODE 0: PCG step;  MODE 1: y = out_scale * A' x (x behind tm_z, no p_old, no dot)
+// MODE 0: PCG step;  MODE 1: y = out_scale * A' v  (v behind tm_r; no Dinv scaling, no p_old, no x, no dot)
 template <typename T, int MODE>
 __global__ void __launch_bounds__(512)
-k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p0,
-           const __grid_constant__ CUtensorMap tm_p1, const __grid_constant__ CUtensorMap tm_D,
-           const __grid_constant__ CUtensorMap tm_ex, const __grid_constant__ CUtensorMap tm_ey,
-           const __grid_constant__ CUtensorMap tm_ez, const TmaArgs<T> a)
+k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_dinv,
+           const __grid_constant__ CUtensorMap tm_p0, const __grid_constant__ CUtensorMap tm_p1,
+           const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_ex,
+           const __grid_constant__ CUtensorMap tm_ey, const __grid_constant__ CUtensorMap tm_ez,
+           const TmaArgs<T> a)
 {
     constexpr int VEC = VecN<T>::value;
     extern __shared__ unsigned char smem_raw[];
@@ -76,13 +84,14 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
     const int warp = tid >> 5, lane = tid & 31;
     const bool is_producer = (warp == NCW);
 
-    T beta = T(0);
+    T beta = T(0), alpha_prev = T(0);
     const CUtensorMap *tm_pin = &tm_p0;
     T *pout = nullptr;
     if (MODE == 0) {
         if (a.st->done) return;
         const int it = a.st->iter_cur;
         beta = (T)a.st->beta;
+        alpha_prev = (T)a.st->alpha;           // alpha of the previous iteration (0 before the first)
         tm_pin = (it & 1) ? &tm_p1 : &tm_p0;
         pout = (it & 1) ? a.pbuf0 : a.pbuf1;
     }
@@ -113,45 +122,55 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
                     const uint32_t ph = (cnt / NS) & 1;
                     mbar_wait(&empty_bar[s], ph ^ 1);
                     unsigned char *slot = base + (size_t)s * L.slot;
-                    const bool coef = (q >= k0) && (q < k1);
+                    const bool centre = (q >= k0) && (q < k1);   // q is a plane this tile writes
                     const bool ez = (q >= k0);
-                    uint32_t bytes = L.bZ * (MODE == 0 ? 2 : 1);
+                    uint32_t bytes = L.bZ * (MODE == 0 ? 3 : 1);
                     if (ez) bytes += L.bEZ;
-                    if (coef) bytes += L.bD + L.bEX + L.bEY;
+                    if (centre) bytes += L.bEX + L.bEY + (MODE == 0 ? L.bD : L.bZ);
                     mbar_expect_tx(&full_bar[s], bytes);
-                    tma_load_3d(slot, &tm_z, x0 - VEC, j0 - 1, q, &full_bar[s]);
-                    if (MODE == 0) tma_load_3d(slot + L.szZ, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s]);
-                    if (ez) tma_load_3d(slot + 2 * L.szZ + L.szD + L.szEX + L.szEY, &tm_ez, x0, j0, q, &full_bar[s]);
-                    if (coef) {
-                        tma_load_3d(slot + 2 * L.szZ, &tm_D, x0, j0, q, &full_bar[s]);
-                        tma_load_3d(slot + 2 * L.szZ + L.szD, &tm_ex, x0, j0, q, &full_bar[s]);
-                        tma_load_3d(slot + 2 * L.szZ + L.szD + L.szEX, &tm_ey, x0, j0, q, &full_bar[s]);
+                    tma_load_3d(slot + L.oR, &tm_r, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                    if (MODE == 0) {
+                        tma_load_3d(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                        tma_load_3d(slot + L.oPp, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                    } else if (centre) {
+                        tma_load_3d(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                    }
+                    if (ez) tma_load_3d(slot + L.oEZ, &tm_ez, x0, j0, q, &full_bar[s]);
+                    if (centre) {
+                        if (MODE == 0) tma_load_3d(slot + L.oX, &tm_x, x0, j0, q, &full_bar[s]);
+                        tma_load_3d(slot + L.oEX, &tm_ex, x0, j0, q, &full_bar[s]);
+                        tma_load_3d(slot + L.oEY, &tm_ey, x0, j0, q, &full_bar[s]);
                     }
                 }
             }
         }
         __syncwarp();
     } else {
-        const int BWc = TXV + 2;                       // vectors per row of the z/p boxes
+        const int BWc = TXV + 2;                       // vectors per row of the haloed boxes
         const int tx = tid % TXV, ty = tid / TXV;
         const bool intile = ty < TY;
-        const int own = (ty + 1) * BWc + tx + 1;       // own cell in the z/p boxes
-        const int cown = ty * TXV + tx;                // own cell in D / ezm boxes
+        const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
+        const int cown = ty * TXV + tx;                // own cell in the x / ezm / eym boxes
         const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
 
-        // p_new = z + beta*p_old in place over the halo cells of slot s; returns the own cell's p_new
+        // p_new = Dinv*r + beta*p_old (steps 6-7) in place in the r box; returns the own cell's p_new
+        auto pnew_cell = [&](Vec<T> *R, const Vec<T> *Dv, const Vec<T> *Pp, int c) -> Vec<T> {
+            Vec<T> v = R[c];
+            if (MODE == 0) {
+                const Vec<T> dv = Dv[c], pv = Pp[c];
+#pragma unroll
+                for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], dv.a[e] * v.a[e]);
+            }
+            return v;
+        };
         auto update = [&](unsigned char *slot, bool with_halo) -> Vec<T> {
-            Vec<T> *Z = reinterpret_cast<Vec<T> *>(slot);
-            const Vec<T> *Pp = reinterpret_cast<const Vec<T> *>(slot + L.szZ);
+            Vec<T> *R = reinterpret_cast<Vec<T> *>(slot + L.oR);
+            const Vec<T> *Dv = reinterpret_cast<const Vec<T> *>(slot + L.oDv);
+            const Vec<T> *Pp = reinterpret_cast<const Vec<T> *>(slot + L.oPp);
             Vec<T> v = zerov<T>();
             if (intile) {
-                v = Z[own];
-                if (MODE == 0) {
-                    const Vec<T> pv = Pp[own];
-#pragma unroll
-                    for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], v.a[e]);
-                    if (with_halo) Z[own] = v;
-                }
+                v = pnew_cell(R, Dv, Pp, own);
+                if (MODE == 0 && with_halo) R[own] = v;
             }
             if (MODE == 0 && with_halo) {
                 for (int h = NCT - 1 - tid; h < nextra; h += NCT) {
@@ -159,11 +178,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
                     if (h < TXV) c = h + 1;
                     else if (h < 2 * TXV) c = (TY + 1) * BWc + (h - TXV) + 1;
                     else { const int cc = h - 2 * TXV, side = cc / TY, r = cc - side * TY; c = (r + 1) * BWc + (side ? TXV + 1 : 0); }
-                    Vec<T> w = Z[c];
-                    const Vec<T> pv = Pp[c];
-#pragma unroll
-                    for (int e = 0; e < VEC; e++) w.a[e] = fma(beta, pv.a[e], w.a[e]);
-                    Z[c] = w;
+                    R[c] = pnew_cell(R, Dv, Pp, c);
                 }
             }
             return v;
@@ -197,7 +212,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
             mbar_wait(&full_bar[sk], (cnt / NS) & 1);
             unsigned char *slotk = base + (size_t)sk * L.slot;
             Vec<T> pc = update(slotk, true);
-            Vec<T> ezc = intile ? reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ + L.szD + L.szEX + L.szEY)[cown] : zerov<T>();
+            Vec<T> ezc = intile ? reinterpret_cast<const Vec<T> *>(slotk + L.oEZ)[cown] : zerov<T>();
             cnt++;
             named_bar_sync(1, NCT);
 
@@ -206,25 +221,25 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
                 mbar_wait(&full_bar[s1], (cnt / NS) & 1);
                 unsigned char *slot1 = base + (size_t)s1 * L.slot;
                 const Vec<T> pn = update(slot1, k + 1 < k1);
-                const Vec<T> ezn = intile ? reinterpret_cast<const Vec<T> *>(slot1 + 2 * L.szZ + L.szD + L.szEX + L.szEY)[cown] : zerov<T>();
+                const Vec<T> ezn = intile ? reinterpret_cast<const Vec<T> *>(slot1 + L.oEZ)[cown] : zerov<T>();
                 if (active) {
-                    const Vec<T> *Zk = reinterpret_cast<const Vec<T> *>(slotk);
-                    const Vec<T> *Dk = reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ);
-                    const Vec<T> *EXk = reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ + L.szD);
-                    const Vec<T> *EYk = reinterpret_cast<const Vec<T> *>(slotk + 2 * L.szZ + L.szD + L.szEX);
+                    const Vec<T> *Zk = reinterpret_cast<const Vec<T> *>(slotk + L.oR);     // p_new(k) box
+                    const Vec<T> *EXk = reinterpret_cast<const Vec<T> *>(slotk + L.oEX);
+                    const Vec<T> *EYk = reinterpret_cast<const Vec<T> *>(slotk + L.oEY);
                     const Vec<T> up = Zk[own - BWc], dn = Zk[own + BWc];
                     const T left = Zk[own - 1].a[VEC - 1], right = Zk[own + 1].a[0];
-                    const Vec<T> d = Dk[cown];
+                    const Vec<T> dinv = reinterpret_cast<const Vec<T> *>(slotk + L.oDv)[own];
                     const Vec<T> ex = EXk[ty * (TXV + 1) + tx];
                     const T exr = EXk[ty * (TXV + 1) + tx + 1].a[0];
                     const Vec<T> eyl = EYk[cown], eyh = EYk[cown + TXV];
+                    const size_t idx = ((size_t)k * ny + j) * P + i0;
                     Vec<T> ap;
 #pragma unroll
                     for (int e = 0; e < VEC; e++) {
                         const T pl = (e == 0) ? left : pc.a[e == 0 ? 0 : e - 1];
                         const T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
                         const T exh = (e == VEC - 1) ? exr : ex.a[e == VEC - 1 ? e : e + 1];
-                        T v = d.a[e] * pc.a[e];
+                        T v = (T(1) / dinv.a[e]) * pc.a[e];       // D = 1/Dinv: the diagonal of Eq. 3
                         v = fma(-ex.a[e], pl, v);
                         v = fma(-exh, pr, v);
                         v = fma(-eyl.a[e], up.a[e], v);
@@ -235,9 +250,16 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
                         if (MODE == 0) acc = fma((double)pc.a[e], (double)v, acc);
                         ap.a[e] = (MODE == 1) ? (T)((double)v * a.out_scale) : v;
                     }
-                    const size_t idx = ((size_t)k * ny + j) * P + i0;
                     stv(a.Ap + idx, ap);
-                    if (MODE == 0) stv(pout + idx, pc);
+                    if (MODE == 0) {
+                        stv(pout + idx, pc);
+                        // phi_{l-1} = phi_{l-2} + alpha_{l-1} p_{l-2}  (step 5 of the previous iteration)
+                        Vec<T> xv = reinterpret_cast<const Vec<T> *>(slotk + L.oX)[cown];
+                        const Vec<T> po = reinterpret_cast<const Vec<T> *>(slotk + L.oPp)[own];
+#pragma unroll
+                        for (int e = 0; e < VEC; e++) xv.a[e] = fma(alpha_prev, po.a[e], xv.a[e]);
+                        stv(a.x + idx, xv);
+                    }
                 }
                 named_bar_sync(1, NCT);   // p_new(k+1) box complete; everyone is done with slot sk
                 release(sk);
@@ -249,6 +271,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
     }
 
     if (MODE == 0) {
+        // stage 1 -> per-block partial; stage 2 by the last block to take a ticket (fixed order: deterministic)
         const double tot = block_sum(acc, red);
         const int nblk = gridDim.x;
         if (tid == 0) {
@@ -267,7 +290,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUt
                 st->pAp = pAp;
                 if (!(pAp > 0.0) || !isfinite(pAp)) {          // breakdown: not SPD / NaN
                     if (st->latch) { st->done = 1; st->iters = st->iter_cur; st->status = 5; }
-                    st->alpha = 0.0;
+                    st->alpha = 0.0;                            // x already holds the last good iterate
                 } else {
                     st->alpha = st->rz / pAp;                   // step 5
                 }
