@@ -26,8 +26,10 @@ import numpy as np  # noqa: E402
 
 METRIC = "pcg_iterations_per_s"
 UNIT = "iterations/s"
-WORDS_SPMV = 8      # z, p, eps_x, eps_y, eps_z, D read; p, Ap written
-WORDS_VEC = 8       # x, p, r, Ap, Dinv read; x, r, z written
+# Algorithmic words per node per launch ("tighter variant": z never stored, phi update deferred)
+WORDS_SPMV = 10     # r, Dinv, p, x, eps_x, eps_y, eps_z read; p, x, Ap written
+WORDS_VEC = 4       # r, Ap, Dinv read; r written
+WORDS_NORTH_STAR = 16   # the north-star accounting (8 + 8) the >=70 %-of-peak target is stated in
 TOL = {"f32": 1e-5, "f64": 1e-10}
 GRID = {1: 33, 2: 65, 3: 129, 4: 257, 5: 385}
 
@@ -285,14 +287,19 @@ def run_ours(args, rank, local_rank, world):
     spmv_bytes = WORDS_SPMV * elt * n_node
     ach = spmv_bytes / (ms_spmv * 1e-3) / 1e9
     iter_bytes = (WORDS_SPMV + WORDS_VEC) * elt * n_node
+    ns_bytes = WORDS_NORTH_STAR * elt * n_node
     roofline = {"bound": "hbm", "kernel": "k_spmv", "achieved": ach, "peak": peak, "unit": "GB/s",
                 "frac": ach / peak, "traffic": ncu_traffic(f"k_spmv:{wl}"), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": spmv_bytes, "ms_per_launch": ms_spmv,
                 "k_vec": {"achieved": WORDS_VEC * elt * n_node / (ms_vec * 1e-3) / 1e9, "ms_per_launch": ms_vec},
                 "iteration": {"achieved": iter_bytes * iters / (ms_local * 1e-3) / 1e9,
                               "frac": iter_bytes * iters / (ms_local * 1e-3) / 1e9 / peak,
-                              "frac_of_8TBs": iter_bytes * iters / (ms_local * 1e-3) / 8e12,
-                              "note": "16 words/node/iteration over the whole timed solves (init, polls, un-pad included)"}}
+                              "north_star_16word_GBs": ns_bytes * iters / (ms_local * 1e-3) / 1e9,
+                              "north_star_16word_frac_of_measured": ns_bytes * iters / (ms_local * 1e-3) / 1e9 / peak,
+                              "north_star_16word_frac_of_8TBs": ns_bytes * iters / (ms_local * 1e-3) / 8e12,
+                              "note": "achieved/frac: the 14 words/node/iteration this implementation moves, over the whole "
+                                      "timed solves (init, polls, un-pad included); north_star_*: the same time charged with "
+                                      "the 16-word accounting of SURVEY.md 8(d)"}}
 
     line = None
     if rank == 0:
