@@ -150,8 +150,7 @@ pb_status ensure(pb_handle *h)
         return s;
     }
     w.vec_grid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * env_int("PB_VEC_BPS", 8));
-    PB_TRY(setup_tma<T>(h, w));
-    const size_t need = (size_t)w.qgrid > (size_t)2 * w.vec_grid ? (size_t)w.qgrid : (size_t)2 * w.vec_grid;
+    const size_t need = (size_t)kNumSM * 8 > (size_t)2 * w.vec_grid ? (size_t)kNumSM * 8 : (size_t)2 * w.vec_grid;
     if (need > h->partials_cap) {
         if (h->partials) cudaFree(h->partials);
         h->partials = nullptr;
@@ -167,6 +166,7 @@ pb_status ensure(pb_handle *h)
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     PB_TRY(build_b<T>(h, w));
+    PB_TRY(setup_tma<T>(h, w));
     w.ready = true;
     return PB_OK;
 }
@@ -220,53 +220,31 @@ pb_status make_map(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, i
     return PB_OK;
 }
 
-// tile / ring / grid selection and tensor maps for k_spmv_tma
+struct TileCfg { int TXV, TY, NS, bps, TZ; };   // TZ = 0: derive from the tile count
+
+// apply one tile / ring / grid configuration: sizes, persistent grid, tensor maps
 template <typename T>
-pb_status setup_tma(pb_handle *h, Work<T> &w)
+pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
 {
     constexpr int VEC = VecN<T>::value;
     const int rowvecs = w.P / VEC;
-    const int maxv = 256 / VEC - 2 < 62 ? 256 / VEC - 2 : 62;       // box inner dimension <= 256 elements
-    int ntx = (rowvecs + maxv - 1) / maxv;
-    int TXV = (rowvecs + ntx - 1) / ntx;
-    TXV = env_int("PB_TXV", TXV);
-    if (TXV < 1) TXV = 1;
-    if (TXV > maxv) TXV = maxv;
-    if (TXV > rowvecs) TXV = rowvecs;
-    int TY = env_int("PB_TY", 4);
-    if (TY < 1) TY = 1;
-    if (TY > h->ny) TY = h->ny;
-    while (TXV * TY > 448 && TY > 1) TY--;
-    // ring depth: up to 4 slots with two blocks per SM if that leaves >= 3, else one block with a deep ring
-    const size_t slot_bytes = slot_layout(TXV, TY).slot;
-    int NS = (int)((116000 - 256) / slot_bytes);
-    if (NS > 4) NS = 4;
-    if (NS < 3) NS = (int)((232000 - 1280) / slot_bytes);
-    NS = env_int("PB_NS", NS);
-    if (NS < 3) NS = 3;
-    if (NS > kMaxStages) NS = kMaxStages;
+    const int TXV = c.TXV, TY = c.TY, NS = c.NS;
     w.qTXV = TXV; w.qTY = TY; w.qns = NS;
     w.qntx = (rowvecs + TXV - 1) / TXV;
     w.qnty = (h->ny + TY - 1) / TY;
     w.qthreads = (TXV * TY + 31) / 32 * 32 + 32;
     const SlotLayout L = slot_layout(TXV, TY);
     w.qsmem = (size_t)NS * L.slot + 128;
-    if (w.qsmem > 227 * 1024) return PB_ERR_INVALID_ARG;
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.qsmem));
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.qsmem));
-    int bps = 1;
-    PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_spmv_tma<T, 0>, w.qthreads, w.qsmem));
-    if (bps < 1) bps = 1;
-    bps = env_int("PB_BPS", bps);
-    const int slots = kNumSM * bps;
-    // z-chunks: enough tiles for ~2 per resident block, chunks of at least 8 planes
+    if (w.qsmem > 226 * 1024 || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
+    const int slots = kNumSM * c.bps;
     const int xy = w.qntx * w.qnty;
-    int ntz = (2 * slots + xy - 1) / xy;
-    if (ntz < 1) ntz = 1;
-    int TZ = (h->nz + ntz - 1) / ntz;
-    if (TZ < 8) TZ = 8;
-    TZ = env_int("PB_TZ", TZ);
-    if (TZ < 1) TZ = 1;
+    int TZ = c.TZ;
+    if (TZ <= 0) {
+        int ntz = (int)((1.9 * slots + xy - 1) / xy);   // smallest z split with ~2 tiles per resident block
+        if (ntz < 1) ntz = 1;
+        TZ = (h->nz + ntz - 1) / ntz;
+        if (TZ < 8) TZ = 8;
+    }
     if (TZ > h->nz) TZ = h->nz;
     w.qTZ = TZ;
     w.qntz = (h->nz + TZ - 1) / TZ;
@@ -281,9 +259,110 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     PB_TRY(make_map<T>(&w.tm_ex, w.exm, w.P, h->ny, h->nz, (TXV + 1) * VEC, TY));
     PB_TRY(make_map<T>(&w.tm_ey, w.eym, w.P, h->ny + 1, h->nz, TXV * VEC, TY + 1));
     PB_TRY(make_map<T>(&w.tm_ez, w.ezm, w.P, h->ny, h->nz + 1, TXV * VEC, TY));
+    return PB_OK;
+}
+
+template <typename T, int MODE> void launch_spmv(pb_handle *h, Work<T> &w, double out_scale);
+
+// deepest ring (<= 6 slots) that lets `bps` blocks of this tile share one SM's shared memory
+inline int ring_depth(int TXV, int TY, int bps)
+{
+    const size_t per_block = (size_t)232448 / bps - 1024 - 1152;   // 227 KB per SM, 1 KB reserved per block, statics
+    int NS = (int)(per_block / slot_layout(TXV, TY).slot);
+    return NS > 6 ? 6 : NS;
+}
+
+// Tile / ring / grid selection for k_spmv_tma.  Explicit PB_TXV/PB_TY/PB_NS/PB_BPS/PB_TZ win; otherwise a
+// short list of candidates (x splits of about 0.5-1 KB rows, 2-8 rows, 1-4 blocks per SM, the deepest ring
+// that fits) is timed on the handle's own arrays -- three launches each -- and the fastest is kept, like an
+// FFT plan.  PB_AUTOTUNE=0 takes the first feasible candidate instead (fully static choice).
+template <typename T>
+pb_status setup_tma(pb_handle *h, Work<T> &w)
+{
+    constexpr int VEC = VecN<T>::value;
+    const int rowvecs = w.P / VEC;
+    const int maxv = 256 / VEC - 2;                                  // box inner dimension <= 256 elements
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+    int ntx0 = (rowvecs + 32) / 64;                                  // rows of about 64 vectors (1 KB)
+    if (ntx0 < 1) ntx0 = 1;
+    while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
+    TileCfg cand[64];
+    int nc = 0;
+    const bool forced = getenv("PB_TXV") || getenv("PB_TY") || getenv("PB_NS") || getenv("PB_BPS") || getenv("PB_TZ");
+    if (forced) {
+        TileCfg c;
+        c.TXV = env_int("PB_TXV", (rowvecs + ntx0 - 1) / ntx0);
+        if (c.TXV < 1) c.TXV = 1;
+        if (c.TXV > maxv) c.TXV = maxv;
+        if (c.TXV > rowvecs) c.TXV = rowvecs;
+        c.TY = env_int("PB_TY", 4);
+        if (c.TY < 1) c.TY = 1;
+        if (c.TY > h->ny) c.TY = h->ny;
+        while (c.TXV * c.TY > 448 && c.TY > 1) c.TY--;
+        c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2) >= 4 ? 2 : 1);
+        if (c.bps < 1) c.bps = 1;
+        c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps));
+        c.TZ = env_int("PB_TZ", 0);
+        cand[nc++] = c;
+    } else {
+        static const int tys[] = {8, 4, 6, 3, 2};
+        for (int dx = 0; dx < 2; dx++) {
+            const int ntx = ntx0 + dx;
+            const int TXV = (rowvecs + ntx - 1) / ntx;
+            if (dx && TXV * VEC < 64) break;
+            for (int ty : tys) {
+                int TY = ty > h->ny ? h->ny : ty;
+                if (TXV * TY > 448) continue;
+                for (int bps = 1; bps <= 4; bps++) {
+                    const int NS = ring_depth(TXV, TY, bps);
+                    if (NS < 4 && !(NS == 3 && bps >= 2)) continue;
+                    const int cthreads = ((TXV * TY + 31) / 32 * 32) * bps;
+                    if (cthreads < 256 || cthreads > 1024) continue;     // consumer threads per SM
+                    if (nc < 64) cand[nc++] = TileCfg{TXV, TY, NS, bps, 0};
+                }
+            }
+        }
+        if (nc == 0) cand[nc++] = TileCfg{(rowvecs + ntx0 - 1) / ntx0, h->ny < 4 ? h->ny : 4, 4, 1, 0};
+    }
+    int best = 0;
+    const bool tune = nc > 1 && env_int("PB_AUTOTUNE", 1) != 0 && (double)h->nx * h->ny * h->nz >= 2.0e5;
+    if (tune) {
+        cudaEvent_t e0, e1;
+        PB_CUDA(cudaEventCreate(&e0));
+        PB_CUDA(cudaEventCreate(&e1));
+        PB_CUDA(cudaMemsetAsync(w.r, 0, w.npad * sizeof(T), h->stream));
+        PB_CUDA(cudaMemsetAsync(w.p0, 0, w.npad * sizeof(T), h->stream));
+        PB_CUDA(cudaMemsetAsync(w.p1, 0, w.npad * sizeof(T), h->stream));
+        PB_CUDA(cudaMemsetAsync(w.x, 0, w.npad * sizeof(T), h->stream));
+        k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
+        float tbest = 1e30f;
+        for (int i = 0; i < nc; i++) {
+            if (configure_tma<T>(h, w, cand[i]) != PB_OK) continue;
+            if ((size_t)w.qgrid > h->partials_cap) continue;
+            launch_spmv<T, 0>(h, w, 1.0);
+            cudaEventRecord(e0, h->stream);
+            for (int rep = 0; rep < 3; rep++) launch_spmv<T, 0>(h, w, 1.0);
+            cudaEventRecord(e1, h->stream);
+            if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+                cudaEventDestroy(e0); cudaEventDestroy(e1);
+                return PB_ERR_CUDA;
+            }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (getenv("PB_VERBOSE"))
+                fprintf(stderr, "pb: tune TXV=%d TY=%d NS=%d bps=%d TZ=%d grid=%d: %.4f ms\n", cand[i].TXV, cand[i].TY,
+                        cand[i].NS, cand[i].bps, w.qTZ, w.qgrid, ms / 3);
+            if (ms < tbest) { tbest = ms; best = i; }
+        }
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+    }
+    PB_TRY(configure_tma<T>(h, w, cand[best]));
     if (getenv("PB_VERBOSE"))
-        fprintf(stderr, "pb: k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d tiles=%ldx grid=%d threads=%d smem=%zu bps=%d\n",
-                sizeof(T) == 4 ? "f32" : "f64", TXV, TY, TZ, NS, ntiles, w.qgrid, w.qthreads, w.qsmem, bps);
+        fprintf(stderr, "pb: k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
+                sizeof(T) == 4 ? "f32" : "f64", w.qTXV, w.qTY, w.qTZ, w.qns, cand[best].bps,
+                w.qntx * w.qnty * w.qntz, w.qgrid, w.qthreads, w.qsmem, tune ? " (autotuned)" : "");
     return PB_OK;
 }
 
