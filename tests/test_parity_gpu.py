@@ -4,6 +4,8 @@ Tolerances are BASELINE.json's north_star: fp64 SpMV 1e-12 (componentwise backwa
 Reading 20), fp64 solve to 1e-10 within 1e-8 max|phi|, fp32 solve to 1e-5 within 1e-4 max|phi|,
 iteration counts within 5 % (at least +-1).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -244,4 +246,45 @@ def test_fullsize_385_spmv_and_solve_properties(pkg, pbref):
         b = ref.b()
         true = np.linalg.norm(b - ref.apply(g["phi"].astype(np.float64))) / np.linalg.norm(b)
         assert true < 1e-4, true
+    ref.close()
+
+
+TILE_ENV = ("PB_TXV", "PB_TY", "PB_NS", "PB_BPS", "PB_TZ", "PB_AUTOTUNE")
+TILE_CONFIGS = [dict(PB_AUTOTUNE=0), dict(PB_TXV=7, PB_TY=3, PB_NS=3, PB_BPS=2, PB_TZ=5),
+                dict(PB_TXV=20, PB_TY=8, PB_NS=6, PB_BPS=1, PB_TZ=99), dict(PB_TXV=5, PB_TY=2, PB_NS=4, PB_BPS=4, PB_TZ=1),
+                dict(PB_TXV=13, PB_TY=5, PB_NS=5, PB_BPS=3, PB_TZ=33), dict()]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_tiling_independence(pkg, pbref, prec):
+    """Every tile / ring / grid configuration of k_spmv_tma (halo boxes, TMA zero fill, ring hand-off, ragged
+    tiles) must give the SAME SpMV bit for bit -- a node's arithmetic does not depend on the tiling -- and
+    solves that agree with the oracle.  (compute-sanitizer is closed on this pool; this is the race/halo check.)"""
+    inp = random_operator(77, 45, 38, seed=21)
+    dt = np.float64 if prec == "f64" else np.float32
+    x = np.random.default_rng(2).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(dt)
+    ref = pbref.from_inputs(inp)
+    tol = 1e-10 if prec == "f64" else 1e-5
+    o = ref.solve(tol, 5000)
+    scale = np.max(np.abs(o["phi"]))
+    saved = {k: os.environ.pop(k, None) for k in TILE_ENV}
+    try:
+        y0 = None
+        for cfg in TILE_CONFIGS:
+            for k in TILE_ENV:
+                os.environ.pop(k, None)
+            os.environ.update({k: str(v) for k, v in cfg.items()})
+            with pkg.PBSolver(*inp.args()) as s:
+                y = s.apply(x, prec)
+                runs = [s.solve(tol, 5000, prec, check_every=9) for _ in range(2)]
+            if y0 is None:
+                y0 = y
+            assert np.array_equal(y, y0), cfg
+            assert np.array_equal(runs[0]["phi"], runs[1]["phi"]) and runs[0]["iters"] == runs[1]["iters"], cfg
+            assert abs(runs[0]["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), cfg
+            assert np.max(np.abs(runs[0]["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale, cfg
+    finally:
+        for k in TILE_ENV:
+            os.environ.pop(k, None)
+        os.environ.update({k: v for k, v in saved.items() if v is not None})
     ref.close()
