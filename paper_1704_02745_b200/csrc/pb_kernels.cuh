@@ -22,6 +22,7 @@
 // pads stay exactly 0 through the iteration and never contribute to a dot product.
 #pragma once
 #include "pb_internal.cuh"
+#include "pb_tma.cuh"
 
 namespace pb {
 
@@ -55,6 +56,7 @@ struct VecArgs {
     const T *b;               // k_init only
     T *x, *pzero;             // k_init only: phi_0 = 0 and the p buffer to clear
     size_t nvec;              // number of 16-byte vectors in a padded node array
+    int l2hints;              // 1: keep r and Dinv in L2 for the next k_spmv_tma, stream Ap
     State *st;
     double *partials;         // 2 per block
 };
@@ -95,13 +97,15 @@ __global__ void __launch_bounds__(256) k_vec(const VecArgs<T> a)
     __shared__ int s_last;
     if (a.st->done) return;
     const T alpha = (T)a.st->alpha;
+    const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0);
     double s_rz = 0.0, s_rr = 0.0;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < a.nvec; v += stride) {
         const size_t idx = (a.nvec - 1 - v) * VEC;
-        Vec<T> rv = ldv(a.r + idx);
-        const Vec<T> qv = ldv(a.Ap + idx);
-        const Vec<T> dv = ldv(a.Dinv + idx);
+        Vec<T> rv, qv, dv;
+        ld16_hint(rv.a, a.r + idx, pol_keep);
+        ld16_hint(qv.a, a.Ap + idx, pol_stream);
+        ld16_hint(dv.a, a.Dinv + idx, pol_keep);
 #pragma unroll
         for (int e = 0; e < VEC; e++) {
             rv.a[e] = fma(-alpha, qv.a[e], rv.a[e]);      // r_l = r_{l-1} - alpha A p     (step 5)
@@ -109,7 +113,7 @@ __global__ void __launch_bounds__(256) k_vec(const VecArgs<T> a)
             s_rz = fma((double)rv.a[e], (double)zv, s_rz);
             s_rr = fma((double)rv.a[e], (double)rv.a[e], s_rr);
         }
-        stv(a.r + idx, rv);
+        st16_hint(a.r + idx, rv.a, pol_keep);
     }
     reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, false);
 }

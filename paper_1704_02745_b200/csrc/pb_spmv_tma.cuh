@@ -33,6 +33,7 @@ struct TmaArgs {
     int TXV, TY, TZ;
     int ntx, nty, ntz, ntiles;
     int nstage;
+    int l2hints;             // 1: evict_last on r/Dinv/Ap (re-read by k_vec), evict_first on the streamed arrays
     State *st;
     double *partials;        // one per block
     double out_scale;        // MODE 1 only
@@ -109,6 +110,8 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     double acc = 0.0;
     if (is_producer) {
         if (lane == 0) {
+            const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0),
+                           pol_pold = l2_policy((a.l2hints & 4) ? 1 : 0);
             uint32_t cnt = 0;
             for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
                 int b = tile;
@@ -128,18 +131,18 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                     if (ez) bytes += L.bEZ;
                     if (centre) bytes += L.bEX + L.bEY + (MODE == 0 ? L.bD : L.bZ);
                     mbar_expect_tx(&full_bar[s], bytes);
-                    tma_load_3d(slot + L.oR, &tm_r, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                    tma_load_3d_hint(slot + L.oR, &tm_r, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
                     if (MODE == 0) {
-                        tma_load_3d(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s]);
-                        tma_load_3d(slot + L.oPp, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
+                        tma_load_3d_hint(slot + L.oPp, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s], pol_pold);
                     } else if (centre) {
-                        tma_load_3d(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s]);
+                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
                     }
-                    if (ez) tma_load_3d(slot + L.oEZ, &tm_ez, x0, j0, q, &full_bar[s]);
+                    if (ez) tma_load_3d_hint(slot + L.oEZ, &tm_ez, x0, j0, q, &full_bar[s], pol_stream);
                     if (centre) {
-                        if (MODE == 0) tma_load_3d(slot + L.oX, &tm_x, x0, j0, q, &full_bar[s]);
-                        tma_load_3d(slot + L.oEX, &tm_ex, x0, j0, q, &full_bar[s]);
-                        tma_load_3d(slot + L.oEY, &tm_ey, x0, j0, q, &full_bar[s]);
+                        if (MODE == 0) tma_load_3d_hint(slot + L.oX, &tm_x, x0, j0, q, &full_bar[s], pol_stream);
+                        tma_load_3d_hint(slot + L.oEX, &tm_ex, x0, j0, q, &full_bar[s], pol_stream);
+                        tma_load_3d_hint(slot + L.oEY, &tm_ey, x0, j0, q, &full_bar[s], pol_stream);
                     }
                 }
             }
@@ -152,6 +155,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
         const int cown = ty * TXV + tx;                // own cell in the x / ezm / eym boxes
         const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
+        const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0);
 
         // p_new = Dinv*r + beta*p_old (steps 6-7) in place in the r box; returns the own cell's p_new
         auto pnew_cell = [&](Vec<T> *R, const Vec<T> *Dv, const Vec<T> *Pp, int c) -> Vec<T> {
@@ -250,15 +254,15 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                         if (MODE == 0) acc = fma((double)pc.a[e], (double)v, acc);
                         ap.a[e] = (MODE == 1) ? (T)((double)v * a.out_scale) : v;
                     }
-                    stv(a.Ap + idx, ap);
+                    st16_hint(a.Ap + idx, ap.a, pol_keep);
                     if (MODE == 0) {
-                        stv(pout + idx, pc);
+                        st16_hint(pout + idx, pc.a, pol_stream);
                         // phi_{l-1} = phi_{l-2} + alpha_{l-1} p_{l-2}  (step 5 of the previous iteration)
                         Vec<T> xv = reinterpret_cast<const Vec<T> *>(slotk + L.oX)[cown];
                         const Vec<T> po = reinterpret_cast<const Vec<T> *>(slotk + L.oPp)[own];
 #pragma unroll
                         for (int e = 0; e < VEC; e++) xv.a[e] = fma(alpha_prev, po.a[e], xv.a[e]);
-                        stv(a.x + idx, xv);
+                        st16_hint(a.x + idx, xv.a, pol_stream);
                     }
                 }
                 named_bar_sync(1, NCT);   // p_new(k+1) box complete; everyone is done with slot sk
