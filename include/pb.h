@@ -104,6 +104,13 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
                    void *phi_out, pb_memspace where, int *iters_out, double *relres_out);
 
 /*
+ * pb_set_preconditioner -- kind 1 (default): Jacobi, M = diag(A); kind 0: M = I, i.e. the
+ * unpreconditioned CG the paper times as "GPU/CG" (its listing is sign-garbled, so it is run
+ * as the PCG recurrence of PAPER.md:104-126 with z = r, DESIGN.md Reading 1).  Applies to later solves.
+ */
+pb_status pb_set_preconditioner(pb_handle *h, int kind);
+
+/*
  * pb_iterate -- benchmarking/profiling entry: enqueue exactly `n_iter` PCG iterations
  * (K_spmv + K_vec pairs, PAPER.md:115-126 steps 4-8) with the convergence latch disabled,
  * continuing from the state left by pb_solve_begin.  Does not synchronise.  Used by

@@ -18,7 +18,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
-           "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count")
+           "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -59,6 +59,7 @@ def load_library():
     lib.pb_version.restype = ci
     lib.pb_profile.argtypes = [vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(cd)]
     lib.pb_launch_count.argtypes = [vp]
+    lib.pb_set_preconditioner.argtypes = [vp, ci]
     lib.pb_launch_count.restype = ctypes.c_longlong
     for name in EXPORTS:
         getattr(lib, name)
@@ -193,6 +194,12 @@ class PBSolver:
         if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
             raise PBError(st, "pb_solve")
         return dict(phi=out, iters=it.value, relres=rel.value, status=st)
+
+    def set_preconditioner(self, jacobi: bool):
+        """True (default): Jacobi-PCG; False: unpreconditioned CG (M = I)."""
+        st = load_library().pb_set_preconditioner(self._h, 1 if jacobi else 0)
+        if st != PB_OK:
+            raise PBError(st, "pb_set_preconditioner")
 
     def solve_begin(self, precision):
         st = load_library().pb_solve_begin(self._h, _prec(precision)[0])

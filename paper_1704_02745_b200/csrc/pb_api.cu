@@ -55,6 +55,7 @@ struct pb_handle {
     Work<double> wd;
     int use_graph;
     long long launches;          // kernels enqueued so far (graph-contained ones included)
+    int precond;                 // 1 Jacobi (default), 0 none
     int l2hints;                 // PB_L2HINTS (default 1): L2 eviction-priority hints across the two kernels
     int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
 };
@@ -176,7 +177,7 @@ template <typename T>
 VecArgs<T> vec_args(pb_handle *h, Work<T> &w)
 {
     VecArgs<T> a;
-    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.l2hints = h->l2hints; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
+    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.l2hints = h->l2hints; a.precond = h->precond; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
     return a;
 }
 
@@ -375,7 +376,7 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap; a.x = w.x;
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
     a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
-    a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->l2hints;
+    a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->l2hints; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
     k_spmv_tma<T, MODE><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
         MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
@@ -605,6 +606,7 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
     h->nx = nx; h->ny = ny; h->nz = nz; h->h = hh;
     h->use_graph = env_int("PB_NO_GRAPH", 0) ? 0 : 1;
     h->l2hints = env_int("PB_L2HINTS", 0);
+    h->precond = 1;
     pb_status s = PB_OK;
     auto body = [&]() -> pb_status {
         PB_CUDA(cudaGetDevice(&h->device));
@@ -669,6 +671,18 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out)
                           : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out);
+}
+
+pb_status pb_set_preconditioner(pb_handle *h, int kind)
+{
+    if (!h || (kind != 0 && kind != 1)) return PB_ERR_INVALID_ARG;
+    if (h->precond != kind) {
+        h->precond = kind;
+        // captured graphs hold the kernel arguments by value
+        if (h->wf.graph) { cudaGraphExecDestroy(h->wf.graph); h->wf.graph = nullptr; }
+        if (h->wd.graph) { cudaGraphExecDestroy(h->wd.graph); h->wd.graph = nullptr; }
+    }
+    return PB_OK;
 }
 
 pb_status pb_solve_begin(pb_handle *h, pb_precision prec)

@@ -56,6 +56,7 @@ struct VecArgs {
     const T *b;               // k_init only
     T *x, *pzero;             // k_init only: phi_0 = 0 and the p buffer to clear
     size_t nvec;              // number of 16-byte vectors in a padded node array
+    int precond;              // 1: Jacobi (z = Dinv r), 0: M = I (z = r)
     int l2hints;              // 1: keep r and Dinv in L2 for the next k_spmv_tma, stream Ap
     State *st;
     double *partials;         // 2 per block
@@ -109,7 +110,7 @@ __global__ void __launch_bounds__(256) k_vec(const VecArgs<T> a)
 #pragma unroll
         for (int e = 0; e < VEC; e++) {
             rv.a[e] = fma(-alpha, qv.a[e], rv.a[e]);      // r_l = r_{l-1} - alpha A p     (step 5)
-            const T zv = dv.a[e] * rv.a[e];               // M z_l = r_l, M = D            (step 6)
+            const T zv = a.precond ? dv.a[e] * rv.a[e] : rv.a[e];   // M z_l = r_l, M = D or I   (step 6)
             s_rz = fma((double)rv.a[e], (double)zv, s_rz);
             s_rr = fma((double)rv.a[e], (double)rv.a[e], s_rr);
         }
@@ -133,7 +134,7 @@ __global__ void __launch_bounds__(256) k_init(const VecArgs<T> a)
         const Vec<T> dv = ldv(a.Dinv + idx);
 #pragma unroll
         for (int e = 0; e < VEC; e++) {
-            const T zv = dv.a[e] * rv.a[e];
+            const T zv = a.precond ? dv.a[e] * rv.a[e] : rv.a[e];
             s_rz = fma((double)rv.a[e], (double)zv, s_rz);
             s_rr = fma((double)rv.a[e], (double)rv.a[e], s_rr);
         }

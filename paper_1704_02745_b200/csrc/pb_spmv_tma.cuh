@@ -33,6 +33,7 @@ struct TmaArgs {
     int TXV, TY, TZ;
     int ntx, nty, ntz, ntiles;
     int nstage;
+    int precond;             // 1: M = diag(A) (Jacobi); 0: M = I (plain CG)
     int l2hints;             // 1: evict_last on r/Dinv/Ap (re-read by k_vec), evict_first on the streamed arrays
     State *st;
     double *partials;        // one per block
@@ -155,15 +156,22 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
         const int cown = ty * TXV + tx;                // own cell in the x / ezm / eym boxes
         const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
+        const bool precond = a.precond != 0;
         const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0);
 
         // p_new = Dinv*r + beta*p_old (steps 6-7) in place in the r box; returns the own cell's p_new
         auto pnew_cell = [&](Vec<T> *R, const Vec<T> *Dv, const Vec<T> *Pp, int c) -> Vec<T> {
             Vec<T> v = R[c];
             if (MODE == 0) {
-                const Vec<T> dv = Dv[c], pv = Pp[c];
+                const Vec<T> pv = Pp[c];
+                if (precond) {
+                    const Vec<T> dv = Dv[c];
 #pragma unroll
-                for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], dv.a[e] * v.a[e]);
+                    for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], dv.a[e] * v.a[e]);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], v.a[e]);
+                }
             }
             return v;
         };

@@ -288,3 +288,26 @@ def test_tiling_independence(pkg, pbref, prec):
             os.environ.pop(k, None)
         os.environ.update({k: v for k, v in saved.items() if v is not None})
     ref.close()
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_unpreconditioned_cg_variant(pkg, pbref, prec, tol):
+    """NEXT row f3: the paper's GPU/CG (PAPER.md:76-94) = the same recurrence with M = I.  Same parity bar;
+    and Jacobi needs fewer iterations than CG on heterogeneous eps."""
+    inp = born_ion()
+    ref = pbref.from_inputs(inp)
+    o_cg = ref.solve(tol, 5000, precond=False)
+    o_pcg = ref.solve(tol, 5000, precond=True)
+    with pkg.PBSolver(*inp.args()) as s:
+        s.set_preconditioner(False)
+        g_cg = s.solve(tol, 5000, prec)
+        s.set_preconditioner(True)
+        g_pcg = s.solve(tol, 5000, prec)
+    ref.close()
+    scale = np.max(np.abs(o_pcg["phi"]))
+    lim = 1e-8 if prec == "f64" else 1e-4
+    for g, o in ((g_cg, o_cg), (g_pcg, o_pcg)):
+        assert g["status"] == 0
+        assert abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (g["iters"], o["iters"])
+        assert np.max(np.abs(g["phi"] - o["phi"])) <= lim * scale
+    assert g_pcg["iters"] < g_cg["iters"]
