@@ -49,6 +49,8 @@ def parse_args(argv=None):
     ap.add_argument("--cpu-sample-iters", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="also run this many solves of config 5's perturbed-charge batch on the same operator")
     return ap.parse_args(argv)
 
 
@@ -278,6 +280,27 @@ def run_ours(args, rank, local_rank, world):
                "h2d_bytes_per_step": int(rhs.nbytes + bc.nbytes), "d2h_bytes_per_step": int(n_node * elt + 96)}
         del rhs_h, bc_h, out_h
 
+    # ---- optional: the MD-snapshot batch (same operator, seeded charge perturbations), pb_set_rhs + pb_solve ----
+    batch = None
+    if args.batch > 0 and "charges" in inp.meta:
+        from workloads import perturbed_charges
+
+        t_b, it_b = 0.0, []
+        for sidx in range(args.batch):
+            rhs_s, bc_s = perturbed_charges(inp, world * sidx + rank, device=f"cuda:{local_rank}")
+            rhs_d = torch.from_numpy(np.ascontiguousarray(rhs_s)).to(dev)
+            bc_d = torch.from_numpy(np.ascontiguousarray(bc_s)).to(dev)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            solver.set_rhs(rhs_d, bc_d)
+            it_b.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
+            torch.cuda.synchronize()
+            t_b += time.perf_counter() - t0
+            del rhs_d, bc_d
+        batch = {"solves": args.batch, "solves_per_s": args.batch / t_b, "ms_per_solve": 1e3 * t_b / args.batch,
+                 "mean_iters": float(np.mean(it_b)), "min_iters": int(min(it_b)), "max_iters": int(max(it_b)),
+                 "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member, this rank only"}
+
     # ---- roofline of the dominant kernel (K_spmv), CUDA events around every launch ----------------
     solver.solve_begin(prec)
     solver.iterate(prec, 5)
@@ -327,6 +350,8 @@ def run_ours(args, rank, local_rank, world):
                            "create_ms": 1e3 * t_create, "input_generation_s": t_gen},
                 "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
                 "roofline": roofline, "cpu_baseline": cpu}
+        if batch is not None:
+            line["batch"] = batch
     solver.close()
     if world > 1:
         dist.barrier()
