@@ -104,6 +104,29 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
                    void *phi_out, pb_memspace where, int *iters_out, double *relres_out);
 
 /*
+ * pb_create_from_atoms -- NEXT row f1, the paper's stated next step "integrated grid stencil setup on GPU"
+ * (PAPER.md:11, 283): build the inputs of Eq. 3 on the device from atoms and hand them to pb_create.
+ *   centres [n_atoms][3] (x,y,z; node (i,j,k) sits at (i h, j h, k h)), radii [n_atoms], charges [n_atoms]
+ *   node is solute iff it lies within some atom sphere (d^2 <= R^2); eps_in there, eps_out elsewhere and on the
+ *   ghost layer; face eps = harmonic mean of its two nodes; kbar2 = kbar2_solvent on solvent
+ *   nodes, 0 in the solute; charges spread trilinearly, rhs = 4 pi q/h^3; ghost Dirichlet values =
+ *   sum_i q_i exp(-kappa r_i)/(eps_out r_i) with kappa^2 = kbar2_solvent/eps_out (free-space boundary).
+ * Needs nx,ny,nz >= 2.  The handle keeps the atom positions for pb_set_charges.
+ */
+pb_status pb_create_from_atoms(pb_handle **out, int nx, int ny, int nz, double h, int n_atoms,
+                               const double *centres, const double *radii, const double *charges,
+                               double eps_in, double eps_out, double kbar2_solvent,
+                               pb_memspace where, void *cuda_stream);
+
+/* pb_set_charges -- same atoms and operator, new charges [n_atoms]: new rhs and ghost values (an MD-snapshot-style
+ * batch member).  Only for handles made by pb_create_from_atoms. */
+pb_status pb_set_charges(pb_handle *h, const double *charges, pb_memspace where);
+
+/* pb_get_field -- copy one of the handle's dense fp64 input fields to the host (tests of pb_create_from_atoms):
+ * which = 0 eps_x, 1 eps_y, 2 eps_z, 3 kbar2, 4 rhs, 5 bc (layouts as in pb_create; a NULL input reads as zeros). */
+pb_status pb_get_field(pb_handle *h, int which, double *out_host);
+
+/*
  * pb_set_preconditioner -- kind 1 (default): Jacobi, M = diag(A); kind 0: M = I, i.e. the
  * unpreconditioned CG the paper times as "GPU/CG" (its listing is sign-garbled, so it is run
  * as the PCG recurrence of PAPER.md:104-126 with z = r, DESIGN.md Reading 1).  Applies to later solves.

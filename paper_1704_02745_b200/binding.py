@@ -18,7 +18,8 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
-           "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner")
+           "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
+           "pb_set_charges", "pb_get_field")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -60,6 +61,9 @@ def load_library():
     lib.pb_profile.argtypes = [vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(cd)]
     lib.pb_launch_count.argtypes = [vp]
     lib.pb_set_preconditioner.argtypes = [vp, ci]
+    lib.pb_create_from_atoms.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, ci, vp, vp, vp, cd, cd, cd, ci, vp]
+    lib.pb_set_charges.argtypes = [vp, vp, ci]
+    lib.pb_get_field.argtypes = [vp, ci, vp]
     lib.pb_launch_count.restype = ctypes.c_longlong
     for name in EXPORTS:
         getattr(lib, name)
@@ -137,6 +141,46 @@ class PBSolver:
             self._h = None
             raise PBError(st, "pb_create")
 
+    @classmethod
+    def from_atoms(cls, nx, ny, nz, h, centres, radii, charges, eps_in, eps_out, kbar2_solvent, stream=None):
+        """pb_create_from_atoms: grid / stencil setup on the GPU (mask, face eps, salt map, charges, DH ghosts)."""
+        lib = load_library()
+        self = cls.__new__(cls)
+        self.nx, self.ny, self.nz, self.h = int(nx), int(ny), int(nz), float(h)
+        na = int(np.asarray(radii).shape[0]) if not _is_torch(radii) else int(radii.numel())
+        c, s1, k1 = _marshal(centres, np.float64, 3 * na, "centres")
+        r, s2, k2 = _marshal(radii, np.float64, na, "radii")
+        q, s3, k3 = _marshal(charges, np.float64, na, "charges")
+        self._h = ctypes.c_void_p()
+        st = lib.pb_create_from_atoms(ctypes.byref(self._h), self.nx, self.ny, self.nz, self.h, na, c, r, q,
+                                      float(eps_in), float(eps_out), float(kbar2_solvent), _one_space([s1, s2, s3]),
+                                      ctypes.c_void_p(int(stream) if stream else None))
+        del k1, k2, k3
+        if st != PB_OK:
+            self._h = None
+            raise PBError(st, "pb_create_from_atoms")
+        self.n_atoms = na
+        return self
+
+    def set_charges(self, charges):
+        q, sp, keep = _marshal(charges, np.float64, self.n_atoms, "charges")
+        st = load_library().pb_set_charges(self._h, q, sp)
+        del keep
+        if st != PB_OK:
+            raise PBError(st, "pb_set_charges")
+
+    def field(self, name):
+        """Dense fp64 input field held by the handle: eps_x, eps_y, eps_z, kbar2, rhs or bc (numpy)."""
+        nx, ny, nz = self.nx, self.ny, self.nz
+        shapes = {"eps_x": (nz, ny, nx + 1), "eps_y": (nz, ny + 1, nx), "eps_z": (nz + 1, ny, nx),
+                  "kbar2": (nz, ny, nx), "rhs": (nz, ny, nx), "bc": (2 * (nz * ny + nz * nx + ny * nx),)}
+        which = list(shapes).index(name)
+        out = np.empty(shapes[name], dtype=np.float64)
+        st = load_library().pb_get_field(self._h, which, ctypes.c_void_p(out.ctypes.data))
+        if st != PB_OK:
+            raise PBError(st, "pb_get_field")
+        return out
+
     @property
     def shape(self):
         return (self.nz, self.ny, self.nx)
@@ -199,7 +243,8 @@ class PBSolver:
         """True (default): Jacobi-PCG; False: unpreconditioned CG (M = I)."""
         st = load_library().pb_set_preconditioner(self._h, 1 if jacobi else 0)
         if st != PB_OK:
-            raise PBError(st, "pb_set_preconditioner")
+            raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
+           "pb_set_charges", "pb_get_field")
 
     def solve_begin(self, precision):
         st = load_library().pb_solve_begin(self._h, _prec(precision)[0])

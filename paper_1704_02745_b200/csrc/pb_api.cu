@@ -6,6 +6,7 @@
 #include "pb_kernels.cuh"
 #include "pb_spmv_tma.cuh"
 #include "pb_setup.cuh"
+#include "pb_grid.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -56,6 +57,10 @@ struct pb_handle {
     int use_graph;
     long long launches;          // kernels enqueued so far (graph-contained ones included)
     int precond;                 // 1 Jacobi (default), 0 none
+    // pb_create_from_atoms keeps the atom geometry for pb_set_charges
+    double *atoms_c;             // [n_atoms][3], device
+    int n_atoms;
+    double atoms_eps_out, atoms_kappa;
     int l2hints;                 // PB_L2HINTS (default 1): L2 eviction-priority hints across the two kernels
     int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
 };
@@ -431,6 +436,7 @@ pb_status ensure_stage(pb_handle *h, size_t bytes)
 {
     if (bytes <= h->stage_bytes) return PB_OK;
     if (h->stage) cudaFree(h->stage);
+    if (h->atoms_c) cudaFree(h->atoms_c);
     h->stage = nullptr;
     h->stage_bytes = 0;
     PB_CUDA(cudaMalloc(&h->stage, bytes));
@@ -579,6 +585,7 @@ pb_status pb_destroy(pb_handle *h)
     if (h->partials) cudaFree(h->partials);
     if (h->bad) cudaFree(h->bad);
     if (h->stage) cudaFree(h->stage);
+    if (h->atoms_c) cudaFree(h->atoms_c);
     if (h->pinned) cudaFreeHost(h->pinned);
     if (h->pinned_state) cudaFreeHost(h->pinned_state);
     for (int i = 0; i < 2; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
@@ -777,3 +784,124 @@ const char *pb_strerror(pb_status s)
 int pb_version(void) { return 100; }
 
 }  // extern "C"
+
+// ---- NEXT row f1: grid / stencil setup on the GPU ---------------------------------------------------------
+namespace {
+struct DevTmp {                      // frees its device allocations on scope exit
+    void *p[12]; int n = 0;
+    ~DevTmp() { for (int i = 0; i < n; i++) if (p[i]) cudaFree(p[i]); }
+    pb_status get(void **out, size_t bytes) {
+        *out = nullptr;
+        PB_CUDA(cudaMalloc(out, bytes ? bytes : 8));
+        p[n++] = *out;
+        return PB_OK;
+    }
+    void release(void *q) { for (int i = 0; i < n; i++) if (p[i] == q) p[i] = nullptr; }
+};
+
+// rhs (dense [nz][ny][nx]) and bc from charges on the stored / given atom geometry
+pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
+                            double eps_out, double kappa, double *d_rhs, double *d_bc, cudaStream_t st)
+{
+    const size_t n = (size_t)nx * ny * nz;
+    const size_t nbc = 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx);
+    PB_CUDA(cudaMemsetAsync(d_rhs, 0, n * sizeof(double), st));
+    k_grid_spread<<<grid_for((size_t)n_atoms, 128, kNumSM * 8), 128, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh, d_rhs);
+    k_grid_rhs<<<grid_for(n, 256, kNumSM * 16), 256, 0, st>>>(d_rhs, n, 4.0 * 3.141592653589793, pow(hh, 3.0));
+    k_grid_dh<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
+                                                                            eps_out, kappa, d_bc);
+    PB_CUDA(cudaGetLastError());
+    return PB_OK;
+}
+}  // namespace
+
+extern "C" pb_status pb_create_from_atoms(pb_handle **out, int nx, int ny, int nz, double hh, int n_atoms,
+                                          const double *centres, const double *radii, const double *charges,
+                                          double eps_in, double eps_out, double kbar2_solvent,
+                                          pb_memspace where, void *cuda_stream)
+{
+    if (!out) return PB_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (nx < 2 || ny < 2 || nz < 2 || !(hh > 0.0) || !std::isfinite(hh) || n_atoms < 0 || (n_atoms && (!centres || !radii || !charges)) ||
+        !(eps_in > 0.0) || !(eps_out > 0.0) || !(kbar2_solvent >= 0.0) || !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    if ((double)nx * ny * nz > 2.0e9) return PB_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return PB_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;     // NULL: legacy default stream, ordered before the handle's own
+    const size_t n = (size_t)nx * ny * nz;
+    const size_t nbc = 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx);
+    const cudaMemcpyKind kind = where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    DevTmp tmp;
+    double *d_c, *d_R, *d_q, *ex, *ey, *ez, *kb, *rhs, *bc;
+    unsigned char *mask;
+    PB_TRY(tmp.get((void **)&d_c, (size_t)n_atoms * 3 * sizeof(double)));
+    PB_TRY(tmp.get((void **)&d_R, (size_t)n_atoms * sizeof(double)));
+    PB_TRY(tmp.get((void **)&d_q, (size_t)n_atoms * sizeof(double)));
+    PB_TRY(tmp.get((void **)&mask, n));
+    PB_TRY(tmp.get((void **)&ex, (size_t)nz * ny * (nx + 1) * sizeof(double)));
+    PB_TRY(tmp.get((void **)&ey, (size_t)nz * (ny + 1) * nx * sizeof(double)));
+    PB_TRY(tmp.get((void **)&ez, (size_t)(nz + 1) * ny * nx * sizeof(double)));
+    PB_TRY(tmp.get((void **)&kb, n * sizeof(double)));
+    PB_TRY(tmp.get((void **)&rhs, n * sizeof(double)));
+    PB_TRY(tmp.get((void **)&bc, nbc * sizeof(double)));
+    if (n_atoms) {
+        PB_CUDA(cudaMemcpyAsync(d_c, centres, (size_t)n_atoms * 3 * sizeof(double), kind, st));
+        PB_CUDA(cudaMemcpyAsync(d_R, radii, (size_t)n_atoms * sizeof(double), kind, st));
+        PB_CUDA(cudaMemcpyAsync(d_q, charges, (size_t)n_atoms * sizeof(double), kind, st));
+    }
+    PB_CUDA(cudaMemsetAsync(mask, 0, n, st));
+    if (n_atoms) k_grid_mask<<<n_atoms < 65535 ? n_atoms : 65535, 128, 0, st>>>(d_c, d_R, n_atoms, nx, ny, nz, hh, mask);
+    const size_t nf = (size_t)(nz + 1) * (ny + 1) * (nx + 1);
+    k_grid_faces<<<grid_for(nf, 256, kNumSM * 16), 256, 0, st>>>(mask, nx, ny, nz, eps_in, eps_out, kbar2_solvent,
+                                                                 ex, ey, ez, kb);
+    PB_CUDA(cudaGetLastError());
+    const double kappa = sqrt(kbar2_solvent / eps_out);
+    PB_TRY(charges_to_rhs_bc(d_c, d_q, n_atoms, nx, ny, nz, hh, eps_out, kappa, rhs, bc, st));
+    pb_handle *h = nullptr;
+    PB_TRY(pb_create(&h, nx, ny, nz, hh, ex, ey, ez, kb, rhs, bc, PB_DEVICE, cuda_stream));
+    h->atoms_c = d_c; tmp.release(d_c);
+    h->n_atoms = n_atoms; h->atoms_eps_out = eps_out; h->atoms_kappa = kappa;
+    h->launches += 5;
+    *out = h;
+    return PB_OK;
+}
+
+extern "C" pb_status pb_set_charges(pb_handle *h, const double *charges, pb_memspace where)
+{
+    if (!h || !h->atoms_c || (h->n_atoms && !charges) || !valid_space(where)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    const size_t n = (size_t)h->nx * h->ny * h->nz;
+    const size_t nbc = 2 * ((size_t)h->nz * h->ny + (size_t)h->nz * h->nx + (size_t)h->ny * h->nx);
+    DevTmp tmp;
+    double *d_q;
+    PB_TRY(tmp.get((void **)&d_q, (size_t)h->n_atoms * sizeof(double)));
+    PB_CUDA(cudaMemcpyAsync(d_q, charges, (size_t)h->n_atoms * sizeof(double),
+                            where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
+    if (!h->rhs) PB_CUDA(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
+    if (!h->bc) PB_CUDA(cudaMalloc((void **)&h->bc, (nbc + 8) * sizeof(double)));
+    PB_TRY(charges_to_rhs_bc(h->atoms_c, d_q, h->n_atoms, h->nx, h->ny, h->nz, h->h, h->atoms_eps_out,
+                             h->atoms_kappa, h->rhs, h->bc, h->stream));
+    h->launches += 3;
+    h->wf.b_ready = false;
+    h->wd.b_ready = false;
+    if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));
+    if (h->wd.ready) PB_TRY(build_b<double>(h, h->wd));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}
+
+extern "C" pb_status pb_get_field(pb_handle *h, int which, double *out_host)
+{
+    if (!h || !out_host || which < 0 || which > 5) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    const size_t n = (size_t)h->nx * h->ny * h->nz;
+    const size_t sizes[6] = {(size_t)h->nz * h->ny * (h->nx + 1), (size_t)h->nz * (h->ny + 1) * h->nx,
+                             (size_t)(h->nz + 1) * h->ny * h->nx, n, n,
+                             2 * ((size_t)h->nz * h->ny + (size_t)h->nz * h->nx + (size_t)h->ny * h->nx)};
+    const double *src[6] = {h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->rhs, h->bc};
+    if (!src[which]) { memset(out_host, 0, sizes[which] * sizeof(double)); return PB_OK; }   // NULL input = zeros
+    PB_CUDA(cudaMemcpyAsync(out_host, src[which], sizes[which] * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}

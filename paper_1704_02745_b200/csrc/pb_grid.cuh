@@ -1,0 +1,142 @@
+// pb_grid.cuh -- grid / stencil setup on the GPU (NEXT row f1; the paper's own stated next step,
+// "integrated grid stencil setup on GPU"): from atoms (centres, radii, charges) to the
+// inputs of Eq. 3: solute mask, harmonic-mean face dielectrics, salt map
+// (Stern mask of Eq. 1-2), trilinearly spread grid charges, and the free-space Debye-Hueckel ghost values
+// (PAPER.md:182).  Readings: DESIGN.md 8-11, 13, 18.  fp64 throughout; decisions that produce integers
+// (inside / outside a sphere, the base node of a charge) use explicitly rounded operations (__dmul_rn ...)
+// so that no FMA contraction can flip them relative to a plain IEEE evaluation.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pb {
+
+// one block per atom (grid-stride): mark every node of the atom's bounding box with d^2 <= R^2
+__global__ void k_grid_mask(const double *__restrict__ c, const double *__restrict__ rad, int n_atoms,
+                            int nx, int ny, int nz, double h, unsigned char *mask)
+{
+    for (int a = blockIdx.x; a < n_atoms; a += gridDim.x) {
+        const double cx = c[3 * a], cy = c[3 * a + 1], cz = c[3 * a + 2], R = rad[a];
+        const int i_lo = max(0, (int)ceil((cx - R) / h)), i_hi = min(nx - 1, (int)floor((cx + R) / h));
+        const int j_lo = max(0, (int)ceil((cy - R) / h)), j_hi = min(ny - 1, (int)floor((cy + R) / h));
+        const int k_lo = max(0, (int)ceil((cz - R) / h)), k_hi = min(nz - 1, (int)floor((cz + R) / h));
+        if (i_lo > i_hi || j_lo > j_hi || k_lo > k_hi) continue;
+        const int bx = i_hi - i_lo + 1, by = j_hi - j_lo + 1, bz = k_hi - k_lo + 1;
+        const double R2 = __dmul_rn(R, R);
+        for (int t = threadIdx.x; t < bx * by * bz; t += blockDim.x) {
+            const int i = i_lo + t % bx, j = j_lo + (t / bx) % by, k = k_lo + t / (bx * by);
+            const double dx = __dsub_rn(__dmul_rn((double)i, h), cx);
+            const double dy = __dsub_rn(__dmul_rn((double)j, h), cy);
+            const double dz = __dsub_rn(__dmul_rn((double)k, h), cz);
+            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dz, dz), __dmul_rn(dy, dy)), __dmul_rn(dx, dx));
+            if (d2 <= R2) mask[((size_t)k * ny + j) * nx + i] = 1;   // every writer stores the same value
+        }
+    }
+}
+
+__device__ __forceinline__ double node_eps(const unsigned char *mask, int nx, int ny, int nz, int k, int j, int i,
+                                           double eps_in, double eps_out)
+{
+    if (k < 0 || k >= nz || j < 0 || j >= ny || i < 0 || i >= nx) return eps_out;   // ghost layer = solvent
+    return mask[((size_t)k * ny + j) * nx + i] ? eps_in : eps_out;
+}
+__device__ __forceinline__ double harmonic(double a, double b)
+{
+    return __ddiv_rn(__dmul_rn(__dmul_rn(2.0, a), b), __dadd_rn(a, b));
+}
+
+// face dielectrics (harmonic mean of the two nodes a face joins) and the salt map, one pass over (nz+1)(ny+1)(nx+1)
+__global__ void k_grid_faces(const unsigned char *__restrict__ mask, int nx, int ny, int nz, double eps_in,
+                             double eps_out, double kbar2_solvent, double *eps_x, double *eps_y, double *eps_z,
+                             double *kbar2)
+{
+    const size_t total = (size_t)(nz + 1) * (ny + 1) * (nx + 1);
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(t % (nx + 1));
+        const size_t q = t / (nx + 1);
+        const int j = (int)(q % (ny + 1)), k = (int)(q / (ny + 1));
+        const double e = node_eps(mask, nx, ny, nz, k, j, i, eps_in, eps_out);
+        if (k < nz && j < ny)
+            eps_x[((size_t)k * ny + j) * (nx + 1) + i] = harmonic(node_eps(mask, nx, ny, nz, k, j, i - 1, eps_in, eps_out), e);
+        if (k < nz && i < nx)
+            eps_y[((size_t)k * (ny + 1) + j) * nx + i] = harmonic(node_eps(mask, nx, ny, nz, k, j - 1, i, eps_in, eps_out), e);
+        if (j < ny && i < nx)
+            eps_z[((size_t)k * ny + j) * nx + i] = harmonic(node_eps(mask, nx, ny, nz, k - 1, j, i, eps_in, eps_out), e);
+        if (k < nz && j < ny && i < nx)
+            kbar2[((size_t)k * ny + j) * nx + i] = mask[((size_t)k * ny + j) * nx + i] ? 0.0 : kbar2_solvent;
+    }
+}
+
+// trilinear spreading of the point charges to their 8 surrounding nodes (q must be zeroed before)
+__global__ void k_grid_spread(const double *__restrict__ c, const double *__restrict__ charge, int n_atoms,
+                              int nx, int ny, int nz, double h, double *q)
+{
+    for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < n_atoms; a += gridDim.x * blockDim.x) {
+        const double g[3] = {c[3 * a] / h, c[3 * a + 1] / h, c[3 * a + 2] / h};
+        const int n[3] = {nx, ny, nz};
+        int base[3];
+        double fr[3];
+        for (int d = 0; d < 3; d++) {
+            base[d] = min(max((int)floor(g[d]), 0), n[d] - 2);
+            fr[d] = __dsub_rn(g[d], (double)base[d]);
+        }
+        const double qa = charge[a];
+        for (int dz = 0; dz < 2; dz++) {
+            const double wz = dz ? fr[2] : __dsub_rn(1.0, fr[2]);
+            for (int dy = 0; dy < 2; dy++) {
+                const double wy = dy ? fr[1] : __dsub_rn(1.0, fr[1]);
+                for (int dx = 0; dx < 2; dx++) {
+                    const double wx = dx ? fr[0] : __dsub_rn(1.0, fr[0]);
+                    const double v = __dmul_rn(__dmul_rn(__dmul_rn(qa, wz), wy), wx);
+                    atomicAdd(&q[((size_t)(base[2] + dz) * ny + base[1] + dy) * nx + base[0] + dx], v);
+                }
+            }
+        }
+    }
+}
+
+// rhs = (4 pi) q / h^3, in place
+__global__ void k_grid_rhs(double *q, size_t n, double four_pi, double h3)
+{
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x)
+        q[t] = __ddiv_rn(__dmul_rn(four_pi, q[t]), h3);
+}
+
+// Debye-Hueckel ghost values: bc[g] = (1/eps_out) sum_a q_a exp(-kappa r_ga)/r_ga, atoms in index order.
+// One thread per ghost node, atoms staged through shared memory in tiles of DH_TILE.  Plain-ALU-bound.
+constexpr int DH_TILE = 256;
+__global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ c, const double *__restrict__ charge,
+                                                     int n_atoms, int nx, int ny, int nz, double h, double eps_out,
+                                                     double kappa, double *bc)
+{
+    __shared__ double sc[DH_TILE][4];
+    const size_t n_xy = (size_t)ny * nx, n_zy = (size_t)nz * ny, n_zx = (size_t)nz * nx;
+    const size_t nbc = 2 * (n_zy + n_zx + n_xy);
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double gx = 0.0, gy = 0.0, gz = 0.0;
+    if (t < 2 * n_zy) {                                   // x-, x+ : [nz][ny]
+        const size_t u = t % n_zy;
+        gx = (t < n_zy) ? -h : nx * h; gy = (double)(u % ny) * h; gz = (double)(u / ny) * h;
+    } else if (t < 2 * n_zy + 2 * n_zx) {                 // y-, y+ : [nz][nx]
+        const size_t v = t - 2 * n_zy, u = v % n_zx;
+        gy = (v < n_zx) ? -h : ny * h; gx = (double)(u % nx) * h; gz = (double)(u / nx) * h;
+    } else if (t < nbc) {                                 // z-, z+ : [ny][nx]
+        const size_t v = t - 2 * n_zy - 2 * n_zx, u = v % n_xy;
+        gz = (v < n_xy) ? -h : nz * h; gx = (double)(u % nx) * h; gy = (double)(u / nx) * h;
+    }
+    double acc = 0.0;
+    for (int a0 = 0; a0 < n_atoms; a0 += DH_TILE) {
+        const int a = a0 + threadIdx.x;
+        if (a < n_atoms) { sc[threadIdx.x][0] = c[3 * a]; sc[threadIdx.x][1] = c[3 * a + 1]; sc[threadIdx.x][2] = c[3 * a + 2]; sc[threadIdx.x][3] = charge[a]; }
+        __syncthreads();
+        const int m = min(DH_TILE, n_atoms - a0);
+        for (int s = 0; s < m; s++) {
+            const double dx = gx - sc[s][0], dy = gy - sc[s][1], dz = gz - sc[s][2];
+            const double r = sqrt((dx * dx + dy * dy) + dz * dz);
+            acc += sc[s][3] * (exp(-kappa * r) / r);
+        }
+        __syncthreads();
+    }
+    if (t < nbc) bc[t] = acc / eps_out;
+}
+
+}  // namespace pb

@@ -1,0 +1,95 @@
+"""-m gpu: NEXT row f1 -- pb_create_from_atoms (grid / stencil setup on the GPU) against oracle/pbsetup_ref.py.
+
+Bar: integer-like decisions (solute mask, which of the three face values, salt on/off) bit-exact; face values
+bit-exact (same IEEE operations); trilinear charges 1e-13 (atomic accumulation order); Debye-Hueckel ghost values
+1e-12 relative to the sum of |terms| (exp differs by an ulp between libm and CUDA); then the solve through the
+atom-built handle against the solver oracle fed by the setup oracle."""
+import math
+
+import numpy as np
+import pytest
+
+from workloads import pb_inputs as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pkg(cuda_device):
+    from paper_1704_02745_b200 import build as pb_build
+
+    pb_build.build()
+    import paper_1704_02745_b200 as p
+
+    p.load_library()
+    return p
+
+
+def atoms(n_atoms, nx, ny, nz, h, seed):
+    rng = np.random.Generator(np.random.PCG64(W.SEED0 + 500 + seed))
+    L = np.array([(nx - 1) * h, (ny - 1) * h, (nz - 1) * h])
+    c = W.atoms_uniform(n_atoms, 0.15 * L, 0.85 * L, rng)
+    c[0] = [0.2, 0.3, L[2] - 0.1]                       # one atom hugging a corner: clipped bounding box
+    r = rng.uniform(1.2, 2.0, n_atoms)
+    q = rng.normal(0.0, 0.4, n_atoms)
+    return c, r, q
+
+
+@pytest.mark.parametrize("shape,na", [((21, 17, 13), 12), ((33, 33, 33), 1), ((40, 23, 31), 60)])
+def test_fields_match_setup_oracle(pkg, shape, na):
+    from oracle import pbsetup_ref as S
+
+    nx, ny, nz = shape
+    h, eps_in, eps_out, kb = 0.5, 1.0, 80.0, W.KBAR2_150MM_300K
+    if na == 1:
+        c, r, q = np.array([[8.0, 8.0, 8.0]]), np.array([2.0]), np.array([1.0])      # config 1 (Born ion)
+    else:
+        c, r, q = atoms(na, nx, ny, nz, h, na)
+    ref = S.setup(nx, ny, nz, h, c, r, q, eps_in, eps_out, kb)
+    with pkg.PBSolver.from_atoms(nx, ny, nz, h, c, r, q, eps_in, eps_out, kb) as s:
+        for name in ("eps_x", "eps_y", "eps_z", "kbar2"):
+            assert np.array_equal(s.field(name), ref[name]), name           # bit-exact
+        rhs = s.field("rhs")
+        assert np.max(np.abs(rhs - ref["rhs"])) <= 1e-13 * np.max(np.abs(ref["rhs"]))
+        assert np.array_equal(rhs != 0, ref["rhs"] != 0)
+        bc = s.field("bc")
+        kappa = math.sqrt(kb / eps_out)
+        g = S.ghost_positions(nx, ny, nz, h)
+        rr = np.linalg.norm(g[:, None, :] - c[None, :, :], axis=2)
+        scale = (np.abs(q)[None, :] * np.exp(-kappa * rr) / rr).sum(1) / eps_out
+        assert np.all(np.abs(bc - ref["bc"]) <= 1e-12 * scale)
+        # new charges on the same atoms (pb_set_charges): rhs and bc follow, operator untouched
+        q2 = q + 0.05
+        s.set_charges(q2)
+        ref2 = S.setup(nx, ny, nz, h, c, r, q2, eps_in, eps_out, kb)
+        assert np.max(np.abs(s.field("rhs") - ref2["rhs"])) <= 1e-13 * np.max(np.abs(ref2["rhs"]))
+        assert np.all(np.abs(s.field("bc") - ref2["bc"]) <= 1e-12 * (scale + 0.05 * (np.exp(-kappa * rr) / rr).sum(1) / eps_out))
+        assert np.array_equal(s.field("eps_x"), ref["eps_x"])
+
+
+def test_solve_through_atom_built_handle(pkg):
+    from oracle import pbref, pbsetup_ref as S
+
+    nx, ny, nz, h = 40, 23, 31, 0.5
+    c, r, q = atoms(60, nx, ny, nz, h, 60)
+    f = S.setup(nx, ny, nz, h, c, r, q, 1.0, 80.0, W.KBAR2_150MM_300K)
+    o = pbref.PBRef(nx, ny, nz, h, f["eps_x"], f["eps_y"], f["eps_z"], f["kbar2"], f["rhs"], f["bc"]).solve(1e-10, 5000)
+    with pkg.PBSolver.from_atoms(nx, ny, nz, h, c, r, q, 1.0, 80.0, W.KBAR2_150MM_300K) as s:
+        g = s.solve(1e-10, 5000, "f64")
+        g32 = s.solve(1e-5, 5000, "f32")
+    scale = np.max(np.abs(o["phi"]))
+    assert g["status"] == 0 and abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"]))
+    assert np.max(np.abs(g["phi"] - o["phi"])) <= 1e-8 * scale
+    assert np.max(np.abs(g32["phi"] - o["phi"])) <= 1e-4 * scale
+
+
+def test_from_atoms_edge_cases(pkg):
+    # no atoms: pure solvent, zero rhs and ghost values -> phi = 0 in 0 iterations
+    with pkg.PBSolver.from_atoms(9, 8, 7, 0.5, np.zeros((0, 3)), np.zeros(0), np.zeros(0), 1.0, 80.0, 1.0) as s:
+        assert np.all(s.field("eps_y") == 80.0) and np.all(s.field("kbar2") == 1.0) and not s.field("rhs").any()
+        g = s.solve(1e-8, 50, "f64")
+        assert g["iters"] == 0 and not g["phi"].any()
+    with pytest.raises(pkg.PBError):
+        pkg.PBSolver.from_atoms(1, 8, 7, 0.5, np.zeros((1, 3)), np.ones(1), np.ones(1), 1.0, 80.0, 1.0)
+    with pytest.raises(pkg.PBError):
+        pkg.PBSolver.from_atoms(9, 8, 7, 0.5, np.ones((1, 3)), np.ones(1), np.ones(1), -1.0, 80.0, 1.0)
