@@ -49,6 +49,8 @@ def parse_args(argv=None):
     ap.add_argument("--cpu-sample-iters", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--setup-from-atoms", action="store_true",
+                    help="also time pb_create_from_atoms / pb_set_charges (GPU grid setup, NEXT row f1)")
     ap.add_argument("--batch", type=int, default=0,
                     help="also run this many solves of config 5's perturbed-charge batch on the same operator")
     return ap.parse_args(argv)
@@ -301,6 +303,40 @@ def run_ours(args, rank, local_rank, world):
                  "mean_iters": float(np.mean(it_b)), "min_iters": int(min(it_b)), "max_iters": int(max(it_b)),
                  "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member, this rank only"}
 
+    # ---- optional (NEXT row f1): the same problem built on the GPU from atoms, and a charge update ---------------
+    setup = None
+    if args.setup_from_atoms and "charges" in inp.meta:
+        from workloads import perturbed_charge_values
+
+        m = inp.meta
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        s2 = pkg.PBSolver.from_atoms(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], m["radii"], m["charges"],
+                                     m["eps_in"], m["eps_out"], m["kbar2_solvent"], stream=stream.cuda_stream)
+        torch.cuda.synchronize()
+        t_fa = time.perf_counter() - t0
+        nb = min(args.batch, 10) if args.batch > 0 else 3
+        t_sc, t_sv, it_sc = 0.0, 0.0, []
+        for sidx in range(nb):
+            qs = perturbed_charge_values(inp, sidx)
+            t0 = time.perf_counter()
+            s2.set_charges(qs)
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            it_sc.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
+            torch.cuda.synchronize()
+            t_sc += t1 - t0
+            t_sv += time.perf_counter() - t1
+        s2.close()
+        nbc = 2 * (inp.nz * inp.ny + inp.nz * inp.nx + inp.ny * inp.nx)
+        terms = float(nbc) * len(m["charges"])
+        setup = {"create_from_atoms_ms": 1e3 * t_fa, "set_charges_ms": 1e3 * t_sc / nb, "solve_ms": 1e3 * t_sv / nb,
+                 "mean_iters": float(np.mean(it_sc)), "members": nb, "atoms": int(len(m["charges"])),
+                 "dh_terms": terms, "dh_gterms_per_s": terms / (t_sc / nb) / 1e9,
+                 "host_generator_s": t_gen,
+                 "note": "pb_create_from_atoms = mask + faces + salt + charges + Debye-Hueckel ghosts + pb_create "
+                         "(incl. plan autotune); set_charges = charge spreading + the fp64 DH boundary sum (ALU-bound)"}
+
     # ---- roofline of the dominant kernel (K_spmv), CUDA events around every launch ----------------
     solver.solve_begin(prec)
     solver.iterate(prec, 5)
@@ -352,6 +388,8 @@ def run_ours(args, rank, local_rank, world):
                 "roofline": roofline, "cpu_baseline": cpu}
         if batch is not None:
             line["batch"] = batch
+        if setup is not None:
+            line["setup_from_atoms"] = setup
     solver.close()
     if world > 1:
         dist.barrier()

@@ -129,10 +129,12 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ 
         if (a < n_atoms) { sc[threadIdx.x][0] = c[3 * a]; sc[threadIdx.x][1] = c[3 * a + 1]; sc[threadIdx.x][2] = c[3 * a + 2]; sc[threadIdx.x][3] = charge[a]; }
         __syncthreads();
         const int m = min(DH_TILE, n_atoms - a0);
+#pragma unroll 4
         for (int s = 0; s < m; s++) {
             const double dx = gx - sc[s][0], dy = gy - sc[s][1], dz = gz - sc[s][2];
-            const double r = sqrt((dx * dx + dy * dy) + dz * dz);
-            acc += sc[s][3] * (exp(-kappa * r) / r);
+            const double d2 = (dx * dx + dy * dy) + dz * dz;
+            const double ir = rsqrt(d2);                   // 1/r and r = d2/r: one special-function call, no division
+            acc += sc[s][3] * (exp(-kappa * (d2 * ir)) * ir);
         }
         __syncthreads();
     }

@@ -9,6 +9,7 @@ from .pb_inputs import (  # noqa: F401
     PBInputs,
     born_ion,
     make_config,
+    perturbed_charge_values,
     perturbed_charges,
     random_operator,
 )

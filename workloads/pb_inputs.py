@@ -370,14 +370,20 @@ def make_config(cfg: int, device=None, n_atoms=None) -> PBInputs:
     raise ValueError(f"unknown config {cfg}")
 
 
+def perturbed_charge_values(inp: PBInputs, s: int) -> np.ndarray:
+    """Charges of batch member s (q_i += N(0,0.05), total re-fixed); RNG PCG64(170402745 + 1000 + s)."""
+    m = inp.meta
+    rng = np.random.Generator(np.random.PCG64(SEED0 + 1000 + s))
+    return _fix_total_charge(m["charges"] + rng.normal(0.0, 0.05, m["charges"].size))
+
+
 def perturbed_charges(inp: PBInputs, s: int, device=None):
     """Batch member s of config 5's 50-solve batch: q_i += N(0,0.05), total re-fixed.
 
     Same operator; returns (rhs, bc) for pb_set_rhs.  RNG PCG64(170402745 + 1000 + s).
     """
     m = inp.meta
-    rng = np.random.Generator(np.random.PCG64(SEED0 + 1000 + s))
-    q = _fix_total_charge(m["charges"] + rng.normal(0.0, 0.05, m["charges"].size))
+    q = perturbed_charge_values(inp, s)
     qn = spread_trilinear(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], q)
     rhs = 4.0 * math.pi * qn / inp.h ** 3
     bc = debye_huckel_ghost(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], q, m["eps_out"],
