@@ -152,6 +152,12 @@ pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spm
 /* Number of CUDA kernels this handle has enqueued so far (those inside launched graphs included). */
 long long pb_launch_count(pb_handle *h);
 
+/* Size of the handle's coefficient palette: when the three face-dielectric arrays hold <= 256 distinct values
+ * (every molecular map built from eps_in / eps_out and their harmonic mean, does) they are stored
+ * exactly as one byte per face plus a table and decoded inside the SpMV; 0 = full-precision face arrays.
+ * PB_PALETTE=0 in the environment disables the palette. */
+int pb_palette_size(pb_handle *h);
+
 /* pb_destroy(NULL) is a no-op.  Frees every device allocation of the handle. */
 pb_status pb_destroy(pb_handle *h);
 

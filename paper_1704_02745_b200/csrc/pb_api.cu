@@ -32,6 +32,11 @@ struct Work {
     int qTXV = 0, qTY = 0, qTZ = 0, qntx = 0, qnty = 0, qntz = 0, qns = 0, qgrid = 0, qthreads = 0;
     size_t qsmem = 0;
     CUtensorMap tm_r, tm_tmp, tm_dinv, tm_p0, tm_p1, tm_x, tm_ex, tm_ey, tm_ez;
+    // coefficient palette (pb_setup.cuh): byte face indices + table, instead of exm/eym/ezm
+    bool pal = false;
+    unsigned char *exi = nullptr, *eyi = nullptr, *ezi = nullptr;
+    T *lut = nullptr;
+    int Pb = 0;
 };
 
 }  // namespace
@@ -57,6 +62,8 @@ struct pb_handle {
     int use_graph;
     long long launches;          // kernels enqueued so far (graph-contained ones included)
     int precond;                 // 1 Jacobi (default), 0 none
+    PalTable *pal_table;         // device; distinct face values of the operator
+    int pal_n;                   // -1: not examined yet, 0: more than 256 distinct values, else the table size
     // pb_create_from_atoms keeps the atom geometry for pb_set_charges
     double *atoms_c;             // [n_atoms][3], device
     int n_atoms;
@@ -77,6 +84,14 @@ namespace {
             cudaGetLastError();                                                \
             return (e__ == cudaErrorMemoryAllocation) ? PB_ERR_ALLOC : PB_ERR_CUDA; \
         }                                                                      \
+    } while (0)
+
+// cudaMalloc / cudaFree can return cudaSuccess and still leave a non-sticky "invalid argument" in the runtime's
+// last-error slot (observed on driver 580.159 / CUDA 12.9); clear it so later launch checks see only their own errors.
+#define PB_ALLOC(call)            \
+    do {                          \
+        PB_CUDA(call);            \
+        (void)cudaGetLastError(); \
     } while (0)
 
 #define PB_TRY(expr)                       \
@@ -108,7 +123,7 @@ constexpr int kNumSM = 148;   // B200
 template <typename T>
 pb_status alloc_arr(T **p, size_t n)
 {
-    PB_CUDA(cudaMalloc((void **)p, (n + 64) * sizeof(T)));   // slack: vector tails never fault
+    PB_ALLOC(cudaMalloc((void **)p, (n + 64) * sizeof(T)));   // slack: vector tails never fault
     return PB_OK;
 }
 
@@ -118,6 +133,9 @@ void free_work(Work<T> &w)
     T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.tmp, &w.p0, &w.p1, &w.Ap};
     for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
+    unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi};
+    for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
+    if (w.lut) { cudaFree(w.lut); w.lut = nullptr; }
     w.ready = w.b_ready = false;
 }
 
@@ -148,9 +166,39 @@ pb_status ensure(pb_handle *h)
     w.P = ((h->nx + 1 + align - 1) / align) * align;
     w.npad = (size_t)h->nz * h->ny * w.P;
     const size_t n_ey = (size_t)h->nz * (h->ny + 1) * w.P, n_ez = (size_t)(h->nz + 1) * h->ny * w.P;
+    // distinct face values of the operator -> palette or full-precision face arrays (decided once per handle)
+    if (h->pal_n < 0) {
+        h->pal_n = 0;
+        if (env_int("PB_PALETTE", 1)) {
+            if (!h->pal_table) PB_ALLOC(cudaMalloc((void **)&h->pal_table, sizeof(PalTable)));
+            k_pal_reset<<<1, 256, 0, h->stream>>>(h->pal_table);
+            const size_t ns[3] = {(size_t)h->nz * h->ny * (h->nx + 1), (size_t)h->nz * (h->ny + 1) * h->nx,
+                                  (size_t)(h->nz + 1) * h->ny * h->nx};
+            const double *arrs[3] = {h->eps_x, h->eps_y, h->eps_z};
+            for (int a = 0; a < 3; a++)
+                k_pal_collect<<<grid_for(ns[a], 256, kNumSM * 8), 256, 0, h->stream>>>(arrs[a], ns[a], h->pal_table);
+            k_pal_finish<<<1, 256, 0, h->stream>>>(h->pal_table);
+            PB_CUDA(cudaGetLastError());
+            int n = 0;
+            PB_CUDA(cudaMemcpyAsync(&n, &h->pal_table->n, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            PB_CUDA(cudaStreamSynchronize(h->stream));
+            h->pal_n = n;
+            h->launches += 5;
+        }
+    }
+    w.pal = h->pal_n > 0;
+    w.Pb = (w.P + 15) / 16 * 16;
     pb_status s = PB_OK;
-    if ((s = alloc_arr(&w.exm, w.npad)) || (s = alloc_arr(&w.eym, n_ey)) || (s = alloc_arr(&w.ezm, n_ez)) ||
-        (s = alloc_arr(&w.D, w.npad)) || (s = alloc_arr(&w.Dinv, w.npad)) || (s = alloc_arr(&w.b, w.npad)) ||
+    if (w.pal) {
+        const size_t b_ex = (size_t)h->nz * h->ny * w.Pb, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pb,
+                     b_ez = (size_t)(h->nz + 1) * h->ny * w.Pb;
+        if ((s = alloc_arr(&w.exi, b_ex)) || (s = alloc_arr(&w.eyi, b_ey)) || (s = alloc_arr(&w.ezi, b_ez)) ||
+            (s = alloc_arr(&w.lut, (size_t)kPalMax))) { free_work(w); return s; }
+    } else if ((s = alloc_arr(&w.exm, w.npad)) || (s = alloc_arr(&w.eym, n_ey)) || (s = alloc_arr(&w.ezm, n_ez))) {
+        free_work(w);
+        return s;
+    }
+    if ((s = alloc_arr(&w.D, w.npad)) || (s = alloc_arr(&w.Dinv, w.npad)) || (s = alloc_arr(&w.b, w.npad)) ||
         (s = alloc_arr(&w.x, w.npad)) || (s = alloc_arr(&w.r, w.npad)) || (s = alloc_arr(&w.tmp, w.npad)) ||
         (s = alloc_arr(&w.p0, w.npad)) || (s = alloc_arr(&w.p1, w.npad)) || (s = alloc_arr(&w.Ap, w.npad))) {
         free_work(w);
@@ -162,7 +210,7 @@ pb_status ensure(pb_handle *h)
         if (h->partials) cudaFree(h->partials);
         h->partials = nullptr;
         h->partials_cap = 0;
-        PB_CUDA(cudaMalloc((void **)&h->partials, need * sizeof(double)));
+        PB_ALLOC(cudaMalloc((void **)&h->partials, need * sizeof(double)));
         h->partials_cap = need;
     }
     PB_CUDA(cudaMemsetAsync(h->bad, 0, sizeof(int), h->stream));
@@ -170,6 +218,12 @@ pb_status ensure(pb_handle *h)
     k_setup_coeff<T><<<grid_for(total, 256, kNumSM * 16), 256, 0, h->stream>>>(
         h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
         w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
+    if (w.pal) {
+        k_setup_pal_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pb, 256, kNumSM * 16), 256, 0, h->stream>>>(
+            h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pb, h->pal_table, w.exi, w.eyi, w.ezi);
+        k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
+        h->launches += 2;
+    }
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     PB_TRY(build_b<T>(h, w));
@@ -227,6 +281,21 @@ pb_status make_map(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, i
     return PB_OK;
 }
 
+// byte tensor [planes][rows][Pb] of face indices, box = bw bytes x by rows x 1 plane, zero fill outside
+pb_status make_map_u8(CUtensorMap *tm, const unsigned char *ptr, int Pb, int rows, int planes, int bw, int by)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return PB_ERR_CUDA;
+    const cuuint64_t dims[3] = {(cuuint64_t)Pb, (cuuint64_t)rows, (cuuint64_t)planes};
+    const cuuint64_t strides[2] = {(cuuint64_t)Pb, (cuuint64_t)Pb * rows};
+    const cuuint32_t box[3] = {(cuuint32_t)bw, (cuuint32_t)by, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void *)ptr, dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? PB_OK : PB_ERR_CUDA;
+}
+
 struct TileCfg { int TXV, TY, NS, bps, TZ; };   // TZ = 0: derive from the tile count
 
 // apply one tile / ring / grid configuration: sizes, persistent grid, tensor maps
@@ -240,9 +309,9 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qntx = (rowvecs + TXV - 1) / TXV;
     w.qnty = (h->ny + TY - 1) / TY;
     w.qthreads = (TXV * TY + 31) / 32 * 32 + 32;
-    const SlotLayout L = slot_layout(TXV, TY);
+    const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0);
     w.qsmem = (size_t)NS * L.slot + 128;
-    if (w.qsmem > 226 * 1024 || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
+    if (w.qsmem > 224 * 1024 || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
     const int slots = kNumSM * c.bps;
     const int xy = w.qntx * w.qnty;
     int TZ = c.TZ;
@@ -263,19 +332,25 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_x, w.x, w.P, h->ny, h->nz, TXV * VEC, TY));
-    PB_TRY(make_map<T>(&w.tm_ex, w.exm, w.P, h->ny, h->nz, (TXV + 1) * VEC, TY));
-    PB_TRY(make_map<T>(&w.tm_ey, w.eym, w.P, h->ny + 1, h->nz, TXV * VEC, TY + 1));
-    PB_TRY(make_map<T>(&w.tm_ez, w.ezm, w.P, h->ny, h->nz + 1, TXV * VEC, TY));
+    if (w.pal) {
+        PB_TRY(make_map_u8(&w.tm_ex, w.exi, w.Pb, h->ny, h->nz, L.bw, TY));
+        PB_TRY(make_map_u8(&w.tm_ey, w.eyi, w.Pb, h->ny + 1, h->nz, L.bw, TY + 1));
+        PB_TRY(make_map_u8(&w.tm_ez, w.ezi, w.Pb, h->ny, h->nz + 1, L.bw, TY));
+    } else {
+        PB_TRY(make_map<T>(&w.tm_ex, w.exm, w.P, h->ny, h->nz, (TXV + 1) * VEC, TY));
+        PB_TRY(make_map<T>(&w.tm_ey, w.eym, w.P, h->ny + 1, h->nz, TXV * VEC, TY + 1));
+        PB_TRY(make_map<T>(&w.tm_ez, w.ezm, w.P, h->ny, h->nz + 1, TXV * VEC, TY));
+    }
     return PB_OK;
 }
 
 template <typename T, int MODE> void launch_spmv(pb_handle *h, Work<T> &w, double out_scale);
 
 // deepest ring (<= 6 slots) that lets `bps` blocks of this tile share one SM's shared memory
-inline int ring_depth(int TXV, int TY, int bps)
+inline int ring_depth(int TXV, int TY, int bps, int pal_vec)
 {
-    const size_t per_block = (size_t)232448 / bps - 1024 - 1152;   // 227 KB per SM, 1 KB reserved per block, statics
-    int NS = (int)(per_block / slot_layout(TXV, TY).slot);
+    const size_t per_block = (size_t)232448 / bps - 1024 - 3200;   // 227 KB per SM, 1 KB reserved per block, statics
+    int NS = (int)(per_block / slot_layout(TXV, TY, pal_vec).slot);
     return NS > 6 ? 6 : NS;
 }
 
@@ -289,8 +364,11 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     constexpr int VEC = VecN<T>::value;
     const int rowvecs = w.P / VEC;
     const int maxv = 256 / VEC - 2;                                  // box inner dimension <= 256 elements
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+    const int max_dyn = 224 * 1024;
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
     int ntx0 = (rowvecs + 32) / 64;                                  // rows of about 64 vectors (1 KB)
     if (ntx0 < 1) ntx0 = 1;
     while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
@@ -307,9 +385,9 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         if (c.TY < 1) c.TY = 1;
         if (c.TY > h->ny) c.TY = h->ny;
         while (c.TXV * c.TY > 448 && c.TY > 1) c.TY--;
-        c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2) >= 4 ? 2 : 1);
+        c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0) >= 4 ? 2 : 1);
         if (c.bps < 1) c.bps = 1;
-        c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps));
+        c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0));
         c.TZ = env_int("PB_TZ", 0);
         cand[nc++] = c;
     } else {
@@ -322,7 +400,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
                 int TY = ty > h->ny ? h->ny : ty;
                 if (TXV * TY > 448) continue;
                 for (int bps = 1; bps <= 4; bps++) {
-                    const int NS = ring_depth(TXV, TY, bps);
+                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0);
                     if (NS < 4 && !(NS == 3 && bps >= 2)) continue;
                     const int cthreads = ((TXV * TY + 31) / 32 * 32) * bps;
                     if (cthreads < 256 || cthreads > 1024) continue;     // consumer threads per SM
@@ -367,8 +445,8 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     }
     PB_TRY(configure_tma<T>(h, w, cand[best]));
     if (getenv("PB_VERBOSE"))
-        fprintf(stderr, "pb: k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
-                sizeof(T) == 4 ? "f32" : "f64", w.qTXV, w.qTY, w.qTZ, w.qns, cand[best].bps,
+        fprintf(stderr, "pb: palette %d; k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
+                h->pal_n, sizeof(T) == 4 ? "f32" : "f64", w.qTXV, w.qTY, w.qTZ, w.qns, cand[best].bps,
                 w.qntx * w.qnty * w.qntz, w.qgrid, w.qthreads, w.qsmem, tune ? " (autotuned)" : "");
     return PB_OK;
 }
@@ -383,8 +461,13 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
     a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->l2hints; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
-    k_spmv_tma<T, MODE><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
-        MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
+    a.lut = w.lut;
+    if (w.pal)
+        k_spmv_tma<T, MODE, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+            MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
+    else
+        k_spmv_tma<T, MODE, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+            MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
 }
 
 // enqueue n PCG iterations: (k_spmv, k_vec) pairs, nothing else
@@ -435,11 +518,10 @@ pb_status get_graph(pb_handle *h, Work<T> &w, int m)
 pb_status ensure_stage(pb_handle *h, size_t bytes)
 {
     if (bytes <= h->stage_bytes) return PB_OK;
-    if (h->stage) cudaFree(h->stage);
-    if (h->atoms_c) cudaFree(h->atoms_c);
+    if (h->stage) PB_ALLOC(cudaFree(h->stage));
     h->stage = nullptr;
     h->stage_bytes = 0;
-    PB_CUDA(cudaMalloc(&h->stage, bytes));
+    PB_ALLOC(cudaMalloc(&h->stage, bytes));
     h->stage_bytes = bytes;
     return PB_OK;
 }
@@ -518,7 +600,7 @@ pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_
         *dst = nullptr;
         return PB_OK;
     }
-    if (!*dst) PB_CUDA(cudaMalloc((void **)dst, (n + 8) * sizeof(double)));
+    if (!*dst) PB_ALLOC(cudaMalloc((void **)dst, (n + 8) * sizeof(double)));
     PB_CUDA(cudaMemcpyAsync(*dst, src, n * sizeof(double),
                             where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
     return PB_OK;
@@ -586,6 +668,7 @@ pb_status pb_destroy(pb_handle *h)
     if (h->bad) cudaFree(h->bad);
     if (h->stage) cudaFree(h->stage);
     if (h->atoms_c) cudaFree(h->atoms_c);
+    if (h->pal_table) cudaFree(h->pal_table);
     if (h->pinned) cudaFreeHost(h->pinned);
     if (h->pinned_state) cudaFreeHost(h->pinned_state);
     for (int i = 0; i < 2; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
@@ -614,16 +697,17 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
     h->use_graph = env_int("PB_NO_GRAPH", 0) ? 0 : 1;
     h->l2hints = env_int("PB_L2HINTS", 0);
     h->precond = 1;
+    h->pal_n = -1;
     pb_status s = PB_OK;
     auto body = [&]() -> pb_status {
         PB_CUDA(cudaGetDevice(&h->device));
         if (cuda_stream) { h->stream = (cudaStream_t)cuda_stream; h->own_stream = false; }
         else { PB_CUDA(cudaStreamCreate(&h->stream)); h->own_stream = true; }   // blocking: orders with stream 0
-        PB_CUDA(cudaMalloc((void **)&h->st, sizeof(State)));
+        PB_ALLOC(cudaMalloc((void **)&h->st, sizeof(State)));
         PB_CUDA(cudaMemsetAsync(h->st, 0, sizeof(State), h->stream));
-        PB_CUDA(cudaMalloc((void **)&h->bad, sizeof(int)));
-        PB_CUDA(cudaHostAlloc((void **)&h->pinned, 8 * sizeof(int), cudaHostAllocDefault));
-        PB_CUDA(cudaHostAlloc((void **)&h->pinned_state, sizeof(State), cudaHostAllocDefault));
+        PB_ALLOC(cudaMalloc((void **)&h->bad, sizeof(int)));
+        PB_ALLOC(cudaHostAlloc((void **)&h->pinned, 8 * sizeof(int), cudaHostAllocDefault));
+        PB_ALLOC(cudaHostAlloc((void **)&h->pinned_state, sizeof(State), cudaHostAllocDefault));
         PB_CUDA(cudaEventCreateWithFlags(&h->ev[0], cudaEventDisableTiming));
         PB_CUDA(cudaEventCreateWithFlags(&h->ev[1], cudaEventDisableTiming));
         const size_t n = (size_t)nx * ny * nz;
@@ -718,6 +802,8 @@ pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spm
 
 long long pb_launch_count(pb_handle *h) { return h ? h->launches : 0; }
 
+int pb_palette_size(pb_handle *h) { return (h && h->pal_n > 0) ? h->pal_n : 0; }
+
 pb_status pb_query(pb_handle *h, int what, double *out_host)
 {
     if (!h || !out_host || what < 0 || what > 7) return PB_ERR_INVALID_ARG;
@@ -792,7 +878,7 @@ struct DevTmp {                      // frees its device allocations on scope ex
     ~DevTmp() { for (int i = 0; i < n; i++) if (p[i]) cudaFree(p[i]); }
     pb_status get(void **out, size_t bytes) {
         *out = nullptr;
-        PB_CUDA(cudaMalloc(out, bytes ? bytes : 8));
+        PB_ALLOC(cudaMalloc(out, bytes ? bytes : 8));
         p[n++] = *out;
         return PB_OK;
     }
@@ -878,8 +964,8 @@ extern "C" pb_status pb_set_charges(pb_handle *h, const double *charges, pb_mems
     PB_TRY(tmp.get((void **)&d_q, (size_t)h->n_atoms * sizeof(double)));
     PB_CUDA(cudaMemcpyAsync(d_q, charges, (size_t)h->n_atoms * sizeof(double),
                             where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
-    if (!h->rhs) PB_CUDA(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
-    if (!h->bc) PB_CUDA(cudaMalloc((void **)&h->bc, (nbc + 8) * sizeof(double)));
+    if (!h->rhs) PB_ALLOC(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
+    if (!h->bc) PB_ALLOC(cudaMalloc((void **)&h->bc, (nbc + 8) * sizeof(double)));
     PB_TRY(charges_to_rhs_bc(h->atoms_c, d_q, h->n_atoms, h->nx, h->ny, h->nz, h->h, h->atoms_eps_out,
                              h->atoms_kappa, h->rhs, h->bc, h->stream));
     h->launches += 3;

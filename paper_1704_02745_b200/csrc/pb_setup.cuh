@@ -24,7 +24,7 @@ __global__ void k_setup_coeff(const double *__restrict__ eps_x, const double *__
         const int k = (int)(q / (ny + 1));
         if (k < nz && j < ny) {
             const size_t row = (size_t)k * ny + j;
-            exm[row * P + i] = (i <= nx) ? (T)eps_x[row * (nx + 1) + i] : T(0);
+            if (exm) exm[row * P + i] = (i <= nx) ? (T)eps_x[row * (nx + 1) + i] : T(0);
             double d = 1.0;
             if (i < nx) {
                 d = eps_x[row * (nx + 1) + i] + eps_x[row * (nx + 1) + i + 1]
@@ -36,9 +36,9 @@ __global__ void k_setup_coeff(const double *__restrict__ eps_x, const double *__
             D[row * P + i] = (T)d;
             Dinv[row * P + i] = (T)(1.0 / d);
         }
-        if (k < nz)
+        if (k < nz && eym)
             eym[((size_t)k * (ny + 1) + j) * P + i] = (i < nx) ? (T)eps_y[((size_t)k * (ny + 1) + j) * nx + i] : T(0);
-        if (j < ny)
+        if (j < ny && ezm)
             ezm[((size_t)k * ny + j) * P + i] = (i < nx) ? (T)eps_z[((size_t)k * ny + j) * nx + i] : T(0);
     }
 }
@@ -114,6 +114,119 @@ __global__ void k_set_state(State *st, double tol2, int maxiter, int latch)
     st->ticket_vec = 0u;
     st->alpha = 0.0;
     st->beta = 0.0;
+}
+
+}  // namespace pb
+
+// ---------------------------------------------------------------------------------------
+// Coefficient palette.  A molecular dielectric map takes very few distinct face values (eps_in,
+// eps_out and their harmonic mean), so the three face arrays can be stored exactly
+// as one byte per face indexing a table of <= 256 values -- a storage format in the sense of
+// PAPER.md:251-261 (fewer bytes per row than DIA's seven bands), decoded on the fly in k_spmv_tma.
+// Operators with more than 256 distinct face values keep the full-precision arrays.
+// ---------------------------------------------------------------------------------------
+namespace pb {
+
+constexpr int kPalMax = 256;
+constexpr int kPalHash = 1024;
+constexpr unsigned long long kPalEmpty = 0xFFFFFFFFFFFFFFFFull;
+
+struct PalTable {
+    unsigned long long keys[kPalHash];   // open-addressing set of the distinct bit patterns
+    int count;
+    int overflow;
+    int n;                               // final size (k_pal_finish)
+    double vals[kPalMax];                // sorted ascending
+};
+
+__global__ void k_pal_reset(PalTable *t)
+{
+    for (int i = threadIdx.x; i < kPalHash; i += blockDim.x) t->keys[i] = kPalEmpty;
+    if (threadIdx.x == 0) { t->count = 0; t->overflow = 0; t->n = 0; }
+}
+
+__device__ __forceinline__ void pal_insert(PalTable *t, double v)
+{
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(v);
+    unsigned int slot = (unsigned int)((bits * 0x9E3779B97F4A7C15ull) >> 54);      // 10 bits
+    for (int probe = 0; probe < kPalHash; probe++, slot = (slot + 1) & (kPalHash - 1)) {
+        const unsigned long long cur = t->keys[slot];
+        if (cur == bits) return;
+        if (cur == kPalEmpty) {
+            const unsigned long long old = atomicCAS(&t->keys[slot], kPalEmpty, bits);
+            if (old == kPalEmpty) { if (atomicAdd(&t->count, 1) >= kPalMax) t->overflow = 1; return; }
+            if (old == bits) return;
+        }
+    }
+    t->overflow = 1;
+}
+
+// collect the distinct values of one dense fp64 array (consecutive equal values are skipped cheaply)
+__global__ void k_pal_collect(const double *__restrict__ a, size_t n, PalTable *t)
+{
+    volatile int *ovf = &t->overflow;
+    if (*ovf) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) pal_insert(t, 0.0);                   // the pad value
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const double v = a[i];
+        if (i > 0 && a[i - 1] == v && (i % 4096)) continue;                         // run of equal values
+        pal_insert(t, v);
+        if (*ovf) return;
+    }
+}
+
+// one block: gather the keys and sort them ascending by value (rank sort, <= 256 entries)
+__global__ void k_pal_finish(PalTable *t)
+{
+    __shared__ double v[kPalMax];
+    __shared__ int cnt;
+    if (threadIdx.x == 0) {
+        cnt = 0;
+        if (!t->overflow)
+            for (int i = 0; i < kPalHash && cnt < kPalMax; i++)
+                if (t->keys[i] != kPalEmpty) v[cnt++] = __longlong_as_double((long long)t->keys[i]);
+    }
+    __syncthreads();
+    const int n = t->overflow ? 0 : cnt;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        int rank = 0;
+        for (int j = 0; j < n; j++) rank += (v[j] < v[i]) || (v[j] == v[i] && j < i);
+        t->vals[rank] = v[i];
+    }
+    if (threadIdx.x == 0) t->n = n;
+}
+
+__device__ __forceinline__ unsigned char pal_index(const PalTable *t, double v)
+{
+    int lo = 0, hi = t->n - 1;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (t->vals[mid] < v) lo = mid + 1; else hi = mid; }
+    return (unsigned char)lo;
+}
+
+// byte index arrays in the padded layouts of exm / eym / ezm (row pitch Pb bytes, Pb >= P), pad = index of 0.0
+__global__ void k_setup_pal_idx(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
+                                const double *__restrict__ eps_z, int nx, int ny, int nz, int Pb,
+                                const PalTable *t, unsigned char *exi, unsigned char *eyi, unsigned char *ezi)
+{
+    const unsigned char zero = pal_index(t, 0.0);
+    const size_t total = (size_t)(nz + 1) * (ny + 1) * Pb;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(q % Pb);
+        const size_t u = q / Pb;
+        const int j = (int)(u % (ny + 1)), k = (int)(u / (ny + 1));
+        if (k < nz && j < ny)
+            exi[((size_t)k * ny + j) * Pb + i] = (i <= nx) ? pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i]) : zero;
+        if (k < nz)
+            eyi[((size_t)k * (ny + 1) + j) * Pb + i] = (i < nx) ? pal_index(t, eps_y[((size_t)k * (ny + 1) + j) * nx + i]) : zero;
+        if (j < ny)
+            ezi[((size_t)k * ny + j) * Pb + i] = (i < nx) ? pal_index(t, eps_z[((size_t)k * ny + j) * nx + i]) : zero;
+    }
+}
+
+template <typename T>
+__global__ void k_pal_lut(const PalTable *t, T *lut)
+{
+    for (int i = threadIdx.x; i < kPalMax; i += blockDim.x) lut[i] = (i < t->n) ? (T)t->vals[i] : T(0);
 }
 
 }  // namespace pb

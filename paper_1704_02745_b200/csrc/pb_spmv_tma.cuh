@@ -38,23 +38,30 @@ struct TmaArgs {
     State *st;
     double *partials;        // one per block
     double out_scale;        // MODE 1 only
+    const T *lut;            // PAL only: palette values (256 entries)
 };
 
 __host__ __device__ inline size_t align128(size_t v) { return (v + 127) & ~(size_t)127; }
 
-// byte sizes of the boxes of one item (also the smem carve-up of a ring slot)
+// byte sizes of the boxes of one item (also the smem carve-up of a ring slot).  With a coefficient
+// palette the three face boxes hold one byte per face, rows of `bw` bytes (a multiple of 16 for the TMA).
 struct SlotLayout {
     size_t szZ, szD, szEX, szEY, szEZ, slot;
     size_t oR, oDv, oPp, oEZ, oX, oEX, oEY;   // offsets of the boxes inside a slot
     uint32_t bZ, bD, bEX, bEY, bEZ;           // exact box bytes (what the TMA delivers)
+    int bw;                                   // palette only: bytes per row of a face-index box
 };
-__host__ __device__ inline SlotLayout slot_layout(int TXV, int TY) {
+__host__ __device__ inline SlotLayout slot_layout(int TXV, int TY, int pal_vec /* 0: no palette, else VEC */) {
     SlotLayout L;
     L.bZ = (uint32_t)(TY + 2) * (TXV + 2) * 16;
     L.bD = (uint32_t)TY * TXV * 16;
-    L.bEX = (uint32_t)TY * (TXV + 1) * 16;
-    L.bEY = (uint32_t)(TY + 1) * TXV * 16;
-    L.bEZ = L.bD;
+    if (pal_vec) {
+        L.bw = (TXV * pal_vec + 16 + 15) / 16 * 16;   // box starts at x0 rounded down to 16 B: up to 16-VEC bytes of lead-in
+        L.bEX = (uint32_t)TY * L.bw; L.bEY = (uint32_t)(TY + 1) * L.bw; L.bEZ = (uint32_t)TY * L.bw;
+    } else {
+        L.bw = 0;
+        L.bEX = (uint32_t)TY * (TXV + 1) * 16; L.bEY = (uint32_t)(TY + 1) * TXV * 16; L.bEZ = L.bD;
+    }
     L.szZ = align128(L.bZ); L.szD = align128(L.bD); L.szEX = align128(L.bEX);
     L.szEY = align128(L.bEY); L.szEZ = align128(L.bEZ);
     L.oR = 0; L.oDv = L.szZ; L.oPp = 2 * L.szZ;
@@ -64,7 +71,8 @@ __host__ __device__ inline SlotLayout slot_layout(int TXV, int TY) {
 }
 
 // MODE 0: PCG step;  MODE 1: y = out_scale * A' v  (v behind tm_r; no Dinv scaling, no p_old, no x, no dot)
-template <typename T, int MODE>
+// PAL: the eps_x/eps_y/eps_z maps are byte-index tensors decoded through the 256-entry table a.lut
+template <typename T, int MODE, bool PAL>
 __global__ void __launch_bounds__(512)
 k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_dinv,
            const __grid_constant__ CUtensorMap tm_p0, const __grid_constant__ CUtensorMap tm_p1,
@@ -78,6 +86,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     __shared__ __align__(8) uint64_t empty_bar[kMaxStages];
     __shared__ double red[32];
     __shared__ int s_last;
+    __shared__ T lut[PAL ? 256 : 1];
 
     const int tid = threadIdx.x;
     const int nthr = blockDim.x;
@@ -99,13 +108,15 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     }
     const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
     const int TXV = a.TXV, TY = a.TY, TZ = a.TZ, NS = a.nstage;
-    const SlotLayout L = slot_layout(TXV, TY);
+    const SlotLayout L = slot_layout(TXV, TY, PAL ? VEC : 0);
     unsigned char *base = (unsigned char *)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
 
     if (tid == 0) {
         for (int s = 0; s < NS; s++) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], NCW); }
         mbar_fence_init();
     }
+    if (PAL)
+        for (int i = tid; i < 256; i += nthr) lut[i] = a.lut[i];
     __syncthreads();
 
     double acc = 0.0;
@@ -139,11 +150,12 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                     } else if (centre) {
                         tma_load_3d_hint(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
                     }
-                    if (ez) tma_load_3d_hint(slot + L.oEZ, &tm_ez, x0, j0, q, &full_bar[s], pol_stream);
+                    const int xc = PAL ? (x0 & ~15) : x0;      // byte-index boxes start 16-byte aligned
+                    if (ez) tma_load_3d_hint(slot + L.oEZ, &tm_ez, xc, j0, q, &full_bar[s], pol_stream);
                     if (centre) {
                         if (MODE == 0) tma_load_3d_hint(slot + L.oX, &tm_x, x0, j0, q, &full_bar[s], pol_stream);
-                        tma_load_3d_hint(slot + L.oEX, &tm_ex, x0, j0, q, &full_bar[s], pol_stream);
-                        tma_load_3d_hint(slot + L.oEY, &tm_ey, x0, j0, q, &full_bar[s], pol_stream);
+                        tma_load_3d_hint(slot + L.oEX, &tm_ex, xc, j0, q, &full_bar[s], pol_stream);
+                        tma_load_3d_hint(slot + L.oEY, &tm_ey, xc, j0, q, &full_bar[s], pol_stream);
                     }
                 }
             }
@@ -195,6 +207,23 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             }
             return v;
         };
+        // VEC face coefficients starting at this thread's first node, row `row` of a face box
+        int lead = 0;                                  // PAL: bytes between the aligned box start and x0
+        auto coef = [&](const unsigned char *box, int row, int row_vecs) -> Vec<T> {
+            if (!PAL) return reinterpret_cast<const Vec<T> *>(box)[row * row_vecs + tx];
+            const unsigned char *p = box + row * L.bw + lead + tx * VEC;
+            Vec<T> v;
+            if (VEC == 4) {
+                const uint32_t w = *reinterpret_cast<const uint32_t *>(p);
+#pragma unroll
+                for (int e = 0; e < VEC; e++) v.a[e] = lut[(w >> (8 * e)) & 255u];
+            } else {
+                const uint32_t w = *reinterpret_cast<const unsigned short *>(p);
+#pragma unroll
+                for (int e = 0; e < VEC; e++) v.a[e] = lut[(w >> (8 * e)) & 255u];
+            }
+            return v;
+        };
         auto release = [&](int s) {                    // this warp is done with ring slot s
             fence_proxy_async();
             __syncwarp();
@@ -212,6 +241,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             const bool active = intile && (i0 < P) && (j < ny);
             const int nvalid = nx - i0;
             const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
+            lead = x0 & 15;
 
             // item k0-1: only the own column's value is needed
             int s = cnt % NS;
@@ -224,7 +254,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             mbar_wait(&full_bar[sk], (cnt / NS) & 1);
             unsigned char *slotk = base + (size_t)sk * L.slot;
             Vec<T> pc = update(slotk, true);
-            Vec<T> ezc = intile ? reinterpret_cast<const Vec<T> *>(slotk + L.oEZ)[cown] : zerov<T>();
+            Vec<T> ezc = intile ? coef(slotk + L.oEZ, ty, TXV) : zerov<T>();
             cnt++;
             named_bar_sync(1, NCT);
 
@@ -233,17 +263,16 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                 mbar_wait(&full_bar[s1], (cnt / NS) & 1);
                 unsigned char *slot1 = base + (size_t)s1 * L.slot;
                 const Vec<T> pn = update(slot1, k + 1 < k1);
-                const Vec<T> ezn = intile ? reinterpret_cast<const Vec<T> *>(slot1 + L.oEZ)[cown] : zerov<T>();
+                const Vec<T> ezn = intile ? coef(slot1 + L.oEZ, ty, TXV) : zerov<T>();
                 if (active) {
                     const Vec<T> *Zk = reinterpret_cast<const Vec<T> *>(slotk + L.oR);     // p_new(k) box
-                    const Vec<T> *EXk = reinterpret_cast<const Vec<T> *>(slotk + L.oEX);
-                    const Vec<T> *EYk = reinterpret_cast<const Vec<T> *>(slotk + L.oEY);
                     const Vec<T> up = Zk[own - BWc], dn = Zk[own + BWc];
                     const T left = Zk[own - 1].a[VEC - 1], right = Zk[own + 1].a[0];
                     const Vec<T> dinv = reinterpret_cast<const Vec<T> *>(slotk + L.oDv)[own];
-                    const Vec<T> ex = EXk[ty * (TXV + 1) + tx];
-                    const T exr = EXk[ty * (TXV + 1) + tx + 1].a[0];
-                    const Vec<T> eyl = EYk[cown], eyh = EYk[cown + TXV];
+                    const Vec<T> ex = coef(slotk + L.oEX, ty, TXV + 1);
+                    const T exr = PAL ? lut[slotk[L.oEX + ty * L.bw + lead + tx * VEC + VEC]]
+                                      : reinterpret_cast<const Vec<T> *>(slotk + L.oEX)[ty * (TXV + 1) + tx + 1].a[0];
+                    const Vec<T> eyl = coef(slotk + L.oEY, ty, TXV), eyh = coef(slotk + L.oEY, ty + 1, TXV);
                     const size_t idx = ((size_t)k * ny + j) * P + i0;
                     Vec<T> ap;
 #pragma unroll

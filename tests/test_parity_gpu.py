@@ -311,3 +311,33 @@ def test_unpreconditioned_cg_variant(pkg, pbref, prec, tol):
         assert abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (g["iters"], o["iters"])
         assert np.max(np.abs(g["phi"] - o["phi"])) <= lim * scale
     assert g_pcg["iters"] < g_cg["iters"]
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_palette_and_full_precision_coefficients_agree(pkg, pbref, prec, tol):
+    """The coefficient palette (<= 256 distinct face values stored as bytes + table) is an exact storage format:
+    the SpMV must be bit-identical with the full-precision face arrays (PB_PALETTE=0), and operators with more
+    than 256 distinct values must fall back to them."""
+    inp = make_config(2)                       # molecular map: eps in {1, 80, 160/81}
+    x = np.random.default_rng(4).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(np.float64 if prec == "f64" else np.float32)
+    saved = os.environ.pop("PB_PALETTE", None)
+    try:
+        with pkg.PBSolver(*inp.args()) as s:
+            assert s.palette_size() == 4       # the three face values and the pad value 0
+            y_pal = s.apply(x, prec)
+            g_pal = s.solve(tol, 5000, prec)
+        os.environ["PB_PALETTE"] = "0"
+        with pkg.PBSolver(*inp.args()) as s:
+            assert s.palette_size() == 0
+            y_full = s.apply(x, prec)
+            g_full = s.solve(tol, 5000, prec)
+    finally:
+        os.environ.pop("PB_PALETTE", None)
+        if saved is not None:
+            os.environ["PB_PALETTE"] = saved
+    assert np.array_equal(y_pal, y_full)
+    assert abs(g_pal["iters"] - g_full["iters"]) <= 1
+    assert np.max(np.abs(g_pal["phi"] - g_full["phi"])) <= (1e-9 if prec == "f64" else 1e-4) * np.max(np.abs(g_full["phi"]))
+    many = random_operator(21, 9, 8, seed=6, two_valued=False)      # ~5000 distinct face values
+    with pkg.PBSolver(*many.args()) as s:
+        assert s.palette_size() == 0
