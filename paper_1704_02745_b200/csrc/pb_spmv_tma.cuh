@@ -24,6 +24,9 @@ namespace pb {
 
 constexpr int kMaxStages = 8;
 
+__device__ __forceinline__ float rcp_rn(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double rcp_rn(double x) { return __drcp_rn(x); }
+
 template <typename T>
 struct TmaArgs {
     T *pbuf0, *pbuf1;        // iteration l reads buf[l&1] (through its tensor map), writes buf[(l+1)&1]
@@ -171,6 +174,14 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         const bool precond = a.precond != 0;
         const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0);
 
+        // halo cell h of the haloed boxes: two rows (above / below the tile), then two columns (left / right)
+        auto halo_cell = [&](int h) -> int {
+            if (h < TXV) return h + 1;
+            if (h < 2 * TXV) return (TY + 1) * BWc + (h - TXV) + 1;
+            const int cc = h - 2 * TXV, side = cc / TY, r = cc - side * TY;
+            return (r + 1) * BWc + (side ? TXV + 1 : 0);
+        };
+        const int extra0 = (NCT - 1 - tid < nextra) ? halo_cell(NCT - 1 - tid) : -1;   // this thread's halo cell
         // p_new = Dinv*r + beta*p_old (steps 6-7) in place in the r box; returns the own cell's p_new
         auto pnew_cell = [&](Vec<T> *R, const Vec<T> *Dv, const Vec<T> *Pp, int c) -> Vec<T> {
             Vec<T> v = R[c];
@@ -197,11 +208,9 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                 if (MODE == 0 && with_halo) R[own] = v;
             }
             if (MODE == 0 && with_halo) {
-                for (int h = NCT - 1 - tid; h < nextra; h += NCT) {
-                    int c;
-                    if (h < TXV) c = h + 1;
-                    else if (h < 2 * TXV) c = (TY + 1) * BWc + (h - TXV) + 1;
-                    else { const int cc = h - 2 * TXV, side = cc / TY, r = cc - side * TY; c = (r + 1) * BWc + (side ? TXV + 1 : 0); }
+                if (extra0 >= 0) R[extra0] = pnew_cell(R, Dv, Pp, extra0);
+                for (int h = NCT - 1 - tid + NCT; h < nextra; h += NCT) {      // only when the halo outnumbers the threads
+                    const int c = halo_cell(h);
                     R[c] = pnew_cell(R, Dv, Pp, c);
                 }
             }
@@ -280,13 +289,15 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                         const T pl = (e == 0) ? left : pc.a[e == 0 ? 0 : e - 1];
                         const T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
                         const T exh = (e == VEC - 1) ? exr : ex.a[e == VEC - 1 ? e : e + 1];
-                        T v = (T(1) / dinv.a[e]) * pc.a[e];       // D = 1/Dinv: the diagonal of Eq. 3
+                        // two short FMA chains instead of one of seven (latency), summed at the end
+                        T v = rcp_rn(dinv.a[e]) * pc.a[e];        // D = 1/Dinv (correctly rounded): the diagonal of Eq. 3
                         v = fma(-ex.a[e], pl, v);
                         v = fma(-exh, pr, v);
                         v = fma(-eyl.a[e], up.a[e], v);
-                        v = fma(-eyh.a[e], dn.a[e], v);
-                        v = fma(-ezc.a[e], pm.a[e], v);
-                        v = fma(-ezn.a[e], pn.a[e], v);
+                        T w = -eyh.a[e] * dn.a[e];
+                        w = fma(-ezc.a[e], pm.a[e], w);
+                        w = fma(-ezn.a[e], pn.a[e], w);
+                        v += w;
                         if (e >= nvalid) v = T(0);     // pad column: exm[nx] is node nx-1's face, not a row of A
                         if (MODE == 0) acc = fma((double)pc.a[e], (double)v, acc);
                         ap.a[e] = (MODE == 1) ? (T)((double)v * a.out_scale) : v;
