@@ -112,7 +112,9 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
     const int TXV = a.TXV, TY = a.TY, TZ = a.TZ, NS = a.nstage;
     const SlotLayout L = slot_layout(TXV, TY, PAL ? VEC : 0);
-    unsigned char *base = (unsigned char *)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    // 128-byte aligned ring base; plain pointer arithmetic on the __shared__ symbol keeps the address space known
+    // to the compiler (LDS/STS instead of generic LD/ST)
+    unsigned char *base = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
 
     if (tid == 0) {
         for (int s = 0; s < NS; s++) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], NCW); }
