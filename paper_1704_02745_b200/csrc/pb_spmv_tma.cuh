@@ -129,7 +129,8 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         if (lane == 0) {
             const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0),
                            pol_pold = l2_policy((a.l2hints & 4) ? 1 : 0);
-            uint32_t cnt = 0;
+            int s = 0;                                  // ring slot of the next item and its phase parity
+            uint32_t ph = 0;
             for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
                 int b = tile;
                 const int bx = b % a.ntx; b /= a.ntx;
@@ -137,11 +138,9 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                 const int bz = b / a.nty;
                 const int x0 = bx * TXV * VEC, j0 = by * TY;
                 const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
-                for (int q = k0 - 1; q <= k1; q++, cnt++) {
-                    const int s = cnt % NS;
-                    const uint32_t ph = (cnt / NS) & 1;
+                for (int q = k0 - 1; q <= k1; q++, s = (s + 1 == NS) ? 0 : s + 1, ph ^= (s == 0)) {
                     mbar_wait(&empty_bar[s], ph ^ 1);
-                    unsigned char *slot = base + (size_t)s * L.slot;
+                    unsigned char *slot = base + s * (uint32_t)L.slot;
                     const bool centre = (q >= k0) && (q < k1);   // q is a plane this tile writes
                     const bool ez = (q >= k0);
                     uint32_t bytes = L.bZ * (MODE == 0 ? 3 : 1);
@@ -241,7 +240,11 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             if (lane == 0) mbar_arrive(&empty_bar[s]);
         };
 
-        uint32_t cnt = 0;
+        int rs = 0;                                    // ring slot of the next item and its phase parity
+        uint32_t rp = 0;
+        auto advance = [&]() { rs = (rs + 1 == NS) ? 0 : rs + 1; rp ^= (rs == 0); };
+        const uint32_t slot_bytes = (uint32_t)L.slot;
+        const size_t plane = (size_t)ny * P;
         for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
             int b = tile;
             const int bx = b % a.ntx; b /= a.ntx;
@@ -255,24 +258,24 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             lead = x0 & 15;
 
             // item k0-1: only the own column's value is needed
-            int s = cnt % NS;
-            mbar_wait(&full_bar[s], (cnt / NS) & 1);
-            Vec<T> pm = update(base + (size_t)s * L.slot, false);
-            release(s);
-            cnt++;
+            mbar_wait(&full_bar[rs], rp);
+            Vec<T> pm = update(base + rs * slot_bytes, false);
+            release(rs);
+            advance();
             // item k0
-            int sk = cnt % NS;
-            mbar_wait(&full_bar[sk], (cnt / NS) & 1);
-            unsigned char *slotk = base + (size_t)sk * L.slot;
+            int sk = rs;
+            mbar_wait(&full_bar[sk], rp);
+            unsigned char *slotk = base + sk * slot_bytes;
             Vec<T> pc = update(slotk, true);
             Vec<T> ezc = intile ? coef(slotk + L.oEZ, ty, TXV) : zerov<T>();
-            cnt++;
+            advance();
             named_bar_sync(1, NCT);
 
-            for (int k = k0; k < k1; k++) {
-                const int s1 = cnt % NS;
-                mbar_wait(&full_bar[s1], (cnt / NS) & 1);
-                unsigned char *slot1 = base + (size_t)s1 * L.slot;
+            size_t idx = ((size_t)k0 * ny + j) * P + i0;
+            for (int k = k0; k < k1; k++, idx += plane) {
+                const int s1 = rs;
+                mbar_wait(&full_bar[s1], rp);
+                unsigned char *slot1 = base + s1 * slot_bytes;
                 const Vec<T> pn = update(slot1, k + 1 < k1);
                 const Vec<T> ezn = intile ? coef(slot1 + L.oEZ, ty, TXV) : zerov<T>();
                 if (active) {
@@ -284,7 +287,6 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                     const T exr = PAL ? lut[slotk[L.oEX + ty * L.bw + lead + tx * VEC + VEC]]
                                       : reinterpret_cast<const Vec<T> *>(slotk + L.oEX)[ty * (TXV + 1) + tx + 1].a[0];
                     const Vec<T> eyl = coef(slotk + L.oEY, ty, TXV), eyh = coef(slotk + L.oEY, ty + 1, TXV);
-                    const size_t idx = ((size_t)k * ny + j) * P + i0;
                     Vec<T> ap;
 #pragma unroll
                     for (int e = 0; e < VEC; e++) {
@@ -318,7 +320,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                 named_bar_sync(1, NCT);   // p_new(k+1) box complete; everyone is done with slot sk
                 release(sk);
                 pm = pc; pc = pn; ezc = ezn; sk = s1; slotk = slot1;
-                cnt++;
+                advance();
             }
             release(sk);                  // item k1 (only its own-column values were used)
         }
