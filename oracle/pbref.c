@@ -248,7 +248,8 @@ int pbref_get_diag(pbref *s, double *d_out)
  * Returns PBREF_OK, PBREF_MAXITER (phi = last iterate) or PBREF_BREAKDOWN (p.Ap <= 0 or NaN).
  */
 int pbref_solve(pbref *s, double tol, int maxiter, int precond, double *phi,
-                int *iters_out, double *relres_out, double *true_relres_out, double *resid_hist)
+                int *iters_out, double *relres_out, double *true_relres_out, double *resid_hist,
+                const double *phi0 /* initial guess of step 1; NULL = 0 as in the paper's runs */)
 {
     if (!s || !phi || !(tol > 0.0) || maxiter < 0) return PBREF_INVALID;
     const size_t n = (size_t)s->nx * s->ny * s->nz;
@@ -260,10 +261,18 @@ int pbref_solve(pbref *s, double tol, int maxiter, int precond, double *phi,
     const double *b = s->b, *D = s->D;
     int status = PBREF_OK;
 
-    /* step 1: l = 0, phi_0 = 0 so r_0 = b - A phi_0 = b */
+    /* step 1: l = 0, r_0 = b - A phi_0; phi_0 = 0 in the paper's runs gives r_0 = b */
     int l = 0;
-    PAR_FOR
+    if (phi0) {
+        PAR_FOR
+    for (size_t c = 0; c < n; c++) phi[c] = phi0[c];
+        pbref_apply(s, phi, Ap);
+        PAR_FOR
+    for (size_t c = 0; c < n; c++) r[c] = b[c] - Ap[c];
+    } else {
+        PAR_FOR
     for (size_t c = 0; c < n; c++) { phi[c] = 0.0; r[c] = b[c]; }
+    }
     const double bb = dot(s, b, b);
     /* step 2: solve M z_0 = r_0, p_0 = z_0 */
     PAR_FOR

@@ -43,7 +43,7 @@ def _load():
         lib.pbref_apply.argtypes = [vp, _dp, _dp]
         lib.pbref_get_b.argtypes = [vp, _dp]
         lib.pbref_get_diag.argtypes = [vp, _dp]
-        lib.pbref_solve.argtypes = [vp, cd, ci, ci, _dp, ctypes.POINTER(ci), _dp, _dp, _dp]
+        lib.pbref_solve.argtypes = [vp, cd, ci, ci, _dp, ctypes.POINTER(ci), _dp, _dp, _dp, _dp]
         lib.pbref_destroy.argtypes = [vp]
         lib.pbref_num_threads.restype = ci
         _lib = lib
@@ -105,15 +105,16 @@ class PBRef:
         _load().pbref_get_diag(self._h, _ptr(out))
         return out.reshape(self.shape)
 
-    def solve(self, tol, maxiter, precond=True, history=False):
+    def solve(self, tol, maxiter, precond=True, history=False, phi0=None):
         """Jacobi-PCG.  Returns dict(phi, iters, relres, true_relres, status)."""
         phi = np.empty(self.nx * self.ny * self.nz)
         it = ctypes.c_int(0)
         rel = ctypes.c_double(0.0)
         trel = ctypes.c_double(0.0)
         hist = np.zeros(maxiter + 1) if history else None
+        x0 = None if phi0 is None else _f64(phi0).reshape(-1)
         st = _load().pbref_solve(self._h, float(tol), int(maxiter), 1 if precond else 0, _ptr(phi),
-                                 ctypes.byref(it), ctypes.byref(rel), ctypes.byref(trel), _ptr(hist))
+                                 ctypes.byref(it), ctypes.byref(rel), ctypes.byref(trel), _ptr(hist), _ptr(x0))
         if st not in (OK, MAXITER, BREAKDOWN):
             raise RuntimeError(f"pbref_solve failed: status {st}")
         out = dict(phi=phi.reshape(self.shape), iters=it.value, relres=rel.value,

@@ -318,3 +318,26 @@ def test_thread_count_does_not_change_bits():
         root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
         outs.append(subprocess.check_output([sys.executable, "-c", code], env=env, cwd=root))
     assert outs[0] == outs[1]
+
+
+def test_initial_guess_step1_general_phi0():
+    """Step 1 with a general phi_0 (r_0 = b - A phi_0), pinned against the dense direct solve:
+    the exact solution as phi_0 stops at l = 0; any phi_0 converges to the same x; the first residual equals
+    ||b - A phi_0|| / ||b|| computed from the dense matrix."""
+    nx, ny, nz = 7, 6, 5
+    inp = random_operator(nx, ny, nz, 5)
+    A = dense_from_eq3(nx, ny, nz, inp.h, inp.eps_x, inp.eps_y, inp.eps_z, inp.kbar2)
+    o = pbref.from_inputs(inp)
+    b = o.b().ravel()
+    x = np.linalg.solve(A, b)
+    exact = o.solve(1e-9, 100, phi0=x.reshape(nz, ny, nx))
+    assert exact["iters"] == 0 and np.array_equal(exact["phi"].ravel(), x)
+    g = np.random.default_rng(1).standard_normal(x.size)
+    res = o.solve(1e-12, 2000, phi0=g.reshape(nz, ny, nx), history=True)
+    assert np.abs(res["phi"].ravel() - x).max() <= 1e-10 * np.abs(x).max()
+    assert abs(res["history"][0] - np.linalg.norm(b - A @ g) / np.linalg.norm(b)) <= 1e-12 * res["history"][0]
+    # a guess close to the solution needs fewer iterations than phi_0 = 0
+    near = o.solve(1e-10, 2000, phi0=(x * (1 + 1e-4 * g)).reshape(nz, ny, nx))
+    cold = o.solve(1e-10, 2000)
+    assert near["iters"] < cold["iters"]
+    assert np.abs(near["phi"].ravel() - x).max() <= 1e-8 * np.abs(x).max()
