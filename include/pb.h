@@ -104,6 +104,15 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
                    void *phi_out, pb_memspace where, int *iters_out, double *relres_out);
 
 /*
+ * pb_solve_from -- pb_solve with a given initial guess phi_0 (step 1 of PAPER.md:108: r_0 = b - A phi_0; the
+ * paper's own runs use phi_0 = 0).  phi0 has the layout, precision and memory space of phi_out
+ * and may alias it; NULL = 0.  The stopping rule stays ||r_l|| / ||b|| < tol.  Meant for sequences of nearby
+ * right-hand sides (MD snapshots): start from the previous potential (NEXT row f2).
+ */
+pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
+                        const void *phi0, void *phi_out, pb_memspace where, int *iters_out, double *relres_out);
+
+/*
  * pb_create_from_atoms -- NEXT row f1, the paper's stated next step "integrated grid stencil setup on GPU"
  * (PAPER.md:11, 283): build the inputs of Eq. 3 on the device from atoms and hand them to pb_create.
  *   centres [n_atoms][3] (x,y,z; node (i,j,k) sits at (i h, j h, k h)), radii [n_atoms], charges [n_atoms]

@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size")
+           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -52,6 +52,7 @@ def load_library():
     lib.pb_apply.argtypes = [vp, ci, vp, vp, ci]
     lib.pb_solve.argtypes = [vp, cd, ci, ci, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd)]
     lib.pb_solve_begin.argtypes = [vp, ci]
+    lib.pb_solve_from.argtypes = [vp, cd, ci, ci, ci, vp, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd)]
     lib.pb_iterate.argtypes = [vp, ci, ci]
     lib.pb_destroy.argtypes = [vp]
     lib.pb_query.argtypes = [vp, ci, vp]
@@ -217,7 +218,7 @@ class PBSolver:
             raise PBError(st, "pb_apply")
         return y
 
-    def solve(self, tol, maxiter, precision="f64", check_every=32, out=None):
+    def solve(self, tol, maxiter, precision="f64", check_every=32, out=None, phi0=None):
         """Jacobi-PCG.  Returns dict(phi, iters, relres, status).
 
         `out`: optional numpy array / torch tensor (host or CUDA) receiving phi; default a new numpy array.
@@ -234,8 +235,16 @@ class PBSolver:
             raise TypeError("out must be contiguous")
         it = ctypes.c_int(0)
         rel = ctypes.c_double(0.0)
-        st = load_library().pb_solve(self._h, float(tol), int(maxiter), pc, int(check_every), op, so,
-                                     ctypes.byref(it), ctypes.byref(rel))
+        if phi0 is None:
+            st = load_library().pb_solve(self._h, float(tol), int(maxiter), pc, int(check_every), op, so,
+                                         ctypes.byref(it), ctypes.byref(rel))
+        else:   # initial guess (pb_solve_from): same precision and memory space as the output
+            gp, sg, keep0 = _marshal(phi0, dt, n, "phi0")
+            if sg != so:
+                raise ValueError("phi0 and out must live in the same memory space")
+            st = load_library().pb_solve_from(self._h, float(tol), int(maxiter), pc, int(check_every), gp, op, so,
+                                              ctypes.byref(it), ctypes.byref(rel))
+            del keep0
         if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
             raise PBError(st, "pb_solve")
         return dict(phi=out, iters=it.value, relres=rel.value, status=st)
@@ -245,7 +254,7 @@ class PBSolver:
         st = load_library().pb_set_preconditioner(self._h, 1 if jacobi else 0)
         if st != PB_OK:
             raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size")
+           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from")
 
     def solve_begin(self, precision):
         st = load_library().pb_solve_begin(self._h, _prec(precision)[0])

@@ -152,6 +152,7 @@ pb_status build_b(pb_handle *h, Work<T> &w)
 }
 
 template <typename T> pb_status setup_tma(pb_handle *h, Work<T> &w);
+pb_status ensure_stage(pb_handle *h, size_t bytes);
 
 // Lazily build the arrays of precision T (setup row a0).
 template <typename T>
@@ -485,7 +486,8 @@ pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
 }
 
 template <typename T>
-pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch)
+pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch, const void *phi0 = nullptr,
+                      pb_memspace where = PB_DEVICE)
 {
     PB_TRY(ensure<T>(h));
     Work<T> &w = work<T>(h);
@@ -494,6 +496,20 @@ pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch)
     k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w));
     PB_CUDA(cudaGetLastError());
     h->launches += 2;
+    if (phi0) {   // step 1 with a given phi_0: x = phi_0, r = b - A phi_0
+        const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+        const T *src = (const T *)phi0;
+        if (where == PB_HOST) {
+            PB_TRY(ensure_stage(h, n * sizeof(T)));
+            PB_CUDA(cudaMemcpyAsync(h->stage, phi0, n * sizeof(T), cudaMemcpyHostToDevice, h->stream));
+            src = (const T *)h->stage;
+        }
+        k_pad<T, T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
+        launch_spmv<T, 1>(h, w, 1.0);                      // Ap = A' phi_0
+        k_warm<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w), w.tmp);
+        PB_CUDA(cudaGetLastError());
+        h->launches += 3;
+    }
     return PB_OK;
 }
 
@@ -528,9 +544,9 @@ pb_status ensure_stage(pb_handle *h, size_t bytes)
 
 template <typename T>
 pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, void *phi_out,
-                     pb_memspace where, int *iters_out, double *relres_out)
+                     pb_memspace where, int *iters_out, double *relres_out, const void *phi0 = nullptr)
 {
-    PB_TRY(begin_solve<T>(h, tol, maxiter, 1));
+    PB_TRY(begin_solve<T>(h, tol, maxiter, 1, phi0, where));
     Work<T> &w = work<T>(h);
     const int m = check_every;
     bool graph_ok = h->use_graph && get_graph<T>(h, w, m) == PB_OK;
@@ -762,6 +778,18 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out)
                           : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out);
+}
+
+pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
+                        const void *phi0, void *phi_out, pb_memspace where, int *iters_out, double *relres_out)
+{
+    if (!h || !phi_out || !(tol > 0.0) || !std::isfinite(tol) || maxiter < 0 || check_every < 1 ||
+        !valid_prec(prec) || !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32
+               ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out, phi0)
+               : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out, phi0);
 }
 
 pb_status pb_set_preconditioner(pb_handle *h, int kind)

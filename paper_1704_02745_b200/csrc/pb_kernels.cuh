@@ -5,7 +5,7 @@
 //            Eq. 3, and the p.Ap dot of step 5 in the epilogue.
 //   k_vec  : alpha = rz/pAp (read from the device state); r -= alpha Ap (step 5); r.z = sum r^2 Dinv
 //            (Jacobi) and r.r; then beta (step 7) and the stopping rule of step 3.
-//   k_init : steps 1-2 with phi_0 = 0.
+//   k_init : steps 1-2 with phi_0 = 0;  k_warm: step 1 with a given phi_0.
 //   k_finish : the last pending phi += alpha p and the un-padding of phi (row a6).
 //
 // The solver works on the h^2-scaled system A' = h^2 A, b' = h^2 b (CG iterates and the
@@ -29,10 +29,11 @@ namespace pb {
 // ---------------------------------------------------------------------------------------
 // finaliser shared by k_vec and k_init: beta (step 7) and the stopping rule (step 3)
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void finish_iteration(State *st, double rz_new, double rr, bool init)
+// init: 0 = an iteration, 1 = steps 1-2 with phi_0 = 0 (r_0 = b), 2 = steps 1-2 with a given phi_0 (||b||^2 kept)
+__device__ __forceinline__ void finish_iteration(State *st, double rz_new, double rr, int init)
 {
     if (init) {
-        st->bb = rr;                 // r_0 = b (phi_0 = 0)
+        if (init == 1) st->bb = rr;  // r_0 = b (phi_0 = 0)
         st->beta = 0.0;              // first k_spmv gives p_0 = z_0 (step 2)
         st->iter_cur = 0;
     } else {
@@ -42,6 +43,7 @@ __device__ __forceinline__ void finish_iteration(State *st, double rz_new, doubl
     st->rz = rz_new;
     st->rr = rr;
     if (!st->latch) return;
+    if (init == 2) { st->done = 0; st->status = 0; }   // re-decide what the phi_0 = 0 pass latched
     const double bb = st->bb;
     const int l = st->iter_cur;
     if (!isfinite(rr) || !isfinite(rz_new)) { st->done = 1; st->iters = l; st->status = 5; }
@@ -64,7 +66,7 @@ struct VecArgs {
 
 // stage 1 + stage 2 of the two dots of k_vec / k_init, then the finaliser
 __device__ __forceinline__ void reduce_and_finish(State *st, double *partials, double s_rz, double s_rr,
-                                                  double *red, int *s_last, bool init)
+                                                  double *red, int *s_last, int init)
 {
     const double t_rz = block_sum(s_rz, red);
     const double t_rr = block_sum(s_rr, red);
@@ -116,7 +118,7 @@ __global__ void __launch_bounds__(256) k_vec(const VecArgs<T> a)
         }
         st16_hint(a.r + idx, rv.a, pol_keep);
     }
-    reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, false);
+    reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, 0);
 }
 
 // steps 1-2 with phi_0 = 0: x = 0, r = b, p buffer cleared, r.z and r.r
@@ -142,7 +144,35 @@ __global__ void __launch_bounds__(256) k_init(const VecArgs<T> a)
         stv(a.pzero + idx, zerov<T>());
         stv(a.r + idx, rv);
     }
-    reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, true);
+    reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, 1);
+}
+
+// step 1 with a given initial guess (r_0 = b - A phi_0), run after k_init and after k_spmv_tma<MODE 1>
+// has put A'phi_0 into Ap:  x = phi_0 (padded, in `x0`),  r = b - A'phi_0,  r.z and r.r;  ||b||^2 stays from k_init.
+template <typename T>
+__global__ void __launch_bounds__(256) k_warm(const VecArgs<T> a, const T *__restrict__ x0)
+{
+    constexpr int VEC = VecN<T>::value;
+    __shared__ double red[32];
+    __shared__ int s_last;
+    double s_rz = 0.0, s_rr = 0.0;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < a.nvec; v += stride) {
+        const size_t idx = v * VEC;
+        Vec<T> rv = ldv(a.b + idx);
+        const Vec<T> qv = ldv(a.Ap + idx);
+        const Vec<T> dv = ldv(a.Dinv + idx);
+#pragma unroll
+        for (int e = 0; e < VEC; e++) {
+            rv.a[e] = rv.a[e] - qv.a[e];
+            const T zv = a.precond ? dv.a[e] * rv.a[e] : rv.a[e];
+            s_rz = fma((double)rv.a[e], (double)zv, s_rz);
+            s_rr = fma((double)rv.a[e], (double)rv.a[e], s_rr);
+        }
+        stv(a.x + idx, ldv(x0 + idx));
+        stv(a.r + idx, rv);
+    }
+    reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, 2);
 }
 
 // row a6: phi_out (dense [nz][ny][nx], type S) = x + alpha*p -- the phi update of the last

@@ -341,3 +341,34 @@ def test_palette_and_full_precision_coefficients_agree(pkg, pbref, prec, tol):
     many = random_operator(21, 9, 8, seed=6, two_valued=False)      # ~5000 distinct face values
     with pkg.PBSolver(*many.args()) as s:
         assert s.palette_size() == 0
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_warm_start_matches_oracle(pkg, pbref, prec, tol):
+    """NEXT row f2 (part): pb_solve_from = step 1 with a given phi_0.  Snapshot-style use: solve,
+    perturb the charges (new rhs and ghost values), restart from the previous potential.  Iteration counts and
+    potentials must match the oracle run from the same phi_0; the restart must need fewer iterations."""
+    inp = make_config(2)
+    from workloads import perturbed_charges
+
+    rhs2, bc2 = perturbed_charges(inp, 0, device="cpu")
+    ref = pbref.from_inputs(inp)
+    dt = np.float64 if prec == "f64" else np.float32
+    with pkg.PBSolver(*inp.args()) as s:
+        first = s.solve(tol, 5000, prec)
+        s.set_rhs(rhs2, bc2)
+        ref.set_rhs(rhs2, bc2)
+        cold = s.solve(tol, 5000, prec)
+        warm = s.solve(tol, 5000, prec, phi0=first["phi"].copy())
+        again = s.solve(tol, 5000, prec, phi0=warm["phi"].astype(dt))       # already converged -> 0 or 1 iterations
+    o_warm = ref.solve(tol, 5000, phi0=first["phi"].astype(np.float64))
+    o_cold = ref.solve(tol, 5000)
+    ref.close()
+    scale = np.max(np.abs(o_cold["phi"]))
+    lim = 1e-8 if prec == "f64" else 1e-4
+    assert warm["status"] == 0 and warm["relres"] < tol
+    assert abs(warm["iters"] - o_warm["iters"]) <= max(1, round(0.05 * o_warm["iters"])), (warm["iters"], o_warm["iters"])
+    assert np.max(np.abs(warm["phi"] - o_warm["phi"])) <= lim * scale
+    assert np.max(np.abs(warm["phi"] - cold["phi"])) <= 10 * lim * scale
+    assert warm["iters"] < cold["iters"]
+    assert again["iters"] <= 1
