@@ -287,7 +287,8 @@ def run_ours(args, rank, local_rank, world):
     if args.batch > 0 and "charges" in inp.meta:
         from workloads import perturbed_charges
 
-        t_b, it_b = 0.0, []
+        t_b, it_b, t_w, it_w = 0.0, [], 0.0, []
+        out_w = torch.empty_like(out_d)
         for sidx in range(args.batch):
             rhs_s, bc_s = perturbed_charges(inp, world * sidx + rank, device=f"cuda:{local_rank}")
             rhs_d = torch.from_numpy(np.ascontiguousarray(rhs_s)).to(dev)
@@ -298,10 +299,22 @@ def run_ours(args, rank, local_rank, world):
             it_b.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
             torch.cuda.synchronize()
             t_b += time.perf_counter() - t0
+            # the same member restarted from the previous member's potential (pb_solve_from, NEXT row f2)
+            if sidx == 0:
+                out_w.copy_(out_d)
+            else:
+                t0 = time.perf_counter()
+                it_w.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_w,
+                                         phi0=out_w)["iters"])
+                torch.cuda.synchronize()
+                t_w += time.perf_counter() - t0
             del rhs_d, bc_d
         batch = {"solves": args.batch, "solves_per_s": args.batch / t_b, "ms_per_solve": 1e3 * t_b / args.batch,
                  "mean_iters": float(np.mean(it_b)), "min_iters": int(min(it_b)), "max_iters": int(max(it_b)),
-                 "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member, this rank only"}
+                 "warm_start": ({"mean_iters": float(np.mean(it_w)), "ms_per_solve": 1e3 * t_w / len(it_w)}
+                                if it_w else None),
+                 "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member, this rank only; warm_start: "
+                         "the same members solved again from the previous member's potential (pb_solve_from)"}
 
     # ---- optional (NEXT row f1): the same problem built on the GPU from atoms, and a charge update ---------------
     setup = None
