@@ -5,6 +5,7 @@
 #include "../../include/pb.h"
 #include "pb_kernels.cuh"
 #include "pb_spmv_tma.cuh"
+#include "pb_persist.cuh"
 #include "pb_setup.cuh"
 #include "pb_grid.cuh"
 
@@ -32,6 +33,9 @@ struct Work {
     int qTXV = 0, qTY = 0, qTZ = 0, qntx = 0, qnty = 0, qntz = 0, qns = 0, qgrid = 0, qthreads = 0;
     size_t qsmem = 0;
     CUtensorMap tm_r, tm_tmp, tm_dinv, tm_p0, tm_p1, tm_x, tm_ex, tm_ey, tm_ez;
+    // L2-resident grids: the whole loop as one cooperative kernel (pb_persist.cuh)
+    bool persist = false;
+    int pgrid = 0;
     // coefficient palette (pb_setup.cuh): byte face indices + table, instead of exm/eym/ezm
     bool pal = false;
     unsigned char *exi = nullptr, *eyi = nullptr, *ezi = nullptr;
@@ -189,7 +193,19 @@ pb_status ensure(pb_handle *h)
     }
     w.pal = h->pal_n > 0;
     w.Pb = (w.P + 15) / 16 * 16;
+    // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
+    {
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
+        const double mb = 11.0 * (double)w.npad * sizeof(T) / 1.0e6;
+        w.persist = coop && env_int("PB_PERSIST", 1) != 0 && mb <= (double)env_int("PB_PERSIST_MAX_MB", 64);
+    }
     pb_status s = PB_OK;
+    if (w.pal && w.persist &&
+        ((s = alloc_arr(&w.exm, w.npad)) || (s = alloc_arr(&w.eym, n_ey)) || (s = alloc_arr(&w.ezm, n_ez)))) {
+        free_work(w);
+        return s;
+    }
     if (w.pal) {
         const size_t b_ex = (size_t)h->nz * h->ny * w.Pb, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pb,
                      b_ez = (size_t)(h->nz + 1) * h->ny * w.Pb;
@@ -206,7 +222,15 @@ pb_status ensure(pb_handle *h)
         return s;
     }
     w.vec_grid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * env_int("PB_VEC_BPS", 8));
-    const size_t need = (size_t)kNumSM * 8 > (size_t)2 * w.vec_grid ? (size_t)kNumSM * 8 : (size_t)2 * w.vec_grid;
+    if (w.persist) {
+        int bps = 0;
+        PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T>, 256, 0));
+        if (bps < 1) w.persist = false;
+        bps = bps > env_int("PB_PERSIST_BPS", 4) ? env_int("PB_PERSIST_BPS", 4) : bps;
+        w.pgrid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * bps);
+    }
+    size_t need = (size_t)kNumSM * 8 > (size_t)2 * w.vec_grid ? (size_t)kNumSM * 8 : (size_t)2 * w.vec_grid;
+    if ((size_t)3 * w.pgrid > need) need = (size_t)3 * w.pgrid;
     if (need > h->partials_cap) {
         if (h->partials) cudaFree(h->partials);
         h->partials = nullptr;
@@ -549,10 +573,21 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     PB_TRY(begin_solve<T>(h, tol, maxiter, 1, phi0, where));
     Work<T> &w = work<T>(h);
     const int m = check_every;
-    bool graph_ok = h->use_graph && get_graph<T>(h, w, m) == PB_OK;
+    if (w.persist) {
+        // L2-resident grid: steps 3-8 in one cooperative kernel, exit decided on the device
+        PersistArgs<T> pa;
+        pa.x = w.x; pa.r = w.r; pa.p0 = w.p0; pa.p1 = w.p1; pa.Ap = w.Ap;
+        pa.Dinv = w.Dinv; pa.exm = w.exm; pa.eym = w.eym; pa.ezm = w.ezm;
+        pa.nx = h->nx; pa.ny = h->ny; pa.nz = h->nz; pa.P = w.P; pa.precond = h->precond;
+        pa.st = h->st; pa.partials = h->partials;
+        void *kargs[] = {(void *)&pa};
+        PB_CUDA(cudaLaunchCooperativeKernel((const void *)k_pcg_persistent<T>, dim3(w.pgrid), dim3(256), kargs, 0, h->stream));
+        h->launches += 1;
+    }
+    bool graph_ok = !w.persist && h->use_graph && get_graph<T>(h, w, m) == PB_OK;
     // chunk c is enqueued before the latch of chunk c-1 is waited for, so the device never idles
     const long max_chunks = (long)maxiter / m + 2;
-    int seen_done = 0;
+    int seen_done = w.persist ? 1 : 0;
     for (long c = 0; c < max_chunks + 1 && !seen_done; c++) {
         if (graph_ok) { PB_CUDA(cudaGraphLaunch(w.graph, h->stream)); h->launches += 2LL * m; }
         else PB_TRY(enqueue_iterations<T>(h, w, m));

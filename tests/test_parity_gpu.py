@@ -249,7 +249,7 @@ def test_fullsize_385_spmv_and_solve_properties(pkg, pbref):
     ref.close()
 
 
-TILE_ENV = ("PB_TXV", "PB_TY", "PB_NS", "PB_BPS", "PB_TZ", "PB_AUTOTUNE")
+TILE_ENV = ("PB_TXV", "PB_TY", "PB_NS", "PB_BPS", "PB_TZ", "PB_AUTOTUNE", "PB_PERSIST")
 TILE_CONFIGS = [dict(PB_AUTOTUNE=0), dict(PB_TXV=7, PB_TY=3, PB_NS=3, PB_BPS=2, PB_TZ=5),
                 dict(PB_TXV=20, PB_TY=8, PB_NS=6, PB_BPS=1, PB_TZ=99), dict(PB_TXV=5, PB_TY=2, PB_NS=4, PB_BPS=4, PB_TZ=1),
                 dict(PB_TXV=13, PB_TY=5, PB_NS=5, PB_BPS=3, PB_TZ=33), dict()]
@@ -274,6 +274,7 @@ def test_tiling_independence(pkg, pbref, prec):
             for k in TILE_ENV:
                 os.environ.pop(k, None)
             os.environ.update({k: str(v) for k, v in cfg.items()})
+            os.environ["PB_PERSIST"] = "0"          # small grid: force the two-kernel TMA path under test
             with pkg.PBSolver(*inp.args()) as s:
                 y = s.apply(x, prec)
                 runs = [s.solve(tol, 5000, prec, check_every=9) for _ in range(2)]
@@ -372,3 +373,43 @@ def test_warm_start_matches_oracle(pkg, pbref, prec, tol):
     assert np.max(np.abs(warm["phi"] - cold["phi"])) <= 10 * lim * scale
     assert warm["iters"] < cold["iters"]
     assert again["iters"] <= 1
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_persistent_and_two_kernel_paths_agree(pkg, pbref, prec, tol):
+    """NEXT row f2 (part): L2-resident grids run steps 3-8 in one cooperative kernel (k_pcg_persistent); larger ones
+    (or PB_PERSIST=0) through k_spmv_tma + k_vec.  Both must meet the oracle bar, agree with each other, stop on
+    maxiter identically, honour the M = I variant and a warm start, and be bitwise repeatable."""
+    inp = make_config(2)
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(tol, 5000)
+    o_cg = ref.solve(tol, 5000, precond=False)
+    o7 = ref.solve(tol, 7)
+    ref.close()
+    scale = np.max(np.abs(o["phi"]))
+    lim = 1e-8 if prec == "f64" else 1e-4
+    saved = os.environ.pop("PB_PERSIST", None)
+    res = {}
+    try:
+        for mode in ("1", "0"):
+            os.environ["PB_PERSIST"] = mode
+            with pkg.PBSolver(*inp.args()) as s:
+                a, b = s.solve(tol, 5000, prec), s.solve(tol, 5000, prec)
+                assert np.array_equal(a["phi"], b["phi"]) and a["iters"] == b["iters"]
+                m7 = s.solve(tol, 7, prec)
+                w = s.solve(tol, 5000, prec, phi0=a["phi"].copy())
+                s.set_preconditioner(False)
+                cg = s.solve(tol, 5000, prec)
+            res[mode] = (a, m7, cg, w)
+    finally:
+        os.environ.pop("PB_PERSIST", None)
+        if saved is not None:
+            os.environ["PB_PERSIST"] = saved
+    for a, m7, cg, w in res.values():
+        assert a["status"] == 0 and abs(a["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"]))
+        assert np.max(np.abs(a["phi"] - o["phi"])) <= lim * scale
+        assert m7["status"] == pkg.binding.PB_ERR_MAXITER and m7["iters"] == 7
+        assert np.max(np.abs(m7["phi"] - o7["phi"])) <= lim * scale
+        assert abs(cg["iters"] - o_cg["iters"]) <= max(1, round(0.05 * o_cg["iters"]))
+        assert w["iters"] <= 1
+    assert np.max(np.abs(res["1"][0]["phi"] - res["0"][0]["phi"])) <= lim * scale
