@@ -198,7 +198,7 @@ pb_status ensure(pb_handle *h)
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
         const double mb = 11.0 * (double)w.npad * sizeof(T) / 1.0e6;
-        w.persist = coop && env_int("PB_PERSIST", 1) != 0 && mb <= (double)env_int("PB_PERSIST_MAX_MB", 64);
+        w.persist = coop && env_int("PB_PERSIST", 1) != 0 && mb <= (double)env_int("PB_PERSIST_MAX_MB", 100);
     }
     pb_status s = PB_OK;
     if (w.pal && w.persist &&
