@@ -413,3 +413,29 @@ def test_persistent_and_two_kernel_paths_agree(pkg, pbref, prec, tol):
         assert abs(cg["iters"] - o_cg["iters"]) <= max(1, round(0.05 * o_cg["iters"]))
         assert w["iters"] <= 1
     assert np.max(np.abs(res["1"][0]["phi"] - res["0"][0]["phi"])) <= lim * scale
+
+
+@pytest.mark.slow
+def test_config5_headline_parity_full_size(pkg, pbref):
+    """BASELINE.json configs[4] (385^3, 60 000 atoms) exactly as bench.py runs it (autotuned plan, palette,
+    check_every 32): the fp32 solve to 1e-5 and the fp64 solve to 1e-10 against the full oracle solves -- every node,
+    the north-star tolerances.  (The oracle needs about a minute on the GPU box's host cores.)"""
+    inp = make_config(5, device="cuda")
+    ref = pbref.from_inputs(inp)
+    o32 = ref.solve(1e-5, 5000)
+    o64 = ref.solve(1e-10, 5000)
+    ref.close()
+    scale = np.max(np.abs(o64["phi"]))
+    with pkg.PBSolver(*inp.args()) as s:
+        assert s.palette_size() == 4
+        g32 = s.solve(1e-5, 20000, "f32", check_every=32)
+        g64 = s.solve(1e-10, 20000, "f64", check_every=32)
+    assert g32["status"] == 0 and g64["status"] == 0
+    assert abs(g32["iters"] - o32["iters"]) <= round(0.05 * o32["iters"]), (g32["iters"], o32["iters"])
+    assert abs(g64["iters"] - o64["iters"]) <= round(0.05 * o64["iters"]), (g64["iters"], o64["iters"])
+    e32 = np.max(np.abs(g32["phi"] - o32["phi"])) / scale
+    e32t = np.max(np.abs(g32["phi"] - o64["phi"])) / scale
+    e64 = np.max(np.abs(g64["phi"] - o64["phi"])) / scale
+    print(f"config5: fp32 iters {g32['iters']} (oracle {o32['iters']}) err {e32:.2e} / {e32t:.2e}; "
+          f"fp64 iters {g64['iters']} (oracle {o64['iters']}) err {e64:.2e}")
+    assert e32 <= 1e-4 and e32t <= 1e-4 and e64 <= 1e-8
