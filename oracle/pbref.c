@@ -55,6 +55,7 @@ typedef struct pbref {
     double *D;                       /* diag(A) */
     double *plane;                   /* nz per-plane partial sums */
     int have_rhs;
+    int periodic;                    /* 1: periodic boundary condition: indices wrap, no ghost layer */
 } pbref;
 
 /* face dielectrics touching node (i,j,k), in the paper's notation */
@@ -111,7 +112,7 @@ int pbref_set_rhs(pbref *s, const double *rhs, const double *bc)
         for (int j = 0; j < ny; j++)
             for (int i = 0; i < nx; i++) {
                 double v = rhs ? rhs[NODE(s,i,j,k)] : 0.0;
-                if (bc) {
+                if (bc && !s->periodic) {
                     if (i == 0)      v += ih2 * EXM(s,i,j,k) * ghost_xm(s, bc, j, k);
                     if (i == nx - 1) v += ih2 * EXP(s,i,j,k) * ghost_xp(s, bc, j, k);
                     if (j == 0)      v += ih2 * EYM(s,i,j,k) * ghost_ym(s, bc, i, k);
@@ -176,12 +177,15 @@ static void apply_plane(const pbref *s, const double *x, double *y, int k)
     for (int j = 0; j < ny; j++)
         for (int i = 0; i < nx; i++) {
             const double xc = x[NODE(s,i,j,k)];
-            const double xim = (i > 0)      ? x[NODE(s,i-1,j,k)] : 0.0;
-            const double xip = (i < nx - 1) ? x[NODE(s,i+1,j,k)] : 0.0;
-            const double xjm = (j > 0)      ? x[NODE(s,i,j-1,k)] : 0.0;
-            const double xjp = (j < ny - 1) ? x[NODE(s,i,j+1,k)] : 0.0;
-            const double xkm = (k > 0)      ? x[NODE(s,i,j,k-1)] : 0.0;
-            const double xkp = (k < nz - 1) ? x[NODE(s,i,j,k+1)] : 0.0;
+            /* neighbours outside the grid: the ghost layer (value 0 here, its Dirichlet value sits in b) or, with the
+             * periodic boundary condition, the node on the opposite side (phi(-1) = phi(n-1), phi(n) = phi(0)) */
+            const int per = s->periodic;
+            const double xim = (i > 0)      ? x[NODE(s,i-1,j,k)] : (per ? x[NODE(s,nx-1,j,k)] : 0.0);
+            const double xip = (i < nx - 1) ? x[NODE(s,i+1,j,k)] : (per ? x[NODE(s,0,j,k)]    : 0.0);
+            const double xjm = (j > 0)      ? x[NODE(s,i,j-1,k)] : (per ? x[NODE(s,i,ny-1,k)] : 0.0);
+            const double xjp = (j < ny - 1) ? x[NODE(s,i,j+1,k)] : (per ? x[NODE(s,i,0,k)]    : 0.0);
+            const double xkm = (k > 0)      ? x[NODE(s,i,j,k-1)] : (per ? x[NODE(s,i,j,nz-1)] : 0.0);
+            const double xkp = (k < nz - 1) ? x[NODE(s,i,j,k+1)] : (per ? x[NODE(s,i,j,0)]    : 0.0);
             double v = 0.0;
             v += -ih2 * EXM(s,i,j,k) * (xim - xc);
             v += -ih2 * EXP(s,i,j,k) * (xip - xc);
@@ -220,6 +224,16 @@ static double dot(pbref *s, const double *u, const double *v)
     double tot = 0.0;
     for (int k = 0; k < s->nz; k++) tot += s->plane[k];
     return tot;
+}
+
+/* Periodic boundary condition (the paper's PBC runs): the face f = 0 and the face
+ * f = n of each direction are the same physical face (the caller passes equal values), the neighbour across it is
+ * the node on the opposite side, and there are no ghost values.  Call before pbref_set_rhs. */
+int pbref_set_periodic(pbref *s, int flag)
+{
+    if (!s) return PBREF_INVALID;
+    s->periodic = flag ? 1 : 0;
+    return PBREF_OK;
 }
 
 int pbref_get_b(pbref *s, double *b_out)

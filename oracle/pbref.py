@@ -45,6 +45,7 @@ def _load():
         lib.pbref_get_diag.argtypes = [vp, _dp]
         lib.pbref_solve.argtypes = [vp, cd, ci, ci, _dp, ctypes.POINTER(ci), _dp, _dp, _dp, _dp]
         lib.pbref_destroy.argtypes = [vp]
+        lib.pbref_set_periodic.argtypes = [vp, ci]
         lib.pbref_num_threads.restype = ci
         _lib = lib
     return _lib
@@ -86,6 +87,10 @@ class PBRef:
         rh, bcv = _f64(rhs), _f64(bc)
         st = _load().pbref_set_rhs(self._h, _ptr(rh), _ptr(bcv))
         assert st == OK
+
+    def set_periodic(self, flag=True):
+        """Periodic boundary condition; call set_rhs afterwards to drop the ghost fold-in."""
+        assert _load().pbref_set_periodic(self._h, 1 if flag else 0) == OK
 
     def apply(self, x):
         """y = A x (Eq. 3 left-hand side, 1/h^2 included, ghost x = 0)."""

@@ -4,7 +4,7 @@ import itertools
 import numpy as np
 
 
-def dense_from_eq3(nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2):
+def dense_from_eq3(nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2, periodic=False):
     """Dense A assembled row by row straight from PAPER.md Eq. 3 (lines 50-62), tiny grids only.
 
     Each of the six bracketed terms -h^-2 eps_f [phi(nbr) - phi(c)] contributes +eps_f/h^2 to the
@@ -24,6 +24,8 @@ def dense_from_eq3(nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2):
             A[c, c] += e / h ** 2
             if 0 <= a < nx and 0 <= b_ < ny and 0 <= c_ < nz:
                 A[c, idx(a, b_, c_)] -= e / h ** 2
+            elif periodic:      # the neighbour across the box face is the node on the other side
+                A[c, idx(a % nx, b_ % ny, c_ % nz)] -= e / h ** 2
         A[c, c] += kbar2[k, j, i]
     return A
 

@@ -341,3 +341,42 @@ def test_initial_guess_step1_general_phi0():
     cold = o.solve(1e-10, 2000)
     assert near["iters"] < cold["iters"]
     assert np.abs(near["phi"].ravel() - x).max() <= 1e-8 * np.abs(x).max()
+
+
+def _periodic_faces(inp):
+    """Make face f = n equal to face f = 0 in each direction (one physical face under the periodic condition)."""
+    ex, ey, ez = inp.eps_x.copy(), inp.eps_y.copy(), inp.eps_z.copy()
+    ex[:, :, -1] = ex[:, :, 0]
+    ey[:, -1, :] = ey[:, 0, :]
+    ez[-1] = ez[0]
+    return ex, ey, ez
+
+
+def test_periodic_boundary_condition():
+    """The paper's PBC variant, pinned by (i) the closed-form Fourier eigenpairs of
+    the uniform periodic 7-point operator, (ii) a dense matrix assembled row by row from Eq. 3 with wrapped
+    neighbours, (iii) symmetry, and (iv) the dense direct solve."""
+    nx, ny, nz, h, eps, k2 = 8, 6, 5, 0.5, 3.0, 0.7
+    ex, ey, ez = uniform_eps(nx, ny, nz, eps)
+    o = pbref.PBRef(nx, ny, nz, h, ex, ey, ez, np.full((nz, ny, nx), k2))
+    o.set_periodic(True)
+    i, j, k = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij")
+    for (p, q, r) in [(0, 0, 0), (1, 0, 0), (2, 1, 3), (3, 2, 1)]:
+        for fn in (np.cos, np.sin):
+            v = fn(2 * np.pi * (p * i / nx + q * j / ny + r * k / nz)).transpose(2, 1, 0)
+            lam = 4 * eps / h ** 2 * (np.sin(np.pi * p / nx) ** 2 + np.sin(np.pi * q / ny) ** 2
+                                      + np.sin(np.pi * r / nz) ** 2) + k2
+            assert np.abs(o.apply(v) - lam * v).max() <= 1e-12 * max(lam, 1.0)
+    inp = random_operator(6, 5, 4, 9)
+    ex, ey, ez = _periodic_faces(inp)
+    A = dense_from_eq3(6, 5, 4, inp.h, ex, ey, ez, inp.kbar2, periodic=True)
+    assert np.array_equal(A, A.T) and np.linalg.eigvalsh(A).min() > 0
+    o = pbref.PBRef(6, 5, 4, inp.h, ex, ey, ez, inp.kbar2)
+    o.set_periodic(True)
+    o.set_rhs(inp.rhs, inp.bc)                         # ghost values are ignored under the periodic condition
+    assert np.array_equal(o.b(), inp.rhs)
+    x = np.random.default_rng(2).standard_normal((4, 5, 6))
+    assert np.abs(o.apply(x).ravel() - A @ x.ravel()).max() <= 1e-11 * np.abs(A @ x.ravel()).max()
+    res = o.solve(1e-12, 2000)
+    sol = np.linalg.solve(A, inp.rhs.ravel())
+    assert res["status"] == pbref.OK and np.abs(res["phi"].ravel() - sol).max() <= 1e-10 * np.abs(sol).max()
