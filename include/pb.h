@@ -143,6 +143,14 @@ pb_status pb_get_field(pb_handle *h, int which, double *out_host);
 pb_status pb_set_preconditioner(pb_handle *h, int kind);
 
 /*
+ * pb_set_boundary -- kind 0 (default): the free-space condition, Dirichlet values on the ghost layer; kind 1: the
+ * periodic boundary condition the paper also times.  Periodic: the neighbour across
+ * a box face is the node on the opposite side; face f = 0 and face f = n of a direction are one physical face (the
+ * caller passes equal values); bc is ignored.  In a matrix-free kernel the paper's "6 extra bands" are index wraps.
+ */
+pb_status pb_set_boundary(pb_handle *h, int kind);
+
+/*
  * pb_iterate -- benchmarking/profiling entry: enqueue exactly `n_iter` PCG iterations
  * (K_spmv + K_vec pairs, PAPER.md:115-126 steps 4-8) with the convergence latch disabled,
  * continuing from the state left by pb_solve_begin.  Does not synchronise.  Used by

@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from")
+           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -62,6 +62,7 @@ def load_library():
     lib.pb_profile.argtypes = [vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(cd)]
     lib.pb_launch_count.argtypes = [vp]
     lib.pb_set_preconditioner.argtypes = [vp, ci]
+    lib.pb_set_boundary.argtypes = [vp, ci]
     lib.pb_create_from_atoms.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, ci, vp, vp, vp, cd, cd, cd, ci, vp]
     lib.pb_set_charges.argtypes = [vp, vp, ci]
     lib.pb_get_field.argtypes = [vp, ci, vp]
@@ -254,7 +255,13 @@ class PBSolver:
         st = load_library().pb_set_preconditioner(self._h, 1 if jacobi else 0)
         if st != PB_OK:
             raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from")
+           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary")
+
+    def set_periodic(self, periodic: bool):
+        """False (default): Dirichlet ghost layer; True: periodic boundary condition."""
+        st = load_library().pb_set_boundary(self._h, 1 if periodic else 0)
+        if st != PB_OK:
+            raise PBError(st, "pb_set_boundary")
 
     def solve_begin(self, precision):
         st = load_library().pb_solve_begin(self._h, _prec(precision)[0])

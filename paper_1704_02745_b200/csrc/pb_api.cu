@@ -66,6 +66,7 @@ struct pb_handle {
     int use_graph;
     long long launches;          // kernels enqueued so far (graph-contained ones included)
     int precond;                 // 1 Jacobi (default), 0 none
+    int periodic;                // 0 Dirichlet ghost layer (free-space condition, default), 1 periodic
     PalTable *pal_table;         // device; distinct face values of the operator
     int pal_n;                   // -1: not examined yet, 0: more than 256 distinct values, else the table size
     // pb_create_from_atoms keeps the atom geometry for pb_set_charges
@@ -148,7 +149,7 @@ pb_status build_b(pb_handle *h, Work<T> &w)
 {
     const double h2 = h->h * h->h;
     k_setup_b<T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
-        h->eps_x, h->eps_y, h->eps_z, h->rhs, h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b);
+        h->eps_x, h->eps_y, h->eps_z, h->rhs, h->periodic ? nullptr : h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     w.b_ready = true;
@@ -495,6 +496,21 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
             MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
 }
 
+// periodic boundary condition: the wrap terms k_spmv_tma cannot see (k_wrap), right after it
+template <typename T, int MODE>
+void launch_wrap(pb_handle *h, Work<T> &w, double out_scale)
+{
+    if (!h->periodic) return;
+    WrapArgs<T> a;
+    a.pbuf0 = MODE == 0 ? w.p0 : w.tmp; a.pbuf1 = w.p1; a.Ap = w.Ap;
+    a.eps_x = h->eps_x; a.eps_y = h->eps_y; a.eps_z = h->eps_z;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P; a.out_scale = out_scale;
+    a.st = h->st; a.partials = h->partials;
+    const size_t shell = 2 * ((size_t)h->ny * h->nx + (size_t)h->nz * h->nx + (size_t)h->nz * h->ny);
+    k_wrap<T, MODE><<<grid_for(shell, 256, kNumSM * 2), 256, 0, h->stream>>>(a);
+    h->launches += 1;
+}
+
 // enqueue n PCG iterations: (k_spmv, k_vec) pairs, nothing else
 template <typename T>
 pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
@@ -502,6 +518,7 @@ pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
     const VecArgs<T> va = vec_args<T>(h, w);
     for (int it = 0; it < n; it++) {
         launch_spmv<T, 0>(h, w, 1.0);
+        launch_wrap<T, 0>(h, w, 1.0);
         k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
     }
     PB_CUDA(cudaGetLastError());
@@ -530,6 +547,7 @@ pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch, const vo
         }
         k_pad<T, T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
         launch_spmv<T, 1>(h, w, 1.0);                      // Ap = A' phi_0
+        launch_wrap<T, 1>(h, w, 1.0);
         k_warm<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w), w.tmp);
         PB_CUDA(cudaGetLastError());
         h->launches += 3;
@@ -545,7 +563,7 @@ pb_status get_graph(pb_handle *h, Work<T> &w, int m)
     cudaGraph_t g = nullptr;
     PB_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
     pb_status s = enqueue_iterations<T>(h, w, m);
-    h->launches -= 2LL * m;          // captured, not executed
+    h->launches -= (2LL + (h->periodic ? 1 : 0)) * m;          // captured, not executed
     cudaError_t e = cudaStreamEndCapture(h->stream, &g);
     if (s != PB_OK || e != cudaSuccess || !g) { cudaGetLastError(); return PB_ERR_CUDA; }
     e = cudaGraphInstantiate(&w.graph, g, 0);
@@ -578,7 +596,7 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
         PersistArgs<T> pa;
         pa.x = w.x; pa.r = w.r; pa.p0 = w.p0; pa.p1 = w.p1; pa.Ap = w.Ap;
         pa.Dinv = w.Dinv; pa.exm = w.exm; pa.eym = w.eym; pa.ezm = w.ezm;
-        pa.nx = h->nx; pa.ny = h->ny; pa.nz = h->nz; pa.P = w.P; pa.precond = h->precond;
+        pa.nx = h->nx; pa.ny = h->ny; pa.nz = h->nz; pa.P = w.P; pa.precond = h->precond; pa.periodic = h->periodic;
         pa.st = h->st; pa.partials = h->partials;
         void *kargs[] = {(void *)&pa};
         PB_CUDA(cudaLaunchCooperativeKernel((const void *)k_pcg_persistent<T>, dim3(w.pgrid), dim3(256), kargs, 0, h->stream));
@@ -589,7 +607,7 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     const long max_chunks = (long)maxiter / m + 2;
     int seen_done = w.persist ? 1 : 0;
     for (long c = 0; c < max_chunks + 1 && !seen_done; c++) {
-        if (graph_ok) { PB_CUDA(cudaGraphLaunch(w.graph, h->stream)); h->launches += 2LL * m; }
+        if (graph_ok) { PB_CUDA(cudaGraphLaunch(w.graph, h->stream)); h->launches += (2LL + (h->periodic ? 1 : 0)) * m; }
         else PB_TRY(enqueue_iterations<T>(h, w, m));
         int *slot = h->pinned + 4 * (c & 1);
         PB_CUDA(cudaMemcpyAsync(slot, &h->st->done, 4 * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
@@ -634,6 +652,7 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
     const int g = grid_for(w.npad, 256, kNumSM * 16);
     k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
     launch_spmv<T, 1>(h, w, 1.0 / (h->h * h->h));
+    launch_wrap<T, 1>(h, w, 1.0 / (h->h * h->h));
     k_unpad<T, T><<<g, 256, 0, h->stream>>>(w.Ap, dst, h->nx, w.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
     h->launches += 3;
@@ -678,6 +697,7 @@ pb_status profile_impl(pb_handle *h, int n_iter, double *ms_spmv, double *ms_vec
         PB_CUDA(cudaEventRecord(ev[0], h->stream));
         for (int it = 0; it < n_iter; it++) {
             launch_spmv<T, 0>(h, w, 1.0);
+            launch_wrap<T, 0>(h, w, 1.0);
             PB_CUDA(cudaEventRecord(ev[2 * it + 1], h->stream));
             k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
             PB_CUDA(cudaEventRecord(ev[2 * it + 2], h->stream));
@@ -835,6 +855,22 @@ pb_status pb_set_preconditioner(pb_handle *h, int kind)
         // captured graphs hold the kernel arguments by value
         if (h->wf.graph) { cudaGraphExecDestroy(h->wf.graph); h->wf.graph = nullptr; }
         if (h->wd.graph) { cudaGraphExecDestroy(h->wd.graph); h->wd.graph = nullptr; }
+    }
+    return PB_OK;
+}
+
+pb_status pb_set_boundary(pb_handle *h, int kind)
+{
+    if (!h || (kind != 0 && kind != 1)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    if (h->periodic != kind) {
+        h->periodic = kind;
+        if (h->wf.graph) { cudaGraphExecDestroy(h->wf.graph); h->wf.graph = nullptr; }
+        if (h->wd.graph) { cudaGraphExecDestroy(h->wd.graph); h->wd.graph = nullptr; }
+        h->wf.b_ready = false;           // b loses / regains the ghost fold-in
+        h->wd.b_ready = false;
+        if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));
+        if (h->wd.ready) PB_TRY(build_b<double>(h, h->wd));
     }
     return PB_OK;
 }

@@ -194,3 +194,97 @@ __global__ void k_finish(const T *__restrict__ x, const T *__restrict__ pbuf0, c
 }
 
 }  // namespace pb
+
+// ---------------------------------------------------------------------------------------
+// Periodic boundary condition.  k_spmv_tma computes A'p with p = 0 outside the
+// grid; under the periodic condition the neighbour across a box face is the node on the opposite side, so the
+// nodes of the boundary shell lack the terms  -eps_face * p(opposite node).  k_wrap adds them (one thread per
+// shell node, so every A'p entry has one writer), corrects p.Ap and recomputes alpha with the stopping checks of
+// the k_spmv_tma finaliser.  In a matrix-free kernel the paper's "6 extra bands" are just these index wraps.
+// ---------------------------------------------------------------------------------------
+namespace pb {
+
+template <typename T>
+struct WrapArgs {
+    const T *pbuf0, *pbuf1;   // MODE 0: p = buf[(l+1)&1] (what k_spmv_tma just wrote);  MODE 1: pbuf0 = the input vector
+    T *Ap;
+    const double *eps_x, *eps_y, *eps_z;   // dense fp64 inputs: only the outer faces f = 0 and f = n are read
+    int nx, ny, nz, P;
+    double out_scale;         // MODE 1
+    State *st;
+    double *partials;
+};
+
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) k_wrap(const WrapArgs<T> a)
+{
+    __shared__ double red[32];
+    __shared__ int s_last;
+    const T *p = a.pbuf0;
+    if (MODE == 0) {
+        if (a.st->done) return;
+        p = (a.st->iter_cur & 1) ? a.pbuf0 : a.pbuf1;
+    }
+    const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
+    // shell nodes, each owned once: the two z faces (full planes), then the y faces of the inner planes, then the x faces
+    const size_t n_z = (size_t)(nz > 1 ? 2 : 1) * ny * nx;
+    const int kin = nz > 2 ? nz - 2 : 0;                       // inner planes 1..nz-2
+    const size_t n_y = (size_t)kin * (ny > 1 ? 2 : 1) * nx;
+    const int jin = ny > 2 ? ny - 2 : 0;
+    const size_t n_x = (size_t)kin * jin * (nx > 1 ? 2 : 1);
+    const size_t total = n_z + n_y + n_x;
+    double acc = 0.0;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+        int i, j, k;
+        if (t < n_z) {
+            const size_t u = t % ((size_t)ny * nx);
+            k = (t < (size_t)ny * nx) ? 0 : nz - 1; j = (int)(u / nx); i = (int)(u % nx);
+        } else if (t < n_z + n_y) {
+            const size_t v = t - n_z, per_k = (size_t)(ny > 1 ? 2 : 1) * nx, u = v % per_k;
+            k = 1 + (int)(v / per_k); j = (u < (size_t)nx) ? 0 : ny - 1; i = (int)(u % nx);
+        } else {
+            const size_t v = t - n_z - n_y, per_j = (nx > 1 ? 2 : 1), per_k = (size_t)jin * per_j, u = v % per_k;
+            k = 1 + (int)(v / per_k); j = 1 + (int)(u / per_j); i = (u % per_j) ? nx - 1 : 0;
+        }
+        const size_t row = (size_t)k * ny + j, idx = row * P + i;
+        T d = T(0);                                            // the missing terms -eps_f * p(opposite)
+        if (i == 0)      d = fma(-(T)a.eps_x[row * (nx + 1)], p[row * P + nx - 1], d);
+        if (i == nx - 1) d = fma(-(T)a.eps_x[row * (nx + 1) + nx], p[row * P], d);
+        if (j == 0)      d = fma(-(T)a.eps_y[((size_t)k * (ny + 1)) * nx + i], p[((size_t)k * ny + ny - 1) * P + i], d);
+        if (j == ny - 1) d = fma(-(T)a.eps_y[((size_t)k * (ny + 1) + ny) * nx + i], p[((size_t)k * ny) * P + i], d);
+        if (k == 0)      d = fma(-(T)a.eps_z[(size_t)j * nx + i], p[((size_t)(nz - 1) * ny + j) * P + i], d);
+        if (k == nz - 1) d = fma(-(T)a.eps_z[((size_t)nz * ny + j) * nx + i], p[((size_t)j) * P + i], d);
+        if (MODE == 1) d = (T)((double)d * a.out_scale);
+        a.Ap[idx] += d;
+        if (MODE == 0) acc = fma((double)p[idx], (double)d, acc);
+    }
+    if (MODE == 0) {
+        const double tot = block_sum(acc, red);
+        const int nblk = gridDim.x;
+        if (threadIdx.x == 0) {
+            a.partials[blockIdx.x] = tot;
+            __threadfence();
+            const unsigned int t = atomicAdd(&a.st->ticket_spmv, 1u);
+            s_last = (t == (unsigned int)(nblk - 1));
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const double dp = final_sum(a.partials, nblk, red);
+            if (threadIdx.x == 0) {
+                State *st = a.st;
+                st->ticket_spmv = 0u;
+                const double pAp = st->pAp + dp;
+                st->pAp = pAp;
+                if (!(pAp > 0.0) || !isfinite(pAp)) {
+                    if (st->latch) { st->done = 1; st->iters = st->iter_cur; st->status = 5; }
+                    st->alpha = 0.0;
+                } else {
+                    st->alpha = st->rz / pAp;
+                }
+            }
+        }
+    }
+}
+
+}  // namespace pb

@@ -17,6 +17,7 @@ struct PersistArgs {
     const T *Dinv, *exm, *eym, *ezm;
     int nx, ny, nz, P;
     int precond;
+    int periodic;            // 1: neighbours wrap, 0: ghost p = 0
     State *st;
     double *partials;        // 3 regions of gridDim.x doubles: p.Ap | r.z | r.r
 };
@@ -46,7 +47,7 @@ __global__ void __launch_bounds__(256) k_pcg_persistent(const PersistArgs<T> a)
     const size_t nvec = (size_t)nz * ny * rowvecs;
     const size_t stride = (size_t)gridDim.x * blockDim.x, first = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int G = gridDim.x;
-    const bool precond = a.precond != 0;
+    const bool precond = a.precond != 0, per = a.periodic != 0;
 
     // every block carries the scalars of PAPER.md:106-126 in registers
     double rz = st->rz, rr = st->rr;
@@ -75,12 +76,14 @@ __global__ void __launch_bounds__(256) k_pcg_persistent(const PersistArgs<T> a)
             const int j = (int)(row % ny), k = (int)(row / ny), i0 = iv * VEC;
             const size_t idx = v * VEC;
             const Vec<T> pc = ldv(pout + idx);
-            const Vec<T> up = (j > 0) ? ldv(pout + idx - P) : zerov<T>();
-            const Vec<T> dn = (j < ny - 1) ? ldv(pout + idx + P) : zerov<T>();
-            const Vec<T> pm = (k > 0) ? ldv(pout + idx - (size_t)ny * P) : zerov<T>();
-            const Vec<T> pp = (k < nz - 1) ? ldv(pout + idx + (size_t)ny * P) : zerov<T>();
-            const T left = (i0 > 0) ? pout[idx - 1] : T(0);
+            const size_t rowbase = idx - i0, planebase = (size_t)k * ny * P, colbase = (size_t)j * P + i0;
+            const Vec<T> up = (j > 0) ? ldv(pout + idx - P) : (per ? ldv(pout + planebase + (size_t)(ny - 1) * P + i0) : zerov<T>());
+            const Vec<T> dn = (j < ny - 1) ? ldv(pout + idx + P) : (per ? ldv(pout + planebase + i0) : zerov<T>());
+            const Vec<T> pm = (k > 0) ? ldv(pout + idx - (size_t)ny * P) : (per ? ldv(pout + (size_t)(nz - 1) * ny * P + colbase) : zerov<T>());
+            const Vec<T> pp = (k < nz - 1) ? ldv(pout + idx + (size_t)ny * P) : (per ? ldv(pout + colbase) : zerov<T>());
+            const T left = (i0 > 0) ? pout[idx - 1] : (per ? pout[rowbase + nx - 1] : T(0));
             const T right = (i0 + VEC < P) ? pout[idx + VEC] : T(0);
+            const T wrap0 = per ? pout[rowbase] : T(0);       // right neighbour of node nx-1
             const Vec<T> dinv = ldv(a.Dinv + idx), ex = ldv(a.exm + idx);
             const T exr = (i0 + VEC < P) ? a.exm[idx + VEC] : T(0);
             const size_t yidx = ((size_t)k * (ny + 1) + j) * P + i0;
@@ -90,7 +93,8 @@ __global__ void __launch_bounds__(256) k_pcg_persistent(const PersistArgs<T> a)
 #pragma unroll
             for (int e = 0; e < VEC; e++) {
                 const T pl = (e == 0) ? left : pc.a[e == 0 ? 0 : e - 1];
-                const T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
+                T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
+                if (i0 + e == nx - 1) pr = wrap0;             // pad column (0) or, periodic, node 0 of the row
                 const T exh = (e == VEC - 1) ? exr : ex.a[e == VEC - 1 ? e : e + 1];
                 T s = rcp_rn(dinv.a[e]) * pc.a[e];            // D = 1/Dinv, as in k_spmv_tma
                 s = fma(-ex.a[e], pl, s);

@@ -439,3 +439,60 @@ def test_config5_headline_parity_full_size(pkg, pbref):
     print(f"config5: fp32 iters {g32['iters']} (oracle {o32['iters']}) err {e32:.2e} / {e32t:.2e}; "
           f"fp64 iters {g64['iters']} (oracle {o64['iters']}) err {e64:.2e}")
     assert e32 <= 1e-4 and e32t <= 1e-4 and e64 <= 1e-8
+
+
+def _periodic_inputs(shape, seed):
+    inp = random_operator(*shape, seed=seed)
+    inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]        # face f = n is face f = 0 under the periodic condition
+    inp.eps_y[:, -1, :] = inp.eps_y[:, 0, :]
+    inp.eps_z[-1] = inp.eps_z[0]
+    return inp
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (2, 3, 1), (13, 9, 7), (77, 45, 38), (130, 21, 37)])
+def test_periodic_boundary_spmv(pkg, pbref, shape):
+    """NEXT row f3: the paper's PBC variant -- index wraps instead of ghost zeros."""
+    nx, ny, nz = shape
+    inp = _periodic_inputs(shape, 31)
+    ref = pbref.from_inputs(inp)
+    ref.set_periodic(True)
+    x = np.random.default_rng(3).uniform(-1, 1, (nz, ny, nx))
+    with pkg.PBSolver(*inp.args()) as s:
+        y_dir = s.apply(x, "f64")
+        s.set_periodic(True)
+        y = s.apply(x, "f64")
+        y32 = s.apply(x.astype(np.float32), "f32")
+        s.set_periodic(False)
+        assert np.array_equal(s.apply(x, "f64"), y_dir)
+    yr = ref.apply(x)
+    bound = backward_bound(inp, x) + 1e-300
+    assert np.all(np.abs(y - yr) <= 1e-12 * bound * 2)
+    assert np.all(np.abs(y32 - yr) <= 2e-6 * bound)
+    ref.close()
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+@pytest.mark.parametrize("persist", ["1", "0"])
+def test_periodic_boundary_solve(pkg, pbref, prec, tol, persist):
+    inp = _periodic_inputs((45, 23, 19), 32)
+    ref = pbref.from_inputs(inp)
+    ref.set_periodic(True)
+    ref.set_rhs(inp.rhs, inp.bc)
+    o = ref.solve(tol, 5000)
+    ref.close()
+    saved = os.environ.pop("PB_PERSIST", None)
+    os.environ["PB_PERSIST"] = persist
+    try:
+        with pkg.PBSolver(*inp.args()) as s:
+            s.set_periodic(True)
+            assert np.allclose(s.b(), inp.rhs, rtol=1e-14)       # no ghost fold-in
+            g = s.solve(tol, 5000, prec, check_every=8)
+            g2 = s.solve(tol, 5000, prec, check_every=8)
+    finally:
+        os.environ.pop("PB_PERSIST", None)
+        if saved is not None:
+            os.environ["PB_PERSIST"] = saved
+    scale = np.max(np.abs(o["phi"]))
+    assert g["status"] == 0 and abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (g["iters"], o["iters"])
+    assert np.max(np.abs(g["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale
+    assert np.array_equal(g["phi"], g2["phi"])
