@@ -365,7 +365,9 @@ def run_ours(args, rank, local_rank, world):
     spmv_node = (WORDS_SPMV - 3) * elt + 3 if pal else WORDS_SPMV * elt
     spmv_bytes = spmv_node * n_node
     ach = spmv_bytes / (ms_spmv * 1e-3) / 1e9
-    vec_bytes = WORDS_VEC * elt * n_node
+    pald = solver.diag_palette_size()
+    vec_node = (WORDS_VEC - 1) * elt + 1 if pald else WORDS_VEC * elt     # Dinv as one index byte (diagonal palette)
+    vec_bytes = vec_node * n_node
     iter_bytes = spmv_bytes + vec_bytes
     ns_bytes = WORDS_NORTH_STAR * elt * n_node
     t_solve = ms_local * 1e-3
@@ -376,7 +378,7 @@ def run_ours(args, rank, local_rank, world):
                 "survey_10word": {"bytes_per_launch": WORDS_SPMV * elt * n_node,
                                   "GBs": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9},
                 "k_vec": {"achieved": vec_bytes / (ms_vec * 1e-3) / 1e9, "frac": vec_bytes / (ms_vec * 1e-3) / 1e9 / peak,
-                          "bytes_per_node": WORDS_VEC * elt, "ms_per_launch": ms_vec},
+                          "bytes_per_node": vec_node, "diag_palette_size": pald, "ms_per_launch": ms_vec},
                 "iteration": {"achieved": iter_bytes * iters / t_solve / 1e9,
                               "frac": iter_bytes * iters / t_solve / 1e9 / peak,
                               "north_star_16word_GBs": ns_bytes * iters / t_solve / 1e9,

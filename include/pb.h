@@ -175,6 +175,11 @@ long long pb_launch_count(pb_handle *h);
  * PB_PALETTE=0 in the environment disables the palette. */
 int pb_palette_size(pb_handle *h);
 
+/* Size of the diagonal palette: with a face palette and a few-valued salt map the Jacobi diagonal also takes <= 256
+ * distinct values, and k_vec then reads one index byte per node instead of a Dinv word (exact: the table holds
+ * (T)(1/d)); 0 = Dinv array.  PB_PALETTE_D=0 disables it. */
+int pb_diag_palette_size(pb_handle *h);
+
 /* pb_destroy(NULL) is a no-op.  Frees every device allocation of the handle. */
 pb_status pb_destroy(pb_handle *h);
 

@@ -19,7 +19,8 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary")
+           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
+           "pb_diag_palette_size")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -67,6 +68,7 @@ def load_library():
     lib.pb_set_charges.argtypes = [vp, vp, ci]
     lib.pb_get_field.argtypes = [vp, ci, vp]
     lib.pb_palette_size.argtypes = [vp]
+    lib.pb_diag_palette_size.argtypes = [vp]
     lib.pb_launch_count.restype = ctypes.c_longlong
     for name in EXPORTS:
         getattr(lib, name)
@@ -255,7 +257,8 @@ class PBSolver:
         st = load_library().pb_set_preconditioner(self._h, 1 if jacobi else 0)
         if st != PB_OK:
             raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary")
+           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
+           "pb_diag_palette_size")
 
     def set_periodic(self, periodic: bool):
         """False (default): Dirichlet ghost layer; True: periodic boundary condition."""
@@ -283,6 +286,9 @@ class PBSolver:
 
     def palette_size(self) -> int:
         return int(load_library().pb_palette_size(self._h))
+
+    def diag_palette_size(self) -> int:
+        return int(load_library().pb_diag_palette_size(self._h))
 
     def launch_count(self) -> int:
         return int(load_library().pb_launch_count(self._h))

@@ -40,6 +40,10 @@ struct Work {
     bool pal = false;
     unsigned char *exi = nullptr, *eyi = nullptr, *ezi = nullptr;
     T *lut = nullptr;
+    // diagonal palette for k_vec: index byte per node + Dinv table
+    bool pald = false;
+    unsigned char *dvi = nullptr;
+    T *dlut = nullptr;
     int Pb = 0;
 };
 
@@ -68,6 +72,8 @@ struct pb_handle {
     int precond;                 // 1 Jacobi (default), 0 none
     int periodic;                // 0 Dirichlet ghost layer (free-space condition, default), 1 periodic
     PalTable *pal_table;         // device; distinct face values of the operator
+    PalTable *pald_table;        // device; distinct diagonal values
+    int pald_n;                  // -1 unknown, 0 none, else table size
     int pal_n;                   // -1: not examined yet, 0: more than 256 distinct values, else the table size
     // pb_create_from_atoms keeps the atom geometry for pb_set_charges
     double *atoms_c;             // [n_atoms][3], device
@@ -141,6 +147,8 @@ void free_work(Work<T> &w)
     unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi};
     for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.lut) { cudaFree(w.lut); w.lut = nullptr; }
+    if (w.dvi) { cudaFree(w.dvi); w.dvi = nullptr; }
+    if (w.dlut) { cudaFree(w.dlut); w.dlut = nullptr; }
     w.ready = w.b_ready = false;
 }
 
@@ -192,7 +200,24 @@ pb_status ensure(pb_handle *h)
             h->launches += 5;
         }
     }
+    if (h->pald_n < 0) {
+        h->pald_n = 0;
+        if (h->pal_n > 0 && env_int("PB_PALETTE_D", 1)) {     // few face values -> few diagonals (unless kbar2 varies)
+            if (!h->pald_table) PB_ALLOC(cudaMalloc((void **)&h->pald_table, sizeof(PalTable)));
+            k_pal_reset<<<1, 256, 0, h->stream>>>(h->pald_table);
+            k_pal_collect_diag<<<grid_for((size_t)h->nx * h->ny * h->nz, 256, kNumSM * 8), 256, 0, h->stream>>>(
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, h->pald_table);
+            k_pal_finish<<<1, 256, 0, h->stream>>>(h->pald_table);
+            PB_CUDA(cudaGetLastError());
+            int n = 0;
+            PB_CUDA(cudaMemcpyAsync(&n, &h->pald_table->n, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            PB_CUDA(cudaStreamSynchronize(h->stream));
+            h->pald_n = n;
+            h->launches += 3;
+        }
+    }
     w.pal = h->pal_n > 0;
+    w.pald = h->pald_n > 0;
     w.Pb = (w.P + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
@@ -204,6 +229,10 @@ pb_status ensure(pb_handle *h)
     pb_status s = PB_OK;
     if (w.pal && w.persist &&
         ((s = alloc_arr(&w.exm, w.npad)) || (s = alloc_arr(&w.eym, n_ey)) || (s = alloc_arr(&w.ezm, n_ez)))) {
+        free_work(w);
+        return s;
+    }
+    if (w.pald && ((s = alloc_arr(&w.dvi, w.npad)) || (s = alloc_arr(&w.dlut, (size_t)kPalMax)))) {
         free_work(w);
         return s;
     }
@@ -250,6 +279,12 @@ pb_status ensure(pb_handle *h)
         k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
         h->launches += 2;
     }
+    if (w.pald) {
+        k_setup_diag_idx<<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
+            h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P, h->pald_table, w.dvi);
+        k_pal_lut_dinv<T><<<1, 256, 0, h->stream>>>(h->pald_table, w.dlut);
+        h->launches += 2;
+    }
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     PB_TRY(build_b<T>(h, w));
@@ -262,7 +297,7 @@ template <typename T>
 VecArgs<T> vec_args(pb_handle *h, Work<T> &w)
 {
     VecArgs<T> a;
-    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.l2hints = h->l2hints; a.precond = h->precond; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
+    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.l2hints = h->l2hints; a.precond = h->precond; a.dvi = w.dvi; a.dlut = w.dlut; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
     return a;
 }
 
@@ -519,7 +554,8 @@ pb_status enqueue_iterations(pb_handle *h, Work<T> &w, int n)
     for (int it = 0; it < n; it++) {
         launch_spmv<T, 0>(h, w, 1.0);
         launch_wrap<T, 0>(h, w, 1.0);
-        k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
+        if (w.pald) k_vec<T, true><<<w.vec_grid, 256, 0, h->stream>>>(va);
+        else k_vec<T, false><<<w.vec_grid, 256, 0, h->stream>>>(va);
     }
     PB_CUDA(cudaGetLastError());
     h->launches += 2LL * n;
@@ -699,7 +735,8 @@ pb_status profile_impl(pb_handle *h, int n_iter, double *ms_spmv, double *ms_vec
             launch_spmv<T, 0>(h, w, 1.0);
             launch_wrap<T, 0>(h, w, 1.0);
             PB_CUDA(cudaEventRecord(ev[2 * it + 1], h->stream));
-            k_vec<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
+            if (w.pald) k_vec<T, true><<<w.vec_grid, 256, 0, h->stream>>>(va);
+            else k_vec<T, false><<<w.vec_grid, 256, 0, h->stream>>>(va);
             PB_CUDA(cudaEventRecord(ev[2 * it + 2], h->stream));
         }
         PB_CUDA(cudaGetLastError());
@@ -740,6 +777,7 @@ pb_status pb_destroy(pb_handle *h)
     if (h->stage) cudaFree(h->stage);
     if (h->atoms_c) cudaFree(h->atoms_c);
     if (h->pal_table) cudaFree(h->pal_table);
+    if (h->pald_table) cudaFree(h->pald_table);
     if (h->pinned) cudaFreeHost(h->pinned);
     if (h->pinned_state) cudaFreeHost(h->pinned_state);
     for (int i = 0; i < 2; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
@@ -769,6 +807,7 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
     h->l2hints = env_int("PB_L2HINTS", 0);
     h->precond = 1;
     h->pal_n = -1;
+    h->pald_n = -1;
     pb_status s = PB_OK;
     auto body = [&]() -> pb_status {
         PB_CUDA(cudaGetDevice(&h->device));
@@ -902,6 +941,8 @@ pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spm
 long long pb_launch_count(pb_handle *h) { return h ? h->launches : 0; }
 
 int pb_palette_size(pb_handle *h) { return (h && h->pal_n > 0) ? h->pal_n : 0; }
+
+int pb_diag_palette_size(pb_handle *h) { return (h && h->pald_n > 0) ? h->pald_n : 0; }
 
 pb_status pb_query(pb_handle *h, int what, double *out_host)
 {

@@ -60,6 +60,8 @@ struct VecArgs {
     size_t nvec;              // number of 16-byte vectors in a padded node array
     int precond;              // 1: Jacobi (z = Dinv r), 0: M = I (z = r)
     int l2hints;              // 1: keep r and Dinv in L2 for the next k_spmv_tma, stream Ap
+    const unsigned char *dvi; // PALD: one index byte per node into dlut instead of the Dinv word (k_vec only)
+    const T *dlut;            // PALD: 256 values of Dinv
     State *st;
     double *partials;         // 2 per block
 };
@@ -92,31 +94,62 @@ __device__ __forceinline__ void reduce_and_finish(State *st, double *partials, d
 
 // 4 words per node: reads r, Ap, Dinv; writes r.  The sweep runs from the END of the arrays
 // towards the start: k_spmv_tma finishes at high z, so its last-written Ap lines are still in L2.
-template <typename T>
+template <typename T, bool PALD>
 __global__ void __launch_bounds__(256) k_vec(const VecArgs<T> a)
 {
     constexpr int VEC = VecN<T>::value;
     __shared__ double red[32];
     __shared__ int s_last;
+    __shared__ T dlut[PALD ? 256 : 1];
     if (a.st->done) return;
+    if (PALD) {
+        for (int i = threadIdx.x; i < 256; i += blockDim.x) dlut[i] = a.dlut[i];
+        __syncthreads();
+    }
     const T alpha = (T)a.st->alpha;
     const uint64_t pol_keep = l2_policy((a.l2hints & 1) ? 2 : 0), pol_stream = l2_policy((a.l2hints & 2) ? 1 : 0);
     double s_rz = 0.0, s_rr = 0.0;
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < a.nvec; v += stride) {
-        const size_t idx = (a.nvec - 1 - v) * VEC;
-        Vec<T> rv, qv, dv;
-        ld16_hint(rv.a, a.r + idx, pol_keep);
-        ld16_hint(qv.a, a.Ap + idx, pol_stream);
-        ld16_hint(dv.a, a.Dinv + idx, pol_keep);
+    // two vectors per thread and pass (both fully coalesced across the warp): all loads are issued before the first
+    // use, which is what keeps enough bytes in flight when a vector is only two fp64 nodes
+    const size_t chunk = 2 * (size_t)blockDim.x, stride = (size_t)gridDim.x * chunk;
+    for (size_t v0 = (size_t)blockIdx.x * chunk + threadIdx.x; v0 < a.nvec; v0 += stride) {
+        const size_t v1 = v0 + blockDim.x;
+        const bool two = v1 < a.nvec;
+        const size_t idx0 = (a.nvec - 1 - v0) * VEC, idx1 = two ? (a.nvec - 1 - v1) * VEC : idx0;
+        Vec<T> r0, q0, d0, r1, q1, d1;
+        ld16_hint(r0.a, a.r + idx0, pol_keep);
+        ld16_hint(q0.a, a.Ap + idx0, pol_stream);
+        ld16_hint(r1.a, a.r + idx1, pol_keep);
+        ld16_hint(q1.a, a.Ap + idx1, pol_stream);
+        if (PALD) {
+            const uint32_t w0 = (VEC == 4) ? *reinterpret_cast<const uint32_t *>(a.dvi + idx0)
+                                           : (uint32_t)*reinterpret_cast<const unsigned short *>(a.dvi + idx0);
+            const uint32_t w1 = (VEC == 4) ? *reinterpret_cast<const uint32_t *>(a.dvi + idx1)
+                                           : (uint32_t)*reinterpret_cast<const unsigned short *>(a.dvi + idx1);
+#pragma unroll
+            for (int e = 0; e < VEC; e++) { d0.a[e] = dlut[(w0 >> (8 * e)) & 255u]; d1.a[e] = dlut[(w1 >> (8 * e)) & 255u]; }
+        } else {
+            ld16_hint(d0.a, a.Dinv + idx0, pol_keep);
+            ld16_hint(d1.a, a.Dinv + idx1, pol_keep);
+        }
 #pragma unroll
         for (int e = 0; e < VEC; e++) {
-            rv.a[e] = fma(-alpha, qv.a[e], rv.a[e]);      // r_l = r_{l-1} - alpha A p     (step 5)
-            const T zv = a.precond ? dv.a[e] * rv.a[e] : rv.a[e];   // M z_l = r_l, M = D or I   (step 6)
-            s_rz = fma((double)rv.a[e], (double)zv, s_rz);
-            s_rr = fma((double)rv.a[e], (double)rv.a[e], s_rr);
+            r0.a[e] = fma(-alpha, q0.a[e], r0.a[e]);      // r_l = r_{l-1} - alpha A p     (step 5)
+            const T zv = a.precond ? d0.a[e] * r0.a[e] : r0.a[e];   // M z_l = r_l, M = D or I   (step 6)
+            s_rz = fma((double)r0.a[e], (double)zv, s_rz);
+            s_rr = fma((double)r0.a[e], (double)r0.a[e], s_rr);
         }
-        st16_hint(a.r + idx, rv.a, pol_keep);
+        st16_hint(a.r + idx0, r0.a, pol_keep);
+        if (two) {
+#pragma unroll
+            for (int e = 0; e < VEC; e++) {
+                r1.a[e] = fma(-alpha, q1.a[e], r1.a[e]);
+                const T zv = a.precond ? d1.a[e] * r1.a[e] : r1.a[e];
+                s_rz = fma((double)r1.a[e], (double)zv, s_rz);
+                s_rr = fma((double)r1.a[e], (double)r1.a[e], s_rr);
+            }
+            st16_hint(a.r + idx1, r1.a, pol_keep);
+        }
     }
     reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, 0);
 }

@@ -230,3 +230,64 @@ __global__ void k_pal_lut(const PalTable *t, T *lut)
 }
 
 }  // namespace pb
+
+// ---------------------------------------------------------------------------------------
+// Diagonal palette.  With palette-able face dielectrics and a two-valued salt map the Jacobi diagonal
+// D' = sum of six face eps + h^2 kbar2 also takes few distinct values (56 at most for three face values), so k_vec
+// can read one index byte per node instead of a Dinv word.  The table holds the fp64 diagonals; the lookup table
+// in precision T is (T)(1/d), bit-identical to the Dinv array k_setup_coeff writes.
+// ---------------------------------------------------------------------------------------
+namespace pb {
+
+__device__ __forceinline__ double diag_of(const double *eps_x, const double *eps_y, const double *eps_z,
+                                          const double *kbar2, double h2, int nx, int ny, int i, int j, int k)
+{
+    const size_t row = (size_t)k * ny + j;
+    double d = eps_x[row * (nx + 1) + i] + eps_x[row * (nx + 1) + i + 1]
+             + eps_y[((size_t)k * (ny + 1) + j) * nx + i] + eps_y[((size_t)k * (ny + 1) + j + 1) * nx + i]
+             + eps_z[row * nx + i] + eps_z[((size_t)(k + 1) * ny + j) * nx + i];
+    if (kbar2) d += h2 * kbar2[row * nx + i];
+    return d;
+}
+
+__global__ void k_pal_collect_diag(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
+                                   const double *__restrict__ eps_z, const double *__restrict__ kbar2, double h2,
+                                   int nx, int ny, int nz, PalTable *t)
+{
+    volatile int *ovf = &t->overflow;
+    if (*ovf) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) pal_insert(t, 1.0);                   // the pad value
+    const size_t n = (size_t)nx * ny * nz;
+    double prev = -1.0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(q % nx), j = (int)((q / nx) % ny), k = (int)(q / ((size_t)nx * ny));
+        const double d = diag_of(eps_x, eps_y, eps_z, kbar2, h2, nx, ny, i, j, k);
+        if (d == prev) continue;
+        prev = d;
+        pal_insert(t, d);
+        if (*ovf) return;
+    }
+}
+
+// byte index of D per padded node ([nz][ny][P], pad = index of 1.0)
+__global__ void k_setup_diag_idx(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
+                                 const double *__restrict__ eps_z, const double *__restrict__ kbar2, double h2,
+                                 int nx, int ny, int nz, int P, const PalTable *t, unsigned char *dvi)
+{
+    const unsigned char one = pal_index(t, 1.0);
+    const size_t total = (size_t)nz * ny * P;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(q % P);
+        const size_t row = q / P;
+        const int j = (int)(row % ny), k = (int)(row / ny);
+        dvi[q] = (i < nx) ? pal_index(t, diag_of(eps_x, eps_y, eps_z, kbar2, h2, nx, ny, i, j, k)) : one;
+    }
+}
+
+template <typename T>
+__global__ void k_pal_lut_dinv(const PalTable *t, T *lut)
+{
+    for (int i = threadIdx.x; i < kPalMax; i += blockDim.x) lut[i] = (i < t->n) ? (T)(1.0 / t->vals[i]) : T(1);
+}
+
+}  // namespace pb

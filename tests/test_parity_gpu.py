@@ -496,3 +496,29 @@ def test_periodic_boundary_solve(pkg, pbref, prec, tol, persist):
     assert g["status"] == 0 and abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (g["iters"], o["iters"])
     assert np.max(np.abs(g["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale
     assert np.array_equal(g["phi"], g2["phi"])
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_diagonal_palette_is_exact(pkg, prec, tol):
+    """k_vec reading Dinv through the diagonal palette (index byte + table of (T)(1/d)) must reproduce the Dinv-array
+    run bit for bit; an operator whose salt map varies from node to node must fall back to the array."""
+    inp = make_config(2)
+    saved = {k: os.environ.pop(k, None) for k in ("PB_PALETTE_D", "PB_PERSIST")}
+    os.environ["PB_PERSIST"] = "0"                 # the two-kernel path is the one that uses k_vec
+    try:
+        with pkg.PBSolver(*inp.args()) as s:
+            assert 0 < s.diag_palette_size() <= 56
+            a = s.solve(tol, 5000, prec)
+        os.environ["PB_PALETTE_D"] = "0"
+        with pkg.PBSolver(*inp.args()) as s:
+            assert s.diag_palette_size() == 0
+            b = s.solve(tol, 5000, prec)
+        many = random_operator(21, 9, 8, seed=6, two_valued=True, salted=True)    # kbar2 ~ U[0,2] per node
+        with pkg.PBSolver(*many.args()) as s:
+            assert s.palette_size() > 0 and s.diag_palette_size() == 0
+    finally:
+        for k, v in saved.items():
+            os.environ.pop(k, None)
+            if v is not None:
+                os.environ[k] = v
+    assert a["iters"] == b["iters"] and np.array_equal(a["phi"], b["phi"])
