@@ -92,7 +92,8 @@ pb_status pb_apply(pb_handle *h, pb_precision prec, const void *x, void *y, pb_m
  *   check_every the host reads the 8-byte on-device {done, iters} latch once per this many
  *               iterations (>= 1); there is no other host<->device traffic during the solve.
  *               The returned iterate is exactly the one at which the test first passed,
- *               whatever check_every is.
+ *               whatever check_every is.  (Grids whose working set fits the L2 run the whole loop in
+ *               one cooperative kernel and are not polled at all.)
  *   phi_out     [nz][ny][nx] in `prec`, caller-allocated, host or device per `where`.
  *   iters_out   l at exit = number of A*p products (may be NULL).
  *   relres_out  ||r_l||/||b|| at exit (may be NULL).
