@@ -522,3 +522,48 @@ def test_diagonal_palette_is_exact(pkg, prec, tol):
             if v is not None:
                 os.environ[k] = v
     assert a["iters"] == b["iters"] and np.array_equal(a["phi"], b["phi"])
+
+
+def test_randomised_shapes_and_options(pkg, pbref):
+    """Seeded sweep over odd shapes and every switch (periodic / Dirichlet, Jacobi / M = I, palette or not, persistent
+    or two-kernel path, fp32 / fp64, warm start): SpMV within the componentwise bound, solves within the north-star
+    tolerances of the oracle run with the same options."""
+    rng = np.random.default_rng(20260704)
+    saved = os.environ.pop("PB_PERSIST", None)
+    try:
+        for case in range(24):
+            nx, ny, nz = (int(v) for v in rng.integers(1, 41, 3))
+            periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), bool(rng.integers(2))
+            persist, prec = str(int(rng.integers(2))), ("f64", "f32")[int(rng.integers(2))]
+            inp = _periodic_inputs((nx, ny, nz), 100 + case) if periodic else random_operator(nx, ny, nz, seed=100 + case)
+            if not two_valued:
+                inp.eps_x[...] = rng.uniform(1, 80, inp.eps_x.shape)
+                if periodic:
+                    inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
+            tol = 1e-10 if prec == "f64" else 1e-5
+            ref = pbref.from_inputs(inp)
+            ref.set_periodic(periodic)
+            ref.set_rhs(inp.rhs, inp.bc)
+            o = ref.solve(tol, 4000, precond=jacobi)
+            x = rng.uniform(-1, 1, (nz, ny, nx))
+            yr = ref.apply(x)
+            os.environ["PB_PERSIST"] = persist
+            with pkg.PBSolver(*inp.args()) as s:
+                s.set_periodic(periodic)
+                s.set_preconditioner(jacobi)
+                y = s.apply(x.astype(np.float64 if prec == "f64" else np.float32), prec)
+                g = s.solve(tol, 4000, prec, check_every=int(rng.integers(1, 40)))
+                w = s.solve(tol, 4000, prec, phi0=g["phi"].copy())
+            ref.close()
+            tag = (case, nx, ny, nz, periodic, jacobi, two_valued, persist, prec)
+            bound = backward_bound(inp, x) + 1e-300
+            assert np.all(np.abs(y - yr) <= (2e-12 if prec == "f64" else 2e-6) * bound), tag
+            assert g["status"] == o["status"] == 0, tag
+            assert abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), tag + (g["iters"], o["iters"])
+            scale = np.max(np.abs(o["phi"])) + 1e-300
+            assert np.max(np.abs(g["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale, tag
+            assert w["iters"] <= 1, tag
+    finally:
+        os.environ.pop("PB_PERSIST", None)
+        if saved is not None:
+            os.environ["PB_PERSIST"] = saved
