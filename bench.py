@@ -177,7 +177,7 @@ def run_reference(args, rank, world):
         dev = "cpu"
     inp, rhs, bc = build_inputs(args.config, 0, 1, dev)
     n_node = inp.n
-    sample = args.cpu_sample_iters or max(2, min(200, int(3.0e8 / n_node)))
+    sample = args.cpu_sample_iters or max(2, min(200, int(1.2e9 / n_node)))
     ref = pbref.from_inputs(inp)
     for _ in range(args.warmup):
         ref.solve(tol, min(sample, 2))
