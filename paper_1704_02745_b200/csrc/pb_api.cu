@@ -542,7 +542,7 @@ void launch_wrap(pb_handle *h, Work<T> &w, double out_scale)
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P; a.out_scale = out_scale;
     a.st = h->st; a.partials = h->partials;
     const size_t shell = 2 * ((size_t)h->ny * h->nx + (size_t)h->nz * h->nx + (size_t)h->nz * h->ny);
-    k_wrap<T, MODE><<<grid_for(shell, 256, kNumSM * 2), 256, 0, h->stream>>>(a);
+    k_wrap<T, MODE><<<grid_for(shell, 256, kNumSM * 8), 256, 0, h->stream>>>(a);
     h->launches += 1;
 }
 
