@@ -503,8 +503,9 @@ def test_diagonal_palette_is_exact(pkg, prec, tol):
     """k_vec reading Dinv through the diagonal palette (index byte + table of (T)(1/d)) must reproduce the Dinv-array
     run bit for bit; an operator whose salt map varies from node to node must fall back to the array."""
     inp = make_config(2)
-    saved = {k: os.environ.pop(k, None) for k in ("PB_PALETTE_D", "PB_PERSIST")}
+    saved = {k: os.environ.pop(k, None) for k in ("PB_PALETTE_D", "PB_PERSIST", "PB_AUTOTUNE")}
     os.environ["PB_PERSIST"] = "0"                 # the two-kernel path is the one that uses k_vec
+    os.environ["PB_AUTOTUNE"] = "0"                # same static plan in both handles: same reduction order
     try:
         with pkg.PBSolver(*inp.args()) as s:
             assert 0 < s.diag_palette_size() <= 56
