@@ -17,6 +17,9 @@
  * and return a pb_status.  There is no global state.  One handle = one operator on one
  * device and one CUDA stream.  A handle is not thread-safe; distinct handles are independent.
  * There is NO CPU fallback: without a CUDA device every compute call returns PB_ERR_CUDA.
+ * Determinism: every reduction has a fixed order for a fixed launch plan, so repeated solves on one handle are
+ * bit-identical.  pb_create picks the SpMV plan by timing candidates (like an FFT plan), so two handles for the same
+ * operator may differ in the last bits of the dot products; PB_AUTOTUNE=0 in the environment pins a static plan.
  *
  * Array layouts (all caller arrays are dense C arrays of fp64 unless stated otherwise):
  *   eps_x [nz][ny][nx+1]  face f lies between node i=f-1 and node i=f; the paper's
