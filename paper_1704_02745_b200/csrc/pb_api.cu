@@ -34,7 +34,7 @@ struct Work {
     size_t qsmem = 0;
     CUtensorMap tm_r, tm_tmp, tm_dinv, tm_p0, tm_p1, tm_x, tm_ex, tm_ey, tm_ez;
     // L2-resident grids: the whole loop as one cooperative kernel (pb_persist.cuh)
-    bool persist = false;
+    bool persist = false, pfused = false;
     int pgrid = 0;
     // coefficient palette (pb_setup.cuh): byte face indices + table, instead of exm/eym/ezm
     bool pal = false;
@@ -253,8 +253,11 @@ pb_status ensure(pb_handle *h)
     }
     w.vec_grid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * env_int("PB_VEC_BPS", 8));
     if (w.persist) {
+        // tiny grids: barriers dominate -> the two-barrier form that recomputes p at the neighbours
+        w.pfused = (double)w.npad <= (double)env_int("PB_PERSIST_FUSED_MAX_KNODES", 600) * 1.0e3;
         int bps = 0;
-        PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T>, 256, 0));
+        if (w.pfused) PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T, true>, 256, 0));
+        else PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T, false>, 256, 0));
         if (bps < 1) w.persist = false;
         bps = bps > env_int("PB_PERSIST_BPS", 4) ? env_int("PB_PERSIST_BPS", 4) : bps;
         w.pgrid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * bps);
@@ -635,7 +638,8 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
         pa.nx = h->nx; pa.ny = h->ny; pa.nz = h->nz; pa.P = w.P; pa.precond = h->precond; pa.periodic = h->periodic;
         pa.st = h->st; pa.partials = h->partials;
         void *kargs[] = {(void *)&pa};
-        PB_CUDA(cudaLaunchCooperativeKernel((const void *)k_pcg_persistent<T>, dim3(w.pgrid), dim3(256), kargs, 0, h->stream));
+        const void *fn = w.pfused ? (const void *)k_pcg_persistent<T, true> : (const void *)k_pcg_persistent<T, false>;
+        PB_CUDA(cudaLaunchCooperativeKernel(fn, dim3(w.pgrid), dim3(256), kargs, 0, h->stream));
         h->launches += 1;
     }
     bool graph_ok = !w.persist && h->use_graph && get_graph<T>(h, w, m) == PB_OK;

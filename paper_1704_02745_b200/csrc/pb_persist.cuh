@@ -33,8 +33,11 @@ __device__ __forceinline__ double all_sum(const double *partials, int n, double 
     return v;
 }
 
-template <typename T>
-__global__ void __launch_bounds__(256) k_pcg_persistent(const PersistArgs<T> a)
+// FUSED: p = z + beta p is recomputed at the centre and its six neighbours inside the stencil pass (21 instead of 7
+// L1/L2-resident loads) instead of in a pass of its own: two grid barriers per iteration instead of three, which is
+// what counts on grids so small that the barriers dominate.
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(256, FUSED ? 2 : 3) k_pcg_persistent(const PersistArgs<T> a)
 {
     namespace cg = cooperative_groups;
     constexpr int VEC = VecN<T>::value;
@@ -57,17 +60,24 @@ __global__ void __launch_bounds__(256) k_pcg_persistent(const PersistArgs<T> a)
     T beta = T(0);
     T *pin = a.p0, *pout = a.p1;              // k_init cleared p0
 
-    while (!done) {
-        // step 6-7: z = Dinv r (or r), p = z + beta p
-        for (size_t v = first; v < nvec; v += stride) {
-            const size_t idx = v * VEC;
-            const Vec<T> rv = ldv(a.r + idx), dv = ldv(a.Dinv + idx), po = ldv(pin + idx);
-            Vec<T> pn;
+    // p_new = z + beta p_old at an arbitrary vector / scalar position (steps 6-7)
+    auto pnew_v = [&](const T *pin_, size_t idx) -> Vec<T> {
+        const Vec<T> rv = ldv(a.r + idx), dv = ldv(a.Dinv + idx), po = ldv(pin_ + idx);
+        Vec<T> pn;
 #pragma unroll
-            for (int e = 0; e < VEC; e++) pn.a[e] = fma(beta, po.a[e], precond ? dv.a[e] * rv.a[e] : rv.a[e]);
-            stv(pout + idx, pn);
+        for (int e = 0; e < VEC; e++) pn.a[e] = fma(beta, po.a[e], precond ? dv.a[e] * rv.a[e] : rv.a[e]);
+        return pn;
+    };
+    auto pnew_s = [&](const T *pin_, size_t idx) -> T {
+        return fma(beta, pin_[idx], precond ? a.Dinv[idx] * a.r[idx] : a.r[idx]);
+    };
+
+    while (!done) {
+        if (!FUSED) {
+            // step 6-7: z = Dinv r (or r), p = z + beta p
+            for (size_t v = first; v < nvec; v += stride) stv(pout + v * VEC, pnew_v(pin, v * VEC));
+            grid.sync();
         }
-        grid.sync();
         // step 5a: Ap = A'p from the face dielectrics (ghost p = 0), partial p.Ap
         double acc = 0.0;
         for (size_t v = first; v < nvec; v += stride) {
@@ -75,15 +85,19 @@ __global__ void __launch_bounds__(256) k_pcg_persistent(const PersistArgs<T> a)
             const size_t row = v / rowvecs;
             const int j = (int)(row % ny), k = (int)(row / ny), i0 = iv * VEC;
             const size_t idx = v * VEC;
-            const Vec<T> pc = ldv(pout + idx);
+            // neighbour values of p: read back (three-barrier form) or recomputed from r, Dinv, p_old (FUSED)
+            auto PV = [&](size_t at) -> Vec<T> { return FUSED ? pnew_v(pin, at) : ldv(pout + at); };
+            auto PS = [&](size_t at) -> T { return FUSED ? pnew_s(pin, at) : pout[at]; };
+            const Vec<T> pc = PV(idx);
+            if (FUSED) stv(pout + idx, pc);
             const size_t rowbase = idx - i0, planebase = (size_t)k * ny * P, colbase = (size_t)j * P + i0;
-            const Vec<T> up = (j > 0) ? ldv(pout + idx - P) : (per ? ldv(pout + planebase + (size_t)(ny - 1) * P + i0) : zerov<T>());
-            const Vec<T> dn = (j < ny - 1) ? ldv(pout + idx + P) : (per ? ldv(pout + planebase + i0) : zerov<T>());
-            const Vec<T> pm = (k > 0) ? ldv(pout + idx - (size_t)ny * P) : (per ? ldv(pout + (size_t)(nz - 1) * ny * P + colbase) : zerov<T>());
-            const Vec<T> pp = (k < nz - 1) ? ldv(pout + idx + (size_t)ny * P) : (per ? ldv(pout + colbase) : zerov<T>());
-            const T left = (i0 > 0) ? pout[idx - 1] : (per ? pout[rowbase + nx - 1] : T(0));
-            const T right = (i0 + VEC < P) ? pout[idx + VEC] : T(0);
-            const T wrap0 = per ? pout[rowbase] : T(0);       // right neighbour of node nx-1
+            const Vec<T> up = (j > 0) ? PV(idx - P) : (per ? PV(planebase + (size_t)(ny - 1) * P + i0) : zerov<T>());
+            const Vec<T> dn = (j < ny - 1) ? PV(idx + P) : (per ? PV(planebase + i0) : zerov<T>());
+            const Vec<T> pm = (k > 0) ? PV(idx - (size_t)ny * P) : (per ? PV((size_t)(nz - 1) * ny * P + colbase) : zerov<T>());
+            const Vec<T> pp = (k < nz - 1) ? PV(idx + (size_t)ny * P) : (per ? PV(colbase) : zerov<T>());
+            const T left = (i0 > 0) ? PS(idx - 1) : (per ? PS(rowbase + nx - 1) : T(0));
+            const T right = (i0 + VEC < P) ? PS(idx + VEC) : T(0);
+            const T wrap0 = per ? PS(rowbase) : T(0);         // right neighbour of node nx-1
             const Vec<T> dinv = ldv(a.Dinv + idx), ex = ldv(a.exm + idx);
             const T exr = (i0 + VEC < P) ? a.exm[idx + VEC] : T(0);
             const size_t yidx = ((size_t)k * (ny + 1) + j) * P + i0;
