@@ -165,6 +165,7 @@ pb_status build_b(pb_handle *h, Work<T> &w)
 }
 
 template <typename T> pb_status setup_tma(pb_handle *h, Work<T> &w);
+template <typename T> pb_status tune_vec(pb_handle *h, Work<T> &w);
 pb_status ensure_stage(pb_handle *h, size_t bytes);
 
 // Lazily build the arrays of precision T (setup row a0).
@@ -251,7 +252,7 @@ pb_status ensure(pb_handle *h)
         free_work(w);
         return s;
     }
-    w.vec_grid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * env_int("PB_VEC_BPS", 8));
+    w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, kNumSM * env_int("PB_VEC_BPS", 4));   // 2 vectors per thread and pass
     if (w.persist) {
         // tiny grids: barriers dominate -> the two-barrier form that recomputes p at the neighbours
         w.pfused = (double)w.npad <= (double)env_int("PB_PERSIST_FUSED_MAX_KNODES", 600) * 1.0e3;
@@ -262,7 +263,7 @@ pb_status ensure(pb_handle *h)
         bps = bps > env_int("PB_PERSIST_BPS", 4) ? env_int("PB_PERSIST_BPS", 4) : bps;
         w.pgrid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * bps);
     }
-    size_t need = (size_t)kNumSM * 8 > (size_t)2 * w.vec_grid ? (size_t)kNumSM * 8 : (size_t)2 * w.vec_grid;
+    size_t need = (size_t)kNumSM * 16 > (size_t)2 * w.vec_grid ? (size_t)kNumSM * 16 : (size_t)2 * w.vec_grid;
     if ((size_t)3 * w.pgrid > need) need = (size_t)3 * w.pgrid;
     if (need > h->partials_cap) {
         if (h->partials) cudaFree(h->partials);
@@ -292,6 +293,7 @@ pb_status ensure(pb_handle *h)
     h->launches += 1;
     PB_TRY(build_b<T>(h, w));
     PB_TRY(setup_tma<T>(h, w));
+    PB_TRY(tune_vec<T>(h, w));
     w.ready = true;
     return PB_OK;
 }
@@ -532,6 +534,48 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     else
         k_spmv_tma<T, MODE, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
             MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
+}
+
+// k_vec is a plain stream, but its rate depends measurably on how many blocks share an SM (DRAM page / bank
+// interleaving of the concurrent streams): time 3-8 blocks per SM once per handle, like the SpMV plan.
+template <typename T>
+pb_status tune_vec(pb_handle *h, Work<T> &w)
+{
+    if (getenv("PB_VEC_BPS") || env_int("PB_AUTOTUNE", 1) == 0 || (double)h->nx * h->ny * h->nz < 2.0e6) return PB_OK;
+    cudaEvent_t e0, e1;
+    PB_CUDA(cudaEventCreate(&e0));
+    PB_CUDA(cudaEventCreate(&e1));
+    PB_CUDA(cudaMemsetAsync(w.r, 0, w.npad * sizeof(T), h->stream));
+    PB_CUDA(cudaMemsetAsync(w.Ap, 0, w.npad * sizeof(T), h->stream));
+    k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
+    static const int cand[] = {3, 4, 5, 6, 8};
+    float tbest = 1e30f;
+    int best = w.vec_grid;
+    for (int c : cand) {
+        w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, kNumSM * c);
+        if ((size_t)2 * w.vec_grid > h->partials_cap) continue;
+        const VecArgs<T> va = vec_args<T>(h, w);
+        auto launch = [&]() {
+            if (w.pald) k_vec<T, true><<<w.vec_grid, 256, 0, h->stream>>>(va);
+            else k_vec<T, false><<<w.vec_grid, 256, 0, h->stream>>>(va);
+        };
+        launch();
+        cudaEventRecord(e0, h->stream);
+        for (int rep = 0; rep < 3; rep++) launch();
+        cudaEventRecord(e1, h->stream);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+            cudaEventDestroy(e0); cudaEventDestroy(e1);
+            return PB_ERR_CUDA;
+        }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (getenv("PB_VERBOSE")) fprintf(stderr, "pb: tune k_vec %d blocks/SM (grid %d): %.4f ms\n", c, w.vec_grid, ms / 3);
+        if (ms < tbest) { tbest = ms; best = w.vec_grid; }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    w.vec_grid = best;
+    return PB_OK;
 }
 
 // periodic boundary condition: the wrap terms k_spmv_tma cannot see (k_wrap), right after it
