@@ -147,6 +147,14 @@ pb_status pb_get_field(pb_handle *h, int which, double *out_host);
 pb_status pb_set_preconditioner(pb_handle *h, int kind);
 
 /*
+ * pb_residual -- the TRUE relative residual ||b - A phi||_2 / ||b||_2 of a caller-supplied potential ([nz][ny][nx] in
+ * `prec`), evaluated with the SpMV kernel in that precision and fp64 sums.  pb_solve tests and returns the recurrence
+ * residual (DESIGN.md Reading 5); with fp32 storage the true residual stagnates near 1e-6..1e-5 while
+ * the recurrence keeps falling, which is what this call makes visible.
+ */
+pb_status pb_residual(pb_handle *h, pb_precision prec, const void *phi, pb_memspace where, double *relres_out);
+
+/*
  * pb_set_boundary -- kind 0 (default): the free-space condition, Dirichlet values on the ghost layer; kind 1: the
  * periodic boundary condition the paper also times.  Periodic: the neighbour across
  * a box face is the node on the opposite side; face f = 0 and face f = n of a direction are one physical face (the

@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size")
+           "pb_diag_palette_size", "pb_residual")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -64,6 +64,7 @@ def load_library():
     lib.pb_launch_count.argtypes = [vp]
     lib.pb_set_preconditioner.argtypes = [vp, ci]
     lib.pb_set_boundary.argtypes = [vp, ci]
+    lib.pb_residual.argtypes = [vp, ci, vp, ci, ctypes.POINTER(cd)]
     lib.pb_create_from_atoms.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, ci, vp, vp, vp, cd, cd, cd, ci, vp]
     lib.pb_set_charges.argtypes = [vp, vp, ci]
     lib.pb_get_field.argtypes = [vp, ci, vp]
@@ -258,13 +259,26 @@ class PBSolver:
         if st != PB_OK:
             raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size")
+           "pb_diag_palette_size", "pb_residual")
 
     def set_periodic(self, periodic: bool):
         """False (default): Dirichlet ghost layer; True: periodic boundary condition."""
         st = load_library().pb_set_boundary(self._h, 1 if periodic else 0)
         if st != PB_OK:
             raise PBError(st, "pb_set_boundary")
+
+    def residual(self, phi, precision=None):
+        """True relative residual ||b - A phi|| / ||b|| of `phi` (numpy or CUDA tensor), pb_residual."""
+        if precision is None:
+            precision = PB_F32 if str(phi.dtype).endswith("float32") else PB_F64
+        pc, dt = _prec(precision)
+        pp, sp, keep = _marshal(phi, dt, self.nx * self.ny * self.nz, "phi")
+        out = ctypes.c_double(0.0)
+        st = load_library().pb_residual(self._h, pc, pp, sp, ctypes.byref(out))
+        del keep
+        if st != PB_OK:
+            raise PBError(st, "pb_residual")
+        return out.value
 
     def solve_begin(self, precision):
         st = load_library().pb_solve_begin(self._h, _prec(precision)[0])

@@ -746,6 +746,34 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
     return PB_OK;
 }
 
+// true residual ||b - A phi|| / ||b|| of a caller-supplied potential, in the arithmetic of precision T
+template <typename T>
+pb_status residual_impl(pb_handle *h, const void *phi, pb_memspace where, double *relres_out)
+{
+    PB_TRY(ensure<T>(h));
+    Work<T> &w = work<T>(h);
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    const T *src = (const T *)phi;
+    if (where == PB_HOST) {
+        PB_TRY(ensure_stage(h, n * sizeof(T)));
+        PB_CUDA(cudaMemcpyAsync(h->stage, phi, n * sizeof(T), cudaMemcpyHostToDevice, h->stream));
+        src = (const T *)h->stage;
+    }
+    k_pad<T, T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
+    launch_spmv<T, 1>(h, w, 1.0);
+    launch_wrap<T, 1>(h, w, 1.0);
+    k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
+    k_true_residual<T><<<grid_for(w.npad / VecN<T>::value, 256, kNumSM * 4), 256, 0, h->stream>>>(
+        w.b, w.Ap, w.npad / VecN<T>::value, h->st, h->partials);
+    PB_CUDA(cudaGetLastError());
+    h->launches += 4;
+    PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    const State &st = *h->pinned_state;
+    *relres_out = (st.bb > 0.0) ? sqrt(st.rr / st.bb) : 0.0;
+    return PB_OK;
+}
+
 // copy a caller array (host or device) into a fresh/existing device array of n doubles
 pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_memspace where)
 {
@@ -932,6 +960,14 @@ pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec
     return prec == PB_F32
                ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out, phi0)
                : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out, phi0);
+}
+
+pb_status pb_residual(pb_handle *h, pb_precision prec, const void *phi, pb_memspace where, double *relres_out)
+{
+    if (!h || !phi || !relres_out || !valid_prec(prec) || !valid_space(where)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? residual_impl<float>(h, phi, where, relres_out)
+                          : residual_impl<double>(h, phi, where, relres_out);
 }
 
 pb_status pb_set_preconditioner(pb_handle *h, int kind)

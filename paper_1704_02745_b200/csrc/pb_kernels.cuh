@@ -320,4 +320,39 @@ __global__ void __launch_bounds__(256) k_wrap(const WrapArgs<T> a)
     }
 }
 
+// ||b - A'phi||^2 and ||b||^2 (A'phi in Ap): the TRUE residual of a given potential, as opposed to the recurrence
+// residual the iteration tests (DESIGN.md Reading 5).  Same two-stage deterministic reduction; result in st->rr, st->bb.
+template <typename T>
+__global__ void __launch_bounds__(256) k_true_residual(const T *__restrict__ b, const T *__restrict__ Ap, size_t nvec,
+                                                       State *st, double *partials)
+{
+    constexpr int VEC = VecN<T>::value;
+    __shared__ double red[32];
+    __shared__ int s_last;
+    double s_rr = 0.0, s_bb = 0.0;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += (size_t)gridDim.x * blockDim.x) {
+        const Vec<T> bv = ldv(b + v * VEC), qv = ldv(Ap + v * VEC);
+#pragma unroll
+        for (int e = 0; e < VEC; e++) {
+            const double d = (double)bv.a[e] - (double)qv.a[e];
+            s_rr = fma(d, d, s_rr);
+            s_bb = fma((double)bv.a[e], (double)bv.a[e], s_bb);
+        }
+    }
+    const double t_rr = block_sum(s_rr, red), t_bb = block_sum(s_bb, red);
+    const int nblk = gridDim.x;
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = t_rr;
+        partials[nblk + blockIdx.x] = t_bb;
+        __threadfence();
+        s_last = (atomicAdd(&st->ticket_vec, 1u) == (unsigned int)(nblk - 1));
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        const double rr = final_sum(partials, nblk, red), bb = final_sum(partials + nblk, nblk, red);
+        if (threadIdx.x == 0) { st->ticket_vec = 0u; st->rr = rr; st->bb = bb; }
+    }
+}
+
 }  // namespace pb

@@ -568,3 +568,22 @@ def test_randomised_shapes_and_options(pkg, pbref):
         os.environ.pop("PB_PERSIST", None)
         if saved is not None:
             os.environ["PB_PERSIST"] = saved
+
+
+def test_true_residual_matches_oracle(pkg, pbref):
+    """pb_residual = ||b - A phi|| / ||b|| against the oracle's recomputed residual (Reading 5), and the fp32 story of
+    SURVEY hard part 4: the recurrence residual passes 1e-7 while the true residual of the fp32 iterate stagnates."""
+    inp = make_config(2)
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(1e-6, 5000)
+    b = ref.b()
+    with pkg.PBSolver(*inp.args()) as s:
+        assert abs(s.residual(o["phi"], "f64") - o["true_relres"]) <= 1e-6 * o["true_relres"]
+        assert s.residual(np.zeros_like(o["phi"]), "f64") == 1.0
+        g = s.solve(1e-7, 5000, "f32")
+        t32 = s.residual(g["phi"], "f32")
+        t64 = s.residual(g["phi"].astype(np.float64), "f64")
+    true = np.linalg.norm(b - ref.apply(g["phi"].astype(np.float64))) / np.linalg.norm(b)
+    ref.close()
+    assert g["relres"] < 1e-7 < true                      # fp32 storage: recurrence below, truth above
+    assert abs(t64 - true) <= 1e-6 * true and abs(t32 - true) <= 0.2 * true
