@@ -362,11 +362,12 @@ def run_ours(args, rank, local_rank, world):
     # + 3 index bytes (the three face arrays are stored losslessly as one byte per face).  ncu's DRAM byte count
     # (`traffic`) is compared with exactly this number.  The same time charged with SURVEY's uncompressed 10 words is
     # given under `survey_10word` for reference (it exceeds the copy peak because fewer bytes are really moved).
-    spmv_node = (WORDS_SPMV - 3) * elt + 3 if pal else WORDS_SPMV * elt
+    # ... and 6 words + 4 index bytes when the Jacobi diagonal too fits a palette (pb_bytes_per_node reports the format).
+    spmv_node = solver.bytes_per_node(prec, 0)
     spmv_bytes = spmv_node * n_node
     ach = spmv_bytes / (ms_spmv * 1e-3) / 1e9
     pald = solver.diag_palette_size()
-    vec_node = (WORDS_VEC - 1) * elt + 1 if pald else WORDS_VEC * elt     # Dinv as one index byte (diagonal palette)
+    vec_node = solver.bytes_per_node(prec, 1)       # Dinv as one index byte with the diagonal palette
     vec_bytes = vec_node * n_node
     iter_bytes = spmv_bytes + vec_bytes
     ns_bytes = WORDS_NORTH_STAR * elt * n_node

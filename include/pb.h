@@ -192,6 +192,14 @@ int pb_palette_size(pb_handle *h);
  * (T)(1/d)); 0 = Dinv array.  PB_PALETTE_D=0 disables it. */
 int pb_diag_palette_size(pb_handle *h);
 
+/* Bytes per grid node and launch that kernel `kernel` (0: k_spmv_tma, the PCG step; 1: k_vec) has to move in the
+ * storage format this handle uses for `prec` -- the algorithmic bytes of bench.py's roofline:
+ * k_spmv_tma reads r, p, x and writes p, x, Ap (6 words) plus Dinv (a word, or one index byte with the diagonal
+ * palette; PB_PALETTE_DS=0 keeps the word) plus the three face coefficients (3 words, or 3 index bytes with the
+ * palette); k_vec reads r, Ap, writes r (3 words) plus Dinv (word or byte).  Builds the work arrays of `prec` if
+ * they do not exist yet; -1 on error. */
+int pb_bytes_per_node(pb_handle *h, pb_precision prec, int kernel);
+
 /* pb_destroy(NULL) is a no-op.  Frees every device allocation of the handle. */
 pb_status pb_destroy(pb_handle *h);
 

@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size", "pb_residual")
+           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -64,6 +64,8 @@ def load_library():
     lib.pb_launch_count.argtypes = [vp]
     lib.pb_set_preconditioner.argtypes = [vp, ci]
     lib.pb_set_boundary.argtypes = [vp, ci]
+    lib.pb_bytes_per_node.argtypes = [vp, ci, ci]
+    lib.pb_bytes_per_node.restype = ci
     lib.pb_residual.argtypes = [vp, ci, vp, ci, ctypes.POINTER(cd)]
     lib.pb_create_from_atoms.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, ci, vp, vp, vp, cd, cd, cd, ci, vp]
     lib.pb_set_charges.argtypes = [vp, vp, ci]
@@ -259,7 +261,7 @@ class PBSolver:
         if st != PB_OK:
             raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size", "pb_residual")
+           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node")
 
     def set_periodic(self, periodic: bool):
         """False (default): Dirichlet ghost layer; True: periodic boundary condition."""
@@ -279,6 +281,14 @@ class PBSolver:
         if st != PB_OK:
             raise PBError(st, "pb_residual")
         return out.value
+
+    def bytes_per_node(self, precision, kernel):
+        """Bytes per node and launch of kernel 0 (k_spmv_tma) / 1 (k_vec) in this handle's storage format."""
+        pc, _ = _prec(precision)
+        n = load_library().pb_bytes_per_node(self._h, pc, int(kernel))
+        if n < 0:
+            raise PBError(PB_ERR_CUDA, "pb_bytes_per_node")
+        return n
 
     def solve_begin(self, precision):
         st = load_library().pb_solve_begin(self._h, _prec(precision)[0])

@@ -43,6 +43,9 @@ struct Work {
     // diagonal palette for k_vec: index byte per node + Dinv table
     bool pald = false;
     unsigned char *dvi = nullptr;
+    size_t qmaxdyn = 224 * 1024;     // dynamic shared memory the chosen k_spmv_tma variant may use
+    unsigned char *dvib = nullptr;   // the same indices in rows of Pb bytes (TMA strides are multiples of 16)
+    bool pald_s = false;             // k_spmv_tma reads Dinv through the index tensor too
     T *dlut = nullptr;
     int Pb = 0;
 };
@@ -148,6 +151,7 @@ void free_work(Work<T> &w)
     for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.lut) { cudaFree(w.lut); w.lut = nullptr; }
     if (w.dvi) { cudaFree(w.dvi); w.dvi = nullptr; }
+    if (w.dvib) { cudaFree(w.dvib); w.dvib = nullptr; }
     if (w.dlut) { cudaFree(w.dlut); w.dlut = nullptr; }
     w.ready = w.b_ready = false;
 }
@@ -219,6 +223,7 @@ pb_status ensure(pb_handle *h)
     }
     w.pal = h->pal_n > 0;
     w.pald = h->pald_n > 0;
+    w.pald_s = w.pald && w.pal && env_int("PB_PALETTE_DS", 1) != 0;
     w.Pb = (w.P + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
@@ -237,6 +242,7 @@ pb_status ensure(pb_handle *h)
         free_work(w);
         return s;
     }
+    if (w.pald_s && (s = alloc_arr(&w.dvib, (size_t)h->nz * h->ny * w.Pb))) { free_work(w); return s; }
     if (w.pal) {
         const size_t b_ex = (size_t)h->nz * h->ny * w.Pb, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pb,
                      b_ez = (size_t)(h->nz + 1) * h->ny * w.Pb;
@@ -288,6 +294,11 @@ pb_status ensure(pb_handle *h)
             h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P, h->pald_table, w.dvi);
         k_pal_lut_dinv<T><<<1, 256, 0, h->stream>>>(h->pald_table, w.dlut);
         h->launches += 2;
+        if (w.pald_s) {
+            k_setup_diag_idx<<<grid_for((size_t)h->nz * h->ny * w.Pb, 256, kNumSM * 16), 256, 0, h->stream>>>(
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, h->pald_table, w.dvib);
+            h->launches += 1;
+        }
     }
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
@@ -375,9 +386,9 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qntx = (rowvecs + TXV - 1) / TXV;
     w.qnty = (h->ny + TY - 1) / TY;
     w.qthreads = (TXV * TY + 31) / 32 * 32 + 32;
-    const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0);
+    const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0, w.pald_s);
     w.qsmem = (size_t)NS * L.slot + 128;
-    if (w.qsmem > 224 * 1024 || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
+    if (w.qsmem > w.qmaxdyn || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
     const int slots = kNumSM * c.bps;
     const int xy = w.qntx * w.qnty;
     int TZ = c.TZ;
@@ -394,7 +405,8 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qgrid = (int)(ntiles < slots ? ntiles : slots);
     PB_TRY(make_map<T>(&w.tm_r, w.r, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_tmp, w.tmp, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
-    PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    if (w.pald_s) PB_TRY(make_map_u8(&w.tm_dinv, w.dvib, w.Pb, h->ny, h->nz, L.bwd, TY + 2));
+    else PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_x, w.x, w.P, h->ny, h->nz, TXV * VEC, TY));
@@ -413,10 +425,11 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
 template <typename T, int MODE> void launch_spmv(pb_handle *h, Work<T> &w, double out_scale);
 
 // deepest ring (<= 6 slots) that lets `bps` blocks of this tile share one SM's shared memory
-inline int ring_depth(int TXV, int TY, int bps, int pal_vec)
+inline int ring_depth(int TXV, int TY, int bps, int pal_vec, bool pald)
 {
-    const size_t per_block = (size_t)232448 / bps - 1024 - 3200;   // 227 KB per SM, 1 KB reserved per block, statics
-    int NS = (int)(per_block / slot_layout(TXV, TY, pal_vec).slot);
+    // 227 KB per SM, 1 KB reserved per block, statics (barriers, reduction scratch, up to three 256-entry tables)
+    const size_t per_block = (size_t)232448 / bps - 1024 - 3200 - (pald ? 2 * 256 * (16 / pal_vec) : 0);
+    int NS = (int)(per_block / slot_layout(TXV, TY, pal_vec, pald).slot);
     return NS > 6 ? 6 : NS;
 }
 
@@ -429,12 +442,22 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
 {
     constexpr int VEC = VecN<T>::value;
     const int rowvecs = w.P / VEC;
-    const int maxv = 256 / VEC - 2;                                  // box inner dimension <= 256 elements
-    const int max_dyn = 224 * 1024;
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
-    PB_CUDA(cudaFuncSetAttribute(k_spmv_tma<T, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+    // box inner dimension <= 256 elements (byte-index boxes: the haloed row plus 16 bytes of lead-in)
+    const int maxv = (w.pal ? 240 : 256) / VEC - 2;
+    // dynamic + static shared memory <= 227 KB per block; the static part depends on the variant (its tables)
+    auto allow = [&](auto kernel, size_t *max_dyn) -> pb_status {
+        cudaFuncAttributes fa;
+        PB_CUDA(cudaFuncGetAttributes(&fa, kernel));
+        const size_t lim = (size_t)232448 - fa.sharedSizeBytes;
+        PB_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim));
+        if (max_dyn) *max_dyn = lim;
+        return PB_OK;
+    };
+    size_t lim0 = 0, lim1 = 0;
+    if (w.pald_s) { PB_TRY(allow(k_spmv_tma<T, 0, true, true>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, true>, &lim1)); }
+    else if (w.pal) { PB_TRY(allow(k_spmv_tma<T, 0, true, false>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, false>, &lim1)); }
+    else { PB_TRY(allow(k_spmv_tma<T, 0, false, false>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, false, false>, &lim1)); }
+    w.qmaxdyn = lim0 < lim1 ? lim0 : lim1;
     int ntx0 = (rowvecs + 32) / 64;                                  // rows of about 64 vectors (1 KB)
     if (ntx0 < 1) ntx0 = 1;
     while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
@@ -451,9 +474,9 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         if (c.TY < 1) c.TY = 1;
         if (c.TY > h->ny) c.TY = h->ny;
         while (c.TXV * c.TY > 448 && c.TY > 1) c.TY--;
-        c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0) >= 4 ? 2 : 1);
+        c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s) >= 4 ? 2 : 1);
         if (c.bps < 1) c.bps = 1;
-        c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0));
+        c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s));
         c.TZ = env_int("PB_TZ", 0);
         cand[nc++] = c;
     } else {
@@ -466,7 +489,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
                 int TY = ty > h->ny ? h->ny : ty;
                 if (TXV * TY > 448) continue;
                 for (int bps = 1; bps <= 4; bps++) {
-                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0);
+                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0, w.pald_s);
                     if (NS < 4 && !(NS == 3 && bps >= 2)) continue;
                     const int cthreads = ((TXV * TY + 31) / 32 * 32) * bps;
                     if (cthreads < 256 || cthreads > 1024) continue;     // consumer threads per SM
@@ -511,8 +534,8 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     }
     PB_TRY(configure_tma<T>(h, w, cand[best]));
     if (getenv("PB_VERBOSE"))
-        fprintf(stderr, "pb: palette %d; k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
-                h->pal_n, sizeof(T) == 4 ? "f32" : "f64", w.qTXV, w.qTY, w.qTZ, w.qns, cand[best].bps,
+        fprintf(stderr, "pb: palette %d (diagonal %d); k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
+                h->pal_n, w.pald_s ? h->pald_n : 0, sizeof(T) == 4 ? "f32" : "f64", w.qTXV, w.qTY, w.qTZ, w.qns, cand[best].bps,
                 w.qntx * w.qnty * w.qntz, w.qgrid, w.qthreads, w.qsmem, tune ? " (autotuned)" : "");
     return PB_OK;
 }
@@ -527,12 +550,15 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
     a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->l2hints; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
-    a.lut = w.lut;
-    if (w.pal)
-        k_spmv_tma<T, MODE, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+    a.lut = w.lut; a.dlut = w.dlut;
+    if (w.pald_s)
+        k_spmv_tma<T, MODE, true, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+            MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
+    else if (w.pal)
+        k_spmv_tma<T, MODE, true, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
             MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
     else
-        k_spmv_tma<T, MODE, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+        k_spmv_tma<T, MODE, false, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
             MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
 }
 
@@ -744,6 +770,17 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
         PB_CUDA(cudaMemcpyAsync(y, dst, n * sizeof(T), cudaMemcpyDeviceToHost, h->stream));
     PB_CUDA(cudaStreamSynchronize(h->stream));
     return PB_OK;
+}
+
+template <typename T>
+int bytes_per_node_impl(pb_handle *h, int kernel)
+{
+    if (ensure<T>(h) != PB_OK) return -1;
+    const Work<T> &w = work<T>(h);
+    const int e = (int)sizeof(T);
+    if (kernel == 0)      // r, p_old, x in; p, x, Ap out; Dinv; three face coefficients
+        return 6 * e + (w.pald_s ? 1 : e) + (w.pal ? 3 : 3 * e);
+    return 3 * e + (w.pald ? 1 : e);      // r, Ap in; r out; Dinv
 }
 
 // true residual ||b - A phi|| / ||b|| of a caller-supplied potential, in the arithmetic of precision T
@@ -1025,6 +1062,13 @@ pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spm
 long long pb_launch_count(pb_handle *h) { return h ? h->launches : 0; }
 
 int pb_palette_size(pb_handle *h) { return (h && h->pal_n > 0) ? h->pal_n : 0; }
+
+int pb_bytes_per_node(pb_handle *h, pb_precision prec, int kernel)
+{
+    if (!h || !valid_prec(prec) || kernel < 0 || kernel > 1) return -1;
+    if (cudaSetDevice(h->device) != cudaSuccess) return -1;
+    return prec == PB_F32 ? bytes_per_node_impl<float>(h, kernel) : bytes_per_node_impl<double>(h, kernel);
+}
 
 int pb_diag_palette_size(pb_handle *h) { return (h && h->pald_n > 0) ? h->pald_n : 0; }
 

@@ -42,6 +42,7 @@ struct TmaArgs {
     double *partials;        // one per block
     double out_scale;        // MODE 1 only
     const T *lut;            // PAL only: palette values (256 entries)
+    const T *dlut;           // PALD only: the distinct values of Dinv (256 entries)
 };
 
 __host__ __device__ inline size_t align128(size_t v) { return (v + 127) & ~(size_t)127; }
@@ -49,15 +50,19 @@ __host__ __device__ inline size_t align128(size_t v) { return (v + 127) & ~(size
 // byte sizes of the boxes of one item (also the smem carve-up of a ring slot).  With a coefficient
 // palette the three face boxes hold one byte per face, rows of `bw` bytes (a multiple of 16 for the TMA).
 struct SlotLayout {
-    size_t szZ, szD, szEX, szEY, szEZ, slot;
+    size_t szZ, szD, szEX, szEY, szEZ, szDv, slot;
     size_t oR, oDv, oPp, oEZ, oX, oEX, oEY;   // offsets of the boxes inside a slot
-    uint32_t bZ, bD, bEX, bEY, bEZ;           // exact box bytes (what the TMA delivers)
+    uint32_t bZ, bD, bEX, bEY, bEZ, bDv;      // exact box bytes (what the TMA delivers)
     int bw;                                   // palette only: bytes per row of a face-index box
+    int bwd;                                  // diagonal palette only: bytes per row of the haloed Dinv-index box
 };
-__host__ __device__ inline SlotLayout slot_layout(int TXV, int TY, int pal_vec /* 0: no palette, else VEC */) {
+__host__ __device__ inline SlotLayout slot_layout(int TXV, int TY, int pal_vec /* 0: no palette, else VEC */,
+                                                  bool pald = false) {
     SlotLayout L;
     L.bZ = (uint32_t)(TY + 2) * (TXV + 2) * 16;
     L.bD = (uint32_t)TY * TXV * 16;
+    L.bwd = pald ? ((TXV + 2) * pal_vec + 16 + 15) / 16 * 16 : 0;
+    L.bDv = pald ? (uint32_t)(TY + 2) * L.bwd : L.bZ;
     if (pal_vec) {
         L.bw = (TXV * pal_vec + 16 + 15) / 16 * 16;   // box starts at x0 rounded down to 16 B: up to 16-VEC bytes of lead-in
         L.bEX = (uint32_t)TY * L.bw; L.bEY = (uint32_t)(TY + 1) * L.bw; L.bEZ = (uint32_t)TY * L.bw;
@@ -66,16 +71,18 @@ __host__ __device__ inline SlotLayout slot_layout(int TXV, int TY, int pal_vec /
         L.bEX = (uint32_t)TY * (TXV + 1) * 16; L.bEY = (uint32_t)(TY + 1) * TXV * 16; L.bEZ = L.bD;
     }
     L.szZ = align128(L.bZ); L.szD = align128(L.bD); L.szEX = align128(L.bEX);
-    L.szEY = align128(L.bEY); L.szEZ = align128(L.bEZ);
-    L.oR = 0; L.oDv = L.szZ; L.oPp = 2 * L.szZ;
-    L.oEZ = 3 * L.szZ; L.oX = L.oEZ + L.szEZ; L.oEX = L.oX + L.szD; L.oEY = L.oEX + L.szEX;
+    L.szEY = align128(L.bEY); L.szEZ = align128(L.bEZ); L.szDv = align128(L.bDv);
+    L.oR = 0; L.oDv = L.szZ; L.oPp = L.oDv + L.szDv;
+    L.oEZ = L.oPp + L.szZ; L.oX = L.oEZ + L.szEZ; L.oEX = L.oX + L.szD; L.oEY = L.oEX + L.szEX;
     L.slot = L.oEY + L.szEY;
     return L;
 }
 
 // MODE 0: PCG step;  MODE 1: y = out_scale * A' v  (v behind tm_r; no Dinv scaling, no p_old, no x, no dot)
 // PAL: the eps_x/eps_y/eps_z maps are byte-index tensors decoded through the 256-entry table a.lut
-template <typename T, int MODE, bool PAL>
+// PALD (with PAL): Dinv too is a byte-index tensor (haloed box), decoded through a.dlut; D = 1/Dinv from a second
+// table built at kernel start with the same correctly rounded reciprocal
+template <typename T, int MODE, bool PAL, bool PALD>
 __global__ void __launch_bounds__(512)
 k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_dinv,
            const __grid_constant__ CUtensorMap tm_p0, const __grid_constant__ CUtensorMap tm_p1,
@@ -90,6 +97,8 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     __shared__ double red[32];
     __shared__ int s_last;
     __shared__ T lut[PAL ? 256 : 1];
+    __shared__ T lutDinv[PALD ? 256 : 1];
+    __shared__ T lutD[PALD ? 256 : 1];
 
     const int tid = threadIdx.x;
     const int nthr = blockDim.x;
@@ -111,7 +120,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     }
     const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
     const int TXV = a.TXV, TY = a.TY, TZ = a.TZ, NS = a.nstage;
-    const SlotLayout L = slot_layout(TXV, TY, PAL ? VEC : 0);
+    const SlotLayout L = slot_layout(TXV, TY, PAL ? VEC : 0, PALD);
     // 128-byte aligned ring base; plain pointer arithmetic on the __shared__ symbol keeps the address space known
     // to the compiler (LDS/STS instead of generic LD/ST)
     unsigned char *base = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
@@ -122,6 +131,8 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
     }
     if (PAL)
         for (int i = tid; i < 256; i += nthr) lut[i] = a.lut[i];
+    if (PALD)
+        for (int i = tid; i < 256; i += nthr) { const T d = a.dlut[i]; lutDinv[i] = d; lutD[i] = rcp_rn(d); }
     __syncthreads();
 
     double acc = 0.0;
@@ -143,16 +154,17 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                     unsigned char *slot = base + s * (uint32_t)L.slot;
                     const bool centre = (q >= k0) && (q < k1);   // q is a plane this tile writes
                     const bool ez = (q >= k0);
-                    uint32_t bytes = L.bZ * (MODE == 0 ? 3 : 1);
+                    uint32_t bytes = (MODE == 0) ? 2 * L.bZ + L.bDv : L.bZ;
                     if (ez) bytes += L.bEZ;
-                    if (centre) bytes += L.bEX + L.bEY + (MODE == 0 ? L.bD : L.bZ);
+                    if (centre) bytes += L.bEX + L.bEY + (MODE == 0 ? L.bD : L.bDv);
+                    const int xd = PALD ? ((x0 - VEC) & ~15) : x0 - VEC;   // byte-index box: 16-byte aligned start
                     mbar_expect_tx(&full_bar[s], bytes);
                     tma_load_3d_hint(slot + L.oR, &tm_r, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
                     if (MODE == 0) {
-                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
+                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, xd, j0 - 1, q, &full_bar[s], pol_keep);
                         tma_load_3d_hint(slot + L.oPp, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s], pol_pold);
                     } else if (centre) {
-                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
+                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, xd, j0 - 1, q, &full_bar[s], pol_keep);
                     }
                     const int xc = PAL ? (x0 & ~15) : x0;      // byte-index boxes start 16-byte aligned
                     if (ez) tma_load_3d_hint(slot + L.oEZ, &tm_ez, xc, j0, q, &full_bar[s], pol_stream);
@@ -170,6 +182,8 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         const int tx = tid % TXV, ty = tid / TXV;
         const bool intile = ty < TY;
         const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
+        const int own_d = (ty + 1) * L.bwd + (tx + 1) * VEC;   // PALD: its byte offset in the Dinv-index box
+        int lead_d = 0;                                // PALD: bytes between that box's aligned start and x0 - VEC
         const int cown = ty * TXV + tx;                // own cell in the x / ezm / eym boxes
         const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
         const bool precond = a.precond != 0;
@@ -183,13 +197,25 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             return (r + 1) * BWc + (side ? TXV + 1 : 0);
         };
         const int extra0 = (NCT - 1 - tid < nextra) ? halo_cell(NCT - 1 - tid) : -1;   // this thread's halo cell
+        auto cell_d = [&](int c) -> int { const int row = c / BWc; return row * L.bwd + (c - row * BWc) * VEC; };
+        const int extra0_d = (PALD && extra0 >= 0) ? cell_d(extra0) : 0;
+        // VEC values of a 256-entry table selected by the VEC index bytes at p
+        auto decode = [&](const T *table, const unsigned char *p) -> Vec<T> {
+            const uint32_t w = (VEC == 4) ? *reinterpret_cast<const uint32_t *>(p)
+                                          : (uint32_t)*reinterpret_cast<const unsigned short *>(p);
+            Vec<T> v;
+#pragma unroll
+            for (int e = 0; e < VEC; e++) v.a[e] = table[(w >> (8 * e)) & 255u];
+            return v;
+        };
         // p_new = Dinv*r + beta*p_old (steps 6-7) in place in the r box; returns the own cell's p_new
-        auto pnew_cell = [&](Vec<T> *R, const Vec<T> *Dv, const Vec<T> *Pp, int c) -> Vec<T> {
+        auto pnew_cell = [&](Vec<T> *R, const Vec<T> *Dv, const Vec<T> *Pp, int c, int cd) -> Vec<T> {
             Vec<T> v = R[c];
             if (MODE == 0) {
                 const Vec<T> pv = Pp[c];
                 if (precond) {
-                    const Vec<T> dv = Dv[c];
+                    const Vec<T> dv = PALD ? decode(lutDinv, reinterpret_cast<const unsigned char *>(Dv) + lead_d + cd)
+                                           : Dv[c];
 #pragma unroll
                     for (int e = 0; e < VEC; e++) v.a[e] = fma(beta, pv.a[e], dv.a[e] * v.a[e]);
                 } else {
@@ -205,14 +231,14 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             const Vec<T> *Pp = reinterpret_cast<const Vec<T> *>(slot + L.oPp);
             Vec<T> v = zerov<T>();
             if (intile) {
-                v = pnew_cell(R, Dv, Pp, own);
+                v = pnew_cell(R, Dv, Pp, own, own_d);
                 if (MODE == 0 && with_halo) R[own] = v;
             }
             if (MODE == 0 && with_halo) {
-                if (extra0 >= 0) R[extra0] = pnew_cell(R, Dv, Pp, extra0);
+                if (extra0 >= 0) R[extra0] = pnew_cell(R, Dv, Pp, extra0, extra0_d);
                 for (int h = NCT - 1 - tid + NCT; h < nextra; h += NCT) {      // only when the halo outnumbers the threads
                     const int c = halo_cell(h);
-                    R[c] = pnew_cell(R, Dv, Pp, c);
+                    R[c] = pnew_cell(R, Dv, Pp, c, PALD ? cell_d(c) : 0);
                 }
             }
             return v;
@@ -256,6 +282,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
             const int nvalid = nx - i0;
             const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
             lead = x0 & 15;
+            lead_d = (x0 - VEC) & 15;
 
             // item k0-1: only the own column's value is needed
             mbar_wait(&full_bar[rs], rp);
@@ -282,7 +309,15 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                     const Vec<T> *Zk = reinterpret_cast<const Vec<T> *>(slotk + L.oR);     // p_new(k) box
                     const Vec<T> up = Zk[own - BWc], dn = Zk[own + BWc];
                     const T left = Zk[own - 1].a[VEC - 1], right = Zk[own + 1].a[0];
-                    const Vec<T> dinv = reinterpret_cast<const Vec<T> *>(slotk + L.oDv)[own];
+                    // D = 1/Dinv (correctly rounded): the diagonal of Eq. 3
+                    Vec<T> D;
+                    if (PALD) {
+                        D = decode(lutD, slotk + L.oDv + lead_d + own_d);
+                    } else {
+                        const Vec<T> dinv = reinterpret_cast<const Vec<T> *>(slotk + L.oDv)[own];
+#pragma unroll
+                        for (int e = 0; e < VEC; e++) D.a[e] = rcp_rn(dinv.a[e]);
+                    }
                     const Vec<T> ex = coef(slotk + L.oEX, ty, TXV + 1);
                     const T exr = PAL ? lut[slotk[L.oEX + ty * L.bw + lead + tx * VEC + VEC]]
                                       : reinterpret_cast<const Vec<T> *>(slotk + L.oEX)[ty * (TXV + 1) + tx + 1].a[0];
@@ -294,7 +329,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                         const T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
                         const T exh = (e == VEC - 1) ? exr : ex.a[e == VEC - 1 ? e : e + 1];
                         // two short FMA chains instead of one of seven (latency), summed at the end
-                        T v = rcp_rn(dinv.a[e]) * pc.a[e];        // D = 1/Dinv (correctly rounded): the diagonal of Eq. 3
+                        T v = D.a[e] * pc.a[e];
                         v = fma(-ex.a[e], pl, v);
                         v = fma(-exh, pr, v);
                         v = fma(-eyl.a[e], up.a[e], v);
