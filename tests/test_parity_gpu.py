@@ -291,6 +291,46 @@ def test_tiling_independence(pkg, pbref, prec):
     ref.close()
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_tiling_independence_with_both_palettes(pkg, prec):
+    """k_spmv_tma with the face palette AND Dinv read through the diagonal palette (haloed byte box, every lead-in
+    0/4/8/12 of the 16-byte aligned box start under the forced tilings): the SpMV and one PCG step's vectors must be
+    bit-identical across tilings and identical to the word formats (PB_PALETTE_DS=0, PB_PALETTE=0)."""
+    inp = random_operator(77, 45, 38, seed=33, salted=False, two_valued=True)      # kbar2 = 0: few distinct diagonals
+    dt = np.float64 if prec == "f64" else np.float32
+    x = np.random.default_rng(5).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(dt)
+    keys = TILE_ENV + ("PB_PALETTE_DS", "PB_PALETTE")
+    saved = {k: os.environ.pop(k, None) for k in keys}
+    try:
+        ref_y = ref_p = ref_ap = None
+        for fmt in (dict(), dict(PB_PALETTE_DS=0), dict(PB_PALETTE=0)):
+            for cfg in TILE_CONFIGS:
+                for k in keys:
+                    os.environ.pop(k, None)
+                os.environ.update({k: str(v) for k, v in {**cfg, **fmt}.items()})
+                os.environ["PB_PERSIST"] = "0"
+                with pkg.PBSolver(*inp.args()) as s:
+                    if not fmt:
+                        assert s.palette_size() > 0 and s.diag_palette_size() > 0
+                        assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
+                    y = s.apply(x, prec)
+                    s.solve_begin(prec)
+                    s.iterate(prec, 2)
+                    p2, ap2 = s.vector("p"), s.vector("Ap")
+                if ref_y is None:
+                    ref_y, ref_p, ref_ap = y, p2, ap2
+                assert np.array_equal(y, ref_y), (fmt, cfg)
+                # p and Ap after two iterations: alpha/beta come from tiling-dependent summation orders, so compare
+                # to rounding, not bitwise
+                eps = 1e-5 if prec == "f32" else 1e-13
+                assert np.max(np.abs(p2 - ref_p)) <= eps * np.max(np.abs(ref_p)), (fmt, cfg)
+                assert np.max(np.abs(ap2 - ref_ap)) <= eps * np.max(np.abs(ref_ap)), (fmt, cfg)
+    finally:
+        for k in keys:
+            os.environ.pop(k, None)
+        os.environ.update({k: v for k, v in saved.items() if v is not None})
+
+
 @pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
 def test_unpreconditioned_cg_variant(pkg, pbref, prec, tol):
     """NEXT row f3: the paper's GPU/CG (PAPER.md:76-94) = the same recurrence with M = I.  Same parity bar;
