@@ -393,10 +393,21 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     const int xy = w.qntx * w.qnty;
     int TZ = c.TZ;
     if (TZ <= 0) {
-        int ntz = (int)((1.9 * slots + xy - 1) / xy);   // smallest z split with ~2 tiles per resident block
-        if (ntz < 1) ntz = 1;
-        TZ = (h->nz + ntz - 1) / ntz;
-        if (TZ < 8) TZ = 8;
+        // z split: blocks stride over the tile list, so the launch lasts ceil(tiles / slots) tiles.  Take the split
+        // whose tile count fills those waves best (a count just above a multiple of the grid wastes up to a whole
+        // wave), charging each tile its two halo planes (about one plane's worth of traffic); fewest tiles on ties.
+        double best = -1.0;
+        int best_ntz = 1;
+        const int max_ntz = h->nz / 8 > 1 ? h->nz / 8 : 1;
+        for (int ntz = 1; ntz <= max_ntz && (long)xy * ntz <= 8L * slots + xy; ntz++) {
+            const int tz = (h->nz + ntz - 1) / ntz;
+            const long tiles = (long)xy * ((h->nz + tz - 1) / tz);
+            const long waves = (tiles + slots - 1) / slots;
+            const double fill = (double)tiles / (double)(waves * slots);
+            const double score = fill * tz / (tz + 1.0);
+            if (score > best + 1e-9) { best = score; best_ntz = ntz; }
+        }
+        TZ = (h->nz + best_ntz - 1) / best_ntz;
     }
     if (TZ > h->nz) TZ = h->nz;
     w.qTZ = TZ;
