@@ -147,6 +147,18 @@ pb_status pb_get_field(pb_handle *h, int which, double *out_host);
 pb_status pb_set_preconditioner(pb_handle *h, int kind);
 
 /*
+ * pb_solve_refined -- mixed-precision iterative refinement ("fp32-inner / fp64-outer"): phi and
+ * the true residual r = b - A phi are kept in fp64; each correction A d = r is a Jacobi-PCG solve (PAPER.md:104-126,
+ * the kernels of pb_solve) in fp32 to `inner_tol` relative to ||r|| (1e-5 is what fp32 storage delivers; the last
+ * correction only closes the remaining gap); phi += d.  Stops when the TRUE relative residual ||b - A phi||/||b||
+ * <= tol (written to *relres_out), after `maxiter` inner iterations in total (PB_ERR_MAXITER, phi_out = last
+ * iterate) or on a breakdown.  phi_out: [nz][ny][nx] fp64, host or device per `where`.  *outer_out = number of
+ * corrections, *iters_out = inner PCG iterations in total.  Builds both the fp32 and the fp64 work arrays.
+ */
+pb_status pb_solve_refined(pb_handle *h, double tol, int maxiter, double inner_tol, int check_every, double *phi_out,
+                           pb_memspace where, int *outer_out, int *iters_out, double *relres_out);
+
+/*
  * pb_residual -- the TRUE relative residual ||b - A phi||_2 / ||b||_2 of a caller-supplied potential ([nz][ny][nx] in
  * `prec`), evaluated with the SpMV kernel in that precision and fp64 sums.  pb_solve tests and returns the recurrence
  * residual (DESIGN.md Reading 5); with fp32 storage the true residual stagnates near 1e-6..1e-5 while

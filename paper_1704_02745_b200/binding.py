@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node")
+           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -66,6 +66,8 @@ def load_library():
     lib.pb_set_boundary.argtypes = [vp, ci]
     lib.pb_bytes_per_node.argtypes = [vp, ci, ci]
     lib.pb_bytes_per_node.restype = ci
+    lib.pb_solve_refined.argtypes = [vp, cd, ci, cd, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(ci),
+                                     ctypes.POINTER(cd)]
     lib.pb_residual.argtypes = [vp, ci, vp, ci, ctypes.POINTER(cd)]
     lib.pb_create_from_atoms.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, ci, vp, vp, vp, cd, cd, cd, ci, vp]
     lib.pb_set_charges.argtypes = [vp, vp, ci]
@@ -255,13 +257,29 @@ class PBSolver:
             raise PBError(st, "pb_solve")
         return dict(phi=out, iters=it.value, relres=rel.value, status=st)
 
+    def solve_refined(self, tol, maxiter, inner_tol=1e-5, check_every=32, out=None):
+        """Mixed-precision iterative refinement (pb_solve_refined): fp64 potential and true residual, fp32 Jacobi-PCG
+        corrections.  Returns dict(phi [fp64], outer, iters [inner PCG iterations in total], relres [TRUE], status)."""
+        n = self.nx * self.ny * self.nz
+        if out is None:
+            out = np.empty(self.shape, dtype=np.float64)
+        if not _is_torch(out) and (out.dtype != np.float64 or not out.flags.c_contiguous):
+            raise TypeError("out must be a C-contiguous float64 array")
+        op, so, keep = _marshal(out, np.float64, n, "out")
+        if _is_torch(out) and keep.data_ptr() != out.data_ptr():
+            raise TypeError("out must be contiguous")
+        outer, it, rel = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_double(0.0)
+        st = load_library().pb_solve_refined(self._h, float(tol), int(maxiter), float(inner_tol), int(check_every),
+                                             op, so, ctypes.byref(outer), ctypes.byref(it), ctypes.byref(rel))
+        if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
+            raise PBError(st, "pb_solve_refined")
+        return dict(phi=out, outer=outer.value, iters=it.value, relres=rel.value, status=st)
+
     def set_preconditioner(self, jacobi: bool):
         """True (default): Jacobi-PCG; False: unpreconditioned CG (M = I)."""
         st = load_library().pb_set_preconditioner(self._h, 1 if jacobi else 0)
         if st != PB_OK:
-            raise PBError(st, "pb_set_preconditioner", "pb_create_from_atoms",
-           "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node")
+            raise PBError(st, "pb_set_preconditioner")
 
     def set_periodic(self, periodic: bool):
         """False (default): Dirichlet ghost layer; True: periodic boundary condition."""

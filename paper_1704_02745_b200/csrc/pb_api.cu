@@ -704,9 +704,9 @@ pb_status ensure_stage(pb_handle *h, size_t bytes)
     return PB_OK;
 }
 
+// steps 1-8 until the device latch is set (converged, maxiter or breakdown); the iterate stays on the device
 template <typename T>
-pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, void *phi_out,
-                     pb_memspace where, int *iters_out, double *relres_out, const void *phi0 = nullptr)
+pb_status run_solve(pb_handle *h, double tol, int maxiter, int check_every, const void *phi0, pb_memspace where)
 {
     PB_TRY(begin_solve<T>(h, tol, maxiter, 1, phi0, where));
     Work<T> &w = work<T>(h);
@@ -738,6 +738,15 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
             seen_done = h->pinned[4 * ((c - 1) & 1)];
         }
     }
+    return PB_OK;
+}
+
+template <typename T>
+pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, void *phi_out,
+                     pb_memspace where, int *iters_out, double *relres_out, const void *phi0 = nullptr)
+{
+    PB_TRY(run_solve<T>(h, tol, maxiter, check_every, phi0, where));
+    Work<T> &w = work<T>(h);
     // a6: un-pad x -> phi_out, read the final scalars
     const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
     T *dst = (T *)phi_out;
@@ -754,6 +763,74 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     if (iters_out) *iters_out = st.iters;
     if (relres_out) *relres_out = (st.bb > 0.0) ? sqrt(st.rr / st.bb) : 0.0;
     return (pb_status)st.status;
+}
+
+// Mixed-precision iterative refinement: the potential and the true residual r = b - A phi live in
+// fp64 (k_spmv_tma<double, MODE 1> + k_true_residual); each correction A d = r is a Jacobi-PCG solve in fp32 (the
+// same kernels as pb_solve) to `inner_tol` relative to ||r||; phi += d in fp64.  The result meets
+// the fp64 tolerance on the TRUE residual at close to the fp32 iteration rate.
+pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, int check_every, double *phi_out,
+                       pb_memspace where, int *outer_out, int *iters_out, double *relres_out)
+{
+    PB_TRY(ensure<double>(h));
+    PB_TRY(ensure<float>(h));
+    Work<double> &wd = h->wd;
+    Work<float> &wf = h->wf;
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    const size_t nvec_d = wd.npad / VecN<double>::value;
+    // phi (padded fp64) is kept in wd.tmp, the input tensor of the MODE 1 SpMV
+    PB_CUDA(cudaMemsetAsync(wd.tmp, 0, wd.npad * sizeof(double), h->stream));
+    int total = 0, outer = 0;
+    double relres = 1.0;
+    pb_status status = PB_ERR_MAXITER;
+    for (;; outer++) {
+        launch_spmv<double, 1>(h, wd, 1.0);
+        launch_wrap<double, 1>(h, wd, 1.0);
+        k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
+        k_true_residual<double><<<grid_for(nvec_d, 256, kNumSM * 4), 256, 0, h->stream>>>(wd.b, wd.Ap, nvec_d, h->st,
+                                                                                          h->partials, wd.r);
+        PB_CUDA(cudaGetLastError());
+        h->launches += 3;
+        PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        const double rr = h->pinned_state->rr, bb = h->pinned_state->bb;
+        relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+        if (!(relres == relres)) { status = PB_ERR_BREAKDOWN; break; }
+        if (relres <= tol) { status = PB_OK; break; }
+        if (total >= maxiter || outer >= 40) break;
+        // correction solve in fp32 on the right-hand side r; the last one only has to close the remaining gap
+        double tin = 0.3 * tol / relres;
+        if (tin < inner_tol) tin = inner_tol;
+        if (tin > 0.1) tin = 0.1;
+        k_repad<double, float><<<grid_for(wf.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(wd.r, wd.P, wf.b, wf.P,
+                                                                                           h->nx, rows);
+        h->launches += 1;
+        wf.b_ready = true;
+        const pb_status rs = run_solve<float>(h, tin, maxiter - total, check_every, nullptr, PB_DEVICE);
+        wf.b_ready = false;                      // wf.b holds a residual, not b: rebuilt before the next plain solve
+        if (rs != PB_OK) return rs;
+        k_finish_add<float, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(
+            wf.x, wf.p0, wf.p1, h->st, wd.tmp, h->nx, wf.P, wd.P, rows);
+        PB_CUDA(cudaGetLastError());
+        h->launches += 1;
+        PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        total += h->pinned_state->iters;
+        if (h->pinned_state->status == (int)PB_ERR_BREAKDOWN) { status = PB_ERR_BREAKDOWN; break; }
+    }
+    h->last_prec = PB_F64;
+    double *dst = phi_out;
+    if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(double))); dst = (double *)h->stage; }
+    k_unpad<double, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(wd.tmp, dst, h->nx, wd.P, rows, 1.0);
+    PB_CUDA(cudaGetLastError());
+    h->launches += 1;
+    if (where == PB_HOST)
+        PB_CUDA(cudaMemcpyAsync(phi_out, dst, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    if (outer_out) *outer_out = outer;
+    if (iters_out) *iters_out = total;
+    if (relres_out) *relres_out = relres;
+    return status;
 }
 
 template <typename T>
@@ -1008,6 +1085,15 @@ pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec
     return prec == PB_F32
                ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out, phi0)
                : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out, phi0);
+}
+
+pb_status pb_solve_refined(pb_handle *h, double tol, int maxiter, double inner_tol, int check_every, double *phi_out,
+                           pb_memspace where, int *outer_out, int *iters_out, double *relres_out)
+{
+    if (!h || !phi_out || !(tol > 0.0) || !(inner_tol > 0.0) || maxiter < 0 || check_every < 1 || !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return refined_impl(h, tol, maxiter, inner_tol, check_every, phi_out, where, outer_out, iters_out, relres_out);
 }
 
 pb_status pb_residual(pb_handle *h, pb_precision prec, const void *phi, pb_memspace where, double *relres_out)

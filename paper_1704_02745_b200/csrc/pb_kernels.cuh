@@ -324,20 +324,23 @@ __global__ void __launch_bounds__(256) k_wrap(const WrapArgs<T> a)
 // residual the iteration tests (DESIGN.md Reading 5).  Same two-stage deterministic reduction; result in st->rr, st->bb.
 template <typename T>
 __global__ void __launch_bounds__(256) k_true_residual(const T *__restrict__ b, const T *__restrict__ Ap, size_t nvec,
-                                                       State *st, double *partials)
+                                                       State *st, double *partials, T *rout = nullptr)
 {
     constexpr int VEC = VecN<T>::value;
     __shared__ double red[32];
     __shared__ int s_last;
     double s_rr = 0.0, s_bb = 0.0;
     for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += (size_t)gridDim.x * blockDim.x) {
-        const Vec<T> bv = ldv(b + v * VEC), qv = ldv(Ap + v * VEC);
+        Vec<T> bv = ldv(b + v * VEC);
+        const Vec<T> qv = ldv(Ap + v * VEC);
 #pragma unroll
         for (int e = 0; e < VEC; e++) {
             const double d = (double)bv.a[e] - (double)qv.a[e];
             s_rr = fma(d, d, s_rr);
             s_bb = fma((double)bv.a[e], (double)bv.a[e], s_bb);
+            bv.a[e] = (T)d;
         }
+        if (rout) stv(rout + v * VEC, bv);          // r = b - A'phi kept (iterative refinement)
     }
     const double t_rr = block_sum(s_rr, red), t_bb = block_sum(s_bb, red);
     const int nblk = gridDim.x;
@@ -352,6 +355,33 @@ __global__ void __launch_bounds__(256) k_true_residual(const T *__restrict__ b, 
         __threadfence();
         const double rr = final_sum(partials, nblk, red), bb = final_sum(partials + nblk, nblk, red);
         if (threadIdx.x == 0) { st->ticket_vec = 0u; st->rr = rr; st->bb = bb; }
+    }
+}
+
+// Mixed-precision iterative refinement: the fp64 residual becomes the fp32 right-hand side, and
+// the fp32 correction x + alpha p (its last update still pending, as in k_finish) is added to the fp64 potential.
+template <typename S, typename T>
+__global__ void k_repad(const S *__restrict__ src, int Ps, T *dst, int Pd, int nx, size_t rows)
+{
+    const size_t total = rows * Pd;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(t % Pd);
+        const size_t row = t / Pd;
+        dst[t] = (i < nx) ? (T)src[row * Ps + i] : T(0);
+    }
+}
+
+template <typename T, typename S>
+__global__ void k_finish_add(const T *__restrict__ x, const T *__restrict__ pbuf0, const T *__restrict__ pbuf1,
+                             const State *st, S *acc, int nx, int P, int Pacc, size_t rows)
+{
+    const T alpha = (T)st->alpha;
+    const T *p = (st->iter_cur & 1) ? pbuf1 : pbuf0;
+    const size_t total = rows * nx;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(t % nx);
+        const size_t row = t / nx;
+        acc[row * Pacc + i] += (S)fma(alpha, p[row * P + i], x[row * P + i]);
     }
 }
 

@@ -627,3 +627,28 @@ def test_true_residual_matches_oracle(pkg, pbref):
     ref.close()
     assert g["relres"] < 1e-7 < true                      # fp32 storage: recurrence below, truth above
     assert abs(t64 - true) <= 1e-6 * true and abs(t32 - true) <= 0.2 * true
+
+
+@pytest.mark.parametrize("cfg", [2, "born", "random"])
+def test_mixed_precision_refinement_matches_fp64_oracle(pkg, pbref, cfg):
+    """NEXT row f3 (fp32-inner / fp64-outer iterative refinement): the result is the solution of A phi = b to 1e-10 on
+    the TRUE residual -- same bar as the fp64 solve (within 1e-8 max|phi| of the oracle run to 1e-10) -- although every
+    PCG iteration ran in fp32; a plain fp32 solve cannot get there (its true residual stagnates near 1e-6)."""
+    inp = make_config(2) if cfg == 2 else born_ion() if cfg == "born" else random_operator(45, 31, 38, seed=8)
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(1e-10, 5000)
+    b = ref.b()
+    with pkg.PBSolver(*inp.args()) as s:
+        g = s.solve_refined(1e-10, 5000)
+        assert g["status"] == 0 and g["relres"] <= 1e-10 and 2 <= g["outer"] <= 6
+        assert abs(s.residual(g["phi"], "f64") - g["relres"]) <= 1e-3 * g["relres"] + 1e-16
+        f = s.solve(1e-10, 5000, "f32")                      # wf.b must have been rebuilt after the refinement
+        d = s.solve(1e-10, 5000, "f64")
+    true = np.linalg.norm(b - ref.apply(g["phi"])) / np.linalg.norm(b)
+    ref.close()
+    scale = np.max(np.abs(o["phi"]))
+    assert true <= 2e-10
+    assert np.max(np.abs(g["phi"] - o["phi"])) <= 1e-8 * scale
+    assert np.max(np.abs(d["phi"] - o["phi"])) <= 1e-8 * scale
+    assert np.max(np.abs(f["phi"] - o["phi"])) <= 1e-4 * scale
+    assert g["iters"] <= 4 * o["iters"]
