@@ -53,6 +53,8 @@ def parse_args(argv=None):
                     help="also time pb_create_from_atoms / pb_set_charges (GPU grid setup, NEXT row f1)")
     ap.add_argument("--batch", type=int, default=0,
                     help="also run this many solves of config 5's perturbed-charge batch on the same operator")
+    ap.add_argument("--refined", action="store_true",
+                    help="also time pb_solve_refined (fp32-inner / fp64-outer, NEXT row f3) against the fp64 solve, to 1e-10")
     return ap.parse_args(argv)
 
 
@@ -316,6 +318,25 @@ def run_ours(args, rank, local_rank, world):
                  "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member, this rank only; warm_start: "
                          "the same members solved again from the previous member's potential (pb_solve_from)"}
 
+    # ---- optional (NEXT row f3): mixed-precision iterative refinement against the plain fp64 solve ----------------
+    refined = None
+    if args.refined:
+        out64 = torch.empty((inp.nz, inp.ny, inp.nx), dtype=torch.float64, device=dev)
+        tms = {}
+        for name, fn in (("refined", lambda: solver.solve_refined(1e-10, args.maxiter, 1e-5, args.check_every, out=out64)),
+                         ("f64", lambda: solver.solve(1e-10, args.maxiter, "f64", check_every=args.check_every, out=out64))):
+            fn()                                                # builds the work arrays / warms up
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r_ = fn()
+            torch.cuda.synchronize()
+            tms[name] = (1e3 * (time.perf_counter() - t0), r_, solver.residual(out64, "f64"))
+        refined = {"tol": 1e-10, "refined_ms": tms["refined"][0], "outer": tms["refined"][1]["outer"],
+                   "inner_iterations": tms["refined"][1]["iters"], "true_relres": tms["refined"][2],
+                   "f64_ms": tms["f64"][0], "f64_iterations": tms["f64"][1]["iters"], "f64_true_relres": tms["f64"][2],
+                   "note": "pb_solve_refined: fp64 potential and true residual, fp32 Jacobi-PCG corrections (inner_tol 1e-5)"}
+        del out64
+
     # ---- optional (NEXT row f1): the same problem built on the GPU from atoms, and a charge update ---------------
     setup = None
     if args.setup_from_atoms and "charges" in inp.meta:
@@ -419,6 +440,8 @@ def run_ours(args, rank, local_rank, world):
             line["batch"] = batch
         if setup is not None:
             line["setup_from_atoms"] = setup
+        if refined is not None:
+            line["refined"] = refined
     solver.close()
     if world > 1:
         dist.barrier()
