@@ -361,15 +361,28 @@ def run_ours(args, rank, local_rank, world):
             torch.cuda.synchronize()
             t_sc += t1 - t0
             t_sv += time.perf_counter() - t1
+        # the same charge updates with the boundary terms in fp32 (pb_set_setup_precision)
+        s2.set_setup_precision("f32")
+        t_sc32, it_sc32 = 0.0, []
+        for sidx in range(nb):
+            qs = perturbed_charge_values(inp, sidx)
+            t0 = time.perf_counter()
+            s2.set_charges(qs)
+            torch.cuda.synchronize()
+            t_sc32 += time.perf_counter() - t0
+            it_sc32.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
         s2.close()
         nbc = 2 * (inp.nz * inp.ny + inp.nz * inp.nx + inp.ny * inp.nx)
         terms = float(nbc) * len(m["charges"])
         setup = {"create_from_atoms_ms": 1e3 * t_fa, "set_charges_ms": 1e3 * t_sc / nb, "solve_ms": 1e3 * t_sv / nb,
                  "mean_iters": float(np.mean(it_sc)), "members": nb, "atoms": int(len(m["charges"])),
                  "dh_terms": terms, "dh_gterms_per_s": terms / (t_sc / nb) / 1e9,
+                 "set_charges_f32_ms": 1e3 * t_sc32 / nb, "dh_f32_gterms_per_s": terms / (t_sc32 / nb) / 1e9,
+                 "mean_iters_f32_boundary": float(np.mean(it_sc32)),
                  "host_generator_s": t_gen,
                  "note": "pb_create_from_atoms = mask + faces + salt + charges + Debye-Hueckel ghosts + pb_create "
-                         "(incl. plan autotune); set_charges = charge spreading + the fp64 DH boundary sum (ALU-bound)"}
+                         "(incl. plan autotune); set_charges = charge spreading + the fp64 DH boundary sum (ALU-bound); "
+                         "set_charges_f32 = the same with the boundary terms in fp32 (pb_set_setup_precision)"}
 
     # ---- roofline of the dominant kernel (K_spmv), CUDA events around every launch ----------------
     solver.solve_begin(prec)

@@ -135,6 +135,16 @@ pb_status pb_create_from_atoms(pb_handle **out, int nx, int ny, int nz, double h
  * batch member).  Only for handles made by pb_create_from_atoms. */
 pb_status pb_set_charges(pb_handle *h, const double *charges, pb_memspace where);
 
+/*
+ * pb_set_setup_precision -- arithmetic of the Debye-Hueckel boundary sum in later pb_set_charges calls (SURVEY.md 8(f)
+ * f1; the sum has n_ghost x n_atoms terms, 5.3e10 at config 5, and is plain-ALU-bound).  PB_F64 (default): every term
+ * in fp64, parity with the fp64 setup oracle to rounding.  PB_F32: terms in fp32 (coordinates relative to the box
+ * centre, hardware rsqrt / exp2, Kahan-compensated fp32 partial sums per 256 atoms, fp64 across tiles): boundary values
+ * within a few 1e-7 of the largest term of the fp64 ones -- enough for an fp32 solve -- at several times the rate.
+ * The charge spreading and b stay fp64 either way.
+ */
+pb_status pb_set_setup_precision(pb_handle *h, pb_precision prec);
+
 /* pb_get_field -- copy one of the handle's dense fp64 input fields to the host (tests of pb_create_from_atoms):
  * which = 0 eps_x, 1 eps_y, 2 eps_z, 3 kbar2, 4 rhs, 5 bc (layouts as in pb_create; a NULL input reads as zeros). */
 pb_status pb_get_field(pb_handle *h, int which, double *out_host);

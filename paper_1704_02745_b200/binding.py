@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined")
+           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined", "pb_set_setup_precision")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -68,6 +68,7 @@ def load_library():
     lib.pb_bytes_per_node.restype = ci
     lib.pb_solve_refined.argtypes = [vp, cd, ci, cd, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(cd)]
+    lib.pb_set_setup_precision.argtypes = [vp, ci]
     lib.pb_residual.argtypes = [vp, ci, vp, ci, ctypes.POINTER(cd)]
     lib.pb_create_from_atoms.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, ci, vp, vp, vp, cd, cd, cd, ci, vp]
     lib.pb_set_charges.argtypes = [vp, vp, ci]
@@ -274,6 +275,13 @@ class PBSolver:
         if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
             raise PBError(st, "pb_solve_refined")
         return dict(phi=out, outer=outer.value, iters=it.value, relres=rel.value, status=st)
+
+    def set_setup_precision(self, precision):
+        """'f64' (default) or 'f32': arithmetic of the Debye-Hueckel boundary sum in set_charges."""
+        pc, _ = _prec(precision)
+        st = load_library().pb_set_setup_precision(self._h, pc)
+        if st != PB_OK:
+            raise PBError(st, "pb_set_setup_precision")
 
     def set_preconditioner(self, jacobi: bool):
         """True (default): Jacobi-PCG; False: unpreconditioned CG (M = I)."""

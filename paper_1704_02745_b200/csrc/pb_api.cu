@@ -82,6 +82,7 @@ struct pb_handle {
     double *atoms_c;             // [n_atoms][3], device
     int n_atoms;
     double atoms_eps_out, atoms_kappa;
+    bool dh_f32 = false;         // pb_set_charges evaluates the Debye-Hueckel boundary terms in fp32
     int l2hints;                 // PB_L2HINTS (default 1): L2 eviction-priority hints across the two kernels
     int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
 };
@@ -1252,15 +1253,20 @@ struct DevTmp {                      // frees its device allocations on scope ex
 
 // rhs (dense [nz][ny][nx]) and bc from charges on the stored / given atom geometry
 pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
-                            double eps_out, double kappa, double *d_rhs, double *d_bc, cudaStream_t st)
+                            double eps_out, double kappa, double *d_rhs, double *d_bc, cudaStream_t st,
+                            bool dh_f32 = false)
 {
     const size_t n = (size_t)nx * ny * nz;
     const size_t nbc = 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx);
     PB_CUDA(cudaMemsetAsync(d_rhs, 0, n * sizeof(double), st));
     k_grid_spread<<<grid_for((size_t)n_atoms, 128, kNumSM * 8), 128, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh, d_rhs);
     k_grid_rhs<<<grid_for(n, 256, kNumSM * 16), 256, 0, st>>>(d_rhs, n, 4.0 * 3.141592653589793, pow(hh, 3.0));
-    k_grid_dh<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
-                                                                            eps_out, kappa, d_bc);
+    if (dh_f32)
+        k_grid_dh_f32<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
+                                                                                    eps_out, kappa, d_bc);
+    else
+        k_grid_dh<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
+                                                                                eps_out, kappa, d_bc);
     PB_CUDA(cudaGetLastError());
     return PB_OK;
 }
@@ -1332,13 +1338,20 @@ extern "C" pb_status pb_set_charges(pb_handle *h, const double *charges, pb_mems
     if (!h->rhs) PB_ALLOC(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
     if (!h->bc) PB_ALLOC(cudaMalloc((void **)&h->bc, (nbc + 8) * sizeof(double)));
     PB_TRY(charges_to_rhs_bc(h->atoms_c, d_q, h->n_atoms, h->nx, h->ny, h->nz, h->h, h->atoms_eps_out,
-                             h->atoms_kappa, h->rhs, h->bc, h->stream));
+                             h->atoms_kappa, h->rhs, h->bc, h->stream, h->dh_f32));
     h->launches += 3;
     h->wf.b_ready = false;
     h->wd.b_ready = false;
     if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));
     if (h->wd.ready) PB_TRY(build_b<double>(h, h->wd));
     PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}
+
+extern "C" pb_status pb_set_setup_precision(pb_handle *h, pb_precision prec)
+{
+    if (!h || !valid_prec(prec)) return PB_ERR_INVALID_ARG;
+    h->dh_f32 = (prec == PB_F32);
     return PB_OK;
 }
 

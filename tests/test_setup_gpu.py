@@ -67,6 +67,40 @@ def test_fields_match_setup_oracle(pkg, shape, na):
         assert np.array_equal(s.field("eps_x"), ref["eps_x"])
 
 
+def test_fp32_boundary_sum(pkg):
+    """pb_set_setup_precision(PB_F32): the Debye-Hueckel ghost values with every term in fp32 (hardware rsqrt / exp2,
+    Kahan partial sums) stay within 2e-6 of the sum of |terms| of the fp64 setup oracle (an fp32 term carries a few
+    1e-7; the bound is on the term scale because charges of both signs cancel), the charge grid stays fp64-exact, and
+    an fp32 solve on that boundary is still within the fp32 bar of the oracle's solve on the exact boundary."""
+    from oracle import pbref, pbsetup_ref as S
+
+    nx, ny, nz, h = 40, 23, 31, 0.5
+    eps_in, eps_out, kb = 1.0, 80.0, W.KBAR2_150MM_300K
+    c, r, q = atoms(300, nx, ny, nz, h, 61)              # more than one 256-atom tile, odd tail
+    c = c[:299]; r = r[:299]; q = q[:299]
+    q2 = q + 0.05
+    ref = S.setup(nx, ny, nz, h, c, r, q2, eps_in, eps_out, kb)
+    kappa = math.sqrt(kb / eps_out)
+    g = S.ghost_positions(nx, ny, nz, h)
+    rr = np.linalg.norm(g[:, None, :] - c[None, :, :], axis=2)
+    scale = (np.abs(q2)[None, :] * np.exp(-kappa * rr) / rr).sum(1) / eps_out
+    o = pbref.PBRef(nx, ny, nz, h, ref["eps_x"], ref["eps_y"], ref["eps_z"], ref["kbar2"], ref["rhs"],
+                    ref["bc"]).solve(1e-10, 5000)
+    with pkg.PBSolver.from_atoms(nx, ny, nz, h, c, r, q, eps_in, eps_out, kb) as s:
+        s.set_setup_precision("f32")
+        s.set_charges(q2)
+        bc32 = s.field("bc")
+        err = np.abs(bc32 - ref["bc"])
+        assert np.all(err <= 2e-6 * scale)
+        assert np.max(err / scale) > 1e-12               # it really is the fp32 kernel
+        assert np.max(np.abs(s.field("rhs") - ref["rhs"])) <= 1e-13 * np.max(np.abs(ref["rhs"]))
+        g32 = s.solve(1e-5, 5000, "f32")
+        s.set_setup_precision("f64")
+        s.set_charges(q2)
+        assert np.all(np.abs(s.field("bc") - ref["bc"]) <= 1e-12 * scale)
+    assert np.max(np.abs(g32["phi"] - o["phi"])) <= 1e-4 * np.max(np.abs(o["phi"]))
+
+
 def test_solve_through_atom_built_handle(pkg):
     from oracle import pbref, pbsetup_ref as S
 
