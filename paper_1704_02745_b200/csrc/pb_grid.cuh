@@ -145,6 +145,9 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ 
 // Kahan-compensated fp32 partial sums per atom tile, tiles added in fp64): ~2 special-function operations per term
 // instead of an fp64 rsqrt and exp, for callers who solve in fp32 anyway (pb_set_setup_precision).  Values agree with
 // the fp64 kernel to a few 1e-7 of the largest term.
+__device__ __forceinline__ float mufu_rsq(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 __global__ void __launch_bounds__(DH_TILE) k_grid_dh_f32(const double *__restrict__ c, const double *__restrict__ charge,
                                                          int n_atoms, int nx, int ny, int nz, double h, double eps_out,
                                                          double kappa, double *bc)
@@ -181,8 +184,8 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh_f32(const double *__restric
             const float4 A = sc[s], B = sc[s + 1];
             const float ax = fx - A.x, ay = fy - A.y, az = fz - A.z, bx = fx - B.x, by = fy - B.y, bz = fz - B.z;
             const float da = fmaf(az, az, fmaf(ay, ay, ax * ax)), db = fmaf(bz, bz, fmaf(by, by, bx * bx));
-            const float ia = rsqrtf(da), ib = rsqrtf(db);
-            const float ta = A.w * (exp2f(nk * (da * ia)) * ia), tb = B.w * (exp2f(nk * (db * ib)) * ib);
+            const float ia = mufu_rsq(da), ib = mufu_rsq(db);
+            const float ta = A.w * (mufu_ex2(nk * (da * ia)) * ia), tb = B.w * (mufu_ex2(nk * (db * ib)) * ib);
             const float ya = ta - k0, yb = tb - k1;
             const float ua = s0 + ya, ub = s1 + yb;
             k0 = (ua - s0) - ya; k1 = (ub - s1) - yb;
@@ -192,8 +195,8 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh_f32(const double *__restric
             const float4 A = sc[s];
             const float ax = fx - A.x, ay = fy - A.y, az = fz - A.z;
             const float da = fmaf(az, az, fmaf(ay, ay, ax * ax));
-            const float ia = rsqrtf(da);
-            const float ya = A.w * (exp2f(nk * (da * ia)) * ia) - k0;
+            const float ia = mufu_rsq(da);
+            const float ya = A.w * (mufu_ex2(nk * (da * ia)) * ia) - k0;
             const float ua = s0 + ya;
             k0 = (ua - s0) - ya; s0 = ua;
         }
