@@ -523,7 +523,9 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         PB_CUDA(cudaMemsetAsync(w.x, 0, w.npad * sizeof(T), h->stream));
         k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
         float tbest = 1e30f;
+        float tms[64];
         for (int i = 0; i < nc; i++) {
+            tms[i] = 1e30f;
             if (configure_tma<T>(h, w, cand[i]) != PB_OK) continue;
             if ((size_t)w.qgrid > h->partials_cap) continue;
             launch_spmv<T, 0>(h, w, 1.0);
@@ -539,7 +541,40 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
             if (getenv("PB_VERBOSE"))
                 fprintf(stderr, "pb: tune TXV=%d TY=%d NS=%d bps=%d TZ=%d grid=%d: %.4f ms\n", cand[i].TXV, cand[i].TY,
                         cand[i].NS, cand[i].bps, w.qTZ, w.qgrid, ms / 3);
+            tms[i] = ms;
             if (ms < tbest) { tbest = ms; best = i; }
+        }
+        // second pass: the three fastest plans are within the noise of three launches of each other; time them
+        // again the way the solver runs them -- alternating with k_vec, twelve iterations each
+        int fin[3] = {-1, -1, -1};
+        for (int f = 0; f < 3; f++) {
+            float tb = 1e30f;
+            for (int i = 0; i < nc; i++)
+                if (tms[i] < tb && i != fin[0] && i != fin[1]) { tb = tms[i]; fin[f] = i; }
+        }
+        if (fin[1] >= 0 && (size_t)2 * w.vec_grid <= h->partials_cap) {
+            const VecArgs<T> va = vec_args<T>(h, w);
+            tbest = 1e30f;
+            for (int f = 0; f < 3 && fin[f] >= 0; f++) {
+                if (configure_tma<T>(h, w, cand[fin[f]]) != PB_OK) continue;
+                cudaEventRecord(e0, h->stream);
+                for (int rep = 0; rep < 12; rep++) {
+                    launch_spmv<T, 0>(h, w, 1.0);
+                    if (w.pald) k_vec<T, true><<<w.vec_grid, 256, 0, h->stream>>>(va);
+                    else k_vec<T, false><<<w.vec_grid, 256, 0, h->stream>>>(va);
+                }
+                cudaEventRecord(e1, h->stream);
+                if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+                    cudaEventDestroy(e0); cudaEventDestroy(e1);
+                    return PB_ERR_CUDA;
+                }
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, e0, e1);
+                if (getenv("PB_VERBOSE"))
+                    fprintf(stderr, "pb: tune (pass 2) TXV=%d TY=%d NS=%d bps=%d: %.4f ms per iteration\n", cand[fin[f]].TXV,
+                            cand[fin[f]].TY, cand[fin[f]].NS, cand[fin[f]].bps, ms / 12);
+                if (ms < tbest) { tbest = ms; best = fin[f]; }
+            }
         }
         cudaEventDestroy(e0);
         cudaEventDestroy(e1);
