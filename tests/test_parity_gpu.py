@@ -652,3 +652,27 @@ def test_mixed_precision_refinement_matches_fp64_oracle(pkg, pbref, cfg):
     assert np.max(np.abs(d["phi"] - o["phi"])) <= 1e-8 * scale
     assert np.max(np.abs(f["phi"] - o["phi"])) <= 1e-4 * scale
     assert g["iters"] <= 4 * o["iters"]
+
+
+@pytest.mark.parametrize("persist", ["0", "1"])
+def test_refinement_periodic_and_two_kernel_path(pkg, pbref, persist):
+    """pb_solve_refined under the periodic boundary condition (wrap terms in the fp64 residual and in the fp32
+    corrections), through the persistent kernel and through the two-kernel TMA path."""
+    inp = _periodic_inputs((45, 23, 19), 32)
+    ref = pbref.from_inputs(inp)
+    ref.set_periodic(True)
+    ref.set_rhs(inp.rhs, inp.bc)
+    o = ref.solve(1e-10, 5000)
+    ref.close()
+    saved = os.environ.pop("PB_PERSIST", None)
+    os.environ["PB_PERSIST"] = persist
+    try:
+        with pkg.PBSolver(*inp.args()) as s:
+            s.set_periodic(True)
+            g = s.solve_refined(1e-10, 5000, check_every=8)
+    finally:
+        os.environ.pop("PB_PERSIST", None)
+        if saved is not None:
+            os.environ["PB_PERSIST"] = saved
+    assert g["status"] == 0 and g["relres"] <= 1e-10
+    assert np.max(np.abs(g["phi"] - o["phi"])) <= 1e-8 * np.max(np.abs(o["phi"]))
