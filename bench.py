@@ -68,12 +68,16 @@ def measured_peak():
 
 
 def ncu_traffic(workload_key):
-    """dram bytes per K_spmv launch from the committed ncu --set full summary, or None."""
+    """dram bytes per K_spmv launch from the committed ncu --set full summary (profiles/ncu_traffic.csv), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(workload_key)
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for line in f:
+                cols = line.strip().split(",")
+                if len(cols) >= 2 and cols[0] == workload_key:
+                    return int(cols[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
