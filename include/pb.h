@@ -206,7 +206,9 @@ long long pb_launch_count(pb_handle *h);
 /* Size of the handle's coefficient palette: when the three face-dielectric arrays hold <= 256 distinct values
  * (every molecular map built from eps_in / eps_out and their harmonic mean, does) they are stored
  * exactly as one byte per face plus a table and decoded inside the SpMV; 0 = full-precision face arrays.
- * PB_PALETTE=0 in the environment disables the palette. */
+ * The index bytes are stored pre-multiplied by the element size (the kernel adds them to the table address without a
+ * shift), so a precision uses the palette only when size * sizeof(element) <= 256, i.e. up to 64 values in fp32 and
+ * 32 in fp64 (pb_bytes_per_node tells which format a precision got).  PB_PALETTE=0 disables the palette. */
 int pb_palette_size(pb_handle *h);
 
 /* Size of the diagonal palette: with a face palette and a few-valued salt map the Jacobi diagonal also takes <= 256

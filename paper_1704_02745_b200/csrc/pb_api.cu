@@ -222,9 +222,10 @@ pb_status ensure(pb_handle *h)
             h->launches += 3;
         }
     }
-    w.pal = h->pal_n > 0;
-    w.pald = h->pald_n > 0;
-    w.pald_s = w.pald && w.pal && env_int("PB_PALETTE_DS", 1) != 0;
+    // k_spmv_tma decodes through tables addressed by pre-scaled index bytes: n * sizeof(T) <= 256 entries-bytes
+    w.pal = h->pal_n > 0 && (size_t)h->pal_n * sizeof(T) <= 256;
+    w.pald = w.pal && h->pald_n > 0;
+    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && env_int("PB_PALETTE_DS", 1) != 0;
     w.Pb = (w.P + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
@@ -286,18 +287,18 @@ pb_status ensure(pb_handle *h)
         w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
     if (w.pal) {
         k_setup_pal_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pb, 256, kNumSM * 16), 256, 0, h->stream>>>(
-            h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pb, h->pal_table, w.exi, w.eyi, w.ezi);
+            h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pal_table, w.exi, w.eyi, w.ezi);
         k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
         h->launches += 2;
     }
     if (w.pald) {
         k_setup_diag_idx<<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
-            h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P, h->pald_table, w.dvi);
+            h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P, 1, h->pald_table, w.dvi);
         k_pal_lut_dinv<T><<<1, 256, 0, h->stream>>>(h->pald_table, w.dlut);
         h->launches += 2;
         if (w.pald_s) {
             k_setup_diag_idx<<<grid_for((size_t)h->nz * h->ny * w.Pb, 256, kNumSM * 16), 256, 0, h->stream>>>(
-                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, h->pald_table, w.dvib);
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pald_table, w.dvib);
             h->launches += 1;
         }
     }
@@ -386,7 +387,7 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qTXV = TXV; w.qTY = TY; w.qns = NS;
     w.qntx = (rowvecs + TXV - 1) / TXV;
     w.qnty = (h->ny + TY - 1) / TY;
-    w.qthreads = (TXV * TY + 31) / 32 * 32 + 32;
+    w.qthreads = (spmv_row_threads(TXV) * TY + 31) / 32 * 32 + 32;
     const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0, w.pald_s);
     w.qsmem = (size_t)NS * L.slot + 128;
     if (w.qsmem > w.qmaxdyn || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
@@ -485,7 +486,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         c.TY = env_int("PB_TY", 4);
         if (c.TY < 1) c.TY = 1;
         if (c.TY > h->ny) c.TY = h->ny;
-        while (c.TXV * c.TY > 448 && c.TY > 1) c.TY--;
+        while (spmv_row_threads(c.TXV) * c.TY > 448 && c.TY > 1) c.TY--;
         c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s) >= 4 ? 2 : 1);
         if (c.bps < 1) c.bps = 1;
         c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s));
@@ -499,11 +500,11 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
             if (dx && TXV * VEC < 64) break;
             for (int ty : tys) {
                 int TY = ty > h->ny ? h->ny : ty;
-                if (TXV * TY > 448) continue;
+                if (spmv_row_threads(TXV) * TY > 448) continue;
                 for (int bps = 1; bps <= 4; bps++) {
                     const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0, w.pald_s);
                     if (NS < 4 && !(NS == 3 && bps >= 2)) continue;
-                    const int cthreads = ((TXV * TY + 31) / 32 * 32) * bps;
+                    const int cthreads = ((spmv_row_threads(TXV) * TY + 31) / 32 * 32) * bps;
                     if (cthreads < 256 || cthreads > 1024) continue;     // consumer threads per SM
                     if (nc < 64) cand[nc++] = TileCfg{TXV, TY, NS, bps, 0};
                 }

@@ -203,23 +203,25 @@ __device__ __forceinline__ unsigned char pal_index(const PalTable *t, double v)
     return (unsigned char)lo;
 }
 
-// byte index arrays in the padded layouts of exm / eym / ezm (row pitch Pb bytes, Pb >= P), pad = index of 0.0
+// byte index arrays in the padded layouts of exm / eym / ezm (row pitch Pb bytes, Pb >= P), pad = index of 0.0.
+// Every byte is the table index times `scale` (the element size of the decoding table, n * scale <= 256): the
+// kernel then adds the byte to the table's address with no shift.
 __global__ void k_setup_pal_idx(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
-                                const double *__restrict__ eps_z, int nx, int ny, int nz, int Pb,
+                                const double *__restrict__ eps_z, int nx, int ny, int nz, int Pb, int scale,
                                 const PalTable *t, unsigned char *exi, unsigned char *eyi, unsigned char *ezi)
 {
-    const unsigned char zero = pal_index(t, 0.0);
+    const unsigned char zero = (unsigned char)(pal_index(t, 0.0) * scale);
     const size_t total = (size_t)(nz + 1) * (ny + 1) * Pb;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         const int i = (int)(q % Pb);
         const size_t u = q / Pb;
         const int j = (int)(u % (ny + 1)), k = (int)(u / (ny + 1));
         if (k < nz && j < ny)
-            exi[((size_t)k * ny + j) * Pb + i] = (i <= nx) ? pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i]) : zero;
+            exi[((size_t)k * ny + j) * Pb + i] = (i <= nx) ? (unsigned char)(pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i]) * scale) : zero;
         if (k < nz)
-            eyi[((size_t)k * (ny + 1) + j) * Pb + i] = (i < nx) ? pal_index(t, eps_y[((size_t)k * (ny + 1) + j) * nx + i]) : zero;
+            eyi[((size_t)k * (ny + 1) + j) * Pb + i] = (i < nx) ? (unsigned char)(pal_index(t, eps_y[((size_t)k * (ny + 1) + j) * nx + i]) * scale) : zero;
         if (j < ny)
-            ezi[((size_t)k * ny + j) * Pb + i] = (i < nx) ? pal_index(t, eps_z[((size_t)k * ny + j) * nx + i]) : zero;
+            ezi[((size_t)k * ny + j) * Pb + i] = (i < nx) ? (unsigned char)(pal_index(t, eps_z[((size_t)k * ny + j) * nx + i]) * scale) : zero;
     }
 }
 
@@ -272,15 +274,15 @@ __global__ void k_pal_collect_diag(const double *__restrict__ eps_x, const doubl
 // byte index of D per padded node ([nz][ny][P], pad = index of 1.0)
 __global__ void k_setup_diag_idx(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
                                  const double *__restrict__ eps_z, const double *__restrict__ kbar2, double h2,
-                                 int nx, int ny, int nz, int P, const PalTable *t, unsigned char *dvi)
+                                 int nx, int ny, int nz, int P, int scale, const PalTable *t, unsigned char *dvi)
 {
-    const unsigned char one = pal_index(t, 1.0);
+    const unsigned char one = (unsigned char)(pal_index(t, 1.0) * scale);
     const size_t total = (size_t)nz * ny * P;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         const int i = (int)(q % P);
         const size_t row = q / P;
         const int j = (int)(row % ny), k = (int)(row / ny);
-        dvi[q] = (i < nx) ? pal_index(t, diag_of(eps_x, eps_y, eps_z, kbar2, h2, nx, ny, i, j, k)) : one;
+        dvi[q] = (i < nx) ? (unsigned char)(pal_index(t, diag_of(eps_x, eps_y, eps_z, kbar2, h2, nx, ny, i, j, k)) * scale) : one;
     }
 }
 

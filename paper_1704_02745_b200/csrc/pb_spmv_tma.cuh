@@ -45,6 +45,7 @@ struct TmaArgs {
     const T *dlut;           // PALD only: the distinct values of Dinv (256 entries)
 };
 
+__host__ __device__ inline int spmv_row_threads(int TXV) { return (TXV + 7) & ~7; }   // consumer threads per tile row
 __host__ __device__ inline size_t align128(size_t v) { return (v + 127) & ~(size_t)127; }
 
 // byte sizes of the boxes of one item (also the smem carve-up of a ring slot).  With a coefficient
@@ -179,8 +180,11 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         __syncwarp();
     } else {
         const int BWc = TXV + 2;                       // vectors per row of the haloed boxes
-        const int tx = tid % TXV, ty = tid / TXV;
-        const bool intile = ty < TY;
+        // a tile row takes a multiple of 8 threads: a quarter-warp (one 128-byte shared-memory wavefront of a 16-byte
+        // access) then never straddles two rows of the haloed boxes, whose 2-vector gap would make it a bank conflict
+        const int TXP = spmv_row_threads(TXV);
+        const int tx = tid % TXP, ty = tid / TXP;
+        const bool intile = ty < TY && tx < TXV;
         const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
         const int own_d = (ty + 1) * L.bwd + (tx + 1) * VEC;   // PALD: its byte offset in the Dinv-index box
         int lead_d = 0;                                // PALD: bytes between that box's aligned start and x0 - VEC
@@ -199,13 +203,17 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         const int extra0 = (NCT - 1 - tid < nextra) ? halo_cell(NCT - 1 - tid) : -1;   // this thread's halo cell
         auto cell_d = [&](int c) -> int { const int row = c / BWc; return row * L.bwd + (c - row * BWc) * VEC; };
         const int extra0_d = (PALD && extra0 >= 0) ? cell_d(extra0) : 0;
-        // VEC values of a 256-entry table selected by the VEC index bytes at p
+        // VEC values of a table selected by the VEC index bytes at p.  The bytes are pre-scaled byte offsets into
+        // the table (k_setup_pal_idx): one PRMT and one LDS per value.
+        auto entry = [&](const T *table, uint32_t off) -> T {
+            return *reinterpret_cast<const T *>(reinterpret_cast<const unsigned char *>(table) + off);
+        };
         auto decode = [&](const T *table, const unsigned char *p) -> Vec<T> {
             const uint32_t w = (VEC == 4) ? *reinterpret_cast<const uint32_t *>(p)
                                           : (uint32_t)*reinterpret_cast<const unsigned short *>(p);
             Vec<T> v;
 #pragma unroll
-            for (int e = 0; e < VEC; e++) v.a[e] = table[(w >> (8 * e)) & 255u];
+            for (int e = 0; e < VEC; e++) v.a[e] = entry(table, __byte_perm(w, 0u, 0x4440u + e));
             return v;
         };
         // p_new = Dinv*r + beta*p_old (steps 6-7) in place in the r box; returns the own cell's p_new
@@ -247,18 +255,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
         int lead = 0;                                  // PAL: bytes between the aligned box start and x0
         auto coef = [&](const unsigned char *box, int row, int row_vecs) -> Vec<T> {
             if (!PAL) return reinterpret_cast<const Vec<T> *>(box)[row * row_vecs + tx];
-            const unsigned char *p = box + row * L.bw + lead + tx * VEC;
-            Vec<T> v;
-            if (VEC == 4) {
-                const uint32_t w = *reinterpret_cast<const uint32_t *>(p);
-#pragma unroll
-                for (int e = 0; e < VEC; e++) v.a[e] = lut[(w >> (8 * e)) & 255u];
-            } else {
-                const uint32_t w = *reinterpret_cast<const unsigned short *>(p);
-#pragma unroll
-                for (int e = 0; e < VEC; e++) v.a[e] = lut[(w >> (8 * e)) & 255u];
-            }
-            return v;
+            return decode(lut, box + row * L.bw + lead + tx * VEC);
         };
         auto release = [&](int s) {                    // this warp is done with ring slot s
             fence_proxy_async();
@@ -319,7 +316,7 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                         for (int e = 0; e < VEC; e++) D.a[e] = rcp_rn(dinv.a[e]);
                     }
                     const Vec<T> ex = coef(slotk + L.oEX, ty, TXV + 1);
-                    const T exr = PAL ? lut[slotk[L.oEX + ty * L.bw + lead + tx * VEC + VEC]]
+                    const T exr = PAL ? entry(lut, slotk[L.oEX + ty * L.bw + lead + tx * VEC + VEC])
                                       : reinterpret_cast<const Vec<T> *>(slotk + L.oEX)[ty * (TXV + 1) + tx + 1].a[0];
                     const Vec<T> eyl = coef(slotk + L.oEY, ty, TXV), eyh = coef(slotk + L.oEY, ty + 1, TXV);
                     Vec<T> ap;
