@@ -3,6 +3,7 @@ brute-force lattice counts, the three face values a two-valued dielectric map ca
 conservation of trilinear spreading, closed-form single-charge potentials, and the analytic fixtures of
 tests/golden/born_analytic.txt."""
 import itertools
+import os
 import math
 
 import numpy as np
@@ -99,3 +100,75 @@ def test_setup_feeds_the_solver_oracle_born_ion():
     vac = pbref.PBRef(n, n, n, h, *one, None, f["rhs"], bc_vac).solve(1e-10, 2000)
     rf = sol["phi"][16, 16, 16] - vac["phi"][16, 16, 16]
     assert abs(rf - (-0.49375)) < 0.05 * 0.49375
+
+
+# ---------------------------------------------------------------------------------------------
+# Reading 9: kbar2 = eps_out * kappa_D^2, "+ kappa^2 phi" of Eq. 3 with "all the related
+# coefficients in Boltzmann term ... absorbed into kappa^2".  Pins with salt != 0 (catch kappa = sqrt(kbar2),
+# kappa = kbar2/eps_out, a dropped Boltzmann term, a wrong unit conversion of the ionic strength).
+# ---------------------------------------------------------------------------------------------
+def _kbar2_from_codata(ionic_mol_per_l, temp_k):
+    """2 N_A e^2 I / (eps0 kB T) in 1/Angstrom^2 -- CODATA-2018 constants written out here, not imported."""
+    n_a, e, eps0, k_b = 6.02214076e23, 1.602176634e-19, 8.8541878128e-12, 1.380649e-23
+    per_m2 = 2.0 * n_a * e * e * (ionic_mol_per_l * 1000.0) / (eps0 * k_b * temp_k)
+    return per_m2 * 1e-20
+
+
+def test_debye_length_of_the_configs_salt():
+    """0.15 M 1:1 salt, 300 K, eps_out = 80: Debye length 7.954 A (tests/golden/debye_length.txt), i.e.
+    kbar2 = eps_out / lambda_D^2 = 1.26456 A^-2 -- the constant workloads/ hands to both sides."""
+    from workloads import KBAR2_150MM_300K
+
+    golden = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "debye_length.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()[:2]
+                golden[k] = float(v)
+    kb = _kbar2_from_codata(0.15, 300.0)
+    assert abs(kb - golden["kbar2_150mM_300K_per_A2"]) < 5e-6
+    assert abs(math.sqrt(80.0 / kb) - golden["debye_length_A_eps80"]) < 5e-4
+    assert abs(KBAR2_150MM_300K - kb) < 1e-12
+    # textbook cross-check (water, 25 C, eps = 78.5): lambda_D = 3.04 A / sqrt(I[mol/l]) to three digits
+    assert abs(math.sqrt(78.5 / _kbar2_from_codata(1.0, 298.15)) - 3.04) < 0.01
+
+
+def test_setup_kappa_with_salt_closed_form_boundary():
+    """setup() must put kappa = sqrt(kbar2_solvent / eps_out) into the Debye-Hueckel ghost values: one charge,
+    salt on, against q exp(-r/lambda_D)/(eps_out r) with lambda_D from the CODATA formula above."""
+    nx, ny, nz, h = 7, 6, 5, 0.5
+    kb = _kbar2_from_codata(0.15, 300.0)
+    lam = math.sqrt(80.0 / kb)
+    c = np.array([[1.3, 1.1, 0.9]])
+    f = S.setup(nx, ny, nz, h, c, [1.0], [0.8], 1.0, 80.0, kb)
+    r = np.linalg.norm(S.ghost_positions(nx, ny, nz, h) - c[0], axis=1)
+    assert np.allclose(f["bc"], 0.8 * np.exp(-r / lam) / (80.0 * r), rtol=1e-13)
+    assert np.all(f["kbar2"][~f["mask"]] == kb) and np.all(f["kbar2"][f["mask"]] == 0.0)
+    # the two plausible misreadings are far outside that tolerance
+    for wrong in (math.sqrt(kb), kb / 80.0):
+        assert not np.allclose(f["bc"], 0.8 * np.exp(-wrong * r) / (80.0 * r), rtol=1e-3)
+
+
+def test_yukawa_potential_pins_the_boltzmann_term():
+    """One point charge in uniform salted solvent (eps = 80 everywhere, kbar2 = eps kappa^2 on every node): the
+    solution of Eq. 3 is the screened Coulomb potential q exp(-kappa r)/(eps r).  setup() -> Jacobi-PCG oracle must
+    reproduce it to discretisation accuracy (measured 0.8 % for r >= 3 A at h = 0.5 A; a missing '+kappa^2 phi'
+    gives 35 %, kappa = sqrt(kbar2) or kbar2/eps in the boundary values 100 % and more)."""
+    from oracle import pbref
+
+    n, h = 41, 0.5
+    kb = _kbar2_from_codata(0.15, 300.0)
+    kappa = math.sqrt(kb / 80.0)
+    c = [[10.25, 10.25, 10.25]]                        # cell centre: the general 8-node spreading, no solute node
+    f = S.setup(n, n, n, h, c, [1e-3], [1.0], 80.0, 80.0, kb)
+    assert not f["mask"].any() and np.all(f["kbar2"] == kb)
+    sol = pbref.PBRef(n, n, n, h, f["eps_x"], f["eps_y"], f["eps_z"], f["kbar2"], f["rhs"], f["bc"]).solve(1e-11, 5000)
+    z, y, x = np.meshgrid(*(np.arange(n) * h,) * 3, indexing="ij")
+    r = np.sqrt((x - c[0][0]) ** 2 + (y - c[0][1]) ** 2 + (z - c[0][2]) ** 2)
+    ana = np.exp(-kappa * r) / (80.0 * r)
+    far = r >= 3.0
+    assert sol["status"] == 0
+    assert np.max(np.abs(sol["phi"] - ana)[far] / ana[far]) < 0.015
+    # without the Boltzmann term the same boundary values give a visibly different interior
+    nosalt = pbref.PBRef(n, n, n, h, f["eps_x"], f["eps_y"], f["eps_z"], None, f["rhs"], f["bc"]).solve(1e-11, 5000)
+    assert np.max(np.abs(nosalt["phi"] - ana)[far] / ana[far]) > 0.2
