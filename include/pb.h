@@ -14,12 +14,14 @@
  * paper's right-hand side h^-3 q(i,j,k) is whatever the caller passes as `rhs`.
  *
  * All entry points are extern "C", take plain pointers and sizes, never throw or abort,
- * and return a pb_status.  There is no global state.  One handle = one operator on one
- * device and one CUDA stream.  A handle is not thread-safe; distinct handles are independent.
+ * and return a pb_status.  There is no global state: every tunable is per-handle state set with pb_set_option
+ * (the only environment variable read is PB_VERBOSE, which turns on diagnostics on stderr).  One handle = one
+ * operator on one device and one CUDA stream.  A handle is not thread-safe; distinct handles are independent.
  * There is NO CPU fallback: without a CUDA device every compute call returns PB_ERR_CUDA.
  * Determinism: every reduction has a fixed order for a fixed launch plan, so repeated solves on one handle are
- * bit-identical.  pb_create picks the SpMV plan by timing candidates (like an FFT plan), so two handles for the same
- * operator may differ in the last bits of the dot products; PB_AUTOTUNE=0 in the environment pins a static plan.
+ * bit-identical.  The SpMV plan of a precision is picked by timing candidates when its work arrays are first built
+ * (like an FFT plan), so two handles for the same operator may differ in the last bits of the dot products;
+ * pb_set_option(h, PB_OPT_AUTOTUNE, 0) pins the static plan, pb_get_plan reports the plan in use.
  *
  * Array layouts (all caller arrays are dense C arrays of fp64 unless stated otherwise):
  *   eps_x [nz][ny][nx+1]  face f lies between node i=f-1 and node i=f; the paper's
@@ -61,8 +63,10 @@ typedef enum { PB_HOST = 0, PB_DEVICE = 1 } pb_memspace;
  * pb_create -- build the operator of Eq. 3 and, if rhs or bc is given,
  * the right-hand side b of Eq. 4 with the ghost Dirichlet terms eps_f*g/h^2 folded in.
  * Inputs are COPIED (the caller may free them on return).  The handle owns all device
- * memory it allocates.  cuda_stream is a cudaStream_t (NULL = the default stream) on
- * which every later call of this handle enqueues its work.
+ * memory it allocates.  cuda_stream is a cudaStream_t on which every later call of this handle
+ * enqueues its work; NULL = the handle creates (and owns) a blocking stream of its own.
+ * pb_create only copies the inputs and checks the diagonal; the padded work arrays of a precision
+ * (and the launch plan) are built on first use or by pb_prepare.
  * Errors: nx,ny,nz < 1, h <= 0 or non-finite, NULL eps/out pointers -> PB_ERR_INVALID_ARG;
  * a node whose diagonal sum(eps_f)/h^2 + kbar2 is <= 0 or non-finite -> PB_ERR_NOT_SPD;
  * allocation / CUDA failures -> PB_ERR_ALLOC / PB_ERR_CUDA.  On error *out = NULL.
@@ -74,7 +78,9 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double h,
 
 /*
  * pb_set_rhs -- same operator, new right-hand side (Eq. 4: b = rhs + ghost fold-in).
- * Used for the many-snapshot workload the paper motivates.  Copies its inputs.
+ * Used for the many-snapshot workload the paper motivates.  Copies its inputs: the call returns
+ * after the copies are complete (host or device), so the caller may free or overwrite them.  Device inputs must be
+ * complete when the call is made (the handle's stream is not ordered against the stream that produced them).
  */
 pb_status pb_set_rhs(pb_handle *h, const double *rhs, const double *bc, pb_memspace where);
 
@@ -185,6 +191,62 @@ pb_status pb_residual(pb_handle *h, pb_precision prec, const void *phi, pb_memsp
 pb_status pb_set_boundary(pb_handle *h, int kind);
 
 /*
+ * Per-handle options ("no global state").  pb_set_option drops the work arrays and the plan of
+ * both precisions when the value changes; they are rebuilt on the next use (pb_prepare / pb_solve / ...).
+ * Invalid option or value -> PB_ERR_INVALID_ARG.
+ */
+typedef enum {
+    PB_OPT_PERSIST = 0,              /* 1 (default): grids whose working set fits the L2 run the whole loop in one
+                                        cooperative kernel; 0: always k_spmv_tma + k_vec                              */
+    PB_OPT_PERSIST_MAX_MB = 1,       /* working-set limit of that path in MB (default 100)                           */
+    PB_OPT_PERSIST_FUSED_MAX_KNODES = 2, /* below this many thousand padded nodes the two-barrier form (default 600) */
+    PB_OPT_PERSIST_BLOCKS_PER_SM = 3,/* cap on co-resident blocks of the cooperative kernel (default 4)              */
+    PB_OPT_PALETTE = 4,              /* 1 (default): face dielectrics with few distinct values stored as index bytes */
+    PB_OPT_PALETTE_DIAG = 5,         /* 1 (default): k_vec reads Dinv through the diagonal palette                   */
+    PB_OPT_PALETTE_DIAG_SPMV = 6,    /* 1 (default): k_spmv_tma too                                                  */
+    PB_OPT_AUTOTUNE = 7,             /* 1 (default): time candidate plans; 0: first feasible candidate (static)      */
+    PB_OPT_TILE_TXV = 8,             /* k_spmv_tma tile: 16-byte vectors per row (0 = automatic, default)            */
+    PB_OPT_TILE_TY = 9,              /*                  rows                                                        */
+    PB_OPT_TILE_TZ = 10,             /*                  planes per tile                                             */
+    PB_OPT_RING_SLOTS = 11,          /*                  shared-memory ring depth                                    */
+    PB_OPT_BLOCKS_PER_SM = 12,       /*                  persistent blocks per SM                                    */
+    PB_OPT_VEC_BLOCKS_PER_SM = 13,   /* k_vec blocks per SM (0 = automatic)                                          */
+    PB_OPT_GRAPH = 14,               /* 1 (default): check_every iterations are launched as one CUDA graph           */
+    PB_OPT_L2_HINTS = 15,            /* bit mask of L2 eviction-priority hints (default 0: none; measured not to help) */
+    PB_OPT_COUNT_ = 16
+} pb_option;
+
+pb_status pb_set_option(pb_handle *h, pb_option opt, int value);
+pb_status pb_get_option(pb_handle *h, pb_option opt, int *value_out);
+
+/* The launch plan of one precision (what bench.py prints and tests pin). */
+typedef struct {
+    int precision;            /* PB_F32 / PB_F64                                                        */
+    int num_sm;               /* multiprocessors of the handle's device                                */
+    int persist;              /* 1: pb_solve runs the cooperative kernel (L2-resident grid)            */
+    int persist_fused;        /*    its two-barrier form                                               */
+    int persist_grid;         /*    its grid                                                           */
+    int palette_size;         /* distinct face values (0: more than 256)                               */
+    int diag_palette_size;    /* distinct diagonal values (0: none / too many)                         */
+    int face_palette;         /* 1: this precision stores face coefficients as index bytes             */
+    int diag_palette_vec;     /* 1: k_vec reads Dinv as an index byte                                  */
+    int diag_palette_spmv;    /* 1: k_spmv_tma reads Dinv as an index byte                             */
+    int txv, ty, tz;          /* k_spmv_tma tile: vectors x rows x planes                              */
+    int ring_slots, blocks_per_sm, tiles, grid, threads, smem_bytes;
+    int autotuned;            /* 1: picked by timing, 0: static / forced                               */
+    int vec_grid, vec_threads;/* k_vec launch                                                          */
+    int spmv_bytes_per_node;  /* stored-format bytes per node and launch, as pb_bytes_per_node         */
+    int vec_bytes_per_node;
+    int pitch;                /* padded row length in elements                                         */
+    int reserved[8];
+} pb_plan;
+
+/* pb_prepare -- build the work arrays of `prec` (setup row a0: padded coefficients, diagonal, folded b) and pick
+ * the launch plan now instead of on first use.  pb_get_plan does the same and reports the plan. */
+pb_status pb_prepare(pb_handle *h, pb_precision prec);
+pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out);
+
+/*
  * pb_iterate -- benchmarking/profiling entry: enqueue exactly `n_iter` PCG iterations
  * (K_spmv + K_vec pairs, PAPER.md:115-126 steps 4-8) with the convergence latch disabled,
  * continuing from the state left by pb_solve_begin.  Does not synchronise.  Used by
@@ -208,18 +270,18 @@ long long pb_launch_count(pb_handle *h);
  * exactly as one byte per face plus a table and decoded inside the SpMV; 0 = full-precision face arrays.
  * The index bytes are stored pre-multiplied by the element size (the kernel adds them to the table address without a
  * shift), so a precision uses the palette only when size * sizeof(element) <= 256, i.e. up to 64 values in fp32 and
- * 32 in fp64 (pb_bytes_per_node tells which format a precision got).  PB_PALETTE=0 disables the palette. */
+ * 32 in fp64 (pb_bytes_per_node tells which format a precision got).  PB_OPT_PALETTE = 0 disables the palette. */
 int pb_palette_size(pb_handle *h);
 
 /* Size of the diagonal palette: with a face palette and a few-valued salt map the Jacobi diagonal also takes <= 256
  * distinct values, and k_vec then reads one index byte per node instead of a Dinv word (exact: the table holds
- * (T)(1/d)); 0 = Dinv array.  PB_PALETTE_D=0 disables it. */
+ * (T)(1/d)); 0 = Dinv array.  PB_OPT_PALETTE_DIAG = 0 disables it. */
 int pb_diag_palette_size(pb_handle *h);
 
 /* Bytes per grid node and launch that kernel `kernel` (0: k_spmv_tma, the PCG step; 1: k_vec) has to move in the
  * storage format this handle uses for `prec` -- the algorithmic bytes of bench.py's roofline:
  * k_spmv_tma reads r, p, x and writes p, x, Ap (6 words) plus Dinv (a word, or one index byte with the diagonal
- * palette; PB_PALETTE_DS=0 keeps the word) plus the three face coefficients (3 words, or 3 index bytes with the
+ * palette; PB_OPT_PALETTE_DIAG_SPMV = 0 keeps the word) plus the three face coefficients (3 words, or 3 index bytes with the
  * palette); k_vec reads r, Ap, writes r (3 words) plus Dinv (word or byte).  Builds the work arrays of `prec` if
  * they do not exist yet; -1 on error. */
 int pb_bytes_per_node(pb_handle *h, pb_precision prec, int kernel);

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     PB_F32,
     PB_F64,
     PB_HOST,
+    OPTIONS,
     PBError,
     PBSolver,
     STATUS_NAMES,

@@ -20,7 +20,23 @@ STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_E
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
-           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined", "pb_set_setup_precision")
+           "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined", "pb_set_setup_precision", "pb_set_option", "pb_get_option",
+           "pb_prepare", "pb_get_plan")
+
+# pb_option (include/pb.h), by name
+OPTIONS = {"persist": 0, "persist_max_mb": 1, "persist_fused_max_knodes": 2, "persist_blocks_per_sm": 3,
+           "palette": 4, "palette_diag": 5, "palette_diag_spmv": 6, "autotune": 7, "tile_txv": 8, "tile_ty": 9,
+           "tile_tz": 10, "ring_slots": 11, "blocks_per_sm": 12, "vec_blocks_per_sm": 13, "graph": 14, "l2_hints": 15}
+
+
+class PBPlan(ctypes.Structure):
+    """pb_plan of include/pb.h."""
+    _fields_ = [(n, ctypes.c_int) for n in (
+        "precision", "num_sm", "persist", "persist_fused", "persist_grid", "palette_size", "diag_palette_size",
+        "face_palette", "diag_palette_vec", "diag_palette_spmv", "txv", "ty", "tz", "ring_slots", "blocks_per_sm",
+        "tiles", "grid", "threads", "smem_bytes", "autotuned", "vec_grid", "vec_threads", "spmv_bytes_per_node",
+        "vec_bytes_per_node", "pitch")] + [("reserved", ctypes.c_int * 8)]
+
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
@@ -76,6 +92,10 @@ def load_library():
     lib.pb_palette_size.argtypes = [vp]
     lib.pb_diag_palette_size.argtypes = [vp]
     lib.pb_launch_count.restype = ctypes.c_longlong
+    lib.pb_set_option.argtypes = [vp, ci, ci]
+    lib.pb_get_option.argtypes = [vp, ci, ctypes.POINTER(ci)]
+    lib.pb_prepare.argtypes = [vp, ci]
+    lib.pb_get_plan.argtypes = [vp, ci, ctypes.POINTER(PBPlan)]
     for name in EXPORTS:
         getattr(lib, name)
     _lib = lib
@@ -131,7 +151,7 @@ def _prec(precision):
 class PBSolver:
     """One operator (Eq. 3) on one device/stream: pb_create ... pb_destroy."""
 
-    def __init__(self, nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2=None, rhs=None, bc=None, stream=None):
+    def __init__(self, nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2=None, rhs=None, bc=None, stream=None, options=None):
         lib = load_library()
         self.nx, self.ny, self.nz, self.h = int(nx), int(ny), int(nz), float(h)
         n = self.nx * self.ny * self.nz
@@ -151,9 +171,11 @@ class PBSolver:
         if st != PB_OK:
             self._h = None
             raise PBError(st, "pb_create")
+        self.set_options(options)
 
     @classmethod
-    def from_atoms(cls, nx, ny, nz, h, centres, radii, charges, eps_in, eps_out, kbar2_solvent, stream=None):
+    def from_atoms(cls, nx, ny, nz, h, centres, radii, charges, eps_in, eps_out, kbar2_solvent, stream=None,
+                   options=None):
         """pb_create_from_atoms: grid / stencil setup on the GPU (mask, face eps, salt map, charges, DH ghosts)."""
         lib = load_library()
         self = cls.__new__(cls)
@@ -171,7 +193,39 @@ class PBSolver:
             self._h = None
             raise PBError(st, "pb_create_from_atoms")
         self.n_atoms = na
+        self.set_options(options)
         return self
+
+    def set_option(self, name, value):
+        """pb_set_option: per-handle tunable (names in OPTIONS); drops the work arrays / plan if the value changes."""
+        st = load_library().pb_set_option(self._h, OPTIONS[name], int(value))
+        if st != PB_OK:
+            raise PBError(st, f"pb_set_option({name}, {value})")
+
+    def set_options(self, options):
+        for k, v in (options or {}).items():
+            self.set_option(k, v)
+
+    def get_option(self, name) -> int:
+        out = ctypes.c_int(0)
+        st = load_library().pb_get_option(self._h, OPTIONS[name], ctypes.byref(out))
+        if st != PB_OK:
+            raise PBError(st, "pb_get_option")
+        return out.value
+
+    def prepare(self, precision):
+        """pb_prepare: build the work arrays of a precision and pick its launch plan now."""
+        st = load_library().pb_prepare(self._h, _prec(precision)[0])
+        if st != PB_OK:
+            raise PBError(st, "pb_prepare")
+
+    def plan(self, precision) -> dict:
+        """pb_get_plan as a dict (tile, ring, grids, palettes, bytes per node)."""
+        pl = PBPlan()
+        st = load_library().pb_get_plan(self._h, _prec(precision)[0], ctypes.byref(pl))
+        if st != PB_OK:
+            raise PBError(st, "pb_get_plan")
+        return {n: getattr(pl, n) for n, _ in PBPlan._fields_ if n != "reserved"}
 
     def set_charges(self, charges):
         q, sp, keep = _marshal(charges, np.float64, self.n_atoms, "charges")

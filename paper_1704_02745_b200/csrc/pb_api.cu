@@ -30,7 +30,8 @@ struct Work {
     cudaGraphExec_t graph = nullptr;
     int graph_iters = 0;
     // TMA pipeline configuration of k_spmv_tma (tile, ring depth, persistent grid, tensor maps)
-    int qTXV = 0, qTY = 0, qTZ = 0, qntx = 0, qnty = 0, qntz = 0, qns = 0, qgrid = 0, qthreads = 0;
+    int qTXV = 0, qTY = 0, qTZ = 0, qntx = 0, qnty = 0, qntz = 0, qns = 0, qgrid = 0, qthreads = 0, qbps = 0;
+    bool qtuned = false;
     size_t qsmem = 0;
     CUtensorMap tm_r, tm_tmp, tm_dinv, tm_p0, tm_p1, tm_x, tm_ex, tm_ey, tm_ez;
     // L2-resident grids: the whole loop as one cooperative kernel (pb_persist.cuh)
@@ -70,7 +71,8 @@ struct pb_handle {
     size_t stage_bytes;
     Work<float> wf;
     Work<double> wd;
-    int use_graph;
+    int opt[PB_OPT_COUNT_];     // per-handle options (pb_set_option); no environment variables except PB_VERBOSE
+    int nsm;                     // multiprocessors of the device (cudaDevAttrMultiProcessorCount)
     long long launches;          // kernels enqueued so far (graph-contained ones included)
     int precond;                 // 1 Jacobi (default), 0 none
     int periodic;                // 0 Dirichlet ghost layer (free-space condition, default), 1 periodic
@@ -83,7 +85,6 @@ struct pb_handle {
     int n_atoms;
     double atoms_eps_out, atoms_kappa;
     bool dh_f32 = false;         // pb_set_charges evaluates the Debye-Hueckel boundary terms in fp32
-    int l2hints;                 // PB_L2HINTS (default 1): L2 eviction-priority hints across the two kernels
     int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
 };
 
@@ -93,7 +94,7 @@ namespace {
     do {                                                                       \
         cudaError_t e__ = (call);                                              \
         if (e__ != cudaSuccess) {                                              \
-            if (getenv("PB_VERBOSE"))                                          \
+            if (verbose())                                                     \
                 fprintf(stderr, "pb: %s failed: %s (%s:%d)\n", #call,          \
                         cudaGetErrorString(e__), __FILE__, __LINE__);          \
             cudaGetLastError();                                                \
@@ -119,10 +120,15 @@ template <typename T> Work<T> &work(pb_handle *h);
 template <> Work<float> &work<float>(pb_handle *h) { return h->wf; }
 template <> Work<double> &work<double>(pb_handle *h) { return h->wd; }
 
-int env_int(const char *name, int dflt)
+bool verbose() { static const bool v = getenv("PB_VERBOSE") != nullptr; return v; }
+
+void default_options(int *opt)
 {
-    const char *s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
+    opt[PB_OPT_PERSIST] = 1; opt[PB_OPT_PERSIST_MAX_MB] = 100; opt[PB_OPT_PERSIST_FUSED_MAX_KNODES] = 600;
+    opt[PB_OPT_PERSIST_BLOCKS_PER_SM] = 4; opt[PB_OPT_PALETTE] = 1; opt[PB_OPT_PALETTE_DIAG] = 1;
+    opt[PB_OPT_PALETTE_DIAG_SPMV] = 1; opt[PB_OPT_AUTOTUNE] = 1; opt[PB_OPT_TILE_TXV] = 0; opt[PB_OPT_TILE_TY] = 0;
+    opt[PB_OPT_TILE_TZ] = 0; opt[PB_OPT_RING_SLOTS] = 0; opt[PB_OPT_BLOCKS_PER_SM] = 0; opt[PB_OPT_VEC_BLOCKS_PER_SM] = 0;
+    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0;
 }
 
 inline int grid_for(size_t n, int block, int cap)
@@ -133,7 +139,6 @@ inline int grid_for(size_t n, int block, int cap)
     return (int)g;
 }
 
-constexpr int kNumSM = 148;   // B200
 
 template <typename T>
 pb_status alloc_arr(T **p, size_t n)
@@ -161,7 +166,7 @@ template <typename T>
 pb_status build_b(pb_handle *h, Work<T> &w)
 {
     const double h2 = h->h * h->h;
-    k_setup_b<T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
+    k_setup_b<T><<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(
         h->eps_x, h->eps_y, h->eps_z, h->rhs, h->periodic ? nullptr : h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
@@ -173,7 +178,9 @@ template <typename T> pb_status setup_tma(pb_handle *h, Work<T> &w);
 template <typename T> pb_status tune_vec(pb_handle *h, Work<T> &w);
 pb_status ensure_stage(pb_handle *h, size_t bytes);
 
-// Lazily build the arrays of precision T (setup row a0).
+template <typename T> pb_status build_work(pb_handle *h, Work<T> &w);
+
+// Lazily build the arrays of precision T (setup row a0).  Any failure frees what was allocated so far.
 template <typename T>
 pb_status ensure(pb_handle *h)
 {
@@ -182,6 +189,14 @@ pb_status ensure(pb_handle *h)
         if (!w.b_ready) PB_TRY(build_b<T>(h, w));
         return PB_OK;
     }
+    const pb_status s = build_work<T>(h, w);
+    if (s != PB_OK) { cudaStreamSynchronize(h->stream); cudaGetLastError(); free_work(w); }
+    return s;
+}
+
+template <typename T>
+pb_status build_work(pb_handle *h, Work<T> &w)
+{
     const int align = 32 / (int)sizeof(T);
     w.P = ((h->nx + 1 + align - 1) / align) * align;
     w.npad = (size_t)h->nz * h->ny * w.P;
@@ -189,14 +204,14 @@ pb_status ensure(pb_handle *h)
     // distinct face values of the operator -> palette or full-precision face arrays (decided once per handle)
     if (h->pal_n < 0) {
         h->pal_n = 0;
-        if (env_int("PB_PALETTE", 1)) {
+        if (h->opt[PB_OPT_PALETTE]) {
             if (!h->pal_table) PB_ALLOC(cudaMalloc((void **)&h->pal_table, sizeof(PalTable)));
             k_pal_reset<<<1, 256, 0, h->stream>>>(h->pal_table);
             const size_t ns[3] = {(size_t)h->nz * h->ny * (h->nx + 1), (size_t)h->nz * (h->ny + 1) * h->nx,
                                   (size_t)(h->nz + 1) * h->ny * h->nx};
             const double *arrs[3] = {h->eps_x, h->eps_y, h->eps_z};
             for (int a = 0; a < 3; a++)
-                k_pal_collect<<<grid_for(ns[a], 256, kNumSM * 8), 256, 0, h->stream>>>(arrs[a], ns[a], h->pal_table);
+                k_pal_collect<<<grid_for(ns[a], 256, h->nsm * 8), 256, 0, h->stream>>>(arrs[a], ns[a], h->pal_table);
             k_pal_finish<<<1, 256, 0, h->stream>>>(h->pal_table);
             PB_CUDA(cudaGetLastError());
             int n = 0;
@@ -208,10 +223,10 @@ pb_status ensure(pb_handle *h)
     }
     if (h->pald_n < 0) {
         h->pald_n = 0;
-        if (h->pal_n > 0 && env_int("PB_PALETTE_D", 1)) {     // few face values -> few diagonals (unless kbar2 varies)
+        if (h->pal_n > 0 && h->opt[PB_OPT_PALETTE_DIAG]) {     // few face values -> few diagonals (unless kbar2 varies)
             if (!h->pald_table) PB_ALLOC(cudaMalloc((void **)&h->pald_table, sizeof(PalTable)));
             k_pal_reset<<<1, 256, 0, h->stream>>>(h->pald_table);
-            k_pal_collect_diag<<<grid_for((size_t)h->nx * h->ny * h->nz, 256, kNumSM * 8), 256, 0, h->stream>>>(
+            k_pal_collect_diag<<<grid_for((size_t)h->nx * h->ny * h->nz, 256, h->nsm * 8), 256, 0, h->stream>>>(
                 h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, h->pald_table);
             k_pal_finish<<<1, 256, 0, h->stream>>>(h->pald_table);
             PB_CUDA(cudaGetLastError());
@@ -225,14 +240,14 @@ pb_status ensure(pb_handle *h)
     // k_spmv_tma decodes through tables addressed by pre-scaled index bytes: n * sizeof(T) <= 256 entries-bytes
     w.pal = h->pal_n > 0 && (size_t)h->pal_n * sizeof(T) <= 256;
     w.pald = w.pal && h->pald_n > 0;
-    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && env_int("PB_PALETTE_DS", 1) != 0;
+    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
     w.Pb = (w.P + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
         const double mb = 11.0 * (double)w.npad * sizeof(T) / 1.0e6;
-        w.persist = coop && env_int("PB_PERSIST", 1) != 0 && mb <= (double)env_int("PB_PERSIST_MAX_MB", 100);
+        w.persist = coop && h->opt[PB_OPT_PERSIST] != 0 && mb <= (double)h->opt[PB_OPT_PERSIST_MAX_MB];
     }
     pb_status s = PB_OK;
     if (w.pal && w.persist &&
@@ -260,18 +275,19 @@ pb_status ensure(pb_handle *h)
         free_work(w);
         return s;
     }
-    w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, kNumSM * env_int("PB_VEC_BPS", 4));   // 2 vectors per thread and pass
+    w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, h->nsm * (h->opt[PB_OPT_VEC_BLOCKS_PER_SM] > 0 ? h->opt[PB_OPT_VEC_BLOCKS_PER_SM] : 4));   // 2 vectors per thread and pass
     if (w.persist) {
         // tiny grids: barriers dominate -> the two-barrier form that recomputes p at the neighbours
-        w.pfused = (double)w.npad <= (double)env_int("PB_PERSIST_FUSED_MAX_KNODES", 600) * 1.0e3;
+        w.pfused = (double)w.npad <= (double)h->opt[PB_OPT_PERSIST_FUSED_MAX_KNODES] * 1.0e3;
         int bps = 0;
-        if (w.pfused) PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T, true>, 256, 0));
-        else PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T, false>, 256, 0));
-        if (bps < 1) w.persist = false;
-        bps = bps > env_int("PB_PERSIST_BPS", 4) ? env_int("PB_PERSIST_BPS", 4) : bps;
-        w.pgrid = grid_for(w.npad / VecN<T>::value, 256, kNumSM * bps);
+        const cudaError_t eo = w.pfused ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T, true>, 256, 0)
+                                        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pcg_persistent<T, false>, 256, 0);
+        if (eo != cudaSuccess) { cudaGetLastError(); bps = 0; }
+        if (bps < 1) { w.persist = false; bps = 1; }      // no co-residency on this device/partition: two-kernel path
+        bps = bps > h->opt[PB_OPT_PERSIST_BLOCKS_PER_SM] ? h->opt[PB_OPT_PERSIST_BLOCKS_PER_SM] : bps;
+        w.pgrid = grid_for(w.npad / VecN<T>::value, 256, h->nsm * bps);
     }
-    size_t need = (size_t)kNumSM * 16 > (size_t)2 * w.vec_grid ? (size_t)kNumSM * 16 : (size_t)2 * w.vec_grid;
+    size_t need = (size_t)h->nsm * 16 > (size_t)2 * w.vec_grid ? (size_t)h->nsm * 16 : (size_t)2 * w.vec_grid;
     if ((size_t)3 * w.pgrid > need) need = (size_t)3 * w.pgrid;
     if (need > h->partials_cap) {
         if (h->partials) cudaFree(h->partials);
@@ -282,22 +298,22 @@ pb_status ensure(pb_handle *h)
     }
     PB_CUDA(cudaMemsetAsync(h->bad, 0, sizeof(int), h->stream));
     const size_t total = (size_t)(h->nz + 1) * (h->ny + 1) * w.P;
-    k_setup_coeff<T><<<grid_for(total, 256, kNumSM * 16), 256, 0, h->stream>>>(
+    k_setup_coeff<T><<<grid_for(total, 256, h->nsm * 16), 256, 0, h->stream>>>(
         h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
         w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
     if (w.pal) {
-        k_setup_pal_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pb, 256, kNumSM * 16), 256, 0, h->stream>>>(
+        k_setup_pal_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
             h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pal_table, w.exi, w.eyi, w.ezi);
         k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
         h->launches += 2;
     }
     if (w.pald) {
-        k_setup_diag_idx<<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(
+        k_setup_diag_idx<<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(
             h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P, 1, h->pald_table, w.dvi);
         k_pal_lut_dinv<T><<<1, 256, 0, h->stream>>>(h->pald_table, w.dlut);
         h->launches += 2;
         if (w.pald_s) {
-            k_setup_diag_idx<<<grid_for((size_t)h->nz * h->ny * w.Pb, 256, kNumSM * 16), 256, 0, h->stream>>>(
+            k_setup_diag_idx<<<grid_for((size_t)h->nz * h->ny * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
                 h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pald_table, w.dvib);
             h->launches += 1;
         }
@@ -315,7 +331,7 @@ template <typename T>
 VecArgs<T> vec_args(pb_handle *h, Work<T> &w)
 {
     VecArgs<T> a;
-    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.l2hints = h->l2hints; a.precond = h->precond; a.dvi = w.dvi; a.dlut = w.dlut; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
+    a.r = w.r; a.Ap = w.Ap; a.Dinv = w.Dinv; a.b = w.b; a.x = w.x; a.pzero = w.p0; a.l2hints = h->opt[PB_OPT_L2_HINTS]; a.precond = h->precond; a.dvi = w.dvi; a.dlut = w.dlut; a.nvec = w.npad / VecN<T>::value; a.st = h->st; a.partials = h->partials;
     return a;
 }
 
@@ -354,7 +370,7 @@ pb_status make_map(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, i
                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
-        if (getenv("PB_VERBOSE")) fprintf(stderr, "pb: cuTensorMapEncodeTiled failed (%d)\n", (int)r);
+        if (verbose()) fprintf(stderr, "pb: cuTensorMapEncodeTiled failed (%d)\n", (int)r);
         return PB_ERR_CUDA;
     }
     return PB_OK;
@@ -384,14 +400,14 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     constexpr int VEC = VecN<T>::value;
     const int rowvecs = w.P / VEC;
     const int TXV = c.TXV, TY = c.TY, NS = c.NS;
-    w.qTXV = TXV; w.qTY = TY; w.qns = NS;
+    w.qTXV = TXV; w.qTY = TY; w.qns = NS; w.qbps = c.bps;
     w.qntx = (rowvecs + TXV - 1) / TXV;
     w.qnty = (h->ny + TY - 1) / TY;
     w.qthreads = (spmv_row_threads(TXV) * TY + 31) / 32 * 32 + 32;
     const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0, w.pald_s);
     w.qsmem = (size_t)NS * L.slot + 128;
     if (w.qsmem > w.qmaxdyn || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
-    const int slots = kNumSM * c.bps;
+    const int slots = h->nsm * c.bps;
     const int xy = w.qntx * w.qnty;
     int TZ = c.TZ;
     if (TZ <= 0) {
@@ -476,21 +492,24 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
     while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
     TileCfg cand[64];
     int nc = 0;
-    const bool forced = getenv("PB_TXV") || getenv("PB_TY") || getenv("PB_NS") || getenv("PB_BPS") || getenv("PB_TZ");
+    const int *o = h->opt;
+    auto opt_or = [&](pb_option k, int dflt) { return o[k] > 0 ? o[k] : dflt; };
+    const bool forced = o[PB_OPT_TILE_TXV] > 0 || o[PB_OPT_TILE_TY] > 0 || o[PB_OPT_RING_SLOTS] > 0 ||
+                        o[PB_OPT_BLOCKS_PER_SM] > 0 || o[PB_OPT_TILE_TZ] > 0;
     if (forced) {
         TileCfg c;
-        c.TXV = env_int("PB_TXV", (rowvecs + ntx0 - 1) / ntx0);
+        c.TXV = opt_or(PB_OPT_TILE_TXV, (rowvecs + ntx0 - 1) / ntx0);
         if (c.TXV < 1) c.TXV = 1;
         if (c.TXV > maxv) c.TXV = maxv;
         if (c.TXV > rowvecs) c.TXV = rowvecs;
-        c.TY = env_int("PB_TY", 4);
+        c.TY = opt_or(PB_OPT_TILE_TY, 4);
         if (c.TY < 1) c.TY = 1;
         if (c.TY > h->ny) c.TY = h->ny;
         while (spmv_row_threads(c.TXV) * c.TY > 448 && c.TY > 1) c.TY--;
-        c.bps = env_int("PB_BPS", ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s) >= 4 ? 2 : 1);
+        c.bps = opt_or(PB_OPT_BLOCKS_PER_SM, ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s) >= 4 ? 2 : 1);
         if (c.bps < 1) c.bps = 1;
-        c.NS = env_int("PB_NS", ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s));
-        c.TZ = env_int("PB_TZ", 0);
+        c.NS = opt_or(PB_OPT_RING_SLOTS, ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s));
+        c.TZ = o[PB_OPT_TILE_TZ];
         cand[nc++] = c;
     } else {
         static const int tys[] = {8, 4, 6, 3, 2};
@@ -513,7 +532,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         if (nc == 0) cand[nc++] = TileCfg{(rowvecs + ntx0 - 1) / ntx0, h->ny < 4 ? h->ny : 4, 4, 1, 0};
     }
     int best = 0;
-    const bool tune = nc > 1 && env_int("PB_AUTOTUNE", 1) != 0 && (double)h->nx * h->ny * h->nz >= 2.0e5;
+    const bool tune = nc > 1 && h->opt[PB_OPT_AUTOTUNE] != 0 && (double)h->nx * h->ny * h->nz >= 2.0e5;
     if (tune) {
         cudaEvent_t e0, e1;
         PB_CUDA(cudaEventCreate(&e0));
@@ -539,7 +558,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
             }
             float ms = 0.f;
             cudaEventElapsedTime(&ms, e0, e1);
-            if (getenv("PB_VERBOSE"))
+            if (verbose())
                 fprintf(stderr, "pb: tune TXV=%d TY=%d NS=%d bps=%d TZ=%d grid=%d: %.4f ms\n", cand[i].TXV, cand[i].TY,
                         cand[i].NS, cand[i].bps, w.qTZ, w.qgrid, ms / 3);
             tms[i] = ms;
@@ -571,7 +590,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
                 }
                 float ms = 0.f;
                 cudaEventElapsedTime(&ms, e0, e1);
-                if (getenv("PB_VERBOSE"))
+                if (verbose())
                     fprintf(stderr, "pb: tune (pass 2) TXV=%d TY=%d NS=%d bps=%d: %.4f ms per iteration\n", cand[fin[f]].TXV,
                             cand[fin[f]].TY, cand[fin[f]].NS, cand[fin[f]].bps, ms / 12);
                 if (ms < tbest) { tbest = ms; best = fin[f]; }
@@ -581,7 +600,8 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         cudaEventDestroy(e1);
     }
     PB_TRY(configure_tma<T>(h, w, cand[best]));
-    if (getenv("PB_VERBOSE"))
+    w.qtuned = tune;
+    if (verbose())
         fprintf(stderr, "pb: palette %d (diagonal %d); k_spmv_tma<%s> TXV=%d TY=%d TZ=%d NS=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
                 h->pal_n, w.pald_s ? h->pald_n : 0, sizeof(T) == 4 ? "f32" : "f64", w.qTXV, w.qTY, w.qTZ, w.qns, cand[best].bps,
                 w.qntx * w.qnty * w.qntz, w.qgrid, w.qthreads, w.qsmem, tune ? " (autotuned)" : "");
@@ -596,7 +616,7 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.pbuf0 = w.p0; a.pbuf1 = w.p1; a.Ap = w.Ap; a.x = w.x;
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
     a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
-    a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->l2hints; a.precond = h->precond;
+    a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->opt[PB_OPT_L2_HINTS]; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
     a.lut = w.lut; a.dlut = w.dlut;
     if (w.pald_s)
@@ -615,7 +635,7 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
 template <typename T>
 pb_status tune_vec(pb_handle *h, Work<T> &w)
 {
-    if (getenv("PB_VEC_BPS") || env_int("PB_AUTOTUNE", 1) == 0 || (double)h->nx * h->ny * h->nz < 2.0e6) return PB_OK;
+    if (h->opt[PB_OPT_VEC_BLOCKS_PER_SM] > 0 || h->opt[PB_OPT_AUTOTUNE] == 0 || (double)h->nx * h->ny * h->nz < 2.0e6) return PB_OK;
     cudaEvent_t e0, e1;
     PB_CUDA(cudaEventCreate(&e0));
     PB_CUDA(cudaEventCreate(&e1));
@@ -626,7 +646,7 @@ pb_status tune_vec(pb_handle *h, Work<T> &w)
     float tbest = 1e30f;
     int best = w.vec_grid;
     for (int c : cand) {
-        w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, kNumSM * c);
+        w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, h->nsm * c);
         if ((size_t)2 * w.vec_grid > h->partials_cap) continue;
         const VecArgs<T> va = vec_args<T>(h, w);
         auto launch = [&]() {
@@ -643,7 +663,7 @@ pb_status tune_vec(pb_handle *h, Work<T> &w)
         }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
-        if (getenv("PB_VERBOSE")) fprintf(stderr, "pb: tune k_vec %d blocks/SM (grid %d): %.4f ms\n", c, w.vec_grid, ms / 3);
+        if (verbose()) fprintf(stderr, "pb: tune k_vec %d blocks/SM (grid %d): %.4f ms\n", c, w.vec_grid, ms / 3);
         if (ms < tbest) { tbest = ms; best = w.vec_grid; }
     }
     cudaEventDestroy(e0);
@@ -663,7 +683,7 @@ void launch_wrap(pb_handle *h, Work<T> &w, double out_scale)
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P; a.out_scale = out_scale;
     a.st = h->st; a.partials = h->partials;
     const size_t shell = 2 * ((size_t)h->ny * h->nx + (size_t)h->nz * h->nx + (size_t)h->nz * h->ny);
-    k_wrap<T, MODE><<<grid_for(shell, 256, kNumSM * 8), 256, 0, h->stream>>>(a);
+    k_wrap<T, MODE><<<grid_for(shell, 256, h->nsm * 8), 256, 0, h->stream>>>(a);
     h->launches += 1;
 }
 
@@ -702,7 +722,7 @@ pb_status begin_solve(pb_handle *h, double tol, int maxiter, int latch, const vo
             PB_CUDA(cudaMemcpyAsync(h->stage, phi0, n * sizeof(T), cudaMemcpyHostToDevice, h->stream));
             src = (const T *)h->stage;
         }
-        k_pad<T, T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
+        k_pad<T, T><<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
         launch_spmv<T, 1>(h, w, 1.0);                      // Ap = A' phi_0
         launch_wrap<T, 1>(h, w, 1.0);
         k_warm<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w), w.tmp);
@@ -757,10 +777,16 @@ pb_status run_solve(pb_handle *h, double tol, int maxiter, int check_every, cons
         pa.st = h->st; pa.partials = h->partials;
         void *kargs[] = {(void *)&pa};
         const void *fn = w.pfused ? (const void *)k_pcg_persistent<T, true> : (const void *)k_pcg_persistent<T, false>;
-        PB_CUDA(cudaLaunchCooperativeKernel(fn, dim3(w.pgrid), dim3(256), kargs, 0, h->stream));
-        h->launches += 1;
+        if (cudaLaunchCooperativeKernel(fn, dim3(w.pgrid), dim3(256), kargs, 0, h->stream) == cudaSuccess) {
+            h->launches += 1;
+        } else {
+            // e.g. fewer SMs available than the occupancy query promised (MPS / MIG): fall back for good
+            cudaGetLastError();
+            if (verbose()) fprintf(stderr, "pb: cooperative launch refused, using the two-kernel path\n");
+            w.persist = false;
+        }
     }
-    bool graph_ok = !w.persist && h->use_graph && get_graph<T>(h, w, m) == PB_OK;
+    bool graph_ok = !w.persist && h->opt[PB_OPT_GRAPH] && get_graph<T>(h, w, m) == PB_OK;
     // chunk c is enqueued before the latch of chunk c-1 is waited for, so the device never idles
     const long max_chunks = (long)maxiter / m + 2;
     int seen_done = w.persist ? 1 : 0;
@@ -788,7 +814,7 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
     T *dst = (T *)phi_out;
     if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(T))); dst = (T *)h->stage; }
-    k_finish<T, T><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(w.x, w.p0, w.p1, h->st, dst, h->nx, w.P, rows);
+    k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.x, w.p0, w.p1, h->st, dst, h->nx, w.P, rows);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     if (where == PB_HOST)
@@ -824,7 +850,7 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
         launch_spmv<double, 1>(h, wd, 1.0);
         launch_wrap<double, 1>(h, wd, 1.0);
         k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
-        k_true_residual<double><<<grid_for(nvec_d, 256, kNumSM * 4), 256, 0, h->stream>>>(wd.b, wd.Ap, nvec_d, h->st,
+        k_true_residual<double><<<grid_for(nvec_d, 256, h->nsm * 4), 256, 0, h->stream>>>(wd.b, wd.Ap, nvec_d, h->st,
                                                                                           h->partials, wd.r);
         PB_CUDA(cudaGetLastError());
         h->launches += 3;
@@ -839,14 +865,14 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
         double tin = 0.3 * tol / relres;
         if (tin < inner_tol) tin = inner_tol;
         if (tin > 0.1) tin = 0.1;
-        k_repad<double, float><<<grid_for(wf.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(wd.r, wd.P, wf.b, wf.P,
+        k_repad<double, float><<<grid_for(wf.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(wd.r, wd.P, wf.b, wf.P,
                                                                                            h->nx, rows);
         h->launches += 1;
         wf.b_ready = true;
         const pb_status rs = run_solve<float>(h, tin, maxiter - total, check_every, nullptr, PB_DEVICE);
         wf.b_ready = false;                      // wf.b holds a residual, not b: rebuilt before the next plain solve
         if (rs != PB_OK) return rs;
-        k_finish_add<float, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(
+        k_finish_add<float, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
             wf.x, wf.p0, wf.p1, h->st, wd.tmp, h->nx, wf.P, wd.P, rows);
         PB_CUDA(cudaGetLastError());
         h->launches += 1;
@@ -858,7 +884,7 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
     h->last_prec = PB_F64;
     double *dst = phi_out;
     if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(double))); dst = (double *)h->stage; }
-    k_unpad<double, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(wd.tmp, dst, h->nx, wd.P, rows, 1.0);
+    k_unpad<double, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(wd.tmp, dst, h->nx, wd.P, rows, 1.0);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     if (where == PB_HOST)
@@ -884,7 +910,7 @@ pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
         src = (const T *)h->stage;
         dst = (T *)h->stage;
     }
-    const int g = grid_for(w.npad, 256, kNumSM * 16);
+    const int g = grid_for(w.npad, 256, h->nsm * 16);
     k_pad<T, T><<<g, 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
     launch_spmv<T, 1>(h, w, 1.0 / (h->h * h->h));
     launch_wrap<T, 1>(h, w, 1.0 / (h->h * h->h));
@@ -921,11 +947,11 @@ pb_status residual_impl(pb_handle *h, const void *phi, pb_memspace where, double
         PB_CUDA(cudaMemcpyAsync(h->stage, phi, n * sizeof(T), cudaMemcpyHostToDevice, h->stream));
         src = (const T *)h->stage;
     }
-    k_pad<T, T><<<grid_for(w.npad, 256, kNumSM * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
+    k_pad<T, T><<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
     launch_spmv<T, 1>(h, w, 1.0);
     launch_wrap<T, 1>(h, w, 1.0);
     k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
-    k_true_residual<T><<<grid_for(w.npad / VecN<T>::value, 256, kNumSM * 4), 256, 0, h->stream>>>(
+    k_true_residual<T><<<grid_for(w.npad / VecN<T>::value, 256, h->nsm * 4), 256, 0, h->stream>>>(
         w.b, w.Ap, w.npad / VecN<T>::value, h->st, h->partials);
     PB_CUDA(cudaGetLastError());
     h->launches += 4;
@@ -1041,14 +1067,15 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
     pb_handle *h = new (std::nothrow) pb_handle();
     if (!h) return PB_ERR_ALLOC;
     h->nx = nx; h->ny = ny; h->nz = nz; h->h = hh;
-    h->use_graph = env_int("PB_NO_GRAPH", 0) ? 0 : 1;
-    h->l2hints = env_int("PB_L2HINTS", 0);
+    default_options(h->opt);
     h->precond = 1;
     h->pal_n = -1;
     h->pald_n = -1;
     pb_status s = PB_OK;
     auto body = [&]() -> pb_status {
         PB_CUDA(cudaGetDevice(&h->device));
+        PB_CUDA(cudaDeviceGetAttribute(&h->nsm, cudaDevAttrMultiProcessorCount, h->device));
+        if (h->nsm < 1) return PB_ERR_CUDA;
         if (cuda_stream) { h->stream = (cudaStream_t)cuda_stream; h->own_stream = false; }
         else { PB_CUDA(cudaStreamCreate(&h->stream)); h->own_stream = true; }   // blocking: orders with stream 0
         PB_ALLOC(cudaMalloc((void **)&h->st, sizeof(State)));
@@ -1065,8 +1092,13 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
         PB_TRY(take_copy(h, &h->kbar2, kbar2, n, where));
         PB_TRY(take_copy(h, &h->rhs, rhs, n, where));
         PB_TRY(take_copy(h, &h->bc, bc, 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx), where));
-        // the fp64 operator is always built: it carries the SPD check of the diagonal
-        PB_TRY(ensure<double>(h));
+        // SPD check on the diagonal alone; the padded work arrays of a precision and its launch
+        // plan are built on first use (or by pb_prepare), so an fp32-only caller never pays for the fp64 set
+        PB_CUDA(cudaMemsetAsync(h->bad, 0, sizeof(int), h->stream));
+        k_check_diag<<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(h->eps_x, h->eps_y, h->eps_z, h->kbar2,
+                                                                        hh * hh, nx, ny, nz, h->bad);
+        PB_CUDA(cudaGetLastError());
+        h->launches += 1;
         int bad = 0;
         PB_CUDA(cudaMemcpyAsync(&bad, h->bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
         PB_CUDA(cudaStreamSynchronize(h->stream));
@@ -1090,7 +1122,77 @@ pb_status pb_set_rhs(pb_handle *h, const double *rhs, const double *bc, pb_memsp
     h->wd.b_ready = false;
     if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));
     if (h->wd.ready) PB_TRY(build_b<double>(h, h->wd));
-    if (where == PB_HOST) PB_CUDA(cudaStreamSynchronize(h->stream));   // caller may free on return
+    PB_CUDA(cudaStreamSynchronize(h->stream));   // the inputs are copied: the caller may free or overwrite them on return
+    return PB_OK;
+}
+
+pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
+{
+    if (!h || (int)opt < 0 || (int)opt >= (int)PB_OPT_COUNT_ || value < 0) return PB_ERR_INVALID_ARG;
+    switch (opt) {
+    case PB_OPT_PERSIST: case PB_OPT_PALETTE: case PB_OPT_PALETTE_DIAG: case PB_OPT_PALETTE_DIAG_SPMV:
+    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH:
+        if (value > 1) return PB_ERR_INVALID_ARG;
+        break;
+    case PB_OPT_PERSIST_BLOCKS_PER_SM:
+        if (value < 1 || value > 32) return PB_ERR_INVALID_ARG;
+        break;
+    case PB_OPT_RING_SLOTS:
+        if (value != 0 && (value < 3 || value > kMaxStages)) return PB_ERR_INVALID_ARG;
+        break;
+    case PB_OPT_BLOCKS_PER_SM: case PB_OPT_VEC_BLOCKS_PER_SM:
+        if (value > 32) return PB_ERR_INVALID_ARG;
+        break;
+    default: break;
+    }
+    if (h->opt[opt] == value) return PB_OK;
+    PB_CUDA(cudaSetDevice(h->device));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    h->opt[opt] = value;
+    // work arrays, palettes and plans depend on the options: drop them, the next use rebuilds
+    free_work(h->wf);
+    free_work(h->wd);
+    h->pal_n = -1;
+    h->pald_n = -1;
+    return PB_OK;
+}
+
+pb_status pb_get_option(pb_handle *h, pb_option opt, int *value_out)
+{
+    if (!h || !value_out || (int)opt < 0 || (int)opt >= (int)PB_OPT_COUNT_) return PB_ERR_INVALID_ARG;
+    *value_out = h->opt[opt];
+    return PB_OK;
+}
+
+pb_status pb_prepare(pb_handle *h, pb_precision prec)
+{
+    if (!h || !valid_prec(prec)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    PB_TRY(prec == PB_F32 ? ensure<float>(h) : ensure<double>(h));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}
+
+pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
+{
+    if (!h || !out || !valid_prec(prec)) return PB_ERR_INVALID_ARG;
+    PB_TRY(pb_prepare(h, prec));
+    memset(out, 0, sizeof(*out));
+    out->precision = (int)prec;
+    out->num_sm = h->nsm;
+    out->palette_size = h->pal_n > 0 ? h->pal_n : 0;
+    out->diag_palette_size = h->pald_n > 0 ? h->pald_n : 0;
+    auto fill = [&](const auto &w) {
+        out->persist = w.persist; out->persist_fused = w.persist && w.pfused; out->persist_grid = w.persist ? w.pgrid : 0;
+        out->face_palette = w.pal; out->diag_palette_vec = w.pald; out->diag_palette_spmv = w.pald_s;
+        out->txv = w.qTXV; out->ty = w.qTY; out->tz = w.qTZ; out->ring_slots = w.qns; out->blocks_per_sm = w.qbps;
+        out->tiles = w.qntx * w.qnty * w.qntz; out->grid = w.qgrid; out->threads = w.qthreads;
+        out->smem_bytes = (int)w.qsmem; out->autotuned = w.qtuned;
+        out->vec_grid = w.vec_grid; out->vec_threads = 256; out->pitch = w.P;
+    };
+    if (prec == PB_F32) fill(h->wf); else fill(h->wd);
+    out->spmv_bytes_per_node = pb_bytes_per_node(h, prec, 0);
+    out->vec_bytes_per_node = pb_bytes_per_node(h, prec, 1);
     return PB_OK;
 }
 
@@ -1222,7 +1324,7 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
     const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
     PB_TRY(ensure_stage(h, n * sizeof(double)));
     if (what >= 3) {   // work vectors of the last solve, h^2-scaled system, converted to fp64
-        const int g = grid_for(n, 256, kNumSM * 16);
+        const int g = grid_for(n, 256, h->nsm * 16);
         if (h->last_prec == PB_F32) {
             Work<float> &w = h->wf;
             if (!w.ready) return PB_ERR_INVALID_ARG;
@@ -1247,7 +1349,7 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
     }
     PB_TRY(ensure<double>(h));
     Work<double> &w = h->wd;
-    k_unpad<double, double><<<grid_for(n, 256, kNumSM * 16), 256, 0, h->stream>>>(
+    k_unpad<double, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
         what == 0 ? w.D : w.b, (double *)h->stage, h->nx, w.P, rows, 1.0 / (h->h * h->h));
     PB_CUDA(cudaGetLastError());
     PB_CUDA(cudaMemcpyAsync(out_host, h->stage, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -1287,16 +1389,21 @@ struct DevTmp {                      // frees its device allocations on scope ex
     void release(void *q) { for (int i = 0; i < n; i++) if (p[i] == q) p[i] = nullptr; }
 };
 
-// rhs (dense [nz][ny][nx]) and bc from charges on the stored / given atom geometry
+// rhs (dense [nz][ny][nx]) and bc from charges on the stored / given atom geometry.  `scratch` = one double
+// (sum |q|) followed by one int (the bad-atom flag), device.
 pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
-                            double eps_out, double kappa, double *d_rhs, double *d_bc, cudaStream_t st,
-                            bool dh_f32 = false)
+                            double eps_out, double kappa, double *d_rhs, double *d_bc, double *scratch, int nsm,
+                            cudaStream_t st, bool dh_f32 = false)
 {
     const size_t n = (size_t)nx * ny * nz;
     const size_t nbc = 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx);
+    int *d_bad = reinterpret_cast<int *>(scratch + 1);
+    PB_CUDA(cudaMemsetAsync(scratch, 0, 2 * sizeof(double), st));
     PB_CUDA(cudaMemsetAsync(d_rhs, 0, n * sizeof(double), st));
-    k_grid_spread<<<grid_for((size_t)n_atoms, 128, kNumSM * 8), 128, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh, d_rhs);
-    k_grid_rhs<<<grid_for(n, 256, kNumSM * 16), 256, 0, st>>>(d_rhs, n, 4.0 * 3.141592653589793, pow(hh, 3.0));
+    k_grid_check<<<1, 1024, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh, scratch, d_bad);
+    k_grid_spread<<<grid_for((size_t)n_atoms, 128, nsm * 8), 128, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh, scratch,
+                                                                         reinterpret_cast<long long *>(d_rhs));
+    k_grid_rhs<<<grid_for(n, 256, nsm * 16), 256, 0, st>>>(d_rhs, n, 4.0 * 3.141592653589793, pow(hh, 3.0), scratch);
     if (dh_f32)
         k_grid_dh_f32<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
                                                                                     eps_out, kappa, d_bc);
@@ -1304,7 +1411,10 @@ pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, i
         k_grid_dh<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
                                                                                 eps_out, kappa, d_bc);
     PB_CUDA(cudaGetLastError());
-    return PB_OK;
+    int bad = 0;
+    PB_CUDA(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    return bad ? PB_ERR_INVALID_ARG : PB_OK;      // an atom outside the box [0,(n-1)h]^3 or a non-finite charge
 }
 }  // namespace
 
@@ -1325,9 +1435,13 @@ extern "C" pb_status pb_create_from_atoms(pb_handle **out, int nx, int ny, int n
     const size_t n = (size_t)nx * ny * nz;
     const size_t nbc = 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx);
     const cudaMemcpyKind kind = where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    int dev = 0, nsm = 0;
+    PB_CUDA(cudaGetDevice(&dev));
+    PB_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
     DevTmp tmp;
-    double *d_c, *d_R, *d_q, *ex, *ey, *ez, *kb, *rhs, *bc;
+    double *d_c, *d_R, *d_q, *ex, *ey, *ez, *kb, *rhs, *bc, *scratch;
     unsigned char *mask;
+    PB_TRY(tmp.get((void **)&scratch, 2 * sizeof(double)));
     PB_TRY(tmp.get((void **)&d_c, (size_t)n_atoms * 3 * sizeof(double)));
     PB_TRY(tmp.get((void **)&d_R, (size_t)n_atoms * sizeof(double)));
     PB_TRY(tmp.get((void **)&d_q, (size_t)n_atoms * sizeof(double)));
@@ -1346,16 +1460,16 @@ extern "C" pb_status pb_create_from_atoms(pb_handle **out, int nx, int ny, int n
     PB_CUDA(cudaMemsetAsync(mask, 0, n, st));
     if (n_atoms) k_grid_mask<<<n_atoms < 65535 ? n_atoms : 65535, 128, 0, st>>>(d_c, d_R, n_atoms, nx, ny, nz, hh, mask);
     const size_t nf = (size_t)(nz + 1) * (ny + 1) * (nx + 1);
-    k_grid_faces<<<grid_for(nf, 256, kNumSM * 16), 256, 0, st>>>(mask, nx, ny, nz, eps_in, eps_out, kbar2_solvent,
+    k_grid_faces<<<grid_for(nf, 256, nsm * 16), 256, 0, st>>>(mask, nx, ny, nz, eps_in, eps_out, kbar2_solvent,
                                                                  ex, ey, ez, kb);
     PB_CUDA(cudaGetLastError());
     const double kappa = sqrt(kbar2_solvent / eps_out);
-    PB_TRY(charges_to_rhs_bc(d_c, d_q, n_atoms, nx, ny, nz, hh, eps_out, kappa, rhs, bc, st));
+    PB_TRY(charges_to_rhs_bc(d_c, d_q, n_atoms, nx, ny, nz, hh, eps_out, kappa, rhs, bc, scratch, nsm, st));
     pb_handle *h = nullptr;
     PB_TRY(pb_create(&h, nx, ny, nz, hh, ex, ey, ez, kb, rhs, bc, PB_DEVICE, cuda_stream));
     h->atoms_c = d_c; tmp.release(d_c);
     h->n_atoms = n_atoms; h->atoms_eps_out = eps_out; h->atoms_kappa = kappa;
-    h->launches += 5;
+    h->launches += 6;
     *out = h;
     return PB_OK;
 }
@@ -1367,15 +1481,16 @@ extern "C" pb_status pb_set_charges(pb_handle *h, const double *charges, pb_mems
     const size_t n = (size_t)h->nx * h->ny * h->nz;
     const size_t nbc = 2 * ((size_t)h->nz * h->ny + (size_t)h->nz * h->nx + (size_t)h->ny * h->nx);
     DevTmp tmp;
-    double *d_q;
+    double *d_q, *scratch;
     PB_TRY(tmp.get((void **)&d_q, (size_t)h->n_atoms * sizeof(double)));
+    PB_TRY(tmp.get((void **)&scratch, 2 * sizeof(double)));
     PB_CUDA(cudaMemcpyAsync(d_q, charges, (size_t)h->n_atoms * sizeof(double),
                             where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
     if (!h->rhs) PB_ALLOC(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
     if (!h->bc) PB_ALLOC(cudaMalloc((void **)&h->bc, (nbc + 8) * sizeof(double)));
     PB_TRY(charges_to_rhs_bc(h->atoms_c, d_q, h->n_atoms, h->nx, h->ny, h->nz, h->h, h->atoms_eps_out,
-                             h->atoms_kappa, h->rhs, h->bc, h->stream, h->dh_f32));
-    h->launches += 3;
+                             h->atoms_kappa, h->rhs, h->bc, scratch, h->nsm, h->stream, h->dh_f32));
+    h->launches += 4;
     h->wf.b_ready = false;
     h->wd.b_ready = false;
     if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));

@@ -7,6 +7,7 @@
 // so that no FMA contraction can flip them relative to a plain IEEE evaluation.
 #pragma once
 #include <cuda_runtime.h>
+#include "pb_internal.cuh"
 
 namespace pb {
 
@@ -66,10 +67,44 @@ __global__ void k_grid_faces(const unsigned char *__restrict__ mask, int nx, int
     }
 }
 
-// trilinear spreading of the point charges to their 8 surrounding nodes (q must be zeroed before)
-__global__ void k_grid_spread(const double *__restrict__ c, const double *__restrict__ charge, int n_atoms,
-                              int nx, int ny, int nz, double h, double *q)
+// Atom check + charge scale, one block, fixed order: every centre must lie inside the box [0,(n-1)h]^3 (an atom
+// outside would get extrapolated -- negative -- trilinear weights, and one sitting on a ghost node a 1/0 in the
+// boundary sum), and sum |q_a| bounds every node's accumulated charge, which fixes the fixed-point scale below.
+__global__ void k_grid_check(const double *__restrict__ c, const double *__restrict__ charge, int n_atoms,
+                             int nx, int ny, int nz, double h, double *sum_abs, int *bad)
 {
+    __shared__ double red[32];
+    double s = 0.0;
+    const double hi[3] = {(nx - 1) * h, (ny - 1) * h, (nz - 1) * h};
+    for (int a = threadIdx.x; a < n_atoms; a += blockDim.x) {
+        s += fabs(charge[a]);
+        for (int d = 0; d < 3; d++) {
+            const double v = c[3 * a + d];
+            if (!(v >= 0.0 && v <= hi[d])) *bad = 1;          // also catches NaN
+        }
+        if (!isfinite(charge[a])) *bad = 1;
+    }
+    const double tot = block_sum(s, red);
+    if (threadIdx.x == 0) *sum_abs = tot;
+}
+
+// fixed-point scale 2^(62 - e) with sum|q| < 2^e: every partial sum fits a signed 64-bit integer
+__device__ __forceinline__ int spread_shift(double sum_abs)
+{
+    int e = 0;
+    if (sum_abs > 0.0) frexp(sum_abs, &e);
+    return 62 - e;
+}
+
+// Trilinear spreading of the point charges to their 8 surrounding nodes (q(i,j,k) of Eq. 3).  Nodes
+// shared by several atoms are accumulated with integer atomics in 64-bit fixed point (resolution sum|q| * 2^-62,
+// far below an fp64 ulp of any node charge that matters): integer addition is associative, so the result does not
+// depend on the order in which the atoms arrive -- bitwise reproducible, unlike a floating-point atomicAdd.
+// `acc` is the rhs buffer viewed as int64 and zeroed before; k_grid_rhs converts it in place.
+__global__ void k_grid_spread(const double *__restrict__ c, const double *__restrict__ charge, int n_atoms,
+                              int nx, int ny, int nz, double h, const double *sum_abs, long long *acc)
+{
+    const double scale = ldexp(1.0, spread_shift(*sum_abs));
     for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < n_atoms; a += gridDim.x * blockDim.x) {
         const double g[3] = {c[3 * a] / h, c[3 * a + 1] / h, c[3 * a + 2] / h};
         const int n[3] = {nx, ny, nz};
@@ -87,18 +122,24 @@ __global__ void k_grid_spread(const double *__restrict__ c, const double *__rest
                 for (int dx = 0; dx < 2; dx++) {
                     const double wx = dx ? fr[0] : __dsub_rn(1.0, fr[0]);
                     const double v = __dmul_rn(__dmul_rn(__dmul_rn(qa, wz), wy), wx);
-                    atomicAdd(&q[((size_t)(base[2] + dz) * ny + base[1] + dy) * nx + base[0] + dx], v);
+                    const long long fx = __double2ll_rn(__dmul_rn(v, scale));
+                    if (fx != 0)
+                        atomicAdd((unsigned long long *)&acc[((size_t)(base[2] + dz) * ny + base[1] + dy) * nx + base[0] + dx],
+                                  (unsigned long long)fx);
                 }
             }
         }
     }
 }
 
-// rhs = (4 pi) q / h^3, in place
-__global__ void k_grid_rhs(double *q, size_t n, double four_pi, double h3)
+// rhs = (4 pi) q / h^3 in place, q = fixed-point accumulator * 2^-shift
+__global__ void k_grid_rhs(double *q, size_t n, double four_pi, double h3, const double *sum_abs)
 {
-    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x)
-        q[t] = __ddiv_rn(__dmul_rn(four_pi, q[t]), h3);
+    const double inv = ldexp(1.0, -spread_shift(*sum_abs));
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        const double qn = __dmul_rn((double)reinterpret_cast<const long long *>(q)[t], inv);
+        q[t] = __ddiv_rn(__dmul_rn(four_pi, qn), h3);
+    }
 }
 
 // Debye-Hueckel ghost values: bc[g] = (1/eps_out) sum_a q_a exp(-kappa r_ga)/r_ga, atoms in index order.

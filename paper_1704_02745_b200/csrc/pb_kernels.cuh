@@ -222,7 +222,8 @@ __global__ void k_finish(const T *__restrict__ x, const T *__restrict__ pbuf0, c
          t += (size_t)gridDim.x * blockDim.x) {
         const int i = (int)(t % nx);
         const size_t row = t / nx;
-        dst[t] = (S)fma(alpha, p[row * P + i], x[row * P + i]);
+        // alpha = 0: nothing pending (no iteration ran, or a breakdown: p may hold non-finite values, 0*NaN = NaN)
+        dst[t] = (alpha == T(0)) ? (S)x[row * P + i] : (S)fma(alpha, p[row * P + i], x[row * P + i]);
     }
 }
 
@@ -381,7 +382,7 @@ __global__ void k_finish_add(const T *__restrict__ x, const T *__restrict__ pbuf
     for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
         const int i = (int)(t % nx);
         const size_t row = t / nx;
-        acc[row * Pacc + i] += (S)fma(alpha, p[row * P + i], x[row * P + i]);
+        acc[row * Pacc + i] += (alpha == T(0)) ? (S)x[row * P + i] : (S)fma(alpha, p[row * P + i], x[row * P + i]);
     }
 }
 

@@ -252,6 +252,20 @@ __device__ __forceinline__ double diag_of(const double *eps_x, const double *eps
     return d;
 }
 
+// SPD check of pb_create: every diagonal entry of Eq. 3 must be positive and finite (M = D must be invertible,
+// PAPER.md:138-140; "symmetric and positive-definite coefficient matrices")
+__global__ void k_check_diag(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
+                             const double *__restrict__ eps_z, const double *__restrict__ kbar2, double h2,
+                             int nx, int ny, int nz, int *bad)
+{
+    const size_t n = (size_t)nx * ny * nz;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(q % nx), j = (int)((q / nx) % ny), k = (int)(q / ((size_t)nx * ny));
+        const double d = diag_of(eps_x, eps_y, eps_z, kbar2, h2, nx, ny, i, j, k);
+        if (!(d > 0.0) || !isfinite(d)) *bad = 1;
+    }
+}
+
 __global__ void k_pal_collect_diag(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
                                    const double *__restrict__ eps_z, const double *__restrict__ kbar2, double h2,
                                    int nx, int ny, int nz, PalTable *t)

@@ -4,8 +4,6 @@ Tolerances are BASELINE.json's north_star: fp64 SpMV 1e-12 (componentwise backwa
 Reading 20), fp64 solve to 1e-10 within 1e-8 max|phi|, fp32 solve to 1e-5 within 1e-4 max|phi|,
 iteration counts within 5 % (at least +-1).
 """
-import os
-
 import numpy as np
 import pytest
 
@@ -33,10 +31,12 @@ def pbref():
     return m
 
 
-def backward_bound(inp, x):
-    """(D|x| + sum_f eps_f |x_nbr|)/h^2 per node: the scale of the terms of one row of Eq. 3."""
+def backward_bound(inp, x, periodic=False):
+    """(D|x| + sum_f eps_f |x_nbr|)/h^2 per node: the scale of the terms of one row of Eq. 3 (DESIGN.md Reading 20).
+    Periodic: the neighbour across a box face is the node on the opposite side, so its
+    |x| counts too (wrap padding instead of the zero ghost layer)."""
     ax = np.abs(x)
-    p = np.pad(ax, 1)
+    p = np.pad(ax, 1, mode="wrap") if periodic else np.pad(ax, 1)
     ex, ey, ez = inp.eps_x, inp.eps_y, inp.eps_z
     s = (ex[:, :, :-1] * (p[1:-1, 1:-1, :-2] + ax) + ex[:, :, 1:] * (p[1:-1, 1:-1, 2:] + ax)
          + ey[:, :-1, :] * (p[1:-1, :-2, 1:-1] + ax) + ey[:, 1:, :] * (p[1:-1, 2:, 1:-1] + ax)
@@ -249,10 +249,11 @@ def test_fullsize_385_spmv_and_solve_properties(pkg, pbref):
     ref.close()
 
 
-TILE_ENV = ("PB_TXV", "PB_TY", "PB_NS", "PB_BPS", "PB_TZ", "PB_AUTOTUNE", "PB_PERSIST")
-TILE_CONFIGS = [dict(PB_AUTOTUNE=0), dict(PB_TXV=7, PB_TY=3, PB_NS=3, PB_BPS=2, PB_TZ=5),
-                dict(PB_TXV=20, PB_TY=8, PB_NS=6, PB_BPS=1, PB_TZ=99), dict(PB_TXV=5, PB_TY=2, PB_NS=4, PB_BPS=4, PB_TZ=1),
-                dict(PB_TXV=13, PB_TY=5, PB_NS=5, PB_BPS=3, PB_TZ=33), dict()]
+# per-handle options (pb_set_option): forced tiles / rings / grids of k_spmv_tma, the static plan, the autotuned plan
+TILE_CONFIGS = [dict(autotune=0), dict(tile_txv=7, tile_ty=3, ring_slots=3, blocks_per_sm=2, tile_tz=5),
+                dict(tile_txv=20, tile_ty=8, ring_slots=6, blocks_per_sm=1, tile_tz=99),
+                dict(tile_txv=5, tile_ty=2, ring_slots=4, blocks_per_sm=4, tile_tz=1),
+                dict(tile_txv=13, tile_ty=5, ring_slots=5, blocks_per_sm=3, tile_tz=33), dict()]
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
@@ -267,27 +268,23 @@ def test_tiling_independence(pkg, pbref, prec):
     tol = 1e-10 if prec == "f64" else 1e-5
     o = ref.solve(tol, 5000)
     scale = np.max(np.abs(o["phi"]))
-    saved = {k: os.environ.pop(k, None) for k in TILE_ENV}
-    try:
-        y0 = None
-        for cfg in TILE_CONFIGS:
-            for k in TILE_ENV:
-                os.environ.pop(k, None)
-            os.environ.update({k: str(v) for k, v in cfg.items()})
-            os.environ["PB_PERSIST"] = "0"          # small grid: force the two-kernel TMA path under test
-            with pkg.PBSolver(*inp.args()) as s:
-                y = s.apply(x, prec)
-                runs = [s.solve(tol, 5000, prec, check_every=9) for _ in range(2)]
-            if y0 is None:
-                y0 = y
-            assert np.array_equal(y, y0), cfg
-            assert np.array_equal(runs[0]["phi"], runs[1]["phi"]) and runs[0]["iters"] == runs[1]["iters"], cfg
-            assert abs(runs[0]["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), cfg
-            assert np.max(np.abs(runs[0]["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale, cfg
-    finally:
-        for k in TILE_ENV:
-            os.environ.pop(k, None)
-        os.environ.update({k: v for k, v in saved.items() if v is not None})
+    y0 = None
+    for cfg in TILE_CONFIGS:
+        # small grid: persist=0 forces the two-kernel TMA path under test
+        with pkg.PBSolver(*inp.args(), options=dict(cfg, persist=0)) as s:
+            y = s.apply(x, prec)
+            runs = [s.solve(tol, 5000, prec, check_every=9) for _ in range(2)]
+            plan = s.plan(prec)
+        if "tile_txv" in cfg:
+            assert (plan["txv"], plan["ty"], plan["ring_slots"], plan["blocks_per_sm"]) == (
+                cfg["tile_txv"], cfg["tile_ty"], cfg["ring_slots"], cfg["blocks_per_sm"]), (cfg, plan)
+            assert plan["tz"] == min(cfg["tile_tz"], inp.nz) and not plan["autotuned"] and not plan["persist"]
+        if y0 is None:
+            y0 = y
+        assert np.array_equal(y, y0), cfg
+        assert np.array_equal(runs[0]["phi"], runs[1]["phi"]) and runs[0]["iters"] == runs[1]["iters"], cfg
+        assert abs(runs[0]["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), cfg
+        assert np.max(np.abs(runs[0]["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale, cfg
     ref.close()
 
 
@@ -299,36 +296,25 @@ def test_tiling_independence_with_both_palettes(pkg, prec):
     inp = random_operator(77, 45, 38, seed=33, salted=False, two_valued=True)      # kbar2 = 0: few distinct diagonals
     dt = np.float64 if prec == "f64" else np.float32
     x = np.random.default_rng(5).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(dt)
-    keys = TILE_ENV + ("PB_PALETTE_DS", "PB_PALETTE")
-    saved = {k: os.environ.pop(k, None) for k in keys}
-    try:
-        ref_y = ref_p = ref_ap = None
-        for fmt in (dict(), dict(PB_PALETTE_DS=0), dict(PB_PALETTE=0)):
-            for cfg in TILE_CONFIGS:
-                for k in keys:
-                    os.environ.pop(k, None)
-                os.environ.update({k: str(v) for k, v in {**cfg, **fmt}.items()})
-                os.environ["PB_PERSIST"] = "0"
-                with pkg.PBSolver(*inp.args()) as s:
-                    if not fmt:
-                        assert s.palette_size() > 0 and s.diag_palette_size() > 0
-                        assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
-                    y = s.apply(x, prec)
-                    s.solve_begin(prec)
-                    s.iterate(prec, 2)
-                    p2, ap2 = s.vector("p"), s.vector("Ap")
-                if ref_y is None:
-                    ref_y, ref_p, ref_ap = y, p2, ap2
-                assert np.array_equal(y, ref_y), (fmt, cfg)
-                # p and Ap after two iterations: alpha/beta come from tiling-dependent summation orders, so compare
-                # to rounding, not bitwise
-                eps = 1e-5 if prec == "f32" else 1e-13
-                assert np.max(np.abs(p2 - ref_p)) <= eps * np.max(np.abs(ref_p)), (fmt, cfg)
-                assert np.max(np.abs(ap2 - ref_ap)) <= eps * np.max(np.abs(ref_ap)), (fmt, cfg)
-    finally:
-        for k in keys:
-            os.environ.pop(k, None)
-        os.environ.update({k: v for k, v in saved.items() if v is not None})
+    ref_y = ref_p = ref_ap = None
+    for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette=0)):
+        for cfg in TILE_CONFIGS:
+            with pkg.PBSolver(*inp.args(), options={**cfg, **fmt, "persist": 0}) as s:
+                y = s.apply(x, prec)
+                if not fmt:
+                    assert s.palette_size() > 0 and s.diag_palette_size() > 0
+                    assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
+                s.solve_begin(prec)
+                s.iterate(prec, 2)
+                p2, ap2 = s.vector("p"), s.vector("Ap")
+            if ref_y is None:
+                ref_y, ref_p, ref_ap = y, p2, ap2
+            assert np.array_equal(y, ref_y), (fmt, cfg)
+            # p and Ap after two iterations: alpha/beta come from tiling-dependent summation orders, so compare
+            # to rounding, not bitwise
+            eps = 1e-5 if prec == "f32" else 1e-13
+            assert np.max(np.abs(p2 - ref_p)) <= eps * np.max(np.abs(ref_p)), (fmt, cfg)
+            assert np.max(np.abs(ap2 - ref_ap)) <= eps * np.max(np.abs(ref_ap)), (fmt, cfg)
 
 
 @pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
@@ -361,26 +347,21 @@ def test_palette_and_full_precision_coefficients_agree(pkg, pbref, prec, tol):
     than 256 distinct values must fall back to them."""
     inp = make_config(2)                       # molecular map: eps in {1, 80, 160/81}
     x = np.random.default_rng(4).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(np.float64 if prec == "f64" else np.float32)
-    saved = os.environ.pop("PB_PALETTE", None)
-    try:
-        with pkg.PBSolver(*inp.args()) as s:
-            assert s.palette_size() == 4       # the three face values and the pad value 0
-            y_pal = s.apply(x, prec)
-            g_pal = s.solve(tol, 5000, prec)
-        os.environ["PB_PALETTE"] = "0"
-        with pkg.PBSolver(*inp.args()) as s:
-            assert s.palette_size() == 0
-            y_full = s.apply(x, prec)
-            g_full = s.solve(tol, 5000, prec)
-    finally:
-        os.environ.pop("PB_PALETTE", None)
-        if saved is not None:
-            os.environ["PB_PALETTE"] = saved
+    with pkg.PBSolver(*inp.args()) as s:
+        y_pal = s.apply(x, prec)
+        assert s.palette_size() == 4       # the three face values and the pad value 0
+        g_pal = s.solve(tol, 5000, prec)
+        # the same handle with the palette switched off: work arrays and plan are rebuilt (options are handle state)
+        s.set_option("palette", 0)
+        y_full = s.apply(x, prec)
+        assert s.palette_size() == 0 and s.get_option("palette") == 0
+        g_full = s.solve(tol, 5000, prec)
     assert np.array_equal(y_pal, y_full)
     assert abs(g_pal["iters"] - g_full["iters"]) <= 1
     assert np.max(np.abs(g_pal["phi"] - g_full["phi"])) <= (1e-9 if prec == "f64" else 1e-4) * np.max(np.abs(g_full["phi"]))
     many = random_operator(21, 9, 8, seed=6, two_valued=False)      # ~5000 distinct face values
     with pkg.PBSolver(*many.args()) as s:
+        s.prepare(prec)
         assert s.palette_size() == 0
 
 
@@ -428,23 +409,17 @@ def test_persistent_and_two_kernel_paths_agree(pkg, pbref, prec, tol):
     ref.close()
     scale = np.max(np.abs(o["phi"]))
     lim = 1e-8 if prec == "f64" else 1e-4
-    saved = os.environ.pop("PB_PERSIST", None)
     res = {}
-    try:
-        for mode in ("1", "0"):
-            os.environ["PB_PERSIST"] = mode
-            with pkg.PBSolver(*inp.args()) as s:
-                a, b = s.solve(tol, 5000, prec), s.solve(tol, 5000, prec)
-                assert np.array_equal(a["phi"], b["phi"]) and a["iters"] == b["iters"]
-                m7 = s.solve(tol, 7, prec)
-                w = s.solve(tol, 5000, prec, phi0=a["phi"].copy())
-                s.set_preconditioner(False)
-                cg = s.solve(tol, 5000, prec)
-            res[mode] = (a, m7, cg, w)
-    finally:
-        os.environ.pop("PB_PERSIST", None)
-        if saved is not None:
-            os.environ["PB_PERSIST"] = saved
+    for mode in ("1", "0"):
+        with pkg.PBSolver(*inp.args(), options=dict(persist=int(mode))) as s:
+            a, b = s.solve(tol, 5000, prec), s.solve(tol, 5000, prec)
+            assert s.plan(prec)["persist"] == int(mode)
+            assert np.array_equal(a["phi"], b["phi"]) and a["iters"] == b["iters"]
+            m7 = s.solve(tol, 7, prec)
+            w = s.solve(tol, 5000, prec, phi0=a["phi"].copy())
+            s.set_preconditioner(False)
+            cg = s.solve(tol, 5000, prec)
+        res[mode] = (a, m7, cg, w)
     for a, m7, cg, w in res.values():
         assert a["status"] == 0 and abs(a["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"]))
         assert np.max(np.abs(a["phi"] - o["phi"])) <= lim * scale
@@ -467,9 +442,9 @@ def test_config5_headline_parity_full_size(pkg, pbref):
     ref.close()
     scale = np.max(np.abs(o64["phi"]))
     with pkg.PBSolver(*inp.args()) as s:
-        assert s.palette_size() == 4
         g32 = s.solve(1e-5, 20000, "f32", check_every=32)
         g64 = s.solve(1e-10, 20000, "f64", check_every=32)
+        assert s.palette_size() == 4
     assert g32["status"] == 0 and g64["status"] == 0
     assert abs(g32["iters"] - o32["iters"]) <= round(0.05 * o32["iters"]), (g32["iters"], o32["iters"])
     assert abs(g64["iters"] - o64["iters"]) <= round(0.05 * o64["iters"]), (g64["iters"], o64["iters"])
@@ -505,8 +480,8 @@ def test_periodic_boundary_spmv(pkg, pbref, shape):
         s.set_periodic(False)
         assert np.array_equal(s.apply(x, "f64"), y_dir)
     yr = ref.apply(x)
-    bound = backward_bound(inp, x) + 1e-300
-    assert np.all(np.abs(y - yr) <= 1e-12 * bound * 2)
+    bound = backward_bound(inp, x, periodic=True) + 1e-300
+    assert np.all(np.abs(y - yr) <= 1e-12 * bound)
     assert np.all(np.abs(y32 - yr) <= 2e-6 * bound)
     ref.close()
 
@@ -520,18 +495,11 @@ def test_periodic_boundary_solve(pkg, pbref, prec, tol, persist):
     ref.set_rhs(inp.rhs, inp.bc)
     o = ref.solve(tol, 5000)
     ref.close()
-    saved = os.environ.pop("PB_PERSIST", None)
-    os.environ["PB_PERSIST"] = persist
-    try:
-        with pkg.PBSolver(*inp.args()) as s:
-            s.set_periodic(True)
-            assert np.allclose(s.b(), inp.rhs, rtol=1e-14)       # no ghost fold-in
-            g = s.solve(tol, 5000, prec, check_every=8)
-            g2 = s.solve(tol, 5000, prec, check_every=8)
-    finally:
-        os.environ.pop("PB_PERSIST", None)
-        if saved is not None:
-            os.environ["PB_PERSIST"] = saved
+    with pkg.PBSolver(*inp.args(), options=dict(persist=int(persist))) as s:
+        s.set_periodic(True)
+        assert np.allclose(s.b(), inp.rhs, rtol=1e-14)       # no ghost fold-in
+        g = s.solve(tol, 5000, prec, check_every=8)
+        g2 = s.solve(tol, 5000, prec, check_every=8)
     scale = np.max(np.abs(o["phi"]))
     assert g["status"] == 0 and abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (g["iters"], o["iters"])
     assert np.max(np.abs(g["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale
@@ -543,25 +511,18 @@ def test_diagonal_palette_is_exact(pkg, prec, tol):
     """k_vec reading Dinv through the diagonal palette (index byte + table of (T)(1/d)) must reproduce the Dinv-array
     run bit for bit; an operator whose salt map varies from node to node must fall back to the array."""
     inp = make_config(2)
-    saved = {k: os.environ.pop(k, None) for k in ("PB_PALETTE_D", "PB_PERSIST", "PB_AUTOTUNE")}
-    os.environ["PB_PERSIST"] = "0"                 # the two-kernel path is the one that uses k_vec
-    os.environ["PB_AUTOTUNE"] = "0"                # same static plan in both handles: same reduction order
-    try:
-        with pkg.PBSolver(*inp.args()) as s:
-            assert 0 < s.diag_palette_size() <= 56
-            a = s.solve(tol, 5000, prec)
-        os.environ["PB_PALETTE_D"] = "0"
-        with pkg.PBSolver(*inp.args()) as s:
-            assert s.diag_palette_size() == 0
-            b = s.solve(tol, 5000, prec)
-        many = random_operator(21, 9, 8, seed=6, two_valued=True, salted=True)    # kbar2 ~ U[0,2] per node
-        with pkg.PBSolver(*many.args()) as s:
-            assert s.palette_size() > 0 and s.diag_palette_size() == 0
-    finally:
-        for k, v in saved.items():
-            os.environ.pop(k, None)
-            if v is not None:
-                os.environ[k] = v
+    # persist=0: the two-kernel path is the one that uses k_vec; autotune=0: the same static plan in both runs,
+    # hence the same reduction order
+    with pkg.PBSolver(*inp.args(), options=dict(persist=0, autotune=0)) as s:
+        a = s.solve(tol, 5000, prec)
+        assert 0 < s.diag_palette_size() <= 56 and s.plan(prec)["diag_palette_vec"] == 1
+        s.set_option("palette_diag", 0)
+        b = s.solve(tol, 5000, prec)
+        assert s.diag_palette_size() == 0 and s.plan(prec)["diag_palette_vec"] == 0
+    many = random_operator(21, 9, 8, seed=6, two_valued=True, salted=True)    # kbar2 ~ U[0,2] per node
+    with pkg.PBSolver(*many.args()) as s:
+        s.prepare(prec)
+        assert s.palette_size() > 0 and s.diag_palette_size() == 0
     assert a["iters"] == b["iters"] and np.array_equal(a["phi"], b["phi"])
 
 
@@ -570,44 +531,37 @@ def test_randomised_shapes_and_options(pkg, pbref):
     or two-kernel path, fp32 / fp64, warm start): SpMV within the componentwise bound, solves within the north-star
     tolerances of the oracle run with the same options."""
     rng = np.random.default_rng(20260704)
-    saved = os.environ.pop("PB_PERSIST", None)
-    try:
-        for case in range(24):
-            nx, ny, nz = (int(v) for v in rng.integers(1, 41, 3))
-            periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), bool(rng.integers(2))
-            persist, prec = str(int(rng.integers(2))), ("f64", "f32")[int(rng.integers(2))]
-            inp = _periodic_inputs((nx, ny, nz), 100 + case) if periodic else random_operator(nx, ny, nz, seed=100 + case)
-            if not two_valued:
-                inp.eps_x[...] = rng.uniform(1, 80, inp.eps_x.shape)
-                if periodic:
-                    inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
-            tol = 1e-10 if prec == "f64" else 1e-5
-            ref = pbref.from_inputs(inp)
-            ref.set_periodic(periodic)
-            ref.set_rhs(inp.rhs, inp.bc)
-            o = ref.solve(tol, 4000, precond=jacobi)
-            x = rng.uniform(-1, 1, (nz, ny, nx))
-            yr = ref.apply(x)
-            os.environ["PB_PERSIST"] = persist
-            with pkg.PBSolver(*inp.args()) as s:
-                s.set_periodic(periodic)
-                s.set_preconditioner(jacobi)
-                y = s.apply(x.astype(np.float64 if prec == "f64" else np.float32), prec)
-                g = s.solve(tol, 4000, prec, check_every=int(rng.integers(1, 40)))
-                w = s.solve(tol, 4000, prec, phi0=g["phi"].copy())
-            ref.close()
-            tag = (case, nx, ny, nz, periodic, jacobi, two_valued, persist, prec)
-            bound = backward_bound(inp, x) + 1e-300
-            assert np.all(np.abs(y - yr) <= (2e-12 if prec == "f64" else 2e-6) * bound), tag
-            assert g["status"] == o["status"] == 0, tag
-            assert abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), tag + (g["iters"], o["iters"])
-            scale = np.max(np.abs(o["phi"])) + 1e-300
-            assert np.max(np.abs(g["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale, tag
-            assert w["iters"] <= 1, tag
-    finally:
-        os.environ.pop("PB_PERSIST", None)
-        if saved is not None:
-            os.environ["PB_PERSIST"] = saved
+    for case in range(24):
+        nx, ny, nz = (int(v) for v in rng.integers(1, 41, 3))
+        periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), bool(rng.integers(2))
+        persist, prec = int(rng.integers(2)), ("f64", "f32")[int(rng.integers(2))]
+        inp = _periodic_inputs((nx, ny, nz), 100 + case) if periodic else random_operator(nx, ny, nz, seed=100 + case)
+        if not two_valued:
+            inp.eps_x[...] = rng.uniform(1, 80, inp.eps_x.shape)
+            if periodic:
+                inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
+        tol = 1e-10 if prec == "f64" else 1e-5
+        ref = pbref.from_inputs(inp)
+        ref.set_periodic(periodic)
+        ref.set_rhs(inp.rhs, inp.bc)
+        o = ref.solve(tol, 4000, precond=jacobi)
+        x = rng.uniform(-1, 1, (nz, ny, nx))
+        yr = ref.apply(x)
+        with pkg.PBSolver(*inp.args(), options=dict(persist=persist)) as s:
+            s.set_periodic(periodic)
+            s.set_preconditioner(jacobi)
+            y = s.apply(x.astype(np.float64 if prec == "f64" else np.float32), prec)
+            g = s.solve(tol, 4000, prec, check_every=int(rng.integers(1, 40)))
+            w = s.solve(tol, 4000, prec, phi0=g["phi"].copy())
+        ref.close()
+        tag = (case, nx, ny, nz, periodic, jacobi, two_valued, persist, prec)
+        bound = backward_bound(inp, x, periodic=periodic) + 1e-300
+        assert np.all(np.abs(y - yr) <= (1e-12 if prec == "f64" else 2e-6) * bound), tag
+        assert g["status"] == o["status"] == 0, tag
+        assert abs(g["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), tag + (g["iters"], o["iters"])
+        scale = np.max(np.abs(o["phi"])) + 1e-300
+        assert np.max(np.abs(g["phi"] - o["phi"])) <= (1e-8 if prec == "f64" else 1e-4) * scale, tag
+        assert w["iters"] <= 1, tag
 
 
 def test_true_residual_matches_oracle(pkg, pbref):
@@ -664,15 +618,180 @@ def test_refinement_periodic_and_two_kernel_path(pkg, pbref, persist):
     ref.set_rhs(inp.rhs, inp.bc)
     o = ref.solve(1e-10, 5000)
     ref.close()
-    saved = os.environ.pop("PB_PERSIST", None)
-    os.environ["PB_PERSIST"] = persist
-    try:
-        with pkg.PBSolver(*inp.args()) as s:
-            s.set_periodic(True)
-            g = s.solve_refined(1e-10, 5000, check_every=8)
-    finally:
-        os.environ.pop("PB_PERSIST", None)
-        if saved is not None:
-            os.environ["PB_PERSIST"] = saved
+    with pkg.PBSolver(*inp.args(), options=dict(persist=int(persist))) as s:
+        s.set_periodic(True)
+        g = s.solve_refined(1e-10, 5000, check_every=8)
     assert g["status"] == 0 and g["relres"] <= 1e-10
     assert np.max(np.abs(g["phi"] - o["phi"])) <= 1e-8 * np.max(np.abs(o["phi"]))
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs[3] (257^3, eps_in = 4) and the config-5 batch members (PAPER.md:182 defines the
+# workload family: eps 80 / solute, harmonic faces, free-space boundary; PAPER.md:23 the snapshot stream)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.slow
+def test_solve_config4_257(pkg, pbref):
+    """configs[3]: 257^3, 20 000-atom globule, eps_in = 4 (palette {0, 4, 7.619, 80}: another face table, another
+    diagonal table, another autotuned plan than config 5), fp32 to 1e-5 and fp64 to 1e-10 -- every node against the
+    full oracle solves, iteration counts within 5 %."""
+    inp = make_config(4, device="cuda")
+    assert inp.meta["eps_in"] == 4.0 and set(np.unique(inp.eps_x)) == {4.0, 80.0, 2 * 4.0 * 80.0 / 84.0}
+    ref = pbref.from_inputs(inp)
+    o32 = ref.solve(1e-5, 5000)
+    o64 = ref.solve(1e-10, 5000)
+    ref.close()
+    scale = np.max(np.abs(o64["phi"]))
+    with pkg.PBSolver(*inp.args()) as s:
+        g32 = s.solve(1e-5, 20000, "f32", check_every=32)
+        g64 = s.solve(1e-10, 20000, "f64", check_every=32)
+        p32, p64 = s.plan("f32"), s.plan("f64")
+    assert p32["palette_size"] == 4 and p32["face_palette"] and not p32["persist"] and not p64["persist"]
+    assert g32["status"] == 0 and g64["status"] == 0 and g32["relres"] < 1e-5 and g64["relres"] < 1e-10
+    assert abs(g32["iters"] - o32["iters"]) <= round(0.05 * o32["iters"]), (g32["iters"], o32["iters"])
+    assert abs(g64["iters"] - o64["iters"]) <= round(0.05 * o64["iters"]), (g64["iters"], o64["iters"])
+    e32 = np.max(np.abs(g32["phi"] - o32["phi"])) / scale
+    e32t = np.max(np.abs(g32["phi"] - o64["phi"])) / scale
+    e64 = np.max(np.abs(g64["phi"] - o64["phi"])) / scale
+    print(f"config4: fp32 iters {g32['iters']} (oracle {o32['iters']}) err {e32:.2e} / {e32t:.2e}; "
+          f"fp64 iters {g64['iters']} (oracle {o64['iters']}) err {e64:.2e}; plan {p32['txv']}x{p32['ty']}x{p32['tz']}")
+    assert e32 <= 1e-4 and e32t <= 1e-4 and e64 <= 1e-8
+
+
+@pytest.mark.slow
+def test_config5_batch_member_parity(pkg, pbref):
+    """One member of configs[4]'s 50-solve batch (seeded charge perturbation N(0, 0.05) e on the same operator) at the
+    full 385^3, fp32 to 1e-5, against the oracle's own solve of that member -- through pb_set_rhs (host-generated
+    rhs / ghost values) and through pb_set_charges on an atom-built handle (rhs and the 5.3e10-term boundary sum made
+    on the GPU); every node, north-star fp32 bar."""
+    from workloads import perturbed_charge_values, perturbed_charges
+
+    member = 7
+    inp = make_config(5, device="cuda")
+    rhs_s, bc_s = perturbed_charges(inp, member, device="cuda")
+    ref = pbref.from_inputs(inp)
+    ref.set_rhs(rhs_s, bc_s)
+    o = ref.solve(1e-5, 5000)
+    ref.close()
+    scale = np.max(np.abs(o["phi"]))
+    with pkg.PBSolver(*inp.args()) as s:
+        base = s.solve(1e-5, 20000, "f32", check_every=32)
+        s.set_rhs(rhs_s, bc_s)
+        g = s.solve(1e-5, 20000, "f32", check_every=32)
+    m = inp.meta
+    with pkg.PBSolver.from_atoms(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], m["radii"], m["charges"], m["eps_in"],
+                                 m["eps_out"], m["kbar2_solvent"]) as s2:
+        s2.set_charges(perturbed_charge_values(inp, member))
+        g2 = s2.solve(1e-5, 20000, "f32", check_every=32)
+    for r in (g, g2):
+        assert r["status"] == 0 and r["relres"] < 1e-5
+        assert abs(r["iters"] - o["iters"]) <= round(0.05 * o["iters"]), (r["iters"], o["iters"])
+        assert np.max(np.abs(r["phi"] - o["phi"])) <= 1e-4 * scale
+    # the member really is another right-hand side than the unperturbed one
+    assert np.max(np.abs(g["phi"] - base["phi"])) > 1e-3 * scale
+    print(f"config5 member {member}: iters set_rhs {g['iters']} / set_charges {g2['iters']} (oracle {o['iters']}), "
+          f"err {np.max(np.abs(g['phi'] - o['phi'])) / scale:.2e} / {np.max(np.abs(g2['phi'] - o['phi'])) / scale:.2e}")
+
+
+# ---------------------------------------------------------------------------------------------
+# failure paths (SURVEY.md section 5, Reading 17) on both solve paths
+# ---------------------------------------------------------------------------------------------
+def _indefinite_operator(shape=(17, 13, 11)):
+    """Uniform eps = 80, no salt, one interior face at -300: both adjacent diagonals stay positive (5*80 - 300 = 100,
+    pb_create accepts it) but the 2x2 block [[100, 300], [300, 100]] is indefinite, so A is not SPD."""
+    nx, ny, nz = shape
+    inp = random_operator(nx, ny, nz, seed=77, salted=False)
+    inp.eps_x[...] = 80.0
+    inp.eps_y[...] = 80.0
+    inp.eps_z[...] = 80.0
+    inp.eps_x[nz // 2, ny // 2, nx // 2] = -300.0
+    return inp
+
+
+@pytest.mark.parametrize("persist", [1, 0])
+def test_breakdown_returns_last_good_iterate(pkg, pbref, persist):
+    """p.Ap <= 0 on an indefinite operator: PB_ERR_BREAKDOWN, iters and phi = the oracle's at its own breakdown (the last
+    iterate before the failed step), on the cooperative path and on the two-kernel path, whatever check_every is."""
+    inp = _indefinite_operator()
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(1e-12, 500)
+    ref.close()
+    assert o["status"] == pbref.BREAKDOWN and o["iters"] >= 1
+    scale = np.max(np.abs(o["phi"]))
+    with pkg.PBSolver(*inp.args(), options=dict(persist=persist)) as s:
+        assert np.all(s.diag() > 0)
+        for ce in (1, 7, 1000):                          # 1000 > maxiter: one chunk covers the whole solve
+            g = s.solve(1e-12, 500, "f64", check_every=ce)
+            assert g["status"] == pkg.binding.PB_ERR_BREAKDOWN, (ce, g["status"])
+            assert g["iters"] == o["iters"], (ce, g["iters"], o["iters"])
+            assert np.all(np.isfinite(g["phi"]))
+            assert np.max(np.abs(g["phi"] - o["phi"])) <= 1e-8 * scale
+        g32 = s.solve(1e-12, 500, "f32", check_every=5)
+        assert g32["status"] == pkg.binding.PB_ERR_BREAKDOWN and np.all(np.isfinite(g32["phi"]))
+        # the handle is still usable afterwards
+        s.set_rhs(None, None)
+        assert s.solve(1e-6, 10, "f64")["iters"] == 0
+
+
+@pytest.mark.parametrize("persist", [1, 0])
+@pytest.mark.parametrize("bad", [np.nan, np.inf])
+def test_non_finite_rhs_is_a_breakdown(pkg, pbref, persist, bad):
+    """NaN / Inf in rhs: PB_ERR_BREAKDOWN at l = 0 with phi = 0 (finite), never a hang or PB_ERR_MAXITER; same as the
+    oracle's verdict."""
+    inp = random_operator(19, 11, 6, seed=4)
+    rhs = inp.rhs.copy()
+    rhs[3, 5, 7] = bad
+    ref = pbref.from_inputs(inp)
+    ref.set_rhs(rhs, inp.bc)
+    o = ref.solve(1e-8, 50)
+    ref.close()
+    assert o["status"] == pbref.BREAKDOWN and o["iters"] == 0
+    with pkg.PBSolver(*inp.args(), options=dict(persist=persist)) as s:
+        s.set_rhs(rhs, inp.bc)
+        for prec in ("f64", "f32"):
+            g = s.solve(1e-8, 50, prec, check_every=4)
+            assert g["status"] == pkg.binding.PB_ERR_BREAKDOWN and g["iters"] == 0
+            assert not g["phi"].any()
+        s.set_rhs(inp.rhs, inp.bc)                        # a good right-hand side afterwards solves normally
+        assert s.solve(1e-8, 500, "f64")["status"] == 0
+
+
+def test_check_every_larger_than_maxiter(pkg, pbref):
+    inp = random_operator(19, 11, 6, seed=4)
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(1e-12, 7)
+    o_conv = ref.solve(1e-6, 1000)
+    ref.close()
+    with pkg.PBSolver(*inp.args(), options=dict(persist=0)) as s:
+        g = s.solve(1e-12, 7, "f64", check_every=4096)
+        assert g["status"] == pkg.binding.PB_ERR_MAXITER and g["iters"] == 7
+        assert np.max(np.abs(g["phi"] - o["phi"])) <= 1e-10 * np.max(np.abs(o["phi"]))
+        c = s.solve(1e-6, 1000, "f64", check_every=4096)
+        assert c["status"] == 0 and c["iters"] == o_conv["iters"]
+
+
+def test_options_are_handle_state(pkg):
+    """pb_set_option / pb_get_option / pb_get_plan: two handles in one process configured differently, invalid values
+    rejected, the plan reports what runs."""
+    inp = make_config(2)
+    with pkg.PBSolver(*inp.args(), options=dict(persist=0, palette=0, autotune=0)) as a, \
+            pkg.PBSolver(*inp.args()) as b:
+        pa, pb_ = a.plan("f32"), b.plan("f32")
+        assert pa["persist"] == 0 and pa["face_palette"] == 0 and pa["palette_size"] == 0 and not pa["autotuned"]
+        assert pa["spmv_bytes_per_node"] == 40 and pa["vec_bytes_per_node"] == 16
+        assert pb_["persist"] == 1 and pb_["face_palette"] == 1 and pb_["palette_size"] == 4
+        assert pb_["spmv_bytes_per_node"] == 28 and pb_["vec_bytes_per_node"] == 13
+        assert pa["num_sm"] == pb_["num_sm"] >= 1 and pa["grid"] >= 1 and pa["threads"] % 32 == 0
+        assert a.get_option("palette") == 0 and b.get_option("palette") == 1
+        ga, gb = a.solve(1e-5, 5000, "f32"), b.solve(1e-5, 5000, "f32")
+        assert abs(ga["iters"] - gb["iters"]) <= 1
+        for name, val in (("ring_slots", 2), ("ring_slots", 9), ("persist", 2), ("palette", -1), ("blocks_per_sm", 33)):
+            with pytest.raises(pkg.PBError):
+                a.set_option(name, val)
+        # a forced tile larger than the grid / the thread budget is clamped, and the plan says what really runs
+        a.set_option("tile_ty", 400)
+        a.set_option("tile_txv", 60)
+        pc = a.plan("f32")
+        assert pc["ty"] <= inp.ny and pc["txv"] <= pc["pitch"] // 4 and pc["threads"] <= 512
+        a.set_option("tile_ty", 0)
+        a.set_option("tile_txv", 0)
+        assert a.plan("f32")["txv"] == pa["txv"] and a.solve(1e-5, 5000, "f32")["iters"] == ga["iters"]

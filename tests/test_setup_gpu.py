@@ -127,3 +127,25 @@ def test_from_atoms_edge_cases(pkg):
         pkg.PBSolver.from_atoms(1, 8, 7, 0.5, np.zeros((1, 3)), np.ones(1), np.ones(1), 1.0, 80.0, 1.0)
     with pytest.raises(pkg.PBError):
         pkg.PBSolver.from_atoms(9, 8, 7, 0.5, np.ones((1, 3)), np.ones(1), np.ones(1), -1.0, 80.0, 1.0)
+
+
+def test_atoms_outside_the_box_are_rejected_and_charges_are_reproducible(pkg):
+    """An atom outside [0, (n-1)h]^3 would get extrapolated trilinear weights (and, on a ghost node, 1/0 in the
+    boundary sum): PB_ERR_INVALID_ARG.  The charge grid accumulates in 64-bit fixed point, so repeated spreading of
+    the same charges is bit-identical even where many atoms share nodes."""
+    nx, ny, nz, h = 21, 17, 13, 0.5
+    c, r, q = atoms(40, nx, ny, nz, h, 9)
+    for bad in ([-0.1, 2.0, 2.0], [2.0, (ny - 1) * h + 0.01, 2.0], [2.0, 2.0, float("nan")]):
+        cb = c.copy()
+        cb[5] = bad
+        with pytest.raises(pkg.PBError) as e:
+            pkg.PBSolver.from_atoms(nx, ny, nz, h, cb, r, q, 1.0, 80.0, 1.0)
+        assert e.value.status == pkg.binding.PB_ERR_INVALID_ARG
+    c[:20] = c[20:] + 0.01                                # pairs of atoms in the same cell: shared nodes
+    with pkg.PBSolver.from_atoms(nx, ny, nz, h, c, r, q, 1.0, 80.0, 1.0) as s:
+        first = s.field("rhs")
+        for _ in range(3):
+            s.set_charges(q)
+            assert np.array_equal(s.field("rhs"), first)
+        with pytest.raises(pkg.PBError):
+            s.set_charges(np.where(np.arange(40) == 3, np.inf, q))
