@@ -51,8 +51,13 @@ def parse_args(argv=None):
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--setup-from-atoms", action="store_true",
                     help="also time pb_create_from_atoms / pb_set_charges (GPU grid setup, NEXT row f1)")
-    ap.add_argument("--batch", type=int, default=0,
-                    help="also run this many solves of config 5's perturbed-charge batch on the same operator")
+    ap.add_argument("--batch", type=int, default=None,
+                    help="solves of config 5's perturbed-charge batch on the same operator (default: 50 at --gpus 1 "
+                         "--config 5, else 0)")
+    ap.add_argument("--no-variants", action="store_true",
+                    help="skip the other-precision and no-palette legs of the roofline record")
+    ap.add_argument("--cpu-per-config", action="store_true",
+                    help="also time the oracle on every smaller config (1 thread too for <= 129^3), BASELINE.md section 3")
     ap.add_argument("--refined", action="store_true",
                     help="also time pb_solve_refined (fp32-inner / fp64-outer, NEXT row f3) against the fp64 solve, to 1e-10")
     return ap.parse_args(argv)
@@ -205,6 +210,44 @@ def run_reference(args, rank, world):
             "gpu_launches": 0}
 
 
+def plan_summary(solver, prec):
+    """The launch plan that produced a number (pb_get_plan), as it goes into the JSON line."""
+    pl = solver.plan(prec)
+    keep = ("txv", "ty", "tz", "ring_slots", "blocks_per_sm", "tiles", "grid", "threads", "smem_bytes", "autotuned",
+            "vec_grid", "vec_threads", "persist", "face_palette", "diag_palette_vec", "diag_palette_spmv",
+            "palette_size", "diag_palette_size", "num_sm", "pitch")
+    return {k: pl[k] for k in keep}
+
+
+def timed_solves(solver, torch, stream, prec, tol, args, out, steps, warmup):
+    """`steps` complete pb_solve calls on device-resident data, CUDA events on the handle's stream."""
+    for _ in range(warmup):
+        res = solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    iters = 0
+    e0.record(stream)
+    for _ in range(steps):
+        res = solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out)
+        iters += res["iters"]
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return iters, e0.elapsed_time(e1), res
+
+
+def kernel_roofline(solver, prec, n_node, profile_iters, peak):
+    """CUDA events around every launch of the two kernels (pb_profile), charged with the bytes the handle's storage
+    format has to move (pb_bytes_per_node)."""
+    solver.solve_begin(prec)
+    solver.iterate(prec, 5)
+    ms_spmv, ms_vec = solver.profile(prec, profile_iters)
+    spmv_node, vec_node = solver.bytes_per_node(prec, 0), solver.bytes_per_node(prec, 1)
+    ach_s = spmv_node * n_node / (ms_spmv * 1e-3) / 1e9
+    ach_v = vec_node * n_node / (ms_vec * 1e-3) / 1e9
+    return {"spmv_ms": ms_spmv, "vec_ms": ms_vec, "spmv_bytes_per_node": spmv_node, "vec_bytes_per_node": vec_node,
+            "spmv_GBs": ach_s, "spmv_frac": ach_s / peak, "vec_GBs": ach_v, "vec_frac": ach_v / peak}
+
+
 def run_ours(args, rank, local_rank, world):
     import torch
 
@@ -237,6 +280,7 @@ def run_ours(args, rank, local_rank, world):
     t_create = time.perf_counter()
     solver = pkg.PBSolver(inp.nx, inp.ny, inp.nz, inp.h, inp.eps_x, inp.eps_y, inp.eps_z, inp.kbar2, rhs, bc,
                           stream=stream.cuda_stream)
+    solver.prepare(prec)                     # work arrays of this precision + plan autotune (pb_prepare)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     out_d = torch.empty(solver.shape, dtype=tdt, device=dev)
@@ -288,39 +332,11 @@ def run_ours(args, rank, local_rank, world):
                "h2d_bytes_per_step": int(rhs.nbytes + bc.nbytes), "d2h_bytes_per_step": int(n_node * elt + 96)}
         del rhs_h, bc_h, out_h
 
-    # ---- optional: the MD-snapshot batch (same operator, seeded charge perturbations), pb_set_rhs + pb_solve ----
+    # ---- the MD-snapshot batch (same operator, seeded charge perturbations), N = 1 default at config 5 ----
     batch = None
-    if args.batch > 0 and "charges" in inp.meta:
-        from workloads import perturbed_charges
-
-        t_b, it_b, t_w, it_w = 0.0, [], 0.0, []
-        out_w = torch.empty_like(out_d)
-        for sidx in range(args.batch):
-            rhs_s, bc_s = perturbed_charges(inp, world * sidx + rank, device=f"cuda:{local_rank}")
-            rhs_d = torch.from_numpy(np.ascontiguousarray(rhs_s)).to(dev)
-            bc_d = torch.from_numpy(np.ascontiguousarray(bc_s)).to(dev)
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            solver.set_rhs(rhs_d, bc_d)
-            it_b.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
-            torch.cuda.synchronize()
-            t_b += time.perf_counter() - t0
-            # the same member restarted from the previous member's potential (pb_solve_from, NEXT row f2)
-            if sidx == 0:
-                out_w.copy_(out_d)
-            else:
-                t0 = time.perf_counter()
-                it_w.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_w,
-                                         phi0=out_w)["iters"])
-                torch.cuda.synchronize()
-                t_w += time.perf_counter() - t0
-            del rhs_d, bc_d
-        batch = {"solves": args.batch, "solves_per_s": args.batch / t_b, "ms_per_solve": 1e3 * t_b / args.batch,
-                 "mean_iters": float(np.mean(it_b)), "min_iters": int(min(it_b)), "max_iters": int(max(it_b)),
-                 "warm_start": ({"mean_iters": float(np.mean(it_w)), "ms_per_solve": 1e3 * t_w / len(it_w)}
-                                if it_w else None),
-                 "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member, this rank only; warm_start: "
-                         "the same members solved again from the previous member's potential (pb_solve_from)"}
+    n_batch = args.batch if args.batch is not None else (50 if (world == 1 and args.config == 5) else 0)
+    if n_batch > 0 and "charges" in inp.meta:
+        batch = run_batch(args, solver, inp, prec, tol, n_batch, rank, world, local_rank, dev, out_d, torch)
 
     # ---- optional (NEXT row f3): mixed-precision iterative refinement against the plain fp64 solve ----------------
     refined = None
@@ -344,80 +360,38 @@ def run_ours(args, rank, local_rank, world):
     # ---- optional (NEXT row f1): the same problem built on the GPU from atoms, and a charge update ---------------
     setup = None
     if args.setup_from_atoms and "charges" in inp.meta:
-        from workloads import perturbed_charge_values
-
-        m = inp.meta
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        s2 = pkg.PBSolver.from_atoms(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], m["radii"], m["charges"],
-                                     m["eps_in"], m["eps_out"], m["kbar2_solvent"], stream=stream.cuda_stream)
-        torch.cuda.synchronize()
-        t_fa = time.perf_counter() - t0
-        nb = min(args.batch, 10) if args.batch > 0 else 3
-        t_sc, t_sv, it_sc = 0.0, 0.0, []
-        for sidx in range(nb):
-            qs = perturbed_charge_values(inp, sidx)
-            t0 = time.perf_counter()
-            s2.set_charges(qs)
-            torch.cuda.synchronize()
-            t1 = time.perf_counter()
-            it_sc.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
-            torch.cuda.synchronize()
-            t_sc += t1 - t0
-            t_sv += time.perf_counter() - t1
-        # the same charge updates with the boundary terms in fp32 (pb_set_setup_precision)
-        s2.set_setup_precision("f32")
-        t_sc32, it_sc32 = 0.0, []
-        for sidx in range(nb):
-            qs = perturbed_charge_values(inp, sidx)
-            t0 = time.perf_counter()
-            s2.set_charges(qs)
-            torch.cuda.synchronize()
-            t_sc32 += time.perf_counter() - t0
-            it_sc32.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
-        s2.close()
-        nbc = 2 * (inp.nz * inp.ny + inp.nz * inp.nx + inp.ny * inp.nx)
-        terms = float(nbc) * len(m["charges"])
-        setup = {"create_from_atoms_ms": 1e3 * t_fa, "set_charges_ms": 1e3 * t_sc / nb, "solve_ms": 1e3 * t_sv / nb,
-                 "mean_iters": float(np.mean(it_sc)), "members": nb, "atoms": int(len(m["charges"])),
-                 "dh_terms": terms, "dh_gterms_per_s": terms / (t_sc / nb) / 1e9,
-                 "set_charges_f32_ms": 1e3 * t_sc32 / nb, "dh_f32_gterms_per_s": terms / (t_sc32 / nb) / 1e9,
-                 "mean_iters_f32_boundary": float(np.mean(it_sc32)),
-                 "host_generator_s": t_gen,
-                 "note": "pb_create_from_atoms = mask + faces + salt + charges + Debye-Hueckel ghosts + pb_create "
-                         "(incl. plan autotune); set_charges = charge spreading + the fp64 DH boundary sum (ALU-bound); "
-                         "set_charges_f32 = the same with the boundary terms in fp32 (pb_set_setup_precision)"}
+        setup = run_setup_from_atoms(args, pkg, inp, prec, tol, stream, out_d, t_gen, n_batch, torch)
 
     # ---- roofline of the dominant kernel (K_spmv), CUDA events around every launch ----------------
-    solver.solve_begin(prec)
-    solver.iterate(prec, 5)
-    ms_spmv, ms_vec = solver.profile(prec, args.profile_iters)
     peak, peak_src = measured_peak()
     wl = workload_name(args.config, prec, tol)
-    pal = solver.palette_size()
-    # Bytes per launch.  `achieved` counts the bytes k_spmv_tma HAS to move in its storage format: 10 words per node
-    # (tighter variant) -- or, when the operator's face dielectrics fit a <= 256-entry palette, 7 words
-    # + 3 index bytes (the three face arrays are stored losslessly as one byte per face).  ncu's DRAM byte count
-    # (`traffic`) is compared with exactly this number.  The same time charged with SURVEY's uncompressed 10 words is
-    # given under `survey_10word` for reference (it exceeds the copy peak because fewer bytes are really moved).
-    # ... and 6 words + 4 index bytes when the Jacobi diagonal too fits a palette (pb_bytes_per_node reports the format).
-    spmv_node = solver.bytes_per_node(prec, 0)
-    spmv_bytes = spmv_node * n_node
-    ach = spmv_bytes / (ms_spmv * 1e-3) / 1e9
-    pald = solver.diag_palette_size()
-    vec_node = solver.bytes_per_node(prec, 1)       # Dinv as one index byte with the diagonal palette
-    vec_bytes = vec_node * n_node
+    kr = kernel_roofline(solver, prec, n_node, args.profile_iters, peak)
+    ms_spmv, ms_vec = kr["spmv_ms"], kr["vec_ms"]
+    pal, pald = solver.palette_size(), solver.diag_palette_size()
+    # Bytes per launch.  `achieved` counts the bytes k_spmv_tma HAS to move in the storage format the handle uses
+    # (pb_bytes_per_node): 10 words per node (tighter variant), or 6 words + 4 index bytes when the face
+    # dielectrics and the Jacobi diagonal fit the palettes (lossless byte indices).  The same time charged with SURVEY's
+    # uncompressed 10 words is given under `survey_10word` (it exceeds the copy peak because fewer bytes really move).
+    spmv_bytes = kr["spmv_bytes_per_node"] * n_node
+    vec_bytes = kr["vec_bytes_per_node"] * n_node
     iter_bytes = spmv_bytes + vec_bytes
     ns_bytes = WORDS_NORTH_STAR * elt * n_node
     t_solve = ms_local * 1e-3
-    roofline = {"bound": "hbm", "kernel": "k_spmv_tma", "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": ncu_traffic(f"k_spmv:{wl}"), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": spmv_bytes, "bytes_per_node": spmv_node, "palette_size": pal,
-                "ms_per_launch": ms_spmv,
+    committed = ncu_traffic(f"k_spmv:{wl}")
+    roofline = {"bound": "hbm", "kernel": "k_spmv_tma", "achieved": kr["spmv_GBs"], "peak": peak, "unit": "GB/s",
+                "frac": kr["spmv_frac"], "traffic": committed, "traffic_ncu_committed": committed,
+                "traffic_source": "profiles/ncu_traffic.csv: dram__bytes of a committed ncu --set full capture of this "
+                                  "kernel and workload; NOT measured in this run",
+                "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": spmv_bytes, "bytes_per_node": kr["spmv_bytes_per_node"],
+                "bytes_accounting": "stored-format bytes (pb_bytes_per_node): what physically has to cross HBM; "
+                                    "SURVEY 8(d)'s uncompressed words are in survey_10word / iteration.north_star_*",
+                "palette_size": pal, "ms_per_launch": ms_spmv, "plan": plan_summary(solver, prec),
                 "survey_10word": {"bytes_per_launch": WORDS_SPMV * elt * n_node,
-                                  "GBs": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9},
-                "k_vec": {"achieved": vec_bytes / (ms_vec * 1e-3) / 1e9, "frac": vec_bytes / (ms_vec * 1e-3) / 1e9 / peak,
-                          "bytes_per_node": vec_node, "diag_palette_size": pald, "ms_per_launch": ms_vec},
+                                  "GBs": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9,
+                                  "frac": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9 / peak},
+                "k_vec": {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
+                          "diag_palette_size": pald, "ms_per_launch": ms_vec},
                 "iteration": {"achieved": iter_bytes * iters / t_solve / 1e9,
                               "frac": iter_bytes * iters / t_solve / 1e9 / peak,
                               "north_star_16word_GBs": ns_bytes * iters / t_solve / 1e9,
@@ -427,20 +401,25 @@ def run_ours(args, rank, local_rank, world):
                                       "the whole timed solves (init, polls, finish included); north_star_*: the same time "
                                       "charged with SURVEY.md 8(d)'s 16 words per node per iteration"}}
 
+    # ---- the other precision and the word (no-palette) format of the same workload, N = 1 only --------------------
+    if world == 1 and not args.no_variants:
+        other = "f64" if prec == "f32" else "f32"
+        try:
+            roofline[other] = variant_leg(solver, torch, stream, other, TOL[other], args, inp, peak)
+            solver.set_option("palette", 0)        # word format: 40 B (fp32) / 80 B (fp64) per node in k_spmv_tma
+            roofline["no_palette"] = variant_leg(solver, torch, stream, prec, tol, args, inp, peak)
+            roofline["no_palette"]["note"] = ("PB_OPT_PALETTE = 0: face dielectrics and Dinv as full words, the format an "
+                                              "operator with a continuum of face values (e.g. fractional-edge harmonic "
+                                              "weights, PAPER.md:182) gets")
+            solver.set_option("palette", 1)
+        except pkg.PBError as e:                   # e.g. out of memory on a smaller device: report, do not hide
+            roofline["variants_error"] = str(e)
+
     line = None
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            from oracle import pbref
-
-            sample = args.cpu_sample_iters or max(2, min(400, int(1.2e10 / n_node)))
-            ref = pbref.from_inputs(inp)
-            t0 = time.perf_counter()
-            o = ref.solve(tol, sample)
-            dt = time.perf_counter() - t0
-            ref.close()
-            cpu = {"value": o["iters"] / dt, "unit": UNIT, "cores": pbref.num_threads(), "kind": "oracle",
-                   "sample": f"first {o['iters']} PCG iterations of {wl} (fp64 C/OpenMP oracle, {dt:.1f} s)"}
+            cpu = cpu_baseline(args, inp, tol, wl)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
@@ -466,11 +445,177 @@ def run_ours(args, rank, local_rank, world):
     return line
 
 
+def variant_leg(solver, torch, stream, prec, tol, args, inp, peak):
+    """One warm-up and two timed solves plus the per-kernel roofline of another precision / storage format of the
+    SAME workload and handle (the headline `value` is not touched by this)."""
+    tdt = torch.float32 if prec == "f32" else torch.float64
+    solver.prepare(prec)
+    out = torch.empty(solver.shape, dtype=tdt, device=f"cuda:{torch.cuda.current_device()}")
+    iters, ms, res = timed_solves(solver, torch, stream, prec, tol, args, out, steps=2, warmup=1)
+    kr = kernel_roofline(solver, prec, inp.n, max(10, args.profile_iters // 2), peak)
+    del out
+    return {"dtype": prec, "tol": tol, "value": iters / (ms * 1e-3), "unit": UNIT, "iterations_per_solve": res["iters"],
+            "final_relres": res["relres"], "ms_per_solve": ms / 2, "kernel": "k_spmv_tma",
+            "achieved": kr["spmv_GBs"], "frac": kr["spmv_frac"], "bytes_per_node": kr["spmv_bytes_per_node"],
+            "ms_per_launch": kr["spmv_ms"],
+            "k_vec": {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
+                      "ms_per_launch": kr["vec_ms"]},
+            "iteration_frac": (kr["spmv_bytes_per_node"] + kr["vec_bytes_per_node"]) * inp.n * iters / (ms * 1e-3) / 1e9 / peak,
+            "plan": plan_summary(solver, prec)}
+
+
+def run_batch(args, solver, inp, prec, tol, n_batch, rank, world, local_rank, dev, out_d, torch):
+    """Config 5's perturbed-charge batch on one operator: pb_set_rhs + pb_solve per member (cold start), and each member
+    solved again from the previous member's potential (pb_solve_from, NEXT row f2)."""
+    from workloads import perturbed_charges
+
+    t_b, it_b, t_w, it_w, t_gen = 0.0, [], 0.0, [], 0.0
+    out_w = torch.empty_like(out_d)
+    for sidx in range(n_batch):
+        t0 = time.perf_counter()
+        rhs_s, bc_s = perturbed_charges(inp, world * sidx + rank, device=f"cuda:{local_rank}")
+        rhs_d = torch.from_numpy(np.ascontiguousarray(rhs_s)).to(dev)
+        bc_d = torch.from_numpy(np.ascontiguousarray(bc_s)).to(dev)
+        torch.cuda.synchronize()
+        t_gen += time.perf_counter() - t0
+        t0 = time.perf_counter()
+        solver.set_rhs(rhs_d, bc_d)
+        it_b.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
+        torch.cuda.synchronize()
+        t_b += time.perf_counter() - t0
+        if sidx == 0:
+            out_w.copy_(out_d)
+        else:
+            t0 = time.perf_counter()
+            it_w.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_w,
+                                     phi0=out_w)["iters"])
+            torch.cuda.synchronize()
+            t_w += time.perf_counter() - t0
+        del rhs_d, bc_d
+    return {"solves": n_batch, "solves_per_s": n_batch / t_b, "ms_per_solve": 1e3 * t_b / n_batch,
+            "iterations_per_s": float(np.sum(it_b)) / t_b,
+            "mean_iters": float(np.mean(it_b)), "min_iters": int(min(it_b)), "max_iters": int(max(it_b)),
+            "warm_start": ({"mean_iters": float(np.mean(it_w)), "ms_per_solve": 1e3 * t_w / len(it_w),
+                            "solves_per_s": len(it_w) / t_w} if it_w else None),
+            "member_generation_s": t_gen,
+            "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member (wall clock, sequential), this rank only; "
+                    "warm_start: the same members solved again from the previous member's potential (pb_solve_from); "
+                    "member_generation_s = host/torch generation of the members' rhs and ghost values, not timed above"}
+
+
+def run_setup_from_atoms(args, pkg, inp, prec, tol, stream, out_d, t_gen, n_batch, torch):
+    from workloads import perturbed_charge_values
+
+    m = inp.meta
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    s2 = pkg.PBSolver.from_atoms(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], m["radii"], m["charges"],
+                                 m["eps_in"], m["eps_out"], m["kbar2_solvent"], stream=stream.cuda_stream)
+    torch.cuda.synchronize()
+    t_fa = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    s2.prepare(prec)
+    torch.cuda.synchronize()
+    t_prep = time.perf_counter() - t0
+    nb = min(n_batch, 10) if n_batch > 0 else 3
+    t_sc, t_sv, it_sc = 0.0, 0.0, []
+    for sidx in range(nb):
+        qs = perturbed_charge_values(inp, sidx)
+        t0 = time.perf_counter()
+        s2.set_charges(qs)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        it_sc.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
+        torch.cuda.synchronize()
+        t_sc += t1 - t0
+        t_sv += time.perf_counter() - t1
+    # the same charge updates with the boundary terms in fp32 (pb_set_setup_precision)
+    s2.set_setup_precision("f32")
+    t_sc32, it_sc32 = 0.0, []
+    for sidx in range(nb):
+        qs = perturbed_charge_values(inp, sidx)
+        t0 = time.perf_counter()
+        s2.set_charges(qs)
+        torch.cuda.synchronize()
+        t_sc32 += time.perf_counter() - t0
+        it_sc32.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
+    s2.close()
+    nbc = 2 * (inp.nz * inp.ny + inp.nz * inp.nx + inp.ny * inp.nx)
+    terms = float(nbc) * len(m["charges"])
+    return {"create_from_atoms_ms": 1e3 * t_fa, "prepare_ms": 1e3 * t_prep, "set_charges_ms": 1e3 * t_sc / nb,
+            "solve_ms": 1e3 * t_sv / nb,
+            "mean_iters": float(np.mean(it_sc)), "members": nb, "atoms": int(len(m["charges"])),
+            "dh_terms": terms, "dh_gterms_per_s": terms / (t_sc / nb) / 1e9,
+            "set_charges_f32_ms": 1e3 * t_sc32 / nb, "dh_f32_gterms_per_s": terms / (t_sc32 / nb) / 1e9,
+            "mean_iters_f32_boundary": float(np.mean(it_sc32)),
+            "host_generator_s": t_gen,
+            "note": "pb_create_from_atoms = mask + faces + salt + charges + Debye-Hueckel ghosts + pb_create; prepare = "
+                    "work arrays + plan autotune; set_charges = charge spreading + the fp64 DH boundary sum (ALU-bound); "
+                    "set_charges_f32 = the same with the boundary terms in fp32 (pb_set_setup_precision)"}
+
+
+def cpu_baseline(args, inp, tol, wl):
+    """The fp64 oracle, as it stands, on the host cores: a bounded sample of the benchmarked workload, plus (BASELINE.md
+    section 3) every smaller config, with 1 thread as well for grids <= 129^3 (the paper's CPU/CG is single-core,
+    PAPER.md:184).  A reported baseline, not the target."""
+    from oracle import pbref
+    from workloads import make_config
+
+    n_node = inp.n
+    sample = args.cpu_sample_iters or max(2, min(400, int(1.2e10 / n_node)))
+    ncores = pbref.num_threads()
+    ref = pbref.from_inputs(inp)
+    t0 = time.perf_counter()
+    o = ref.solve(tol, sample)
+    dt = time.perf_counter() - t0
+    ref.close()
+    cpu = {"value": o["iters"] / dt, "unit": UNIT, "cores": ncores, "kind": "oracle", "dtype": "f64",
+           "sample": f"first {o['iters']} PCG iterations of {wl} (fp64 C/OpenMP oracle, {dt:.1f} s)"}
+    if args.cpu_per_config:
+        per = {}
+        for cfg in range(1, args.config):
+            ci = make_config(cfg, device="cuda")
+            for ptol in sorted({TOL["f32"], TOL["f64"]}, reverse=True):
+                for threads in ([ncores, 1] if GRID[cfg] <= 129 else [ncores]):
+                    budget = int(6e8 / ci.n) + 2 if threads > 1 else int(1.5e8 / ci.n) + 2
+                    pbref.set_num_threads(threads)
+                    r = pbref.from_inputs(ci)
+                    t0 = time.perf_counter()
+                    oo = r.solve(ptol, min(5000, budget))
+                    d = time.perf_counter() - t0
+                    r.close()
+                    per[f"config{cfg}_{GRID[cfg]}^3_tol{ptol:g}_{threads}thr"] = {
+                        "iterations": oo["iters"], "converged": oo["status"] == 0, "s": d,
+                        "iterations_per_s": oo["iters"] / d if d > 0 else None}
+            pbref.set_num_threads(ncores)
+        cpu["per_config"] = per
+    return cpu
+
+
+def self_launch(args, argv):
+    """`python bench.py --gpus N` (N > 1) started without a launcher: start the N local ranks ourselves, the way the
+    driver does (torch.distributed.run, one rank per GPU, rendezvous on 127.0.0.1)."""
+    import socket
+    import subprocess
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+    return subprocess.call(cmd)
+
+
 def main(argv=None):
+    argv = list(sys.argv[1:] if argv is None else argv)
     args = parse_args(argv)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(self_launch(args, argv))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; reporting n_gpus={world}", file=sys.stderr)
     if args.impl == "reference":
         line = run_reference(args, rank, world)
     else:

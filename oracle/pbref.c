@@ -76,6 +76,17 @@ int pbref_num_threads(void)
 #endif
 }
 
+/* thread count for the timed CPU baseline (bench.py: all cores, and 1 thread for grids <= 129^3 like the paper's
+ * single-core CPU/CG); results do not depend on it (whole planes per thread, see above) */
+void pbref_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 static double *dup_array(const double *src, size_t n)
 {
     double *d = (double *)malloc((n ? n : 1) * sizeof(double));

@@ -47,12 +47,18 @@ def _load():
         lib.pbref_destroy.argtypes = [vp]
         lib.pbref_set_periodic.argtypes = [vp, ci]
         lib.pbref_num_threads.restype = ci
+        lib.pbref_set_num_threads.argtypes = [ci]
         _lib = lib
     return _lib
 
 
 def num_threads() -> int:
     return int(_load().pbref_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    """OpenMP threads of later oracle calls (timing only: results are bit-identical for any count)."""
+    _load().pbref_set_num_threads(int(n))
 
 
 def _ptr(a):

@@ -58,3 +58,19 @@ def test_single_rank_aggregate_is_identity():
 
     assert bench.aggregate(7, 3.5, 1) == (7.0, 3.5)
     assert bench.workload_name(5, "f32", 1e-5) == "config5_385^3_f32_tol1e-05"
+
+
+def test_gpus_flag_launches_its_own_ranks():
+    """`python bench.py --gpus 2` started WITHOUT a launcher must start two local ranks itself (torch.distributed.run on
+    127.0.0.1) and report n_gpus 2; on the reference arm rank 0 alone works and prints, rank 1 exits 0."""
+    import json
+    import subprocess
+
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    env["OMP_NUM_THREADS"] = "2"
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--config", "1",
+                        "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [json.loads(l) for l in p.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # one JSON line, from rank 0
+    assert lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2 and lines[0]["value"] > 0
