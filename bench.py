@@ -54,6 +54,8 @@ def parse_args(argv=None):
     ap.add_argument("--batch", type=int, default=None,
                     help="solves of config 5's perturbed-charge batch on the same operator (default: 50 at --gpus 1 "
                          "--config 5, else 0)")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="per-handle option for the benchmarked solver (pb_set_option names of the binding), repeatable")
     ap.add_argument("--no-variants", action="store_true",
                     help="skip the other-precision and no-palette legs of the roofline record")
     ap.add_argument("--cpu-per-config", action="store_true",
@@ -214,7 +216,7 @@ def plan_summary(solver, prec):
     """The launch plan that produced a number (pb_get_plan), as it goes into the JSON line."""
     pl = solver.plan(prec)
     keep = ("txv", "ty", "tz", "ring_slots", "blocks_per_sm", "tiles", "grid", "threads", "smem_bytes", "autotuned",
-            "vec_grid", "vec_threads", "persist", "face_palette", "diag_palette_vec", "diag_palette_spmv",
+            "vec_grid", "vec_threads", "persist", "face_palette", "face_quad", "diag_palette_vec", "diag_palette_spmv",
             "palette_size", "diag_palette_size", "num_sm", "pitch")
     return {k: pl[k] for k in keep}
 
@@ -278,8 +280,9 @@ def run_ours(args, rank, local_rank, world):
 
     stream = torch.cuda.Stream(device=dev)
     t_create = time.perf_counter()
+    options = {k: int(v) for k, v in (kv.split("=", 1) for kv in args.opt)}
     solver = pkg.PBSolver(inp.nx, inp.ny, inp.nz, inp.h, inp.eps_x, inp.eps_y, inp.eps_z, inp.kbar2, rhs, bc,
-                          stream=stream.cuda_stream)
+                          stream=stream.cuda_stream, options=options)
     solver.prepare(prec)                     # work arrays of this precision + plan autotune (pb_prepare)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
@@ -429,7 +432,7 @@ def run_ours(args, rank, local_rank, world):
                            "parallelism": f"replicas x{world} (one right-hand side per GPU)",
                            "l2": "working set 11 arrays x %.0f MB >> 126 MB L2 (inputs larger than L2)"
                                  % (n_node * elt / 1e6) if n_node * elt * 11 > 4e8 else "working set fits L2",
-                           "create_ms": 1e3 * t_create, "input_generation_s": t_gen},
+                           "create_ms": 1e3 * t_create, "input_generation_s": t_gen, "options": options},
                 "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
                 "roofline": roofline, "cpu_baseline": cpu}
         if batch is not None:

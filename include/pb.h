@@ -213,7 +213,9 @@ typedef enum {
     PB_OPT_VEC_BLOCKS_PER_SM = 13,   /* k_vec blocks per SM (0 = automatic)                                          */
     PB_OPT_GRAPH = 14,               /* 1 (default): check_every iterations are launched as one CUDA graph           */
     PB_OPT_L2_HINTS = 15,            /* bit mask of L2 eviction-priority hints (default 0: none; measured not to help) */
-    PB_OPT_COUNT_ = 16
+    PB_OPT_PALETTE_QUAD = 16,        /* 1 (default): face palettes of <= 4 values as 2-bit indices, four nodes per byte
+                                        (k_spmv_quad); 0: one index byte per face (k_spmv_tma)                         */
+    PB_OPT_COUNT_ = 17
 } pb_option;
 
 pb_status pb_set_option(pb_handle *h, pb_option opt, int value);
@@ -238,7 +240,8 @@ typedef struct {
     int spmv_bytes_per_node;  /* stored-format bytes per node and launch, as pb_bytes_per_node         */
     int vec_bytes_per_node;
     int pitch;                /* padded row length in elements                                         */
-    int reserved[8];
+    int face_quad;            /* 1: faces as 2-bit indices, four nodes per byte (k_spmv_quad)          */
+    int reserved[7];
 } pb_plan;
 
 /* pb_prepare -- build the work arrays of `prec` (setup row a0: padded coefficients, diagonal, folded b) and pick

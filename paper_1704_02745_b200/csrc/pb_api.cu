@@ -5,6 +5,7 @@
 #include "../../include/pb.h"
 #include "pb_kernels.cuh"
 #include "pb_spmv_tma.cuh"
+#include "pb_spmv_quad.cuh"
 #include "pb_persist.cuh"
 #include "pb_setup.cuh"
 #include "pb_grid.cuh"
@@ -49,6 +50,11 @@ struct Work {
     bool pald_s = false;             // k_spmv_tma reads Dinv through the index tensor too
     T *dlut = nullptr;
     int Pb = 0;
+    // quad format (k_spmv_quad): face palettes of <= 4 values as 2-bit indices, four nodes per byte
+    bool quad = false;
+    unsigned char *exq = nullptr, *exqp = nullptr, *eyq = nullptr, *ezq = nullptr;
+    int Pq = 0;
+    CUtensorMap tm_exqp;
 };
 
 }  // namespace
@@ -128,7 +134,7 @@ void default_options(int *opt)
     opt[PB_OPT_PERSIST_BLOCKS_PER_SM] = 4; opt[PB_OPT_PALETTE] = 1; opt[PB_OPT_PALETTE_DIAG] = 1;
     opt[PB_OPT_PALETTE_DIAG_SPMV] = 1; opt[PB_OPT_AUTOTUNE] = 1; opt[PB_OPT_TILE_TXV] = 0; opt[PB_OPT_TILE_TY] = 0;
     opt[PB_OPT_TILE_TZ] = 0; opt[PB_OPT_RING_SLOTS] = 0; opt[PB_OPT_BLOCKS_PER_SM] = 0; opt[PB_OPT_VEC_BLOCKS_PER_SM] = 0;
-    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0;
+    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_PALETTE_QUAD] = 1;
 }
 
 inline int grid_for(size_t n, int block, int cap)
@@ -153,7 +159,7 @@ void free_work(Work<T> &w)
     T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.tmp, &w.p0, &w.p1, &w.Ap};
     for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
-    unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi};
+    unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi, &w.exq, &w.exqp, &w.eyq, &w.ezq};
     for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.lut) { cudaFree(w.lut); w.lut = nullptr; }
     if (w.dvi) { cudaFree(w.dvi); w.dvi = nullptr; }
@@ -240,8 +246,11 @@ pb_status build_work(pb_handle *h, Work<T> &w)
     // k_spmv_tma decodes through tables addressed by pre-scaled index bytes: n * sizeof(T) <= 256 entries-bytes
     w.pal = h->pal_n > 0 && (size_t)h->pal_n * sizeof(T) <= 256;
     w.pald = w.pal && h->pald_n > 0;
-    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
+    w.quad = w.pal && h->pal_n <= 4 && h->opt[PB_OPT_PALETTE_QUAD] != 0;
+    // k_spmv_tma: pre-scaled index bytes (n * sizeof(T) <= 256); k_spmv_quad: plain index bytes into a pair table
+    w.pald_s = w.pald && (w.quad || (size_t)h->pald_n * sizeof(T) <= 256) && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
     w.Pb = (w.P + 15) / 16 * 16;
+    w.Pq = ((w.P + 3) / 4 + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
         int coop = 0;
@@ -260,7 +269,12 @@ pb_status build_work(pb_handle *h, Work<T> &w)
         return s;
     }
     if (w.pald_s && (s = alloc_arr(&w.dvib, (size_t)h->nz * h->ny * w.Pb))) { free_work(w); return s; }
-    if (w.pal) {
+    if (w.quad) {
+        const size_t b_ex = (size_t)h->nz * h->ny * w.Pq, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pq,
+                     b_ez = (size_t)(h->nz + 1) * h->ny * w.Pq;
+        if ((s = alloc_arr(&w.exq, b_ex)) || (s = alloc_arr(&w.exqp, b_ex)) || (s = alloc_arr(&w.eyq, b_ey)) ||
+            (s = alloc_arr(&w.ezq, b_ez)) || (s = alloc_arr(&w.lut, (size_t)kPalMax))) { free_work(w); return s; }
+    } else if (w.pal) {
         const size_t b_ex = (size_t)h->nz * h->ny * w.Pb, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pb,
                      b_ez = (size_t)(h->nz + 1) * h->ny * w.Pb;
         if ((s = alloc_arr(&w.exi, b_ex)) || (s = alloc_arr(&w.eyi, b_ey)) || (s = alloc_arr(&w.ezi, b_ez)) ||
@@ -301,7 +315,12 @@ pb_status build_work(pb_handle *h, Work<T> &w)
     k_setup_coeff<T><<<grid_for(total, 256, h->nsm * 16), 256, 0, h->stream>>>(
         h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
         w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
-    if (w.pal) {
+    if (w.quad) {
+        k_setup_quad_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pq, 256, h->nsm * 16), 256, 0, h->stream>>>(
+            h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pq, h->pal_table, w.exq, w.exqp, w.eyq, w.ezq);
+        k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
+        h->launches += 2;
+    } else if (w.pal) {
         k_setup_pal_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
             h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pal_table, w.exi, w.eyi, w.ezi);
         k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
@@ -314,7 +333,8 @@ pb_status build_work(pb_handle *h, Work<T> &w)
         h->launches += 2;
         if (w.pald_s) {
             k_setup_diag_idx<<<grid_for((size_t)h->nz * h->ny * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
-                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pald_table, w.dvib);
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, w.quad ? 1 : (int)sizeof(T),
+                h->pald_table, w.dvib);
             h->launches += 1;
         }
     }
@@ -405,7 +425,8 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qnty = (h->ny + TY - 1) / TY;
     w.qthreads = (spmv_row_threads(TXV) * TY + 31) / 32 * 32 + 32;
     const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0, w.pald_s);
-    w.qsmem = (size_t)NS * L.slot + 128;
+    const QuadLayout Q = quad_layout(TXV, TY, VEC, w.pald_s);
+    w.qsmem = w.quad ? (size_t)NS * Q.slot + 2 * Q.pn + 128 : (size_t)NS * L.slot + 128;
     if (w.qsmem > w.qmaxdyn || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
     const int slots = h->nsm * c.bps;
     const int xy = w.qntx * w.qnty;
@@ -434,12 +455,17 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qgrid = (int)(ntiles < slots ? ntiles : slots);
     PB_TRY(make_map<T>(&w.tm_r, w.r, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_tmp, w.tmp, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
-    if (w.pald_s) PB_TRY(make_map_u8(&w.tm_dinv, w.dvib, w.Pb, h->ny, h->nz, L.bwd, TY + 2));
+    if (w.pald_s) PB_TRY(make_map_u8(&w.tm_dinv, w.dvib, w.Pb, h->ny, h->nz, w.quad ? Q.bwd : L.bwd, TY + 2));
     else PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_x, w.x, w.P, h->ny, h->nz, TXV * VEC, TY));
-    if (w.pal) {
+    if (w.quad) {
+        PB_TRY(make_map_u8(&w.tm_ex, w.exq, w.Pq, h->ny, h->nz, Q.bwq, TY));
+        PB_TRY(make_map_u8(&w.tm_exqp, w.exqp, w.Pq, h->ny, h->nz, Q.bwq, TY));
+        PB_TRY(make_map_u8(&w.tm_ey, w.eyq, w.Pq, h->ny + 1, h->nz, Q.bwq, TY + 1));
+        PB_TRY(make_map_u8(&w.tm_ez, w.ezq, w.Pq, h->ny, h->nz + 1, Q.bwq, TY));
+    } else if (w.pal) {
         PB_TRY(make_map_u8(&w.tm_ex, w.exi, w.Pb, h->ny, h->nz, L.bw, TY));
         PB_TRY(make_map_u8(&w.tm_ey, w.eyi, w.Pb, h->ny + 1, h->nz, L.bw, TY + 1));
         PB_TRY(make_map_u8(&w.tm_ez, w.ezi, w.Pb, h->ny, h->nz + 1, L.bw, TY));
@@ -454,8 +480,16 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
 template <typename T, int MODE> void launch_spmv(pb_handle *h, Work<T> &w, double out_scale);
 
 // deepest ring (<= 6 slots) that lets `bps` blocks of this tile share one SM's shared memory
-inline int ring_depth(int TXV, int TY, int bps, int pal_vec, bool pald)
+inline int ring_depth(int TXV, int TY, int bps, int pal_vec, bool pald, int quad_vec = 0)
 {
+    if (quad_vec) {
+        // k_spmv_quad: statics = barriers + the quadruple table (256 x 4 values) + the pair table; two p_new planes
+        const QuadLayout Q = quad_layout(TXV, TY, quad_vec, pald);
+        const long per_block = (long)232448 / bps - 1024 - 1200 - 256 * 4 * (16 / quad_vec) - (pald ? 512 * (16 / quad_vec) : 0)
+                               - 2 * (long)Q.pn - 128;
+        const int NS = per_block > 0 ? (int)(per_block / (long)Q.slot) : 0;
+        return NS > kMaxStages ? kMaxStages : NS;
+    }
     // 227 KB per SM, 1 KB reserved per block, statics (barriers, reduction scratch, up to three 256-entry tables)
     const size_t per_block = (size_t)232448 / bps - 1024 - 3200 - (pald ? 2 * 256 * (16 / pal_vec) : 0);
     int NS = (int)(per_block / slot_layout(TXV, TY, pal_vec, pald).slot);
@@ -483,7 +517,9 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         return PB_OK;
     };
     size_t lim0 = 0, lim1 = 0;
-    if (w.pald_s) { PB_TRY(allow(k_spmv_tma<T, 0, true, true>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, true>, &lim1)); }
+    if (w.quad && w.pald_s) { PB_TRY(allow(k_spmv_quad<T, 0, true>, &lim0)); PB_TRY(allow(k_spmv_quad<T, 1, true>, &lim1)); }
+    else if (w.quad) { PB_TRY(allow(k_spmv_quad<T, 0, false>, &lim0)); PB_TRY(allow(k_spmv_quad<T, 1, false>, &lim1)); }
+    else if (w.pald_s) { PB_TRY(allow(k_spmv_tma<T, 0, true, true>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, true>, &lim1)); }
     else if (w.pal) { PB_TRY(allow(k_spmv_tma<T, 0, true, false>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, false>, &lim1)); }
     else { PB_TRY(allow(k_spmv_tma<T, 0, false, false>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, false, false>, &lim1)); }
     w.qmaxdyn = lim0 < lim1 ? lim0 : lim1;
@@ -506,9 +542,9 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         if (c.TY < 1) c.TY = 1;
         if (c.TY > h->ny) c.TY = h->ny;
         while (spmv_row_threads(c.TXV) * c.TY > 448 && c.TY > 1) c.TY--;
-        c.bps = opt_or(PB_OPT_BLOCKS_PER_SM, ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s) >= 4 ? 2 : 1);
+        c.bps = opt_or(PB_OPT_BLOCKS_PER_SM, ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s, w.quad ? VEC : 0) >= 4 ? 2 : 1);
         if (c.bps < 1) c.bps = 1;
-        c.NS = opt_or(PB_OPT_RING_SLOTS, ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s));
+        c.NS = opt_or(PB_OPT_RING_SLOTS, ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s, w.quad ? VEC : 0));
         c.TZ = o[PB_OPT_TILE_TZ];
         cand[nc++] = c;
     } else {
@@ -521,7 +557,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
                 int TY = ty > h->ny ? h->ny : ty;
                 if (spmv_row_threads(TXV) * TY > 448) continue;
                 for (int bps = 1; bps <= 4; bps++) {
-                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0, w.pald_s);
+                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0, w.pald_s, w.quad ? VEC : 0);
                     if (NS < 4 && !(NS == 3 && bps >= 2)) continue;
                     const int cthreads = ((spmv_row_threads(TXV) * TY + 31) / 32 * 32) * bps;
                     if (cthreads < 256 || cthreads > 1024) continue;     // consumer threads per SM
@@ -619,6 +655,21 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->opt[PB_OPT_L2_HINTS]; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
     a.lut = w.lut; a.dlut = w.dlut;
+    if (w.quad) {
+        QuadArgs<T> q;
+        q.pbuf0 = w.p0; q.pbuf1 = w.p1; q.Ap = w.Ap; q.x = w.x;
+        q.nx = h->nx; q.ny = h->ny; q.nz = h->nz; q.P = w.P;
+        q.TXV = w.qTXV; q.TY = w.qTY; q.TZ = w.qTZ; q.ntx = w.qntx; q.nty = w.qnty; q.ntz = w.qntz;
+        q.ntiles = a.ntiles; q.nstage = w.qns; q.precond = h->precond;
+        q.st = h->st; q.partials = h->partials; q.out_scale = out_scale; q.lut = w.lut; q.dlut = w.dlut;
+        if (w.pald_s)
+            k_spmv_quad<T, MODE, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+                MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_exqp, w.tm_ey, w.tm_ez, q);
+        else
+            k_spmv_quad<T, MODE, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
+                MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_exqp, w.tm_ey, w.tm_ez, q);
+        return;
+    }
     if (w.pald_s)
         k_spmv_tma<T, MODE, true, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
             MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
@@ -930,7 +981,7 @@ int bytes_per_node_impl(pb_handle *h, int kernel)
     const Work<T> &w = work<T>(h);
     const int e = (int)sizeof(T);
     if (kernel == 0)      // r, p_old, x in; p, x, Ap out; Dinv; three face coefficients
-        return 6 * e + (w.pald_s ? 1 : e) + (w.pal ? 3 : 3 * e);
+        return 6 * e + (w.pald_s ? 1 : e) + (w.quad ? 1 : w.pal ? 3 : 3 * e);   // quad: 4 arrays x 2 bits per node
     return 3 * e + (w.pald ? 1 : e);      // r, Ap in; r out; Dinv
 }
 
@@ -1131,7 +1182,7 @@ pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
     if (!h || (int)opt < 0 || (int)opt >= (int)PB_OPT_COUNT_ || value < 0) return PB_ERR_INVALID_ARG;
     switch (opt) {
     case PB_OPT_PERSIST: case PB_OPT_PALETTE: case PB_OPT_PALETTE_DIAG: case PB_OPT_PALETTE_DIAG_SPMV:
-    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH:
+    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH: case PB_OPT_PALETTE_QUAD:
         if (value > 1) return PB_ERR_INVALID_ARG;
         break;
     case PB_OPT_PERSIST_BLOCKS_PER_SM:
@@ -1184,7 +1235,7 @@ pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
     out->diag_palette_size = h->pald_n > 0 ? h->pald_n : 0;
     auto fill = [&](const auto &w) {
         out->persist = w.persist; out->persist_fused = w.persist && w.pfused; out->persist_grid = w.persist ? w.pgrid : 0;
-        out->face_palette = w.pal; out->diag_palette_vec = w.pald; out->diag_palette_spmv = w.pald_s;
+        out->face_palette = w.pal; out->diag_palette_vec = w.pald; out->diag_palette_spmv = w.pald_s; out->face_quad = w.quad;
         out->txv = w.qTXV; out->ty = w.qTY; out->tz = w.qTZ; out->ring_slots = w.qns; out->blocks_per_sm = w.qbps;
         out->tiles = w.qntx * w.qnty * w.qntz; out->grid = w.qgrid; out->threads = w.qthreads;
         out->smem_bytes = (int)w.qsmem; out->autotuned = w.qtuned;

@@ -225,6 +225,44 @@ __global__ void k_setup_pal_idx(const double *__restrict__ eps_x, const double *
     }
 }
 
+// Quad index arrays for palettes of at most four values (k_spmv_quad): 2 bits per face, four consecutive nodes of a
+// row per byte (node i -> bits 2(i&3) of byte i>>2), rows of Pq bytes.  exq holds the MINUS x-face of every node
+// (face i), exqp its PLUS x-face (face i+1), eyq / ezq the minus y- / z-faces with one extra row / plane (the plus
+// face of a node is the minus face of its neighbour).  Pad nodes (i >= nx) get the index of 0.0.
+__global__ void k_setup_quad_idx(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
+                                 const double *__restrict__ eps_z, int nx, int ny, int nz, int Pq,
+                                 const PalTable *t, unsigned char *exq, unsigned char *exqp, unsigned char *eyq,
+                                 unsigned char *ezq)
+{
+    const unsigned int zero = pal_index(t, 0.0);
+    const size_t total = (size_t)(nz + 1) * (ny + 1) * Pq;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        const int bq = (int)(q % Pq);
+        const size_t u = q / Pq;
+        const int j = (int)(u % (ny + 1)), k = (int)(u / (ny + 1));
+        unsigned int bm = 0, bp = 0, by = 0, bz = 0;
+        for (int f = 0; f < 4; f++) {
+            const int i = 4 * bq + f;
+            unsigned int im = zero, ip = zero, iy = zero, iz = zero;
+            if (i < nx) {
+                if (k < nz && j < ny) {
+                    im = pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i]);
+                    ip = pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i + 1]);
+                }
+                if (k < nz) iy = pal_index(t, eps_y[((size_t)k * (ny + 1) + j) * nx + i]);
+                if (j < ny) iz = pal_index(t, eps_z[((size_t)k * ny + j) * nx + i]);
+            }
+            bm |= im << (2 * f); bp |= ip << (2 * f); by |= iy << (2 * f); bz |= iz << (2 * f);
+        }
+        if (k < nz && j < ny) {
+            exq[((size_t)k * ny + j) * Pq + bq] = (unsigned char)bm;
+            exqp[((size_t)k * ny + j) * Pq + bq] = (unsigned char)bp;
+        }
+        if (k < nz) eyq[((size_t)k * (ny + 1) + j) * Pq + bq] = (unsigned char)by;
+        if (j < ny) ezq[((size_t)k * ny + j) * Pq + bq] = (unsigned char)bz;
+    }
+}
+
 template <typename T>
 __global__ void k_pal_lut(const PalTable *t, T *lut)
 {

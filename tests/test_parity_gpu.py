@@ -297,13 +297,18 @@ def test_tiling_independence_with_both_palettes(pkg, prec):
     dt = np.float64 if prec == "f64" else np.float32
     x = np.random.default_rng(5).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(dt)
     ref_y = ref_p = ref_ap = None
-    for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette=0)):
+    # storage formats: quad (2-bit faces, k_spmv_quad) with Dinv index bytes / with Dinv words; byte palette
+    # (k_spmv_tma) with / without the diagonal palette; full words
+    for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette_quad=0), dict(palette_quad=0, palette_diag_spmv=0),
+                dict(palette=0)):
         for cfg in TILE_CONFIGS:
             with pkg.PBSolver(*inp.args(), options={**cfg, **fmt, "persist": 0}) as s:
                 y = s.apply(x, prec)
                 if not fmt:
-                    assert s.palette_size() > 0 and s.diag_palette_size() > 0
-                    assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
+                    assert s.palette_size() > 0 and s.diag_palette_size() > 0 and s.plan(prec)["face_quad"] == 1
+                    assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 2
+                if fmt == dict(palette_quad=0):
+                    assert s.plan(prec)["face_quad"] == 0 and s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
                 s.solve_begin(prec)
                 s.iterate(prec, 2)
                 p2, ap2 = s.vector("p"), s.vector("Ap")
@@ -533,13 +538,16 @@ def test_randomised_shapes_and_options(pkg, pbref):
     rng = np.random.default_rng(20260704)
     for case in range(24):
         nx, ny, nz = (int(v) for v in rng.integers(1, 41, 3))
-        periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), bool(rng.integers(2))
+        periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), int(rng.integers(3))
         persist, prec = int(rng.integers(2)), ("f64", "f32")[int(rng.integers(2))]
         inp = _periodic_inputs((nx, ny, nz), 100 + case) if periodic else random_operator(nx, ny, nz, seed=100 + case)
-        if not two_valued:
+        if two_valued == 0:          # a continuum of face values: word format
             inp.eps_x[...] = rng.uniform(1, 80, inp.eps_x.shape)
-            if periodic:
-                inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
+        elif two_valued == 2:        # seven face values: byte palette (k_spmv_tma), not the 2-bit quad format
+            inp.eps_y[...] = rng.choice([1.0, 2.0, 4.0, 20.0, 78.5, 80.0], inp.eps_y.shape)
+        if periodic:
+            inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
+            inp.eps_y[:, -1, :] = inp.eps_y[:, 0, :]
         tol = 1e-10 if prec == "f64" else 1e-5
         ref = pbref.from_inputs(inp)
         ref.set_periodic(periodic)
@@ -779,7 +787,7 @@ def test_options_are_handle_state(pkg):
         assert pa["persist"] == 0 and pa["face_palette"] == 0 and pa["palette_size"] == 0 and not pa["autotuned"]
         assert pa["spmv_bytes_per_node"] == 40 and pa["vec_bytes_per_node"] == 16
         assert pb_["persist"] == 1 and pb_["face_palette"] == 1 and pb_["palette_size"] == 4
-        assert pb_["spmv_bytes_per_node"] == 28 and pb_["vec_bytes_per_node"] == 13
+        assert pb_["spmv_bytes_per_node"] == 26 and pb_["vec_bytes_per_node"] == 13 and pb_["face_quad"] == 1
         assert pa["num_sm"] == pb_["num_sm"] >= 1 and pa["grid"] >= 1 and pa["threads"] % 32 == 0
         assert a.get_option("palette") == 0 and b.get_option("palette") == 1
         ga, gb = a.solve(1e-5, 5000, "f32"), b.solve(1e-5, 5000, "f32")
