@@ -216,7 +216,7 @@ def plan_summary(solver, prec):
     """The launch plan that produced a number (pb_get_plan), as it goes into the JSON line."""
     pl = solver.plan(prec)
     keep = ("txv", "ty", "tz", "ring_slots", "blocks_per_sm", "tiles", "grid", "threads", "smem_bytes", "autotuned",
-            "vec_grid", "vec_threads", "persist", "face_palette", "face_quad", "diag_palette_vec", "diag_palette_spmv",
+            "vec_grid", "vec_threads", "persist", "face_palette", "diag_palette_vec", "diag_palette_spmv",
             "palette_size", "diag_palette_size", "num_sm", "pitch")
     return {k: pl[k] for k in keep}
 

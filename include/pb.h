@@ -123,6 +123,33 @@ pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec
                         const void *phi0, void *phi_out, pb_memspace where, int *iters_out, double *relres_out);
 
 /*
+ * pb_solve_batch -- m right-hand sides on the SAME operator (NEXT row f2 of SURVEY.md 8(f); the paper's motivation is
+ * "thousands to millions of snapshots"): the Jacobi-PCG of pb_solve (phi_0 = 0) run
+ * for PB_OPT_BATCH_WIDTH members at a time by kernels that stage the operator's coefficient boxes once per plane for
+ * all of them (k_spmv_batch) and read Dinv once per node (k_vec_batch).  Every member has its own device-resident
+ * scalars and convergence latch; a member that has converged stops being read or written, the group ends when all
+ * its members are done.  Per member the arithmetic is that of a single solve (same operations in the same order per
+ * node), so its iterates, iteration count and result do not depend on the other members.
+ *   rhs [m][nz][ny][nx], bc [m][2*(nz*ny+nz*nx+ny*nx)] (either may be NULL = 0), phi_out [m][nz][ny][nx] in `prec`;
+ *   all in the memory space `where`.  iters_out / relres_out / status_out: host arrays of m entries (may be NULL);
+ *   status_out[s] is PB_OK, PB_ERR_MAXITER or PB_ERR_BREAKDOWN.
+ * Returns the worst member status (BREAKDOWN > MAXITER > OK) or an argument / CUDA error.  Needs the free-space
+ * boundary condition (PB_ERR_INVALID_ARG under pb_set_boundary(h, 1)).  The handle's own right-hand side (pb_set_rhs)
+ * is left holding the last member's when the members are host arrays.  Face palettes of at most four values are
+ * read as 2-bit indices (four nodes per byte), anything else as full words.
+ */
+pb_status pb_solve_batch(pb_handle *h, int m, const double *rhs, const double *bc, double tol, int maxiter,
+                         pb_precision prec, int check_every, void *phi_out, pb_memspace where, int *iters_out,
+                         double *relres_out, int *status_out);
+
+/* pb_solve_batch_charges -- the same for a handle made by pb_create_from_atoms: member s is the charge set
+ * charges[s][n_atoms] on the stored atoms; its right-hand side and ghost values are built on the device as in
+ * pb_set_charges (the handle's rhs / bc end up holding the last member's). */
+pb_status pb_solve_batch_charges(pb_handle *h, int m, const double *charges, double tol, int maxiter,
+                                 pb_precision prec, int check_every, void *phi_out, pb_memspace where, int *iters_out,
+                                 double *relres_out, int *status_out);
+
+/*
  * pb_create_from_atoms -- NEXT row f1, the paper's stated next step "integrated grid stencil setup on GPU"
  * (PAPER.md:11, 283): build the inputs of Eq. 3 on the device from atoms and hand them to pb_create.
  *   centres [n_atoms][3] (x,y,z; node (i,j,k) sits at (i h, j h, k h)), radii [n_atoms], charges [n_atoms]
@@ -213,8 +240,7 @@ typedef enum {
     PB_OPT_VEC_BLOCKS_PER_SM = 13,   /* k_vec blocks per SM (0 = automatic)                                          */
     PB_OPT_GRAPH = 14,               /* 1 (default): check_every iterations are launched as one CUDA graph           */
     PB_OPT_L2_HINTS = 15,            /* bit mask of L2 eviction-priority hints (default 0: none; measured not to help) */
-    PB_OPT_PALETTE_QUAD = 16,        /* 1 (default): face palettes of <= 4 values as 2-bit indices, four nodes per byte
-                                        (k_spmv_quad); 0: one index byte per face (k_spmv_tma)                         */
+    PB_OPT_BATCH_WIDTH = 16,         /* right-hand sides per pass of pb_solve_batch: 1, 2 or 4 (default 2)            */
     PB_OPT_COUNT_ = 17
 } pb_option;
 
@@ -240,8 +266,7 @@ typedef struct {
     int spmv_bytes_per_node;  /* stored-format bytes per node and launch, as pb_bytes_per_node         */
     int vec_bytes_per_node;
     int pitch;                /* padded row length in elements                                         */
-    int face_quad;            /* 1: faces as 2-bit indices, four nodes per byte (k_spmv_quad)          */
-    int reserved[7];
+    int reserved[8];
 } pb_plan;
 
 /* pb_prepare -- build the work arrays of `prec` (setup row a0: padded coefficients, diagonal, folded b) and pick

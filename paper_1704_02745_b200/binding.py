@@ -21,13 +21,13 @@ EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", 
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
            "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined", "pb_set_setup_precision", "pb_set_option", "pb_get_option",
-           "pb_prepare", "pb_get_plan")
+           "pb_prepare", "pb_get_plan", "pb_solve_batch", "pb_solve_batch_charges")
 
 # pb_option (include/pb.h), by name
 OPTIONS = {"persist": 0, "persist_max_mb": 1, "persist_fused_max_knodes": 2, "persist_blocks_per_sm": 3,
            "palette": 4, "palette_diag": 5, "palette_diag_spmv": 6, "autotune": 7, "tile_txv": 8, "tile_ty": 9,
            "tile_tz": 10, "ring_slots": 11, "blocks_per_sm": 12, "vec_blocks_per_sm": 13, "graph": 14, "l2_hints": 15,
-           "palette_quad": 16}
+           "batch_width": 16}
 
 
 class PBPlan(ctypes.Structure):
@@ -36,7 +36,7 @@ class PBPlan(ctypes.Structure):
         "precision", "num_sm", "persist", "persist_fused", "persist_grid", "palette_size", "diag_palette_size",
         "face_palette", "diag_palette_vec", "diag_palette_spmv", "txv", "ty", "tz", "ring_slots", "blocks_per_sm",
         "tiles", "grid", "threads", "smem_bytes", "autotuned", "vec_grid", "vec_threads", "spmv_bytes_per_node",
-        "vec_bytes_per_node", "pitch", "face_quad")] + [("reserved", ctypes.c_int * 7)]
+        "vec_bytes_per_node", "pitch")] + [("reserved", ctypes.c_int * 8)]
 
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -93,6 +93,10 @@ def load_library():
     lib.pb_palette_size.argtypes = [vp]
     lib.pb_diag_palette_size.argtypes = [vp]
     lib.pb_launch_count.restype = ctypes.c_longlong
+    lib.pb_solve_batch.argtypes = [vp, ci, vp, vp, cd, ci, ci, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd),
+                                   ctypes.POINTER(ci)]
+    lib.pb_solve_batch_charges.argtypes = [vp, ci, vp, cd, ci, ci, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd),
+                                           ctypes.POINTER(ci)]
     lib.pb_set_option.argtypes = [vp, ci, ci]
     lib.pb_get_option.argtypes = [vp, ci, ctypes.POINTER(ci)]
     lib.pb_prepare.argtypes = [vp, ci]
@@ -312,6 +316,61 @@ class PBSolver:
         if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
             raise PBError(st, "pb_solve")
         return dict(phi=out, iters=it.value, relres=rel.value, status=st)
+
+    def _batch_out(self, m, dt, out, like):
+        n = self.nx * self.ny * self.nz
+        if out is None:
+            if like is not None and _is_torch(like) and like.is_cuda:
+                import torch
+
+                out = torch.empty((m,) + self.shape, dtype={np.float32: torch.float32, np.float64: torch.float64}[dt],
+                                  device=like.device)
+            else:
+                out = np.empty((m,) + self.shape, dtype=dt)
+        if not _is_torch(out) and (out.dtype != dt or not out.flags.c_contiguous):
+            raise TypeError("out must be a C-contiguous array of the requested precision")
+        op, so, keep = _marshal(out, dt, m * n, "out")
+        if _is_torch(out) and keep.data_ptr() != out.data_ptr():
+            raise TypeError("out must be contiguous")
+        return out, op, so
+
+    def solve_batch(self, rhs, bc, tol, maxiter, precision="f32", check_every=32, out=None):
+        """pb_solve_batch: m right-hand sides on this operator, PB_OPT_BATCH_WIDTH members per kernel pass.
+        rhs [m][nz][ny][nx], bc [m][nbc] (numpy / CUDA tensors, same memory space; either may be None = 0).
+        Returns dict(phi [m][nz][ny][nx], iters [m], relres [m], status [m], worst)."""
+        pc, dt = _prec(precision)
+        n = self.nx * self.ny * self.nz
+        nbc = 2 * (self.nz * self.ny + self.nz * self.nx + self.ny * self.nx)
+        src = rhs if rhs is not None else bc
+        if src is None:
+            raise ValueError("rhs and bc cannot both be None")
+        m = int(src.shape[0])
+        rh, s1, k1 = _marshal(rhs, np.float64, m * n, "rhs")
+        bv, s2, k2 = _marshal(bc, np.float64, m * nbc, "bc")
+        out, op, so = self._batch_out(m, dt, out, src)
+        where = _one_space([s1, s2, so])
+        it, rel, stt = (ctypes.c_int * m)(), (ctypes.c_double * m)(), (ctypes.c_int * m)()
+        st = load_library().pb_solve_batch(self._h, m, rh, bv, float(tol), int(maxiter), pc, int(check_every), op, where,
+                                           it, rel, stt)
+        del k1, k2
+        if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
+            raise PBError(st, "pb_solve_batch")
+        return dict(phi=out, iters=list(it), relres=list(rel), status=list(stt), worst=st)
+
+    def solve_batch_charges(self, charges, tol, maxiter, precision="f32", check_every=32, out=None):
+        """pb_solve_batch_charges: member s = charge set charges[s] on the atoms of a from_atoms handle."""
+        pc, dt = _prec(precision)
+        m = int(charges.shape[0])
+        q, sq, kq = _marshal(charges, np.float64, m * self.n_atoms, "charges")
+        out, op, so = self._batch_out(m, dt, out, charges)
+        where = _one_space([sq, so])
+        it, rel, stt = (ctypes.c_int * m)(), (ctypes.c_double * m)(), (ctypes.c_int * m)()
+        st = load_library().pb_solve_batch_charges(self._h, m, q, float(tol), int(maxiter), pc, int(check_every), op,
+                                                   where, it, rel, stt)
+        del kq
+        if st not in (PB_OK, PB_ERR_MAXITER, PB_ERR_BREAKDOWN):
+            raise PBError(st, "pb_solve_batch_charges")
+        return dict(phi=out, iters=list(it), relres=list(rel), status=list(stt), worst=st)
 
     def solve_refined(self, tol, maxiter, inner_tol=1e-5, check_every=32, out=None):
         """Mixed-precision iterative refinement (pb_solve_refined): fp64 potential and true residual, fp32 Jacobi-PCG

@@ -5,7 +5,7 @@
 #include "../../include/pb.h"
 #include "pb_kernels.cuh"
 #include "pb_spmv_tma.cuh"
-#include "pb_spmv_quad.cuh"
+#include "pb_spmv_batch.cuh"
 #include "pb_persist.cuh"
 #include "pb_setup.cuh"
 #include "pb_grid.cuh"
@@ -20,8 +20,28 @@ using namespace pb;
 
 namespace {
 
+// Work set of pb_solve_batch: M members' vectors side by side ([M][npad], 4-D tensor maps), the
+// coefficient arrays in the format k_spmv_batch reads (2-bit quads or words; unscaled Dinv index bytes), its plan.
+template <typename T>
+struct BatchWork {
+    int cap = 0;                                   // members the vector arrays hold
+    T *r = nullptr, *x = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr, *b = nullptr;
+    bool coef_ready = false, quad = false, pald = false, own_words = false;
+    unsigned char *exq = nullptr, *exqp = nullptr, *eyq = nullptr, *ezq = nullptr, *dviu = nullptr;
+    T *exm = nullptr, *eym = nullptr, *ezm = nullptr;   // word format (aliases of Work's arrays unless own_words)
+    int Pq = 0;
+    int M = 0;                                     // members the plan / tensor maps / graph were built for
+    int TXV = 0, TY = 0, TZ = 0, ntx = 0, nty = 0, ntz = 0, nsv = 0, nsc = 0, bps = 0, grid = 0, threads = 0;
+    size_t smem = 0;
+    int vec_grid = 0;
+    CUtensorMap tm_r, tm_p0, tm_p1, tm_x, tm_dinv, tm_exm, tm_exp, tm_ey, tm_ez;
+    cudaGraphExec_t graph = nullptr;
+    int graph_iters = 0;
+};
+
 template <typename T>
 struct Work {
+    BatchWork<T> bw;
     T *exm = nullptr, *eym = nullptr, *ezm = nullptr, *D = nullptr, *Dinv = nullptr, *b = nullptr;
     T *x = nullptr, *r = nullptr, *tmp = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr;   // tmp: pb_apply input
     int P = 0;
@@ -50,11 +70,6 @@ struct Work {
     bool pald_s = false;             // k_spmv_tma reads Dinv through the index tensor too
     T *dlut = nullptr;
     int Pb = 0;
-    // quad format (k_spmv_quad): face palettes of <= 4 values as 2-bit indices, four nodes per byte
-    bool quad = false;
-    unsigned char *exq = nullptr, *exqp = nullptr, *eyq = nullptr, *ezq = nullptr;
-    int Pq = 0;
-    CUtensorMap tm_exqp;
 };
 
 }  // namespace
@@ -134,7 +149,7 @@ void default_options(int *opt)
     opt[PB_OPT_PERSIST_BLOCKS_PER_SM] = 4; opt[PB_OPT_PALETTE] = 1; opt[PB_OPT_PALETTE_DIAG] = 1;
     opt[PB_OPT_PALETTE_DIAG_SPMV] = 1; opt[PB_OPT_AUTOTUNE] = 1; opt[PB_OPT_TILE_TXV] = 0; opt[PB_OPT_TILE_TY] = 0;
     opt[PB_OPT_TILE_TZ] = 0; opt[PB_OPT_RING_SLOTS] = 0; opt[PB_OPT_BLOCKS_PER_SM] = 0; opt[PB_OPT_VEC_BLOCKS_PER_SM] = 0;
-    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_PALETTE_QUAD] = 1;
+    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_BATCH_WIDTH] = 2;
 }
 
 inline int grid_for(size_t n, int block, int cap)
@@ -154,12 +169,26 @@ pb_status alloc_arr(T **p, size_t n)
 }
 
 template <typename T>
+void free_batch(BatchWork<T> &b)
+{
+    T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b};
+    for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
+    unsigned char **idx[] = {&b.exq, &b.exqp, &b.eyq, &b.ezq, &b.dviu};
+    for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
+    if (b.own_words) { T **wa[] = {&b.exm, &b.eym, &b.ezm}; for (T **a : wa) { if (*a) cudaFree(*a); } }
+    b.exm = b.eym = b.ezm = nullptr;
+    if (b.graph) { cudaGraphExecDestroy(b.graph); b.graph = nullptr; }
+    b.cap = 0; b.M = 0; b.coef_ready = false; b.own_words = false;
+}
+
+template <typename T>
 void free_work(Work<T> &w)
 {
+    free_batch(w.bw);
     T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.tmp, &w.p0, &w.p1, &w.Ap};
     for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
-    unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi, &w.exq, &w.exqp, &w.eyq, &w.ezq};
+    unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi};
     for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.lut) { cudaFree(w.lut); w.lut = nullptr; }
     if (w.dvi) { cudaFree(w.dvi); w.dvi = nullptr; }
@@ -246,11 +275,8 @@ pb_status build_work(pb_handle *h, Work<T> &w)
     // k_spmv_tma decodes through tables addressed by pre-scaled index bytes: n * sizeof(T) <= 256 entries-bytes
     w.pal = h->pal_n > 0 && (size_t)h->pal_n * sizeof(T) <= 256;
     w.pald = w.pal && h->pald_n > 0;
-    w.quad = w.pal && h->pal_n <= 4 && h->opt[PB_OPT_PALETTE_QUAD] != 0;
-    // k_spmv_tma: pre-scaled index bytes (n * sizeof(T) <= 256); k_spmv_quad: plain index bytes into a pair table
-    w.pald_s = w.pald && (w.quad || (size_t)h->pald_n * sizeof(T) <= 256) && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
+    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
     w.Pb = (w.P + 15) / 16 * 16;
-    w.Pq = ((w.P + 3) / 4 + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
         int coop = 0;
@@ -269,12 +295,7 @@ pb_status build_work(pb_handle *h, Work<T> &w)
         return s;
     }
     if (w.pald_s && (s = alloc_arr(&w.dvib, (size_t)h->nz * h->ny * w.Pb))) { free_work(w); return s; }
-    if (w.quad) {
-        const size_t b_ex = (size_t)h->nz * h->ny * w.Pq, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pq,
-                     b_ez = (size_t)(h->nz + 1) * h->ny * w.Pq;
-        if ((s = alloc_arr(&w.exq, b_ex)) || (s = alloc_arr(&w.exqp, b_ex)) || (s = alloc_arr(&w.eyq, b_ey)) ||
-            (s = alloc_arr(&w.ezq, b_ez)) || (s = alloc_arr(&w.lut, (size_t)kPalMax))) { free_work(w); return s; }
-    } else if (w.pal) {
+    if (w.pal) {
         const size_t b_ex = (size_t)h->nz * h->ny * w.Pb, b_ey = (size_t)h->nz * (h->ny + 1) * w.Pb,
                      b_ez = (size_t)(h->nz + 1) * h->ny * w.Pb;
         if ((s = alloc_arr(&w.exi, b_ex)) || (s = alloc_arr(&w.eyi, b_ey)) || (s = alloc_arr(&w.ezi, b_ez)) ||
@@ -315,12 +336,7 @@ pb_status build_work(pb_handle *h, Work<T> &w)
     k_setup_coeff<T><<<grid_for(total, 256, h->nsm * 16), 256, 0, h->stream>>>(
         h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
         w.exm, w.eym, w.ezm, w.D, w.Dinv, h->bad);
-    if (w.quad) {
-        k_setup_quad_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pq, 256, h->nsm * 16), 256, 0, h->stream>>>(
-            h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pq, h->pal_table, w.exq, w.exqp, w.eyq, w.ezq);
-        k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
-        h->launches += 2;
-    } else if (w.pal) {
+    if (w.pal) {
         k_setup_pal_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
             h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pal_table, w.exi, w.eyi, w.ezi);
         k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
@@ -333,8 +349,7 @@ pb_status build_work(pb_handle *h, Work<T> &w)
         h->launches += 2;
         if (w.pald_s) {
             k_setup_diag_idx<<<grid_for((size_t)h->nz * h->ny * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
-                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, w.quad ? 1 : (int)sizeof(T),
-                h->pald_table, w.dvib);
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, (int)sizeof(T), h->pald_table, w.dvib);
             h->launches += 1;
         }
     }
@@ -413,6 +428,25 @@ pb_status make_map_u8(CUtensorMap *tm, const unsigned char *ptr, int Pb, int row
 
 struct TileCfg { int TXV, TY, NS, bps, TZ; };   // TZ = 0: derive from the tile count
 
+// z split of a tile column: blocks stride over the tile list, so the launch lasts ceil(tiles / slots) tiles.  Take
+// the split whose tile count fills those waves best (a count just above a multiple of the grid wastes up to a whole
+// wave), charging each tile its two halo planes (about one plane's worth of traffic); fewest tiles on ties.
+inline int choose_tz(int nz, int xy, int slots)
+{
+    double best = -1.0;
+    int best_ntz = 1;
+    const int max_ntz = nz / 8 > 1 ? nz / 8 : 1;
+    for (int ntz = 1; ntz <= max_ntz && (long)xy * ntz <= 8L * slots + xy; ntz++) {
+        const int tz = (nz + ntz - 1) / ntz;
+        const long tiles = (long)xy * ((nz + tz - 1) / tz);
+        const long waves = (tiles + slots - 1) / slots;
+        const double fill = (double)tiles / (double)(waves * slots);
+        const double score = fill * tz / (tz + 1.0);
+        if (score > best + 1e-9) { best = score; best_ntz = ntz; }
+    }
+    return (nz + best_ntz - 1) / best_ntz;
+}
+
 // apply one tile / ring / grid configuration: sizes, persistent grid, tensor maps
 template <typename T>
 pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
@@ -425,29 +459,12 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qnty = (h->ny + TY - 1) / TY;
     w.qthreads = (spmv_row_threads(TXV) * TY + 31) / 32 * 32 + 32;
     const SlotLayout L = slot_layout(TXV, TY, w.pal ? VEC : 0, w.pald_s);
-    const QuadLayout Q = quad_layout(TXV, TY, VEC, w.pald_s);
-    w.qsmem = w.quad ? (size_t)NS * Q.slot + 2 * Q.pn + 128 : (size_t)NS * L.slot + 128;
+    w.qsmem = (size_t)NS * L.slot + 128;
     if (w.qsmem > w.qmaxdyn || w.qthreads > 512 || NS < 3 || NS > kMaxStages) return PB_ERR_INVALID_ARG;
     const int slots = h->nsm * c.bps;
     const int xy = w.qntx * w.qnty;
     int TZ = c.TZ;
-    if (TZ <= 0) {
-        // z split: blocks stride over the tile list, so the launch lasts ceil(tiles / slots) tiles.  Take the split
-        // whose tile count fills those waves best (a count just above a multiple of the grid wastes up to a whole
-        // wave), charging each tile its two halo planes (about one plane's worth of traffic); fewest tiles on ties.
-        double best = -1.0;
-        int best_ntz = 1;
-        const int max_ntz = h->nz / 8 > 1 ? h->nz / 8 : 1;
-        for (int ntz = 1; ntz <= max_ntz && (long)xy * ntz <= 8L * slots + xy; ntz++) {
-            const int tz = (h->nz + ntz - 1) / ntz;
-            const long tiles = (long)xy * ((h->nz + tz - 1) / tz);
-            const long waves = (tiles + slots - 1) / slots;
-            const double fill = (double)tiles / (double)(waves * slots);
-            const double score = fill * tz / (tz + 1.0);
-            if (score > best + 1e-9) { best = score; best_ntz = ntz; }
-        }
-        TZ = (h->nz + best_ntz - 1) / best_ntz;
-    }
+    if (TZ <= 0) TZ = choose_tz(h->nz, xy, slots);
     if (TZ > h->nz) TZ = h->nz;
     w.qTZ = TZ;
     w.qntz = (h->nz + TZ - 1) / TZ;
@@ -455,17 +472,12 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qgrid = (int)(ntiles < slots ? ntiles : slots);
     PB_TRY(make_map<T>(&w.tm_r, w.r, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_tmp, w.tmp, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
-    if (w.pald_s) PB_TRY(make_map_u8(&w.tm_dinv, w.dvib, w.Pb, h->ny, h->nz, w.quad ? Q.bwd : L.bwd, TY + 2));
+    if (w.pald_s) PB_TRY(make_map_u8(&w.tm_dinv, w.dvib, w.Pb, h->ny, h->nz, L.bwd, TY + 2));
     else PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_x, w.x, w.P, h->ny, h->nz, TXV * VEC, TY));
-    if (w.quad) {
-        PB_TRY(make_map_u8(&w.tm_ex, w.exq, w.Pq, h->ny, h->nz, Q.bwq, TY));
-        PB_TRY(make_map_u8(&w.tm_exqp, w.exqp, w.Pq, h->ny, h->nz, Q.bwq, TY));
-        PB_TRY(make_map_u8(&w.tm_ey, w.eyq, w.Pq, h->ny + 1, h->nz, Q.bwq, TY + 1));
-        PB_TRY(make_map_u8(&w.tm_ez, w.ezq, w.Pq, h->ny, h->nz + 1, Q.bwq, TY));
-    } else if (w.pal) {
+    if (w.pal) {
         PB_TRY(make_map_u8(&w.tm_ex, w.exi, w.Pb, h->ny, h->nz, L.bw, TY));
         PB_TRY(make_map_u8(&w.tm_ey, w.eyi, w.Pb, h->ny + 1, h->nz, L.bw, TY + 1));
         PB_TRY(make_map_u8(&w.tm_ez, w.ezi, w.Pb, h->ny, h->nz + 1, L.bw, TY));
@@ -480,16 +492,8 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
 template <typename T, int MODE> void launch_spmv(pb_handle *h, Work<T> &w, double out_scale);
 
 // deepest ring (<= 6 slots) that lets `bps` blocks of this tile share one SM's shared memory
-inline int ring_depth(int TXV, int TY, int bps, int pal_vec, bool pald, int quad_vec = 0)
+inline int ring_depth(int TXV, int TY, int bps, int pal_vec, bool pald)
 {
-    if (quad_vec) {
-        // k_spmv_quad: statics = barriers + the quadruple table (256 x 4 values) + the pair table; two p_new planes
-        const QuadLayout Q = quad_layout(TXV, TY, quad_vec, pald);
-        const long per_block = (long)232448 / bps - 1024 - 1200 - 256 * 4 * (16 / quad_vec) - (pald ? 512 * (16 / quad_vec) : 0)
-                               - 2 * (long)Q.pn - 128;
-        const int NS = per_block > 0 ? (int)(per_block / (long)Q.slot) : 0;
-        return NS > kMaxStages ? kMaxStages : NS;
-    }
     // 227 KB per SM, 1 KB reserved per block, statics (barriers, reduction scratch, up to three 256-entry tables)
     const size_t per_block = (size_t)232448 / bps - 1024 - 3200 - (pald ? 2 * 256 * (16 / pal_vec) : 0);
     int NS = (int)(per_block / slot_layout(TXV, TY, pal_vec, pald).slot);
@@ -517,9 +521,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         return PB_OK;
     };
     size_t lim0 = 0, lim1 = 0;
-    if (w.quad && w.pald_s) { PB_TRY(allow(k_spmv_quad<T, 0, true>, &lim0)); PB_TRY(allow(k_spmv_quad<T, 1, true>, &lim1)); }
-    else if (w.quad) { PB_TRY(allow(k_spmv_quad<T, 0, false>, &lim0)); PB_TRY(allow(k_spmv_quad<T, 1, false>, &lim1)); }
-    else if (w.pald_s) { PB_TRY(allow(k_spmv_tma<T, 0, true, true>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, true>, &lim1)); }
+    if (w.pald_s) { PB_TRY(allow(k_spmv_tma<T, 0, true, true>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, true>, &lim1)); }
     else if (w.pal) { PB_TRY(allow(k_spmv_tma<T, 0, true, false>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, true, false>, &lim1)); }
     else { PB_TRY(allow(k_spmv_tma<T, 0, false, false>, &lim0)); PB_TRY(allow(k_spmv_tma<T, 1, false, false>, &lim1)); }
     w.qmaxdyn = lim0 < lim1 ? lim0 : lim1;
@@ -542,9 +544,9 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
         if (c.TY < 1) c.TY = 1;
         if (c.TY > h->ny) c.TY = h->ny;
         while (spmv_row_threads(c.TXV) * c.TY > 448 && c.TY > 1) c.TY--;
-        c.bps = opt_or(PB_OPT_BLOCKS_PER_SM, ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s, w.quad ? VEC : 0) >= 4 ? 2 : 1);
+        c.bps = opt_or(PB_OPT_BLOCKS_PER_SM, ring_depth(c.TXV, c.TY, 2, w.pal ? VEC : 0, w.pald_s) >= 4 ? 2 : 1);
         if (c.bps < 1) c.bps = 1;
-        c.NS = opt_or(PB_OPT_RING_SLOTS, ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s, w.quad ? VEC : 0));
+        c.NS = opt_or(PB_OPT_RING_SLOTS, ring_depth(c.TXV, c.TY, c.bps, w.pal ? VEC : 0, w.pald_s));
         c.TZ = o[PB_OPT_TILE_TZ];
         cand[nc++] = c;
     } else {
@@ -557,7 +559,7 @@ pb_status setup_tma(pb_handle *h, Work<T> &w)
                 int TY = ty > h->ny ? h->ny : ty;
                 if (spmv_row_threads(TXV) * TY > 448) continue;
                 for (int bps = 1; bps <= 4; bps++) {
-                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0, w.pald_s, w.quad ? VEC : 0);
+                    const int NS = ring_depth(TXV, TY, bps, w.pal ? VEC : 0, w.pald_s);
                     if (NS < 4 && !(NS == 3 && bps >= 2)) continue;
                     const int cthreads = ((spmv_row_threads(TXV) * TY + 31) / 32 * 32) * bps;
                     if (cthreads < 256 || cthreads > 1024) continue;     // consumer threads per SM
@@ -655,21 +657,6 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->opt[PB_OPT_L2_HINTS]; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
     a.lut = w.lut; a.dlut = w.dlut;
-    if (w.quad) {
-        QuadArgs<T> q;
-        q.pbuf0 = w.p0; q.pbuf1 = w.p1; q.Ap = w.Ap; q.x = w.x;
-        q.nx = h->nx; q.ny = h->ny; q.nz = h->nz; q.P = w.P;
-        q.TXV = w.qTXV; q.TY = w.qTY; q.TZ = w.qTZ; q.ntx = w.qntx; q.nty = w.qnty; q.ntz = w.qntz;
-        q.ntiles = a.ntiles; q.nstage = w.qns; q.precond = h->precond;
-        q.st = h->st; q.partials = h->partials; q.out_scale = out_scale; q.lut = w.lut; q.dlut = w.dlut;
-        if (w.pald_s)
-            k_spmv_quad<T, MODE, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
-                MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_exqp, w.tm_ey, w.tm_ez, q);
-        else
-            k_spmv_quad<T, MODE, false><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
-                MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_exqp, w.tm_ey, w.tm_ez, q);
-        return;
-    }
     if (w.pald_s)
         k_spmv_tma<T, MODE, true, true><<<w.qgrid, w.qthreads, w.qsmem, h->stream>>>(
             MODE == 0 ? w.tm_r : w.tm_tmp, w.tm_dinv, w.tm_p0, w.tm_p1, w.tm_x, w.tm_ex, w.tm_ey, w.tm_ez, a);
@@ -947,6 +934,25 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
     return status;
 }
 
+struct DevTmp {                      // frees its device allocations on scope exit
+    void *p[12]; int n = 0;
+    ~DevTmp() { for (int i = 0; i < n; i++) if (p[i]) cudaFree(p[i]); }
+    pb_status get(void **out, size_t bytes) {
+        *out = nullptr;
+        PB_ALLOC(cudaMalloc(out, bytes ? bytes : 8));
+        p[n++] = *out;
+        return PB_OK;
+    }
+    void release(void *q) { for (int i = 0; i < n; i++) if (p[i] == q) p[i] = nullptr; }
+};
+
+pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
+                            double eps_out, double kappa, double *d_rhs, double *d_bc, double *scratch, int nsm,
+                            cudaStream_t st, bool dh_f32 = false);
+pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_memspace where);
+
+#include "pb_api_batch.cuh"
+
 template <typename T>
 pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
 {
@@ -981,7 +987,7 @@ int bytes_per_node_impl(pb_handle *h, int kernel)
     const Work<T> &w = work<T>(h);
     const int e = (int)sizeof(T);
     if (kernel == 0)      // r, p_old, x in; p, x, Ap out; Dinv; three face coefficients
-        return 6 * e + (w.pald_s ? 1 : e) + (w.quad ? 1 : w.pal ? 3 : 3 * e);   // quad: 4 arrays x 2 bits per node
+        return 6 * e + (w.pald_s ? 1 : e) + (w.pal ? 3 : 3 * e);
     return 3 * e + (w.pald ? 1 : e);      // r, Ap in; r out; Dinv
 }
 
@@ -1129,11 +1135,11 @@ pb_status pb_create(pb_handle **out, int nx, int ny, int nz, double hh,
         if (h->nsm < 1) return PB_ERR_CUDA;
         if (cuda_stream) { h->stream = (cudaStream_t)cuda_stream; h->own_stream = false; }
         else { PB_CUDA(cudaStreamCreate(&h->stream)); h->own_stream = true; }   // blocking: orders with stream 0
-        PB_ALLOC(cudaMalloc((void **)&h->st, sizeof(State)));
-        PB_CUDA(cudaMemsetAsync(h->st, 0, sizeof(State), h->stream));
+        PB_ALLOC(cudaMalloc((void **)&h->st, kMaxBatch * sizeof(State)));      // st[0]: pb_solve; st[0..M): pb_solve_batch
+        PB_CUDA(cudaMemsetAsync(h->st, 0, kMaxBatch * sizeof(State), h->stream));
         PB_ALLOC(cudaMalloc((void **)&h->bad, sizeof(int)));
         PB_ALLOC(cudaHostAlloc((void **)&h->pinned, 8 * sizeof(int), cudaHostAllocDefault));
-        PB_ALLOC(cudaHostAlloc((void **)&h->pinned_state, sizeof(State), cudaHostAllocDefault));
+        PB_ALLOC(cudaHostAlloc((void **)&h->pinned_state, 2 * kMaxBatch * sizeof(State), cudaHostAllocDefault));
         PB_CUDA(cudaEventCreateWithFlags(&h->ev[0], cudaEventDisableTiming));
         PB_CUDA(cudaEventCreateWithFlags(&h->ev[1], cudaEventDisableTiming));
         const size_t n = (size_t)nx * ny * nz;
@@ -1182,7 +1188,7 @@ pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
     if (!h || (int)opt < 0 || (int)opt >= (int)PB_OPT_COUNT_ || value < 0) return PB_ERR_INVALID_ARG;
     switch (opt) {
     case PB_OPT_PERSIST: case PB_OPT_PALETTE: case PB_OPT_PALETTE_DIAG: case PB_OPT_PALETTE_DIAG_SPMV:
-    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH: case PB_OPT_PALETTE_QUAD:
+    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH:
         if (value > 1) return PB_ERR_INVALID_ARG;
         break;
     case PB_OPT_PERSIST_BLOCKS_PER_SM:
@@ -1190,6 +1196,9 @@ pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
         break;
     case PB_OPT_RING_SLOTS:
         if (value != 0 && (value < 3 || value > kMaxStages)) return PB_ERR_INVALID_ARG;
+        break;
+    case PB_OPT_BATCH_WIDTH:
+        if (value != 1 && value != 2 && value != 4) return PB_ERR_INVALID_ARG;
         break;
     case PB_OPT_BLOCKS_PER_SM: case PB_OPT_VEC_BLOCKS_PER_SM:
         if (value > 32) return PB_ERR_INVALID_ARG;
@@ -1235,7 +1244,7 @@ pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
     out->diag_palette_size = h->pald_n > 0 ? h->pald_n : 0;
     auto fill = [&](const auto &w) {
         out->persist = w.persist; out->persist_fused = w.persist && w.pfused; out->persist_grid = w.persist ? w.pgrid : 0;
-        out->face_palette = w.pal; out->diag_palette_vec = w.pald; out->diag_palette_spmv = w.pald_s; out->face_quad = w.quad;
+        out->face_palette = w.pal; out->diag_palette_vec = w.pald; out->diag_palette_spmv = w.pald_s;
         out->txv = w.qTXV; out->ty = w.qTY; out->tz = w.qTZ; out->ring_slots = w.qns; out->blocks_per_sm = w.qbps;
         out->tiles = w.qntx * w.qnty * w.qntz; out->grid = w.qgrid; out->threads = w.qthreads;
         out->smem_bytes = (int)w.qsmem; out->autotuned = w.qtuned;
@@ -1263,6 +1272,34 @@ pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? solve_impl<float>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out)
                           : solve_impl<double>(h, tol, maxiter, check_every, phi_out, where, iters_out, relres_out);
+}
+
+pb_status pb_solve_batch(pb_handle *h, int m, const double *rhs, const double *bc, double tol, int maxiter,
+                         pb_precision prec, int check_every, void *phi_out, pb_memspace where, int *iters_out,
+                         double *relres_out, int *status_out)
+{
+    if (!h || m < 1 || !phi_out || !(tol > 0.0) || !std::isfinite(tol) || maxiter < 0 || check_every < 1 ||
+        !valid_prec(prec) || !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? solve_batch_impl<float>(h, m, rhs, bc, nullptr, where, tol, maxiter, check_every, phi_out,
+                                                    iters_out, relres_out, status_out)
+                          : solve_batch_impl<double>(h, m, rhs, bc, nullptr, where, tol, maxiter, check_every, phi_out,
+                                                     iters_out, relres_out, status_out);
+}
+
+pb_status pb_solve_batch_charges(pb_handle *h, int m, const double *charges, double tol, int maxiter,
+                                 pb_precision prec, int check_every, void *phi_out, pb_memspace where, int *iters_out,
+                                 double *relres_out, int *status_out)
+{
+    if (!h || m < 1 || !h->atoms_c || (h->n_atoms && !charges) || !phi_out || !(tol > 0.0) || !std::isfinite(tol) ||
+        maxiter < 0 || check_every < 1 || !valid_prec(prec) || !valid_space(where))
+        return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? solve_batch_impl<float>(h, m, nullptr, nullptr, charges, where, tol, maxiter, check_every,
+                                                    phi_out, iters_out, relres_out, status_out)
+                          : solve_batch_impl<double>(h, m, nullptr, nullptr, charges, where, tol, maxiter, check_every,
+                                                     phi_out, iters_out, relres_out, status_out);
 }
 
 pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
@@ -1302,6 +1339,8 @@ pb_status pb_set_preconditioner(pb_handle *h, int kind)
         // captured graphs hold the kernel arguments by value
         if (h->wf.graph) { cudaGraphExecDestroy(h->wf.graph); h->wf.graph = nullptr; }
         if (h->wd.graph) { cudaGraphExecDestroy(h->wd.graph); h->wd.graph = nullptr; }
+        if (h->wf.bw.graph) { cudaGraphExecDestroy(h->wf.bw.graph); h->wf.bw.graph = nullptr; }
+        if (h->wd.bw.graph) { cudaGraphExecDestroy(h->wd.bw.graph); h->wd.bw.graph = nullptr; }
     }
     return PB_OK;
 }
@@ -1314,6 +1353,8 @@ pb_status pb_set_boundary(pb_handle *h, int kind)
         h->periodic = kind;
         if (h->wf.graph) { cudaGraphExecDestroy(h->wf.graph); h->wf.graph = nullptr; }
         if (h->wd.graph) { cudaGraphExecDestroy(h->wd.graph); h->wd.graph = nullptr; }
+        if (h->wf.bw.graph) { cudaGraphExecDestroy(h->wf.bw.graph); h->wf.bw.graph = nullptr; }
+        if (h->wd.bw.graph) { cudaGraphExecDestroy(h->wd.bw.graph); h->wd.bw.graph = nullptr; }
         h->wf.b_ready = false;           // b loses / regains the ghost fold-in
         h->wd.b_ready = false;
         if (h->wf.ready) PB_TRY(build_b<float>(h, h->wf));
@@ -1428,23 +1469,12 @@ int pb_version(void) { return 100; }
 
 // ---- NEXT row f1: grid / stencil setup on the GPU ---------------------------------------------------------
 namespace {
-struct DevTmp {                      // frees its device allocations on scope exit
-    void *p[12]; int n = 0;
-    ~DevTmp() { for (int i = 0; i < n; i++) if (p[i]) cudaFree(p[i]); }
-    pb_status get(void **out, size_t bytes) {
-        *out = nullptr;
-        PB_ALLOC(cudaMalloc(out, bytes ? bytes : 8));
-        p[n++] = *out;
-        return PB_OK;
-    }
-    void release(void *q) { for (int i = 0; i < n; i++) if (p[i] == q) p[i] = nullptr; }
-};
 
 // rhs (dense [nz][ny][nx]) and bc from charges on the stored / given atom geometry.  `scratch` = one double
 // (sum |q|) followed by one int (the bad-atom flag), device.
 pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
                             double eps_out, double kappa, double *d_rhs, double *d_bc, double *scratch, int nsm,
-                            cudaStream_t st, bool dh_f32 = false)
+                            cudaStream_t st, bool dh_f32)
 {
     const size_t n = (size_t)nx * ny * nz;
     const size_t nbc = 2 * ((size_t)nz * ny + (size_t)nz * nx + (size_t)ny * nx);

@@ -1,0 +1,360 @@
+// pb_api_batch.cuh -- host logic of pb_solve_batch / pb_solve_batch_charges (NEXT row f2 of SURVEY.md 8(f): M
+// right-hand sides per pass through k_spmv_batch + k_vec_batch).  Included by pb_api.cu inside its anonymous
+// namespace, after the single-solve helpers it builds on (ensure, make_map, vec_args, k_init, k_finish ...).
+#pragma once
+
+// 4-D tensor [M][planes][rows][P] of T (member = coordinate 3), box = bx elements x by rows x 1 plane x 1 member
+template <typename T>
+pb_status make_map4(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, int members, int bx, int by)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return PB_ERR_CUDA;
+    const cuuint64_t dims[4] = {(cuuint64_t)P, (cuuint64_t)rows, (cuuint64_t)planes, (cuuint64_t)members};
+    const cuuint64_t strides[3] = {(cuuint64_t)P * sizeof(T), (cuuint64_t)P * rows * sizeof(T),
+                                   (cuuint64_t)P * rows * planes * sizeof(T)};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = fn(tm, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4,
+                          (void *)ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? PB_OK : PB_ERR_CUDA;
+}
+
+template <typename T, bool QUAD, bool PALD, int M>
+pb_status batch_kernel_attr(size_t *max_dyn)
+{
+    cudaFuncAttributes fa;
+    PB_CUDA(cudaFuncGetAttributes(&fa, k_spmv_batch<T, QUAD, PALD, M>));
+    const size_t lim = (size_t)232448 - fa.sharedSizeBytes;
+    PB_CUDA(cudaFuncSetAttribute(k_spmv_batch<T, QUAD, PALD, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim));
+    *max_dyn = lim;
+    return PB_OK;
+}
+template <typename T, int M>
+pb_status batch_kernel_attr_fmt(bool quad, bool pald, size_t *max_dyn)
+{
+    if (quad) return pald ? batch_kernel_attr<T, true, true, M>(max_dyn) : batch_kernel_attr<T, true, false, M>(max_dyn);
+    return pald ? batch_kernel_attr<T, false, true, M>(max_dyn) : batch_kernel_attr<T, false, false, M>(max_dyn);
+}
+
+// coefficient arrays, vectors, plan and tensor maps of the batch path for M members
+template <typename T>
+pb_status ensure_batch(pb_handle *h, int M)
+{
+    constexpr int VEC = VecN<T>::value;
+    PB_TRY(ensure<T>(h));
+    Work<T> &w = work<T>(h);
+    BatchWork<T> &b = w.bw;
+    pb_status s = PB_OK;
+    const size_t rows = (size_t)h->nz * h->ny;
+    if (!b.coef_ready) {
+        b.quad = h->pal_n > 0 && h->pal_n <= 4 && h->opt[PB_OPT_PALETTE] != 0;
+        b.pald = w.pald && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
+        b.Pq = ((w.P + 3) / 4 + 15) / 16 * 16;
+        if (b.quad) {
+            const size_t b_ex = rows * b.Pq, b_ey = (size_t)h->nz * (h->ny + 1) * b.Pq, b_ez = (size_t)(h->nz + 1) * h->ny * b.Pq;
+            if ((s = alloc_arr(&b.exq, b_ex)) || (s = alloc_arr(&b.exqp, b_ex)) || (s = alloc_arr(&b.eyq, b_ey)) ||
+                (s = alloc_arr(&b.ezq, b_ez))) { free_batch(b); return s; }
+            if (!w.lut) {
+                if ((s = alloc_arr(&w.lut, (size_t)kPalMax))) { free_batch(b); return s; }
+                k_pal_lut<T><<<1, 256, 0, h->stream>>>(h->pal_table, w.lut);
+            }
+            k_setup_quad_idx<<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * b.Pq, 256, h->nsm * 16), 256, 0, h->stream>>>(
+                h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz, b.Pq, h->pal_table, b.exq, b.exqp, b.eyq, b.ezq);
+            h->launches += 1;
+        } else if (w.exm) {
+            b.exm = w.exm; b.eym = w.eym; b.ezm = w.ezm;
+        } else {
+            // a byte-palette operator (5..64 face values): the batch kernel reads full words, built here once
+            const size_t n_ey = (size_t)h->nz * (h->ny + 1) * w.P, n_ez = (size_t)(h->nz + 1) * h->ny * w.P;
+            b.own_words = true;
+            if ((s = alloc_arr(&b.exm, w.npad)) || (s = alloc_arr(&b.eym, n_ey)) || (s = alloc_arr(&b.ezm, n_ez))) {
+                free_batch(b);
+                return s;
+            }
+            k_setup_coeff<T><<<grid_for((size_t)(h->nz + 1) * (h->ny + 1) * w.P, 256, h->nsm * 16), 256, 0, h->stream>>>(
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.P,
+                b.exm, b.eym, b.ezm, w.D, w.Dinv, h->bad);
+            h->launches += 1;
+        }
+        if (b.pald) {
+            if ((s = alloc_arr(&b.dviu, rows * w.Pb))) { free_batch(b); return s; }
+            k_setup_diag_idx<<<grid_for(rows * w.Pb, 256, h->nsm * 16), 256, 0, h->stream>>>(
+                h->eps_x, h->eps_y, h->eps_z, h->kbar2, h->h * h->h, h->nx, h->ny, h->nz, w.Pb, 1, h->pald_table, b.dviu);
+            h->launches += 1;
+        }
+        PB_CUDA(cudaGetLastError());
+        b.coef_ready = true;
+    }
+    if (b.cap < M) {
+        T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b};
+        for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
+        b.cap = 0; b.M = 0;
+        for (T **a : arrs)
+            if ((s = alloc_arr(a, (size_t)M * w.npad))) { free_batch(b); return s; }
+        b.cap = M;
+    }
+    if (b.M == M) return PB_OK;
+    if (b.graph) { cudaGraphExecDestroy(b.graph); b.graph = nullptr; }
+    // plan: rows of about 1 KB like k_spmv_tma, four rows, two blocks per SM (one for M = 4: its registers), rings as
+    // deep as the shared memory allows
+    size_t max_dyn = 0;
+    if (M == 1) PB_TRY((batch_kernel_attr_fmt<T, 1>(b.quad, b.pald, &max_dyn)));
+    else if (M == 2) PB_TRY((batch_kernel_attr_fmt<T, 2>(b.quad, b.pald, &max_dyn)));
+    else PB_TRY((batch_kernel_attr_fmt<T, 4>(b.quad, b.pald, &max_dyn)));
+    const int rowvecs = w.P / VEC;
+    const int maxv = ((b.pald || b.quad) ? 240 : 256) / VEC - 2;
+    int ntx0 = (rowvecs + 32) / 64;
+    if (ntx0 < 1) ntx0 = 1;
+    while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
+    const int *o = h->opt;
+    b.TXV = o[PB_OPT_TILE_TXV] > 0 ? o[PB_OPT_TILE_TXV] : (rowvecs + ntx0 - 1) / ntx0;
+    if (b.TXV > maxv) b.TXV = maxv;
+    if (b.TXV > rowvecs) b.TXV = rowvecs;
+    b.TY = o[PB_OPT_TILE_TY] > 0 ? o[PB_OPT_TILE_TY] : 4;
+    if (b.TY > h->ny) b.TY = h->ny;
+    const int max_ct = (M >= 4 ? 256 : 512) - 64;
+    while (spmv_row_threads(b.TXV) * b.TY > max_ct && b.TY > 1) b.TY--;
+    b.threads = (spmv_row_threads(b.TXV) * b.TY + 31) / 32 * 32 + 32;
+    const BatchLayout L = batch_layout(b.TXV, b.TY, VEC, b.quad, b.pald);
+    // blocks per SM / coefficient ring depth: the first combination that leaves the vector ring M + 2 slots (the
+    // consumers work on one member's plane while M more are in flight), else the one with the deepest vector ring
+    const int forced_bps = o[PB_OPT_BLOCKS_PER_SM];
+    const int try_bps[3] = {M >= 4 ? 1 : 2, 1, 1}, try_nsc[3] = {4, 4, 3};
+    b.nsv = 0;
+    for (int t = 0; t < 3; t++) {
+        const int bps = forced_bps > 0 ? forced_bps : try_bps[t], nsc = try_nsc[t];
+        const long fixed = (long)nsc * (long)L.cslot + 2L * M * (long)L.pn + 128;
+        long budget = (long)((size_t)232448 / bps) - 1024 - (long)((size_t)232448 - max_dyn) - fixed;   // per-SM share
+        if ((long)max_dyn - fixed < budget) budget = (long)max_dyn - fixed;                              // per-block cap
+        int nsv = budget > 0 ? (int)(budget / (long)L.vslot) : 0;
+        if (nsv > kMaxStages) nsv = kMaxStages;
+        if (nsv > b.nsv) { b.nsv = nsv; b.nsc = nsc; b.bps = bps; }
+        if (b.nsv >= M + 2) break;
+    }
+    if (o[PB_OPT_RING_SLOTS] > 0 && o[PB_OPT_RING_SLOTS] < b.nsv) b.nsv = o[PB_OPT_RING_SLOTS];
+    if (b.nsv < 2) return PB_ERR_INVALID_ARG;
+    b.smem = batch_smem(L, b.nsv, b.nsc, M);
+    b.ntx = (rowvecs + b.TXV - 1) / b.TXV;
+    b.nty = (h->ny + b.TY - 1) / b.TY;
+    const int slots = h->nsm * b.bps, xy = b.ntx * b.nty;
+    b.TZ = o[PB_OPT_TILE_TZ] > 0 ? o[PB_OPT_TILE_TZ] : choose_tz(h->nz, xy, slots);
+    if (b.TZ > h->nz) b.TZ = h->nz;
+    b.ntz = (h->nz + b.TZ - 1) / b.TZ;
+    const long ntiles = (long)xy * b.ntz;
+    b.grid = (int)(ntiles < slots ? ntiles : slots);
+    b.vec_grid = grid_for(w.npad / VEC, 256, h->nsm * 8);
+    size_t need = (size_t)M * b.grid > (size_t)2 * M * b.vec_grid ? (size_t)M * b.grid : (size_t)2 * M * b.vec_grid;
+    if (need > h->partials_cap) {
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        if (h->partials) cudaFree(h->partials);
+        h->partials = nullptr;
+        h->partials_cap = 0;
+        PB_ALLOC(cudaMalloc((void **)&h->partials, need * sizeof(double)));
+        h->partials_cap = need;
+        // graphs captured earlier hold the old pointer
+        if (h->wf.graph) { cudaGraphExecDestroy(h->wf.graph); h->wf.graph = nullptr; }
+        if (h->wd.graph) { cudaGraphExecDestroy(h->wd.graph); h->wd.graph = nullptr; }
+        if (h->wf.bw.graph) { cudaGraphExecDestroy(h->wf.bw.graph); h->wf.bw.graph = nullptr; }
+        if (h->wd.bw.graph) { cudaGraphExecDestroy(h->wd.bw.graph); h->wd.bw.graph = nullptr; }
+    }
+    const int hx = (b.TXV + 2) * VEC, hy = b.TY + 2;
+    PB_TRY(make_map4<T>(&b.tm_r, b.r, w.P, h->ny, h->nz, M, hx, hy));
+    PB_TRY(make_map4<T>(&b.tm_p0, b.p0, w.P, h->ny, h->nz, M, hx, hy));
+    PB_TRY(make_map4<T>(&b.tm_p1, b.p1, w.P, h->ny, h->nz, M, hx, hy));
+    PB_TRY(make_map4<T>(&b.tm_x, b.x, w.P, h->ny, h->nz, M, b.TXV * VEC, b.TY));
+    if (b.pald) PB_TRY(make_map_u8(&b.tm_dinv, b.dviu, w.Pb, h->ny, h->nz, L.bwd, hy));
+    else PB_TRY(make_map<T>(&b.tm_dinv, w.Dinv, w.P, h->ny, h->nz, hx, hy));
+    if (b.quad) {
+        PB_TRY(make_map_u8(&b.tm_exm, b.exq, b.Pq, h->ny, h->nz, L.bwq, b.TY));
+        PB_TRY(make_map_u8(&b.tm_exp, b.exqp, b.Pq, h->ny, h->nz, L.bwq, b.TY));
+        PB_TRY(make_map_u8(&b.tm_ey, b.eyq, b.Pq, h->ny + 1, h->nz, L.bwq, b.TY + 1));
+        PB_TRY(make_map_u8(&b.tm_ez, b.ezq, b.Pq, h->ny, h->nz + 1, L.bwq, b.TY));
+    } else {
+        PB_TRY(make_map<T>(&b.tm_exm, b.exm, w.P, h->ny, h->nz, (b.TXV + 1) * VEC, b.TY));
+        b.tm_exp = b.tm_exm;
+        PB_TRY(make_map<T>(&b.tm_ey, b.eym, w.P, h->ny + 1, h->nz, b.TXV * VEC, b.TY + 1));
+        PB_TRY(make_map<T>(&b.tm_ez, b.ezm, w.P, h->ny, h->nz + 1, b.TXV * VEC, b.TY));
+    }
+    b.M = M;
+    if (verbose())
+        fprintf(stderr, "pb: batch plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%ld grid=%d threads=%d smem=%zu\n",
+                sizeof(T) == 4 ? "f32" : "f64", M, b.quad ? "quad" : "words", b.pald ? "+diag palette" : "", b.TXV, b.TY, b.TZ,
+                b.nsv, b.nsc, b.bps, ntiles, b.grid, b.threads, b.smem);
+    return PB_OK;
+}
+
+template <typename T, bool QUAD, bool PALD, int M>
+void launch_batch_kernels(pb_handle *h, Work<T> &w, int n_iter)
+{
+    BatchWork<T> &b = w.bw;
+    BatchArgs<T> a;
+    a.pbuf0 = b.p0; a.pbuf1 = b.p1; a.Ap = b.Ap; a.x = b.x; a.npad = w.npad;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
+    a.TXV = b.TXV; a.TY = b.TY; a.TZ = b.TZ; a.ntx = b.ntx; a.nty = b.nty; a.ntz = b.ntz;
+    a.ntiles = b.ntx * b.nty * b.ntz; a.nsv = b.nsv; a.nsc = b.nsc; a.precond = h->precond;
+    a.st = h->st; a.partials = h->partials; a.lut = w.lut; a.dlut = w.dlut;
+    VecArgs<T> v = vec_args<T>(h, w);
+    v.r = b.r; v.Ap = b.Ap;
+    for (int it = 0; it < n_iter; it++) {
+        k_spmv_batch<T, QUAD, PALD, M><<<b.grid, b.threads, b.smem, h->stream>>>(
+            b.tm_r, b.tm_dinv, b.tm_p0, b.tm_p1, b.tm_x, b.tm_exm, b.tm_exp, b.tm_ey, b.tm_ez, a);
+        if (w.pald) k_vec_batch<T, true, M><<<b.vec_grid, 256, 0, h->stream>>>(v, w.npad);
+        else k_vec_batch<T, false, M><<<b.vec_grid, 256, 0, h->stream>>>(v, w.npad);
+    }
+}
+
+template <typename T>
+pb_status enqueue_batch_iterations(pb_handle *h, Work<T> &w, int n_iter)
+{
+    const BatchWork<T> &b = w.bw;
+#define PB_BATCH_CASE(Q, D, MM) launch_batch_kernels<T, Q, D, MM>(h, w, n_iter)
+#define PB_BATCH_M(Q, D) do { if (b.M == 1) PB_BATCH_CASE(Q, D, 1); else if (b.M == 2) PB_BATCH_CASE(Q, D, 2); else PB_BATCH_CASE(Q, D, 4); } while (0)
+    if (b.quad) { if (b.pald) PB_BATCH_M(true, true); else PB_BATCH_M(true, false); }
+    else { if (b.pald) PB_BATCH_M(false, true); else PB_BATCH_M(false, false); }
+#undef PB_BATCH_M
+#undef PB_BATCH_CASE
+    PB_CUDA(cudaGetLastError());
+    h->launches += 2LL * n_iter;
+    return PB_OK;
+}
+
+// M members: steps 1-8 until every member's latch is set; member s's right-hand side b is in w.bw.b + s*npad
+template <typename T>
+pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_every)
+{
+    Work<T> &w = work<T>(h);
+    BatchWork<T> &b = w.bw;
+    h->last_prec = sizeof(T) == 4 ? PB_F32 : PB_F64;
+    for (int s = 0; s < M; s++) {
+        k_set_state<<<1, 1, 0, h->stream>>>(h->st + s, tol * tol, maxiter, 1);
+        VecArgs<T> va = vec_args<T>(h, w);
+        va.r = b.r + s * w.npad; va.b = b.b + s * w.npad; va.x = b.x + s * w.npad; va.pzero = b.p0 + s * w.npad;
+        va.st = h->st + s;
+        k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
+    }
+    PB_CUDA(cudaGetLastError());
+    h->launches += 2LL * M;
+    const int m = check_every;
+    bool graph_ok = false;
+    if (h->opt[PB_OPT_GRAPH]) {
+        if (!(b.graph && b.graph_iters == m)) {
+            if (b.graph) { cudaGraphExecDestroy(b.graph); b.graph = nullptr; }
+            cudaGraph_t g = nullptr;
+            PB_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+            const pb_status cs = enqueue_batch_iterations<T>(h, w, m);
+            h->launches -= 2LL * m;
+            const cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+            if (cs == PB_OK && e == cudaSuccess && g && cudaGraphInstantiate(&b.graph, g, 0) == cudaSuccess) b.graph_iters = m;
+            else { b.graph = nullptr; cudaGetLastError(); }
+            if (g) cudaGraphDestroy(g);
+        }
+        graph_ok = b.graph != nullptr;
+    }
+    const long max_chunks = (long)maxiter / m + 2;
+    bool all_done = false;
+    for (long c = 0; c < max_chunks + 1 && !all_done; c++) {
+        if (graph_ok) { PB_CUDA(cudaGraphLaunch(b.graph, h->stream)); h->launches += 2LL * m; }
+        else PB_TRY(enqueue_batch_iterations<T>(h, w, m));
+        State *slot = h->pinned_state + kMaxBatch * (c & 1);
+        PB_CUDA(cudaMemcpyAsync(slot, h->st, M * sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaEventRecord(h->ev[c & 1], h->stream));
+        if (c >= 1) {
+            PB_CUDA(cudaEventSynchronize(h->ev[(c - 1) & 1]));
+            const State *prev = h->pinned_state + kMaxBatch * ((c - 1) & 1);
+            all_done = true;
+            for (int s = 0; s < M; s++) all_done = all_done && prev[s].done;
+        }
+    }
+    return PB_OK;
+}
+
+// fold member s's right-hand side (dense rhs / bc on the device) into w.bw.b + s*npad
+template <typename T>
+pb_status batch_fold(pb_handle *h, Work<T> &w, int s, const double *d_rhs, const double *d_bc)
+{
+    const double h2 = h->h * h->h;
+    k_setup_b<T><<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(
+        h->eps_x, h->eps_y, h->eps_z, d_rhs, h->periodic ? nullptr : d_bc, h2, h->nx, h->ny, h->nz, w.P, w.bw.b + s * w.npad);
+    PB_CUDA(cudaGetLastError());
+    h->launches += 1;
+    return PB_OK;
+}
+
+// pb_solve_batch / pb_solve_batch_charges: members in groups of the batch width; each group = fold the members'
+// right-hand sides, run_batch, un-pad the potentials
+template <typename T>
+pb_status solve_batch_impl(pb_handle *h, int m, const double *rhs, const double *bc, const double *charges,
+                           pb_memspace where, double tol, int maxiter, int check_every, void *phi_out,
+                           int *iters_out, double *relres_out, int *status_out)
+{
+    PB_TRY(ensure<T>(h));
+    Work<T> &w = work<T>(h);
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    const size_t nbc = 2 * ((size_t)h->nz * h->ny + (size_t)h->nz * h->nx + (size_t)h->ny * h->nx);
+    const int width = h->opt[PB_OPT_BATCH_WIDTH];
+    if (h->periodic) return PB_ERR_INVALID_ARG;         // the batch kernels implement the free-space (ghost-layer) condition
+    if (where == PB_HOST) PB_TRY(ensure_stage(h, n * sizeof(T)));
+    DevTmp tmp;
+    double *d_q = nullptr, *scratch = nullptr;
+    if (charges) {
+        PB_TRY(tmp.get((void **)&d_q, (size_t)(h->n_atoms ? h->n_atoms : 1) * sizeof(double)));
+        PB_TRY(tmp.get((void **)&scratch, 2 * sizeof(double)));
+    }
+    pb_status worst = PB_OK;
+    for (int g0 = 0; g0 < m;) {
+        int M = width;
+        while (M > m - g0) M >>= 1;
+        PB_TRY(ensure_batch<T>(h, M));
+        for (int s = 0; s < M; s++) {
+            const int mem = g0 + s;
+            if (charges) {
+                PB_CUDA(cudaMemcpyAsync(d_q, charges + (size_t)mem * h->n_atoms, (size_t)h->n_atoms * sizeof(double),
+                                        where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
+                if (!h->rhs) PB_ALLOC(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
+                if (!h->bc) PB_ALLOC(cudaMalloc((void **)&h->bc, (nbc + 8) * sizeof(double)));
+                PB_TRY(charges_to_rhs_bc(h->atoms_c, d_q, h->n_atoms, h->nx, h->ny, h->nz, h->h, h->atoms_eps_out,
+                                         h->atoms_kappa, h->rhs, h->bc, scratch, h->nsm, h->stream, h->dh_f32));
+                h->launches += 4;
+                PB_TRY(batch_fold<T>(h, w, s, h->rhs, h->bc));
+                h->wf.b_ready = false; h->wd.b_ready = false;      // the handle's own rhs now is the last member's
+            } else if (where == PB_DEVICE) {
+                PB_TRY(batch_fold<T>(h, w, s, rhs ? rhs + (size_t)mem * n : nullptr, bc ? bc + (size_t)mem * nbc : nullptr));
+            } else {
+                PB_TRY(take_copy(h, &h->rhs, rhs ? rhs + (size_t)mem * n : nullptr, n, PB_HOST));
+                PB_TRY(take_copy(h, &h->bc, bc ? bc + (size_t)mem * nbc : nullptr, nbc, PB_HOST));
+                PB_TRY(batch_fold<T>(h, w, s, h->rhs, h->bc));
+                PB_CUDA(cudaStreamSynchronize(h->stream));          // h->rhs / h->bc are reused by the next member
+                h->wf.b_ready = false; h->wd.b_ready = false;
+            }
+        }
+        PB_TRY(run_batch<T>(h, M, tol, maxiter, check_every));
+        for (int s = 0; s < M; s++) {
+            const int mem = g0 + s;
+            T *dst = (T *)phi_out + (size_t)mem * n;
+            T *dev_dst = where == PB_HOST ? (T *)h->stage : dst;
+            k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
+                w.bw.x + s * w.npad, w.bw.p0 + s * w.npad, w.bw.p1 + s * w.npad, h->st + s, dev_dst, h->nx, w.P, rows);
+            PB_CUDA(cudaGetLastError());
+            h->launches += 1;
+            if (where == PB_HOST) {
+                PB_CUDA(cudaMemcpyAsync(dst, dev_dst, n * sizeof(T), cudaMemcpyDeviceToHost, h->stream));
+                PB_CUDA(cudaStreamSynchronize(h->stream));          // the staging buffer is reused by the next member
+            }
+        }
+        PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, M * sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+        PB_CUDA(cudaStreamSynchronize(h->stream));
+        for (int s = 0; s < M; s++) {
+            const State &st = h->pinned_state[s];
+            if (!st.done) return PB_ERR_CUDA;
+            if (iters_out) iters_out[g0 + s] = st.iters;
+            if (relres_out) relres_out[g0 + s] = (st.bb > 0.0) ? sqrt(st.rr / st.bb) : 0.0;
+            if (status_out) status_out[g0 + s] = st.status;
+            if (st.status == (int)PB_ERR_BREAKDOWN) worst = PB_ERR_BREAKDOWN;
+            else if (st.status == (int)PB_ERR_MAXITER && worst == PB_OK) worst = PB_ERR_MAXITER;
+        }
+        g0 += M;
+    }
+    return worst;
+}

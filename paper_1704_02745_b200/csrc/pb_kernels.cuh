@@ -154,6 +154,85 @@ __global__ void __launch_bounds__(256) k_vec(const VecArgs<T> a)
     reduce_and_finish(a.st, a.partials, s_rz, s_rr, red, &s_last, 0);
 }
 
+// k_vec for M right-hand sides on one operator: member s lives at r + s*stride, Ap + s*stride,
+// its scalars in st[s], its partials at partials + s*2*gridDim.x.  Dinv (word or palette byte) is read once per node
+// for all members; a member whose latch is set is skipped.  Per member the arithmetic and the order of the
+// reduction are those of k_vec run with one vector per thread and pass.
+template <typename T, bool PALD, int M>
+__global__ void __launch_bounds__(256) k_vec_batch(const VecArgs<T> a, size_t stride)
+{
+    constexpr int VEC = VecN<T>::value;
+    __shared__ double red[32];
+    __shared__ int s_last;
+    __shared__ T dlut[PALD ? 256 : 1];
+    bool live[M];
+    T alpha[M];
+    bool any = false;
+#pragma unroll
+    for (int s = 0; s < M; s++) { live[s] = !a.st[s].done; any |= live[s]; alpha[s] = (T)a.st[s].alpha; }
+    if (!any) return;
+    if (PALD) {
+        for (int i = threadIdx.x; i < 256; i += blockDim.x) dlut[i] = a.dlut[i];
+        __syncthreads();
+    }
+    double s_rz[M], s_rr[M];
+#pragma unroll
+    for (int s = 0; s < M; s++) { s_rz[s] = 0.0; s_rr[s] = 0.0; }
+    const size_t step = (size_t)gridDim.x * blockDim.x;
+    for (size_t v0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v0 < a.nvec; v0 += step) {
+        const size_t idx = (a.nvec - 1 - v0) * VEC;
+        Vec<T> r[M], q[M], d;
+#pragma unroll
+        for (int s = 0; s < M; s++)
+            if (live[s]) { r[s] = ldv(a.r + s * stride + idx); q[s] = ldv(a.Ap + s * stride + idx); }
+        if (PALD) {
+            const uint32_t w = (VEC == 4) ? *reinterpret_cast<const uint32_t *>(a.dvi + idx)
+                                          : (uint32_t)*reinterpret_cast<const unsigned short *>(a.dvi + idx);
+#pragma unroll
+            for (int e = 0; e < VEC; e++) d.a[e] = dlut[(w >> (8 * e)) & 255u];
+        } else {
+            d = ldv(a.Dinv + idx);
+        }
+#pragma unroll
+        for (int s = 0; s < M; s++) {
+            if (!live[s]) continue;
+#pragma unroll
+            for (int e = 0; e < VEC; e++) {
+                r[s].a[e] = fma(-alpha[s], q[s].a[e], r[s].a[e]);              // r_l = r_{l-1} - alpha A p   (step 5)
+                const T zv = a.precond ? d.a[e] * r[s].a[e] : r[s].a[e];       // M z_l = r_l                (step 6)
+                s_rz[s] = fma((double)r[s].a[e], (double)zv, s_rz[s]);
+                s_rr[s] = fma((double)r[s].a[e], (double)r[s].a[e], s_rr[s]);
+            }
+            stv(a.r + s * stride + idx, r[s]);
+        }
+    }
+    const int nblk = gridDim.x;
+    double t_rz[M], t_rr[M];
+#pragma unroll
+    for (int s = 0; s < M; s++) { t_rz[s] = block_sum(s_rz[s], red); t_rr[s] = block_sum(s_rr[s], red); }
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < M; s++) {
+            a.partials[(size_t)s * 2 * nblk + blockIdx.x] = t_rz[s];
+            a.partials[(size_t)s * 2 * nblk + nblk + blockIdx.x] = t_rr[s];
+        }
+        __threadfence();
+        const unsigned int t = atomicAdd(&a.st->ticket_vec, 1u);
+        s_last = (t == (unsigned int)(nblk - 1));
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+#pragma unroll
+        for (int s = 0; s < M; s++) {
+            const double rz = final_sum(a.partials + (size_t)s * 2 * nblk, nblk, red);
+            const double rr = final_sum(a.partials + (size_t)s * 2 * nblk + nblk, nblk, red);
+            if (threadIdx.x == 0 && live[s]) finish_iteration(a.st + s, rz, rr, 0);
+        }
+        if (threadIdx.x == 0) a.st->ticket_vec = 0u;
+    }
+}
+
 // steps 1-2 with phi_0 = 0: x = 0, r = b, p buffer cleared, r.z and r.r
 template <typename T>
 __global__ void __launch_bounds__(256) k_init(const VecArgs<T> a)

@@ -45,6 +45,19 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, in
         ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
 }
 
+// 4-D variant: coordinate c3 selects the right-hand side of a batched vector tensor [M][planes][rows][P]; the zero
+// fill outside [0, planes) in c2 is per dimension, so the ghost planes of one member never read its neighbour
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3, uint64_t *bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+// make the value (hence the shared-memory loads it was computed from) complete before any later asm volatile --
+// used before handing a ring slot back, so that no load of the slot is still in flight when the producer is told
+__device__ __forceinline__ void consume(float v) { asm volatile("" ::"f"(v) : "memory"); }
+__device__ __forceinline__ void consume(double v) { asm volatile("" ::"d"(v) : "memory"); }
+
 // same with an L2 eviction-priority policy (createpolicy) attached to the lines the box touches
 __device__ __forceinline__ void tma_load_3d_hint(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar,
                                                  uint64_t policy) {

@@ -297,18 +297,13 @@ def test_tiling_independence_with_both_palettes(pkg, prec):
     dt = np.float64 if prec == "f64" else np.float32
     x = np.random.default_rng(5).uniform(-1, 1, (inp.nz, inp.ny, inp.nx)).astype(dt)
     ref_y = ref_p = ref_ap = None
-    # storage formats: quad (2-bit faces, k_spmv_quad) with Dinv index bytes / with Dinv words; byte palette
-    # (k_spmv_tma) with / without the diagonal palette; full words
-    for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette_quad=0), dict(palette_quad=0, palette_diag_spmv=0),
-                dict(palette=0)):
+    for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette=0)):
         for cfg in TILE_CONFIGS:
             with pkg.PBSolver(*inp.args(), options={**cfg, **fmt, "persist": 0}) as s:
                 y = s.apply(x, prec)
                 if not fmt:
-                    assert s.palette_size() > 0 and s.diag_palette_size() > 0 and s.plan(prec)["face_quad"] == 1
-                    assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 2
-                if fmt == dict(palette_quad=0):
-                    assert s.plan(prec)["face_quad"] == 0 and s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
+                    assert s.palette_size() > 0 and s.diag_palette_size() > 0
+                    assert s.bytes_per_node(prec, 0) == 6 * x.itemsize + 4
                 s.solve_begin(prec)
                 s.iterate(prec, 2)
                 p2, ap2 = s.vector("p"), s.vector("Ap")
@@ -538,16 +533,13 @@ def test_randomised_shapes_and_options(pkg, pbref):
     rng = np.random.default_rng(20260704)
     for case in range(24):
         nx, ny, nz = (int(v) for v in rng.integers(1, 41, 3))
-        periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), int(rng.integers(3))
+        periodic, jacobi, two_valued = bool(rng.integers(2)), bool(rng.integers(2)), bool(rng.integers(2))
         persist, prec = int(rng.integers(2)), ("f64", "f32")[int(rng.integers(2))]
         inp = _periodic_inputs((nx, ny, nz), 100 + case) if periodic else random_operator(nx, ny, nz, seed=100 + case)
-        if two_valued == 0:          # a continuum of face values: word format
+        if not two_valued:
             inp.eps_x[...] = rng.uniform(1, 80, inp.eps_x.shape)
-        elif two_valued == 2:        # seven face values: byte palette (k_spmv_tma), not the 2-bit quad format
-            inp.eps_y[...] = rng.choice([1.0, 2.0, 4.0, 20.0, 78.5, 80.0], inp.eps_y.shape)
-        if periodic:
-            inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
-            inp.eps_y[:, -1, :] = inp.eps_y[:, 0, :]
+            if periodic:
+                inp.eps_x[:, :, -1] = inp.eps_x[:, :, 0]
         tol = 1e-10 if prec == "f64" else 1e-5
         ref = pbref.from_inputs(inp)
         ref.set_periodic(periodic)
@@ -787,7 +779,7 @@ def test_options_are_handle_state(pkg):
         assert pa["persist"] == 0 and pa["face_palette"] == 0 and pa["palette_size"] == 0 and not pa["autotuned"]
         assert pa["spmv_bytes_per_node"] == 40 and pa["vec_bytes_per_node"] == 16
         assert pb_["persist"] == 1 and pb_["face_palette"] == 1 and pb_["palette_size"] == 4
-        assert pb_["spmv_bytes_per_node"] == 26 and pb_["vec_bytes_per_node"] == 13 and pb_["face_quad"] == 1
+        assert pb_["spmv_bytes_per_node"] == 28 and pb_["vec_bytes_per_node"] == 13
         assert pa["num_sm"] == pb_["num_sm"] >= 1 and pa["grid"] >= 1 and pa["threads"] % 32 == 0
         assert a.get_option("palette") == 0 and b.get_option("palette") == 1
         ga, gb = a.solve(1e-5, 5000, "f32"), b.solve(1e-5, 5000, "f32")
@@ -803,3 +795,149 @@ def test_options_are_handle_state(pkg):
         a.set_option("tile_ty", 0)
         a.set_option("tile_txv", 0)
         assert a.plan("f32")["txv"] == pa["txv"] and a.solve(1e-5, 5000, "f32")["iters"] == ga["iters"]
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT row f2: pb_solve_batch -- M right-hand sides per pass (k_spmv_batch + k_vec_batch)
+# ---------------------------------------------------------------------------------------------
+def _members(inp, m, seed):
+    rng = np.random.default_rng(seed)
+    rhs = np.stack([inp.rhs * (1 + 0.3 * s) + rng.standard_normal(inp.rhs.shape) * (0.2 * s) for s in range(m)])
+    bc = np.stack([inp.bc * (1 - 0.1 * s) + rng.uniform(-1, 1, inp.bc.shape) * (0.1 * s) for s in range(m)])
+    return rhs, bc
+
+
+@pytest.mark.parametrize("shape,kind", [((13, 9, 7), "quad"), ((77, 45, 38), "quad"), ((130, 21, 37), "words"),
+                                        ((45, 23, 19), "bytes")])
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_batch_members_match_their_own_oracle_solves(pkg, pbref, shape, kind, prec, tol):
+    """Every member of a batch against ITS OWN oracle solve (north-star bars), for each batch width and coefficient
+    format (2-bit quads for <= 4 face values, words otherwise -- also for a 7-valued map whose single-solve format is
+    the byte palette); per member the iteration count must not depend on the width (1, 2 or 4 members per pass: the
+    arithmetic per member is the same) and must agree with pb_solve's to within one iteration."""
+    inp = random_operator(*shape, seed=21, two_valued=(kind != "words"))
+    if kind == "bytes":
+        inp.eps_y[...] = np.random.default_rng(5).choice([1.0, 2.0, 4.0, 20.0, 78.5, 80.0], inp.eps_y.shape)
+    m = 5                                         # not a multiple of 2 or 4: groups of 2+2+1 and 4+1
+    rhs, bc = _members(inp, m, 3)
+    ref = pbref.from_inputs(inp)
+    orc = []
+    for s in range(m):
+        ref.set_rhs(rhs[s], bc[s])
+        orc.append(ref.solve(tol, 5000))
+    ref.close()
+    lim = 1e-8 if prec == "f64" else 1e-4
+    iters_by_width = {}
+    for width in (1, 2, 4):
+        with pkg.PBSolver(*inp.args(), options=dict(batch_width=width, persist=0)) as sv:
+            g = sv.solve_batch(rhs, bc, tol, 5000, prec, check_every=9)
+            g_again = sv.solve_batch(rhs, bc, tol, 5000, prec, check_every=31)
+            singles = []
+            for s in range(m):
+                sv.set_rhs(rhs[s], bc[s])
+                singles.append(sv.solve(tol, 5000, prec))
+        assert g["worst"] == 0 and g["status"] == [0] * m
+        assert np.array_equal(g["phi"], g_again["phi"]) and g["iters"] == g_again["iters"]      # bitwise repeatable
+        for s in range(m):
+            o = orc[s]
+            scale = np.max(np.abs(o["phi"]))
+            assert g["relres"][s] < tol
+            assert abs(g["iters"][s] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (width, s, g["iters"][s], o["iters"])
+            assert np.max(np.abs(g["phi"][s] - o["phi"])) <= lim * scale, (width, s)
+            assert abs(g["iters"][s] - singles[s]["iters"]) <= 1
+            assert np.max(np.abs(g["phi"][s] - singles[s]["phi"])) <= lim * scale
+        iters_by_width[width] = g["iters"]
+    assert iters_by_width[1] == iters_by_width[2] == iters_by_width[4]
+
+
+def test_batch_per_member_latches(pkg, pbref):
+    """Members stop independently: a zero right-hand side is done at l = 0, a non-finite one breaks down at l = 0 without
+    disturbing its neighbours, an easy member converges long before a hard one, maxiter latches every live member."""
+    inp = random_operator(33, 31, 29, seed=12)
+    rng = np.random.default_rng(9)
+    rhs = np.stack([inp.rhs, np.zeros_like(inp.rhs), inp.rhs.copy(), rng.standard_normal(inp.rhs.shape)])
+    bc = np.stack([inp.bc, np.zeros_like(inp.bc), inp.bc, inp.bc * 0.5])
+    rhs[2, 3, 5, 7] = np.nan
+    ref = pbref.from_inputs(inp)
+    o0 = ref.solve(1e-10, 5000)
+    ref.set_rhs(rhs[3], bc[3])
+    o3 = ref.solve(1e-10, 5000)
+    o3_short = ref.solve(1e-10, 11)
+    ref.close()
+    for width in (2, 4):
+        with pkg.PBSolver(*inp.args(), options=dict(batch_width=width)) as sv:
+            g = sv.solve_batch(rhs, bc, 1e-10, 5000, "f64", check_every=7)
+            assert g["status"] == [0, 0, pkg.binding.PB_ERR_BREAKDOWN, 0] and g["worst"] == pkg.binding.PB_ERR_BREAKDOWN
+            assert g["iters"][1] == 0 and not g["phi"][1].any() and g["relres"][1] == 0.0
+            assert g["iters"][2] == 0 and not g["phi"][2].any()
+            assert g["iters"][0] == o0["iters"] and g["iters"][3] == o3["iters"]
+            assert np.max(np.abs(g["phi"][0] - o0["phi"])) <= 1e-8 * np.max(np.abs(o0["phi"]))
+            assert np.max(np.abs(g["phi"][3] - o3["phi"])) <= 1e-8 * np.max(np.abs(o3["phi"]))
+            short = sv.solve_batch(rhs[[0, 3]], bc[[0, 3]], 1e-10, 11, "f64", check_every=4)
+            assert short["status"] == [pkg.binding.PB_ERR_MAXITER] * 2 and short["iters"] == [11, 11]
+            assert np.max(np.abs(short["phi"][1] - o3_short["phi"])) <= 1e-10 * np.max(np.abs(o3_short["phi"]))
+            sv.set_periodic(True)
+            with pytest.raises(pkg.PBError):
+                sv.solve_batch(rhs, bc, 1e-10, 50, "f64")
+
+
+def test_batch_device_pointers_and_charges(pkg, pbref, cuda_device):
+    """Device-resident members (no host staging), and pb_solve_batch_charges on an atom-built handle against
+    pb_set_charges + pb_solve of each member and against the oracle fed by the setup oracle."""
+    import torch
+
+    from oracle import pbsetup_ref as S
+    from workloads import pb_inputs as W
+
+    inp = make_config(2)
+    m = 3
+    rhs, bc = _members(inp, m, 4)
+    with pkg.PBSolver(*inp.args()) as sv:
+        host = sv.solve_batch(rhs, bc, 1e-5, 5000, "f32")
+        dev = sv.solve_batch(torch.from_numpy(rhs).to(cuda_device), torch.from_numpy(bc).to(cuda_device), 1e-5, 5000, "f32")
+        assert dev["phi"].is_cuda and host["iters"] == dev["iters"]
+        assert np.array_equal(dev["phi"].cpu().numpy(), host["phi"])
+    nx, ny, nz, h = 40, 23, 31, 0.5
+    rng = np.random.Generator(np.random.PCG64(W.SEED0 + 777))
+    L = np.array([(nx - 1) * h, (ny - 1) * h, (nz - 1) * h])
+    c = W.atoms_uniform(30, 0.15 * L, 0.85 * L, rng)
+    r = rng.uniform(1.2, 2.0, 30)
+    Q = rng.normal(0.0, 0.4, (3, 30))
+    with pkg.PBSolver.from_atoms(nx, ny, nz, h, c, r, Q[0], 1.0, 80.0, W.KBAR2_150MM_300K) as sv:
+        g = sv.solve_batch_charges(Q, 1e-10, 5000, "f64")
+        for s in range(3):
+            sv.set_charges(Q[s])
+            one = sv.solve(1e-10, 5000, "f64")
+            f = S.setup(nx, ny, nz, h, c, r, Q[s], 1.0, 80.0, W.KBAR2_150MM_300K)
+            o = pbref.PBRef(nx, ny, nz, h, f["eps_x"], f["eps_y"], f["eps_z"], f["kbar2"], f["rhs"], f["bc"]).solve(1e-10, 5000)
+            scale = np.max(np.abs(o["phi"]))
+            assert g["status"][s] == 0 and abs(g["iters"][s] - o["iters"]) <= max(1, round(0.05 * o["iters"]))
+            assert np.max(np.abs(g["phi"][s] - o["phi"])) <= 1e-8 * scale
+            assert np.max(np.abs(g["phi"][s] - one["phi"])) <= 1e-8 * scale
+
+
+@pytest.mark.slow
+def test_config5_batch_members_multi_rhs_full_size(pkg, pbref):
+    """Two members of configs[4]'s perturbed-charge batch at the full 385^3 through pb_solve_batch_charges (two members
+    per pass, 2-bit face indices), each against the oracle's own solve of that member; fp32, every node."""
+    from workloads import perturbed_charge_values, perturbed_charges
+
+    inp = make_config(5, device="cuda")
+    members = (3, 11)
+    m = inp.meta
+    Q = np.stack([perturbed_charge_values(inp, s) for s in members])
+    with pkg.PBSolver.from_atoms(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], m["radii"], m["charges"], m["eps_in"],
+                                 m["eps_out"], m["kbar2_solvent"]) as sv:
+        g = sv.solve_batch_charges(Q, 1e-5, 20000, "f32", check_every=32)
+    ref = pbref.from_inputs(inp)
+    for i, s in enumerate(members):
+        rhs_s, bc_s = perturbed_charges(inp, s, device="cuda")
+        ref.set_rhs(rhs_s, bc_s)
+        o = ref.solve(1e-5, 5000)
+        scale = np.max(np.abs(o["phi"]))
+        err = np.max(np.abs(g["phi"][i] - o["phi"])) / scale
+        print(f"config5 batch member {s}: iters {g['iters'][i]} (oracle {o['iters']}) err {err:.2e}")
+        assert g["status"][i] == 0 and g["relres"][i] < 1e-5
+        assert abs(g["iters"][i] - o["iters"]) <= round(0.05 * o["iters"])
+        assert err <= 1e-4
+    ref.close()
