@@ -312,6 +312,13 @@ def run_ours(args, rank, local_rank, world):
     tot_iters, ms = aggregate(iters, ms_local, world, dev)
     value = tot_iters / (ms * 1e-3)
 
+    # ---- roofline of the two kernels, CUDA events around every launch, taken right after the timed solves (same
+    # power / clock state: k_spmv_tma follows the SM clock) ----------------------------------------------------
+    peak, peak_src = measured_peak()
+    with ClockSampler(physical_gpu_index(local_rank)) as clocks_prof:
+        solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)
+        kr = kernel_roofline(solver, prec, n_node, args.profile_iters, peak)
+
     # ---- end-to-end leg: host buffers, H2D of rhs/bc and D2H of phi inside the timed region -------
     e2e = None
     if not args.no_e2e:
@@ -339,7 +346,7 @@ def run_ours(args, rank, local_rank, world):
     batch = None
     n_batch = args.batch if args.batch is not None else (50 if (world == 1 and args.config == 5) else 0)
     if n_batch > 0 and "charges" in inp.meta:
-        batch = run_batch(args, solver, inp, prec, tol, n_batch, rank, world, local_rank, dev, out_d, torch)
+        batch = run_batch(args, pkg, inp, prec, tol, n_batch, rank, world, stream, dev, out_d, torch)
 
     # ---- optional (NEXT row f3): mixed-precision iterative refinement against the plain fp64 solve ----------------
     refined = None
@@ -366,9 +373,7 @@ def run_ours(args, rank, local_rank, world):
         setup = run_setup_from_atoms(args, pkg, inp, prec, tol, stream, out_d, t_gen, n_batch, torch)
 
     # ---- roofline of the dominant kernel (K_spmv), CUDA events around every launch ----------------
-    peak, peak_src = measured_peak()
     wl = workload_name(args.config, prec, tol)
-    kr = kernel_roofline(solver, prec, n_node, args.profile_iters, peak)
     ms_spmv, ms_vec = kr["spmv_ms"], kr["vec_ms"]
     pal, pald = solver.palette_size(), solver.diag_palette_size()
     # Bytes per launch.  `achieved` counts the bytes k_spmv_tma HAS to move in the storage format the handle uses
@@ -389,7 +394,8 @@ def run_ours(args, rank, local_rank, world):
                 "algorithmic_bytes_per_launch": spmv_bytes, "bytes_per_node": kr["spmv_bytes_per_node"],
                 "bytes_accounting": "stored-format bytes (pb_bytes_per_node): what physically has to cross HBM; "
                                     "SURVEY 8(d)'s uncompressed words are in survey_10word / iteration.north_star_*",
-                "palette_size": pal, "ms_per_launch": ms_spmv, "plan": plan_summary(solver, prec),
+                "palette_size": pal, "ms_per_launch": ms_spmv, "clocks_during_profile": clocks_prof.summary(),
+                "plan": plan_summary(solver, prec),
                 "survey_10word": {"bytes_per_launch": WORDS_SPMV * elt * n_node,
                                   "GBs": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9,
                                   "frac": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9 / peak},
@@ -467,43 +473,87 @@ def variant_leg(solver, torch, stream, prec, tol, args, inp, peak):
             "plan": plan_summary(solver, prec)}
 
 
-def run_batch(args, solver, inp, prec, tol, n_batch, rank, world, local_rank, dev, out_d, torch):
-    """Config 5's perturbed-charge batch on one operator: pb_set_rhs + pb_solve per member (cold start), and each member
-    solved again from the previous member's potential (pb_solve_from, NEXT row f2)."""
-    from workloads import perturbed_charges
+def run_batch(args, pkg, inp, prec, tol, n_batch, rank, world, stream, dev, out_d, torch):
+    """Config 5's perturbed-charge batch (BASELINE.json configs[4]: 50 solves, same operator, charges + N(0, 0.05) e) on
+    an atom-built handle -- every member's right-hand side and ghost values are made on the GPU (pb_set_charges /
+    pb_solve_batch_charges, NEXT rows f1 + f2):
+      sequential: pb_set_charges + pb_solve per member (cold start);  warm_start: the same members solved again from
+      the previous member's potential (pb_solve_from);  multi_rhs: pb_solve_batch_charges, 1 / 2 / 4 members per pass."""
+    from workloads import perturbed_charge_values
 
-    t_b, it_b, t_w, it_w, t_gen = 0.0, [], 0.0, [], 0.0
+    m = inp.meta
+    t0 = time.perf_counter()
+    s2 = pkg.PBSolver.from_atoms(inp.nx, inp.ny, inp.nz, inp.h, m["centres"], m["radii"], m["charges"], m["eps_in"],
+                                 m["eps_out"], m["kbar2_solvent"], stream=stream.cuda_stream)
+    s2.prepare(prec)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t0
+    Q = np.stack([perturbed_charge_values(inp, world * sidx + rank) for sidx in range(n_batch)])
+    t_set, t_b, it_b, t_w, it_w = 0.0, 0.0, [], 0.0, []
     out_w = torch.empty_like(out_d)
     for sidx in range(n_batch):
         t0 = time.perf_counter()
-        rhs_s, bc_s = perturbed_charges(inp, world * sidx + rank, device=f"cuda:{local_rank}")
-        rhs_d = torch.from_numpy(np.ascontiguousarray(rhs_s)).to(dev)
-        bc_d = torch.from_numpy(np.ascontiguousarray(bc_s)).to(dev)
+        s2.set_charges(Q[sidx])
         torch.cuda.synchronize()
-        t_gen += time.perf_counter() - t0
-        t0 = time.perf_counter()
-        solver.set_rhs(rhs_d, bc_d)
-        it_b.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
+        t1 = time.perf_counter()
+        it_b.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_d)["iters"])
         torch.cuda.synchronize()
-        t_b += time.perf_counter() - t0
+        t2 = time.perf_counter()
+        t_set += t1 - t0
+        t_b += t2 - t1
         if sidx == 0:
             out_w.copy_(out_d)
         else:
             t0 = time.perf_counter()
-            it_w.append(solver.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_w,
-                                     phi0=out_w)["iters"])
+            it_w.append(s2.solve(tol, args.maxiter, prec, check_every=args.check_every, out=out_w, phi0=out_w)["iters"])
             torch.cuda.synchronize()
             t_w += time.perf_counter() - t0
-        del rhs_d, bc_d
-    return {"solves": n_batch, "solves_per_s": n_batch / t_b, "ms_per_solve": 1e3 * t_b / n_batch,
+    del out_w
+    seq_ms = 1e3 * (t_set + t_b) / n_batch
+    multi = {}
+    Qd = torch.from_numpy(Q).to(dev)
+    tdt = torch.float32 if prec == "f32" else torch.float64
+    for width in (1, 2, 4):
+        nm = n_batch if width == 2 else min(n_batch, 12)
+        nm -= nm % width if nm >= width else 0
+        out_m = torch.empty((nm,) + tuple(out_d.shape), dtype=tdt, device=dev)
+        s2.set_option("batch_width", width)
+        try:
+            s2.solve_batch_charges(Qd[:width], tol, args.maxiter, prec, check_every=args.check_every, out=out_m[:width])  # plan + arrays
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            g = s2.solve_batch_charges(Qd[:nm], tol, args.maxiter, prec, check_every=args.check_every, out=out_m)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            # the members' setup alone (maxiter = 0: charges -> rhs / ghost values -> b, init, un-pad), same call path
+            t0 = time.perf_counter()
+            s2.solve_batch_charges(Qd[:nm], tol, 0, prec, check_every=args.check_every, out=out_m)
+            torch.cuda.synchronize()
+            dt_setup = time.perf_counter() - t0
+            solve_ms = 1e3 * (dt - dt_setup) / nm
+            multi[f"width{width}"] = {"members": nm, "ms_per_member": 1e3 * dt / nm, "solves_per_s": nm / dt,
+                                      "setup_ms_per_member": 1e3 * dt_setup / nm,
+                                      "solve_ms_per_member": solve_ms, "mean_iters": float(np.mean(g["iters"])),
+                                      "ms_per_member_iteration": solve_ms / float(np.mean(g["iters"])),
+                                      "all_converged": all(st == 0 for st in g["status"])}
+        except pkg.PBError as e:
+            multi[f"width{width}"] = {"error": str(e)}
+        del out_m
+    s2.close()
+    seq_solve_ms = 1e3 * t_b / n_batch
+    w2 = multi.get("width2", {})
+    return {"solves": n_batch, "solves_per_s": n_batch / (t_set + t_b), "ms_per_solve": seq_ms,
+            "set_charges_ms": 1e3 * t_set / n_batch, "solve_ms": seq_solve_ms,
             "iterations_per_s": float(np.sum(it_b)) / t_b,
             "mean_iters": float(np.mean(it_b)), "min_iters": int(min(it_b)), "max_iters": int(max(it_b)),
-            "warm_start": ({"mean_iters": float(np.mean(it_w)), "ms_per_solve": 1e3 * t_w / len(it_w),
-                            "solves_per_s": len(it_w) / t_w} if it_w else None),
-            "member_generation_s": t_gen,
-            "note": "device-resident rhs/bc, pb_set_rhs + pb_solve per member (wall clock, sequential), this rank only; "
-                    "warm_start: the same members solved again from the previous member's potential (pb_solve_from); "
-                    "member_generation_s = host/torch generation of the members' rhs and ghost values, not timed above"}
+            "warm_start": ({"mean_iters": float(np.mean(it_w)), "solve_ms": 1e3 * t_w / len(it_w)} if it_w else None),
+            "multi_rhs": multi,
+            "multi_rhs_speedup_width2": (seq_solve_ms / w2["solve_ms_per_member"]) if "solve_ms_per_member" in w2 else None,
+            "handle_create_ms": 1e3 * t_create,
+            "note": "atom-built handle (pb_create_from_atoms), this rank only, wall clock; set_charges = charge spreading + "
+                    "the fp64 Debye-Hueckel boundary sum per member (inside ms_per_solve and ms_per_member; solve_ms_per_member = "
+                    "the call minus the same call with maxiter 0); multi_rhs: pb_solve_batch_charges with PB_OPT_BATCH_WIDTH members "
+                    "per kernel pass (k_spmv_batch + k_vec_batch)"}
 
 
 def run_setup_from_atoms(args, pkg, inp, prec, tol, stream, out_d, t_gen, n_batch, torch):

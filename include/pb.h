@@ -150,6 +150,39 @@ pb_status pb_solve_batch_charges(pb_handle *h, int m, const double *charges, dou
                                  double *relres_out, int *status_out);
 
 /*
+ * z-slab decomposition of ONE solve over several GPUs (NEXT row f4; the paper's node had two
+ * GPUs).  Rank r owns the planes [z0, z0 + nz) of the global grid; pb_create_slab takes ITS part of the
+ * inputs (eps_z with the nz + 1 faces of its planes -- the interface faces are passed to both neighbours --, bc with
+ * z-/z+ entries that are ignored across an interface) and says whether a neighbour rank lies below / above; there the
+ * neighbouring plane is an unknown of the other rank, not the Dirichlet ghost layer, so nothing is folded into b and
+ * the kernels read one ghost plane of r, p and Dinv, refreshed by the caller every iteration.  The library has no
+ * communicator of its own: the exchange is the caller's (NCCL through torch.distributed in the Python package,
+ * paper_1704_02745_b200/slab.py).  One PCG iteration (steps 4-8) on every rank:
+ *     pb_slab_step(h, 0)   K_spmv on the slab; local p.Ap                       -> all-reduce ptrs[2] (1 double)
+ *     pb_slab_step(h, 1)   alpha (step 5), K_vec; local r.z, r.r                -> all-reduce ptrs[3] (2 doubles)
+ *     pb_slab_step(h, 2)   beta, stopping rule, latch (steps 3, 7) -- identical on every rank
+ *     pb_slab_step(h, 4)   pack the boundary planes of r and p into ptrs[0]     -> send halves below / above, receive ptrs[1]
+ *     pb_slab_step(h, 5)   unpack ptrs[1] into the ghost planes
+ * and once per solve: pb_slab_begin (steps 1-2; local r.r, r.z), all-reduce ptrs[3], pb_slab_step(h, 3) (the step-2
+ * finaliser: ||b||^2, beta = 0), the Dinv boundary planes ptrs[4], ptrs[5] sent to the neighbours' ptrs[7], ptrs[6],
+ * then pack / exchange / unpack.  Kernels enqueued after the latch is set do nothing, so the loop may run ahead of
+ * pb_slab_latch (which synchronises).  pb_slab_result un-pads this rank's planes of phi.  All other solve / apply
+ * entry points return PB_ERR_INVALID_ARG for a slab handle.  No periodic boundary.
+ */
+pb_status pb_create_slab(pb_handle **out, int nx, int ny, int nz, double h,
+                         const double *eps_x, const double *eps_y, const double *eps_z,
+                         const double *kbar2, const double *rhs, const double *bc,
+                         pb_memspace where, void *cuda_stream, int neighbour_below, int neighbour_above);
+pb_status pb_slab_begin(pb_handle *h, pb_precision prec, double tol, int maxiter);
+pb_status pb_slab_step(pb_handle *h, int which);
+/* ptrs[8]: device pointers (valid after pb_slab_begin, until the handle's options change): 0 send buffer, 1 receive
+ * buffer (4 planes each: r_lo, p_lo, r_hi, p_hi), 2 p.Ap (1 double), 3 {r.z, r.r} (2 doubles), 4 / 5 Dinv planes 0 and
+ * nz-1, 6 / 7 Dinv ghost planes -1 and nz.  *plane_bytes = ny * pitch * sizeof(element). */
+pb_status pb_slab_pointers(pb_handle *h, void **ptrs, size_t *plane_bytes);
+pb_status pb_slab_latch(pb_handle *h, int *done, int *iters, int *status, double *relres);
+pb_status pb_slab_result(pb_handle *h, void *phi_out, pb_memspace where);
+
+/*
  * pb_create_from_atoms -- NEXT row f1, the paper's stated next step "integrated grid stencil setup on GPU"
  * (PAPER.md:11, 283): build the inputs of Eq. 3 on the device from atoms and hand them to pb_create.
  *   centres [n_atoms][3] (x,y,z; node (i,j,k) sits at (i h, j h, k h)), radii [n_atoms], charges [n_atoms]

@@ -21,7 +21,8 @@ EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", 
            "pb_destroy", "pb_strerror", "pb_query", "pb_version", "pb_profile", "pb_launch_count", "pb_set_preconditioner", "pb_create_from_atoms",
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
            "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined", "pb_set_setup_precision", "pb_set_option", "pb_get_option",
-           "pb_prepare", "pb_get_plan", "pb_solve_batch", "pb_solve_batch_charges")
+           "pb_prepare", "pb_get_plan", "pb_solve_batch", "pb_solve_batch_charges", "pb_create_slab", "pb_slab_begin",
+           "pb_slab_step", "pb_slab_pointers", "pb_slab_latch", "pb_slab_result")
 
 # pb_option (include/pb.h), by name
 OPTIONS = {"persist": 0, "persist_max_mb": 1, "persist_fused_max_knodes": 2, "persist_blocks_per_sm": 3,
@@ -97,6 +98,12 @@ def load_library():
                                    ctypes.POINTER(ci)]
     lib.pb_solve_batch_charges.argtypes = [vp, ci, vp, cd, ci, ci, ci, vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd),
                                            ctypes.POINTER(ci)]
+    lib.pb_create_slab.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, vp, vp, vp, vp, vp, vp, ci, vp, ci, ci]
+    lib.pb_slab_begin.argtypes = [vp, ci, cd, ci]
+    lib.pb_slab_step.argtypes = [vp, ci]
+    lib.pb_slab_pointers.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_size_t)]
+    lib.pb_slab_latch.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(cd)]
+    lib.pb_slab_result.argtypes = [vp, vp, ci]
     lib.pb_set_option.argtypes = [vp, ci, ci]
     lib.pb_get_option.argtypes = [vp, ci, ctypes.POINTER(ci)]
     lib.pb_prepare.argtypes = [vp, ci]

@@ -46,6 +46,7 @@ struct Work {
     T *x = nullptr, *r = nullptr, *tmp = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr;   // tmp: pb_apply input
     int P = 0;
     size_t npad = 0;                 // nz*ny*P
+    size_t goff = 0;                 // z-slab mode: r, p0, p1, Dinv start one ghost plane (ny*P elements) into their allocation
     bool ready = false, b_ready = false;
     int vec_grid = 0;
     cudaGraphExec_t graph = nullptr;
@@ -97,6 +98,11 @@ struct pb_handle {
     long long launches;          // kernels enqueued so far (graph-contained ones included)
     int precond;                 // 1 Jacobi (default), 0 none
     int periodic;                // 0 Dirichlet ghost layer (free-space condition, default), 1 periodic
+    bool slab = false;           // z-slab rank of a multi-GPU solve (pb_create_slab): ghost planes, local sums only
+    int iface_lo = 0, iface_hi = 0;   // the plane below / above belongs to a neighbour rank (not the Dirichlet ghost layer)
+    void *slab_send = nullptr, *slab_recv = nullptr;   // 4 planes each: [r_lo | p_lo | r_hi | p_hi]
+    size_t slab_plane_bytes = 0;
+    int slab_prec = -1;
     PalTable *pal_table;         // device; distinct face values of the operator
     PalTable *pald_table;        // device; distinct diagonal values
     int pald_n;                  // -1 unknown, 0 none, else table size
@@ -185,7 +191,10 @@ template <typename T>
 void free_work(Work<T> &w)
 {
     free_batch(w.bw);
-    T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.Dinv, &w.b, &w.x, &w.r, &w.tmp, &w.p0, &w.p1, &w.Ap};
+    T **ghosted[] = {&w.Dinv, &w.r, &w.p0, &w.p1};
+    for (T **a : ghosted) { if (*a) cudaFree(*a - w.goff); *a = nullptr; }
+    w.goff = 0;
+    T **arrs[] = {&w.exm, &w.eym, &w.ezm, &w.D, &w.b, &w.x, &w.tmp, &w.Ap};
     for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
     if (w.graph) { cudaGraphExecDestroy(w.graph); w.graph = nullptr; }
     unsigned char **idx[] = {&w.exi, &w.eyi, &w.ezi};
@@ -202,7 +211,8 @@ pb_status build_b(pb_handle *h, Work<T> &w)
 {
     const double h2 = h->h * h->h;
     k_setup_b<T><<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(
-        h->eps_x, h->eps_y, h->eps_z, h->rhs, h->periodic ? nullptr : h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b);
+        h->eps_x, h->eps_y, h->eps_z, h->rhs, h->periodic ? nullptr : h->bc, h2, h->nx, h->ny, h->nz, w.P, w.b,
+        h->iface_lo, h->iface_hi);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     w.b_ready = true;
@@ -275,14 +285,15 @@ pb_status build_work(pb_handle *h, Work<T> &w)
     // k_spmv_tma decodes through tables addressed by pre-scaled index bytes: n * sizeof(T) <= 256 entries-bytes
     w.pal = h->pal_n > 0 && (size_t)h->pal_n * sizeof(T) <= 256;
     w.pald = w.pal && h->pald_n > 0;
-    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0;
+    // (z-slab mode: Dinv words in the SpMV -- its ghost planes come from the neighbour rank, whose palette differs)
+    w.pald_s = w.pald && (size_t)h->pald_n * sizeof(T) <= 256 && h->opt[PB_OPT_PALETTE_DIAG_SPMV] != 0 && !h->slab;
     w.Pb = (w.P + 15) / 16 * 16;
     // working set (11 node-sized arrays) small enough to live in L2 -> persistent cooperative kernel for pb_solve
     {
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
         const double mb = 11.0 * (double)w.npad * sizeof(T) / 1.0e6;
-        w.persist = coop && h->opt[PB_OPT_PERSIST] != 0 && mb <= (double)h->opt[PB_OPT_PERSIST_MAX_MB];
+        w.persist = coop && h->opt[PB_OPT_PERSIST] != 0 && mb <= (double)h->opt[PB_OPT_PERSIST_MAX_MB] && !h->slab;
     }
     pb_status s = PB_OK;
     if (w.pal && w.persist &&
@@ -304,11 +315,21 @@ pb_status build_work(pb_handle *h, Work<T> &w)
         free_work(w);
         return s;
     }
-    if ((s = alloc_arr(&w.D, w.npad)) || (s = alloc_arr(&w.Dinv, w.npad)) || (s = alloc_arr(&w.b, w.npad)) ||
-        (s = alloc_arr(&w.x, w.npad)) || (s = alloc_arr(&w.r, w.npad)) || (s = alloc_arr(&w.tmp, w.npad)) ||
-        (s = alloc_arr(&w.p0, w.npad)) || (s = alloc_arr(&w.p1, w.npad)) || (s = alloc_arr(&w.Ap, w.npad))) {
+    if ((s = alloc_arr(&w.D, w.npad)) || (s = alloc_arr(&w.b, w.npad)) || (s = alloc_arr(&w.x, w.npad)) ||
+        (s = alloc_arr(&w.tmp, w.npad)) || (s = alloc_arr(&w.Ap, w.npad))) {
         free_work(w);
         return s;
+    }
+    {   // the haloed arrays; in z-slab mode with one ghost plane below plane 0 and one above plane nz-1 (zeroed: the
+        // Dirichlet ghost layer where there is no neighbour rank; Dinv = 1 there so that p_new(ghost) = 0 exactly)
+        const size_t gp = h->slab ? (size_t)h->ny * w.P : 0;
+        T **ghosted[] = {&w.Dinv, &w.r, &w.p0, &w.p1};
+        for (T **a : ghosted) {
+            if ((s = alloc_arr(a, w.npad + 2 * gp))) { w.goff = 0; free_work(w); return s; }
+            if (gp) PB_CUDA(cudaMemsetAsync(*a, 0, (w.npad + 2 * gp) * sizeof(T), h->stream));
+        }
+        for (T **a : ghosted) *a += gp;
+        w.goff = gp;
     }
     w.vec_grid = grid_for(w.npad / VecN<T>::value, 512, h->nsm * (h->opt[PB_OPT_VEC_BLOCKS_PER_SM] > 0 ? h->opt[PB_OPT_VEC_BLOCKS_PER_SM] : 4));   // 2 vectors per thread and pass
     if (w.persist) {
@@ -470,12 +491,13 @@ pb_status configure_tma(pb_handle *h, Work<T> &w, const TileCfg &c)
     w.qntz = (h->nz + TZ - 1) / TZ;
     const long ntiles = (long)xy * w.qntz;
     w.qgrid = (int)(ntiles < slots ? ntiles : slots);
-    PB_TRY(make_map<T>(&w.tm_r, w.r, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    const int gpl = w.goff ? 2 : 0;      // z-slab mode: ghost planes in the haloed tensors (the kernel adds zoff = 1)
+    PB_TRY(make_map<T>(&w.tm_r, w.r - w.goff, w.P, h->ny, h->nz + gpl, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_tmp, w.tmp, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
     if (w.pald_s) PB_TRY(make_map_u8(&w.tm_dinv, w.dvib, w.Pb, h->ny, h->nz, L.bwd, TY + 2));
-    else PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
-    PB_TRY(make_map<T>(&w.tm_p0, w.p0, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
-    PB_TRY(make_map<T>(&w.tm_p1, w.p1, w.P, h->ny, h->nz, (TXV + 2) * VEC, TY + 2));
+    else PB_TRY(make_map<T>(&w.tm_dinv, w.Dinv - w.goff, w.P, h->ny, h->nz + gpl, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_p0, w.p0 - w.goff, w.P, h->ny, h->nz + gpl, (TXV + 2) * VEC, TY + 2));
+    PB_TRY(make_map<T>(&w.tm_p1, w.p1 - w.goff, w.P, h->ny, h->nz + gpl, (TXV + 2) * VEC, TY + 2));
     PB_TRY(make_map<T>(&w.tm_x, w.x, w.P, h->ny, h->nz, TXV * VEC, TY));
     if (w.pal) {
         PB_TRY(make_map_u8(&w.tm_ex, w.exi, w.Pb, h->ny, h->nz, L.bw, TY));
@@ -655,6 +677,7 @@ void launch_spmv(pb_handle *h, Work<T> &w, double out_scale)
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
     a.TXV = w.qTXV; a.TY = w.qTY; a.TZ = w.qTZ; a.ntx = w.qntx; a.nty = w.qnty; a.ntz = w.qntz;
     a.ntiles = w.qntx * w.qnty * w.qntz; a.nstage = w.qns; a.l2hints = h->opt[PB_OPT_L2_HINTS]; a.precond = h->precond;
+    a.zoff = (MODE == 0 && w.goff) ? 1 : 0;
     a.st = h->st; a.partials = h->partials; a.out_scale = out_scale;
     a.lut = w.lut; a.dlut = w.dlut;
     if (w.pald_s)
@@ -953,6 +976,69 @@ pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_
 
 #include "pb_api_batch.cuh"
 
+// ---- NEXT row f4: one solve over several GPUs, z-slab decomposition -------------------------
+// The library provides the per-rank pieces; the ranks' exchange (halo planes, scalar all-reduces) is the caller's --
+// torch.distributed / NCCL in paper_1704_02745_b200/slab.py.
+template <typename T>
+pb_status slab_begin(pb_handle *h, double tol, int maxiter)
+{
+    PB_TRY(ensure<T>(h));
+    Work<T> &w = work<T>(h);
+    const size_t plane = (size_t)h->ny * w.P;
+    if (h->slab_prec != (int)(sizeof(T) == 4 ? PB_F32 : PB_F64) || !h->slab_send) {
+        if (h->slab_send) { cudaFree(h->slab_send); h->slab_send = nullptr; }
+        if (h->slab_recv) { cudaFree(h->slab_recv); h->slab_recv = nullptr; }
+        PB_ALLOC(cudaMalloc(&h->slab_send, 4 * plane * sizeof(T)));
+        PB_ALLOC(cudaMalloc(&h->slab_recv, 4 * plane * sizeof(T)));
+        PB_CUDA(cudaMemsetAsync(h->slab_recv, 0, 4 * plane * sizeof(T), h->stream));
+        h->slab_plane_bytes = plane * sizeof(T);
+        h->slab_prec = sizeof(T) == 4 ? PB_F32 : PB_F64;
+    }
+    h->last_prec = sizeof(T) == 4 ? PB_F32 : PB_F64;
+    // ghost planes of both p buffers start at 0 (p_0 = z_0: beta = 0 multiplies them, they must be finite)
+    PB_CUDA(cudaMemsetAsync(w.p0 - w.goff, 0, (w.npad + 2 * w.goff) * sizeof(T), h->stream));
+    PB_CUDA(cudaMemsetAsync(w.p1 - w.goff, 0, (w.npad + 2 * w.goff) * sizeof(T), h->stream));
+    k_set_state<<<1, 1, 0, h->stream>>>(h->st, tol * tol, maxiter, 1, 1);
+    k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(vec_args<T>(h, w));       // local r.z, r.r -> State::loc_*
+    PB_CUDA(cudaGetLastError());
+    h->launches += 2;
+    return PB_OK;
+}
+
+template <typename T>
+pb_status slab_pack(pb_handle *h, bool unpack)
+{
+    Work<T> &w = work<T>(h);
+    if (!w.ready || !h->slab_send) return PB_ERR_INVALID_ARG;
+    const size_t plane = (size_t)h->ny * w.P;
+    const int g = grid_for(plane, 256, h->nsm * 4);
+    if (unpack) k_slab_unpack<T><<<g, 256, 0, h->stream>>>(w.r, w.p0, w.p1, h->st, (const T *)h->slab_recv, plane, h->nz,
+                                                          h->iface_lo, h->iface_hi);
+    else k_slab_pack<T><<<g, 256, 0, h->stream>>>(w.r, w.p0, w.p1, h->st, (T *)h->slab_send, plane, h->nz);
+    PB_CUDA(cudaGetLastError());
+    h->launches += 1;
+    return PB_OK;
+}
+
+template <typename T>
+pb_status slab_step(pb_handle *h, int which)
+{
+    Work<T> &w = work<T>(h);
+    if (!w.ready) return PB_ERR_INVALID_ARG;
+    if (which == 0) {
+        launch_spmv<T, 0>(h, w, 1.0);                                        // local p.Ap -> State::pAp
+    } else {
+        k_slab_alpha<<<1, 1, 0, h->stream>>>(h->st);                        // pAp is global now
+        const VecArgs<T> va = vec_args<T>(h, w);
+        if (w.pald) k_vec<T, true><<<w.vec_grid, 256, 0, h->stream>>>(va);  // local r.z, r.r -> State::loc_*
+        else k_vec<T, false><<<w.vec_grid, 256, 0, h->stream>>>(va);
+        h->launches += 1;
+    }
+    PB_CUDA(cudaGetLastError());
+    h->launches += 1;
+    return PB_OK;
+}
+
 template <typename T>
 pb_status apply_impl(pb_handle *h, const void *x, void *y, pb_memspace where)
 {
@@ -1096,6 +1182,8 @@ pb_status pb_destroy(pb_handle *h)
     if (h->partials) cudaFree(h->partials);
     if (h->bad) cudaFree(h->bad);
     if (h->stage) cudaFree(h->stage);
+    if (h->slab_send) cudaFree(h->slab_send);
+    if (h->slab_recv) cudaFree(h->slab_recv);
     if (h->atoms_c) cudaFree(h->atoms_c);
     if (h->pal_table) cudaFree(h->pal_table);
     if (h->pald_table) cudaFree(h->pald_table);
@@ -1183,6 +1271,93 @@ pb_status pb_set_rhs(pb_handle *h, const double *rhs, const double *bc, pb_memsp
     return PB_OK;
 }
 
+pb_status pb_create_slab(pb_handle **out, int nx, int ny, int nz, double hh,
+                         const double *eps_x, const double *eps_y, const double *eps_z,
+                         const double *kbar2, const double *rhs, const double *bc,
+                         pb_memspace where, void *cuda_stream, int neighbour_below, int neighbour_above)
+{
+    PB_TRY(pb_create(out, nx, ny, nz, hh, eps_x, eps_y, eps_z, kbar2, rhs, bc, where, cuda_stream));
+    (*out)->slab = true;
+    (*out)->iface_lo = neighbour_below ? 1 : 0;
+    (*out)->iface_hi = neighbour_above ? 1 : 0;
+    return PB_OK;
+}
+
+pb_status pb_slab_begin(pb_handle *h, pb_precision prec, double tol, int maxiter)
+{
+    if (!h || !h->slab || !valid_prec(prec) || !(tol > 0.0) || maxiter < 0 || h->periodic) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    return prec == PB_F32 ? slab_begin<float>(h, tol, maxiter) : slab_begin<double>(h, tol, maxiter);
+}
+
+pb_status pb_slab_step(pb_handle *h, int which)
+{
+    if (!h || !h->slab || h->slab_prec < 0 || which < 0 || which > 5) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    const bool f32 = h->slab_prec == PB_F32;
+    switch (which) {
+    case 0: case 1: return f32 ? slab_step<float>(h, which) : slab_step<double>(h, which);
+    case 2: case 3:
+        k_slab_finish<<<1, 1, 0, h->stream>>>(h->st, which == 3 ? 1 : 0);
+        PB_CUDA(cudaGetLastError());
+        h->launches += 1;
+        return PB_OK;
+    case 4: return f32 ? slab_pack<float>(h, false) : slab_pack<double>(h, false);
+    default: return f32 ? slab_pack<float>(h, true) : slab_pack<double>(h, true);
+    }
+}
+
+pb_status pb_slab_pointers(pb_handle *h, void **ptrs, size_t *plane_bytes)
+{
+    if (!h || !h->slab || h->slab_prec < 0 || !ptrs || !plane_bytes) return PB_ERR_INVALID_ARG;
+    const size_t pb_ = h->slab_plane_bytes;
+    char *dinv = h->slab_prec == PB_F32 ? (char *)h->wf.Dinv : (char *)h->wd.Dinv;
+    ptrs[0] = h->slab_send;                                  // [r_lo | p_lo | r_hi | p_hi], 4 planes
+    ptrs[1] = h->slab_recv;                                  // [r_below | p_below | r_above | p_above]
+    ptrs[2] = &h->st->pAp;                                   // 1 double: local p.Ap, all-reduced in place
+    ptrs[3] = &h->st->loc_rz;                                // 2 doubles: local r.z, r.r, all-reduced in place
+    ptrs[4] = dinv;                                          // Dinv plane 0        (to the rank below, once)
+    ptrs[5] = dinv + (size_t)(h->nz - 1) * pb_;              // Dinv plane nz-1     (to the rank above, once)
+    ptrs[6] = dinv - pb_;                                    // Dinv ghost plane -1 (from the rank below)
+    ptrs[7] = dinv + (size_t)h->nz * pb_;                    // Dinv ghost plane nz (from the rank above)
+    *plane_bytes = pb_;
+    return PB_OK;
+}
+
+pb_status pb_slab_latch(pb_handle *h, int *done, int *iters, int *status, double *relres)
+{
+    if (!h || !h->slab) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    const State &st = *h->pinned_state;
+    if (done) *done = st.done;
+    if (iters) *iters = st.done ? st.iters : st.iter_cur;
+    if (status) *status = st.status;
+    if (relres) *relres = (st.bb > 0.0) ? sqrt(st.rr / st.bb) : 0.0;
+    return PB_OK;
+}
+
+pb_status pb_slab_result(pb_handle *h, void *phi_out, pb_memspace where)
+{
+    if (!h || !h->slab || h->slab_prec < 0 || !phi_out || !valid_space(where)) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(h->device));
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    const size_t esz = h->slab_prec == PB_F32 ? 4 : 8;
+    void *dst = phi_out;
+    if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * esz)); dst = h->stage; }
+    const int g = grid_for(n, 256, h->nsm * 16);
+    if (h->slab_prec == PB_F32)
+        k_finish<float, float><<<g, 256, 0, h->stream>>>(h->wf.x, h->wf.p0, h->wf.p1, h->st, (float *)dst, h->nx, h->wf.P, rows);
+    else
+        k_finish<double, double><<<g, 256, 0, h->stream>>>(h->wd.x, h->wd.p0, h->wd.p1, h->st, (double *)dst, h->nx, h->wd.P, rows);
+    PB_CUDA(cudaGetLastError());
+    h->launches += 1;
+    if (where == PB_HOST) PB_CUDA(cudaMemcpyAsync(phi_out, dst, n * esz, cudaMemcpyDeviceToHost, h->stream));
+    PB_CUDA(cudaStreamSynchronize(h->stream));
+    return PB_OK;
+}
+
 pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
 {
     if (!h || (int)opt < 0 || (int)opt >= (int)PB_OPT_COUNT_ || value < 0) return PB_ERR_INVALID_ARG;
@@ -1258,6 +1433,7 @@ pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
 
 pb_status pb_apply(pb_handle *h, pb_precision prec, const void *x, void *y, pb_memspace where)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !x || !y || x == y || !valid_prec(prec) || !valid_space(where)) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? apply_impl<float>(h, x, y, where) : apply_impl<double>(h, x, y, where);
@@ -1266,6 +1442,7 @@ pb_status pb_apply(pb_handle *h, pb_precision prec, const void *x, void *y, pb_m
 pb_status pb_solve(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
                    void *phi_out, pb_memspace where, int *iters_out, double *relres_out)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !phi_out || !(tol > 0.0) || !std::isfinite(tol) || maxiter < 0 || check_every < 1 ||
         !valid_prec(prec) || !valid_space(where))
         return PB_ERR_INVALID_ARG;
@@ -1278,6 +1455,7 @@ pb_status pb_solve_batch(pb_handle *h, int m, const double *rhs, const double *b
                          pb_precision prec, int check_every, void *phi_out, pb_memspace where, int *iters_out,
                          double *relres_out, int *status_out)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || m < 1 || !phi_out || !(tol > 0.0) || !std::isfinite(tol) || maxiter < 0 || check_every < 1 ||
         !valid_prec(prec) || !valid_space(where))
         return PB_ERR_INVALID_ARG;
@@ -1292,6 +1470,7 @@ pb_status pb_solve_batch_charges(pb_handle *h, int m, const double *charges, dou
                                  pb_precision prec, int check_every, void *phi_out, pb_memspace where, int *iters_out,
                                  double *relres_out, int *status_out)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || m < 1 || !h->atoms_c || (h->n_atoms && !charges) || !phi_out || !(tol > 0.0) || !std::isfinite(tol) ||
         maxiter < 0 || check_every < 1 || !valid_prec(prec) || !valid_space(where))
         return PB_ERR_INVALID_ARG;
@@ -1305,6 +1484,7 @@ pb_status pb_solve_batch_charges(pb_handle *h, int m, const double *charges, dou
 pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec, int check_every,
                         const void *phi0, void *phi_out, pb_memspace where, int *iters_out, double *relres_out)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !phi_out || !(tol > 0.0) || !std::isfinite(tol) || maxiter < 0 || check_every < 1 ||
         !valid_prec(prec) || !valid_space(where))
         return PB_ERR_INVALID_ARG;
@@ -1317,6 +1497,7 @@ pb_status pb_solve_from(pb_handle *h, double tol, int maxiter, pb_precision prec
 pb_status pb_solve_refined(pb_handle *h, double tol, int maxiter, double inner_tol, int check_every, double *phi_out,
                            pb_memspace where, int *outer_out, int *iters_out, double *relres_out)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !phi_out || !(tol > 0.0) || !(inner_tol > 0.0) || maxiter < 0 || check_every < 1 || !valid_space(where))
         return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
@@ -1325,6 +1506,7 @@ pb_status pb_solve_refined(pb_handle *h, double tol, int maxiter, double inner_t
 
 pb_status pb_residual(pb_handle *h, pb_precision prec, const void *phi, pb_memspace where, double *relres_out)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !phi || !relres_out || !valid_prec(prec) || !valid_space(where)) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? residual_impl<float>(h, phi, where, relres_out)
@@ -1365,6 +1547,7 @@ pb_status pb_set_boundary(pb_handle *h, int kind)
 
 pb_status pb_solve_begin(pb_handle *h, pb_precision prec)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !valid_prec(prec)) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? begin_solve<float>(h, 1.0, 0, 0) : begin_solve<double>(h, 1.0, 0, 0);
@@ -1372,6 +1555,7 @@ pb_status pb_solve_begin(pb_handle *h, pb_precision prec)
 
 pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !valid_prec(prec) || n_iter < 0) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
     if (prec == PB_F32) { if (!h->wf.ready) return PB_ERR_INVALID_ARG; return enqueue_iterations<float>(h, h->wf, n_iter); }
@@ -1381,6 +1565,7 @@ pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
 
 pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spmv, double *ms_vec)
 {
+    if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !valid_prec(prec) || n_iter < 1) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
     return prec == PB_F32 ? profile_impl<float>(h, n_iter, ms_spmv, ms_vec)

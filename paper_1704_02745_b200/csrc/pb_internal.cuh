@@ -27,6 +27,12 @@ struct State {
     int latch;        // 0: never latch (pb_iterate / benchmarking), 1: normal
     unsigned int ticket_spmv;
     unsigned int ticket_vec;
+    // z-slab decomposition of ONE solve over several GPUs (pb_slab_*): the finalisers leave the
+    // LOCAL sums here (pAp above, r.z / r.r below); the caller all-reduces them over the ranks in place, and the
+    // k_slab_alpha / k_slab_finish kernels then take the same decisions on every rank
+    double loc_rz, loc_rr;
+    int slab;
+    int pad_;
 };
 
 // 16-byte vector of T: 4 floats or 2 doubles -> one 128-bit load/store per thread

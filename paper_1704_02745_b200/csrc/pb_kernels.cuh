@@ -87,7 +87,8 @@ __device__ __forceinline__ void reduce_and_finish(State *st, double *partials, d
         const double rr = final_sum(partials + nblk, nblk, red);
         if (threadIdx.x == 0) {
             st->ticket_vec = 0u;
-            finish_iteration(st, rz, rr, init);
+            if (st->slab) { st->loc_rz = rz; st->loc_rr = rr; }      // local sums: k_slab_finish after the all-reduce
+            else finish_iteration(st, rz, rr, init);
         }
     }
 }
@@ -462,6 +463,63 @@ __global__ void k_finish_add(const T *__restrict__ x, const T *__restrict__ pbuf
         const int i = (int)(t % nx);
         const size_t row = t / nx;
         acc[row * Pacc + i] += (alpha == T(0)) ? (S)x[row * P + i] : (S)fma(alpha, p[row * P + i], x[row * P + i]);
+    }
+}
+
+}  // namespace pb
+
+// ---------------------------------------------------------------------------------------
+// z-slab decomposition of one solve over several GPUs (the paper's node had two GPUs,
+// PAPER.md:184).  Each rank owns nz_local planes plus one ghost plane of r, p and Dinv on either side; per iteration
+// the ranks exchange the boundary planes of r and p and all-reduce p.Ap and {r.z, r.r} (the caller does both, with
+// NCCL through torch.distributed; the sums live in the State).  These kernels are the scalar steps that follow an
+// all-reduce -- the same decisions as the single-GPU finalisers, taken identically on every rank.
+// ---------------------------------------------------------------------------------------
+namespace pb {
+
+__global__ void k_slab_alpha(State *st)        // after the all-reduce of st->pAp: step 5
+{
+    if (st->done) return;
+    const double pAp = st->pAp;
+    if (!(pAp > 0.0) || !isfinite(pAp)) {
+        if (st->latch) { st->done = 1; st->iters = st->iter_cur; st->status = 5; }
+        st->alpha = 0.0;
+    } else {
+        st->alpha = st->rz / pAp;
+    }
+}
+
+__global__ void k_slab_finish(State *st, int init)   // after the all-reduce of {loc_rz, loc_rr}: steps 3 and 7
+{
+    if (!init && st->done) return;
+    finish_iteration(st, st->loc_rz, st->loc_rr, init);
+}
+
+// boundary planes -> send buffer [r_lo | p_lo | r_hi | p_hi] (p = the buffer the NEXT k_spmv_tma reads), and
+// receive buffer [r_below | p_below | r_above | p_above] -> ghost planes.  `plane` = ny*P elements.
+template <typename T>
+__global__ void k_slab_pack(const T *__restrict__ r, const T *__restrict__ p0, const T *__restrict__ p1,
+                            const State *st, T *send, size_t plane, int nz)
+{
+    const T *p = (st->iter_cur & 1) ? p1 : p0;
+    const size_t top = (size_t)(nz - 1) * plane;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < plane; t += (size_t)gridDim.x * blockDim.x) {
+        send[t] = r[t];
+        send[plane + t] = p[t];
+        send[2 * plane + t] = r[top + t];
+        send[3 * plane + t] = p[top + t];
+    }
+}
+
+template <typename T>
+__global__ void k_slab_unpack(T *r, T *p0, T *p1, const State *st, const T *__restrict__ recv, size_t plane, int nz,
+                              int iface_lo, int iface_hi)
+{
+    T *p = (st->iter_cur & 1) ? p1 : p0;
+    const size_t above = (size_t)nz * plane;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < plane; t += (size_t)gridDim.x * blockDim.x) {
+        if (iface_lo) { (r - plane)[t] = recv[t]; (p - plane)[t] = recv[plane + t]; }
+        if (iface_hi) { r[above + t] = recv[2 * plane + t]; p[above + t] = recv[3 * plane + t]; }
     }
 }
 

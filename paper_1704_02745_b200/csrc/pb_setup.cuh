@@ -48,7 +48,8 @@ __global__ void k_setup_coeff(const double *__restrict__ eps_x, const double *__
 template <typename T>
 __global__ void k_setup_b(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
                           const double *__restrict__ eps_z, const double *__restrict__ rhs,
-                          const double *__restrict__ bc, double h2, int nx, int ny, int nz, int P, T *b)
+                          const double *__restrict__ bc, double h2, int nx, int ny, int nz, int P, T *b,
+                          int iface_lo = 0, int iface_hi = 0)   // z-slab: the plane below / above belongs to a neighbour rank
 {
     const size_t total = (size_t)nz * ny * P;
     const size_t o_xp = (size_t)nz * ny, o_ym = 2 * o_xp, o_yp = o_ym + (size_t)nz * nx,
@@ -67,8 +68,8 @@ __global__ void k_setup_b(const double *__restrict__ eps_x, const double *__rest
                 if (i == nx - 1) v += eps_x[row * (nx + 1) + nx] * bc[o_xp + (size_t)k * ny + j];
                 if (j == 0)      v += eps_y[((size_t)k * (ny + 1)) * nx + i] * bc[o_ym + (size_t)k * nx + i];
                 if (j == ny - 1) v += eps_y[((size_t)k * (ny + 1) + ny) * nx + i] * bc[o_yp + (size_t)k * nx + i];
-                if (k == 0)      v += eps_z[(size_t)j * nx + i] * bc[o_zm + (size_t)j * nx + i];
-                if (k == nz - 1) v += eps_z[((size_t)nz * ny + j) * nx + i] * bc[o_zp + (size_t)j * nx + i];
+                if (k == 0 && !iface_lo)      v += eps_z[(size_t)j * nx + i] * bc[o_zm + (size_t)j * nx + i];
+                if (k == nz - 1 && !iface_hi) v += eps_z[((size_t)nz * ny + j) * nx + i] * bc[o_zp + (size_t)j * nx + i];
             }
         }
         b[t] = (T)v;
@@ -101,8 +102,11 @@ __global__ void k_unpad(const T *__restrict__ src, S *dst, int nx, int P, size_t
     }
 }
 
-__global__ void k_set_state(State *st, double tol2, int maxiter, int latch)
+__global__ void k_set_state(State *st, double tol2, int maxiter, int latch, int slab = 0)
 {
+    st->slab = slab;
+    st->loc_rz = 0.0;
+    st->loc_rr = 0.0;
     st->tol2 = tol2;
     st->maxiter = maxiter;
     st->latch = latch;

@@ -37,6 +37,7 @@ struct TmaArgs {
     int ntx, nty, ntz, ntiles;
     int nstage;
     int precond;             // 1: M = diag(A) (Jacobi); 0: M = I (plain CG)
+    int zoff;                // z-slab mode: the haloed tensors (r, Dinv, p) start one GHOST plane below plane 0
     int l2hints;             // 1: evict_last on r/Dinv/Ap (re-read by k_vec), evict_first on the streamed arrays
     State *st;
     double *partials;        // one per block
@@ -160,12 +161,13 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                     if (centre) bytes += L.bEX + L.bEY + (MODE == 0 ? L.bD : L.bDv);
                     const int xd = PALD ? ((x0 - VEC) & ~15) : x0 - VEC;   // byte-index box: 16-byte aligned start
                     mbar_expect_tx(&full_bar[s], bytes);
-                    tma_load_3d_hint(slot + L.oR, &tm_r, x0 - VEC, j0 - 1, q, &full_bar[s], pol_keep);
+                    const int qh = q + a.zoff;                  // plane of the haloed tensors (ghost plane = plane 0 in slab mode)
+                    tma_load_3d_hint(slot + L.oR, &tm_r, x0 - VEC, j0 - 1, qh, &full_bar[s], pol_keep);
                     if (MODE == 0) {
-                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, xd, j0 - 1, q, &full_bar[s], pol_keep);
-                        tma_load_3d_hint(slot + L.oPp, tm_pin, x0 - VEC, j0 - 1, q, &full_bar[s], pol_pold);
+                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, xd, j0 - 1, qh, &full_bar[s], pol_keep);
+                        tma_load_3d_hint(slot + L.oPp, tm_pin, x0 - VEC, j0 - 1, qh, &full_bar[s], pol_pold);
                     } else if (centre) {
-                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, xd, j0 - 1, q, &full_bar[s], pol_keep);
+                        tma_load_3d_hint(slot + L.oDv, &tm_dinv, xd, j0 - 1, qh, &full_bar[s], pol_keep);
                     }
                     const int xc = PAL ? (x0 & ~15) : x0;      // byte-index boxes start 16-byte aligned
                     if (ez) tma_load_3d_hint(slot + L.oEZ, &tm_ez, xc, j0, q, &full_bar[s], pol_stream);
@@ -376,7 +378,9 @@ k_spmv_tma(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUt
                 State *st = a.st;
                 st->ticket_spmv = 0u;
                 st->pAp = pAp;
-                if (!(pAp > 0.0) || !isfinite(pAp)) {          // breakdown: not SPD / NaN
+                if (st->slab) {
+                    // z-slab mode: this is the LOCAL sum; alpha follows in k_slab_alpha after the all-reduce
+                } else if (!(pAp > 0.0) || !isfinite(pAp)) {          // breakdown: not SPD / NaN
                     if (st->latch) { st->done = 1; st->iters = st->iter_cur; st->status = 5; }
                     st->alpha = 0.0;                            // x already holds the last good iterate
                 } else {
