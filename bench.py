@@ -56,6 +56,9 @@ def parse_args(argv=None):
                          "--config 5, else 0)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="per-handle option for the benchmarked solver (pb_set_option names of the binding), repeatable")
+    ap.add_argument("--slab", type=int, default=0, metavar="N",
+                    help="instead of replicas: ONE solve cut into z-slabs (NEXT row f4).  Under torchrun one slab per "
+                         "rank (NCCL halo exchange + all-reduces, strong scaling); at --gpus 1: N slabs emulated on one GPU")
     ap.add_argument("--no-variants", action="store_true",
                     help="skip the other-precision and no-palette legs of the roofline record")
     ap.add_argument("--cpu-per-config", action="store_true",
@@ -645,6 +648,80 @@ def cpu_baseline(args, inp, tol, wl):
     return cpu
 
 
+def run_slab(args, rank, local_rank, world):
+    """One solve of the configured workload cut into z-slabs (paper_1704_02745_b200/slab.py): one slab per rank under
+    torchrun (halo planes and the three dot products over NCCL), or args.slab slabs on one GPU.  Strong scaling."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1704_02745_b200 import build as pb_build
+
+    if rank == 0:
+        pb_build.build()
+    if world > 1:
+        dist.barrier()
+    from paper_1704_02745_b200.slab import SlabComm, SlabRank, partition, slab_inputs, solve_slabs
+
+    prec = args.precision
+    tol = args.tol or TOL[prec]
+    inp, rhs, bc = build_inputs(args.config, 0, 1, f"cuda:{local_rank}")
+    nslabs = world if world > 1 else max(1, args.slab)
+    owner = list(range(world)) if world > 1 else [0] * nslabs
+    parts = partition(inp.nz, nslabs)
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        comm = SlabComm(owner, rank, dist)
+        ranks = {}
+        for s in comm.local():
+            z0, nzl = parts[s]
+            ranks[s] = SlabRank(s, nslabs, inp.nx, inp.ny, nzl, inp.h,
+                                *slab_inputs(inp.nx, inp.ny, inp.nz, inp.eps_x, inp.eps_y, inp.eps_z, inp.kbar2, rhs, bc,
+                                             z0, nzl), stream=stream.cuda_stream)
+        for _ in range(max(1, args.warmup)):
+            res = solve_slabs(ranks, comm, tol, args.maxiter, prec, args.check_every, device_result=True)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        iters = 0
+        with ClockSampler(physical_gpu_index(local_rank)) as clocks:
+            e0.record(stream)
+            for _ in range(args.steps):
+                res = solve_slabs(ranks, comm, tol, args.maxiter, prec, args.check_every, device_result=True)
+                iters += res[comm.local()[0]]["iters"]
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+        ms_local = e0.elapsed_time(e1)
+        for r in ranks.values():
+            r.close()
+    _, ms = aggregate(0, ms_local, world, dev)
+    line = None
+    if rank == 0:
+        first = res[comm.local()[0]]
+        line = {"metric": METRIC, "value": iters / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": prec, "data": "synthetic",
+                "config": {"workload": workload_name(args.config, prec, tol), "grid": [inp.nx, inp.ny, inp.nz],
+                           "parallelism": f"one solve, {nslabs} z-slabs" + ("" if world > 1 else " emulated on one GPU"),
+                           "slabs": parts, "iterations_per_solve": first["iters"], "final_relres": first["relres"],
+                           "check_every": args.check_every,
+                           "exchange": "per iteration: 2+2 boundary planes per neighbour, all-reduce of 1 and of 2 doubles"},
+                "clocks": clocks.summary(), "e2e": None, "gpu_launches": None, "roofline": None, "cpu_baseline": None}
+    if world > 1:
+        dist.destroy_process_group()
+    return line
+
+
 def self_launch(args, argv):
     """`python bench.py --gpus N` (N > 1) started without a launcher: start the N local ranks ourselves, the way the
     driver does (torch.distributed.run, one rank per GPU, rendezvous on 127.0.0.1)."""
@@ -671,6 +748,8 @@ def main(argv=None):
         print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; reporting n_gpus={world}", file=sys.stderr)
     if args.impl == "reference":
         line = run_reference(args, rank, world)
+    elif args.slab:
+        line = run_slab(args, rank, local_rank, world)
     else:
         line = run_ours(args, rank, local_rank, world)
     if line is not None:

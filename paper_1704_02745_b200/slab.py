@@ -130,9 +130,16 @@ class SlabRank:
             raise B.PBError(st, "pb_slab_latch")
         return dict(done=bool(d.value), iters=it.value, status=stt.value, relres=rel.value)
 
-    def result(self):
-        out = np.empty((self.nz, self.ny, self.nx), dtype=self.dtype)
-        st = B.load_library().pb_slab_result(self._h, ctypes.c_void_p(out.ctypes.data), B.PB_HOST)
+    def result(self, device=False):
+        """This rank's planes of phi: a numpy array, or (device=True) a CUDA tensor -- no copy to the host."""
+        if device:
+            torch = self._torch
+            out = torch.empty((self.nz, self.ny, self.nx), device="cuda",
+                              dtype=torch.float32 if self.dtype == np.float32 else torch.float64)
+            st = B.load_library().pb_slab_result(self._h, ctypes.c_void_p(out.data_ptr()), B.PB_DEVICE)
+        else:
+            out = np.empty((self.nz, self.ny, self.nx), dtype=self.dtype)
+            st = B.load_library().pb_slab_result(self._h, ctypes.c_void_p(out.ctypes.data), B.PB_HOST)
         if st != B.PB_OK:
             raise B.PBError(st, "pb_slab_result")
         return out
@@ -158,6 +165,7 @@ class SlabComm:
     def __init__(self, owner, my_process=0, dist=None):
         self.owner, self.me, self.dist = list(owner), int(my_process), dist
         self.nslabs = len(self.owner)
+        self.graphs = {}          # CUDA graphs of an iteration chunk, per set of ranks (solve_slabs)
         if dist is None and any(o != self.me for o in self.owner):
             raise ValueError("slabs on other processes need torch.distributed")
 
@@ -196,7 +204,7 @@ class SlabComm:
                 req.wait()
 
 
-def solve_slabs(ranks, comm, tol, maxiter, precision="f32", check_every=32):
+def solve_slabs(ranks, comm, tol, maxiter, precision="f32", check_every=32, use_graph=True, device_result=False):
     """Jacobi-PCG on the slabs of this process (`ranks`: {slab index: SlabRank}), in step with the
     other processes through `comm`.  Returns {slab index: dict(phi [nz_local][ny][nx], iters, relres, status)}."""
     ids = sorted(ranks)
@@ -224,9 +232,7 @@ def solve_slabs(ranks, comm, tol, maxiter, precision="f32", check_every=32):
         for s in ids:
             ranks[s].step(5)
 
-    halo()
-    done, l = False, 0
-    while not done:
+    def chunk():
         for _ in range(check_every):
             for s in ids:
                 ranks[s].step(0)                                   # K_spmv; local p.Ap
@@ -237,10 +243,37 @@ def solve_slabs(ranks, comm, tol, maxiter, precision="f32", check_every=32):
             for s in ids:
                 ranks[s].step(2)                                   # beta, stopping rule (same decision everywhere)
             halo()
+
+    halo()
+    # check_every iterations -- kernels, copies and NCCL calls alike -- captured once into a CUDA graph on the ranks'
+    # stream and replayed until the latch is set (kernels after the latch do nothing); eager launches if capture fails
+    # (the graph is kept on the communicator and reused by later solves of the same ranks: the captured kernels and
+    # copies address the handles' own buffers, which stay put until an option or the precision changes)
+    graph = None
+    if use_graph:
+        key = (tuple(id(ranks[s]) for s in ids), tuple(int(ranks[s].views["send"].data_ptr()) for s in ids),
+               str(precision), int(check_every))
+        graph = comm.graphs.get(key)
+        if graph is None:
+            try:
+                torch.cuda.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=torch.cuda.current_stream()):
+                    chunk()
+                comm.graphs[key] = graph
+            except Exception:
+                graph = None
+                torch.cuda.synchronize()
+    done, l = False, 0                                             # (the capture itself executed nothing)
+    while not done:
+        if graph is not None:
+            graph.replay()
+        else:
+            chunk()
         l += check_every
-        done = ranks[ids[0]].latch()["done"] or l > maxiter + check_every
+        done = ranks[ids[0]].latch()["done"] or l > maxiter + 2 * check_every
     out = {}
     for s in ids:
         st = ranks[s].latch()
-        out[s] = dict(phi=ranks[s].result(), iters=st["iters"], relres=st["relres"], status=st["status"])
+        out[s] = dict(phi=ranks[s].result(device=device_result), iters=st["iters"], relres=st["relres"], status=st["status"])
     return out
