@@ -274,7 +274,11 @@ typedef enum {
     PB_OPT_GRAPH = 14,               /* 1 (default): check_every iterations are launched as one CUDA graph           */
     PB_OPT_L2_HINTS = 15,            /* bit mask of L2 eviction-priority hints (default 0: none; measured not to help) */
     PB_OPT_BATCH_WIDTH = 16,         /* right-hand sides per pass of pb_solve_batch: 1, 2 or 4 (default 2)            */
-    PB_OPT_COUNT_ = 17
+    PB_OPT_FUSED = 17,               /* 1 (default): pb_solve / pb_solve_batch run ONE kernel per iteration (k_pcg_fused:
+                                        K_vec folded into the next K_spmv pass, 34 instead of 41 B per node); 0: K_spmv
+                                        + K_vec.  Periodic boundary, warm starts, refinement, slabs and L2-resident
+                                        grids always take their own paths                                              */
+    PB_OPT_COUNT_ = 18
 } pb_option;
 
 pb_status pb_set_option(pb_handle *h, pb_option opt, int value);
@@ -299,7 +303,11 @@ typedef struct {
     int spmv_bytes_per_node;  /* stored-format bytes per node and launch, as pb_bytes_per_node         */
     int vec_bytes_per_node;
     int pitch;                /* padded row length in elements                                         */
-    int reserved[8];
+    int fused;                /* 1: pb_solve runs k_pcg_fused (one kernel per iteration); then txv ... smem_bytes
+                                 describe ITS plan (ring_slots = vector slots), vec_grid = 0                          */
+    int face_quad;            /* fused / batch kernels: faces as 2-bit indices, four nodes per byte                  */
+    int coef_slots;           /* fused / batch kernels: depth of the coefficient ring                                */
+    int reserved[5];
 } pb_plan;
 
 /* pb_prepare -- build the work arrays of `prec` (setup row a0: padded coefficients, diagonal, folded b) and pick

@@ -6,6 +6,7 @@
 #include "pb_kernels.cuh"
 #include "pb_spmv_tma.cuh"
 #include "pb_spmv_batch.cuh"
+#include "pb_fused.cuh"
 #include "pb_persist.cuh"
 #include "pb_setup.cuh"
 #include "pb_grid.cuh"
@@ -26,6 +27,9 @@ template <typename T>
 struct BatchWork {
     int cap = 0;                                   // members the vector arrays hold
     T *r = nullptr, *x = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr, *b = nullptr;
+    T *r2 = nullptr, *Ap2 = nullptr;               // fused iteration (k_pcg_fused): second buffers of r and A p
+    bool fused = false;                            // the plan / maps / graph below are the fused kernel's
+    FusedMaps vm;
     bool coef_ready = false, quad = false, pald = false, own_words = false;
     unsigned char *exq = nullptr, *exqp = nullptr, *eyq = nullptr, *ezq = nullptr, *dviu = nullptr;
     T *exm = nullptr, *eym = nullptr, *ezm = nullptr;   // word format (aliases of Work's arrays unless own_words)
@@ -113,6 +117,7 @@ struct pb_handle {
     double atoms_eps_out, atoms_kappa;
     bool dh_f32 = false;         // pb_set_charges evaluates the Debye-Hueckel boundary terms in fp32
     int last_prec;               // precision of the last pb_solve/pb_solve_begin (for pb_query 3..7)
+    bool last_fused = false;     // the last pb_solve / pb_solve_begin ran k_pcg_fused on the batch work set
 };
 
 namespace {
@@ -155,7 +160,7 @@ void default_options(int *opt)
     opt[PB_OPT_PERSIST_BLOCKS_PER_SM] = 4; opt[PB_OPT_PALETTE] = 1; opt[PB_OPT_PALETTE_DIAG] = 1;
     opt[PB_OPT_PALETTE_DIAG_SPMV] = 1; opt[PB_OPT_AUTOTUNE] = 1; opt[PB_OPT_TILE_TXV] = 0; opt[PB_OPT_TILE_TY] = 0;
     opt[PB_OPT_TILE_TZ] = 0; opt[PB_OPT_RING_SLOTS] = 0; opt[PB_OPT_BLOCKS_PER_SM] = 0; opt[PB_OPT_VEC_BLOCKS_PER_SM] = 0;
-    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_BATCH_WIDTH] = 2;
+    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_BATCH_WIDTH] = 2; opt[PB_OPT_FUSED] = 1;
 }
 
 inline int grid_for(size_t n, int block, int cap)
@@ -177,7 +182,7 @@ pb_status alloc_arr(T **p, size_t n)
 template <typename T>
 void free_batch(BatchWork<T> &b)
 {
-    T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b};
+    T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b, &b.r2, &b.Ap2};
     for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
     unsigned char **idx[] = {&b.exq, &b.exqp, &b.eyq, &b.ezq, &b.dviu};
     for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
@@ -822,10 +827,62 @@ pb_status ensure_stage(pb_handle *h, size_t bytes)
     return PB_OK;
 }
 
+// pb_solve takes the one-kernel-per-iteration path unless the problem needs a special one
+template <typename T>
+bool fused_eligible(pb_handle *h)
+{
+    if (!h->opt[PB_OPT_FUSED] || h->periodic || h->slab) return false;
+    if (ensure<T>(h) != PB_OK) return false;
+    return !work<T>(h).persist;
+}
+
+struct DevTmp {                      // frees its device allocations on scope exit
+    void *p[12]; int n = 0;
+    ~DevTmp() { for (int i = 0; i < n; i++) if (p[i]) cudaFree(p[i]); }
+    pb_status get(void **out, size_t bytes) {
+        *out = nullptr;
+        PB_ALLOC(cudaMalloc(out, bytes ? bytes : 8));
+        p[n++] = *out;
+        return PB_OK;
+    }
+    void release(void *q) { for (int i = 0; i < n; i++) if (p[i] == q) p[i] = nullptr; }
+};
+
+pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
+                            double eps_out, double kappa, double *d_rhs, double *d_bc, double *scratch, int nsm,
+                            cudaStream_t st, bool dh_f32 = false);
+pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_memspace where);
+
+#include "pb_api_batch.cuh"
+
+// pb_solve_begin: steps 1-2 without a latch, on the path pb_solve would take
+template <typename T>
+pb_status begin_any(pb_handle *h)
+{
+    h->last_fused = false;
+    if (fused_eligible<T>(h)) {
+        PB_TRY(ensure_batch<T>(h, 1, true));
+        PB_TRY(init_batch<T>(h, 1, 1.0, 0, 0, work<T>(h).b));
+        h->last_fused = true;
+        return PB_OK;
+    }
+    return begin_solve<T>(h, 1.0, 0, 0);
+}
+
 // steps 1-8 until the device latch is set (converged, maxiter or breakdown); the iterate stays on the device
 template <typename T>
-pb_status run_solve(pb_handle *h, double tol, int maxiter, int check_every, const void *phi0, pb_memspace where)
+pb_status run_solve(pb_handle *h, double tol, int maxiter, int check_every, const void *phi0, pb_memspace where,
+                    bool allow_fused = true)
 {
+    h->last_fused = false;
+    if (allow_fused && !phi0 && fused_eligible<T>(h)) {
+        // one kernel per iteration (k_pcg_fused) on the batch work set, right-hand side = this handle's b
+        Work<T> &wq = work<T>(h);
+        PB_TRY(ensure_batch<T>(h, 1, true));
+        PB_TRY(run_batch<T>(h, 1, tol, maxiter, check_every, wq.b));
+        h->last_fused = true;
+        return PB_OK;
+    }
     PB_TRY(begin_solve<T>(h, tol, maxiter, 1, phi0, where));
     Work<T> &w = work<T>(h);
     const int m = check_every;
@@ -875,7 +932,10 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
     T *dst = (T *)phi_out;
     if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(T))); dst = (T *)h->stage; }
-    k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.x, w.p0, w.p1, h->st, dst, h->nx, w.P, rows);
+    if (h->last_fused)
+        k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.bw.x, w.bw.p0, w.bw.p1, h->st, dst, h->nx, w.P, rows);
+    else
+        k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.x, w.p0, w.p1, h->st, dst, h->nx, w.P, rows);
     PB_CUDA(cudaGetLastError());
     h->launches += 1;
     if (where == PB_HOST)
@@ -930,7 +990,7 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
                                                                                            h->nx, rows);
         h->launches += 1;
         wf.b_ready = true;
-        const pb_status rs = run_solve<float>(h, tin, maxiter - total, check_every, nullptr, PB_DEVICE);
+        const pb_status rs = run_solve<float>(h, tin, maxiter - total, check_every, nullptr, PB_DEVICE, false);
         wf.b_ready = false;                      // wf.b holds a residual, not b: rebuilt before the next plain solve
         if (rs != PB_OK) return rs;
         k_finish_add<float, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
@@ -957,24 +1017,6 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
     return status;
 }
 
-struct DevTmp {                      // frees its device allocations on scope exit
-    void *p[12]; int n = 0;
-    ~DevTmp() { for (int i = 0; i < n; i++) if (p[i]) cudaFree(p[i]); }
-    pb_status get(void **out, size_t bytes) {
-        *out = nullptr;
-        PB_ALLOC(cudaMalloc(out, bytes ? bytes : 8));
-        p[n++] = *out;
-        return PB_OK;
-    }
-    void release(void *q) { for (int i = 0; i < n; i++) if (p[i] == q) p[i] = nullptr; }
-};
-
-pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, int nx, int ny, int nz, double hh,
-                            double eps_out, double kappa, double *d_rhs, double *d_bc, double *scratch, int nsm,
-                            cudaStream_t st, bool dh_f32 = false);
-pb_status take_copy(pb_handle *h, double **dst, const double *src, size_t n, pb_memspace where);
-
-#include "pb_api_batch.cuh"
 
 // ---- NEXT row f4: one solve over several GPUs, z-slab decomposition -------------------------
 // The library provides the per-rank pieces; the ranks' exchange (halo planes, scalar all-reduces) is the caller's --
@@ -1070,8 +1112,15 @@ template <typename T>
 int bytes_per_node_impl(pb_handle *h, int kernel)
 {
     if (ensure<T>(h) != PB_OK) return -1;
-    const Work<T> &w = work<T>(h);
+    Work<T> &w = work<T>(h);
     const int e = (int)sizeof(T);
+    if (fused_eligible<T>(h)) {
+        // k_pcg_fused: r, A p, p, x in; r, p, x, A p out (8 words); Dinv; the three faces (quad: ex twice, 4 x 2 bits)
+        if (kernel == 1) return 0;
+        if (ensure_batch<T>(h, 1, true) != PB_OK) return -1;
+        const BatchWork<T> &b = w.bw;
+        return 8 * e + (b.pald ? 1 : e) + (b.quad ? 1 : 3 * e);
+    }
     if (kernel == 0)      // r, p_old, x in; p, x, Ap out; Dinv; three face coefficients
         return 6 * e + (w.pald_s ? 1 : e) + (w.pal ? 3 : 3 * e);
     return 3 * e + (w.pald ? 1 : e);      // r, Ap in; r out; Dinv
@@ -1138,6 +1187,23 @@ pb_status profile_impl(pb_handle *h, int n_iter, double *ms_spmv, double *ms_vec
         for (int i = 0; i < ne; i++) PB_CUDA(cudaEventCreate(&ev[i]));
         const VecArgs<T> va = vec_args<T>(h, w);
         PB_CUDA(cudaEventRecord(ev[0], h->stream));
+        if (h->last_fused) {
+            // one kernel per iteration: its time is reported as "spmv", "vec" is 0
+            for (int it = 0; it < n_iter; it++) {
+                PB_TRY(enqueue_batch_iterations<T>(h, w, 1));
+                PB_CUDA(cudaEventRecord(ev[it + 1], h->stream));
+            }
+            PB_CUDA(cudaStreamSynchronize(h->stream));
+            double a = 0.0;
+            for (int it = 0; it < n_iter; it++) {
+                float t1 = 0.f;
+                PB_CUDA(cudaEventElapsedTime(&t1, ev[it], ev[it + 1]));
+                a += t1;
+            }
+            if (ms_spmv) *ms_spmv = a / n_iter;
+            if (ms_vec) *ms_vec = 0.0;
+            return PB_OK;
+        }
         for (int it = 0; it < n_iter; it++) {
             launch_spmv<T, 0>(h, w, 1.0);
             launch_wrap<T, 0>(h, w, 1.0);
@@ -1363,7 +1429,7 @@ pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
     if (!h || (int)opt < 0 || (int)opt >= (int)PB_OPT_COUNT_ || value < 0) return PB_ERR_INVALID_ARG;
     switch (opt) {
     case PB_OPT_PERSIST: case PB_OPT_PALETTE: case PB_OPT_PALETTE_DIAG: case PB_OPT_PALETTE_DIAG_SPMV:
-    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH:
+    case PB_OPT_AUTOTUNE: case PB_OPT_GRAPH: case PB_OPT_FUSED:
         if (value > 1) return PB_ERR_INVALID_ARG;
         break;
     case PB_OPT_PERSIST_BLOCKS_PER_SM:
@@ -1426,7 +1492,18 @@ pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
         out->vec_grid = w.vec_grid; out->vec_threads = 256; out->pitch = w.P;
     };
     if (prec == PB_F32) fill(h->wf); else fill(h->wd);
-    out->spmv_bytes_per_node = pb_bytes_per_node(h, prec, 0);
+    out->spmv_bytes_per_node = pb_bytes_per_node(h, prec, 0);      // (builds the fused plan when pb_solve takes that path)
+    auto fill_fused = [&](const auto &w) {
+        const auto &b = w.bw;
+        if (!(b.fused && b.M == 1)) return;
+        out->fused = 1;
+        out->txv = b.TXV; out->ty = b.TY; out->tz = b.TZ; out->ring_slots = b.nsv; out->blocks_per_sm = b.bps;
+        out->tiles = b.ntx * b.nty * b.ntz; out->grid = b.grid; out->threads = b.threads; out->smem_bytes = (int)b.smem;
+        out->autotuned = 0; out->vec_grid = 0; out->vec_threads = 0;
+        out->face_quad = b.quad; out->coef_slots = b.nsc;
+    };
+    const bool fz = prec == PB_F32 ? fused_eligible<float>(h) : fused_eligible<double>(h);
+    if (fz) { if (prec == PB_F32) fill_fused(h->wf); else fill_fused(h->wd); }
     out->vec_bytes_per_node = pb_bytes_per_node(h, prec, 1);
     return PB_OK;
 }
@@ -1550,7 +1627,7 @@ pb_status pb_solve_begin(pb_handle *h, pb_precision prec)
     if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !valid_prec(prec)) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
-    return prec == PB_F32 ? begin_solve<float>(h, 1.0, 0, 0) : begin_solve<double>(h, 1.0, 0, 0);
+    return prec == PB_F32 ? begin_any<float>(h) : begin_any<double>(h);
 }
 
 pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
@@ -1558,9 +1635,12 @@ pb_status pb_iterate(pb_handle *h, pb_precision prec, int n_iter)
     if (h && h->slab) return PB_ERR_INVALID_ARG;      // a z-slab rank is driven through pb_slab_* only
     if (!h || !valid_prec(prec) || n_iter < 0) return PB_ERR_INVALID_ARG;
     PB_CUDA(cudaSetDevice(h->device));
-    if (prec == PB_F32) { if (!h->wf.ready) return PB_ERR_INVALID_ARG; return enqueue_iterations<float>(h, h->wf, n_iter); }
+    if (prec == PB_F32) {
+        if (!h->wf.ready) return PB_ERR_INVALID_ARG;
+        return h->last_fused ? enqueue_batch_iterations<float>(h, h->wf, n_iter) : enqueue_iterations<float>(h, h->wf, n_iter);
+    }
     if (!h->wd.ready) return PB_ERR_INVALID_ARG;
-    return enqueue_iterations<double>(h, h->wd, n_iter);
+    return h->last_fused ? enqueue_batch_iterations<double>(h, h->wd, n_iter) : enqueue_iterations<double>(h, h->wd, n_iter);
 }
 
 pb_status pb_profile(pb_handle *h, pb_precision prec, int n_iter, double *ms_spmv, double *ms_vec)

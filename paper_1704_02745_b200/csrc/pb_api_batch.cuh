@@ -38,9 +38,27 @@ pb_status batch_kernel_attr_fmt(bool quad, bool pald, size_t *max_dyn)
     return pald ? batch_kernel_attr<T, false, true, M>(max_dyn) : batch_kernel_attr<T, false, false, M>(max_dyn);
 }
 
-// coefficient arrays, vectors, plan and tensor maps of the batch path for M members
+template <typename T, bool QUAD, bool PALD, int M>
+pb_status fused_kernel_attr(size_t *max_dyn)
+{
+    cudaFuncAttributes fa;
+    PB_CUDA(cudaFuncGetAttributes(&fa, k_pcg_fused<T, QUAD, PALD, M>));
+    const size_t lim = (size_t)232448 - fa.sharedSizeBytes;
+    PB_CUDA(cudaFuncSetAttribute(k_pcg_fused<T, QUAD, PALD, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim));
+    *max_dyn = lim;
+    return PB_OK;
+}
+template <typename T, int M>
+pb_status fused_kernel_attr_fmt(bool quad, bool pald, size_t *max_dyn)
+{
+    if (quad) return pald ? fused_kernel_attr<T, true, true, M>(max_dyn) : fused_kernel_attr<T, true, false, M>(max_dyn);
+    return pald ? fused_kernel_attr<T, false, true, M>(max_dyn) : fused_kernel_attr<T, false, false, M>(max_dyn);
+}
+
+// coefficient arrays, vectors, plan and tensor maps of the batch path for M members; `fused`: of k_pcg_fused (one
+// kernel per iteration, M = 1 or 2) instead of k_spmv_batch + k_vec_batch
 template <typename T>
-pb_status ensure_batch(pb_handle *h, int M)
+pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
 {
     constexpr int VEC = VecN<T>::value;
     PB_TRY(ensure<T>(h));
@@ -88,21 +106,26 @@ pb_status ensure_batch(pb_handle *h, int M)
         b.coef_ready = true;
     }
     if (b.cap < M) {
-        T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b};
+        T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b, &b.r2, &b.Ap2};
         for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
         b.cap = 0; b.M = 0;
         for (T **a : arrs)
             if ((s = alloc_arr(a, (size_t)M * w.npad))) { free_batch(b); return s; }
         b.cap = M;
     }
-    if (b.M == M) return PB_OK;
+    if (b.M == M && b.fused == fused) return PB_OK;
     if (b.graph) { cudaGraphExecDestroy(b.graph); b.graph = nullptr; }
     // plan: rows of about 1 KB like k_spmv_tma, four rows, two blocks per SM (one for M = 4: its registers), rings as
     // deep as the shared memory allows
     size_t max_dyn = 0;
-    if (M == 1) PB_TRY((batch_kernel_attr_fmt<T, 1>(b.quad, b.pald, &max_dyn)));
+    if (fused) {
+        if (M == 1) PB_TRY((fused_kernel_attr_fmt<T, 1>(b.quad, b.pald, &max_dyn)));
+        else if (M == 2) PB_TRY((fused_kernel_attr_fmt<T, 2>(b.quad, b.pald, &max_dyn)));
+        else return PB_ERR_INVALID_ARG;
+    } else if (M == 1) PB_TRY((batch_kernel_attr_fmt<T, 1>(b.quad, b.pald, &max_dyn)));
     else if (M == 2) PB_TRY((batch_kernel_attr_fmt<T, 2>(b.quad, b.pald, &max_dyn)));
     else PB_TRY((batch_kernel_attr_fmt<T, 4>(b.quad, b.pald, &max_dyn)));
+    const int max_threads = fused ? (M >= 2 ? 256 : 512) : (M >= 4 ? 256 : 512);      // the kernels' launch bounds
     const int rowvecs = w.P / VEC;
     const int maxv = ((b.pald || b.quad) ? 240 : 256) / VEC - 2;
     int ntx0 = (rowvecs + 32) / 64;
@@ -114,28 +137,30 @@ pb_status ensure_batch(pb_handle *h, int M)
     if (b.TXV > rowvecs) b.TXV = rowvecs;
     b.TY = o[PB_OPT_TILE_TY] > 0 ? o[PB_OPT_TILE_TY] : 4;
     if (b.TY > h->ny) b.TY = h->ny;
-    const int max_ct = (M >= 4 ? 256 : 512) - 64;
+    const int max_ct = max_threads - 64;
     while (spmv_row_threads(b.TXV) * b.TY > max_ct && b.TY > 1) b.TY--;
     b.threads = (spmv_row_threads(b.TXV) * b.TY + 31) / 32 * 32 + 32;
-    const BatchLayout L = batch_layout(b.TXV, b.TY, VEC, b.quad, b.pald);
+    const FusedLayout FL = fused_layout(b.TXV, b.TY, VEC, b.quad, b.pald);
+    const BatchLayout &L = FL.B;
+    const long vslot = fused ? (long)FL.vslot : (long)L.vslot;
     // blocks per SM / coefficient ring depth: the first combination that leaves the vector ring M + 2 slots (the
     // consumers work on one member's plane while M more are in flight), else the one with the deepest vector ring
     const int forced_bps = o[PB_OPT_BLOCKS_PER_SM];
-    const int try_bps[3] = {M >= 4 ? 1 : 2, 1, 1}, try_nsc[3] = {4, 4, 3};
+    const int try_bps[3] = {max_threads == 256 ? 1 : 2, 1, 1}, try_nsc[3] = {4, 4, 3};
     b.nsv = 0;
     for (int t = 0; t < 3; t++) {
         const int bps = forced_bps > 0 ? forced_bps : try_bps[t], nsc = try_nsc[t];
         const long fixed = (long)nsc * (long)L.cslot + 2L * M * (long)L.pn + 128;
         long budget = (long)((size_t)232448 / bps) - 1024 - (long)((size_t)232448 - max_dyn) - fixed;   // per-SM share
         if ((long)max_dyn - fixed < budget) budget = (long)max_dyn - fixed;                              // per-block cap
-        int nsv = budget > 0 ? (int)(budget / (long)L.vslot) : 0;
+        int nsv = budget > 0 ? (int)(budget / vslot) : 0;
         if (nsv > kMaxStages) nsv = kMaxStages;
         if (nsv > b.nsv) { b.nsv = nsv; b.nsc = nsc; b.bps = bps; }
         if (b.nsv >= M + 2) break;
     }
     if (o[PB_OPT_RING_SLOTS] > 0 && o[PB_OPT_RING_SLOTS] < b.nsv) b.nsv = o[PB_OPT_RING_SLOTS];
     if (b.nsv < 2) return PB_ERR_INVALID_ARG;
-    b.smem = batch_smem(L, b.nsv, b.nsc, M);
+    b.smem = fused ? fused_smem(FL, b.nsv, b.nsc, M) : batch_smem(L, b.nsv, b.nsc, M);
     b.ntx = (rowvecs + b.TXV - 1) / b.TXV;
     b.nty = (h->ny + b.TY - 1) / b.TY;
     const int slots = h->nsm * b.bps, xy = b.ntx * b.nty;
@@ -146,6 +171,7 @@ pb_status ensure_batch(pb_handle *h, int M)
     b.grid = (int)(ntiles < slots ? ntiles : slots);
     b.vec_grid = grid_for(w.npad / VEC, 256, h->nsm * 8);
     size_t need = (size_t)M * b.grid > (size_t)2 * M * b.vec_grid ? (size_t)M * b.grid : (size_t)2 * M * b.vec_grid;
+    if ((size_t)M * kFusedSums * b.grid > need) need = (size_t)M * kFusedSums * b.grid;
     if (need > h->partials_cap) {
         PB_CUDA(cudaStreamSynchronize(h->stream));
         if (h->partials) cudaFree(h->partials);
@@ -164,6 +190,12 @@ pb_status ensure_batch(pb_handle *h, int M)
     PB_TRY(make_map4<T>(&b.tm_p0, b.p0, w.P, h->ny, h->nz, M, hx, hy));
     PB_TRY(make_map4<T>(&b.tm_p1, b.p1, w.P, h->ny, h->nz, M, hx, hy));
     PB_TRY(make_map4<T>(&b.tm_x, b.x, w.P, h->ny, h->nz, M, b.TXV * VEC, b.TY));
+    if (fused) {
+        b.vm.r0 = b.tm_r; b.vm.p0 = b.tm_p0; b.vm.p1 = b.tm_p1;
+        PB_TRY(make_map4<T>(&b.vm.r1, b.r2, w.P, h->ny, h->nz, M, hx, hy));
+        PB_TRY(make_map4<T>(&b.vm.q0, b.Ap, w.P, h->ny, h->nz, M, hx, hy));
+        PB_TRY(make_map4<T>(&b.vm.q1, b.Ap2, w.P, h->ny, h->nz, M, hx, hy));
+    }
     if (b.pald) PB_TRY(make_map_u8(&b.tm_dinv, b.dviu, w.Pb, h->ny, h->nz, L.bwd, hy));
     else PB_TRY(make_map<T>(&b.tm_dinv, w.Dinv, w.P, h->ny, h->nz, hx, hy));
     if (b.quad) {
@@ -178,9 +210,10 @@ pb_status ensure_batch(pb_handle *h, int M)
         PB_TRY(make_map<T>(&b.tm_ez, b.ezm, w.P, h->ny, h->nz + 1, b.TXV * VEC, b.TY));
     }
     b.M = M;
+    b.fused = fused;
     if (verbose())
-        fprintf(stderr, "pb: batch plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%ld grid=%d threads=%d smem=%zu\n",
-                sizeof(T) == 4 ? "f32" : "f64", M, b.quad ? "quad" : "words", b.pald ? "+diag palette" : "", b.TXV, b.TY, b.TZ,
+        fprintf(stderr, "pb: %s plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%ld grid=%d threads=%d smem=%zu\n",
+                fused ? "fused" : "batch", sizeof(T) == 4 ? "f32" : "f64", M, b.quad ? "quad" : "words", b.pald ? "+diag palette" : "", b.TXV, b.TY, b.TZ,
                 b.nsv, b.nsc, b.bps, ntiles, b.grid, b.threads, b.smem);
     return PB_OK;
 }
@@ -205,10 +238,34 @@ void launch_batch_kernels(pb_handle *h, Work<T> &w, int n_iter)
     }
 }
 
+template <typename T, bool QUAD, bool PALD, int M>
+void launch_fused_kernels(pb_handle *h, Work<T> &w, int n_iter)
+{
+    BatchWork<T> &b = w.bw;
+    FusedArgs<T> a;
+    a.r0 = b.r; a.r1 = b.r2; a.Ap0 = b.Ap; a.Ap1 = b.Ap2; a.p0 = b.p0; a.p1 = b.p1; a.x = b.x; a.npad = w.npad;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
+    a.TXV = b.TXV; a.TY = b.TY; a.TZ = b.TZ; a.ntx = b.ntx; a.nty = b.nty; a.ntz = b.ntz;
+    a.ntiles = b.ntx * b.nty * b.ntz; a.nsv = b.nsv; a.nsc = b.nsc; a.precond = h->precond;
+    a.st = h->st; a.partials = h->partials; a.lut = w.lut; a.dlut = w.dlut;
+    for (int it = 0; it < n_iter; it++)
+        k_pcg_fused<T, QUAD, PALD, M><<<b.grid, b.threads, b.smem, h->stream>>>(b.vm, b.tm_dinv, b.tm_x, b.tm_exm, b.tm_exp,
+                                                                              b.tm_ey, b.tm_ez, a);
+}
+
 template <typename T>
 pb_status enqueue_batch_iterations(pb_handle *h, Work<T> &w, int n_iter)
 {
     const BatchWork<T> &b = w.bw;
+    if (b.fused) {
+#define PB_FUSED_M(Q, D) do { if (b.M == 1) launch_fused_kernels<T, Q, D, 1>(h, w, n_iter); else launch_fused_kernels<T, Q, D, 2>(h, w, n_iter); } while (0)
+        if (b.quad) { if (b.pald) PB_FUSED_M(true, true); else PB_FUSED_M(true, false); }
+        else { if (b.pald) PB_FUSED_M(false, true); else PB_FUSED_M(false, false); }
+#undef PB_FUSED_M
+        PB_CUDA(cudaGetLastError());
+        h->launches += (long long)n_iter;
+        return PB_OK;
+    }
 #define PB_BATCH_CASE(Q, D, MM) launch_batch_kernels<T, Q, D, MM>(h, w, n_iter)
 #define PB_BATCH_M(Q, D) do { if (b.M == 1) PB_BATCH_CASE(Q, D, 1); else if (b.M == 2) PB_BATCH_CASE(Q, D, 2); else PB_BATCH_CASE(Q, D, 4); } while (0)
     if (b.quad) { if (b.pald) PB_BATCH_M(true, true); else PB_BATCH_M(true, false); }
@@ -221,22 +278,36 @@ pb_status enqueue_batch_iterations(pb_handle *h, Work<T> &w, int n_iter)
 }
 
 // M members: steps 1-8 until every member's latch is set; member s's right-hand side b is in w.bw.b + s*npad
+// steps 1-2 of every member (x = 0, r = b, p cleared, ||b||^2, the l = 0 test); `single_b`: the one right-hand side
+// of pb_solve (w.b) instead of the members' own (w.bw.b)
 template <typename T>
-pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_every)
+pb_status init_batch(pb_handle *h, int M, double tol, int maxiter, int latch, const T *single_b)
 {
     Work<T> &w = work<T>(h);
     BatchWork<T> &b = w.bw;
     h->last_prec = sizeof(T) == 4 ? PB_F32 : PB_F64;
+    if (b.fused) PB_CUDA(cudaMemsetAsync(b.Ap, 0, (size_t)M * w.npad * sizeof(T), h->stream));   // "A p_0" = 0: r_0 = b
     for (int s = 0; s < M; s++) {
-        k_set_state<<<1, 1, 0, h->stream>>>(h->st + s, tol * tol, maxiter, 1);
+        k_set_state<<<1, 1, 0, h->stream>>>(h->st + s, tol * tol, maxiter, latch);
         VecArgs<T> va = vec_args<T>(h, w);
-        va.r = b.r + s * w.npad; va.b = b.b + s * w.npad; va.x = b.x + s * w.npad; va.pzero = b.p0 + s * w.npad;
+        va.r = b.r + s * w.npad; va.b = single_b ? single_b : b.b + s * w.npad; va.x = b.x + s * w.npad;
+        va.pzero = b.p0 + s * w.npad;
         va.st = h->st + s;
         k_init<T><<<w.vec_grid, 256, 0, h->stream>>>(va);
     }
     PB_CUDA(cudaGetLastError());
     h->launches += 2LL * M;
+    return PB_OK;
+}
+
+template <typename T>
+pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_every, const T *single_b = nullptr)
+{
+    Work<T> &w = work<T>(h);
+    BatchWork<T> &b = w.bw;
+    PB_TRY(init_batch<T>(h, M, tol, maxiter, 1, single_b));
     const int m = check_every;
+    const long long per_iter = b.fused ? 1 : 2;
     bool graph_ok = false;
     if (h->opt[PB_OPT_GRAPH]) {
         if (!(b.graph && b.graph_iters == m)) {
@@ -244,7 +315,7 @@ pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_ever
             cudaGraph_t g = nullptr;
             PB_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
             const pb_status cs = enqueue_batch_iterations<T>(h, w, m);
-            h->launches -= 2LL * m;
+            h->launches -= per_iter * m;
             const cudaError_t e = cudaStreamEndCapture(h->stream, &g);
             if (cs == PB_OK && e == cudaSuccess && g && cudaGraphInstantiate(&b.graph, g, 0) == cudaSuccess) b.graph_iters = m;
             else { b.graph = nullptr; cudaGetLastError(); }
@@ -255,7 +326,7 @@ pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_ever
     const long max_chunks = (long)maxiter / m + 2;
     bool all_done = false;
     for (long c = 0; c < max_chunks + 1 && !all_done; c++) {
-        if (graph_ok) { PB_CUDA(cudaGraphLaunch(b.graph, h->stream)); h->launches += 2LL * m; }
+        if (graph_ok) { PB_CUDA(cudaGraphLaunch(b.graph, h->stream)); h->launches += per_iter * m; }
         else PB_TRY(enqueue_batch_iterations<T>(h, w, m));
         State *slot = h->pinned_state + kMaxBatch * (c & 1);
         PB_CUDA(cudaMemcpyAsync(slot, h->st, M * sizeof(State), cudaMemcpyDeviceToHost, h->stream));
@@ -306,7 +377,7 @@ pb_status solve_batch_impl(pb_handle *h, int m, const double *rhs, const double 
     for (int g0 = 0; g0 < m;) {
         int M = width;
         while (M > m - g0) M >>= 1;
-        PB_TRY(ensure_batch<T>(h, M));
+        PB_TRY(ensure_batch<T>(h, M, h->opt[PB_OPT_FUSED] != 0 && M <= 2));
         for (int s = 0; s < M; s++) {
             const int mem = g0 + s;
             if (charges) {

@@ -113,12 +113,20 @@ def test_spmv_device_pointers(pkg, pbref, cuda_device):
     ref.close()
 
 
-def check_solve(pkg, pbref, inp, prec, tol, maxiter=20000, check_every=16):
+# the three ways pb_solve can run an iteration: the default choice (cooperative kernel on L2-resident grids, else
+# k_pcg_fused), one fused kernel per iteration forced (persist = 0), K_spmv + K_vec forced (persist = 0, fused = 0)
+PATHS = {"default": None, "fused": dict(persist=0), "two-kernel": dict(persist=0, fused=0)}
+
+
+def check_solve(pkg, pbref, inp, prec, tol, maxiter=20000, check_every=16, options=None):
     ref = pbref.from_inputs(inp)
     o = ref.solve(tol, maxiter)
     o_tight = ref.solve(1e-10, maxiter) if tol > 1e-10 else o
-    with pkg.PBSolver(*inp.args()) as s:
+    with pkg.PBSolver(*inp.args(), options=options) as s:
         g = s.solve(tol, maxiter, prec, check_every=check_every)
+        if options is not None:
+            pl = s.plan(prec)
+            assert pl["persist"] == 0 and pl["fused"] == options.get("fused", 1), pl
     ref.close()
     scale = np.max(np.abs(o_tight["phi"]))
     lim = 1e-8 if prec == "f64" and tol <= 1e-10 else 1e-4
@@ -131,14 +139,16 @@ def check_solve(pkg, pbref, inp, prec, tol, maxiter=20000, check_every=16):
     return g, o
 
 
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("shape", [(5, 4, 3), (13, 9, 7), (33, 31, 29), (130, 21, 37)])
-def test_solve_fp64_random(pkg, pbref, shape):
-    check_solve(pkg, pbref, random_operator(*shape, seed=11), "f64", 1e-10)
+def test_solve_fp64_random(pkg, pbref, shape, path):
+    check_solve(pkg, pbref, random_operator(*shape, seed=11, two_valued=(shape[0] != 130)), "f64", 1e-10, options=PATHS[path])
 
 
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("shape", [(13, 9, 7), (33, 31, 29), (130, 21, 37)])
-def test_solve_fp32_random(pkg, pbref, shape):
-    check_solve(pkg, pbref, random_operator(*shape, seed=12), "f32", 1e-5)
+def test_solve_fp32_random(pkg, pbref, shape, path):
+    check_solve(pkg, pbref, random_operator(*shape, seed=12, two_valued=(shape[0] != 130)), "f32", 1e-5, options=PATHS[path])
 
 
 def test_solve_born_config1(pkg, pbref):
@@ -156,9 +166,10 @@ def test_solve_born_config1(pkg, pbref):
     assert abs(rf - (-0.49375)) <= 0.05 * 0.49375
 
 
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
-def test_solve_config2_65(pkg, pbref, prec, tol):
-    check_solve(pkg, pbref, make_config(2), prec, tol)
+def test_solve_config2_65(pkg, pbref, prec, tol, path):
+    check_solve(pkg, pbref, make_config(2), prec, tol, options=PATHS[path])
 
 
 @pytest.mark.slow
@@ -271,7 +282,7 @@ def test_tiling_independence(pkg, pbref, prec):
     y0 = None
     for cfg in TILE_CONFIGS:
         # small grid: persist=0 forces the two-kernel TMA path under test
-        with pkg.PBSolver(*inp.args(), options=dict(cfg, persist=0)) as s:
+        with pkg.PBSolver(*inp.args(), options=dict(cfg, persist=0, fused=0)) as s:
             y = s.apply(x, prec)
             runs = [s.solve(tol, 5000, prec, check_every=9) for _ in range(2)]
             plan = s.plan(prec)
@@ -299,7 +310,7 @@ def test_tiling_independence_with_both_palettes(pkg, prec):
     ref_y = ref_p = ref_ap = None
     for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette=0)):
         for cfg in TILE_CONFIGS:
-            with pkg.PBSolver(*inp.args(), options={**cfg, **fmt, "persist": 0}) as s:
+            with pkg.PBSolver(*inp.args(), options={**cfg, **fmt, "persist": 0, "fused": 0}) as s:
                 y = s.apply(x, prec)
                 if not fmt:
                     assert s.palette_size() > 0 and s.diag_palette_size() > 0
@@ -513,7 +524,7 @@ def test_diagonal_palette_is_exact(pkg, prec, tol):
     inp = make_config(2)
     # persist=0: the two-kernel path is the one that uses k_vec; autotune=0: the same static plan in both runs,
     # hence the same reduction order
-    with pkg.PBSolver(*inp.args(), options=dict(persist=0, autotune=0)) as s:
+    with pkg.PBSolver(*inp.args(), options=dict(persist=0, autotune=0, fused=0)) as s:
         a = s.solve(tol, 5000, prec)
         assert 0 < s.diag_palette_size() <= 56 and s.plan(prec)["diag_palette_vec"] == 1
         s.set_option("palette_diag", 0)
@@ -773,8 +784,8 @@ def test_options_are_handle_state(pkg):
     """pb_set_option / pb_get_option / pb_get_plan: two handles in one process configured differently, invalid values
     rejected, the plan reports what runs."""
     inp = make_config(2)
-    with pkg.PBSolver(*inp.args(), options=dict(persist=0, palette=0, autotune=0)) as a, \
-            pkg.PBSolver(*inp.args()) as b:
+    with pkg.PBSolver(*inp.args(), options=dict(persist=0, palette=0, autotune=0, fused=0)) as a, \
+            pkg.PBSolver(*inp.args(), options=dict(fused=0)) as b:
         pa, pb_ = a.plan("f32"), b.plan("f32")
         assert pa["persist"] == 0 and pa["face_palette"] == 0 and pa["palette_size"] == 0 and not pa["autotuned"]
         assert pa["spmv_bytes_per_node"] == 40 and pa["vec_bytes_per_node"] == 16
@@ -787,6 +798,14 @@ def test_options_are_handle_state(pkg):
         for name, val in (("ring_slots", 2), ("ring_slots", 9), ("persist", 2), ("palette", -1), ("blocks_per_sm", 33)):
             with pytest.raises(pkg.PBError):
                 a.set_option(name, val)
+        # the fused iteration (the default off the L2-resident path): one kernel, 8 words + 2 index bytes per node
+        a.set_option("fused", 1)
+        a.set_option("palette", 1)
+        pf = a.plan("f32")
+        assert pf["fused"] == 1 and pf["face_quad"] == 1 and pf["spmv_bytes_per_node"] == 34 and pf["vec_bytes_per_node"] == 0
+        assert abs(a.solve(1e-5, 5000, "f32")["iters"] - gb["iters"]) <= 1
+        a.set_option("fused", 0)
+        a.set_option("palette", 0)
         # a forced tile larger than the grid / the thread budget is clamped, and the plan says what really runs
         a.set_option("tile_ty", 400)
         a.set_option("tile_txv", 60)
@@ -941,3 +960,37 @@ def test_config5_batch_members_multi_rhs_full_size(pkg, pbref):
         assert abs(g["iters"][i] - o["iters"]) <= round(0.05 * o["iters"])
         assert err <= 1e-4
     ref.close()
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_fused_iteration_tilings_and_formats(pkg, pbref, prec, tol):
+    """k_pcg_fused (one kernel per iteration: the residual update deferred into the next pass, every scalar from one
+    reduction with exactly re-summed norms) under forced tiles / rings / grids and in both coefficient formats (2-bit
+    quads, words; Dinv bytes or words): same iteration count as the oracle within 5 % and as the two-kernel path within
+    one, potentials within the north-star bars, bitwise repeatable; maxiter and the l = 0 cases latch identically."""
+    inp = random_operator(77, 45, 38, seed=21)
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(tol, 5000)
+    o9 = ref.solve(tol, 9)
+    ref.close()
+    scale = np.max(np.abs(o["phi"]))
+    lim = 1e-8 if prec == "f64" else 1e-4
+    with pkg.PBSolver(*inp.args(), options=dict(persist=0, fused=0)) as s:
+        two = s.solve(tol, 5000, prec)
+    cfgs = [dict(), dict(tile_txv=7, tile_ty=3, ring_slots=3, blocks_per_sm=2, tile_tz=5),
+            dict(tile_txv=20, tile_ty=8, blocks_per_sm=1, tile_tz=99), dict(tile_txv=5, tile_ty=2, blocks_per_sm=4, tile_tz=1),
+            dict(tile_txv=13, tile_ty=5, ring_slots=4, blocks_per_sm=3, tile_tz=33)]
+    for fmt in (dict(), dict(palette_diag_spmv=0), dict(palette=0)):
+        for cfg in cfgs:
+            with pkg.PBSolver(*inp.args(), options={**cfg, **fmt, "persist": 0}) as s:
+                runs = [s.solve(tol, 5000, prec, check_every=ce) for ce in (9, 64)]
+                short = s.solve(tol, 9, prec, check_every=4)
+                pl = s.plan(prec)
+            assert pl["fused"] == 1 and pl["face_quad"] == (0 if fmt == dict(palette=0) else 1), (fmt, cfg, pl)
+            assert np.array_equal(runs[0]["phi"], runs[1]["phi"]) and runs[0]["iters"] == runs[1]["iters"], (fmt, cfg)
+            assert runs[0]["status"] == 0 and runs[0]["relres"] < tol
+            assert abs(runs[0]["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (fmt, cfg, runs[0]["iters"], o["iters"])
+            assert abs(runs[0]["iters"] - two["iters"]) <= 1, (fmt, cfg)
+            assert np.max(np.abs(runs[0]["phi"] - o["phi"])) <= lim * scale, (fmt, cfg)
+            assert short["status"] == pkg.binding.PB_ERR_MAXITER and short["iters"] == 9
+            assert np.max(np.abs(short["phi"] - o9["phi"])) <= lim * scale, (fmt, cfg)
