@@ -219,7 +219,8 @@ def plan_summary(solver, prec):
     """The launch plan that produced a number (pb_get_plan), as it goes into the JSON line."""
     pl = solver.plan(prec)
     keep = ("txv", "ty", "tz", "ring_slots", "blocks_per_sm", "tiles", "grid", "threads", "smem_bytes", "autotuned",
-            "vec_grid", "vec_threads", "persist", "face_palette", "diag_palette_vec", "diag_palette_spmv",
+            "vec_grid", "vec_threads", "persist", "fused", "face_quad", "coef_slots", "face_palette", "diag_palette_vec",
+            "diag_palette_spmv",
             "palette_size", "diag_palette_size", "num_sm", "pitch")
     return {k: pl[k] for k in keep}
 
@@ -248,9 +249,10 @@ def kernel_roofline(solver, prec, n_node, profile_iters, peak):
     ms_spmv, ms_vec = solver.profile(prec, profile_iters)
     spmv_node, vec_node = solver.bytes_per_node(prec, 0), solver.bytes_per_node(prec, 1)
     ach_s = spmv_node * n_node / (ms_spmv * 1e-3) / 1e9
-    ach_v = vec_node * n_node / (ms_vec * 1e-3) / 1e9
+    ach_v = vec_node * n_node / (ms_vec * 1e-3) / 1e9 if ms_vec > 0 else None      # fused iteration: no K_vec launch
     return {"spmv_ms": ms_spmv, "vec_ms": ms_vec, "spmv_bytes_per_node": spmv_node, "vec_bytes_per_node": vec_node,
-            "spmv_GBs": ach_s, "spmv_frac": ach_s / peak, "vec_GBs": ach_v, "vec_frac": ach_v / peak}
+            "spmv_GBs": ach_s, "spmv_frac": ach_s / peak, "vec_GBs": ach_v,
+            "vec_frac": (ach_v / peak) if ach_v is not None else None}
 
 
 def run_ours(args, rank, local_rank, world):
@@ -389,7 +391,15 @@ def run_ours(args, rank, local_rank, world):
     ns_bytes = WORDS_NORTH_STAR * elt * n_node
     t_solve = ms_local * 1e-3
     committed = ncu_traffic(f"k_spmv:{wl}")
-    roofline = {"bound": "hbm", "kernel": "k_spmv_tma", "achieved": kr["spmv_GBs"], "peak": peak, "unit": "GB/s",
+    plan = plan_summary(solver, prec)
+    fused = bool(plan.get("fused"))
+    kvec = (None if fused else
+            {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
+             "diag_palette_size": pald, "ms_per_launch": ms_vec})
+    roofline = {"bound": "hbm", "kernel": "k_pcg_fused" if fused else "k_spmv_tma",
+                "kernel_note": ("one launch = one whole PCG iteration over all N nodes (K_spmv with K_vec folded in)" if fused
+                                else "one launch = K_spmv over all N nodes; K_vec under k_vec"),
+                "achieved": kr["spmv_GBs"], "peak": peak, "unit": "GB/s",
                 "frac": kr["spmv_frac"], "traffic": committed, "traffic_ncu_committed": committed,
                 "traffic_source": "profiles/ncu_traffic.csv: dram__bytes of a committed ncu --set full capture of this "
                                   "kernel and workload; NOT measured in this run",
@@ -398,12 +408,13 @@ def run_ours(args, rank, local_rank, world):
                 "bytes_accounting": "stored-format bytes (pb_bytes_per_node): what physically has to cross HBM; "
                                     "SURVEY 8(d)'s uncompressed words are in survey_10word / iteration.north_star_*",
                 "palette_size": pal, "ms_per_launch": ms_spmv, "clocks_during_profile": clocks_prof.summary(),
-                "plan": plan_summary(solver, prec),
-                "survey_10word": {"bytes_per_launch": WORDS_SPMV * elt * n_node,
-                                  "GBs": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9,
-                                  "frac": WORDS_SPMV * elt * n_node / (ms_spmv * 1e-3) / 1e9 / peak},
-                "k_vec": {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
-                          "diag_palette_size": pald, "ms_per_launch": ms_vec},
+                "plan": plan,
+                "survey_words": {"words_per_node": WORDS_NORTH_STAR if fused else WORDS_SPMV,
+                                 "bytes_per_launch": (WORDS_NORTH_STAR if fused else WORDS_SPMV) * elt * n_node,
+                                 "GBs": (WORDS_NORTH_STAR if fused else WORDS_SPMV) * elt * n_node / (ms_spmv * 1e-3) / 1e9,
+                                 "note": "the same launch time charged with SURVEY.md 8(d)'s uncompressed words: the whole "
+                                         "16-word iteration for the fused kernel, the 10-word K_spmv otherwise"},
+                "k_vec": kvec,
                 "iteration": {"achieved": iter_bytes * iters / t_solve / 1e9,
                               "frac": iter_bytes * iters / t_solve / 1e9 / peak,
                               "north_star_16word_GBs": ns_bytes * iters / t_solve / 1e9,
@@ -418,6 +429,10 @@ def run_ours(args, rank, local_rank, world):
         other = "f64" if prec == "f32" else "f32"
         try:
             roofline[other] = variant_leg(solver, torch, stream, other, TOL[other], args, inp, peak)
+            if fused:
+                solver.set_option("fused", 0)      # the same workload through K_spmv + K_vec (two launches per iteration)
+                roofline["two_kernel"] = variant_leg(solver, torch, stream, prec, tol, args, inp, peak)
+                solver.set_option("fused", 1)
             solver.set_option("palette", 0)        # word format: 40 B (fp32) / 80 B (fp64) per node in k_spmv_tma
             roofline["no_palette"] = variant_leg(solver, torch, stream, prec, tol, args, inp, peak)
             roofline["no_palette"]["note"] = ("PB_OPT_PALETTE = 0: face dielectrics and Dinv as full words, the format an "
@@ -467,11 +482,13 @@ def variant_leg(solver, torch, stream, prec, tol, args, inp, peak):
     kr = kernel_roofline(solver, prec, inp.n, max(10, args.profile_iters // 2), peak)
     del out
     return {"dtype": prec, "tol": tol, "value": iters / (ms * 1e-3), "unit": UNIT, "iterations_per_solve": res["iters"],
-            "final_relres": res["relres"], "ms_per_solve": ms / 2, "kernel": "k_spmv_tma",
+            "final_relres": res["relres"], "ms_per_solve": ms / 2,
+            "kernel": "k_pcg_fused" if solver.plan(prec)["fused"] else "k_spmv_tma",
             "achieved": kr["spmv_GBs"], "frac": kr["spmv_frac"], "bytes_per_node": kr["spmv_bytes_per_node"],
             "ms_per_launch": kr["spmv_ms"],
-            "k_vec": {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
-                      "ms_per_launch": kr["vec_ms"]},
+            "k_vec": (None if kr["vec_GBs"] is None else
+                      {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
+                       "ms_per_launch": kr["vec_ms"]}),
             "iteration_frac": (kr["spmv_bytes_per_node"] + kr["vec_bytes_per_node"]) * inp.n * iters / (ms * 1e-3) / 1e9 / peak,
             "plan": plan_summary(solver, prec)}
 

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpb.so")
 SOURCES = ["pb_api.cu"]
-DEPS = ["pb_api.cu", "pb_kernels.cuh", "pb_spmv_tma.cuh", "pb_persist.cuh", "pb_tma.cuh", "pb_setup.cuh", "pb_grid.cuh", "pb_internal.cuh", os.path.join("..", "..", "include", "pb.h")]
+DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))) + [os.path.join("..", "..", "include", "pb.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 

@@ -1687,6 +1687,13 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
             if (!w.ready) return PB_ERR_INVALID_ARG;
             const float *src[] = {w.r, w.Dinv, nullptr, w.Ap, w.x};
             const float *sp = src[what - 3];
+            if (h->last_fused && what != 4) {      // k_pcg_fused: the buffers the NEXT pass reads (r is one update behind)
+                PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+                PB_CUDA(cudaStreamSynchronize(h->stream));
+                const int par = h->pinned_state->iter_cur & 1;
+                const float *fs[] = {par ? w.bw.r2 : w.bw.r, nullptr, par ? w.bw.p1 : w.bw.p0, par ? w.bw.Ap2 : w.bw.Ap, w.bw.x};
+                sp = fs[what - 3];
+            }
             if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
                        PB_CUDA(cudaStreamSynchronize(h->stream)); sp = (h->pinned_state->iter_cur & 1) ? w.p1 : w.p0; }
             k_unpad<float, double><<<g, 256, 0, h->stream>>>(sp, (double *)h->stage, h->nx, w.P, rows, 1.0);
@@ -1695,6 +1702,13 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
             if (!w.ready) return PB_ERR_INVALID_ARG;
             const double *src[] = {w.r, w.Dinv, nullptr, w.Ap, w.x};
             const double *sp = src[what - 3];
+            if (h->last_fused && what != 4) {
+                PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
+                PB_CUDA(cudaStreamSynchronize(h->stream));
+                const int par = h->pinned_state->iter_cur & 1;
+                const double *fs[] = {par ? w.bw.r2 : w.bw.r, nullptr, par ? w.bw.p1 : w.bw.p0, par ? w.bw.Ap2 : w.bw.Ap, w.bw.x};
+                sp = fs[what - 3];
+            }
             if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
                        PB_CUDA(cudaStreamSynchronize(h->stream)); sp = (h->pinned_state->iter_cur & 1) ? w.p1 : w.p0; }
             k_unpad<double, double><<<g, 256, 0, h->stream>>>(sp, (double *)h->stage, h->nx, w.P, rows, 1.0);

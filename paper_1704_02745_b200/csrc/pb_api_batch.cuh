@@ -38,25 +38,25 @@ pb_status batch_kernel_attr_fmt(bool quad, bool pald, size_t *max_dyn)
     return pald ? batch_kernel_attr<T, false, true, M>(max_dyn) : batch_kernel_attr<T, false, false, M>(max_dyn);
 }
 
-template <typename T, bool QUAD, bool PALD, int M>
+template <typename T, bool QUAD, bool PALD>
 pb_status fused_kernel_attr(size_t *max_dyn)
 {
     cudaFuncAttributes fa;
-    PB_CUDA(cudaFuncGetAttributes(&fa, k_pcg_fused<T, QUAD, PALD, M>));
+    PB_CUDA(cudaFuncGetAttributes(&fa, k_pcg_fused<T, QUAD, PALD>));
     const size_t lim = (size_t)232448 - fa.sharedSizeBytes;
-    PB_CUDA(cudaFuncSetAttribute(k_pcg_fused<T, QUAD, PALD, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim));
+    PB_CUDA(cudaFuncSetAttribute(k_pcg_fused<T, QUAD, PALD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim));
     *max_dyn = lim;
     return PB_OK;
 }
-template <typename T, int M>
+template <typename T>
 pb_status fused_kernel_attr_fmt(bool quad, bool pald, size_t *max_dyn)
 {
-    if (quad) return pald ? fused_kernel_attr<T, true, true, M>(max_dyn) : fused_kernel_attr<T, true, false, M>(max_dyn);
-    return pald ? fused_kernel_attr<T, false, true, M>(max_dyn) : fused_kernel_attr<T, false, false, M>(max_dyn);
+    if (quad) return pald ? fused_kernel_attr<T, true, true>(max_dyn) : fused_kernel_attr<T, true, false>(max_dyn);
+    return pald ? fused_kernel_attr<T, false, true>(max_dyn) : fused_kernel_attr<T, false, false>(max_dyn);
 }
 
 // coefficient arrays, vectors, plan and tensor maps of the batch path for M members; `fused`: of k_pcg_fused (one
-// kernel per iteration, M = 1 or 2) instead of k_spmv_batch + k_vec_batch
+// kernel per iteration, one member) instead of k_spmv_batch + k_vec_batch
 template <typename T>
 pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
 {
@@ -119,13 +119,12 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     // deep as the shared memory allows
     size_t max_dyn = 0;
     if (fused) {
-        if (M == 1) PB_TRY((fused_kernel_attr_fmt<T, 1>(b.quad, b.pald, &max_dyn)));
-        else if (M == 2) PB_TRY((fused_kernel_attr_fmt<T, 2>(b.quad, b.pald, &max_dyn)));
-        else return PB_ERR_INVALID_ARG;
+        if (M != 1) return PB_ERR_INVALID_ARG;
+        PB_TRY((fused_kernel_attr_fmt<T>(b.quad, b.pald, &max_dyn)));
     } else if (M == 1) PB_TRY((batch_kernel_attr_fmt<T, 1>(b.quad, b.pald, &max_dyn)));
     else if (M == 2) PB_TRY((batch_kernel_attr_fmt<T, 2>(b.quad, b.pald, &max_dyn)));
     else PB_TRY((batch_kernel_attr_fmt<T, 4>(b.quad, b.pald, &max_dyn)));
-    const int max_threads = fused ? (M >= 2 ? 256 : 512) : (M >= 4 ? 256 : 512);      // the kernels' launch bounds
+    const int max_threads = (!fused && M >= 4) ? 256 : 512;      // the kernels' launch bounds
     const int rowvecs = w.P / VEC;
     const int maxv = ((b.pald || b.quad) ? 240 : 256) / VEC - 2;
     int ntx0 = (rowvecs + 32) / 64;
@@ -150,7 +149,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.nsv = 0;
     for (int t = 0; t < 3; t++) {
         const int bps = forced_bps > 0 ? forced_bps : try_bps[t], nsc = try_nsc[t];
-        const long fixed = (long)nsc * (long)L.cslot + 2L * M * (long)L.pn + 128;
+        const long fixed = (long)nsc * (long)L.cslot + (fused ? (long)kFusedPlanes : 2L * M) * (long)L.pn + 128;
         long budget = (long)((size_t)232448 / bps) - 1024 - (long)((size_t)232448 - max_dyn) - fixed;   // per-SM share
         if ((long)max_dyn - fixed < budget) budget = (long)max_dyn - fixed;                              // per-block cap
         int nsv = budget > 0 ? (int)(budget / vslot) : 0;
@@ -160,7 +159,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     }
     if (o[PB_OPT_RING_SLOTS] > 0 && o[PB_OPT_RING_SLOTS] < b.nsv) b.nsv = o[PB_OPT_RING_SLOTS];
     if (b.nsv < 2) return PB_ERR_INVALID_ARG;
-    b.smem = fused ? fused_smem(FL, b.nsv, b.nsc, M) : batch_smem(L, b.nsv, b.nsc, M);
+    b.smem = fused ? fused_smem(FL, b.nsv, b.nsc) : batch_smem(L, b.nsv, b.nsc, M);
     b.ntx = (rowvecs + b.TXV - 1) / b.TXV;
     b.nty = (h->ny + b.TY - 1) / b.TY;
     const int slots = h->nsm * b.bps, xy = b.ntx * b.nty;
@@ -171,7 +170,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.grid = (int)(ntiles < slots ? ntiles : slots);
     b.vec_grid = grid_for(w.npad / VEC, 256, h->nsm * 8);
     size_t need = (size_t)M * b.grid > (size_t)2 * M * b.vec_grid ? (size_t)M * b.grid : (size_t)2 * M * b.vec_grid;
-    if ((size_t)M * kFusedSums * b.grid > need) need = (size_t)M * kFusedSums * b.grid;
+    if ((size_t)kFusedSums * b.grid > need) need = (size_t)kFusedSums * b.grid;
     if (need > h->partials_cap) {
         PB_CUDA(cudaStreamSynchronize(h->stream));
         if (h->partials) cudaFree(h->partials);
@@ -238,19 +237,19 @@ void launch_batch_kernels(pb_handle *h, Work<T> &w, int n_iter)
     }
 }
 
-template <typename T, bool QUAD, bool PALD, int M>
+template <typename T, bool QUAD, bool PALD>
 void launch_fused_kernels(pb_handle *h, Work<T> &w, int n_iter)
 {
     BatchWork<T> &b = w.bw;
     FusedArgs<T> a;
-    a.r0 = b.r; a.r1 = b.r2; a.Ap0 = b.Ap; a.Ap1 = b.Ap2; a.p0 = b.p0; a.p1 = b.p1; a.x = b.x; a.npad = w.npad;
+    a.r0 = b.r; a.r1 = b.r2; a.Ap0 = b.Ap; a.Ap1 = b.Ap2; a.p0 = b.p0; a.p1 = b.p1; a.x = b.x;
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
     a.TXV = b.TXV; a.TY = b.TY; a.TZ = b.TZ; a.ntx = b.ntx; a.nty = b.nty; a.ntz = b.ntz;
     a.ntiles = b.ntx * b.nty * b.ntz; a.nsv = b.nsv; a.nsc = b.nsc; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.lut = w.lut; a.dlut = w.dlut;
     for (int it = 0; it < n_iter; it++)
-        k_pcg_fused<T, QUAD, PALD, M><<<b.grid, b.threads, b.smem, h->stream>>>(b.vm, b.tm_dinv, b.tm_x, b.tm_exm, b.tm_exp,
-                                                                              b.tm_ey, b.tm_ez, a);
+        k_pcg_fused<T, QUAD, PALD><<<b.grid, b.threads, b.smem, h->stream>>>(b.vm, b.tm_dinv, b.tm_x, b.tm_exm, b.tm_exp,
+                                                                           b.tm_ey, b.tm_ez, a);
 }
 
 template <typename T>
@@ -258,10 +257,8 @@ pb_status enqueue_batch_iterations(pb_handle *h, Work<T> &w, int n_iter)
 {
     const BatchWork<T> &b = w.bw;
     if (b.fused) {
-#define PB_FUSED_M(Q, D) do { if (b.M == 1) launch_fused_kernels<T, Q, D, 1>(h, w, n_iter); else launch_fused_kernels<T, Q, D, 2>(h, w, n_iter); } while (0)
-        if (b.quad) { if (b.pald) PB_FUSED_M(true, true); else PB_FUSED_M(true, false); }
-        else { if (b.pald) PB_FUSED_M(false, true); else PB_FUSED_M(false, false); }
-#undef PB_FUSED_M
+        if (b.quad) { if (b.pald) launch_fused_kernels<T, true, true>(h, w, n_iter); else launch_fused_kernels<T, true, false>(h, w, n_iter); }
+        else { if (b.pald) launch_fused_kernels<T, false, true>(h, w, n_iter); else launch_fused_kernels<T, false, false>(h, w, n_iter); }
         PB_CUDA(cudaGetLastError());
         h->launches += (long long)n_iter;
         return PB_OK;
@@ -377,7 +374,7 @@ pb_status solve_batch_impl(pb_handle *h, int m, const double *rhs, const double 
     for (int g0 = 0; g0 < m;) {
         int M = width;
         while (M > m - g0) M >>= 1;
-        PB_TRY(ensure_batch<T>(h, M, h->opt[PB_OPT_FUSED] != 0 && M <= 2));
+        PB_TRY(ensure_batch<T>(h, M, h->opt[PB_OPT_FUSED] != 0 && M == 1));
         for (int s = 0; s < M; s++) {
             const int mem = g0 + s;
             if (charges) {

@@ -1,26 +1,35 @@
-// pb_fused.cuh -- ONE kernel per PCG iteration: k_spmv_batch (pb_spmv_batch.cuh) with K_vec folded in.
+// pb_fused.cuh -- ONE kernel per PCG iteration: K_spmv with K_vec folded in ("single-reduction PCG").
 //
-// The two-kernel iteration (K_spmv, K_vec) needs two passes because step 5's alpha needs
-// p.Ap (a reduction over the whole grid) before r can be updated, and step 7's beta needs r_new.z_new (a second one)
-// before p can.  Here the residual update of iteration l is DEFERRED into the pass of iteration
-// l+1 -- r_l = r_{l-1} - alpha_l A p_l is formed where r and A p_l are staged anyway, halo cells included -- and the
-// scalars of iteration l+1 all come out of ONE reduction at the end of that pass:
-//     p.Ap = sum p v,  v = A p_{l+1}                                                  (step 5)
-//     r_l.z_l = U1 = sum Dinv r_l^2,   r_l.r_l = U2 = sum r_l^2                          (exact, of the stored r_l)
-//     alpha = U1 / p.Ap
-//     r_{l+1}.z_{l+1} = U1 - 2 alpha S1 + alpha^2 S2,   S1 = sum Dinv r_l v,  S2 = sum Dinv v^2    (r_{l+1} = r_l - alpha v)
-//     r_{l+1}.r_{l+1} = U2 - 2 alpha T1 + alpha^2 T2,   T1 = sum r_l v,       T2 = sum v^2
-//     beta = r_{l+1}.z_{l+1} / U1                                                        (step 7)
-// These are the algebraic expansions of the very dot products K_vec computes; because U1 and U2 are re-summed from
-// the stored r_l in every pass, the expansion is only ever one step deep (no drift: the classical single-reduction
-// recurrences carry the norms along and lose them after ~1/eps of reduction).  In exact arithmetic the iterates are
-// those of PAPER.md:104-126; in floating point alpha and beta agree with the two-kernel path to rounding.
-// The stopping rule (step 3) is applied to the predicted ||r_{l+1}||, so the solve stops at the same l.
+// The two-kernel iteration (K_spmv, K_vec) needs two passes over the grid because step 5's
+// alpha needs p.Ap (a reduction over the whole grid) before r can be updated, and step 7's beta needs r_new.z_new (a
+// second one) before p can.  Here the residual update of iteration l is DEFERRED into the pass of
+// iteration l+1 -- r_l = r_{l-1} - alpha_l A p_l is formed where r and A p_l are staged anyway, halo cells included --
+// and every scalar of iteration l+1 comes out of ONE reduction at the end of that pass.  With v = A p_{l+1}:
+//     p.Ap = sum p_{l+1} v                                                               (step 5)
+//     U1 = sum Dinv r_l^2 = r_l.z_l,   U2 = sum r_l^2                (re-summed EXACTLY from the stored r_l, every pass)
+//     alpha_{l+1} = U1 / p.Ap
+//     r_{l+1}.z_{l+1} = U1 - 2 alpha S1 + alpha^2 S2,   S2 = sum Dinv v^2,   S1 = z_l.v = p.Ap - beta_l W,
+//                                                       W = sum (A p_l) p_{l+1}  (= p_l . A p_{l+1}: A is symmetric)
+//     beta_{l+1} = r_{l+1}.z_{l+1} / U1                                                 (step 7)
+// These are algebraic expansions of the very dot products K_vec computes, one step deep: U1 is re-summed in every pass,
+// so nothing drifts (the classical single-reduction recurrences carry the norms along and lose them after ~1/eps of
+// reduction).  W is summed where A p_l and p_{l+1} meet (the update stage), S2 and p.Ap where v is made (the stencil).
+// The stopping rule (step 3) is applied to U2, the exact ||r_l||^2 of the stored residual, at the end of
+// pass l+1: the solve stops at the same l as the two-kernel path and the oracle, and pays one extra pass per solve
+// (x already holds phi_l then: the deferred update x += alpha_l p_l is part of this pass; alpha is zeroed so that
+// k_finish adds nothing).  In exact arithmetic the iterates are those of PAPER.md:104-126.
 //
-// Bytes per node and iteration: reads r, A p_l, p (haloed), x, Dinv, three faces; writes r, p, x, A p_{l+1}:
+// Bytes per node and iteration: reads r, A p_l, p (haloed), x, Dinv, the three faces; writes r, p, x, A p_{l+1}:
 // 8 words + 2 index bytes in the quad format with the diagonal palette (34 B fp32, 66 B fp64) instead of 41 / 77 B
 // in two kernels; r, p and A p are double-buffered (a neighbouring tile reads the old plane while this one writes).
-// Everything else -- rings, p_new planes, coefficient formats, per-member latches -- is k_spmv_batch's.
+//
+// Structure: k_spmv_batch's (pb_spmv_batch.cuh) -- a vector ring {r, A p_l, p_l haloed, x} released right after the
+// update stage, a coefficient ring held one step longer -- with the per-thread state cut to the bone, because this
+// kernel is bound by instruction issue, not by bytes: p_new lives in THREE shared planes (k-1, k, k+1) and is re-read
+// from there instead of being rotated through registers; the step is unrolled twice so that D, Dinv and the z-face of
+// planes k / k+1 alternate between two register sets without moves; every shared address is a 32-bit slot base plus
+// a per-thread offset computed once; inactive lanes run the same instructions on in-range cells and are masked out
+// of the stores and the sums.
 #pragma once
 #include "pb_internal.cuh"
 #include "pb_tma.cuh"
@@ -30,7 +39,8 @@
 
 namespace pb {
 
-constexpr int kFusedSums = 7;        // p.Ap, S1, S2, T1, T2, U1, U2
+constexpr int kFusedSums = 5;        // p.Ap, S2, W, U1, U2
+constexpr int kFusedPlanes = 3;      // p_new planes k-1, k, k+1
 
 // vector slot of the fused kernel: r, A p (old) and p (old) haloed, x un-haloed
 struct FusedLayout {
@@ -45,32 +55,31 @@ __host__ __device__ inline FusedLayout fused_layout(int TXV, int TY, int vec, bo
     F.vslot = F.oAq + align128(F.B.bZ);
     return F;
 }
-__host__ __device__ inline size_t fused_smem(const FusedLayout &F, int nsv, int nsc, int M)
+__host__ __device__ inline size_t fused_smem(const FusedLayout &F, int nsv, int nsc)
 {
-    return (size_t)nsv * F.vslot + (size_t)nsc * F.B.cslot + (size_t)2 * M * F.B.pn + 128;
+    return (size_t)nsv * F.vslot + (size_t)nsc * F.B.cslot + (size_t)kFusedPlanes * F.B.pn + 128;
 }
 
 template <typename T>
 struct FusedArgs {
-    T *r0, *r1, *Ap0, *Ap1, *p0, *p1;   // [M][npad] each: iteration with iter_cur = l reads buffer l & 1, writes the other
+    T *r0, *r1, *Ap0, *Ap1, *p0, *p1;   // iteration with iter_cur = l reads buffer l & 1, writes the other
     T *x;
-    size_t npad;
     int nx, ny, nz, P;
     int TXV, TY, TZ;
     int ntx, nty, ntz, ntiles;
     int nsv, nsc;
     int precond;
-    State *st;               // [M]
-    double *partials;        // [M][kFusedSums][gridDim.x]
+    State *st;
+    double *partials;        // [kFusedSums][gridDim.x]
     const T *lut;
     const T *dlut;
 };
 
-// the six ping-pong vector tensors (4-D [M][nz][ny][P], member = coordinate 3), in one kernel parameter
+// the six ping-pong vector tensors (4-D [1][nz][ny][P]) in one kernel parameter
 struct FusedMaps { CUtensorMap r0, r1, q0, q1, p0, p1; };
 
-template <typename T, bool QUAD, bool PALD, int M>
-__global__ void __launch_bounds__(M >= 2 ? 256 : 512)
+template <typename T, bool QUAD, bool PALD>
+__global__ void __launch_bounds__(512)
 k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtensorMap tm_dinv,
             const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_exm,
             const __grid_constant__ CUtensorMap tm_exp, const __grid_constant__ CUtensorMap tm_ey,
@@ -92,21 +101,10 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
     const int warp = tid >> 5, lane = tid & 31;
     const bool is_producer = (warp == NCW);
 
-    // per-member scalars; a member whose latch is set is skipped by producer and consumers alike
-    T beta[M], alpha_prev[M];                  // beta_l and alpha_l: r_l = r_{l-1} - alpha_l A p_l, x += alpha_l p_l, p_{l+1} = z_l + beta_l p_l
-    bool live[M];
-    int parity[M];
-    bool any = false;
-#pragma unroll
-    for (int s = 0; s < M; s++) {
-        const State *st = a.st + s;
-        live[s] = !st->done;
-        any |= live[s];
-        beta[s] = (T)st->beta;
-        alpha_prev[s] = (T)st->alpha;          // alpha of the previous iteration (0 before the first)
-        parity[s] = st->iter_cur & 1;
-    }
-    if (!any) return;
+    if (a.st->done) return;
+    const T beta = (T)a.st->beta;              // beta_l:  p_{l+1} = z_l + beta_l p_l
+    const T alpha = (T)a.st->alpha;            // alpha_l: r_l = r_{l-1} - alpha_l A p_l,  phi_l = phi_{l-1} + alpha_l p_l
+    const int parity = a.st->iter_cur & 1;
 
     const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
     const int TXV = a.TXV, TY = a.TY, TZ = a.TZ, NSV = a.nsv, NSC = a.nsc;
@@ -114,7 +112,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
     const BatchLayout &L = F.B;
     unsigned char *vbase = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
     unsigned char *cbase = vbase + (size_t)NSV * F.vslot;
-    unsigned char *pnbase = cbase + (size_t)NSC * L.cslot;   // PN[s][parity] at pnbase + (2 s + parity) * L.pn
+    unsigned char *pnbase = cbase + (size_t)NSC * L.cslot;
 
     if (tid == 0) {
         for (int i = 0; i < NSV; i++) { mbar_init(&vfull[i], 1); mbar_init(&vempty[i], NCW); }
@@ -130,16 +128,13 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         for (int i = tid; i < 256; i += nthr) { const T d = a.dlut[i]; ddtab[2 * i] = d; ddtab[2 * i + 1] = rcp_rn(d); }
     __syncthreads();
 
-    double acc[M][kFusedSums];                 // per thread: p.Ap, S1, S2, T1, T2, U1, U2 (see the header)
-#pragma unroll
-    for (int s = 0; s < M; s++)
-#pragma unroll
-        for (int q = 0; q < kFusedSums; q++) acc[s][q] = 0.0;
+    double a_pAp = 0.0, a_S2 = 0.0, a_W = 0.0, a_U1 = 0.0, a_U2 = 0.0;
 
     if (is_producer) {
         if (lane == 0) {
             int vs = 0, cs = 0;
             uint32_t vph = 0, cph = 0;
+            const CUtensorMap *tr = parity ? &vm.r1 : &vm.r0, *tq = parity ? &vm.q1 : &vm.q0, *tp = parity ? &vm.p1 : &vm.p0;
             for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
                 int b = tile;
                 const int bx = b % a.ntx; b /= a.ntx;
@@ -168,16 +163,14 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                         }
                         cs = (cs + 1 == NSC) ? 0 : cs + 1; cph ^= (cs == 0);
                     }
-#pragma unroll
-                    for (int s = 0; s < M; s++) {
-                        if (!live[s]) continue;
+                    {   // vector item q
                         mbar_wait(&vempty[vs], vph ^ 1);
                         unsigned char *slot = vbase + vs * (uint32_t)F.vslot;
                         mbar_expect_tx(&vfull[vs], 3 * L.bZ + (centre ? L.bX : 0u));
-                        tma_load_4d(slot + L.oR, parity[s] ? &vm.r1 : &vm.r0, x0 - VEC, j0 - 1, q, s, &vfull[vs]);
-                        tma_load_4d(slot + F.oAq, parity[s] ? &vm.q1 : &vm.q0, x0 - VEC, j0 - 1, q, s, &vfull[vs]);
-                        tma_load_4d(slot + L.oPp, parity[s] ? &vm.p1 : &vm.p0, x0 - VEC, j0 - 1, q, s, &vfull[vs]);
-                        if (centre) tma_load_4d(slot + L.oX, &tm_x, x0, j0, q, s, &vfull[vs]);
+                        tma_load_4d(slot + L.oR, tr, x0 - VEC, j0 - 1, q, 0, &vfull[vs]);
+                        tma_load_4d(slot + F.oAq, tq, x0 - VEC, j0 - 1, q, 0, &vfull[vs]);
+                        tma_load_4d(slot + L.oPp, tp, x0 - VEC, j0 - 1, q, 0, &vfull[vs]);
+                        if (centre) tma_load_4d(slot + L.oX, &tm_x, x0, j0, q, 0, &vfull[vs]);
                         vs = (vs + 1 == NSV) ? 0 : vs + 1; vph ^= (vs == 0);
                     }
                 }
@@ -185,15 +178,15 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         }
         __syncwarp();
     } else {
+        // ---- consumer warps ---------------------------------------------------------------------------------
         const int BWc = TXV + 2;                       // vectors per row of the haloed boxes
         const int TXP = spmv_row_threads(TXV);
-        const int tx = tid % TXP, ty = tid / TXP;
-        const bool intile = ty < TY && tx < TXV;
+        const int tx0 = tid % TXP, ty0 = tid / TXP;
+        const bool intile = ty0 < TY && tx0 < TXV;
+        // lanes outside the tile run the same instructions on cell (0, 0) of the tile and are masked out below
+        const int tx = intile ? tx0 : 0, ty = intile ? ty0 : 0;
         const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
-        const int own_d = (ty + 1) * L.bwd + (tx + 1) * VEC;   // PALD: its byte offset in the Dinv-index box
-        const int cown = ty * TXV + tx;                // own cell in the un-haloed boxes
         const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
-        const bool precond = a.precond != 0;
         auto halo_cell = [&](int h) -> int {
             if (h < TXV) return h + 1;
             if (h < 2 * TXV) return (TY + 1) * BWc + (h - TXV) + 1;
@@ -202,50 +195,53 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         };
         auto cell_d = [&](int c) -> int { const int row = c / BWc; return row * L.bwd + (c - row * BWc) * VEC; };
         const int extra0 = (NCT - 1 - tid < nextra) ? halo_cell(NCT - 1 - tid) : -1;   // this thread's halo cell
-        const int extra0_d = (PALD && extra0 >= 0) ? cell_d(extra0) : 0;
-        int lead_d = 0;                                // PALD: bytes between the Dinv-index box's aligned start and x0 - VEC
-        int qoff = 0, qfield = 0;                      // QUAD: byte (in a box row) and field offset of this thread's nodes
+        const bool has_x0 = extra0 >= 0;
+        const bool more_halo = nextra > NCT;           // only tiny tiles: the halo outnumbers the threads
+        const bool precond = a.precond != 0;
 
-        // Dinv (and D = 1/Dinv when `D` is given) of haloed-box cell c of a coefficient slot
-        auto load_dinv = [&](const unsigned char *cslot, int c, int cd, Vec<T> &dinv, Vec<T> *D) {
+        const uint32_t sm_v = smem_u32(vbase), sm_c = smem_u32(cbase), sm_pn = smem_u32(pnbase);
+        const uint32_t sm_q = smem_u32(qtab), sm_dd = smem_u32(ddtab);
+        const uint32_t sm_vfull = smem_u32(vfull), sm_vempty = smem_u32(vempty), sm_cfull = smem_u32(cfull),
+                       sm_cempty = smem_u32(cempty);
+        const uint32_t vslot_b = (uint32_t)F.vslot, cslot_b = (uint32_t)L.cslot, pn_b = (uint32_t)L.pn;
+        const uint32_t o_own = (uint32_t)own * 16u;                    // own cell within a haloed vector box / p_new plane
+        const uint32_t o_x0 = has_x0 ? (uint32_t)extra0 * 16u : 0u;    // this thread's halo cell
+        const uint32_t o_r = (uint32_t)L.oR + o_own, o_q = (uint32_t)F.oAq + o_own, o_p = (uint32_t)L.oPp + o_own;
+        const uint32_t o_xbox = (uint32_t)L.oX + (uint32_t)(ty * TXV + tx) * 16u;
+        const uint32_t row16 = (uint32_t)BWc * 16u;
+        T *const r_out = parity ? a.r0 : a.r1, *const q_out = parity ? a.Ap0 : a.Ap1, *const p_out = parity ? a.p0 : a.p1;
+        // per tile (the aligned starts of the byte boxes depend on x0)
+        uint32_t o_dv_own = 0, o_dv_x0 = 0, o_ez = 0, o_exm = 0, o_exp = 0, o_ey0 = 0, o_ey1 = 0, qfield = 0;
+        int lead_d = 0;
+
+        // Dinv and D = 1/Dinv of VEC nodes: index bytes at `addr` -> pair table, or Dinv words at `addr`
+        auto load_dinv = [&](uint32_t addr, Vec<T> &dinv, Vec<T> &D) {
             if (PALD) {
-                const unsigned char *p = cslot + L.oDv + lead_d + cd;
-                const uint32_t w = (VEC == 4) ? *reinterpret_cast<const uint32_t *>(p)
-                                              : (uint32_t)*reinterpret_cast<const unsigned short *>(p);
+                const uint32_t w = (VEC == 4) ? lds_u32(addr) : lds_u16(addr);
 #pragma unroll
-                for (int e = 0; e < VEC; e++) {
-                    const uint32_t i = (w >> (8 * e)) & 255u;
-                    const T *pr = reinterpret_cast<const T *>(reinterpret_cast<const unsigned char *>(ddtab) + i * (2 * sizeof(T)));
-                    if (sizeof(T) == 4) {
-                        const float2 v = *reinterpret_cast<const float2 *>(pr);
-                        dinv.a[e] = (T)v.x; if (D) D->a[e] = (T)v.y;
-                    } else {
-                        const double2 v = *reinterpret_cast<const double2 *>(pr);
-                        dinv.a[e] = (T)v.x; if (D) D->a[e] = (T)v.y;
-                    }
-                }
+                for (int e = 0; e < VEC; e++)
+                    lds_pair(dinv.a[e], D.a[e], sm_dd + ((w >> (8 * e)) & 255u) * (uint32_t)(2 * sizeof(T)));
             } else {
-                dinv = reinterpret_cast<const Vec<T> *>(cslot + L.oDv)[c];
-                if (D) {
+                lds_vec(dinv.a, addr);
 #pragma unroll
-                    for (int e = 0; e < VEC; e++) D->a[e] = rcp_rn(dinv.a[e]);
-                }
+                for (int e = 0; e < VEC; e++) D.a[e] = rcp_rn(dinv.a[e]);
+            }
+            if (!precond) {                                            // M = I: z = r (1 * r is exact)
+#pragma unroll
+                for (int e = 0; e < VEC; e++) dinv.a[e] = T(1);
             }
         };
-        // VEC face coefficients of this thread's nodes, row `row` of a coefficient box
-        auto coef = [&](const unsigned char *box, int row, int row_vecs) -> Vec<T> {
-            if (QUAD) {
-                const uint32_t b = box[row * L.bwq + qoff];
-                return *reinterpret_cast<const Vec<T> *>(reinterpret_cast<const unsigned char *>(qtab) + b * (4 * sizeof(T)) + qfield);
-            }
-            return reinterpret_cast<const Vec<T> *>(box)[row * row_vecs + tx];
+        // VEC face coefficients: quad byte at `addr` -> table of quadruples, or words at `addr`
+        auto coef = [&](uint32_t addr) -> Vec<T> {
+            Vec<T> v;
+            if (QUAD) lds_vec(v.a, sm_q + lds_u8(addr) * (uint32_t)(4 * sizeof(T)) + qfield);
+            else lds_vec(v.a, addr);
+            return v;
         };
-        auto release_vslot = [&](int s_) { __syncwarp(); if (lane == 0) mbar_arrive(&vempty[s_]); };
 
-        int vs = 0, cs = 0;                            // ring slots of the next items and their phase parities
-        uint32_t vph = 0, cph = 0;
-        auto vadvance = [&]() { vs = (vs + 1 == NSV) ? 0 : vs + 1; vph ^= (vs == 0); };
-        auto cadvance = [&]() { cs = (cs + 1 == NSC) ? 0 : cs + 1; cph ^= (cs == 0); };
+        // ring heads: slot index, phase parity and the slot's shared address, advanced together
+        int vs = 0, cs = 0;
+        uint32_t vph = 0, cph = 0, vaddr = sm_v, caddr = sm_c;
         const size_t plane = (size_t)ny * P;
 
         for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
@@ -256,187 +252,217 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             const int x0 = bx * TXV * VEC, j0 = by * TY;
             const int i0 = x0 + tx * VEC, j = j0 + ty;
             const bool active = intile && (i0 < P) && (j < ny);
-            const int nvalid = nx - i0;
+            const T msk = active ? T(1) : T(0);
+            const int nvalid = active ? nx - i0 : 0;   // inactive lanes: A p = 0 (their Dinv may be a zero-filled 0, D = inf)
             const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
             lead_d = (x0 - VEC) & 15;
-            if (QUAD) { qoff = (i0 >> 2) - ((x0 >> 2) & ~15); qfield = (i0 & 3) * (int)sizeof(T); }
-            size_t idx = ((size_t)k0 * ny + j) * P + i0;
-
-            Vec<T> pm[M], pc[M], pn[M], rc[M], rn[M];     // p_new of planes k-1, k, k+1 and r_l of planes k, k+1 (own column)
-#pragma unroll
-            for (int s = 0; s < M; s++) {
-                pm[s] = zerov<T>(); pc[s] = zerov<T>(); pn[s] = zerov<T>(); rc[s] = zerov<T>(); rn[s] = zerov<T>();
+            if (PALD) {
+                o_dv_own = (uint32_t)(L.oDv + lead_d + (ty + 1) * L.bwd + (tx + 1) * VEC);
+                o_dv_x0 = has_x0 ? (uint32_t)(L.oDv + lead_d + cell_d(extra0)) : 0u;
+            } else {
+                o_dv_own = (uint32_t)L.oDv + o_own;
+                o_dv_x0 = (uint32_t)L.oDv + o_x0;
             }
-            Vec<T> Dc = zerov<T>(), Dn = zerov<T>(), ezc = zerov<T>(), ezn = zerov<T>();
-            Vec<T> dvc = zerov<T>(), dvn = zerov<T>();    // Dinv of planes k, k+1 (own column): z_l = Dinv r_l in the sums
+            if (QUAD) {
+                const uint32_t qoff = (uint32_t)((i0 >> 2) - ((x0 >> 2) & ~15));
+                qfield = (uint32_t)(i0 & 3) * (uint32_t)sizeof(T);
+                o_ez = (uint32_t)L.oEZ + (uint32_t)ty * L.bwq + qoff;
+                o_exm = (uint32_t)L.oEXM + (uint32_t)ty * L.bwq + qoff;
+                o_exp = (uint32_t)L.oEXP + (uint32_t)ty * L.bwq + qoff;
+                o_ey0 = (uint32_t)L.oEY + (uint32_t)ty * L.bwq + qoff;
+                o_ey1 = o_ey0 + (uint32_t)L.bwq;
+            } else {
+                o_ez = (uint32_t)L.oEZ + (uint32_t)(ty * TXV + tx) * 16u;
+                o_exm = (uint32_t)L.oEXM + (uint32_t)(ty * (TXV + 1) + tx) * 16u;
+                o_exp = o_exm + 16u;                                   // first element: the plus face of this vector's last node
+                o_ey0 = (uint32_t)L.oEY + (uint32_t)(ty * TXV + tx) * 16u;
+                o_ey1 = o_ey0 + (uint32_t)TXV * 16u;
+            }
+            size_t idx = ((size_t)k0 * ny + j) * P + i0;               // (inactive lanes never use it)
+            // own-cell addresses in the three p_new planes: plane q lives in buffer q mod 3, rotated as the march advances
+            uint32_t pn_m = sm_pn + o_own, pn_c = pn_m + pn_b, pn_n = pn_c + pn_b;
 
-            // "update" of plane kk (the items at the ring heads): p_new of every live member -- own cell into out[s],
-            // and for a plane this tile writes (centre) the haloed box into PN[s][kk & 1], the deferred phi update
-            // and D; the vector slots are handed back, the coefficient slot stays (returned in cslot_out)
-            auto update = [&](int kk, bool centre, Vec<T> *out, Vec<T> *rout, Vec<T> &Dout, Vec<T> &dvout, Vec<T> &ezout,
-                              bool want_ez, size_t xidx) -> const unsigned char * {
-                mbar_wait(&cfull[cs], cph);
-                const unsigned char *cslot = cbase + cs * (uint32_t)L.cslot;
-                Vec<T> dv = zerov<T>(), dvh = zerov<T>();
-                if (intile) load_dinv(cslot, own, own_d, dv, centre ? &Dout : nullptr);
-                dvout = dv;
-                if (centre && extra0 >= 0) load_dinv(cslot, extra0, extra0_d, dvh, nullptr);
-                if (want_ez) ezout = intile ? coef(cslot + L.oEZ, ty, TXV) : zerov<T>();
+            // "update" of the plane at the ring heads -> p_new plane whose own-cell address is `pnw`:
+            // r_l = r_{l-1} - alpha_l A p_l, p_{l+1} = Dinv r_l + beta_l p_l on the own cell (returned; always stored into the plane)
+            // and, for a plane this tile writes (centre), on the halo cells; r_l stored; the deferred phi update; the sums
+            // U1, U2, W.  The vector slot is handed back; the coefficient slot stays (its address is returned).
+            auto update = [&](uint32_t pnw, bool centre, bool want_ez, size_t gidx, Vec<T> &pnew, Vec<T> &Dout, Vec<T> &dvout,
+                              Vec<T> &ezout) -> uint32_t {
+                mbar_wait_a(sm_cfull + 8u * cs, cph);
+                const uint32_t cslot = caddr;
+                Vec<T> dvh, dummy;
+                load_dinv(cslot + o_dv_own, dvout, Dout);
+                if (centre && has_x0) load_dinv(cslot + o_dv_x0, dvh, dummy);
+                if (want_ez) ezout = coef(cslot + o_ez);
+                mbar_wait_a(sm_vfull + 8u * vs, vph);
+                const uint32_t sl = vaddr;
+                Vec<T> rl, qv, pv;
+                lds_vec(rl.a, sl + o_r);
+                lds_vec(qv.a, sl + o_q);
+                lds_vec(pv.a, sl + o_p);
 #pragma unroll
-                for (int s = 0; s < M; s++) {
-                    if (!live[s]) continue;
-                    mbar_wait(&vfull[vs], vph);
-                    const unsigned char *sl = vbase + vs * (uint32_t)F.vslot;
-                    const Vec<T> *R = reinterpret_cast<const Vec<T> *>(sl + L.oR);
-                    const Vec<T> *AQ = reinterpret_cast<const Vec<T> *>(sl + F.oAq);
-                    const Vec<T> *Pp = reinterpret_cast<const Vec<T> *>(sl + L.oPp);
-                    Vec<T> *PN = reinterpret_cast<Vec<T> *>(pnbase + (size_t)(2 * s + (kk & 1)) * L.pn);
-                    // r_l = r_{l-1} - alpha_l A p_l (the deferred step 5), then p_{l+1} = Dinv r_l + beta_l p_l (steps 6-7)
-                    auto pnew = [&](int c, const Vec<T> &d, Vec<T> *pold, Vec<T> *rnew) -> Vec<T> {
-                        Vec<T> v = R[c];
-                        const Vec<T> qv = AQ[c];
-                        const Vec<T> pv = Pp[c];
-#pragma unroll
-                        for (int e = 0; e < VEC; e++) v.a[e] = fma(-alpha_prev[s], qv.a[e], v.a[e]);
-                        if (pold) *pold = pv;
-                        if (rnew) *rnew = v;
-                        if (precond) {
-#pragma unroll
-                            for (int e = 0; e < VEC; e++) v.a[e] = fma(beta[s], pv.a[e], d.a[e] * v.a[e]);
-                        } else {
-#pragma unroll
-                            for (int e = 0; e < VEC; e++) v.a[e] = fma(beta[s], pv.a[e], v.a[e]);
-                        }
-                        return v;
-                    };
-                    Vec<T> v = zerov<T>(), rl = zerov<T>();
-                    if (intile) {
-                        Vec<T> po;
-                        v = pnew(own, dv, &po, &rl);
-                        if (centre) {
-                            PN[own] = v;
-                            if (active) {
-                                stv((parity[s] ? a.r0 : a.r1) + (size_t)s * a.npad + xidx, rl);     // r_l
-                                // phi_{l-1} = phi_{l-2} + alpha_{l-1} p_{l-2}  (step 5 of the previous iteration)
-                                Vec<T> xv = reinterpret_cast<const Vec<T> *>(sl + L.oX)[cown];
-#pragma unroll
-                                for (int e = 0; e < VEC; e++) xv.a[e] = fma(alpha_prev[s], po.a[e], xv.a[e]);
-                                stv(a.x + (size_t)s * a.npad + xidx, xv);
-                            }
-                        }
-                    }
-                    if (centre) {
-                        if (extra0 >= 0) PN[extra0] = pnew(extra0, dvh, nullptr, nullptr);
-                        for (int h = NCT - 1 - tid + NCT; h < nextra; h += NCT) {   // only when the halo outnumbers the threads
-                            const int c = halo_cell(h);
-                            Vec<T> d2;
-                            load_dinv(cslot, c, PALD ? cell_d(c) : 0, d2, nullptr);
-                            PN[c] = pnew(c, d2, nullptr, nullptr);
-                        }
-                    }
-                    out[s] = v;
-                    rout[s] = rl;
-                    consume(v.a[0]);            // R, AQ and Pp of the own cell have been read (x: the store above)
-                    release_vslot(vs);
-                    vadvance();
+                for (int e = 0; e < VEC; e++) {
+                    rl.a[e] = fma(-alpha, qv.a[e], rl.a[e]);                   // r_l (the deferred step 5)
+                    pnew.a[e] = fma(beta, pv.a[e], dvout.a[e] * rl.a[e]);      // p_{l+1} (steps 6-7)
                 }
-                return cslot;
-            };
-
-            // item k0-1: only the own column's values are needed; its coefficient slot goes back after a barrier
-            {
-                const int c0 = cs;
-                update(k0 - 1, false, pm, rn, Dn, dvn, ezn, false, idx);
-                cadvance();
-                named_bar_sync(1, NCT);
-                if (tid == 0) mbar_arrive(&cempty[c0]);
-            }
-            // item k0
-            int ck = cs;
-            const unsigned char *cslotk = update(k0, true, pc, rc, Dc, dvc, ezc, true, idx);
-            cadvance();
-            named_bar_sync(1, NCT);
-
-            for (int k = k0; k < k1; k++, idx += plane) {
-                const int c1 = cs;
-                const unsigned char *cslot1 = update(k + 1, k + 1 < k1, pn, rn, Dn, dvn, ezn, true, idx + plane);
-                cadvance();
-                if (active) {
-                    // the six face coefficients and D of this thread's nodes: decoded once, used by every member
-                    Vec<T> exl, exh;
-                    if (QUAD) {
-                        exl = coef(cslotk + L.oEXM, ty, 0);
-                        exh = coef(cslotk + L.oEXP, ty, 0);
-                    } else {
-                        exl = coef(cslotk + L.oEXM, ty, TXV + 1);
-                        const T exr = reinterpret_cast<const Vec<T> *>(cslotk + L.oEXM)[ty * (TXV + 1) + tx + 1].a[0];
+                sts_vec(pnw, pnew.a);
+                if (centre) {
+                    Vec<T> xv;
+                    lds_vec(xv.a, sl + o_xbox);
+                    T s_u1 = T(0), s_u2 = T(0), s_w = T(0);
 #pragma unroll
-                        for (int e = 0; e < VEC; e++) exh.a[e] = (e == VEC - 1) ? exr : exl.a[e == VEC - 1 ? e : e + 1];
+                    for (int e = 0; e < VEC; e++) {
+                        xv.a[e] = fma(alpha, pv.a[e], xv.a[e]);                // phi_l = phi_{l-1} + alpha_l p_l
+                        s_u1 = fma(dvout.a[e] * rl.a[e], rl.a[e], s_u1);        // r_l.z_l
+                        s_u2 = fma(rl.a[e], rl.a[e], s_u2);                     // ||r_l||^2
+                        s_w = fma(qv.a[e], pnew.a[e], s_w);                     // (A p_l).p_{l+1}
                     }
-                    const Vec<T> eyl = coef(cslotk + L.oEY, ty, TXV), eyh = coef(cslotk + L.oEY, ty + 1, TXV);
-#pragma unroll
-                    for (int s = 0; s < M; s++) {
-                        if (!live[s]) continue;
-                        const Vec<T> *Zk = reinterpret_cast<const Vec<T> *>(pnbase + (size_t)(2 * s + (k & 1)) * L.pn);
-                        const Vec<T> up = Zk[own - BWc], dn = Zk[own + BWc];
-                        const T left = Zk[own - 1].a[VEC - 1], right = Zk[own + 1].a[0];
-                        Vec<T> ap;
-                        // per-plane partial sums in T over this thread's VEC nodes, then one fp64 add per sum
-                        T s_pv = T(0), s_zv = T(0), s_dvv = T(0), s_rv = T(0), s_vv = T(0), s_zr = T(0), s_rr = T(0);
+                    a_U1 += (double)(msk * s_u1);
+                    a_U2 += (double)(msk * s_u2);
+                    a_W += (double)(msk * s_w);
+                    if (active) {
+                        stv(r_out + gidx, rl);
+                        stv(a.x + gidx, xv);
+                    }
+                    if (has_x0) {
+                        const uint32_t h0 = sl + o_x0 - o_own;                  // (o_r etc. include the own-cell offset)
+                        Vec<T> r2, q2, p2;
+                        lds_vec(r2.a, h0 + o_r);
+                        lds_vec(q2.a, h0 + o_q);
+                        lds_vec(p2.a, h0 + o_p);
 #pragma unroll
                         for (int e = 0; e < VEC; e++) {
-                            const T pl = (e == 0) ? left : pc[s].a[e == 0 ? 0 : e - 1];
-                            const T pr = (e == VEC - 1) ? right : pc[s].a[e == VEC - 1 ? e : e + 1];
-                            // same order of operations as k_spmv_tma
-                            T v = Dc.a[e] * pc[s].a[e];
-                            v = fma(-exl.a[e], pl, v);
-                            v = fma(-exh.a[e], pr, v);
-                            v = fma(-eyl.a[e], up.a[e], v);
-                            T w = -eyh.a[e] * dn.a[e];
-                            w = fma(-ezc.a[e], pm[s].a[e], w);
-                            w = fma(-ezn.a[e], pn[s].a[e], w);
-                            v += w;
-                            if (e >= nvalid) v = T(0);     // pad column
-                            const T rl = rc[s].a[e];
-                            const T zl = precond ? dvc.a[e] * rl : rl;          // z_l = M^-1 r_l
-                            const T dv_v = precond ? dvc.a[e] * v : v;
-                            s_pv = fma(pc[s].a[e], v, s_pv);
-                            s_zv = fma(zl, v, s_zv);
-                            s_dvv = fma(dv_v, v, s_dvv);
-                            s_rv = fma(rl, v, s_rv);
-                            s_vv = fma(v, v, s_vv);
-                            s_zr = fma(zl, rl, s_zr);
-                            s_rr = fma(rl, rl, s_rr);
-                            ap.a[e] = v;
+                            r2.a[e] = fma(-alpha, q2.a[e], r2.a[e]);
+                            r2.a[e] = fma(beta, p2.a[e], dvh.a[e] * r2.a[e]);
                         }
-                        acc[s][0] += (double)s_pv; acc[s][1] += (double)s_zv; acc[s][2] += (double)s_dvv;
-                        acc[s][3] += (double)s_rv; acc[s][4] += (double)s_vv; acc[s][5] += (double)s_zr;
-                        acc[s][6] += (double)s_rr;
-                        stv((parity[s] ? a.Ap0 : a.Ap1) + (size_t)s * a.npad + idx, ap);
-                        stv((parity[s] ? a.p0 : a.p1) + (size_t)s * a.npad + idx, pc[s]);
+                        sts_vec(pnw + o_x0 - o_own, r2.a);
+                    }
+                    if (more_halo) {
+                        for (int h = NCT - 1 - tid + NCT; h < nextra; h += NCT) {
+                            const int c = halo_cell(h);
+                            const uint32_t oc = (uint32_t)c * 16u;
+                            Vec<T> d2, r2, q2, p2;
+                            load_dinv(cslot + (PALD ? (uint32_t)(L.oDv + lead_d + cell_d(c)) : (uint32_t)L.oDv + oc), d2, dummy);
+                            lds_vec(r2.a, sl + oc - o_own + o_r);
+                            lds_vec(q2.a, sl + oc - o_own + o_q);
+                            lds_vec(p2.a, sl + oc - o_own + o_p);
+#pragma unroll
+                            for (int e = 0; e < VEC; e++) {
+                                r2.a[e] = fma(-alpha, q2.a[e], r2.a[e]);
+                                r2.a[e] = fma(beta, p2.a[e], d2.a[e] * r2.a[e]);
+                            }
+                            sts_vec(pnw + oc - o_own, r2.a);
+                        }
                     }
                 }
-                named_bar_sync(1, NCT);   // p_new(k+1) boxes complete; everyone is done with coefficient slot ck and p_new(k)
-                if (tid == 0) mbar_arrive(&cempty[ck]);
+                consume(pnew.a[0]);         // r, A p and p of the own cell have been read (x, halo: the stores above)
+                __syncwarp();
+                if (lane == 0) mbar_arrive_a(sm_vempty + 8u * vs);
+                vs++; vaddr += vslot_b;
+                if (vs == NSV) { vs = 0; vaddr = sm_v; vph ^= 1u; }
+                return cslot;
+            };
+            auto cnext = [&]() { cs++; caddr += cslot_b; if (cs == NSC) { cs = 0; caddr = sm_c; cph ^= 1u; } };
+
+            // the stencil of plane k: p_new(k) from plane buffer pc_a (own cell, in-plane neighbours), p_new(k-1) from pm_a,
+            // p_new(k+1) = pn (fresh from the update); coefficient slot cslotk; D, Dinv, ez of plane k and ez of plane k+1
+            auto stencil = [&](uint32_t cslotk, uint32_t pm_a, uint32_t pc_a, const Vec<T> &pn, const Vec<T> &D, const Vec<T> &dv,
+                               const Vec<T> &ezc, const Vec<T> &ezn, size_t gidx) {
+                Vec<T> pc, pm, up, dn, exh;
+                T left, right;
+                lds_vec(pc.a, pc_a);
+                lds_vec(pm.a, pm_a);
+                lds_vec(up.a, pc_a - row16);
+                lds_vec(dn.a, pc_a + row16);
+                lds_one(left, pc_a - (uint32_t)sizeof(T));
+                lds_one(right, pc_a + 16u);
+                const Vec<T> exl = coef(cslotk + o_exm);
+                if (QUAD) {
+                    exh = coef(cslotk + o_exp);
+                } else {
+                    T exr;
+                    lds_one(exr, cslotk + o_exp);
 #pragma unroll
-                for (int s = 0; s < M; s++) { pm[s] = pc[s]; pc[s] = pn[s]; rc[s] = rn[s]; }
-                ezc = ezn; Dc = Dn; dvc = dvn; ck = c1; cslotk = cslot1;
+                    for (int e = 0; e < VEC; e++) exh.a[e] = (e == VEC - 1) ? exr : exl.a[e == VEC - 1 ? e : e + 1];
+                }
+                const Vec<T> eyl = coef(cslotk + o_ey0), eyh = coef(cslotk + o_ey1);
+                Vec<T> ap;
+                T s_pv = T(0), s_dvv = T(0);
+#pragma unroll
+                for (int e = 0; e < VEC; e++) {
+                    const T pl = (e == 0) ? left : pc.a[e == 0 ? 0 : e - 1];
+                    const T pr = (e == VEC - 1) ? right : pc.a[e == VEC - 1 ? e : e + 1];
+                    // same order of operations as k_spmv_tma
+                    T v = D.a[e] * pc.a[e];
+                    v = fma(-exl.a[e], pl, v);
+                    v = fma(-exh.a[e], pr, v);
+                    v = fma(-eyl.a[e], up.a[e], v);
+                    T w = -eyh.a[e] * dn.a[e];
+                    w = fma(-ezc.a[e], pm.a[e], w);
+                    w = fma(-ezn.a[e], pn.a[e], w);
+                    v += w;
+                    if (e >= nvalid) v = T(0);     // pad column
+                    s_pv = fma(pc.a[e], v, s_pv);
+                    s_dvv = fma(dv.a[e] * v, v, s_dvv);
+                    ap.a[e] = v;
+                }
+                a_pAp += (double)(msk * s_pv);
+                a_S2 += (double)(msk * s_dvv);
+                if (active) {
+                    stv(q_out + gidx, ap);
+                    stv(p_out + gidx, pc);
+                }
+            };
+
+            Vec<T> Da, Db, dva, dvb, eza, ezb, pnv;
+            // item k0-1: the own column's p_new(k0-1) into plane buffer m; its coefficient slot goes back after a barrier
+            {
+                const uint32_t c0 = sm_cempty + 8u * cs;
+                update(pn_m, false, false, idx, pnv, Da, dva, eza);
+                cnext();
+                named_bar_sync(1, NCT);
+                if (tid == 0) mbar_arrive_a(c0);
             }
+            // item k0 -> plane buffer c;  D, Dinv, ez of plane k0 in set a
+            uint32_t ck = sm_cempty + 8u * cs;
+            uint32_t cslotk = update(pn_c, true, true, idx, pnv, Da, dva, eza);
+            cnext();
+            named_bar_sync(1, NCT);
+
+            // one step: update plane k+1 (set `n`), stencil of plane k (set `c`), barrier, hand the coefficient slot back
+            auto step = [&](int k, Vec<T> &Dc, Vec<T> &dvc, Vec<T> &ezc, Vec<T> &Dn, Vec<T> &dvn, Vec<T> &ezn) {
+                const uint32_t c1 = sm_cempty + 8u * cs;
+                const uint32_t cslot1 = update(pn_n, k + 1 < k1, true, idx + plane, pnv, Dn, dvn, ezn);
+                cnext();
+                stencil(cslotk, pn_m, pn_c, pnv, Dc, dvc, ezc, ezn, idx);
+                named_bar_sync(1, NCT);   // p_new(k+1) complete; everyone is done with coefficient slot ck and plane buffer m
+                if (tid == 0) mbar_arrive_a(ck);
+                ck = c1; cslotk = cslot1;
+                const uint32_t t = pn_m; pn_m = pn_c; pn_c = pn_n; pn_n = t;
+                idx += plane;
+            };
+            int k = k0;
+            for (; k + 1 < k1; k += 2) {
+                step(k, Da, dva, eza, Db, dvb, ezb);
+                step(k + 1, Db, dvb, ezb, Da, dva, eza);
+            }
+            if (k < k1) step(k, Da, dva, eza, Db, dvb, ezb);
             // coefficient item k1: only Dinv and ez of the own column were used, before the last barrier
-            if (tid == 0) mbar_arrive(&cempty[ck]);
+            if (tid == 0) mbar_arrive_a(ck);
         }
     }
 
     // stage 1 -> per-block partials; stage 2 by the last block to take a ticket (fixed order: deterministic); then every
-    // scalar of the iteration (header) and the stopping rule of step 3 (finish_iteration, pb_kernels.cuh)
+    // scalar of the iteration (header) and the stopping rule of step 3
     const int nblk = gridDim.x;
-#pragma unroll
-    for (int s = 0; s < M; s++)
+    {
+        const double sums[kFusedSums] = {a_pAp, a_S2, a_W, a_U1, a_U2};
 #pragma unroll
         for (int q = 0; q < kFusedSums; q++) {
-            const double t = block_sum(acc[s][q], red);
-            if (tid == 0) a.partials[((size_t)s * kFusedSums + q) * nblk + blockIdx.x] = t;
+            const double t = block_sum(sums[q], red);
+            if (tid == 0) a.partials[(size_t)q * nblk + blockIdx.x] = t;
         }
+    }
     if (tid == 0) {
         __threadfence();
         const unsigned int t = atomicAdd(&a.st->ticket_spmv, 1u);
@@ -445,32 +471,33 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
     __syncthreads();
     if (s_last) {
         __threadfence();
+        double sum[kFusedSums];
 #pragma unroll
-        for (int s = 0; s < M; s++) {
-            double sum[kFusedSums];
-#pragma unroll
-            for (int q = 0; q < kFusedSums; q++) sum[q] = final_sum(a.partials + ((size_t)s * kFusedSums + q) * nblk, nblk, red);
-            if (tid == 0 && live[s]) {
-                State *st = a.st + s;
-                const double pAp = sum[0], S1 = sum[1], S2 = sum[2], T1 = sum[3], T2 = sum[4], U1 = sum[5], U2 = sum[6];
-                st->pAp = pAp;
-                st->rz = U1;                                    // r_l.z_l and ||r_l||^2 of the stored r_l, exactly
-                st->rr = U2;
-                if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(U1) || !isfinite(U2)) {   // breakdown: not SPD / NaN
-                    if (st->latch) { st->done = 1; st->iters = st->iter_cur; st->status = 5; }
-                    st->alpha = 0.0;                            // x already holds the last good iterate
-                } else {
-                    const double alpha = U1 / pAp;              // step 5
-                    st->alpha = alpha;
-                    double rz_new = fma(alpha, fma(alpha, S2, -2.0 * S1), U1);     // r_{l+1}.z_{l+1}
-                    double rr_new = fma(alpha, fma(alpha, T2, -2.0 * T1), U2);     // ||r_{l+1}||^2
-                    if (rz_new < 0.0) rz_new = 0.0;             // cancellation at the rounding floor
-                    if (rr_new < 0.0) rr_new = 0.0;
-                    finish_iteration(st, rz_new, rr_new, 0);    // beta (step 7), l + 1 (step 4), stopping rule (step 3)
-                }
+        for (int q = 0; q < kFusedSums; q++) sum[q] = final_sum(a.partials + (size_t)q * nblk, nblk, red);
+        if (tid == 0) {
+            State *st = a.st;
+            st->ticket_spmv = 0u;
+            const double pAp = sum[0], S2 = sum[1], W = sum[2], U1 = sum[3], U2 = sum[4];
+            const int l = st->iter_cur;                         // this pass formed r_l and phi_l
+            st->pAp = pAp;
+            st->rz = U1;                                        // r_l.z_l and ||r_l||^2 of the stored r_l, exactly
+            st->rr = U2;
+            st->alpha = 0.0;                                    // unless another iteration follows: x = phi_l is final
+            if (st->latch && (!isfinite(U1) || !isfinite(U2))) { st->done = 1; st->iters = l; st->status = 5; }
+            else if (st->latch && (st->bb == 0.0 || U2 < st->tol2 * st->bb)) { st->done = 1; st->iters = l; st->status = 0; }  // step 3
+            else if (st->latch && l >= st->maxiter) { st->done = 1; st->iters = l; st->status = 6; }
+            else if (!(pAp > 0.0) || !isfinite(pAp)) {          // breakdown: not SPD / NaN; x holds the last good iterate
+                if (st->latch) { st->done = 1; st->iters = l; st->status = 5; }
+            } else {
+                const double al = U1 / pAp;                     // step 5
+                const double S1 = pAp - st->beta * W;           // z_l.A p_{l+1}
+                double rz_new = fma(al, fma(al, S2, -2.0 * S1), U1);   // r_{l+1}.z_{l+1}
+                if (rz_new < 0.0) rz_new = 0.0;                 // cancellation at the rounding floor
+                st->alpha = al;
+                st->beta = rz_new / U1;                         // step 7
+                st->iter_cur = l + 1;                           // step 4
             }
         }
-        if (tid == 0) a.st->ticket_spmv = 0u;
     }
 }
 
