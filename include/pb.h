@@ -273,7 +273,8 @@ typedef enum {
     PB_OPT_VEC_BLOCKS_PER_SM = 13,   /* k_vec blocks per SM (0 = automatic)                                          */
     PB_OPT_GRAPH = 14,               /* 1 (default): check_every iterations are launched as one CUDA graph           */
     PB_OPT_L2_HINTS = 15,            /* bit mask of L2 eviction-priority hints (default 0: none; measured not to help) */
-    PB_OPT_BATCH_WIDTH = 16,         /* right-hand sides per pass of pb_solve_batch: 1, 2 or 4 (default 2)            */
+    PB_OPT_BATCH_WIDTH = 16,         /* right-hand sides per kernel pass of pb_solve_batch: 1 (default: one member at a
+                                        time through k_pcg_fused, the fastest measured), 2 or 4 (k_spmv_batch + k_vec_batch) */
     PB_OPT_FUSED = 17,               /* 1 (default): pb_solve / pb_solve_batch run ONE kernel per iteration (k_pcg_fused:
                                         K_vec folded into the next K_spmv pass, 34 instead of 41 B per node); 0: K_spmv
                                         + K_vec.  Periodic boundary, warm starts, refinement, slabs and L2-resident

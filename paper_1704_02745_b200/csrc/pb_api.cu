@@ -160,7 +160,7 @@ void default_options(int *opt)
     opt[PB_OPT_PERSIST_BLOCKS_PER_SM] = 4; opt[PB_OPT_PALETTE] = 1; opt[PB_OPT_PALETTE_DIAG] = 1;
     opt[PB_OPT_PALETTE_DIAG_SPMV] = 1; opt[PB_OPT_AUTOTUNE] = 1; opt[PB_OPT_TILE_TXV] = 0; opt[PB_OPT_TILE_TY] = 0;
     opt[PB_OPT_TILE_TZ] = 0; opt[PB_OPT_RING_SLOTS] = 0; opt[PB_OPT_BLOCKS_PER_SM] = 0; opt[PB_OPT_VEC_BLOCKS_PER_SM] = 0;
-    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_BATCH_WIDTH] = 2; opt[PB_OPT_FUSED] = 1;
+    opt[PB_OPT_GRAPH] = 1; opt[PB_OPT_L2_HINTS] = 0; opt[PB_OPT_BATCH_WIDTH] = 1; opt[PB_OPT_FUSED] = 1;
 }
 
 inline int grid_for(size_t n, int block, int cap)
