@@ -113,6 +113,7 @@ struct pb_handle {
     int pal_n;                   // -1: not examined yet, 0: more than 256 distinct values, else the table size
     // pb_create_from_atoms keeps the atom geometry for pb_set_charges
     double *atoms_c;             // [n_atoms][3], device
+    double *atoms_q = nullptr;   // [n_atoms] charges + 2 doubles of scratch, device (pb_set_charges; allocated once)
     int n_atoms;
     double atoms_eps_out, atoms_kappa;
     bool dh_f32 = false;         // pb_set_charges evaluates the Debye-Hueckel boundary terms in fp32
@@ -1251,6 +1252,7 @@ pb_status pb_destroy(pb_handle *h)
     if (h->slab_send) cudaFree(h->slab_send);
     if (h->slab_recv) cudaFree(h->slab_recv);
     if (h->atoms_c) cudaFree(h->atoms_c);
+    if (h->atoms_q) cudaFree(h->atoms_q);
     if (h->pal_table) cudaFree(h->pal_table);
     if (h->pald_table) cudaFree(h->pald_table);
     if (h->pinned) cudaFreeHost(h->pinned);
@@ -1840,10 +1842,8 @@ extern "C" pb_status pb_set_charges(pb_handle *h, const double *charges, pb_mems
     PB_CUDA(cudaSetDevice(h->device));
     const size_t n = (size_t)h->nx * h->ny * h->nz;
     const size_t nbc = 2 * ((size_t)h->nz * h->ny + (size_t)h->nz * h->nx + (size_t)h->ny * h->nx);
-    DevTmp tmp;
-    double *d_q, *scratch;
-    PB_TRY(tmp.get((void **)&d_q, (size_t)h->n_atoms * sizeof(double)));
-    PB_TRY(tmp.get((void **)&scratch, 2 * sizeof(double)));
+    if (!h->atoms_q) PB_ALLOC(cudaMalloc((void **)&h->atoms_q, ((size_t)h->n_atoms + 2) * sizeof(double)));
+    double *d_q = h->atoms_q, *scratch = h->atoms_q + h->n_atoms;
     PB_CUDA(cudaMemcpyAsync(d_q, charges, (size_t)h->n_atoms * sizeof(double),
                             where == PB_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
     if (!h->rhs) PB_ALLOC(cudaMalloc((void **)&h->rhs, (n + 8) * sizeof(double)));
