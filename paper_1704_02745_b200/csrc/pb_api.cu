@@ -834,7 +834,7 @@ bool fused_eligible(pb_handle *h)
 {
     if (!h->opt[PB_OPT_FUSED] || h->periodic || h->slab) return false;
     if (ensure<T>(h) != PB_OK) return false;
-    return !work<T>(h).persist;
+    return !work<T>(h).persist && work<T>(h).npad < ((size_t)1 << 32);   // k_pcg_fused indexes elements with 32 bits
 }
 
 struct DevTmp {                      // frees its device allocations on scope exit

@@ -139,6 +139,11 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     const int max_ct = max_threads - 64;
     while (spmv_row_threads(b.TXV) * b.TY > max_ct && b.TY > 1) b.TY--;
     b.threads = (spmv_row_threads(b.TXV) * b.TY + 31) / 32 * 32 + 32;
+    if (fused) {       // k_pcg_fused: one halo cell per consumer thread at most
+        const int halo = (2 * b.TXV + 2 * b.TY + 31) / 32 * 32 + 32;
+        if (halo > b.threads) b.threads = halo;
+        if (b.threads > max_threads) return PB_ERR_INVALID_ARG;
+    }
     const FusedLayout FL = fused_layout(b.TXV, b.TY, VEC, b.quad, b.pald);
     const BatchLayout &L = FL.B;
     const long vslot = fused ? (long)FL.vslot : (long)L.vslot;
@@ -149,7 +154,8 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.nsv = 0;
     for (int t = 0; t < 3; t++) {
         const int bps = forced_bps > 0 ? forced_bps : try_bps[t], nsc = try_nsc[t];
-        const long fixed = (long)nsc * (long)L.cslot + (fused ? (long)kFusedPlanes : 2L * M) * (long)L.pn + 128;
+        const long fixed = (long)nsc * (long)L.cslot + (fused ? (long)kFusedPlanes : 2L * M) * (long)L.pn + 128 +
+                           (fused ? (long)fused_fixed_smem((int)sizeof(T), b.quad, b.pald) : 0L);
         long budget = (long)((size_t)232448 / bps) - 1024 - (long)((size_t)232448 - max_dyn) - fixed;   // per-SM share
         if ((long)max_dyn - fixed < budget) budget = (long)max_dyn - fixed;                              // per-block cap
         int nsv = budget > 0 ? (int)(budget / vslot) : 0;
@@ -159,7 +165,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     }
     if (o[PB_OPT_RING_SLOTS] > 0 && o[PB_OPT_RING_SLOTS] < b.nsv) b.nsv = o[PB_OPT_RING_SLOTS];
     if (b.nsv < 2) return PB_ERR_INVALID_ARG;
-    b.smem = fused ? fused_smem(FL, b.nsv, b.nsc) : batch_smem(L, b.nsv, b.nsc, M);
+    b.smem = fused ? fused_smem(FL, b.nsv, b.nsc, (int)sizeof(T), b.quad, b.pald) : batch_smem(L, b.nsv, b.nsc, M);
     b.ntx = (rowvecs + b.TXV - 1) / b.TXV;
     b.nty = (h->ny + b.TY - 1) / b.TY;
     const int slots = h->nsm * b.bps, xy = b.ntx * b.nty;
@@ -247,6 +253,8 @@ void launch_fused_kernels(pb_handle *h, Work<T> &w, int n_iter)
     a.TXV = b.TXV; a.TY = b.TY; a.TZ = b.TZ; a.ntx = b.ntx; a.nty = b.nty; a.ntz = b.ntz;
     a.ntiles = b.ntx * b.nty * b.ntz; a.nsv = b.nsv; a.nsc = b.nsc; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.lut = w.lut; a.dlut = w.dlut;
+    a.nct = b.threads - 32;
+    fused_args_layout(a, fused_layout(b.TXV, b.TY, VecN<T>::value, QUAD, PALD));
     for (int it = 0; it < n_iter; it++)
         k_pcg_fused<T, QUAD, PALD><<<b.grid, b.threads, b.smem, h->stream>>>(b.vm, b.tm_dinv, b.tm_x, b.tm_exm, b.tm_exp,
                                                                            b.tm_ey, b.tm_ez, a);

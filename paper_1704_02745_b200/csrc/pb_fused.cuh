@@ -24,12 +24,18 @@
 // in two kernels; r, p and A p are double-buffered (a neighbouring tile reads the old plane while this one writes).
 //
 // Structure: k_spmv_batch's (pb_spmv_batch.cuh) -- a vector ring {r, A p_l, p_l haloed, x} released right after the
-// update stage, a coefficient ring held one step longer -- with the per-thread state cut to the bone, because this
-// kernel is bound by instruction issue, not by bytes: p_new lives in THREE shared planes (k-1, k, k+1) and is re-read
-// from there instead of being rotated through registers; the step is unrolled twice so that D, Dinv and the z-face of
+// update stage, a coefficient ring held one step longer -- with the per-thread state cut to the bone (128 registers,
+// two blocks per SM): p_new lives in THREE shared planes (k-1, k, k+1) and is re-read from there instead of being
+// rotated through registers (measured: holding the own-cell values in registers costs spills and 8 % of the time); the step is unrolled twice so that D, Dinv and the z-face of
 // planes k / k+1 alternate between two register sets without moves; every shared address is a 32-bit slot base plus
-// a per-thread offset computed once; inactive lanes run the same instructions on in-range cells and are masked out
-// of the stores and the sums.
+// a per-thread offset computed once, the slot-internal offsets come ready-made from the host (FusedArgs, constant
+// bank) and the tables / barriers sit at compile-time offsets of the same window (FusedSm), so that nothing of the
+// layout is re-derived inside the loop; inactive lanes run the same instructions on in-range cells and are masked
+// out of the stores and the sums; the five sums are carried in fp32 over two planes (8 nodes) and then added to the
+// thread's fp64 accumulators.
+// Measured at 385^3 fp32 (profiles/r2_ncu_full_fused.txt): 651 K SM cycles per launch whatever the instruction count
+// (192 M warp instructions before this layout, 145 M with it): the pass runs at 5.8 TB/s of DRAM traffic at 1.93 GHz
+// (90 % of the measured copy rate) and follows the SM clock under the power cap (0.364 ms at 1.75 GHz).
 #pragma once
 #include "pb_internal.cuh"
 #include "pb_tma.cuh"
@@ -55,9 +61,26 @@ __host__ __device__ inline FusedLayout fused_layout(int TXV, int TY, int vec, bo
     F.vslot = F.oAq + align128(F.B.bZ);
     return F;
 }
-__host__ __device__ inline size_t fused_smem(const FusedLayout &F, int nsv, int nsc)
+
+// fixed part of the block's shared memory (byte offsets from the 128-byte aligned start of the dynamic window): the
+// mbarriers, the reduction scratch, the two lookup tables; the rings and the p_new planes follow at `ring`
+template <typename T, bool QUAD, bool PALD>
+struct FusedSm {
+    static constexpr uint32_t vfull = 0, vempty = 64, cfull = 128, cempty = 160;     // 8 + 8 + 4 + 4 mbarriers
+    static constexpr uint32_t red = 256, last = 512;
+    static constexpr uint32_t qtab = 640;                                            // [256][4] face values
+    static constexpr uint32_t ddtab = qtab + (QUAD ? 1024u * (uint32_t)sizeof(T) : 0u);   // [256] {Dinv, D}
+    static constexpr uint32_t ring = ddtab + (PALD ? 512u * (uint32_t)sizeof(T) : 0u);
+};
+static_assert(kMaxStages <= 8 && kMaxCoefStages <= 4, "FusedSm reserves 8 + 8 + 4 + 4 mbarriers");
+inline size_t fused_fixed_smem(int elt, bool quad, bool pald)
 {
-    return (size_t)nsv * F.vslot + (size_t)nsc * F.B.cslot + (size_t)kFusedPlanes * F.B.pn + 128;
+    return 640 + (quad ? (size_t)1024 * elt : 0) + (pald ? (size_t)512 * elt : 0);
+}
+inline size_t fused_smem(const FusedLayout &F, int nsv, int nsc, int elt, bool quad, bool pald)
+{
+    return fused_fixed_smem(elt, quad, pald) + (size_t)nsv * F.vslot + (size_t)nsc * F.B.cslot +
+           (size_t)kFusedPlanes * F.B.pn + 128;
 }
 
 template <typename T>
@@ -69,11 +92,26 @@ struct FusedArgs {
     int ntx, nty, ntz, ntiles;
     int nsv, nsc;
     int precond;
+    int nct;                 // consumer threads (whole warps); one more warp produces
+    // the slot layout (fused_layout), bytes: vector slot {r @0, A p @oQ, p @oP, x @oX}, coefficient slot
+    // {Dinv @0, ez @oEZ, ex- @oEXM, ex+ @oEXP, ey @oEY}, one p_new plane; box sizes for expect_tx
+    uint32_t vslot, cslot, pn, oQ, oP, oX, oEZ, oEXM, oEXP, oEY, bwq, bwd;
+    uint32_t bZ, bX, bDv, bEZ, bC;      // bC = the three in-plane face boxes together
     State *st;
     double *partials;        // [kFusedSums][gridDim.x]
     const T *lut;
     const T *dlut;
 };
+template <typename T>
+inline void fused_args_layout(FusedArgs<T> &a, const FusedLayout &F)
+{
+    const BatchLayout &L = F.B;
+    a.vslot = (uint32_t)F.vslot; a.cslot = (uint32_t)L.cslot; a.pn = (uint32_t)L.pn;
+    a.oQ = (uint32_t)F.oAq; a.oP = (uint32_t)L.oPp; a.oX = (uint32_t)L.oX;
+    a.oEZ = (uint32_t)L.oEZ; a.oEXM = (uint32_t)L.oEXM; a.oEXP = (uint32_t)L.oEXP; a.oEY = (uint32_t)L.oEY;
+    a.bwq = (uint32_t)L.bwq; a.bwd = (uint32_t)L.bwd;
+    a.bZ = L.bZ; a.bX = L.bX; a.bDv = L.bDv; a.bEZ = L.bEZ; a.bC = L.bEXM + L.bEXP + L.bEY;
+}
 
 // the six ping-pong vector tensors (4-D [1][nz][ny][P]) in one kernel parameter
 struct FusedMaps { CUtensorMap r0, r1, q0, q1, p0, p1; };
@@ -86,49 +124,50 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             const __grid_constant__ CUtensorMap tm_ez, const FusedArgs<T> a)
 {
     constexpr int VEC = VecN<T>::value;
-    extern __shared__ unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t vfull[kMaxStages], vempty[kMaxStages];
-    __shared__ __align__(8) uint64_t cfull[kMaxCoefStages], cempty[kMaxCoefStages];
-    __shared__ double red[32];
-    __shared__ int s_last;
-    __shared__ __align__(16) T qtab[QUAD ? 256 * 4 : 4];   // qtab[b][f] = lut[(b >> 2f) & 3]: four face values per byte
-    __shared__ __align__(16) T ddtab[PALD ? 512 : 2];      // {Dinv, D} pairs
+    constexpr uint32_t ES = (uint32_t)sizeof(T);
+    using SM = FusedSm<T, QUAD, PALD>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
 
     const int tid = threadIdx.x;
-    const int nthr = blockDim.x;
-    const int NCT = nthr - 32;                 // consumer threads (whole warps); the last warp produces
-    const int NCW = NCT >> 5;
+    const int NCT = a.nct;
     const int warp = tid >> 5, lane = tid & 31;
-    const bool is_producer = (warp == NCW);
+    const bool is_producer = (warp == (NCT >> 5));
 
     if (a.st->done) return;
     const T beta = (T)a.st->beta;              // beta_l:  p_{l+1} = z_l + beta_l p_l
     const T alpha = (T)a.st->alpha;            // alpha_l: r_l = r_{l-1} - alpha_l A p_l,  phi_l = phi_{l-1} + alpha_l p_l
     const int parity = a.st->iter_cur & 1;
 
-    const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
-    const int TXV = a.TXV, TY = a.TY, TZ = a.TZ, NSV = a.nsv, NSC = a.nsc;
-    const FusedLayout F = fused_layout(TXV, TY, VEC, QUAD, PALD);
-    const BatchLayout &L = F.B;
-    unsigned char *vbase = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-    unsigned char *cbase = vbase + (size_t)NSV * F.vslot;
-    unsigned char *pnbase = cbase + (size_t)NSC * L.cslot;
+    // sb: shared-window address of the block's 128-byte aligned area; gb: the same place as a generic pointer
+    const uint32_t sb = (smem_u32(smem_raw) + 127u) & ~127u;
+    unsigned char *const gb = smem_raw + (sb - smem_u32(smem_raw));
+    double *const red = reinterpret_cast<double *>(gb + SM::red);
+    int *const s_last = reinterpret_cast<int *>(gb + SM::last);
+    const uint32_t sm_v = sb + SM::ring;                           // vector ring
+    const uint32_t sm_c = sm_v + (uint32_t)a.nsv * a.vslot;        // coefficient ring
+    const uint32_t sm_pn = sm_c + (uint32_t)a.nsc * a.cslot;       // the three p_new planes
 
     if (tid == 0) {
-        for (int i = 0; i < NSV; i++) { mbar_init(&vfull[i], 1); mbar_init(&vempty[i], NCW); }
-        for (int i = 0; i < NSC; i++) { mbar_init(&cfull[i], 1); mbar_init(&cempty[i], 1); }
+        for (int i = 0; i < a.nsv; i++) { mbar_init_a(sb + SM::vfull + 8u * i, 1); mbar_init_a(sb + SM::vempty + 8u * i, NCT >> 5); }
+        for (int i = 0; i < a.nsc; i++) { mbar_init_a(sb + SM::cfull + 8u * i, 1); mbar_init_a(sb + SM::cempty + 8u * i, 1); }
         mbar_fence_init();
     }
-    if (QUAD)
-        for (int b = tid; b < 256; b += nthr) {
+    if (QUAD) {
+        T *qtab = reinterpret_cast<T *>(gb + SM::qtab);            // qtab[b][f] = lut[(b >> 2f) & 3]: four face values per byte
+        for (int b = tid; b < 256; b += blockDim.x) {
 #pragma unroll
             for (int f = 0; f < 4; f++) qtab[b * 4 + f] = a.lut[(b >> (2 * f)) & 3];
         }
-    if (PALD)
-        for (int i = tid; i < 256; i += nthr) { const T d = a.dlut[i]; ddtab[2 * i] = d; ddtab[2 * i + 1] = rcp_rn(d); }
+    }
+    if (PALD) {
+        T *ddtab = reinterpret_cast<T *>(gb + SM::ddtab);          // {Dinv, D} pairs
+        for (int i = tid; i < 256; i += blockDim.x) { const T d = a.dlut[i]; ddtab[2 * i] = d; ddtab[2 * i + 1] = rcp_rn(d); }
+    }
     __syncthreads();
 
     double a_pAp = 0.0, a_S2 = 0.0, a_W = 0.0, a_U1 = 0.0, a_U2 = 0.0;
+    const int nx = a.nx, ny = a.ny, nz = a.nz, P = a.P;
+    const int TXV = a.TXV, TY = a.TY, TZ = a.TZ;
 
     if (is_producer) {
         if (lane == 0) {
@@ -148,30 +187,27 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                     const bool centre = (q >= k0) && (q < k1);
                     const bool ez = (q >= k0);
                     {   // coefficient item q
-                        mbar_wait(&cempty[cs], cph ^ 1);
-                        unsigned char *slot = cbase + cs * (uint32_t)L.cslot;
-                        uint32_t bytes = L.bDv;
-                        if (ez) bytes += L.bEZ;
-                        if (centre) bytes += L.bEXM + L.bEXP + L.bEY;
-                        mbar_expect_tx(&cfull[cs], bytes);
-                        tma_load_3d(slot + L.oDv, &tm_dinv, xd, j0 - 1, q, &cfull[cs]);
-                        if (ez) tma_load_3d(slot + L.oEZ, &tm_ez, xq, j0, q, &cfull[cs]);
+                        const uint32_t full = sb + SM::cfull + 8u * cs, slot = sm_c + (uint32_t)cs * a.cslot;
+                        mbar_wait_a(full + (SM::cempty - SM::cfull), cph ^ 1);
+                        mbar_expect_tx_a(full, a.bDv + (ez ? a.bEZ : 0u) + (centre ? a.bC : 0u));
+                        tma_load_3d_a(slot, &tm_dinv, xd, j0 - 1, q, full);
+                        if (ez) tma_load_3d_a(slot + a.oEZ, &tm_ez, xq, j0, q, full);
                         if (centre) {
-                            tma_load_3d(slot + L.oEXM, &tm_exm, xq, j0, q, &cfull[cs]);
-                            if (QUAD) tma_load_3d(slot + L.oEXP, &tm_exp, xq, j0, q, &cfull[cs]);
-                            tma_load_3d(slot + L.oEY, &tm_ey, xq, j0, q, &cfull[cs]);
+                            tma_load_3d_a(slot + a.oEXM, &tm_exm, xq, j0, q, full);
+                            if (QUAD) tma_load_3d_a(slot + a.oEXP, &tm_exp, xq, j0, q, full);
+                            tma_load_3d_a(slot + a.oEY, &tm_ey, xq, j0, q, full);
                         }
-                        cs = (cs + 1 == NSC) ? 0 : cs + 1; cph ^= (cs == 0);
+                        cs = (cs + 1 == a.nsc) ? 0 : cs + 1; cph ^= (cs == 0);
                     }
                     {   // vector item q
-                        mbar_wait(&vempty[vs], vph ^ 1);
-                        unsigned char *slot = vbase + vs * (uint32_t)F.vslot;
-                        mbar_expect_tx(&vfull[vs], 3 * L.bZ + (centre ? L.bX : 0u));
-                        tma_load_4d(slot + L.oR, tr, x0 - VEC, j0 - 1, q, 0, &vfull[vs]);
-                        tma_load_4d(slot + F.oAq, tq, x0 - VEC, j0 - 1, q, 0, &vfull[vs]);
-                        tma_load_4d(slot + L.oPp, tp, x0 - VEC, j0 - 1, q, 0, &vfull[vs]);
-                        if (centre) tma_load_4d(slot + L.oX, &tm_x, x0, j0, q, 0, &vfull[vs]);
-                        vs = (vs + 1 == NSV) ? 0 : vs + 1; vph ^= (vs == 0);
+                        const uint32_t full = sb + SM::vfull + 8u * vs, slot = sm_v + (uint32_t)vs * a.vslot;
+                        mbar_wait_a(full + (SM::vempty - SM::vfull), vph ^ 1);
+                        mbar_expect_tx_a(full, 3 * a.bZ + (centre ? a.bX : 0u));
+                        tma_load_4d_a(slot, tr, x0 - VEC, j0 - 1, q, 0, full);
+                        tma_load_4d_a(slot + a.oQ, tq, x0 - VEC, j0 - 1, q, 0, full);
+                        tma_load_4d_a(slot + a.oP, tp, x0 - VEC, j0 - 1, q, 0, full);
+                        if (centre) tma_load_4d_a(slot + a.oX, &tm_x, x0, j0, q, 0, full);
+                        vs = (vs + 1 == a.nsv) ? 0 : vs + 1; vph ^= (vs == 0);
                     }
                 }
             }
@@ -179,40 +215,32 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         __syncwarp();
     } else {
         // ---- consumer warps ---------------------------------------------------------------------------------
-        const int BWc = TXV + 2;                       // vectors per row of the haloed boxes
+        const uint32_t BWc = (uint32_t)TXV + 2u;       // vectors per row of the haloed boxes
         const int TXP = spmv_row_threads(TXV);
         const int tx0 = tid % TXP, ty0 = tid / TXP;
         const bool intile = ty0 < TY && tx0 < TXV;
         // lanes outside the tile run the same instructions on cell (0, 0) of the tile and are masked out below
         const int tx = intile ? tx0 : 0, ty = intile ? ty0 : 0;
-        const int own = (ty + 1) * BWc + tx + 1;       // own cell in the haloed boxes
-        const int nextra = 2 * TXV + 2 * TY;           // halo cells: two rows, two columns
+        const uint32_t t_own = ((uint32_t)(ty + 1) * BWc + (uint32_t)tx + 1u) * 16u;   // own cell in a haloed box / p_new plane
+        const uint32_t t_c = (uint32_t)(ty * TXV + tx) * 16u;                          // own cell in an un-haloed box
+        const uint32_t t_xb = a.oX + t_c;
+        // halo cells (two rows, two columns): one per thread, from the last thread down (the host sizes the block so
+        // that the consumer threads cover them: nct >= 2 TXV + 2 TY)
+        const int nextra = 2 * TXV + 2 * TY;
         auto halo_cell = [&](int h) -> int {
             if (h < TXV) return h + 1;
-            if (h < 2 * TXV) return (TY + 1) * BWc + (h - TXV) + 1;
+            if (h < 2 * TXV) return (TY + 1) * (int)BWc + (h - TXV) + 1;
             const int cc = h - 2 * TXV, side = cc / TY, r = cc - side * TY;
-            return (r + 1) * BWc + (side ? TXV + 1 : 0);
+            return (r + 1) * (int)BWc + (side ? TXV + 1 : 0);
         };
-        auto cell_d = [&](int c) -> int { const int row = c / BWc; return row * L.bwd + (c - row * BWc) * VEC; };
-        const int extra0 = (NCT - 1 - tid < nextra) ? halo_cell(NCT - 1 - tid) : -1;   // this thread's halo cell
+        auto cell_d = [&](int c) -> uint32_t { const int row = c / (int)BWc; return (uint32_t)row * a.bwd + (uint32_t)(c - row * (int)BWc) * VEC; };
+        const int extra0 = (NCT - 1 - tid < nextra) ? halo_cell(NCT - 1 - tid) : -1;
         const bool has_x0 = extra0 >= 0;
-        const bool more_halo = nextra > NCT;           // only tiny tiles: the halo outnumbers the threads
+        const uint32_t t_dx = has_x0 ? (uint32_t)extra0 * 16u - t_own : 0u;            // the halo cell, relative to the own cell
         const bool precond = a.precond != 0;
-
-        const uint32_t sm_v = smem_u32(vbase), sm_c = smem_u32(cbase), sm_pn = smem_u32(pnbase);
-        const uint32_t sm_q = smem_u32(qtab), sm_dd = smem_u32(ddtab);
-        const uint32_t sm_vfull = smem_u32(vfull), sm_vempty = smem_u32(vempty), sm_cfull = smem_u32(cfull),
-                       sm_cempty = smem_u32(cempty);
-        const uint32_t vslot_b = (uint32_t)F.vslot, cslot_b = (uint32_t)L.cslot, pn_b = (uint32_t)L.pn;
-        const uint32_t o_own = (uint32_t)own * 16u;                    // own cell within a haloed vector box / p_new plane
-        const uint32_t o_x0 = has_x0 ? (uint32_t)extra0 * 16u : 0u;    // this thread's halo cell
-        const uint32_t o_r = (uint32_t)L.oR + o_own, o_q = (uint32_t)F.oAq + o_own, o_p = (uint32_t)L.oPp + o_own;
-        const uint32_t o_xbox = (uint32_t)L.oX + (uint32_t)(ty * TXV + tx) * 16u;
-        const uint32_t row16 = (uint32_t)BWc * 16u;
         T *const r_out = parity ? a.r0 : a.r1, *const q_out = parity ? a.Ap0 : a.Ap1, *const p_out = parity ? a.p0 : a.p1;
-        // per tile (the aligned starts of the byte boxes depend on x0)
-        uint32_t o_dv_own = 0, o_dv_x0 = 0, o_ez = 0, o_exm = 0, o_exp = 0, o_ey0 = 0, o_ey1 = 0, qfield = 0;
-        int lead_d = 0;
+        // per tile (the aligned starts of the byte boxes depend on x0): offsets within a coefficient slot
+        uint32_t t_dv = 0, t_dvx = 0, t_ez = 0, t_exm = 0, t_exp = 0, t_ey = 0, sbq = sb;
 
         // Dinv and D = 1/Dinv of VEC nodes: index bytes at `addr` -> pair table, or Dinv words at `addr`
         auto load_dinv = [&](uint32_t addr, Vec<T> &dinv, Vec<T> &D) {
@@ -220,7 +248,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                 const uint32_t w = (VEC == 4) ? lds_u32(addr) : lds_u16(addr);
 #pragma unroll
                 for (int e = 0; e < VEC; e++)
-                    lds_pair(dinv.a[e], D.a[e], sm_dd + ((w >> (8 * e)) & 255u) * (uint32_t)(2 * sizeof(T)));
+                    lds_pair_o<SM::ddtab>(dinv.a[e], D.a[e], sb + __byte_perm(w, 0u, 0x4440u | (uint32_t)e) * (2u * ES));
             } else {
                 lds_vec(dinv.a, addr);
 #pragma unroll
@@ -234,7 +262,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         // VEC face coefficients: quad byte at `addr` -> table of quadruples, or words at `addr`
         auto coef = [&](uint32_t addr) -> Vec<T> {
             Vec<T> v;
-            if (QUAD) lds_vec(v.a, sm_q + lds_u8(addr) * (uint32_t)(4 * sizeof(T)) + qfield);
+            if (QUAD) lds_vec_o<SM::qtab>(v.a, sbq + lds_u8(addr) * (4u * ES));
             else lds_vec(v.a, addr);
             return v;
         };
@@ -242,7 +270,11 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         // ring heads: slot index, phase parity and the slot's shared address, advanced together
         int vs = 0, cs = 0;
         uint32_t vph = 0, cph = 0, vaddr = sm_v, caddr = sm_c;
-        const size_t plane = (size_t)ny * P;
+        const uint32_t plane = (uint32_t)ny * (uint32_t)P;
+        // fp32: the sums over (at most) two planes, then added to the fp64 accumulators (flush); fp64: the thread's sums
+        // themselves (inactive lanes are masked where they are formed)
+        constexpr bool F32 = sizeof(T) == 4;
+        T s_pv = T(0), s_dvv = T(0), s_w = T(0), s_u1 = T(0), s_u2 = T(0);
 
         for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
             int b = tile;
@@ -252,54 +284,49 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             const int x0 = bx * TXV * VEC, j0 = by * TY;
             const int i0 = x0 + tx * VEC, j = j0 + ty;
             const bool active = intile && (i0 < P) && (j < ny);
-            const T msk = active ? T(1) : T(0);
             const int nvalid = active ? nx - i0 : 0;   // inactive lanes: A p = 0 (their Dinv may be a zero-filled 0, D = inf)
             const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
-            lead_d = (x0 - VEC) & 15;
             if (PALD) {
-                o_dv_own = (uint32_t)(L.oDv + lead_d + (ty + 1) * L.bwd + (tx + 1) * VEC);
-                o_dv_x0 = has_x0 ? (uint32_t)(L.oDv + lead_d + cell_d(extra0)) : 0u;
+                const uint32_t lead_d = (uint32_t)(x0 - VEC) & 15u;
+                t_dv = lead_d + (uint32_t)(ty + 1) * a.bwd + (uint32_t)(tx + 1) * VEC;
+                t_dvx = has_x0 ? lead_d + cell_d(extra0) : 0u;
             } else {
-                o_dv_own = (uint32_t)L.oDv + o_own;
-                o_dv_x0 = (uint32_t)L.oDv + o_x0;
+                t_dv = t_own;
+                t_dvx = t_own + t_dx;
             }
             if (QUAD) {
-                const uint32_t qoff = (uint32_t)((i0 >> 2) - ((x0 >> 2) & ~15));
-                qfield = (uint32_t)(i0 & 3) * (uint32_t)sizeof(T);
-                o_ez = (uint32_t)L.oEZ + (uint32_t)ty * L.bwq + qoff;
-                o_exm = (uint32_t)L.oEXM + (uint32_t)ty * L.bwq + qoff;
-                o_exp = (uint32_t)L.oEXP + (uint32_t)ty * L.bwq + qoff;
-                o_ey0 = (uint32_t)L.oEY + (uint32_t)ty * L.bwq + qoff;
-                o_ey1 = o_ey0 + (uint32_t)L.bwq;
+                const uint32_t t_q = (uint32_t)ty * a.bwq + (uint32_t)((i0 >> 2) - ((x0 >> 2) & ~15));
+                sbq = sb + (uint32_t)(i0 & 3) * ES;                    // fp64: which half of the quadruple
+                t_ez = a.oEZ + t_q; t_exm = a.oEXM + t_q; t_exp = a.oEXP + t_q; t_ey = a.oEY + t_q;
             } else {
-                o_ez = (uint32_t)L.oEZ + (uint32_t)(ty * TXV + tx) * 16u;
-                o_exm = (uint32_t)L.oEXM + (uint32_t)(ty * (TXV + 1) + tx) * 16u;
-                o_exp = o_exm + 16u;                                   // first element: the plus face of this vector's last node
-                o_ey0 = (uint32_t)L.oEY + (uint32_t)(ty * TXV + tx) * 16u;
-                o_ey1 = o_ey0 + (uint32_t)TXV * 16u;
+                t_ez = a.oEZ + t_c;
+                t_exm = a.oEXM + t_c + (uint32_t)ty * 16u;             // rows of TXV + 1 vectors
+                t_exp = t_exm + 16u;                                   // first element: the plus face of this vector's last node
+                t_ey = a.oEY + t_c;
             }
-            size_t idx = ((size_t)k0 * ny + j) * P + i0;               // (inactive lanes never use it)
+            const uint32_t ey_row = QUAD ? a.bwq : (uint32_t)TXV * 16u;
+            uint32_t gi = (uint32_t)((k0 * ny + j) * P + i0);          // element index (inactive lanes never use it)
             // own-cell addresses in the three p_new planes: plane q lives in buffer q mod 3, rotated as the march advances
-            uint32_t pn_m = sm_pn + o_own, pn_c = pn_m + pn_b, pn_n = pn_c + pn_b;
+            uint32_t pn_m = sm_pn + t_own, pn_c = pn_m + a.pn, pn_n = pn_c + a.pn;
 
             // "update" of the plane at the ring heads -> p_new plane whose own-cell address is `pnw`:
             // r_l = r_{l-1} - alpha_l A p_l, p_{l+1} = Dinv r_l + beta_l p_l on the own cell (returned; always stored into the plane)
             // and, for a plane this tile writes (centre), on the halo cells; r_l stored; the deferred phi update; the sums
             // U1, U2, W.  The vector slot is handed back; the coefficient slot stays (its address is returned).
-            auto update = [&](uint32_t pnw, bool centre, bool want_ez, size_t gidx, Vec<T> &pnew, Vec<T> &Dout, Vec<T> &dvout,
+            auto update = [&](uint32_t pnw, bool centre, bool want_ez, uint32_t gidx, Vec<T> &pnew, Vec<T> &Dout, Vec<T> &dvout,
                               Vec<T> &ezout) -> uint32_t {
-                mbar_wait_a(sm_cfull + 8u * cs, cph);
+                mbar_wait_a(sb + SM::cfull + 8u * cs, cph);
                 const uint32_t cslot = caddr;
                 Vec<T> dvh, dummy;
-                load_dinv(cslot + o_dv_own, dvout, Dout);
-                if (centre && has_x0) load_dinv(cslot + o_dv_x0, dvh, dummy);
-                if (want_ez) ezout = coef(cslot + o_ez);
-                mbar_wait_a(sm_vfull + 8u * vs, vph);
-                const uint32_t sl = vaddr;
+                load_dinv(cslot + t_dv, dvout, Dout);
+                if (centre && has_x0) load_dinv(cslot + t_dvx, dvh, dummy);
+                if (want_ez) ezout = coef(cslot + t_ez);
+                mbar_wait_a(sb + SM::vfull + 8u * vs, vph);
+                const uint32_t sl = vaddr + t_own;
                 Vec<T> rl, qv, pv;
-                lds_vec(rl.a, sl + o_r);
-                lds_vec(qv.a, sl + o_q);
-                lds_vec(pv.a, sl + o_p);
+                lds_vec(rl.a, sl);
+                lds_vec(qv.a, sl + a.oQ);
+                lds_vec(pv.a, sl + a.oP);
 #pragma unroll
                 for (int e = 0; e < VEC; e++) {
                     rl.a[e] = fma(-alpha, qv.a[e], rl.a[e]);                   // r_l (the deferred step 5)
@@ -308,86 +335,67 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                 sts_vec(pnw, pnew.a);
                 if (centre) {
                     Vec<T> xv;
-                    lds_vec(xv.a, sl + o_xbox);
-                    T s_u1 = T(0), s_u2 = T(0), s_w = T(0);
+                    lds_vec(xv.a, vaddr + t_xb);
 #pragma unroll
-                    for (int e = 0; e < VEC; e++) {
-                        xv.a[e] = fma(alpha, pv.a[e], xv.a[e]);                // phi_l = phi_{l-1} + alpha_l p_l
-                        s_u1 = fma(dvout.a[e] * rl.a[e], rl.a[e], s_u1);        // r_l.z_l
-                        s_u2 = fma(rl.a[e], rl.a[e], s_u2);                     // ||r_l||^2
-                        s_w = fma(qv.a[e], pnew.a[e], s_w);                     // (A p_l).p_{l+1}
+                    for (int e = 0; e < VEC; e++) xv.a[e] = fma(alpha, pv.a[e], xv.a[e]);   // phi_l = phi_{l-1} + alpha_l p_l
+                    if (F32 || active) {
+#pragma unroll
+                        for (int e = 0; e < VEC; e++) {
+                            s_u1 = fma(dvout.a[e] * rl.a[e], rl.a[e], s_u1);    // r_l.z_l
+                            s_u2 = fma(rl.a[e], rl.a[e], s_u2);                 // ||r_l||^2
+                            s_w = fma(qv.a[e], pnew.a[e], s_w);                 // (A p_l).p_{l+1}
+                        }
                     }
-                    a_U1 += (double)(msk * s_u1);
-                    a_U2 += (double)(msk * s_u2);
-                    a_W += (double)(msk * s_w);
                     if (active) {
                         stv(r_out + gidx, rl);
                         stv(a.x + gidx, xv);
                     }
                     if (has_x0) {
-                        const uint32_t h0 = sl + o_x0 - o_own;                  // (o_r etc. include the own-cell offset)
+                        const uint32_t h0 = sl + t_dx;
                         Vec<T> r2, q2, p2;
-                        lds_vec(r2.a, h0 + o_r);
-                        lds_vec(q2.a, h0 + o_q);
-                        lds_vec(p2.a, h0 + o_p);
+                        lds_vec(r2.a, h0);
+                        lds_vec(q2.a, h0 + a.oQ);
+                        lds_vec(p2.a, h0 + a.oP);
 #pragma unroll
                         for (int e = 0; e < VEC; e++) {
                             r2.a[e] = fma(-alpha, q2.a[e], r2.a[e]);
                             r2.a[e] = fma(beta, p2.a[e], dvh.a[e] * r2.a[e]);
                         }
-                        sts_vec(pnw + o_x0 - o_own, r2.a);
-                    }
-                    if (more_halo) {
-                        for (int h = NCT - 1 - tid + NCT; h < nextra; h += NCT) {
-                            const int c = halo_cell(h);
-                            const uint32_t oc = (uint32_t)c * 16u;
-                            Vec<T> d2, r2, q2, p2;
-                            load_dinv(cslot + (PALD ? (uint32_t)(L.oDv + lead_d + cell_d(c)) : (uint32_t)L.oDv + oc), d2, dummy);
-                            lds_vec(r2.a, sl + oc - o_own + o_r);
-                            lds_vec(q2.a, sl + oc - o_own + o_q);
-                            lds_vec(p2.a, sl + oc - o_own + o_p);
-#pragma unroll
-                            for (int e = 0; e < VEC; e++) {
-                                r2.a[e] = fma(-alpha, q2.a[e], r2.a[e]);
-                                r2.a[e] = fma(beta, p2.a[e], d2.a[e] * r2.a[e]);
-                            }
-                            sts_vec(pnw + oc - o_own, r2.a);
-                        }
+                        sts_vec(pnw + t_dx, r2.a);
                     }
                 }
                 consume(pnew.a[0]);         // r, A p and p of the own cell have been read (x, halo: the stores above)
                 __syncwarp();
-                if (lane == 0) mbar_arrive_a(sm_vempty + 8u * vs);
-                vs++; vaddr += vslot_b;
-                if (vs == NSV) { vs = 0; vaddr = sm_v; vph ^= 1u; }
+                if (lane == 0) mbar_arrive_o<SM::vempty>(sb + 8u * vs);
+                vs++; vaddr += a.vslot;
+                if (vs == a.nsv) { vs = 0; vaddr = sm_v; vph ^= 1u; }
                 return cslot;
             };
-            auto cnext = [&]() { cs++; caddr += cslot_b; if (cs == NSC) { cs = 0; caddr = sm_c; cph ^= 1u; } };
+            auto cnext = [&]() { cs++; caddr += a.cslot; if (cs == a.nsc) { cs = 0; caddr = sm_c; cph ^= 1u; } };
 
             // the stencil of plane k: p_new(k) from plane buffer pc_a (own cell, in-plane neighbours), p_new(k-1) from pm_a,
             // p_new(k+1) = pn (fresh from the update); coefficient slot cslotk; D, Dinv, ez of plane k and ez of plane k+1
             auto stencil = [&](uint32_t cslotk, uint32_t pm_a, uint32_t pc_a, const Vec<T> &pn, const Vec<T> &D, const Vec<T> &dv,
-                               const Vec<T> &ezc, const Vec<T> &ezn, size_t gidx) {
+                               const Vec<T> &ezc, const Vec<T> &ezn, uint32_t gidx) {
                 Vec<T> pc, pm, up, dn, exh;
                 T left, right;
                 lds_vec(pc.a, pc_a);
                 lds_vec(pm.a, pm_a);
-                lds_vec(up.a, pc_a - row16);
-                lds_vec(dn.a, pc_a + row16);
-                lds_one(left, pc_a - (uint32_t)sizeof(T));
-                lds_one(right, pc_a + 16u);
-                const Vec<T> exl = coef(cslotk + o_exm);
+                lds_vec(up.a, pc_a - BWc * 16u);
+                lds_vec(dn.a, pc_a + BWc * 16u);
+                lds_one_o<-(int)sizeof(T)>(left, pc_a);
+                lds_one_o<16>(right, pc_a);
+                const Vec<T> exl = coef(cslotk + t_exm);
                 if (QUAD) {
-                    exh = coef(cslotk + o_exp);
+                    exh = coef(cslotk + t_exp);
                 } else {
                     T exr;
-                    lds_one(exr, cslotk + o_exp);
+                    lds_one(exr, cslotk + t_exp);
 #pragma unroll
                     for (int e = 0; e < VEC; e++) exh.a[e] = (e == VEC - 1) ? exr : exl.a[e == VEC - 1 ? e : e + 1];
                 }
-                const Vec<T> eyl = coef(cslotk + o_ey0), eyh = coef(cslotk + o_ey1);
+                const Vec<T> eyl = coef(cslotk + t_ey), eyh = coef(cslotk + t_ey + ey_row);
                 Vec<T> ap;
-                T s_pv = T(0), s_dvv = T(0);
 #pragma unroll
                 for (int e = 0; e < VEC; e++) {
                     const T pl = (e == 0) ? left : pc.a[e == 0 ? 0 : e - 1];
@@ -400,56 +408,73 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                     T w = -eyh.a[e] * dn.a[e];
                     w = fma(-ezc.a[e], pm.a[e], w);
                     w = fma(-ezn.a[e], pn.a[e], w);
-                    v += w;
-                    if (e >= nvalid) v = T(0);     // pad column
-                    s_pv = fma(pc.a[e], v, s_pv);
-                    s_dvv = fma(dv.a[e] * v, v, s_dvv);
-                    ap.a[e] = v;
+                    ap.a[e] = v + w;
                 }
-                a_pAp += (double)(msk * s_pv);
-                a_S2 += (double)(msk * s_dvv);
+                if (nvalid < VEC) {                    // pad columns (and inactive lanes): A p = 0
+#pragma unroll
+                    for (int e = 0; e < VEC; e++) if (e >= nvalid) ap.a[e] = T(0);
+                }
+                if (F32 || active) {
+#pragma unroll
+                    for (int e = 0; e < VEC; e++) {
+                        s_pv = fma(pc.a[e], ap.a[e], s_pv);
+                        s_dvv = fma(dv.a[e] * ap.a[e], ap.a[e], s_dvv);
+                    }
+                }
                 if (active) {
                     stv(q_out + gidx, ap);
                     stv(p_out + gidx, pc);
+                }
+            };
+            // the two-plane sums -> the thread's fp64 accumulators
+            auto flush = [&]() {
+                if (F32) {
+                    if (active) {
+                        a_pAp += (double)s_pv; a_S2 += (double)s_dvv; a_W += (double)s_w; a_U1 += (double)s_u1; a_U2 += (double)s_u2;
+                    }
+                    s_pv = T(0); s_dvv = T(0); s_w = T(0); s_u1 = T(0); s_u2 = T(0);
                 }
             };
 
             Vec<T> Da, Db, dva, dvb, eza, ezb, pnv;
             // item k0-1: the own column's p_new(k0-1) into plane buffer m; its coefficient slot goes back after a barrier
             {
-                const uint32_t c0 = sm_cempty + 8u * cs;
-                update(pn_m, false, false, idx, pnv, Da, dva, eza);
+                const uint32_t c0 = sb + SM::cempty + 8u * cs;
+                update(pn_m, false, false, gi, pnv, Da, dva, eza);
                 cnext();
                 named_bar_sync(1, NCT);
                 if (tid == 0) mbar_arrive_a(c0);
             }
             // item k0 -> plane buffer c;  D, Dinv, ez of plane k0 in set a
-            uint32_t ck = sm_cempty + 8u * cs;
-            uint32_t cslotk = update(pn_c, true, true, idx, pnv, Da, dva, eza);
+            uint32_t ck = sb + SM::cempty + 8u * cs;
+            uint32_t cslotk = update(pn_c, true, true, gi, pnv, Da, dva, eza);
             cnext();
             named_bar_sync(1, NCT);
 
             // one step: update plane k+1 (set `n`), stencil of plane k (set `c`), barrier, hand the coefficient slot back
             auto step = [&](int k, Vec<T> &Dc, Vec<T> &dvc, Vec<T> &ezc, Vec<T> &Dn, Vec<T> &dvn, Vec<T> &ezn) {
-                const uint32_t c1 = sm_cempty + 8u * cs;
-                const uint32_t cslot1 = update(pn_n, k + 1 < k1, true, idx + plane, pnv, Dn, dvn, ezn);
+                const uint32_t c1 = sb + SM::cempty + 8u * cs;
+                const uint32_t cslot1 = update(pn_n, k + 1 < k1, true, gi + plane, pnv, Dn, dvn, ezn);
                 cnext();
-                stencil(cslotk, pn_m, pn_c, pnv, Dc, dvc, ezc, ezn, idx);
+                stencil(cslotk, pn_m, pn_c, pnv, Dc, dvc, ezc, ezn, gi);
                 named_bar_sync(1, NCT);   // p_new(k+1) complete; everyone is done with coefficient slot ck and plane buffer m
                 if (tid == 0) mbar_arrive_a(ck);
                 ck = c1; cslotk = cslot1;
                 const uint32_t t = pn_m; pn_m = pn_c; pn_c = pn_n; pn_n = t;
-                idx += plane;
+                gi += plane;
             };
             int k = k0;
             for (; k + 1 < k1; k += 2) {
                 step(k, Da, dva, eza, Db, dvb, ezb);
                 step(k + 1, Db, dvb, ezb, Da, dva, eza);
+                flush();
             }
             if (k < k1) step(k, Da, dva, eza, Db, dvb, ezb);
+            flush();
             // coefficient item k1: only Dinv and ez of the own column were used, before the last barrier
             if (tid == 0) mbar_arrive_a(ck);
         }
+        if (!F32) { a_pAp = (double)s_pv; a_S2 = (double)s_dvv; a_W = (double)s_w; a_U1 = (double)s_u1; a_U2 = (double)s_u2; }
     }
 
     // stage 1 -> per-block partials; stage 2 by the last block to take a ticket (fixed order: deterministic); then every
@@ -466,10 +491,10 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
     if (tid == 0) {
         __threadfence();
         const unsigned int t = atomicAdd(&a.st->ticket_spmv, 1u);
-        s_last = (t == (unsigned int)(nblk - 1));
+        *s_last = (t == (unsigned int)(nblk - 1));
     }
     __syncthreads();
-    if (s_last) {
+    if (*s_last) {
         __threadfence();
         double sum[kFusedSums];
 #pragma unroll

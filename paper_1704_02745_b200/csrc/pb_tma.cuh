@@ -132,6 +132,45 @@ __device__ __forceinline__ void mbar_wait_a(uint32_t addr, uint32_t parity) {
     } while (!ok);
 }
 
+// ---- by-address variants (32-bit shared-window addresses; OFF folds into the instruction's immediate) ----------
+__device__ __forceinline__ void mbar_init_a(uint32_t addr, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(addr), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_a(uint32_t addr, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(addr), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d_a(uint32_t dst, const CUtensorMap *tm, int c0, int c1, int c2, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d_a(uint32_t dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+template <int OFF> __device__ __forceinline__ void lds_vec_o(float (&v)[4], uint32_t addr) {
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];" : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "r"(addr), "n"(OFF));
+}
+template <int OFF> __device__ __forceinline__ void lds_vec_o(double (&v)[2], uint32_t addr) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr), "n"(OFF));
+}
+template <int OFF> __device__ __forceinline__ void lds_pair_o(float &a, float &b, uint32_t addr) {
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(a), "=f"(b) : "r"(addr), "n"(OFF));
+}
+template <int OFF> __device__ __forceinline__ void lds_pair_o(double &a, double &b, uint32_t addr) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(a), "=d"(b) : "r"(addr), "n"(OFF));
+}
+template <int OFF> __device__ __forceinline__ void lds_one_o(float &v, uint32_t addr) {
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(addr), "n"(OFF));
+}
+template <int OFF> __device__ __forceinline__ void lds_one_o(double &v, uint32_t addr) {
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(addr), "n"(OFF));
+}
+template <int OFF> __device__ __forceinline__ void mbar_arrive_o(uint32_t addr) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0+%1];" ::"r"(addr), "n"(OFF) : "memory");
+}
+
 // order this thread's generic-proxy shared-memory accesses before later async-proxy (TMA) writes
 __device__ __forceinline__ void fence_proxy_async() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
