@@ -28,6 +28,10 @@ struct BatchWork {
     int cap = 0;                                   // members the vector arrays hold
     T *r = nullptr, *x = nullptr, *p0 = nullptr, *p1 = nullptr, *Ap = nullptr, *b = nullptr;
     T *r2 = nullptr, *Ap2 = nullptr;               // fused iteration (k_pcg_fused): second buffers of r and A p
+    T *vblock = nullptr;                           // the one allocation behind r, Ap, p0, x, r2, Ap2, p1, x2 (in this order)
+    T *x2 = nullptr;                               // fused iteration: second buffer of x (State::xbuf names the current one)
+    unsigned char *cq4 = nullptr;                  // k_pcg_fused: {ez, ex-, ex+, ey} quad indices as one array
+    CUtensorMap tm_q4;
     bool fused = false;                            // the plan / maps / graph below are the fused kernel's
     FusedMaps vm;
     bool coef_ready = false, quad = false, pald = false, own_words = false;
@@ -183,9 +187,10 @@ pb_status alloc_arr(T **p, size_t n)
 template <typename T>
 void free_batch(BatchWork<T> &b)
 {
-    T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b, &b.r2, &b.Ap2};
-    for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
-    unsigned char **idx[] = {&b.exq, &b.exqp, &b.eyq, &b.ezq, &b.dviu};
+    if (b.vblock) cudaFree(b.vblock);
+    if (b.b) cudaFree(b.b);
+    b.vblock = b.b = b.r = b.x = b.p0 = b.p1 = b.Ap = b.r2 = b.Ap2 = b.x2 = nullptr;
+    unsigned char **idx[] = {&b.exq, &b.exqp, &b.eyq, &b.ezq, &b.dviu, &b.cq4};
     for (unsigned char **a : idx) { if (*a) cudaFree(*a); *a = nullptr; }
     if (b.own_words) { T **wa[] = {&b.exm, &b.eym, &b.ezm}; for (T **a : wa) { if (*a) cudaFree(*a); } }
     b.exm = b.eym = b.ezm = nullptr;
@@ -934,7 +939,8 @@ pb_status solve_impl(pb_handle *h, double tol, int maxiter, int check_every, voi
     T *dst = (T *)phi_out;
     if (where == PB_HOST) { PB_TRY(ensure_stage(h, n * sizeof(T))); dst = (T *)h->stage; }
     if (h->last_fused)
-        k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.bw.x, w.bw.p0, w.bw.p1, h->st, dst, h->nx, w.P, rows);
+        k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.bw.x, w.bw.p0, w.bw.p1, h->st, dst, h->nx, w.P, rows,
+                                                                             w.bw.x2);
     else
         k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(w.x, w.p0, w.p1, h->st, dst, h->nx, w.P, rows);
     PB_CUDA(cudaGetLastError());
@@ -1693,7 +1699,8 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
                 PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
                 PB_CUDA(cudaStreamSynchronize(h->stream));
                 const int par = h->pinned_state->iter_cur & 1;
-                const float *fs[] = {par ? w.bw.r2 : w.bw.r, nullptr, par ? w.bw.p1 : w.bw.p0, par ? w.bw.Ap2 : w.bw.Ap, w.bw.x};
+                const float *fs[] = {par ? w.bw.r2 : w.bw.r, nullptr, par ? w.bw.p1 : w.bw.p0, par ? w.bw.Ap2 : w.bw.Ap,
+                                     h->pinned_state->xbuf ? w.bw.x2 : w.bw.x};
                 sp = fs[what - 3];
             }
             if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
@@ -1708,7 +1715,8 @@ pb_status pb_query(pb_handle *h, int what, double *out_host)
                 PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));
                 PB_CUDA(cudaStreamSynchronize(h->stream));
                 const int par = h->pinned_state->iter_cur & 1;
-                const double *fs[] = {par ? w.bw.r2 : w.bw.r, nullptr, par ? w.bw.p1 : w.bw.p0, par ? w.bw.Ap2 : w.bw.Ap, w.bw.x};
+                const double *fs[] = {par ? w.bw.r2 : w.bw.r, nullptr, par ? w.bw.p1 : w.bw.p0, par ? w.bw.Ap2 : w.bw.Ap,
+                                     h->pinned_state->xbuf ? w.bw.x2 : w.bw.x};
                 sp = fs[what - 3];
             }
             if (!sp) { PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));

@@ -5,19 +5,36 @@
 
 // 4-D tensor [M][planes][rows][P] of T (member = coordinate 3), box = bx elements x by rows x 1 plane x 1 member
 template <typename T>
-pb_status make_map4(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, int members, int bx, int by)
+pb_status make_map4(CUtensorMap *tm, const T *ptr, int P, int rows, int planes, int members, int bx, int by, int bm = 1,
+                    size_t member_stride = 0)       // elements between two members (0: dense, P * rows * planes)
 {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return PB_ERR_CUDA;
     const cuuint64_t dims[4] = {(cuuint64_t)P, (cuuint64_t)rows, (cuuint64_t)planes, (cuuint64_t)members};
     const cuuint64_t strides[3] = {(cuuint64_t)P * sizeof(T), (cuuint64_t)P * rows * sizeof(T),
-                                   (cuuint64_t)P * rows * planes * sizeof(T)};
-    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, 1u};
+                                   (cuuint64_t)(member_stride ? member_stride : (size_t)P * rows * planes) * sizeof(T)};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, (cuuint32_t)bm};
     const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     const CUresult r = fn(tm, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4,
                           (void *)ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? PB_OK : PB_ERR_CUDA;
+}
+
+// 4-D byte tensor [members][planes][rows][Pb], box = bw bytes x by rows x 1 plane x bm members
+inline pb_status make_map4_u8(CUtensorMap *tm, const unsigned char *ptr, int Pb, int rows, int planes, int members, int bw,
+                              int by, int bm)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return PB_ERR_CUDA;
+    const cuuint64_t dims[4] = {(cuuint64_t)Pb, (cuuint64_t)rows, (cuuint64_t)planes, (cuuint64_t)members};
+    const cuuint64_t strides[3] = {(cuuint64_t)Pb, (cuuint64_t)Pb * rows, (cuuint64_t)Pb * rows * planes};
+    const cuuint32_t box[4] = {(cuuint32_t)bw, (cuuint32_t)by, 1u, (cuuint32_t)bm};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, (void *)ptr, dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? PB_OK : PB_ERR_CUDA;
 }
 
@@ -106,12 +123,25 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
         b.coef_ready = true;
     }
     if (b.cap < M) {
-        T **arrs[] = {&b.r, &b.x, &b.p0, &b.p1, &b.Ap, &b.b, &b.r2, &b.Ap2};
-        for (T **a : arrs) { if (*a) cudaFree(*a); *a = nullptr; }
+        if (b.vblock) cudaFree(b.vblock);
+        if (b.b) cudaFree(b.b);
+        b.vblock = b.b = nullptr;
         b.cap = 0; b.M = 0;
-        for (T **a : arrs)
-            if ((s = alloc_arr(a, (size_t)M * w.npad))) { free_batch(b); return s; }
+        // one allocation, buffer set 0 then buffer set 1: the four arrays of a set are consecutive (k_pcg_fused fetches
+        // their boxes with one TMA instruction, pb_fused.cuh)
+        const size_t each = (size_t)M * w.npad;
+        if ((s = alloc_arr(&b.vblock, 8 * each)) || (s = alloc_arr(&b.b, each))) { free_batch(b); return s; }
+        b.r = b.vblock; b.Ap = b.r + each; b.p0 = b.Ap + each; b.x = b.p0 + each;
+        b.r2 = b.x + each; b.Ap2 = b.r2 + each; b.p1 = b.Ap2 + each; b.x2 = b.p1 + each;
         b.cap = M;
+    }
+    if (fused && b.quad && !b.cq4) {
+        const size_t one = (size_t)(h->nz + 1) * (h->ny + 1) * b.Pq;
+        if ((s = alloc_arr(&b.cq4, 4 * one))) { free_batch(b); return s; }
+        k_setup_quad4<<<grid_for(one, 256, h->nsm * 16), 256, 0, h->stream>>>(h->eps_x, h->eps_y, h->eps_z, h->nx, h->ny, h->nz,
+                                                                               b.Pq, h->pal_table, b.cq4);
+        PB_CUDA(cudaGetLastError());
+        h->launches += 1;
     }
     if (b.M == M && b.fused == fused) return PB_OK;
     if (b.graph) { cudaGraphExecDestroy(b.graph); b.graph = nullptr; }
@@ -147,6 +177,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     const FusedLayout FL = fused_layout(b.TXV, b.TY, VEC, b.quad, b.pald);
     const BatchLayout &L = FL.B;
     const long vslot = fused ? (long)FL.vslot : (long)L.vslot;
+    const long cslot = fused ? (long)FL.cslot : (long)L.cslot, pnb = fused ? (long)FL.pn : (long)L.pn;
     // blocks per SM / coefficient ring depth: the first combination that leaves the vector ring M + 2 slots (the
     // consumers work on one member's plane while M more are in flight), else the one with the deepest vector ring
     const int forced_bps = o[PB_OPT_BLOCKS_PER_SM];
@@ -154,7 +185,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.nsv = 0;
     for (int t = 0; t < 3; t++) {
         const int bps = forced_bps > 0 ? forced_bps : try_bps[t], nsc = try_nsc[t];
-        const long fixed = (long)nsc * (long)L.cslot + (fused ? (long)kFusedPlanes : 2L * M) * (long)L.pn + 128 +
+        const long fixed = (long)nsc * cslot + (fused ? (long)kFusedPlanes : 2L * M) * pnb + 128 +
                            (fused ? (long)fused_fixed_smem((int)sizeof(T), b.quad, b.pald) : 0L);
         long budget = (long)((size_t)232448 / bps) - 1024 - (long)((size_t)232448 - max_dyn) - fixed;   // per-SM share
         if ((long)max_dyn - fixed < budget) budget = (long)max_dyn - fixed;                              // per-block cap
@@ -195,11 +226,11 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     PB_TRY(make_map4<T>(&b.tm_p0, b.p0, w.P, h->ny, h->nz, M, hx, hy));
     PB_TRY(make_map4<T>(&b.tm_p1, b.p1, w.P, h->ny, h->nz, M, hx, hy));
     PB_TRY(make_map4<T>(&b.tm_x, b.x, w.P, h->ny, h->nz, M, b.TXV * VEC, b.TY));
-    if (fused) {
-        b.vm.r0 = b.tm_r; b.vm.p0 = b.tm_p0; b.vm.p1 = b.tm_p1;
-        PB_TRY(make_map4<T>(&b.vm.r1, b.r2, w.P, h->ny, h->nz, M, hx, hy));
-        PB_TRY(make_map4<T>(&b.vm.q0, b.Ap, w.P, h->ny, h->nz, M, hx, hy));
-        PB_TRY(make_map4<T>(&b.vm.q1, b.Ap2, w.P, h->ny, h->nz, M, hx, hy));
+    if (fused) {       // M = 1: (r, Ap, p0, x) and (r2, Ap2, p1, x2) as four members each
+        const size_t each = (size_t)b.cap * w.npad;                  // the arrays were sized for b.cap members
+        PB_TRY(make_map4<T>(&b.vm.set0, b.r, w.P, h->ny, h->nz, 4, hx, hy, 4, each));
+        PB_TRY(make_map4<T>(&b.vm.set1, b.r2, w.P, h->ny, h->nz, 4, hx, hy, 4, each));
+        if (b.quad) PB_TRY(make_map4_u8(&b.tm_q4, b.cq4, b.Pq, h->ny + 1, h->nz + 1, 4, L.bwq, b.TY + 1, 4));
     }
     if (b.pald) PB_TRY(make_map_u8(&b.tm_dinv, b.dviu, w.Pb, h->ny, h->nz, L.bwd, hy));
     else PB_TRY(make_map<T>(&b.tm_dinv, w.Dinv, w.P, h->ny, h->nz, hx, hy));
@@ -214,6 +245,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
         PB_TRY(make_map<T>(&b.tm_ey, b.eym, w.P, h->ny + 1, h->nz, b.TXV * VEC, b.TY + 1));
         PB_TRY(make_map<T>(&b.tm_ez, b.ezm, w.P, h->ny, h->nz + 1, b.TXV * VEC, b.TY));
     }
+    if (fused && !b.quad) b.tm_q4 = b.tm_dinv;       // word format: the merged quad box does not exist (never fetched)
     b.M = M;
     b.fused = fused;
     if (verbose())
@@ -248,16 +280,17 @@ void launch_fused_kernels(pb_handle *h, Work<T> &w, int n_iter)
 {
     BatchWork<T> &b = w.bw;
     FusedArgs<T> a;
-    a.r0 = b.r; a.r1 = b.r2; a.Ap0 = b.Ap; a.Ap1 = b.Ap2; a.p0 = b.p0; a.p1 = b.p1; a.x = b.x;
+    a.r0 = b.r; a.r1 = b.r2; a.Ap0 = b.Ap; a.Ap1 = b.Ap2; a.p0 = b.p0; a.p1 = b.p1; a.x0 = b.x; a.x1 = b.x2;
     a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.P = w.P;
     a.TXV = b.TXV; a.TY = b.TY; a.TZ = b.TZ; a.ntx = b.ntx; a.nty = b.nty; a.ntz = b.ntz;
     a.ntiles = b.ntx * b.nty * b.ntz; a.nsv = b.nsv; a.nsc = b.nsc; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.lut = w.lut; a.dlut = w.dlut;
     a.nct = b.threads - 32;
+    a.sQ = (size_t)(b.Ap - b.r) * sizeof(T); a.sP = (size_t)(b.p0 - b.r) * sizeof(T); a.sX = (size_t)(b.x - b.r) * sizeof(T);
     fused_args_layout(a, fused_layout(b.TXV, b.TY, VecN<T>::value, QUAD, PALD));
     for (int it = 0; it < n_iter; it++)
-        k_pcg_fused<T, QUAD, PALD><<<b.grid, b.threads, b.smem, h->stream>>>(b.vm, b.tm_dinv, b.tm_x, b.tm_exm, b.tm_exp,
-                                                                           b.tm_ey, b.tm_ez, a);
+        k_pcg_fused<T, QUAD, PALD><<<b.grid, b.threads, b.smem, h->stream>>>(b.vm, b.tm_dinv, b.tm_q4, b.tm_exm, b.tm_ey,
+                                                                           b.tm_ez, a);
 }
 
 template <typename T>
@@ -411,7 +444,8 @@ pb_status solve_batch_impl(pb_handle *h, int m, const double *rhs, const double 
             T *dst = (T *)phi_out + (size_t)mem * n;
             T *dev_dst = where == PB_HOST ? (T *)h->stage : dst;
             k_finish<T, T><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
-                w.bw.x + s * w.npad, w.bw.p0 + s * w.npad, w.bw.p1 + s * w.npad, h->st + s, dev_dst, h->nx, w.P, rows);
+                w.bw.x + s * w.npad, w.bw.p0 + s * w.npad, w.bw.p1 + s * w.npad, h->st + s, dev_dst, h->nx, w.P, rows,
+                w.bw.fused ? w.bw.x2 : nullptr);
             PB_CUDA(cudaGetLastError());
             h->launches += 1;
             if (where == PB_HOST) {

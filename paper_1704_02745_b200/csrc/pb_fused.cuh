@@ -48,17 +48,42 @@ namespace pb {
 constexpr int kFusedSums = 5;        // p.Ap, S2, W, U1, U2
 constexpr int kFusedPlanes = 3;      // p_new planes k-1, k, k+1
 
-// vector slot of the fused kernel: r, A p (old) and p (old) haloed, x un-haloed
+// Slot layout.  The producer warp's TMA issue rate bounds this kernel (measured: leaving out three of nine small boxes
+// per plane, 2 % of the bytes, took 7.5 % off the pass), so the boxes of one plane are fetched with as few TMA
+// instructions as the tensors allow:
+//   vector slot       ONE 4-D box {r, A p, p, x} (all haloed, hy rows): the vectors live in one allocation, buffer
+//                     set 0 = (r0, Ap0, p0, x0) followed by set 1, each set four consecutive "members" of a tensor
+//                     [4][nz][ny][P]; x is double-buffered like the others (same bytes: one read, one write), so
+//                     that the slot looks the same in both parities (State::xbuf names the current x)
+//   coefficient slot  the Dinv box (index bytes or words), then -- quad format -- ONE 4-D box {ez, ex-, ex+, ey} of a
+//                     tensor [4][nz+1][ny+1][Pq] (TY + 1 rows each), or -- word format -- the three face boxes
 struct FusedLayout {
-    BatchLayout B;
-    size_t oAq, vslot;
+    BatchLayout B;                       // box sizes
+    uint32_t bZ, vslot;                  // one haloed vector box; the vector slot (four of them)
+    uint32_t bDv, bQ4, oEZ, oEXM, oEXP, oEY, cslot;
+    uint32_t pn;
 };
 __host__ __device__ inline FusedLayout fused_layout(int TXV, int TY, int vec, bool quad, bool pald)
 {
     FusedLayout F;
     F.B = batch_layout(TXV, TY, vec, quad, pald);
-    F.oAq = F.B.vslot;
-    F.vslot = F.oAq + align128(F.B.bZ);
+    F.bZ = F.B.bZ;
+    F.vslot = (uint32_t)align128(4 * (size_t)F.bZ);
+    F.bDv = F.B.bDv;
+    F.oEZ = (uint32_t)align128(F.bDv);
+    if (quad) {
+        const uint32_t S = (uint32_t)(TY + 1) * (uint32_t)F.B.bwq;   // one array of the merged quad box
+        F.bQ4 = 4 * S;
+        F.oEXM = F.oEZ + S; F.oEXP = F.oEZ + 2 * S; F.oEY = F.oEZ + 3 * S;
+        F.cslot = F.oEZ + (uint32_t)align128(F.bQ4);
+    } else {
+        F.bQ4 = 0;
+        F.oEXM = F.oEZ + (uint32_t)align128(F.B.bEZ);
+        F.oEXP = F.oEXM;
+        F.oEY = F.oEXM + (uint32_t)align128(F.B.bEXM);
+        F.cslot = F.oEY + (uint32_t)align128(F.B.bEY);
+    }
+    F.pn = (uint32_t)align128(F.bZ);
     return F;
 }
 
@@ -79,24 +104,24 @@ inline size_t fused_fixed_smem(int elt, bool quad, bool pald)
 }
 inline size_t fused_smem(const FusedLayout &F, int nsv, int nsc, int elt, bool quad, bool pald)
 {
-    return fused_fixed_smem(elt, quad, pald) + (size_t)nsv * F.vslot + (size_t)nsc * F.B.cslot +
-           (size_t)kFusedPlanes * F.B.pn + 128;
+    return fused_fixed_smem(elt, quad, pald) + (size_t)nsv * F.vslot + (size_t)nsc * F.cslot +
+           (size_t)kFusedPlanes * F.pn + 128;
 }
 
 template <typename T>
 struct FusedArgs {
-    T *r0, *r1, *Ap0, *Ap1, *p0, *p1;   // iteration with iter_cur = l reads buffer l & 1, writes the other
-    T *x;
+    T *r0, *r1, *Ap0, *Ap1, *p0, *p1, *x0, *x1;   // iteration with iter_cur = l reads buffer set l & 1, writes the other
     int nx, ny, nz, P;
     int TXV, TY, TZ;
     int ntx, nty, ntz, ntiles;
     int nsv, nsc;
     int precond;
     int nct;                 // consumer threads (whole warps); one more warp produces
-    // the slot layout (fused_layout), bytes: vector slot {r @0, A p @oQ, p @oP, x @oX}, coefficient slot
-    // {Dinv @0, ez @oEZ, ex- @oEXM, ex+ @oEXP, ey @oEY}, one p_new plane; box sizes for expect_tx
-    uint32_t vslot, cslot, pn, oQ, oP, oX, oEZ, oEXM, oEXP, oEY, bwq, bwd;
-    uint32_t bZ, bX, bDv, bEZ, bC;      // bC = the three in-plane face boxes together
+    // the slot layout (fused_layout), bytes: coefficient slot {Dinv @0, ez @oEZ, ex- @oEXM, ex+ @oEXP, ey @oEY}, one
+    // p_new plane; box sizes for expect_tx (bQ4: the merged quad box; bEZ, bC: the word-format face boxes)
+    uint32_t vslot, cslot, pn, bZ, oEZ, oEXM, oEXP, oEY, bwq, bwd;
+    uint32_t bDv, bQ4, bEZ, bC;
+    size_t sQ, sP, sX;       // bytes from a cell of r to the same cell of A p, p, x in the written buffer set
     State *st;
     double *partials;        // [kFusedSums][gridDim.x]
     const T *lut;
@@ -106,22 +131,20 @@ template <typename T>
 inline void fused_args_layout(FusedArgs<T> &a, const FusedLayout &F)
 {
     const BatchLayout &L = F.B;
-    a.vslot = (uint32_t)F.vslot; a.cslot = (uint32_t)L.cslot; a.pn = (uint32_t)L.pn;
-    a.oQ = (uint32_t)F.oAq; a.oP = (uint32_t)L.oPp; a.oX = (uint32_t)L.oX;
-    a.oEZ = (uint32_t)L.oEZ; a.oEXM = (uint32_t)L.oEXM; a.oEXP = (uint32_t)L.oEXP; a.oEY = (uint32_t)L.oEY;
+    a.vslot = F.vslot; a.cslot = F.cslot; a.pn = F.pn; a.bZ = F.bZ;
+    a.oEZ = F.oEZ; a.oEXM = F.oEXM; a.oEXP = F.oEXP; a.oEY = F.oEY;
     a.bwq = (uint32_t)L.bwq; a.bwd = (uint32_t)L.bwd;
-    a.bZ = L.bZ; a.bX = L.bX; a.bDv = L.bDv; a.bEZ = L.bEZ; a.bC = L.bEXM + L.bEXP + L.bEY;
+    a.bDv = F.bDv; a.bQ4 = F.bQ4; a.bEZ = L.bEZ; a.bC = L.bEXM + L.bEY;
 }
 
-// the six ping-pong vector tensors (4-D [1][nz][ny][P]) in one kernel parameter
-struct FusedMaps { CUtensorMap r0, r1, q0, q1, p0, p1; };
+// the two vector tensors ([4][nz][ny][P]: buffer set 0, buffer set 1) in one kernel parameter
+struct FusedMaps { CUtensorMap set0, set1; };
 
 template <typename T, bool QUAD, bool PALD>
 __global__ void __launch_bounds__(512)
 k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtensorMap tm_dinv,
-            const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_exm,
-            const __grid_constant__ CUtensorMap tm_exp, const __grid_constant__ CUtensorMap tm_ey,
-            const __grid_constant__ CUtensorMap tm_ez, const FusedArgs<T> a)
+            const __grid_constant__ CUtensorMap tm_q4, const __grid_constant__ CUtensorMap tm_exm,
+            const __grid_constant__ CUtensorMap tm_ey, const __grid_constant__ CUtensorMap tm_ez, const FusedArgs<T> a)
 {
     constexpr int VEC = VecN<T>::value;
     constexpr uint32_t ES = (uint32_t)sizeof(T);
@@ -170,10 +193,13 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
     const int TXV = a.TXV, TY = a.TY, TZ = a.TZ;
 
     if (is_producer) {
-        if (lane == 0) {
+        // the whole warp runs the loop (uniform control flow: coordinates, addresses and byte counts stay in uniform
+        // registers, no per-thread waterfall around the TMA instructions); lane 0 issues
+        {
+            const bool leader = lane == 0;
             int vs = 0, cs = 0;
             uint32_t vph = 0, cph = 0;
-            const CUtensorMap *tr = parity ? &vm.r1 : &vm.r0, *tq = parity ? &vm.q1 : &vm.q0, *tp = parity ? &vm.p1 : &vm.p0;
+            const CUtensorMap *tv = parity ? &vm.set1 : &vm.set0;
             for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
                 int b = tile;
                 const int bx = b % a.ntx; b /= a.ntx;
@@ -186,27 +212,33 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                 for (int q = k0 - 1; q <= k1; q++) {
                     const bool centre = (q >= k0) && (q < k1);
                     const bool ez = (q >= k0);
-                    {   // coefficient item q
+                    {   // coefficient item q: Dinv, and from plane k0 on the faces (ex, ey go unused at q = k1)
                         const uint32_t full = sb + SM::cfull + 8u * cs, slot = sm_c + (uint32_t)cs * a.cslot;
                         mbar_wait_a(full + (SM::cempty - SM::cfull), cph ^ 1);
-                        mbar_expect_tx_a(full, a.bDv + (ez ? a.bEZ : 0u) + (centre ? a.bC : 0u));
-                        tma_load_3d_a(slot, &tm_dinv, xd, j0 - 1, q, full);
-                        if (ez) tma_load_3d_a(slot + a.oEZ, &tm_ez, xq, j0, q, full);
-                        if (centre) {
-                            tma_load_3d_a(slot + a.oEXM, &tm_exm, xq, j0, q, full);
-                            if (QUAD) tma_load_3d_a(slot + a.oEXP, &tm_exp, xq, j0, q, full);
-                            tma_load_3d_a(slot + a.oEY, &tm_ey, xq, j0, q, full);
+                        if (leader) {
+                            if (QUAD) {
+                                mbar_expect_tx_a(full, a.bDv + (ez ? a.bQ4 : 0u));
+                                tma_load_3d_a(slot, &tm_dinv, xd, j0 - 1, q, full);
+                                if (ez) tma_load_4d_a(slot + a.oEZ, &tm_q4, xq, j0, q, 0, full);
+                            } else {
+                                mbar_expect_tx_a(full, a.bDv + (ez ? a.bEZ : 0u) + (centre ? a.bC : 0u));
+                                tma_load_3d_a(slot, &tm_dinv, xd, j0 - 1, q, full);
+                                if (ez) tma_load_3d_a(slot + a.oEZ, &tm_ez, xq, j0, q, full);
+                                if (centre) {
+                                    tma_load_3d_a(slot + a.oEXM, &tm_exm, xq, j0, q, full);
+                                    tma_load_3d_a(slot + a.oEY, &tm_ey, xq, j0, q, full);
+                                }
+                            }
                         }
                         cs = (cs + 1 == a.nsc) ? 0 : cs + 1; cph ^= (cs == 0);
                     }
-                    {   // vector item q
+                    {   // vector item q: one box {r, A p, p, x} of the buffer set this pass reads
                         const uint32_t full = sb + SM::vfull + 8u * vs, slot = sm_v + (uint32_t)vs * a.vslot;
                         mbar_wait_a(full + (SM::vempty - SM::vfull), vph ^ 1);
-                        mbar_expect_tx_a(full, 3 * a.bZ + (centre ? a.bX : 0u));
-                        tma_load_4d_a(slot, tr, x0 - VEC, j0 - 1, q, 0, full);
-                        tma_load_4d_a(slot + a.oQ, tq, x0 - VEC, j0 - 1, q, 0, full);
-                        tma_load_4d_a(slot + a.oP, tp, x0 - VEC, j0 - 1, q, 0, full);
-                        if (centre) tma_load_4d_a(slot + a.oX, &tm_x, x0, j0, q, 0, full);
+                        if (leader) {
+                            mbar_expect_tx_a(full, 4u * a.bZ);
+                            tma_load_4d_a(slot, tv, x0 - VEC, j0 - 1, q, 0, full);
+                        }
                         vs = (vs + 1 == a.nsv) ? 0 : vs + 1; vph ^= (vs == 0);
                     }
                 }
@@ -223,7 +255,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         const int tx = intile ? tx0 : 0, ty = intile ? ty0 : 0;
         const uint32_t t_own = ((uint32_t)(ty + 1) * BWc + (uint32_t)tx + 1u) * 16u;   // own cell in a haloed box / p_new plane
         const uint32_t t_c = (uint32_t)(ty * TXV + tx) * 16u;                          // own cell in an un-haloed box
-        const uint32_t t_xb = a.oX + t_c;
+        const uint32_t oQ = a.bZ, oP = 2u * a.bZ, oX = 3u * a.bZ;                      // the vector slot holds (r, A p, p, x)
         // halo cells (two rows, two columns): one per thread, from the last thread down (the host sizes the block so
         // that the consumer threads cover them: nct >= 2 TXV + 2 TY)
         const int nextra = 2 * TXV + 2 * TY;
@@ -238,9 +270,10 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         const bool has_x0 = extra0 >= 0;
         const uint32_t t_dx = has_x0 ? (uint32_t)extra0 * 16u - t_own : 0u;            // the halo cell, relative to the own cell
         const bool precond = a.precond != 0;
-        T *const r_out = parity ? a.r0 : a.r1, *const q_out = parity ? a.Ap0 : a.Ap1, *const p_out = parity ? a.p0 : a.p1;
+        // the buffer set this pass writes: r at out0, then A p, p, x at the constant strides of the allocation
+        char *const out0 = reinterpret_cast<char *>(parity ? a.r0 : a.r1);
         // per tile (the aligned starts of the byte boxes depend on x0): offsets within a coefficient slot
-        uint32_t t_dv = 0, t_dvx = 0, t_ez = 0, t_exm = 0, t_exp = 0, t_ey = 0, sbq = sb;
+        uint32_t t_dv = 0, t_dvx = 0, t_ez = 0, t_exm = 0, sbq = sb;
 
         // Dinv and D = 1/Dinv of VEC nodes: index bytes at `addr` -> pair table, or Dinv words at `addr`
         auto load_dinv = [&](uint32_t addr, Vec<T> &dinv, Vec<T> &D) {
@@ -269,8 +302,8 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
 
         // ring heads: slot index, phase parity and the slot's shared address, advanced together
         int vs = 0, cs = 0;
-        uint32_t vph = 0, cph = 0, vaddr = sm_v, caddr = sm_c;
-        const uint32_t plane = (uint32_t)ny * (uint32_t)P;
+        uint32_t vph = 0, cph = 0;
+        const size_t plane_b = (size_t)ny * (size_t)P * sizeof(T);     // bytes per plane
         // fp32: the sums over (at most) two planes, then added to the fp64 accumulators (flush); fp64: the thread's sums
         // themselves (inactive lanes are masked where they are formed)
         constexpr bool F32 = sizeof(T) == 4;
@@ -297,15 +330,14 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             if (QUAD) {
                 const uint32_t t_q = (uint32_t)ty * a.bwq + (uint32_t)((i0 >> 2) - ((x0 >> 2) & ~15));
                 sbq = sb + (uint32_t)(i0 & 3) * ES;                    // fp64: which half of the quadruple
-                t_ez = a.oEZ + t_q; t_exm = a.oEXM + t_q; t_exp = a.oEXP + t_q; t_ey = a.oEY + t_q;
+                t_ez = t_q;                                            // + a.oEZ / oEXM / oEXP / oEY where it is used
             } else {
-                t_ez = a.oEZ + t_c;
+                t_ez = t_c;
                 t_exm = a.oEXM + t_c + (uint32_t)ty * 16u;             // rows of TXV + 1 vectors
-                t_exp = t_exm + 16u;                                   // first element: the plus face of this vector's last node
-                t_ey = a.oEY + t_c;
             }
             const uint32_t ey_row = QUAD ? a.bwq : (uint32_t)TXV * 16u;
-            uint32_t gi = (uint32_t)((k0 * ny + j) * P + i0);          // element index (inactive lanes never use it)
+            // this thread's cell of plane k in the written r array (inactive lanes never use it)
+            char *po = out0 + (size_t)(uint32_t)((k0 * ny + j) * P + i0) * sizeof(T);
             // own-cell addresses in the three p_new planes: plane q lives in buffer q mod 3, rotated as the march advances
             uint32_t pn_m = sm_pn + t_own, pn_c = pn_m + a.pn, pn_n = pn_c + a.pn;
 
@@ -313,20 +345,20 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             // r_l = r_{l-1} - alpha_l A p_l, p_{l+1} = Dinv r_l + beta_l p_l on the own cell (returned; always stored into the plane)
             // and, for a plane this tile writes (centre), on the halo cells; r_l stored; the deferred phi update; the sums
             // U1, U2, W.  The vector slot is handed back; the coefficient slot stays (its address is returned).
-            auto update = [&](uint32_t pnw, bool centre, bool want_ez, uint32_t gidx, Vec<T> &pnew, Vec<T> &Dout, Vec<T> &dvout,
+            auto update = [&](uint32_t pnw, bool centre, bool want_ez, char *pout, Vec<T> &pnew, Vec<T> &Dout, Vec<T> &dvout,
                               Vec<T> &ezout) -> uint32_t {
                 mbar_wait_a(sb + SM::cfull + 8u * cs, cph);
-                const uint32_t cslot = caddr;
+                const uint32_t cslot = sm_c + (uint32_t)cs * a.cslot;
                 Vec<T> dvh, dummy;
                 load_dinv(cslot + t_dv, dvout, Dout);
                 if (centre && has_x0) load_dinv(cslot + t_dvx, dvh, dummy);
-                if (want_ez) ezout = coef(cslot + t_ez);
+                if (want_ez) ezout = coef(cslot + t_ez + a.oEZ);
                 mbar_wait_a(sb + SM::vfull + 8u * vs, vph);
-                const uint32_t sl = vaddr + t_own;
+                const uint32_t sl = sm_v + (uint32_t)vs * a.vslot + t_own;
                 Vec<T> rl, qv, pv;
                 lds_vec(rl.a, sl);
-                lds_vec(qv.a, sl + a.oQ);
-                lds_vec(pv.a, sl + a.oP);
+                lds_vec(qv.a, sl + oQ);
+                lds_vec(pv.a, sl + oP);
 #pragma unroll
                 for (int e = 0; e < VEC; e++) {
                     rl.a[e] = fma(-alpha, qv.a[e], rl.a[e]);                   // r_l (the deferred step 5)
@@ -335,7 +367,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                 sts_vec(pnw, pnew.a);
                 if (centre) {
                     Vec<T> xv;
-                    lds_vec(xv.a, vaddr + t_xb);
+                    lds_vec(xv.a, sl + oX);
 #pragma unroll
                     for (int e = 0; e < VEC; e++) xv.a[e] = fma(alpha, pv.a[e], xv.a[e]);   // phi_l = phi_{l-1} + alpha_l p_l
                     if (F32 || active) {
@@ -347,15 +379,15 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                         }
                     }
                     if (active) {
-                        stv(r_out + gidx, rl);
-                        stv(a.x + gidx, xv);
+                        stv(reinterpret_cast<T *>(pout), rl);
+                        stv(reinterpret_cast<T *>(pout + a.sX), xv);
                     }
                     if (has_x0) {
                         const uint32_t h0 = sl + t_dx;
                         Vec<T> r2, q2, p2;
                         lds_vec(r2.a, h0);
-                        lds_vec(q2.a, h0 + a.oQ);
-                        lds_vec(p2.a, h0 + a.oP);
+                        lds_vec(q2.a, h0 + oQ);
+                        lds_vec(p2.a, h0 + oP);
 #pragma unroll
                         for (int e = 0; e < VEC; e++) {
                             r2.a[e] = fma(-alpha, q2.a[e], r2.a[e]);
@@ -367,16 +399,16 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                 consume(pnew.a[0]);         // r, A p and p of the own cell have been read (x, halo: the stores above)
                 __syncwarp();
                 if (lane == 0) mbar_arrive_o<SM::vempty>(sb + 8u * vs);
-                vs++; vaddr += a.vslot;
-                if (vs == a.nsv) { vs = 0; vaddr = sm_v; vph ^= 1u; }
+                vs++;
+                if (vs == a.nsv) { vs = 0; vph ^= 1u; }
                 return cslot;
             };
-            auto cnext = [&]() { cs++; caddr += a.cslot; if (cs == a.nsc) { cs = 0; caddr = sm_c; cph ^= 1u; } };
+            auto cnext = [&]() { cs++; if (cs == a.nsc) { cs = 0; cph ^= 1u; } };
 
             // the stencil of plane k: p_new(k) from plane buffer pc_a (own cell, in-plane neighbours), p_new(k-1) from pm_a,
             // p_new(k+1) = pn (fresh from the update); coefficient slot cslotk; D, Dinv, ez of plane k and ez of plane k+1
             auto stencil = [&](uint32_t cslotk, uint32_t pm_a, uint32_t pc_a, const Vec<T> &pn, const Vec<T> &D, const Vec<T> &dv,
-                               const Vec<T> &ezc, const Vec<T> &ezn, uint32_t gidx) {
+                               const Vec<T> &ezc, const Vec<T> &ezn, char *pout) {
                 Vec<T> pc, pm, up, dn, exh;
                 T left, right;
                 lds_vec(pc.a, pc_a);
@@ -385,16 +417,16 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                 lds_vec(dn.a, pc_a + BWc * 16u);
                 lds_one_o<-(int)sizeof(T)>(left, pc_a);
                 lds_one_o<16>(right, pc_a);
-                const Vec<T> exl = coef(cslotk + t_exm);
+                const Vec<T> exl = coef(QUAD ? cslotk + t_ez + a.oEXM : cslotk + t_exm);
                 if (QUAD) {
-                    exh = coef(cslotk + t_exp);
+                    exh = coef(cslotk + t_ez + a.oEXP);
                 } else {
                     T exr;
-                    lds_one(exr, cslotk + t_exp);
+                    lds_one_o<16>(exr, cslotk + t_exm);                // the plus face of this vector's last node
 #pragma unroll
                     for (int e = 0; e < VEC; e++) exh.a[e] = (e == VEC - 1) ? exr : exl.a[e == VEC - 1 ? e : e + 1];
                 }
-                const Vec<T> eyl = coef(cslotk + t_ey), eyh = coef(cslotk + t_ey + ey_row);
+                const Vec<T> eyl = coef(cslotk + t_ez + a.oEY), eyh = coef(cslotk + t_ez + a.oEY + ey_row);
                 Vec<T> ap;
 #pragma unroll
                 for (int e = 0; e < VEC; e++) {
@@ -422,8 +454,8 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
                     }
                 }
                 if (active) {
-                    stv(q_out + gidx, ap);
-                    stv(p_out + gidx, pc);
+                    stv(reinterpret_cast<T *>(pout + a.sQ), ap);
+                    stv(reinterpret_cast<T *>(pout + a.sP), pc);
                 }
             };
             // the two-plane sums -> the thread's fp64 accumulators
@@ -440,28 +472,28 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             // item k0-1: the own column's p_new(k0-1) into plane buffer m; its coefficient slot goes back after a barrier
             {
                 const uint32_t c0 = sb + SM::cempty + 8u * cs;
-                update(pn_m, false, false, gi, pnv, Da, dva, eza);
+                update(pn_m, false, false, po, pnv, Da, dva, eza);
                 cnext();
                 named_bar_sync(1, NCT);
                 if (tid == 0) mbar_arrive_a(c0);
             }
             // item k0 -> plane buffer c;  D, Dinv, ez of plane k0 in set a
-            uint32_t ck = sb + SM::cempty + 8u * cs;
-            uint32_t cslotk = update(pn_c, true, true, gi, pnv, Da, dva, eza);
+            int csk = cs;                                       // the coefficient slot of plane k
+            update(pn_c, true, true, po, pnv, Da, dva, eza);
             cnext();
             named_bar_sync(1, NCT);
 
             // one step: update plane k+1 (set `n`), stencil of plane k (set `c`), barrier, hand the coefficient slot back
             auto step = [&](int k, Vec<T> &Dc, Vec<T> &dvc, Vec<T> &ezc, Vec<T> &Dn, Vec<T> &dvn, Vec<T> &ezn) {
-                const uint32_t c1 = sb + SM::cempty + 8u * cs;
-                const uint32_t cslot1 = update(pn_n, k + 1 < k1, true, gi + plane, pnv, Dn, dvn, ezn);
+                const int cs1 = cs;
+                update(pn_n, k + 1 < k1, true, po + plane_b, pnv, Dn, dvn, ezn);
                 cnext();
-                stencil(cslotk, pn_m, pn_c, pnv, Dc, dvc, ezc, ezn, gi);
-                named_bar_sync(1, NCT);   // p_new(k+1) complete; everyone is done with coefficient slot ck and plane buffer m
-                if (tid == 0) mbar_arrive_a(ck);
-                ck = c1; cslotk = cslot1;
+                stencil(sm_c + (uint32_t)csk * a.cslot, pn_m, pn_c, pnv, Dc, dvc, ezc, ezn, po);
+                named_bar_sync(1, NCT);   // p_new(k+1) complete; everyone is done with coefficient slot csk and plane buffer m
+                if (tid == 0) mbar_arrive_o<SM::cempty>(sb + 8u * (uint32_t)csk);
+                csk = cs1;
                 const uint32_t t = pn_m; pn_m = pn_c; pn_c = pn_n; pn_n = t;
-                gi += plane;
+                po += plane_b;
             };
             int k = k0;
             for (; k + 1 < k1; k += 2) {
@@ -472,7 +504,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             if (k < k1) step(k, Da, dva, eza, Db, dvb, ezb);
             flush();
             // coefficient item k1: only Dinv and ez of the own column were used, before the last barrier
-            if (tid == 0) mbar_arrive_a(ck);
+            if (tid == 0) mbar_arrive_o<SM::cempty>(sb + 8u * (uint32_t)csk);
         }
         if (!F32) { a_pAp = (double)s_pv; a_S2 = (double)s_dvv; a_W = (double)s_w; a_U1 = (double)s_u1; a_U2 = (double)s_u2; }
     }
@@ -508,6 +540,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             st->rz = U1;                                        // r_l.z_l and ||r_l||^2 of the stored r_l, exactly
             st->rr = U2;
             st->alpha = 0.0;                                    // unless another iteration follows: x = phi_l is final
+            st->xbuf = parity ^ 1;                              // ... and sits in the buffer set this pass wrote
             if (st->latch && (!isfinite(U1) || !isfinite(U2))) { st->done = 1; st->iters = l; st->status = 5; }
             else if (st->latch && (st->bb == 0.0 || U2 < st->tol2 * st->bb)) { st->done = 1; st->iters = l; st->status = 0; }  // step 3
             else if (st->latch && l >= st->maxiter) { st->done = 1; st->iters = l; st->status = 6; }

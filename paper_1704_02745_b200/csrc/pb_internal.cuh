@@ -32,7 +32,7 @@ struct State {
     // k_slab_alpha / k_slab_finish kernels then take the same decisions on every rank
     double loc_rz, loc_rr;
     int slab;
-    int pad_;
+    int xbuf;         // k_pcg_fused: which of its two x buffers holds the current iterate (0 after k_init)
 };
 
 // 16-byte vector of T: 4 floats or 2 doubles -> one 128-bit load/store per thread

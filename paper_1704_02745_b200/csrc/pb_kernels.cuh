@@ -293,8 +293,9 @@ __global__ void __launch_bounds__(256) k_warm(const VecArgs<T> a, const T *__res
 // or when no iteration ran).
 template <typename T, typename S>
 __global__ void k_finish(const T *__restrict__ x, const T *__restrict__ pbuf0, const T *__restrict__ pbuf1,
-                         const State *st, S *dst, int nx, int P, size_t rows)
+                         const State *st, S *dst, int nx, int P, size_t rows, const T *__restrict__ x_alt = nullptr)
 {
+    if (x_alt && st->xbuf) x = x_alt;          // k_pcg_fused double-buffers x: st->xbuf names the current one
     const T alpha = (T)st->alpha;
     const T *p = (st->iter_cur & 1) ? pbuf1 : pbuf0;
     const size_t total = rows * nx;

@@ -105,6 +105,7 @@ __global__ void k_unpad(const T *__restrict__ src, S *dst, int nx, int P, size_t
 __global__ void k_set_state(State *st, double tol2, int maxiter, int latch, int slab = 0)
 {
     st->slab = slab;
+    st->xbuf = 0;
     st->loc_rz = 0.0;
     st->loc_rr = 0.0;
     st->tol2 = tol2;
@@ -264,6 +265,39 @@ __global__ void k_setup_quad_idx(const double *__restrict__ eps_x, const double 
         }
         if (k < nz) eyq[((size_t)k * (ny + 1) + j) * Pq + bq] = (unsigned char)by;
         if (j < ny) ezq[((size_t)k * ny + j) * Pq + bq] = (unsigned char)bz;
+    }
+}
+
+// The same indices in ONE array [4][nz+1][ny+1][Pq] = {ez, ex-, ex+, ey} (k_pcg_fused fetches the four boxes of a
+// plane with one TMA instruction); entries outside an array's own range hold the index of 0.0 and are never used.
+__global__ void k_setup_quad4(const double *__restrict__ eps_x, const double *__restrict__ eps_y,
+                              const double *__restrict__ eps_z, int nx, int ny, int nz, int Pq, const PalTable *t,
+                              unsigned char *q4)
+{
+    const unsigned int zero = pal_index(t, 0.0);
+    const size_t total = (size_t)(nz + 1) * (ny + 1) * Pq;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        const int bq = (int)(q % Pq);
+        const size_t u = q / Pq;
+        const int j = (int)(u % (ny + 1)), k = (int)(u / (ny + 1));
+        unsigned int bm = 0, bp = 0, by = 0, bz = 0;
+        for (int f = 0; f < 4; f++) {
+            const int i = 4 * bq + f;
+            unsigned int im = zero, ip = zero, iy = zero, iz = zero;
+            if (i < nx) {
+                if (k < nz && j < ny) {
+                    im = pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i]);
+                    ip = pal_index(t, eps_x[((size_t)k * ny + j) * (nx + 1) + i + 1]);
+                }
+                if (k < nz) iy = pal_index(t, eps_y[((size_t)k * (ny + 1) + j) * nx + i]);
+                if (j < ny) iz = pal_index(t, eps_z[((size_t)k * ny + j) * nx + i]);
+            }
+            bm |= im << (2 * f); bp |= ip << (2 * f); by |= iy << (2 * f); bz |= iz << (2 * f);
+        }
+        q4[q] = (unsigned char)bz;
+        q4[total + q] = (unsigned char)bm;
+        q4[2 * total + q] = (unsigned char)bp;
+        q4[3 * total + q] = (unsigned char)by;
     }
 }
 
