@@ -53,7 +53,8 @@ typedef enum {
     PB_ERR_CUDA = 3,
     PB_ERR_NOT_SPD = 4,     /* a diagonal entry <= 0 or a non-finite coefficient found at create      */
     PB_ERR_BREAKDOWN = 5,   /* p.Ap <= 0 or NaN/Inf met during the solve; phi = last good iterate     */
-    PB_ERR_MAXITER = 6      /* not converged in maxiter; phi, iters and relres are still returned     */
+    PB_ERR_MAXITER = 6,     /* not converged in maxiter; phi, iters and relres are still returned     */
+    PB_ERR_TOO_LARGE = 7    /* pb_residual_noalloc: the grid exceeds the fixed scratch (PB_NOALLOC_MAX_ROWS) */
 } pb_status;
 
 typedef enum { PB_F32 = 0, PB_F64 = 1 } pb_precision;
@@ -361,6 +362,30 @@ pb_status pb_destroy(pb_handle *h);
 
 /* Static, never-NULL description of a status code. */
 const char *pb_strerror(pb_status s);
+
+/*
+ * pb_residual_noalloc -- the true relative residual ||b - A phi|| / ||b|| (A of Eq. 3, b of Eq. 4 with the ghost
+ * Dirichlet terms folded in; the quantity pb_residual reports) for callers that CANNOT ALLOCATE: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  No handle: the call allocates
+ * nothing (no cudaMalloc / cudaFree / allocating library routine) and does not synchronise; it enqueues one 256-byte
+ * memset and one kernel on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream) of the CURRENT device.
+ * Every pointer is a DEVICE pointer on that device, fp64, dense, laid out as for pb_create: eps_x [nz][ny][nx+1],
+ * eps_y [nz][ny+1][nx], eps_z [nz+1][ny][nx], kbar2 / rhs / phi [nz][ny][nx], bc = the six ghost faces; kbar2, rhs
+ * and bc may be NULL (zeros).  Output, written by the kernel: out3[0] = ||b - A phi|| / ||b|| (0 if b = 0),
+ * out3[1] = ||r||^2, out3[2] = ||b||^2 of the h^2-scaled system.  Sums are formed in a fixed order (reproducible).
+ * Scratch: a fixed __device__ array of the library (512 KiB + 256 B, held by every GPU that loads the library until
+ * exit) sized for PB_NOALLOC_MAX_ROWS = 262 144 grid rows (nz * ny, e.g. 512 x 512; nx is free up to 2e9 nodes):
+ * a larger grid -> PB_ERR_TOO_LARGE, nothing enqueued.  Every call on a device SHARES that array: calls that overlap
+ * on the GPU (different streams, different host threads) race -- serialise them.  The array keeps the last call's
+ * partial sums; the one word that must start at zero is cleared on the stream by every call.  The first call on a
+ * device looks the array's device address up (cudaGetSymbolAddress): make it outside stream capture.
+ * Errors: sizes < 1, h <= 0 or non-finite, NULL eps / phi / out3 -> PB_ERR_INVALID_ARG; no device, launch or
+ * memset failure -> PB_ERR_CUDA.  Asynchronous faults (bad device pointers) surface at the caller's next sync.
+ */
+#define PB_NOALLOC_MAX_ROWS 262144
+pb_status pb_residual_noalloc(int nx, int ny, int nz, double h, const double *eps_x, const double *eps_y,
+                              const double *eps_z, const double *kbar2, const double *rhs, const double *bc,
+                              const double *phi, double *out3, void *cuda_stream);
 
 /*
  * pb_query -- read back derived quantities for tests (device -> host copies, fp64):

@@ -17,4 +17,6 @@ from .binding import (  # noqa: F401
     lib_path,
     load_library,
     pb_strerror,
+    residual_noalloc,
+    NOALLOC_MAX_ROWS,
 )

@@ -14,7 +14,7 @@ PB_F32, PB_F64 = 0, 1
 PB_HOST, PB_DEVICE = 0, 1
 PB_OK, PB_ERR_INVALID_ARG, PB_ERR_ALLOC, PB_ERR_CUDA, PB_ERR_NOT_SPD, PB_ERR_BREAKDOWN, PB_ERR_MAXITER = range(7)
 STATUS_NAMES = {0: "PB_OK", 1: "PB_ERR_INVALID_ARG", 2: "PB_ERR_ALLOC", 3: "PB_ERR_CUDA",
-                4: "PB_ERR_NOT_SPD", 5: "PB_ERR_BREAKDOWN", 6: "PB_ERR_MAXITER"}
+                4: "PB_ERR_NOT_SPD", 5: "PB_ERR_BREAKDOWN", 6: "PB_ERR_MAXITER", 7: "PB_ERR_TOO_LARGE"}
 
 # every symbol include/pb.h declares
 EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", "pb_iterate",
@@ -22,7 +22,7 @@ EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", 
            "pb_set_charges", "pb_get_field", "pb_palette_size", "pb_solve_from", "pb_set_boundary",
            "pb_diag_palette_size", "pb_residual", "pb_bytes_per_node", "pb_solve_refined", "pb_set_setup_precision", "pb_set_option", "pb_get_option",
            "pb_prepare", "pb_get_plan", "pb_solve_batch", "pb_solve_batch_charges", "pb_create_slab", "pb_slab_begin",
-           "pb_slab_step", "pb_slab_pointers", "pb_slab_latch", "pb_slab_result")
+           "pb_slab_step", "pb_slab_pointers", "pb_slab_latch", "pb_slab_result", "pb_residual_noalloc")
 
 # pb_option (include/pb.h), by name
 OPTIONS = {"persist": 0, "persist_max_mb": 1, "persist_fused_max_knodes": 2, "persist_blocks_per_sm": 3,
@@ -108,6 +108,7 @@ def load_library():
     lib.pb_get_option.argtypes = [vp, ci, ctypes.POINTER(ci)]
     lib.pb_prepare.argtypes = [vp, ci]
     lib.pb_get_plan.argtypes = [vp, ci, ctypes.POINTER(PBPlan)]
+    lib.pb_residual_noalloc.argtypes = [ci, ci, ci, cd, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     for name in EXPORTS:
         getattr(lib, name)
     _lib = lib
@@ -119,6 +120,37 @@ def pb_strerror(status: int) -> str:
         return load_library().pb_strerror(int(status)).decode()
     except Exception:
         return "?"
+
+
+NOALLOC_MAX_ROWS = 262144      # PB_NOALLOC_MAX_ROWS of include/pb.h
+
+
+def residual_noalloc(nx, ny, nz, h, eps_x, eps_y, eps_z, kbar2, rhs, bc, phi, out3, stream=None):
+    """pb_residual_noalloc: ||b - A phi|| / ||b|| without any allocation, for callers that cannot call cudaMalloc.
+
+    Every array is a CUDA float64 tensor (contiguous, on the current device; kbar2 / rhs / bc may be None); `out3` is
+    the caller's 3-element CUDA float64 tensor {relres, ||r||^2, ||b||^2}, written asynchronously on `stream` (a raw
+    cudaStream_t value; None = the legacy default stream).  Argument marshalling only; nothing is copied or allocated.
+    Grids with nz * ny > NOALLOC_MAX_ROWS raise PBError(PB_ERR_TOO_LARGE).  Calls share one fixed scratch array per
+    GPU: do not let two of them overlap on the device."""
+    def dptr(t, name, count):
+        if t is None:
+            return None
+        if not (_is_torch(t) and t.is_cuda and str(t.dtype) == "torch.float64" and t.is_contiguous() and t.numel() == count):
+            raise ValueError(f"{name}: expected a contiguous CUDA float64 tensor of {count} elements")
+        return ctypes.c_void_p(t.data_ptr())
+
+    nx, ny, nz = int(nx), int(ny), int(nz)
+    n = nx * ny * nz
+    nbc = 2 * (nz * ny + nz * nx + ny * nx)
+    big = nz * ny > NOALLOC_MAX_ROWS          # let the library reject it (before it looks at any pointer)
+    args = [(eps_x, "eps_x", nz * ny * (nx + 1)), (eps_y, "eps_y", nz * (ny + 1) * nx), (eps_z, "eps_z", (nz + 1) * ny * nx),
+            (kbar2, "kbar2", n), (rhs, "rhs", n), (bc, "bc", nbc), (phi, "phi", n), (out3, "out3", 3)]
+    ptrs = [None if big else dptr(t, nm, c) for t, nm, c in args]
+    st = load_library().pb_residual_noalloc(nx, ny, nz, float(h), *ptrs, ctypes.c_void_p(stream) if stream else None)
+    if st != PB_OK:
+        raise PBError(st, "pb_residual_noalloc")
+    return out3
 
 
 def _is_torch(a) -> bool:

@@ -1748,6 +1748,7 @@ const char *pb_strerror(pb_status s)
     case PB_ERR_NOT_SPD: return "operator not symmetric positive definite (non-positive or non-finite diagonal)";
     case PB_ERR_BREAKDOWN: return "PCG breakdown (p.Ap <= 0 or non-finite value)";
     case PB_ERR_MAXITER: return "maximum number of iterations reached before convergence";
+    case PB_ERR_TOO_LARGE: return "grid larger than the fixed scratch of pb_residual_noalloc (nz * ny > PB_NOALLOC_MAX_ROWS)";
     }
     return "unknown status";
 }

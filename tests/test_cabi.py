@@ -32,8 +32,8 @@ def test_exports_every_declared_symbol(lib):
 
 def test_strerror_and_version(lib):
     assert lib.pb_version() >= 100
-    msgs = {lib.pb_strerror(s).decode() for s in range(7)}
-    assert len(msgs) == 7 and all(msgs)
+    msgs = {lib.pb_strerror(s).decode() for s in range(8)}
+    assert len(msgs) == 8 and all(msgs)
     assert lib.pb_strerror(99).decode() == "unknown status"
 
 
