@@ -168,6 +168,10 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     if (b.TY > h->ny) b.TY = h->ny;
     const int max_ct = max_threads - 64;
     while (spmv_row_threads(b.TXV) * b.TY > max_ct && b.TY > 1) b.TY--;
+    // k_pcg_fused takes 128 registers per thread: two blocks share an SM only up to 256 threads each (measured at 385^3
+    // fp64: 65 x 3 tiles, two blocks per SM, 0.654 ms per pass against 0.742 ms for 65 x 4 with one block)
+    if (fused && o[PB_OPT_TILE_TY] <= 0 && o[PB_OPT_BLOCKS_PER_SM] != 1)
+        while ((spmv_row_threads(b.TXV) * b.TY + 31) / 32 * 32 + 32 > 256 && b.TY > 2) b.TY--;
     b.threads = (spmv_row_threads(b.TXV) * b.TY + 31) / 32 * 32 + 32;
     if (fused) {       // k_pcg_fused: one halo cell per consumer thread at most
         const int halo = (2 * b.TXV + 2 * b.TY + 31) / 32 * 32 + 32;
