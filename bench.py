@@ -390,9 +390,9 @@ def run_ours(args, rank, local_rank, world):
     iter_bytes = spmv_bytes + vec_bytes
     ns_bytes = WORDS_NORTH_STAR * elt * n_node
     t_solve = ms_local * 1e-3
-    committed = ncu_traffic(f"k_spmv:{wl}")
     plan = plan_summary(solver, prec)
     fused = bool(plan.get("fused"))
+    committed = ncu_traffic(f"{'k_pcg_fused' if fused else 'k_spmv'}:{wl}")
     kvec = (None if fused else
             {"achieved": kr["vec_GBs"], "frac": kr["vec_frac"], "bytes_per_node": kr["vec_bytes_per_node"],
              "diag_palette_size": pald, "ms_per_launch": ms_vec})
