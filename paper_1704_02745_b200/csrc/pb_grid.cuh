@@ -142,14 +142,49 @@ __global__ void k_grid_rhs(double *q, size_t n, double four_pi, double h3, const
     }
 }
 
+// fp64 1/sqrt(d2) for the boundary sum: MUFU.RSQ seed on the value rounded to fp32 (2^-22) and ONE third-order Newton
+// step (error (5/16) e^3 ~ 3e-21 relative, i.e. correctly rounded up to the last DFMA).  d2 in [2^-126, 2^127].
+__device__ __forceinline__ double dh_rsqrt(double d2)
+{
+    float s;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(d2)));
+    const double y = (double)s;
+    const double e = fma(-(d2 * y), y, 1.0);                   // 1 - d2 y^2
+    return fma(y, fma(0.375, e, 0.5) * e, y);                  // y (1 + e/2 + 3 e^2/8)
+}
+
+// fp64 exp(x) for -700 < x <= 0: x = (64 n + k) ln2/64 + f, |f| <= ln2/128; exp(x) = 2^n * 2^(k/64) * exp(f) with a
+// 64-entry table (shared memory) and a degree-5 Taylor polynomial (remainder f^6/6! < 4e-17); no special cases --
+// the argument range is fixed by the geometry (kappa r <= a few hundred).
+constexpr int DH_EXP_TAB = 64;
+__device__ __forceinline__ double dh_exp_neg(double x, const double *tab)
+{
+    const double MAGIC = 6755399441055744.0;                   // 1.5 * 2^52: the integer lands in the low word
+    const double t = fma(x, 92.332482616893657, MAGIC);        // 64 / ln 2
+    const int m = __double2loint(t);
+    const double mf = t - MAGIC;
+    double f = fma(mf, -1.08304246932675596326e-02, x);        // ln2_hi / 64 (32 significant bits: mf * it is exact)
+    f = fma(mf, -2.98158582698529328128e-12, f);               // ln2_lo / 64
+    double p = fma(f, 1.0 / 120.0, 1.0 / 24.0);
+    p = fma(p, f, 1.0 / 6.0);
+    p = fma(p, f, 0.5);
+    p = fma(p, f, 1.0);
+    p = fma(p, f, 1.0);
+    p *= tab[m & (DH_EXP_TAB - 1)];
+    return __hiloint2double(__double2hiint(p) + ((m >> 6) << 20), __double2loint(p));   // * 2^n (stays normal)
+}
+
 // Debye-Hueckel ghost values: bc[g] = (1/eps_out) sum_a q_a exp(-kappa r_ga)/r_ga, atoms in index order.
-// One thread per ghost node, atoms staged through shared memory in tiles of DH_TILE.  Plain-ALU-bound.
+// One thread per ghost node, atoms staged through shared memory in tiles of DH_TILE.  Plain-ALU-bound (fp64 pipe /
+// issue): 1/r and exp come from the two routines above instead of the general-purpose library ones.
 constexpr int DH_TILE = 256;
 __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ c, const double *__restrict__ charge,
                                                      int n_atoms, int nx, int ny, int nz, double h, double eps_out,
                                                      double kappa, double *bc)
 {
     __shared__ double sc[DH_TILE][4];
+    __shared__ double tab[DH_EXP_TAB];
+    if (threadIdx.x < DH_EXP_TAB) tab[threadIdx.x] = exp2((double)threadIdx.x / DH_EXP_TAB);   // 2^(k/64), library exp2 (< 1 ulp)
     const size_t n_xy = (size_t)ny * nx, n_zy = (size_t)nz * ny, n_zx = (size_t)nz * nx;
     const size_t nbc = 2 * (n_zy + n_zx + n_xy);
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -164,6 +199,7 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ 
         const size_t v = t - 2 * n_zy - 2 * n_zx, u = v % n_xy;
         gz = (v < n_xy) ? -h : nz * h; gx = (double)(u % nx) * h; gy = (double)(u / nx) * h;
     }
+    const double nkappa = -kappa;
     double acc = 0.0;
     for (int a0 = 0; a0 < n_atoms; a0 += DH_TILE) {
         const int a = a0 + threadIdx.x;
@@ -174,8 +210,8 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ 
         for (int s = 0; s < m; s++) {
             const double dx = gx - sc[s][0], dy = gy - sc[s][1], dz = gz - sc[s][2];
             const double d2 = (dx * dx + dy * dy) + dz * dz;
-            const double ir = rsqrt(d2);                   // 1/r and r = d2/r: one special-function call, no division
-            acc += sc[s][3] * (exp(-kappa * (d2 * ir)) * ir);
+            const double ir = dh_rsqrt(d2);                // 1/r, and r = d2/r: no division
+            acc = fma(sc[s][3], dh_exp_neg(nkappa * (d2 * ir), tab) * ir, acc);
         }
         __syncthreads();
     }
