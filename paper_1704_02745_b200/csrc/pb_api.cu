@@ -1778,9 +1778,12 @@ pb_status charges_to_rhs_bc(const double *d_c, const double *d_q, int n_atoms, i
     if (dh_f32)
         k_grid_dh_f32<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
                                                                                     eps_out, kappa, d_bc);
+    else if (dh_fast_range(nx, ny, nz, hh, kappa))
+        k_grid_dh<true><<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
+                                                                                      eps_out, kappa, d_bc);
     else
-        k_grid_dh<<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
-                                                                                eps_out, kappa, d_bc);
+        k_grid_dh<false><<<(unsigned)((nbc + DH_TILE - 1) / DH_TILE), DH_TILE, 0, st>>>(d_c, d_q, n_atoms, nx, ny, nz, hh,
+                                                                                       eps_out, kappa, d_bc);
     PB_CUDA(cudaGetLastError());
     int bad = 0;
     PB_CUDA(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));

@@ -177,7 +177,15 @@ __device__ __forceinline__ double dh_exp_neg(double x, const double *tab)
 // Debye-Hueckel ghost values: bc[g] = (1/eps_out) sum_a q_a exp(-kappa r_ga)/r_ga, atoms in index order.
 // One thread per ghost node, atoms staged through shared memory in tiles of DH_TILE.  Plain-ALU-bound (fp64 pipe /
 // issue): 1/r and exp come from the two routines above instead of the general-purpose library ones.
+// FAST = false: the library rsqrt / exp (any argument), for geometries outside the range the fitted routines assume
+// (dh_fast_range below; no molecular grid gets there).
 constexpr int DH_TILE = 256;
+inline bool dh_fast_range(int nx, int ny, int nz, double h, double kappa)
+{
+    const double rmax2 = h * h * ((double)(nx + 1) * (nx + 1) + (double)(ny + 1) * (ny + 1) + (double)(nz + 1) * (nz + 1));
+    return h * h >= 1e-30 && rmax2 <= 1e30 && kappa * sqrt(rmax2) <= 700.0;      // d2 within fp32 range, exp normal
+}
+template <bool FAST>
 __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ c, const double *__restrict__ charge,
                                                      int n_atoms, int nx, int ny, int nz, double h, double eps_out,
                                                      double kappa, double *bc)
@@ -210,8 +218,9 @@ __global__ void __launch_bounds__(DH_TILE) k_grid_dh(const double *__restrict__ 
         for (int s = 0; s < m; s++) {
             const double dx = gx - sc[s][0], dy = gy - sc[s][1], dz = gz - sc[s][2];
             const double d2 = (dx * dx + dy * dy) + dz * dz;
-            const double ir = dh_rsqrt(d2);                // 1/r, and r = d2/r: no division
-            acc = fma(sc[s][3], dh_exp_neg(nkappa * (d2 * ir), tab) * ir, acc);
+            const double ir = FAST ? dh_rsqrt(d2) : rsqrt(d2);          // 1/r, and r = d2/r: no division
+            const double x = nkappa * (d2 * ir);
+            acc = fma(sc[s][3], (FAST ? dh_exp_neg(x, tab) : exp(x)) * ir, acc);
         }
         __syncthreads();
     }

@@ -67,6 +67,27 @@ def test_fields_match_setup_oracle(pkg, shape, na):
         assert np.array_equal(s.field("eps_x"), ref["eps_x"])
 
 
+@pytest.mark.parametrize("kb", [0.0, 2.0e5])
+def test_boundary_sum_salt_extremes(pkg, kb):
+    """The fp64 boundary sum outside its everyday range: no salt (kappa = 0, every exponential is exactly 1) and a
+    screening so strong (kappa r up to ~800) that the kernel's fitted exp routine does not apply and the library one is
+    used (dh_fast_range) -- ghost values against the setup oracle, 1e-12 of the sum of |terms|."""
+    from oracle import pbsetup_ref as S
+
+    nx, ny, nz, h, eps_in, eps_out = 21, 17, 13, 0.5, 1.0, 80.0
+    c, r, q = atoms(12, nx, ny, nz, h, 12)
+    ref = S.setup(nx, ny, nz, h, c, r, q, eps_in, eps_out, kb)
+    kappa = math.sqrt(kb / eps_out)
+    g = S.ghost_positions(nx, ny, nz, h)
+    rr = np.linalg.norm(g[:, None, :] - c[None, :, :], axis=2)
+    scale = (np.abs(q)[None, :] * np.exp(-kappa * rr) / rr).sum(1) / eps_out
+    with pkg.PBSolver.from_atoms(nx, ny, nz, h, c, r, q, eps_in, eps_out, kb) as s:
+        bc = s.field("bc")
+    assert np.all(np.isfinite(bc)) and np.all(np.abs(bc - ref["bc"]) <= 1e-12 * scale + 1e-300)
+    if kb == 0.0:
+        assert np.max(np.abs(bc)) > 0.0
+
+
 def test_fp32_boundary_sum(pkg):
     """pb_set_setup_precision(PB_F32): the Debye-Hueckel ghost values with every term in fp32 (hardware rsqrt / exp2,
     Kahan partial sums) stay within 2e-6 of the sum of |terms| of the fp64 setup oracle (an fp32 term carries a few
