@@ -881,11 +881,11 @@ pb_status run_solve(pb_handle *h, double tol, int maxiter, int check_every, cons
                     bool allow_fused = true)
 {
     h->last_fused = false;
-    if (allow_fused && !phi0 && fused_eligible<T>(h)) {
+    if (allow_fused && fused_eligible<T>(h)) {
         // one kernel per iteration (k_pcg_fused) on the batch work set, right-hand side = this handle's b
         Work<T> &wq = work<T>(h);
         PB_TRY(ensure_batch<T>(h, 1, true));
-        PB_TRY(run_batch<T>(h, 1, tol, maxiter, check_every, wq.b));
+        PB_TRY(run_batch<T>(h, 1, tol, maxiter, check_every, wq.b, phi0, where));
         h->last_fused = true;
         return PB_OK;
     }
@@ -997,11 +997,15 @@ pb_status refined_impl(pb_handle *h, double tol, int maxiter, double inner_tol, 
                                                                                            h->nx, rows);
         h->launches += 1;
         wf.b_ready = true;
-        const pb_status rs = run_solve<float>(h, tin, maxiter - total, check_every, nullptr, PB_DEVICE, false);
+        const pb_status rs = run_solve<float>(h, tin, maxiter - total, check_every, nullptr, PB_DEVICE);
         wf.b_ready = false;                      // wf.b holds a residual, not b: rebuilt before the next plain solve
         if (rs != PB_OK) return rs;
-        k_finish_add<float, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
-            wf.x, wf.p0, wf.p1, h->st, wd.tmp, h->nx, wf.P, wd.P, rows);
+        if (h->last_fused)                       // the correction went through k_pcg_fused (its own vectors)
+            k_finish_add<float, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
+                wf.bw.x, wf.bw.p0, wf.bw.p1, h->st, wd.tmp, h->nx, wf.P, wd.P, rows, wf.bw.x2);
+        else
+            k_finish_add<float, double><<<grid_for(n, 256, h->nsm * 16), 256, 0, h->stream>>>(
+                wf.x, wf.p0, wf.p1, h->st, wd.tmp, h->nx, wf.P, wd.P, rows);
         PB_CUDA(cudaGetLastError());
         h->launches += 1;
         PB_CUDA(cudaMemcpyAsync(h->pinned_state, h->st, sizeof(State), cudaMemcpyDeviceToHost, h->stream));

@@ -342,12 +342,42 @@ pb_status init_batch(pb_handle *h, int M, double tol, int maxiter, int latch, co
     return PB_OK;
 }
 
+// step 1 with a given phi_0 on the batch work set, member 0, after init_batch: x = phi_0,
+// r = b - A'phi_0 (A'phi_0 through k_spmv_tma<MODE 1> on the handle's own arrays), r.z, r.r, the l = 0 test again;
+// k_pcg_fused's first pass then finds exactly what it finds after a cold start (alpha = beta = 0, "A p_0" = 0, p = 0)
 template <typename T>
-pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_every, const T *single_b = nullptr)
+pb_status warm_batch(pb_handle *h, const T *b_rhs, const void *phi0, pb_memspace where)
+{
+    Work<T> &w = work<T>(h);
+    BatchWork<T> &b = w.bw;
+    const size_t rows = (size_t)h->nz * h->ny, n = rows * h->nx;
+    const T *src = (const T *)phi0;
+    if (where == PB_HOST) {
+        PB_TRY(ensure_stage(h, n * sizeof(T)));
+        PB_CUDA(cudaMemcpyAsync(h->stage, phi0, n * sizeof(T), cudaMemcpyHostToDevice, h->stream));
+        src = (const T *)h->stage;
+    }
+    k_pad<T, T><<<grid_for(w.npad, 256, h->nsm * 16), 256, 0, h->stream>>>(src, w.tmp, h->nx, w.P, rows);
+    launch_spmv<T, 1>(h, w, 1.0);                      // w.Ap = A' phi_0
+    VecArgs<T> va = vec_args<T>(h, w);
+    va.r = b.r; va.x = b.x; va.b = b_rhs;
+    k_warm<T><<<w.vec_grid, 256, 0, h->stream>>>(va, w.tmp);
+    PB_CUDA(cudaGetLastError());
+    h->launches += 3;
+    return PB_OK;
+}
+
+template <typename T>
+pb_status run_batch(pb_handle *h, int M, double tol, int maxiter, int check_every, const T *single_b = nullptr,
+                    const void *phi0 = nullptr, pb_memspace phi0_where = PB_DEVICE)
 {
     Work<T> &w = work<T>(h);
     BatchWork<T> &b = w.bw;
     PB_TRY(init_batch<T>(h, M, tol, maxiter, 1, single_b));
+    if (phi0) {
+        if (M != 1 || !single_b) return PB_ERR_INVALID_ARG;
+        PB_TRY(warm_batch<T>(h, single_b, phi0, phi0_where));
+    }
     const int m = check_every;
     const long long per_iter = b.fused ? 1 : 2;
     bool graph_ok = false;

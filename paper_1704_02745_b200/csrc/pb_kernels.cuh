@@ -455,8 +455,10 @@ __global__ void k_repad(const S *__restrict__ src, int Ps, T *dst, int Pd, int n
 
 template <typename T, typename S>
 __global__ void k_finish_add(const T *__restrict__ x, const T *__restrict__ pbuf0, const T *__restrict__ pbuf1,
-                             const State *st, S *acc, int nx, int P, int Pacc, size_t rows)
+                             const State *st, S *acc, int nx, int P, int Pacc, size_t rows,
+                             const T *__restrict__ x_alt = nullptr)
 {
+    if (x_alt && st->xbuf) x = x_alt;          // k_pcg_fused double-buffers x (as in k_finish)
     const T alpha = (T)st->alpha;
     const T *p = (st->iter_cur & 1) ? pbuf1 : pbuf0;
     const size_t total = rows * nx;

@@ -376,18 +376,22 @@ def test_palette_and_full_precision_coefficients_agree(pkg, pbref, prec, tol):
         assert s.palette_size() == 0
 
 
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
-def test_warm_start_matches_oracle(pkg, pbref, prec, tol):
+def test_warm_start_matches_oracle(pkg, pbref, prec, tol, path):
     """NEXT row f2 (part): pb_solve_from = step 1 with a given phi_0.  Snapshot-style use: solve,
     perturb the charges (new rhs and ghost values), restart from the previous potential.  Iteration counts and
-    potentials must match the oracle run from the same phi_0; the restart must need fewer iterations."""
+    potentials must match the oracle run from the same phi_0; the restart must need fewer iterations.  On each of the
+    three solve paths (the fused one takes its warm start through the same k_warm step as the two-kernel one)."""
     inp = make_config(2)
     from workloads import perturbed_charges
 
     rhs2, bc2 = perturbed_charges(inp, 0, device="cpu")
     ref = pbref.from_inputs(inp)
     dt = np.float64 if prec == "f64" else np.float32
-    with pkg.PBSolver(*inp.args()) as s:
+    with pkg.PBSolver(*inp.args(), options=PATHS[path]) as s:
+        if path == "fused":
+            assert s.plan(prec)["fused"] == 1
         first = s.solve(tol, 5000, prec)
         s.set_rhs(rhs2, bc2)
         ref.set_rhs(rhs2, bc2)
@@ -594,8 +598,9 @@ def test_true_residual_matches_oracle(pkg, pbref):
     assert abs(t64 - true) <= 1e-6 * true and abs(t32 - true) <= 0.2 * true
 
 
+@pytest.mark.parametrize("path", ["default", "fused"])
 @pytest.mark.parametrize("cfg", [2, "born", "random"])
-def test_mixed_precision_refinement_matches_fp64_oracle(pkg, pbref, cfg):
+def test_mixed_precision_refinement_matches_fp64_oracle(pkg, pbref, cfg, path):
     """NEXT row f3 (fp32-inner / fp64-outer iterative refinement): the result is the solution of A phi = b to 1e-10 on
     the TRUE residual -- same bar as the fp64 solve (within 1e-8 max|phi| of the oracle run to 1e-10) -- although every
     PCG iteration ran in fp32; a plain fp32 solve cannot get there (its true residual stagnates near 1e-6)."""
@@ -603,7 +608,7 @@ def test_mixed_precision_refinement_matches_fp64_oracle(pkg, pbref, cfg):
     ref = pbref.from_inputs(inp)
     o = ref.solve(1e-10, 5000)
     b = ref.b()
-    with pkg.PBSolver(*inp.args()) as s:
+    with pkg.PBSolver(*inp.args(), options=PATHS[path]) as s:      # "fused": the corrections run through k_pcg_fused
         g = s.solve_refined(1e-10, 5000)
         assert g["status"] == 0 and g["relres"] <= 1e-10 and 2 <= g["outer"] <= 6
         assert abs(s.residual(g["phi"], "f64") - g["relres"]) <= 1e-3 * g["relres"] + 1e-16
