@@ -42,6 +42,7 @@ struct BatchWork {
     int TXV = 0, TY = 0, TZ = 0, ntx = 0, nty = 0, ntz = 0, nsv = 0, nsc = 0, bps = 0, grid = 0, threads = 0;
     size_t smem = 0;
     int vec_grid = 0;
+    int tuned = 0;                                 // the fused plan was chosen by timing candidates
     CUtensorMap tm_r, tm_p0, tm_p1, tm_x, tm_dinv, tm_exm, tm_exp, tm_ey, tm_ez;
     cudaGraphExec_t graph = nullptr;
     int graph_iters = 0;
@@ -255,6 +256,21 @@ pb_status build_work(pb_handle *h, Work<T> &w)
 {
     const int align = 32 / (int)sizeof(T);
     w.P = ((h->nx + 1 + align - 1) / align) * align;
+    {
+        // Row pitch such that the x tiling of the TMA kernels is EXACT (rows of ntx tiles of txv vectors, same rule as the
+        // plans below): with a ragged last tile -- its boxes hang over the tensor's edge by more than the one halo vector
+        // -- k_pcg_fused's 4-D boxes lose the L2 reuse of the y-halo rows (measured: DRAM reads 1.26x-1.5x the stored
+        // bytes, 8.4-9.2 instead of 6.2-7.0 ps per node at 465^3 ... 513^3 fp32).  Costs at most a few pad vectors per row.
+        constexpr int VEC = VecN<T>::value;
+        const int maxv = 240 / VEC - 2;
+        const int rowvecs = w.P / VEC;
+        int ntx = (rowvecs + 32) / 64;
+        if (ntx < 1) ntx = 1;
+        while ((rowvecs + ntx - 1) / ntx > maxv) ntx++;
+        int txv = (rowvecs + ntx - 1) / ntx;
+        if (((ntx * txv) & 1) && txv + 1 <= maxv) txv++;           // rows stay a multiple of 32 bytes (two vectors)
+        if (!((ntx * txv) & 1) && sizeof(T) == 4) w.P = ntx * txv * VEC;     // fp64: measured no gain (385^3: -3 %)
+    }
     w.npad = (size_t)h->nz * h->ny * w.P;
     const size_t n_ey = (size_t)h->nz * (h->ny + 1) * w.P, n_ez = (size_t)(h->nz + 1) * h->ny * w.P;
     // distinct face values of the operator -> palette or full-precision face arrays (decided once per handle)
@@ -1511,7 +1527,7 @@ pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
         out->fused = 1;
         out->txv = b.TXV; out->ty = b.TY; out->tz = b.TZ; out->ring_slots = b.nsv; out->blocks_per_sm = b.bps;
         out->tiles = b.ntx * b.nty * b.ntz; out->grid = b.grid; out->threads = b.threads; out->smem_bytes = (int)b.smem;
-        out->autotuned = 0; out->vec_grid = 0; out->vec_threads = 0;
+        out->autotuned = b.tuned; out->vec_grid = 0; out->vec_threads = 0;
         out->face_quad = b.quad; out->coef_slots = b.nsc;
     };
     const bool fz = prec == PB_F32 ? fused_eligible<float>(h) : fused_eligible<double>(h);

@@ -72,6 +72,8 @@ pb_status fused_kernel_attr_fmt(bool quad, bool pald, size_t *max_dyn)
     return pald ? fused_kernel_attr<T, false, true>(max_dyn) : fused_kernel_attr<T, false, false>(max_dyn);
 }
 
+template <typename T> pb_status enqueue_batch_iterations(pb_handle *h, Work<T> &w, int n_iter);
+
 // coefficient arrays, vectors, plan and tensor maps of the batch path for M members; `fused`: of k_pcg_fused (one
 // kernel per iteration, one member) instead of k_spmv_batch + k_vec_batch
 template <typename T>
@@ -161,7 +163,9 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     if (ntx0 < 1) ntx0 = 1;
     while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
     const int *o = h->opt;
-    b.TXV = o[PB_OPT_TILE_TXV] > 0 ? o[PB_OPT_TILE_TXV] : (rowvecs + ntx0 - 1) / ntx0;
+    // the plan for tile rows of `txv_c` vectors (0: the option, else rows of about 1 KB), and its tensor maps
+    auto plan_with = [&](int txv_c) -> pb_status {
+    b.TXV = o[PB_OPT_TILE_TXV] > 0 ? o[PB_OPT_TILE_TXV] : txv_c > 0 ? txv_c : (rowvecs + ntx0 - 1) / ntx0;
     if (b.TXV > maxv) b.TXV = maxv;
     if (b.TXV > rowvecs) b.TXV = rowvecs;
     b.TY = o[PB_OPT_TILE_TY] > 0 ? o[PB_OPT_TILE_TY] : 4;
@@ -252,10 +256,56 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     if (fused && !b.quad) b.tm_q4 = b.tm_dinv;       // word format: the merged quad box does not exist (never fetched)
     b.M = M;
     b.fused = fused;
+    return PB_OK;
+    };
+    PB_TRY(plan_with(0));
+    b.tuned = 0;
+    const bool forced = o[PB_OPT_TILE_TXV] > 0 || o[PB_OPT_TILE_TY] > 0 || o[PB_OPT_TILE_TZ] > 0 || o[PB_OPT_RING_SLOTS] > 0 ||
+                        o[PB_OPT_BLOCKS_PER_SM] > 0;
+    if (fused && o[PB_OPT_AUTOTUNE] && !forced && (size_t)h->nx * h->ny * h->nz >= ((size_t)1 << 21)) {
+        // Like an FFT plan: time the pass for rows cut into ntx0 - 1 ... ntx0 + 2 tiles on the handle's own arrays (their
+        // contents do not matter: no latch, every solve re-initialises them) and keep the fastest.  Which width wins
+        // depends on how well neighbouring tiles stay in step (L2 reuse of the halo rows), not only on the tile shape:
+        // e.g. 481 x 481 x 257 fp64 0.917 ms with 61 x 3 tiles, 0.739 ms with 82 x 2.
+        int cand[4], nc = 0;
+        for (int ntx = ntx0 > 1 ? ntx0 - 1 : 1; ntx <= ntx0 + 2 && nc < 4; ntx++) {
+            const int txv = (rowvecs + ntx - 1) / ntx;
+            if (txv > maxv || txv < 8) continue;
+            if (nc && cand[nc - 1] == txv) continue;
+            cand[nc++] = txv;
+        }
+        if (nc > 1) {
+            cudaEvent_t e0 = nullptr, e1 = nullptr;
+            if (cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) == cudaSuccess) {
+                float best = 1e30f;
+                int best_txv = 0;
+                for (int c = 0; c < nc; c++) {
+                    if (plan_with(cand[c]) != PB_OK) continue;
+                    k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
+                    if (enqueue_batch_iterations<T>(h, w, 2) != PB_OK) continue;          // warm-up (both buffer sets)
+                    cudaEventRecord(e0, h->stream);
+                    if (enqueue_batch_iterations<T>(h, w, 4) != PB_OK) continue;
+                    cudaEventRecord(e1, h->stream);
+                    float ms = 0.f;
+                    if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) {
+                        cudaGetLastError();
+                        continue;
+                    }
+                    if (verbose()) fprintf(stderr, "pb: fused plan candidate TXV=%d TY=%d TZ=%d: %.4f ms per pass\n", b.TXV, b.TY, b.TZ, ms / 4);
+                    if (ms < best) { best = ms; best_txv = cand[c]; }
+                }
+                PB_TRY(plan_with(best_txv));
+                b.tuned = best_txv > 0;
+            }
+            if (e0) cudaEventDestroy(e0);
+            if (e1) cudaEventDestroy(e1);
+            PB_CUDA(cudaGetLastError());
+        }
+    }
     if (verbose())
-        fprintf(stderr, "pb: %s plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%ld grid=%d threads=%d smem=%zu\n",
+        fprintf(stderr, "pb: %s plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
                 fused ? "fused" : "batch", sizeof(T) == 4 ? "f32" : "f64", M, b.quad ? "quad" : "words", b.pald ? "+diag palette" : "", b.TXV, b.TY, b.TZ,
-                b.nsv, b.nsc, b.bps, ntiles, b.grid, b.threads, b.smem);
+                b.nsv, b.nsc, b.bps, b.ntx * b.nty * b.ntz, b.grid, b.threads, b.smem, b.tuned ? " (autotuned)" : "");
     return PB_OK;
 }
 
