@@ -92,15 +92,15 @@ __host__ __device__ inline FusedLayout fused_layout(int TXV, int TY, int vec, bo
 template <typename T, bool QUAD, bool PALD>
 struct FusedSm {
     static constexpr uint32_t vfull = 0, vempty = 64, cfull = 128, cempty = 160;     // 8 + 8 + 4 + 4 mbarriers
-    static constexpr uint32_t red = 256, last = 512;
-    static constexpr uint32_t qtab = 640;                                            // [256][4] face values
+    static constexpr uint32_t red = 256, last = 896;                                 // red: [kFusedSums][16 warps] doubles
+    static constexpr uint32_t qtab = 1024;                                           // [256][4] face values
     static constexpr uint32_t ddtab = qtab + (QUAD ? 1024u * (uint32_t)sizeof(T) : 0u);   // [256] {Dinv, D}
     static constexpr uint32_t ring = ddtab + (PALD ? 512u * (uint32_t)sizeof(T) : 0u);
 };
 static_assert(kMaxStages <= 8 && kMaxCoefStages <= 4, "FusedSm reserves 8 + 8 + 4 + 4 mbarriers");
 inline size_t fused_fixed_smem(int elt, bool quad, bool pald)
 {
-    return 640 + (quad ? (size_t)1024 * elt : 0) + (pald ? (size_t)512 * elt : 0);
+    return 1024 + (quad ? (size_t)1024 * elt : 0) + (pald ? (size_t)512 * elt : 0);
 }
 inline size_t fused_smem(const FusedLayout &F, int nsv, int nsc, int elt, bool quad, bool pald)
 {
@@ -509,28 +509,45 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         if (!F32) { a_pAp = (double)s_pv; a_S2 = (double)s_dvv; a_W = (double)s_w; a_U1 = (double)s_u1; a_U2 = (double)s_u2; }
     }
 
-    // stage 1 -> per-block partials; stage 2 by the last block to take a ticket (fixed order: deterministic); then every
-    // scalar of the iteration (header) and the stopping rule of step 3
+    // stage 1 -> per-block partials (warp sums, then thread q adds the warps' values of sum q in warp order); stage 2 by
+    // the last block to take a ticket: warp q adds the blocks' partials of sum q (fixed order: deterministic); then
+    // every scalar of the iteration (header) and the stopping rule of step 3
     const int nblk = gridDim.x;
+    const int nwarp = (int)(blockDim.x >> 5);
     {
         const double sums[kFusedSums] = {a_pAp, a_S2, a_W, a_U1, a_U2};
 #pragma unroll
         for (int q = 0; q < kFusedSums; q++) {
-            const double t = block_sum(sums[q], red);
-            if (tid == 0) a.partials[(size_t)q * nblk + blockIdx.x] = t;
+            const double t = warp_sum(sums[q]);
+            if (lane == 0) red[q * 16 + warp] = t;
         }
+        __syncthreads();
+        if (tid < kFusedSums) {
+            double t = 0.0;
+            for (int w = 0; w < nwarp; w++) t += red[tid * 16 + w];
+            a.partials[(size_t)tid * nblk + blockIdx.x] = t;
+            __threadfence();
+        }
+        __syncwarp();
     }
     if (tid == 0) {
-        __threadfence();
         const unsigned int t = atomicAdd(&a.st->ticket_spmv, 1u);
         *s_last = (t == (unsigned int)(nblk - 1));
     }
     __syncthreads();
     if (*s_last) {
         __threadfence();
+        for (int q = warp; q < kFusedSums; q += nwarp) {
+            const double *pq = a.partials + (size_t)q * nblk;
+            double v = 0.0;
+            for (int i = lane; i < nblk; i += 32) v += __ldcg(pq + i);
+            v = warp_sum(v);
+            if (lane == 0) red[q] = v;
+        }
+        __syncthreads();
         double sum[kFusedSums];
 #pragma unroll
-        for (int q = 0; q < kFusedSums; q++) sum[q] = final_sum(a.partials + (size_t)q * nblk, nblk, red);
+        for (int q = 0; q < kFusedSums; q++) sum[q] = red[q];
         if (tid == 0) {
             State *st = a.st;
             st->ticket_spmv = 0u;
