@@ -280,7 +280,11 @@ typedef enum {
                                         K_vec folded into the next K_spmv pass, 34 instead of 41 B per node); 0: K_spmv
                                         + K_vec.  Periodic boundary, warm starts, refinement, slabs and L2-resident
                                         grids always take their own paths                                              */
-    PB_OPT_COUNT_ = 18
+    PB_OPT_TAIL_POOL = 18,           /* k_pcg_fused: the top ~10 % of the planes are cut into chunks of this many planes
+                                        that the blocks fetch from a device-wide counter when they run out of their
+                                        static tiles (evens out the blocks' finishing times).  0 (default): chunks of 8
+                                        planes when nz >= 64, else off; 1: off; 4..64: on, chunks of that many planes  */
+    PB_OPT_COUNT_ = 19
 } pb_option;
 
 pb_status pb_set_option(pb_handle *h, pb_option opt, int value);
@@ -309,7 +313,8 @@ typedef struct {
                                  describe ITS plan (ring_slots = vector slots), vec_grid = 0                          */
     int face_quad;            /* fused / batch kernels: faces as 2-bit indices, four nodes per byte                  */
     int coef_slots;           /* fused / batch kernels: depth of the coefficient ring                                */
-    int reserved[5];
+    int tail_pool;            /* k_pcg_fused: planes per dynamically scheduled chunk of the top of the grid, 0 = none  */
+    int reserved[4];
 } pb_plan;
 
 /* pb_prepare -- build the work arrays of `prec` (setup row a0: padded coefficients, diagonal, folded b) and pick

@@ -28,7 +28,7 @@ EXPORTS = ("pb_create", "pb_set_rhs", "pb_apply", "pb_solve", "pb_solve_begin", 
 OPTIONS = {"persist": 0, "persist_max_mb": 1, "persist_fused_max_knodes": 2, "persist_blocks_per_sm": 3,
            "palette": 4, "palette_diag": 5, "palette_diag_spmv": 6, "autotune": 7, "tile_txv": 8, "tile_ty": 9,
            "tile_tz": 10, "ring_slots": 11, "blocks_per_sm": 12, "vec_blocks_per_sm": 13, "graph": 14, "l2_hints": 15,
-           "batch_width": 16, "fused": 17}
+           "batch_width": 16, "fused": 17, "tail_pool": 18}
 
 
 class PBPlan(ctypes.Structure):
@@ -37,7 +37,7 @@ class PBPlan(ctypes.Structure):
         "precision", "num_sm", "persist", "persist_fused", "persist_grid", "palette_size", "diag_palette_size",
         "face_palette", "diag_palette_vec", "diag_palette_spmv", "txv", "ty", "tz", "ring_slots", "blocks_per_sm",
         "tiles", "grid", "threads", "smem_bytes", "autotuned", "vec_grid", "vec_threads", "spmv_bytes_per_node",
-        "vec_bytes_per_node", "pitch", "fused", "face_quad", "coef_slots")] + [("reserved", ctypes.c_int * 5)]
+        "vec_bytes_per_node", "pitch", "fused", "face_quad", "coef_slots", "tail_pool")] + [("reserved", ctypes.c_int * 4)]
 
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -43,6 +43,7 @@ struct BatchWork {
     size_t smem = 0;
     int vec_grid = 0;
     int tuned = 0;                                 // the fused plan was chosen by timing candidates
+    int zs = 0, pc = 0, npool = 0;                 // k_pcg_fused: static tiles over [0, zs), pool chunks of pc planes above
     CUtensorMap tm_r, tm_p0, tm_p1, tm_x, tm_dinv, tm_exm, tm_exp, tm_ey, tm_ez;
     cudaGraphExec_t graph = nullptr;
     int graph_iters = 0;
@@ -1469,6 +1470,9 @@ pb_status pb_set_option(pb_handle *h, pb_option opt, int value)
     case PB_OPT_BATCH_WIDTH:
         if (value != 1 && value != 2 && value != 4) return PB_ERR_INVALID_ARG;
         break;
+    case PB_OPT_TAIL_POOL:
+        if (value != 0 && value != 1 && (value < 4 || value > 64)) return PB_ERR_INVALID_ARG;
+        break;
     case PB_OPT_BLOCKS_PER_SM: case PB_OPT_VEC_BLOCKS_PER_SM:
         if (value > 32) return PB_ERR_INVALID_ARG;
         break;
@@ -1528,7 +1532,7 @@ pb_status pb_get_plan(pb_handle *h, pb_precision prec, pb_plan *out)
         out->txv = b.TXV; out->ty = b.TY; out->tz = b.TZ; out->ring_slots = b.nsv; out->blocks_per_sm = b.bps;
         out->tiles = b.ntx * b.nty * b.ntz; out->grid = b.grid; out->threads = b.threads; out->smem_bytes = (int)b.smem;
         out->autotuned = b.tuned; out->vec_grid = 0; out->vec_threads = 0;
-        out->face_quad = b.quad; out->coef_slots = b.nsc;
+        out->face_quad = b.quad; out->coef_slots = b.nsc; out->tail_pool = b.pc;
     };
     const bool fz = prec == PB_F32 ? fused_eligible<float>(h) : fused_eligible<double>(h);
     if (fz) { if (prec == PB_F32) fill_fused(h->wf); else fill_fused(h->wd); }

@@ -164,7 +164,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     while ((rowvecs + ntx0 - 1) / ntx0 > maxv) ntx0++;
     const int *o = h->opt;
     // the plan for tile rows of `txv_c` vectors (0: the option, else rows of about 1 KB), and its tensor maps
-    auto plan_with = [&](int txv_c) -> pb_status {
+    auto plan_with = [&](int txv_c, int pool_c = 0) -> pb_status {
     b.TXV = o[PB_OPT_TILE_TXV] > 0 ? o[PB_OPT_TILE_TXV] : txv_c > 0 ? txv_c : (rowvecs + ntx0 - 1) / ntx0;
     if (b.TXV > maxv) b.TXV = maxv;
     if (b.TXV > rowvecs) b.TXV = rowvecs;
@@ -208,14 +208,21 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.ntx = (rowvecs + b.TXV - 1) / b.TXV;
     b.nty = (h->ny + b.TY - 1) / b.TY;
     const int slots = h->nsm * b.bps, xy = b.ntx * b.nty;
-    b.TZ = o[PB_OPT_TILE_TZ] > 0 ? o[PB_OPT_TILE_TZ] : choose_tz(h->nz, xy, slots);
-    if (b.TZ > h->nz) b.TZ = h->nz;
-    b.ntz = (h->nz + b.TZ - 1) / b.TZ;
+    // k_pcg_fused: the planes [zs, nz) form the dynamically scheduled pool (pool_c planes per chunk, about a tenth of nz)
+    b.zs = h->nz; b.pc = 0; b.npool = 0;
+    if (fused && pool_c >= 4 && h->nz >= 8 * pool_c) {
+        int nch = (h->nz + 5 * pool_c) / (10 * pool_c);
+        if (nch < 1) nch = 1;
+        b.pc = pool_c; b.zs = h->nz - nch * pool_c; b.npool = nch * xy;
+    }
+    b.TZ = o[PB_OPT_TILE_TZ] > 0 ? o[PB_OPT_TILE_TZ] : choose_tz(b.zs, xy, slots);
+    if (b.TZ > b.zs) b.TZ = b.zs;
+    b.ntz = (b.zs + b.TZ - 1) / b.TZ;
     const long ntiles = (long)xy * b.ntz;
     b.grid = (int)(ntiles < slots ? ntiles : slots);
     b.vec_grid = grid_for(w.npad / VEC, 256, h->nsm * 8);
     size_t need = (size_t)M * b.grid > (size_t)2 * M * b.vec_grid ? (size_t)M * b.grid : (size_t)2 * M * b.vec_grid;
-    if ((size_t)kFusedSums * b.grid > need) need = (size_t)kFusedSums * b.grid;
+    if (fused && (size_t)kFusedSums * ((size_t)ntiles + b.npool) > need) need = (size_t)kFusedSums * ((size_t)ntiles + b.npool);
     if (need > h->partials_cap) {
         PB_CUDA(cudaStreamSynchronize(h->stream));
         if (h->partials) cudaFree(h->partials);
@@ -258,7 +265,10 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.fused = fused;
     return PB_OK;
     };
-    PB_TRY(plan_with(0));
+    // measured at 385^3: a tenth of the planes in chunks of 6-13 takes 5-7 % (fp32) / 10 % (fp64) off a pass; 5-15 % of
+    // the planes and chunks of 6-13 planes are equally good
+    const int pool_forced = o[PB_OPT_TAIL_POOL] >= 4 ? o[PB_OPT_TAIL_POOL] : (o[PB_OPT_TAIL_POOL] == 0 && h->nz >= 64) ? 8 : 0;
+    PB_TRY(plan_with(0, pool_forced));
     b.tuned = 0;
     const bool forced = o[PB_OPT_TILE_TXV] > 0 || o[PB_OPT_TILE_TY] > 0 || o[PB_OPT_TILE_TZ] > 0 || o[PB_OPT_RING_SLOTS] > 0 ||
                         o[PB_OPT_BLOCKS_PER_SM] > 0;
@@ -280,7 +290,8 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
                 float best = 1e30f;
                 int best_txv = 0;
                 for (int c = 0; c < nc; c++) {
-                    if (plan_with(cand[c]) != PB_OK) continue;
+                    const int txv_c = cand[c];
+                    if (plan_with(txv_c, pool_forced) != PB_OK) continue;
                     k_set_state<<<1, 1, 0, h->stream>>>(h->st, 1.0, 0, 0);
                     if (enqueue_batch_iterations<T>(h, w, 2) != PB_OK) continue;          // warm-up (both buffer sets)
                     cudaEventRecord(e0, h->stream);
@@ -291,10 +302,10 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
                         cudaGetLastError();
                         continue;
                     }
-                    if (verbose()) fprintf(stderr, "pb: fused plan candidate TXV=%d TY=%d TZ=%d: %.4f ms per pass\n", b.TXV, b.TY, b.TZ, ms / 4);
-                    if (ms < best) { best = ms; best_txv = cand[c]; }
+                    if (verbose()) fprintf(stderr, "pb: fused plan candidate TXV=%d TY=%d TZ=%d pool=%d: %.4f ms per pass\n", b.TXV, b.TY, b.TZ, b.pc, ms / 4);
+                    if (ms < best) { best = ms; best_txv = txv_c; }
                 }
-                PB_TRY(plan_with(best_txv));
+                PB_TRY(plan_with(best_txv, pool_forced));
                 b.tuned = best_txv > 0;
             }
             if (e0) cudaEventDestroy(e0);
@@ -303,9 +314,9 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
         }
     }
     if (verbose())
-        fprintf(stderr, "pb: %s plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%d grid=%d threads=%d smem=%zu%s\n",
+        fprintf(stderr, "pb: %s plan<%s> M=%d %s%s TXV=%d TY=%d TZ=%d vector slots=%d coefficient slots=%d bps=%d tiles=%d (+%d pool chunks of %d planes) grid=%d threads=%d smem=%zu%s\n",
                 fused ? "fused" : "batch", sizeof(T) == 4 ? "f32" : "f64", M, b.quad ? "quad" : "words", b.pald ? "+diag palette" : "", b.TXV, b.TY, b.TZ,
-                b.nsv, b.nsc, b.bps, b.ntx * b.nty * b.ntz, b.grid, b.threads, b.smem, b.tuned ? " (autotuned)" : "");
+                b.nsv, b.nsc, b.bps, b.ntx * b.nty * b.ntz, b.npool, b.pc, b.grid, b.threads, b.smem, b.tuned ? " (autotuned)" : "");
     return PB_OK;
 }
 
@@ -340,6 +351,7 @@ void launch_fused_kernels(pb_handle *h, Work<T> &w, int n_iter)
     a.ntiles = b.ntx * b.nty * b.ntz; a.nsv = b.nsv; a.nsc = b.nsc; a.precond = h->precond;
     a.st = h->st; a.partials = h->partials; a.lut = w.lut; a.dlut = w.dlut;
     a.nct = b.threads - 32;
+    a.zs = b.zs; a.pc = b.pc; a.npool = b.npool; a.ncol = b.ntx * b.nty;
     a.sQ = (size_t)(b.Ap - b.r) * sizeof(T); a.sP = (size_t)(b.p0 - b.r) * sizeof(T); a.sX = (size_t)(b.x - b.r) * sizeof(T);
     fused_args_layout(a, fused_layout(b.TXV, b.TY, VecN<T>::value, QUAD, PALD));
     for (int it = 0; it < n_iter; it++)

@@ -93,6 +93,7 @@ template <typename T, bool QUAD, bool PALD>
 struct FusedSm {
     static constexpr uint32_t vfull = 0, vempty = 64, cfull = 128, cempty = 160;     // 8 + 8 + 4 + 4 mbarriers
     static constexpr uint32_t red = 256, last = 896;                                 // red: [kFusedSums][16 warps] doubles
+    static constexpr uint32_t tq = 904;                                              // 16 tile ids (producer -> consumers)
     static constexpr uint32_t qtab = 1024;                                           // [256][4] face values
     static constexpr uint32_t ddtab = qtab + (QUAD ? 1024u * (uint32_t)sizeof(T) : 0u);   // [256] {Dinv, D}
     static constexpr uint32_t ring = ddtab + (PALD ? 512u * (uint32_t)sizeof(T) : 0u);
@@ -117,13 +118,17 @@ struct FusedArgs {
     int nsv, nsc;
     int precond;
     int nct;                 // consumer threads (whole warps); one more warp produces
+    // tiles: `ntiles` static ones over the planes [0, zs), handed out blockIdx.x, + gridDim.x, ...; then `npool` chunks of
+    // `pc` planes over [zs, nz), every column again, fetched from a device-wide counter by whichever block runs out of
+    // static tiles first (the blocks' speeds differ by several per cent from launch to launch)
+    int zs, pc, npool, ncol;
     // the slot layout (fused_layout), bytes: coefficient slot {Dinv @0, ez @oEZ, ex- @oEXM, ex+ @oEXP, ey @oEY}, one
     // p_new plane; box sizes for expect_tx (bQ4: the merged quad box; bEZ, bC: the word-format face boxes)
     uint32_t vslot, cslot, pn, bZ, oEZ, oEXM, oEXP, oEY, bwq, bwd;
     uint32_t bDv, bQ4, bEZ, bC;
     size_t sQ, sP, sX;       // bytes from a cell of r to the same cell of A p, p, x in the written buffer set
     State *st;
-    double *partials;        // [kFusedSums][gridDim.x]
+    double *partials;        // [kFusedSums][ntiles + npool]: the sums of every tile
     const T *lut;
     const T *dlut;
 };
@@ -135,6 +140,24 @@ inline void fused_args_layout(FusedArgs<T> &a, const FusedLayout &F)
     a.oEZ = F.oEZ; a.oEXM = F.oEXM; a.oEXP = F.oEXP; a.oEY = F.oEY;
     a.bwq = (uint32_t)L.bwq; a.bwd = (uint32_t)L.bwd;
     a.bDv = F.bDv; a.bQ4 = F.bQ4; a.bEZ = L.bEZ; a.bC = L.bEXM + L.bEY;
+}
+
+// tile id -> column (bx, by) and plane range [k0, k1)
+template <typename T>
+__device__ __forceinline__ void fused_tile(const FusedArgs<T> &a, int t, int &bx, int &by, int &k0, int &k1)
+{
+    if (t < a.ntiles) {
+        bx = t % a.ntx; t /= a.ntx;
+        by = t % a.nty;
+        k0 = (t / a.nty) * a.TZ;
+        k1 = min(k0 + a.TZ, a.zs);
+    } else {
+        t -= a.ntiles;
+        const int col = t % a.ncol;
+        bx = col % a.ntx; by = col / a.ntx;
+        k0 = a.zs + (t / a.ncol) * a.pc;
+        k1 = min(k0 + a.pc, a.nz);
+    }
 }
 
 // the two vector tensors ([4][nz][ny][P]: buffer set 0, buffer set 1) in one kernel parameter
@@ -200,13 +223,27 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             int vs = 0, cs = 0;
             uint32_t vph = 0, cph = 0;
             const CUtensorMap *tv = parity ? &vm.set1 : &vm.set0;
-            for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-                int b = tile;
-                const int bx = b % a.ntx; b /= a.ntx;
-                const int by = b % a.nty;
-                const int bz = b / a.nty;
+            int next_static = blockIdx.x;
+            for (uint32_t seq = 0;; seq++) {
+                int tile = -1;
+                if (next_static < a.ntiles) { tile = next_static; next_static += gridDim.x; }
+                else if (a.npool > 0) {
+                    unsigned int c = 0;
+                    if (leader) c = atomicAdd(&a.st->pool_ctr, 1u);
+                    c = __shfl_sync(0xffffffffu, c, 0);
+                    if (c < (unsigned int)a.npool) tile = a.ntiles + (int)c;
+                }
+                // the tile id reaches the consumers with the first item of the tile (the arrive below releases it)
+                if (leader) asm volatile("st.shared.s32 [%0], %1;" ::"r"(sb + SM::tq + 4u * (seq & 15u)), "r"(tile) : "memory");
+                if (tile < 0) {                                        // end marker: an item without data
+                    const uint32_t full = sb + SM::cfull + 8u * cs;
+                    mbar_wait_a(full + (SM::cempty - SM::cfull), cph ^ 1);
+                    if (leader) mbar_arrive_a(full);
+                    break;
+                }
+                int bx, by, k0, k1;
+                fused_tile(a, tile, bx, by, k0, k1);
                 const int x0 = bx * TXV * VEC, j0 = by * TY;
-                const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
                 const int xd = PALD ? ((x0 - VEC) & ~15) : x0 - VEC;   // byte-index box: 16-byte aligned start
                 const int xq = QUAD ? ((x0 >> 2) & ~15) : x0;          // quad-index boxes likewise
                 for (int q = k0 - 1; q <= k1; q++) {
@@ -309,16 +346,18 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         constexpr bool F32 = sizeof(T) == 4;
         T s_pv = T(0), s_dvv = T(0), s_w = T(0), s_u1 = T(0), s_u2 = T(0);
 
-        for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-            int b = tile;
-            const int bx = b % a.ntx; b /= a.ntx;
-            const int by = b % a.nty;
-            const int bz = b / a.nty;
+        for (uint32_t seq = 0;; seq++) {
+            // the producer's tile sequence: its id comes with the first item of the tile
+            mbar_wait_a(sb + SM::cfull + 8u * cs, cph);
+            int tile;
+            asm volatile("ld.shared.s32 %0, [%1];" : "=r"(tile) : "r"(sb + SM::tq + 4u * (seq & 15u)));
+            if (tile < 0) break;
+            int bx, by, k0, k1;
+            fused_tile(a, tile, bx, by, k0, k1);
             const int x0 = bx * TXV * VEC, j0 = by * TY;
             const int i0 = x0 + tx * VEC, j = j0 + ty;
             const bool active = intile && (i0 < P) && (j < ny);
             const int nvalid = active ? nx - i0 : 0;   // inactive lanes: A p = 0 (their Dinv may be a zero-filled 0, D = inf)
-            const int k0 = bz * TZ, k1 = min(k0 + TZ, nz);
             if (PALD) {
                 const uint32_t lead_d = (uint32_t)(x0 - VEC) & 15u;
                 t_dv = lead_d + (uint32_t)(ty + 1) * a.bwd + (uint32_t)(tx + 1) * VEC;
@@ -505,31 +544,37 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
             flush();
             // coefficient item k1: only Dinv and ez of the own column were used, before the last barrier
             if (tid == 0) mbar_arrive_o<SM::cempty>(sb + 8u * (uint32_t)csk);
+            // the five sums of THIS TILE -> partials[q][tile] (consumer warps in warp order): the value does not depend on
+            // which block ran the tile, so the result of the pass is the same whatever the dynamic schedule was
+            {
+                if (!F32) {
+                    a_pAp = (double)s_pv; a_S2 = (double)s_dvv; a_W = (double)s_w; a_U1 = (double)s_u1; a_U2 = (double)s_u2;
+                    s_pv = T(0); s_dvv = T(0); s_w = T(0); s_u1 = T(0); s_u2 = T(0);
+                }
+                const double sums[kFusedSums] = {a_pAp, a_S2, a_W, a_U1, a_U2};
+#pragma unroll
+                for (int q = 0; q < kFusedSums; q++) {
+                    const double t = warp_sum(sums[q]);
+                    if (lane == 0) red[q * 16 + warp] = t;
+                }
+                named_bar_sync(1, NCT);
+                if (tid < kFusedSums) {
+                    double t = 0.0;
+                    for (int w = 0; w < (NCT >> 5); w++) t += red[tid * 16 + w];
+                    a.partials[(size_t)tid * (size_t)(a.ntiles + a.npool) + tile] = t;
+                    __threadfence();
+                }
+                a_pAp = 0.0; a_S2 = 0.0; a_W = 0.0; a_U1 = 0.0; a_U2 = 0.0;
+            }
         }
-        if (!F32) { a_pAp = (double)s_pv; a_S2 = (double)s_dvv; a_W = (double)s_w; a_U1 = (double)s_u1; a_U2 = (double)s_u2; }
     }
 
-    // stage 1 -> per-block partials (warp sums, then thread q adds the warps' values of sum q in warp order); stage 2 by
-    // the last block to take a ticket: warp q adds the blocks' partials of sum q (fixed order: deterministic); then
-    // every scalar of the iteration (header) and the stopping rule of step 3
+    // stage 2 by the last block to take a ticket: warp q adds the tiles' partials of sum q in tile order (deterministic,
+    // and independent of the grid size and of the dynamic schedule); then every scalar of the iteration (header) and
+    // the stopping rule of step 3
     const int nblk = gridDim.x;
     const int nwarp = (int)(blockDim.x >> 5);
-    {
-        const double sums[kFusedSums] = {a_pAp, a_S2, a_W, a_U1, a_U2};
-#pragma unroll
-        for (int q = 0; q < kFusedSums; q++) {
-            const double t = warp_sum(sums[q]);
-            if (lane == 0) red[q * 16 + warp] = t;
-        }
-        __syncthreads();
-        if (tid < kFusedSums) {
-            double t = 0.0;
-            for (int w = 0; w < nwarp; w++) t += red[tid * 16 + w];
-            a.partials[(size_t)tid * nblk + blockIdx.x] = t;
-            __threadfence();
-        }
-        __syncwarp();
-    }
+    __syncthreads();
     if (tid == 0) {
         const unsigned int t = atomicAdd(&a.st->ticket_spmv, 1u);
         *s_last = (t == (unsigned int)(nblk - 1));
@@ -537,10 +582,11 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
     __syncthreads();
     if (*s_last) {
         __threadfence();
+        const int ntot = a.ntiles + a.npool;
         for (int q = warp; q < kFusedSums; q += nwarp) {
-            const double *pq = a.partials + (size_t)q * nblk;
+            const double *pq = a.partials + (size_t)q * ntot;
             double v = 0.0;
-            for (int i = lane; i < nblk; i += 32) v += __ldcg(pq + i);
+            for (int i = lane; i < ntot; i += 32) v += __ldcg(pq + i);
             v = warp_sum(v);
             if (lane == 0) red[q] = v;
         }
@@ -551,6 +597,7 @@ k_pcg_fused(const __grid_constant__ FusedMaps vm, const __grid_constant__ CUtens
         if (tid == 0) {
             State *st = a.st;
             st->ticket_spmv = 0u;
+            st->pool_ctr = 0u;
             const double pAp = sum[0], S2 = sum[1], W = sum[2], U1 = sum[3], U2 = sum[4];
             const int l = st->iter_cur;                         // this pass formed r_l and phi_l
             st->pAp = pAp;

@@ -33,6 +33,8 @@ struct State {
     double loc_rz, loc_rr;
     int slab;
     int xbuf;         // k_pcg_fused: which of its two x buffers holds the current iterate (0 after k_init)
+    unsigned int pool_ctr;   // k_pcg_fused: next chunk of the dynamically scheduled tail (0 between launches)
+    int pad2_;
 };
 
 // 16-byte vector of T: 4 floats or 2 doubles -> one 128-bit load/store per thread

@@ -106,6 +106,7 @@ __global__ void k_set_state(State *st, double tol2, int maxiter, int latch, int 
 {
     st->slab = slab;
     st->xbuf = 0;
+    st->pool_ctr = 0u;
     st->loc_rz = 0.0;
     st->loc_rr = 0.0;
     st->tol2 = tol2;

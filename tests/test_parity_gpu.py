@@ -821,6 +821,35 @@ def test_options_are_handle_state(pkg):
         assert a.plan("f32")["txv"] == pa["txv"] and a.solve(1e-5, 5000, "f32")["iters"] == ga["iters"]
 
 
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_fused_tail_pool_is_schedule_independent(pkg, pbref, prec, tol):
+    """k_pcg_fused hands the top tenth of the planes out dynamically (PB_OPT_TAIL_POOL): which block runs which chunk
+    changes from launch to launch, the result must not -- the sums are formed per tile and added in tile order.  Chunk
+    sizes 4 / 8 (default for nz >= 64) / 10, a size too large for the grid (64: no pool) and pool off: oracle parity, the same iteration count,
+    bitwise repeatable solves, and rejected values."""
+    inp = random_operator(45, 37, 83, seed=12, two_valued=True)         # nz = 83: 3 static z-chunks + the pool
+    ref = pbref.from_inputs(inp)
+    o = ref.solve(tol, 5000)
+    ref.close()
+    scale, lim = np.max(np.abs(o["phi"])), (1e-8 if prec == "f64" else 1e-4)
+    iters = set()
+    for pool in (0, 1, 4, 10, 64):
+        with pkg.PBSolver(*inp.args(), options=dict(persist=0, tail_pool=pool, tile_tz=25)) as s:
+            g1 = s.solve(tol, 5000, prec, check_every=5)
+            g2 = s.solve(tol, 5000, prec, check_every=64)
+            pl = s.plan(prec)
+        assert pl["fused"] == 1 and pl["tail_pool"] == {0: 8, 1: 0, 4: 4, 10: 10, 64: 0}[pool], pl     # 64 > nz / 8: no pool
+        assert g1["status"] == 0 and np.array_equal(g1["phi"], g2["phi"]) and g1["iters"] == g2["iters"], pool
+        assert abs(g1["iters"] - o["iters"]) <= max(1, round(0.05 * o["iters"])), (pool, g1["iters"], o["iters"])
+        assert np.max(np.abs(g1["phi"] - o["phi"])) <= lim * scale, pool
+        iters.add(g1["iters"])
+    assert len(iters) == 1
+    with pkg.PBSolver(*inp.args()) as s:
+        for bad in (2, 3, 65):
+            with pytest.raises(pkg.PBError):
+                s.set_option("tail_pool", bad)
+
+
 # ---------------------------------------------------------------------------------------------
 # NEXT row f2: pb_solve_batch -- M right-hand sides per pass (k_spmv_batch + k_vec_batch), PAPER.md:23
 # ---------------------------------------------------------------------------------------------
