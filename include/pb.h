@@ -280,7 +280,7 @@ typedef enum {
                                         K_vec folded into the next K_spmv pass, 34 instead of 41 B per node); 0: K_spmv
                                         + K_vec.  Periodic boundary, warm starts, refinement, slabs and L2-resident
                                         grids always take their own paths                                              */
-    PB_OPT_TAIL_POOL = 18,           /* k_pcg_fused: the top ~10 % of the planes are cut into chunks of this many planes
+    PB_OPT_TAIL_POOL = 18,           /* k_pcg_fused: the top ~5 % of the planes are cut into chunks of this many planes
                                         that the blocks fetch from a device-wide counter when they run out of their
                                         static tiles (evens out the blocks' finishing times).  0 (default): chunks of 8
                                         planes when nz >= 64, else off; 1: off; 4..64: on, chunks of that many planes  */

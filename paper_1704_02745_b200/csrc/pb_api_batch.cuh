@@ -208,10 +208,12 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.ntx = (rowvecs + b.TXV - 1) / b.TXV;
     b.nty = (h->ny + b.TY - 1) / b.TY;
     const int slots = h->nsm * b.bps, xy = b.ntx * b.nty;
-    // k_pcg_fused: the planes [zs, nz) form the dynamically scheduled pool (pool_c planes per chunk, about a tenth of nz)
+    // k_pcg_fused: the planes [zs, nz) form the dynamically scheduled pool (pool_c planes per chunk, about a twentieth of
+    // nz: at full clock 5-15 % are equally good, under the power cap of a long run the smaller pool's extra halo planes
+    // cost less -- 385^3 fp32 sustained: 10 % pool -1 %, 5 % pool +0.7 % against none)
     b.zs = h->nz; b.pc = 0; b.npool = 0;
     if (fused && pool_c >= 4 && h->nz >= 8 * pool_c) {
-        int nch = (h->nz + 5 * pool_c) / (10 * pool_c);
+        int nch = (h->nz + 10 * pool_c) / (20 * pool_c);
         if (nch < 1) nch = 1;
         b.pc = pool_c; b.zs = h->nz - nch * pool_c; b.npool = nch * xy;
     }
@@ -265,8 +267,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
     b.fused = fused;
     return PB_OK;
     };
-    // measured at 385^3: a tenth of the planes in chunks of 6-13 takes 5-7 % (fp32) / 10 % (fp64) off a pass; 5-15 % of
-    // the planes and chunks of 6-13 planes are equally good
+    // measured at 385^3 at full clock: 5-15 % of the planes in chunks of 6-13 take 5-7 % (fp32) / 10 % (fp64) off a pass
     const int pool_forced = o[PB_OPT_TAIL_POOL] >= 4 ? o[PB_OPT_TAIL_POOL] : (o[PB_OPT_TAIL_POOL] == 0 && h->nz >= 64) ? 8 : 0;
     PB_TRY(plan_with(0, pool_forced));
     b.tuned = 0;
