@@ -288,10 +288,9 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
         if (nc > 1) {
             cudaEvent_t e0 = nullptr, e1 = nullptr;
             if (cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) == cudaSuccess) {
-                float best = 1e30f, t_std = 0.f;
+                float best = 1e30f;
                 int best_txv = 0;
                 const int txv_std = (rowvecs + ntx0 - 1) / ntx0;
-                (void)t_std;
                 for (int c = 0; c < nc; c++) {
                     const int txv_c = cand[c];
                     if (plan_with(txv_c, pool_forced) != PB_OK) continue;
@@ -307,7 +306,7 @@ pb_status ensure_batch(pb_handle *h, int M, bool fused = false)
                     }
                     if (verbose()) fprintf(stderr, "pb: fused plan candidate TXV=%d TY=%d TZ=%d pool=%d: %.4f ms per pass\n", b.TXV, b.TY, b.TZ, b.pc, ms / 6);
                     // six passes are a noisy sample: another width has to beat the standard one (rows of about 1 KB) by 3 %
-                    if (txv_c == txv_std) { t_std = ms; if (ms * 0.97f < best) { best = ms * 0.97f; best_txv = txv_c; } }
+                    if (txv_c == txv_std) { if (ms * 0.97f < best) { best = ms * 0.97f; best_txv = txv_c; } }
                     else if (ms < best) { best = ms; best_txv = txv_c; }
                 }
                 PB_TRY(plan_with(best_txv, pool_forced));
